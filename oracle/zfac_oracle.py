@@ -1,0 +1,163 @@
+"""CPU FP64 ORACLE for the Z-refinement hot path -- TEST INFRASTRUCTURE ONLY.
+
+This file is test infrastructure.  Only `tests/`, `__graft_entry__.smoke()` and
+`bench.py`'s `cpu_baseline` / `--impl reference` legs may import it.  It shares
+no code with the CUDA path (paper_2404_19163_b200/csrc, binding.py) and imports
+nothing from it; it is plain numpy in FP64, with `numpy.matmul` as the only
+library primitive.  No blocking, fusion, symmetry trick or reordering beyond
+what the paper's algorithm states.
+
+What it computes (PAPER.md = /root/reference/PAPER.md):
+
+  Algorithm 2, m = 2, Frobenius norm
+  (PAPER.md:289):
+
+      Z = initial guess; iter = 0; X = Z^T S Z
+      for iter < Nmax:
+          Err[iter] = ||X - I||_F
+          if iter > 0 and Err[iter] > Err[iter-1]^3: break          (Eq. 38)
+          iter += 1
+          Z = Z (a0 I + a1 X + a2 X^2),  a = (15/8, -5/4, 3/8)        (Eq. 13)
+          X = Z^T S Z
+
+  The triple product is formed as A = S Z, then X = Z^T A (Eq. 22, 26,
+  PAPER.md:181-205).  Two algebraically identical forms of the update are
+  provided: the printed X-form above, and the delta-form of Eq. 16
+   written in the residual R = I - X = -delta:
+
+      Z = Z + Z (1/2 R + 3/8 R R)         <=>   Z (15/8 I - 5/4 X + 3/8 X^2)
+
+  (substitute X = I - R).  The delta-form is the default because it is the one
+  BASELINE.json's north_star names; tests pin the two against each other.
+
+Readings of silent / ambiguous points (repeated in DESIGN.md):
+  Q5  the Z returned at the break is the current one (Alg. 2 never rolls back);
+  Q6  `iters` = number of Z updates performed = the stop index; Err has iters+1 entries;
+  Q7  Err of the final Z is always recorded (also when Nmax is reached);
+  Q9  strict '>' as printed; a non-finite Err stops the loop with a flag;
+  Q10 the test is applied unconditionally (as Alg. 2), not only when Err < 1;
+  Q11 Frobenius norm, one sqrt of an FP64 sum of squares.
+
+Pins (tests/test_oracle_pins.py): exact-rational brute force at N <= 4; the
+printed error polynomial c,d,e = 5/8,-15/64,9/64 as a matrix
+identity for non-symmetric Z0; Z -> S^-1/2 from a dense eigendecomposition when
+Z0 ∝ I; Z Z^T = S^-1 for non-commuting Z0; cubic order; stop-rule cases;
+scaling / permutation covariances; diagonal S reduces to N scalar recursions.
+Every function below is pinned; none is "parity unpinned".
+"""
+from __future__ import annotations
+
+import math
+from typing import NamedTuple
+
+import numpy as np
+
+# result flags (same meaning as include/zfac.h, values restated, not imported)
+R_STOPPED = 1     # the parameter-free test fired (Eq. 38 violated)
+R_MAXITER = 2     # Nmax updates were performed without the test firing
+R_NONFINITE = 4   # Err became inf/NaN
+
+STOP_PAPER = 0    # Alg. 2 test
+STOP_FIXED = 1    # run exactly max_iter updates (benchmark / parity mode)
+
+# Polynomial coefficients for m = 2, from Ref. 1's Table I as quoted at PAPER.md:451.
+A0, A1, A2 = 15.0 / 8.0, -5.0 / 4.0, 3.0 / 8.0
+
+
+class RefineResult(NamedTuple):
+    Z: np.ndarray        # final iterate
+    iters: int           # number of Z updates performed
+    err: np.ndarray      # Err[0..iters], ||Z_n^T S Z_n - I||_F
+    flags: int
+
+
+def triple_product(S: np.ndarray, Z: np.ndarray) -> np.ndarray:
+    """X = Z^T S Z via A = S Z, X = Z^T A   (Eq. 22 and Eq. 26)."""
+    A = S @ Z
+    return Z.T @ A
+
+
+def residual(S: np.ndarray, Z: np.ndarray) -> np.ndarray:
+    """R = I - Z^T S Z = -(X - I) = -delta   (Eq. 12, Eq. 33)."""
+    X = triple_product(S, Z)
+    return np.eye(S.shape[0], dtype=X.dtype) - X
+
+
+def err_fro(R: np.ndarray) -> float:
+    """Err = ||X - I||_F = ||R||_F   (Alg. 2; norm choice PAPER.md:289)."""
+    return float(math.sqrt(float(np.sum(R.astype(np.float64) * R.astype(np.float64)))))
+
+
+def update_delta_form(Z: np.ndarray, R: np.ndarray) -> np.ndarray:
+    """Z_{n+1} = Z_n + Z_n (1/2 R + 3/8 R R)   (Eq. 16 form of Eq. 13 with m = 2)."""
+    Q = 0.5 * R + 0.375 * (R @ R)
+    return Z + Z @ Q
+
+
+def update_x_form(Z: np.ndarray, X: np.ndarray) -> np.ndarray:
+    """Z_{n+1} = Z_n (a0 I + a1 X + a2 X^2)   (Eq. 13 as printed; Alg. 2)."""
+    n = X.shape[0]
+    P = A0 * np.eye(n, dtype=X.dtype) + A1 * X + A2 * (X @ X)
+    return Z @ P
+
+
+def refine(S: np.ndarray, Z0: np.ndarray, max_iter: int, stop: int = STOP_PAPER,
+           form: str = "delta", dtype=np.float64) -> RefineResult:
+    """Algorithm 2.  `dtype` exists only so that the paper's
+    `single` scheme (Table I) can be emulated in a pin; the oracle
+    proper is FP64."""
+    if max_iter < 0:
+        raise ValueError("max_iter must be >= 0")
+    S = np.asarray(S, dtype=dtype)
+    Z = np.array(Z0, dtype=dtype, copy=True)
+    n = S.shape[0]
+    eye = np.eye(n, dtype=dtype)
+    err = []
+    flags = 0
+    it = 0
+    X = triple_product(S, Z)
+    while True:
+        R = eye - X
+        err.append(err_fro(R))
+        if not math.isfinite(err[it]):
+            flags |= R_NONFINITE
+            break
+        if stop == STOP_PAPER and it > 0 and err[it] > err[it - 1] ** 3:
+            flags |= R_STOPPED
+            break
+        if it == max_iter:
+            flags |= R_MAXITER
+            break
+        it += 1
+        if form == "delta":
+            Z = update_delta_form(Z, R)
+        elif form == "x":
+            Z = update_x_form(Z, X)
+        else:
+            raise ValueError(form)
+        X = triple_product(S, Z)
+    return RefineResult(Z, it, np.asarray(err, dtype=np.float64), flags)
+
+
+def refine_with_refi(S: np.ndarray, Z0: np.ndarray, max_iter: int, low_dtype=np.float32,
+                     refi_steps: int = 1) -> RefineResult:
+    """Algorithm 3: run Alg. 2 in a lower precision until the
+    test fires, then promote Z, recompute X in FP64 and apply `refi_steps`
+    FP64 updates (Sec. IV.B).  err[] is the low-precision
+    history followed by the FP64 Err before each refinement update and after
+    the last one."""
+    low = refine(S, Z0, max_iter, STOP_PAPER, dtype=low_dtype)
+    S64 = np.asarray(S, dtype=np.float64)
+    Z = np.asarray(low.Z, dtype=np.float64)
+    err = list(low.err)
+    for _ in range(refi_steps):
+        R = residual(S64, Z)
+        err.append(err_fro(R))
+        Z = update_delta_form(Z, R)
+    err.append(err_fro(residual(S64, Z)))
+    return RefineResult(Z, low.iters + refi_steps, np.asarray(err), low.flags)
+
+
+def final_residual_per_sqrt_n(S: np.ndarray, Z: np.ndarray) -> float:
+    """||Z^T S Z - I||_F / sqrt(N), the figure north_star asks to report per mode."""
+    return err_fro(residual(np.asarray(S, np.float64), np.asarray(Z, np.float64))) / math.sqrt(S.shape[0])
