@@ -1,0 +1,148 @@
+/* zfac.h -- C ABI of the B200 (sm_100a) Z-refinement library  (libzfac.so)
+ *
+ * The operation (PAPER.md = arxiv 2404.19163, /root/reference/PAPER.md):
+ *   given a symmetric positive definite overlap matrix S and an initial guess Z0
+ *   with ||Z0^T S Z0 - I||_2 < 1 (Eq. 12, Eq. 14), refine Z so
+ *   that Z^T S Z = I, i.e. Z Z^T = S^-1 (Eq. 10), by Algorithm 2
+ *    with m = 2:
+ *
+ *       R_n   = I - Z_n^T (S Z_n)                     (Eq. 13, 22, 26; R = -(X - I))
+ *       Err[n]= ||R_n||_F                             (Alg. 2)
+ *       stop if n > 0 and Err[n] > Err[n-1]^3         (Eq. 38)
+ *       Z_n+1 = Z_n + Z_n (1/2 R_n + 3/8 R_n R_n)     (Eq. 13/16; = Z(15/8 I - 5/4 X + 3/8 X^2))
+ *
+ * Every step above runs in hand-written CUDA kernels (four fused GEMM kernels per
+ * iteration + an O(N^2) copy-in and copy-out per call); there is no CPU fallback:
+ * on a device that is not sm_100 every entry point that would launch work returns
+ * ZFAC_E_UNSUPPORTED.
+ *
+ * Conventions common to all entry points
+ *   - matrices are dense, ROW-MAJOR, N x N, leading dimension `ld` in ELEMENTS, ld >= N;
+ *     S must be stored in full (both triangles);
+ *   - element type is fixed by the mode: double for ZFAC_MODE_F64, float for
+ *     ZFAC_MODE_SPLIT16 and ZFAC_MODE_TF32 ("The matrices Z and S are stored in
+ *     single precision");
+ *   - pointers named d_* are DEVICE pointers, h_* are HOST pointers; the caller owns
+ *     every buffer including the workspace; the library owns only the small host-side
+ *     context object;
+ *   - all functions return a zfac_status; nothing throws or aborts across the ABI;
+ *   - numerical failure (divergence, NaN) is NOT an error code: it is reported in the
+ *     result flags and Z holds the last iterate, as Alg. 2 would leave it;
+ *   - not checked ("straightforward to check separately"): S symmetric
+ *     positive definite, ||Z0^T S Z0 - I||_2 < 1.
+ */
+#ifndef ZFAC_H_
+#define ZFAC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct zfac_ctx zfac_ctx; /* opaque */
+
+/* Precision mode of the four GEMMs of one iteration.
+ *  SPLIT16: the paper's (h)(h)+(h)(l)+(l)(h) scheme (Sec. III.A-B, Eq. 17-32): each FP32
+ *           operand is split into two 16-bit halves, three tensor-core MMA passes per
+ *           product ((l)(l) dropped, Eq. 25/29/32), FP32 accumulation.
+ *  TF32   : one tensor-core pass on FP32 operands truncated to TF32, FP32 accumulation.
+ *  F64    : the paper's `double` scheme (Table I) on the FP64 tensor pipe. */
+typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2 } zfac_mode;
+
+/* Stop rule.  PAPER: Alg. 2's parameter-free test.  FIXED: perform exactly max_iter updates
+ * (benchmarks, and parity against the oracle "for the same number of iterations"). */
+typedef enum { ZFAC_STOP_PAPER = 0, ZFAC_STOP_FIXED = 1 } zfac_stop;
+
+typedef enum {
+  ZFAC_OK = 0,
+  ZFAC_E_INVALID = 1,     /* bad argument (null, n <= 0, ld < n, max_iter < 0, unknown enum)   */
+  ZFAC_E_UNSUPPORTED = 2, /* current device is not compute capability 10.x                     */
+  ZFAC_E_WORKSPACE = 3,   /* workspace null, misaligned (256 B) or smaller than required       */
+  ZFAC_E_CUDA = 4         /* a CUDA runtime/driver call failed (see zfac_last_cuda_error)      */
+} zfac_status;
+
+/* Result flags written to *flags together with the outputs. */
+enum {
+  ZFAC_R_STOPPED = 1,  /* the test Err[n] > Err[n-1]^3 fired (converged to the precision floor) */
+  ZFAC_R_MAXITER = 2,  /* max_iter updates were performed without the test firing               */
+  ZFAC_R_NONFINITE = 4 /* Err[n] became inf/NaN; iteration stopped                               */
+};
+
+/* Internal buffers that zfac_peek can copy out (parity tests of the individual steps).
+ * After a call, T/R hold the values of the LAST residual evaluation (for the returned Z),
+ * Q the polynomial of the last update performed. */
+typedef enum {
+  ZFAC_BUF_T = 0, /* T = (S Z)^T            step a1, Eq. 22 */
+  ZFAC_BUF_R = 1, /* R = I - Z^T S Z        step a2, Eq. 26 */
+  ZFAC_BUF_Q = 2, /* Q = 1/2 R + 3/8 R R    step a4, Eq. 30-32 */
+  ZFAC_BUF_Z = 3  /* current Z              step a5, Eq. 13 */
+} zfac_buf;
+
+/* Bytes of device workspace zfac_create needs for an n x n problem in `mode`
+ * (internal padded operand buffers, partial sums, staging for zfac_refine_host).
+ * Returns 0 for invalid arguments.  Host function, launches nothing. */
+size_t zfac_workspace_bytes(int64_t n, zfac_mode mode);
+
+/* Create a context for n x n problems in `mode`, bound to the CURRENT device and to the
+ * caller-owned device workspace [d_workspace, d_workspace + bytes), which must be 256-byte
+ * aligned and stay alive and otherwise unused until zfac_destroy.  Builds the TMA tensor maps.
+ * One context serves any number of zfac_refine calls (the MD-step use),
+ * one at a time.  Errors: INVALID, WORKSPACE, UNSUPPORTED, CUDA. */
+zfac_status zfac_create(zfac_ctx** ctx, int64_t n, zfac_mode mode, void* d_workspace, size_t bytes);
+
+/* Algorithm 2 on device buffers.  Asynchronous on `stream` (a cudaStream_t passed as void*;
+ * NULL = default stream): enqueues the copy-in kernels, then for n = 0..max_iter the fused
+ * kernels a1 (T=(S Z)^T), a2 (R = I - Z^T S Z, ||R||_F, stop test), a4 (Q = 1/2 R + 3/8 R R),
+ * a5 (Z += Z Q), then the copy-out; no allocation, no host synchronisation; the stop decision
+ * is taken on the device and later kernels of the call exit at once.  Outputs are valid once
+ * the stream has been synchronised.
+ *   d_S  [in]  n x n, lds;   d_Z0 [in] n x n, ldz0;   d_Z [out] n x n, ldz (may alias d_Z0)
+ *   max_iter   upper bound on the number of Z updates (>= 0; 0 returns Z0 and Err[0])
+ *   d_iters [out] int     number of Z updates performed (= stop index; PAPER counts iters+1 X evaluations)
+ *   d_err   [out] double[max_iter+1]; entries 0..iters hold Err[n] = ||R_n||_F, the rest are untouched
+ *   d_flags [out] int     ZFAC_R_* bits
+ * Errors: INVALID (nothing enqueued), CUDA. */
+zfac_status zfac_refine(zfac_ctx* ctx, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0,
+                        void* d_Z, int64_t ldz, int max_iter, zfac_stop stop, int* d_iters,
+                        double* d_err, int* d_flags, void* stream);
+
+/* Same operation on HOST buffers (pinned memory recommended): copies S and Z0 to the device
+ * staging area of the workspace, runs zfac_refine, copies Z, iters, Err[0..max_iter] and flags
+ * back, and synchronises `stream` before returning.  This is the end-to-end call bench.py times. */
+zfac_status zfac_refine_host(zfac_ctx* ctx, const void* h_S, int64_t lds, const void* h_Z0,
+                             int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, zfac_stop stop,
+                             int* h_iters, double* h_err, int* h_flags, void* stream);
+
+/* Copy an internal buffer (top-left n x n block, converted to the mode's element type) to
+ * d_out (n x n, ld).  Asynchronous on `stream`.  For tests of the individual steps. */
+zfac_status zfac_peek(zfac_ctx* ctx, zfac_buf which, void* d_out, int64_t ld, void* stream);
+
+/* Number of kernels the last zfac_refine / zfac_refine_host call on this context enqueued. */
+int zfac_last_launch_count(const zfac_ctx* ctx);
+
+/* Per-kernel timing for benchmarks.  With profiling enabled, zfac_refine records a CUDA event
+ * on the launching stream before every GEMM kernel and after the last one (a few microseconds
+ * of overhead per kernel).  After the stream has been synchronised, zfac_get_profile returns,
+ * for the last call, up to `cap` entries: tags[i] = step id (1 = a1, 2 = a2, 4 = a4, 5 = a5)
+ * + 16 * iteration index, ms[i] = milliseconds until the next event.  Returns the entry count. */
+zfac_status zfac_set_profile(zfac_ctx* ctx, int enable);
+int zfac_get_profile(zfac_ctx* ctx, int* tags, float* ms, int cap);
+
+/* Padded internal dimension used for n in `mode` (multiple of the tile size). */
+int64_t zfac_padded_n(int64_t n, zfac_mode mode);
+
+/* Destroy the context (host memory only; the workspace stays the caller's). NULL is OK. */
+zfac_status zfac_destroy(zfac_ctx* ctx);
+
+/* Static string for a status code. */
+const char* zfac_status_string(zfac_status s);
+
+/* Last CUDA error string recorded on this thread by a ZFAC_E_CUDA return ("" if none). */
+const char* zfac_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ZFAC_H_ */

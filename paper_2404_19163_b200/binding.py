@@ -1,0 +1,244 @@
+"""ctypes binding of libzfac.so -- the same names as include/zfac.h, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; nothing here computes.
+PyTorch is used only for device memory (the workspace and the I/O tensors) and streams.
+If the shared library is missing or cannot be loaded this module raises: there is no CPU
+or PyTorch fallback path.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libzfac.so")
+
+ZFAC_MODE_SPLIT16, ZFAC_MODE_TF32, ZFAC_MODE_F64 = 0, 1, 2
+ZFAC_STOP_PAPER, ZFAC_STOP_FIXED = 0, 1
+ZFAC_OK, ZFAC_E_INVALID, ZFAC_E_UNSUPPORTED, ZFAC_E_WORKSPACE, ZFAC_E_CUDA = 0, 1, 2, 3, 4
+ZFAC_R_STOPPED, ZFAC_R_MAXITER, ZFAC_R_NONFINITE = 1, 2, 4
+ZFAC_BUF_T, ZFAC_BUF_R, ZFAC_BUF_Q, ZFAC_BUF_Z = 0, 1, 2, 3
+
+MODES = {"split16": ZFAC_MODE_SPLIT16, "tf32": ZFAC_MODE_TF32, "f64": ZFAC_MODE_F64}
+
+# symbols include/zfac.h declares (tests check that the library exports every one)
+EXPORTS = [
+    "zfac_workspace_bytes", "zfac_create", "zfac_refine", "zfac_refine_host", "zfac_peek",
+    "zfac_last_launch_count", "zfac_padded_n", "zfac_destroy", "zfac_status_string",
+    "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile",
+]
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+class ZfacError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = f"{where}: {zfac_status_string(status)}"
+        if status == ZFAC_E_CUDA:
+            msg += f" [{lib().zfac_last_cuda_error().decode()}]"
+        super().__init__(msg)
+
+
+def lib() -> ctypes.CDLL:
+    """Load libzfac.so (built by paper_2404_19163_b200.build / __graft_entry__.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2404_19163_b200.build` "
+                           "(the CUDA extension is required; there is no fallback path)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, sz, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.c_int
+    L.zfac_workspace_bytes.restype = sz
+    L.zfac_workspace_bytes.argtypes = [i64, ci]
+    L.zfac_padded_n.restype = i64
+    L.zfac_padded_n.argtypes = [i64, ci]
+    L.zfac_create.restype = ci
+    L.zfac_create.argtypes = [ctypes.POINTER(vp), i64, ci, vp, sz]
+    L.zfac_refine.restype = ci
+    L.zfac_refine.argtypes = [vp, vp, i64, vp, i64, vp, i64, ci, ci, vp, vp, vp, vp]
+    L.zfac_refine_host.restype = ci
+    L.zfac_refine_host.argtypes = [vp, vp, i64, vp, i64, vp, i64, ci, ci, vp, vp, vp, vp]
+    L.zfac_peek.restype = ci
+    L.zfac_peek.argtypes = [vp, ci, vp, i64, vp]
+    L.zfac_last_launch_count.restype = ci
+    L.zfac_last_launch_count.argtypes = [vp]
+    L.zfac_destroy.restype = ci
+    L.zfac_destroy.argtypes = [vp]
+    L.zfac_status_string.restype = ctypes.c_char_p
+    L.zfac_status_string.argtypes = [ci]
+    L.zfac_last_cuda_error.restype = ctypes.c_char_p
+    L.zfac_last_cuda_error.argtypes = []
+    L.zfac_set_profile.restype = ci
+    L.zfac_set_profile.argtypes = [vp, ci]
+    L.zfac_get_profile.restype = ci
+    L.zfac_get_profile.argtypes = [vp, vp, vp, ci]
+    _lib = L
+    return L
+
+
+# ---------------------------------------------------------------- 1:1 wrappers
+def zfac_status_string(status: int) -> str:
+    return lib().zfac_status_string(int(status)).decode()
+
+
+def zfac_workspace_bytes(n: int, mode: int) -> int:
+    return int(lib().zfac_workspace_bytes(int(n), int(mode)))
+
+
+def zfac_padded_n(n: int, mode: int) -> int:
+    return int(lib().zfac_padded_n(int(n), int(mode)))
+
+
+def zfac_create(n: int, mode: int, d_workspace: int, nbytes: int) -> int:
+    """Returns the opaque context handle (int). Raises ZfacError on failure."""
+    h = ctypes.c_void_p()
+    st = lib().zfac_create(ctypes.byref(h), int(n), int(mode), ctypes.c_void_p(d_workspace), int(nbytes))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_create")
+    return h.value
+
+
+def zfac_refine(ctx: int, d_S: int, lds: int, d_Z0: int, ldz0: int, d_Z: int, ldz: int, max_iter: int,
+                stop: int, d_iters: int, d_err: int, d_flags: int, stream: int = 0) -> None:
+    st = lib().zfac_refine(ctx, d_S, lds, d_Z0, ldz0, d_Z, ldz, int(max_iter), int(stop), d_iters, d_err,
+                           d_flags, ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_refine")
+
+
+def zfac_refine_host(ctx: int, h_S: int, lds: int, h_Z0: int, ldz0: int, h_Z: int, ldz: int, max_iter: int,
+                     stop: int, h_iters: int, h_err: int, h_flags: int, stream: int = 0) -> None:
+    st = lib().zfac_refine_host(ctx, h_S, lds, h_Z0, ldz0, h_Z, ldz, int(max_iter), int(stop), h_iters, h_err,
+                                h_flags, ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_refine_host")
+
+
+def zfac_peek(ctx: int, which: int, d_out: int, ld: int, stream: int = 0) -> None:
+    st = lib().zfac_peek(ctx, int(which), d_out, int(ld), ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_peek")
+
+
+def zfac_last_launch_count(ctx: int) -> int:
+    return int(lib().zfac_last_launch_count(ctx))
+
+
+def zfac_set_profile(ctx: int, enable: bool) -> None:
+    st = lib().zfac_set_profile(ctx, int(bool(enable)))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_set_profile")
+
+
+def zfac_get_profile(ctx: int, cap: int = 1024):
+    """[(step_id, iteration, ms), ...] for the GEMM kernels of the last call (stream must be synchronised)."""
+    tags = (ctypes.c_int * cap)()
+    ms = (ctypes.c_float * cap)()
+    k = lib().zfac_get_profile(ctx, ctypes.addressof(tags), ctypes.addressof(ms), cap)
+    return [(tags[i] & 15, tags[i] >> 4, float(ms[i])) for i in range(k)]
+
+
+def zfac_destroy(ctx: int) -> None:
+    lib().zfac_destroy(ctx)
+
+
+# ---------------------------------------------------------------- convenience holder (marshalling only)
+class Zfac:
+    """Owns a torch uint8 workspace tensor and a zfac context for (n, mode) on the current device."""
+
+    def __init__(self, n: int, mode: str | int, device: str | torch.device = "cuda"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("zfac needs a CUDA device (sm_100a); there is no CPU path")
+        self.n = int(n)
+        self.mode = MODES[mode] if isinstance(mode, str) else int(mode)
+        self.dtype = torch.float64 if self.mode == ZFAC_MODE_F64 else torch.float32
+        self.device = torch.device(device)
+        nbytes = zfac_workspace_bytes(self.n, self.mode)
+        if nbytes == 0:
+            raise ZfacError(ZFAC_E_INVALID, "zfac_workspace_bytes")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            self.ctx = zfac_create(self.n, self.mode, self.workspace.data_ptr(), nbytes)
+
+    def close(self) -> None:
+        if getattr(self, "ctx", None):
+            zfac_destroy(self.ctx)
+            self.ctx = None
+            self.workspace = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, t: torch.Tensor, name: str) -> None:
+        if t.dtype != self.dtype or t.dim() != 2 or t.shape[0] != self.n or t.shape[1] != self.n:
+            raise ValueError(f"{name}: expected {self.n}x{self.n} {self.dtype}, got {tuple(t.shape)} {t.dtype}")
+        if t.stride(1) != 1 or t.stride(0) < self.n:
+            raise ValueError(f"{name}: must be row-major with unit column stride")
+
+    def refine(self, S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, stop: int = ZFAC_STOP_PAPER,
+               out: Optional[torch.Tensor] = None, sync: bool = True):
+        """Device tensors in, device tensors out: (Z, iters, err[0..iters], flags).
+        With sync=False returns the raw device tensors (Z, d_iters, d_err, d_flags)."""
+        self._check(S, "S"); self._check(Z0, "Z0")
+        Z = out if out is not None else torch.empty((self.n, self.n), dtype=self.dtype, device=S.device)
+        self._check(Z, "Z")
+        d_iters = torch.zeros(1, dtype=torch.int32, device=S.device)
+        d_flags = torch.zeros(1, dtype=torch.int32, device=S.device)
+        d_err = torch.full((max_iter + 1,), float("nan"), dtype=torch.float64, device=S.device)
+        stream = torch.cuda.current_stream(S.device).cuda_stream
+        zfac_refine(self.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), Z.data_ptr(), Z.stride(0),
+                    max_iter, stop, d_iters.data_ptr(), d_err.data_ptr(), d_flags.data_ptr(), stream)
+        if not sync:
+            return Z, d_iters, d_err, d_flags
+        torch.cuda.current_stream(S.device).synchronize()
+        it = int(d_iters.item())
+        return Z, it, d_err[: it + 1].cpu().numpy(), int(d_flags.item())
+
+    def refine_host(self, S: torch.Tensor, Z0: torch.Tensor, Z: torch.Tensor, max_iter: int = 40,
+                    stop: int = ZFAC_STOP_PAPER):
+        """Host (pinned) tensors in and out, through zfac_refine_host."""
+        import numpy as np
+        for t, name in ((S, "S"), (Z0, "Z0"), (Z, "Z")):
+            self._check(t, name)
+            if t.is_cuda:
+                raise ValueError(f"{name}: refine_host takes host tensors")
+        iters = ctypes.c_int(0)
+        flags = ctypes.c_int(0)
+        err = np.full(max_iter + 1, np.nan, dtype=np.float64)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        with torch.cuda.device(self.device):
+            zfac_refine_host(self.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), Z.data_ptr(),
+                             Z.stride(0), max_iter, stop, ctypes.addressof(iters), err.ctypes.data,
+                             ctypes.addressof(flags), stream)
+        return Z, iters.value, err[: iters.value + 1], flags.value
+
+    def peek(self, which: int) -> torch.Tensor:
+        out = torch.empty((self.n, self.n), dtype=self.dtype, device=self.device)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        zfac_peek(self.ctx, which, out.data_ptr(), out.stride(0), stream)
+        torch.cuda.current_stream(self.device).synchronize()
+        return out
+
+    def set_profile(self, enable: bool) -> None:
+        zfac_set_profile(self.ctx, enable)
+
+    def get_profile(self):
+        return zfac_get_profile(self.ctx)
+
+    @property
+    def last_launch_count(self) -> int:
+        return zfac_last_launch_count(self.ctx)

@@ -1,0 +1,287 @@
+// C ABI of libzfac (see include/zfac.h).  Host-side sequencing only: every step of the
+// path runs in the kernels of zfac_f64.cuh / zfac_umma.cuh / zfac_io.cuh.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <type_traits>
+
+#include "zfac_common.cuh"
+#include "zfac_io.cuh"
+#include "zfac_f64.cuh"
+#include "zfac_umma.cuh"
+
+using namespace zfac;
+
+static thread_local char g_cuda_err[256] = "";
+
+#define ZF_CUDA(call)                                                                     \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "%s:%d %s: %s", __FILE__, __LINE__, #call, \
+               cudaGetErrorString(e_));                                                   \
+      return ZFAC_E_CUDA;                                                                 \
+    }                                                                                     \
+  } while (0)
+
+struct zfac_ctx {
+  int64_t n, np;
+  int mode;
+  char* ws;
+  size_t ws_bytes;
+  Layout L;
+  int launches;
+  int sm_count;
+  UmmaPlan umma;   // tensor maps + launch geometry for the tcgen05 modes
+  Prof prof;
+};
+
+static bool valid_mode(int m) { return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_F64; }
+
+extern "C" {
+
+size_t zfac_workspace_bytes(int64_t n, zfac_mode mode) {
+  if (n <= 0 || n > (1 << 20) || !valid_mode(mode)) return 0;
+  return make_layout(n, mode).total;
+}
+
+int64_t zfac_padded_n(int64_t n, zfac_mode mode) {
+  if (n <= 0 || !valid_mode(mode)) return 0;
+  return padded_n(n, mode);
+}
+
+const char* zfac_status_string(zfac_status s) {
+  switch (s) {
+    case ZFAC_OK: return "ZFAC_OK";
+    case ZFAC_E_INVALID: return "ZFAC_E_INVALID: invalid argument";
+    case ZFAC_E_UNSUPPORTED: return "ZFAC_E_UNSUPPORTED: device is not sm_100 (no fallback path)";
+    case ZFAC_E_WORKSPACE: return "ZFAC_E_WORKSPACE: workspace null, misaligned or too small";
+    case ZFAC_E_CUDA: return "ZFAC_E_CUDA: CUDA call failed";
+  }
+  return "unknown zfac_status";
+}
+
+const char* zfac_last_cuda_error(void) { return g_cuda_err; }
+
+zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_workspace, size_t bytes) {
+  if (!out) return ZFAC_E_INVALID;
+  *out = nullptr;
+  if (n <= 0 || n > (1 << 20) || !valid_mode(mode)) return ZFAC_E_INVALID;
+  Layout L = make_layout(n, mode);
+  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || bytes < L.total) return ZFAC_E_WORKSPACE;
+  int dev = 0, major = 0, sms = 0;
+  ZF_CUDA(cudaGetDevice(&dev));
+  ZF_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  ZF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (major != 10) return ZFAC_E_UNSUPPORTED;
+  zfac_ctx* c = new (std::nothrow) zfac_ctx();
+  if (!c) return ZFAC_E_INVALID;
+  c->n = n; c->np = L.np; c->mode = mode; c->ws = static_cast<char*>(d_workspace); c->ws_bytes = bytes;
+  c->L = L; c->launches = 0; c->sm_count = sms;
+  if (mode == ZFAC_MODE_F64) {
+    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A1>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A2>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A4>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A5>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+  } else {
+    cudaError_t e = umma_plan_create(&c->umma, L, c->ws, sms);
+    if (e != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_plan_create: %s", cudaGetErrorString(e));
+      delete c;
+      return ZFAC_E_CUDA;
+    }
+  }
+  *out = c;
+  return ZFAC_OK;
+}
+
+zfac_status zfac_destroy(zfac_ctx* ctx) {
+  if (ctx) {
+    for (int i = 0; i < ctx->prof.cap; ++i) cudaEventDestroy(ctx->prof.ev[i]);
+    delete[] ctx->prof.ev;
+    delete[] ctx->prof.tags;
+  }
+  delete ctx;
+  return ZFAC_OK;
+}
+
+zfac_status zfac_set_profile(zfac_ctx* c, int enable) {
+  if (!c) return ZFAC_E_INVALID;
+  if (enable && c->prof.cap == 0) {
+    const int cap = 1024;
+    c->prof.ev = new (std::nothrow) cudaEvent_t[cap];
+    c->prof.tags = new (std::nothrow) int[cap];
+    if (!c->prof.ev || !c->prof.tags) return ZFAC_E_INVALID;
+    for (int i = 0; i < cap; ++i) ZF_CUDA(cudaEventCreate(&c->prof.ev[i]));
+    c->prof.cap = cap;
+  }
+  c->prof.on = enable != 0;
+  c->prof.count = 0;
+  return ZFAC_OK;
+}
+
+int zfac_get_profile(zfac_ctx* c, int* tags, float* ms, int cap) {
+  if (!c || !tags || !ms || c->prof.count < 2) return 0;
+  int k = 0;
+  for (int i = 0; i + 1 < c->prof.count && k < cap; ++i) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, c->prof.ev[i], c->prof.ev[i + 1]) != cudaSuccess) return k;
+    tags[k] = c->prof.tags[i];
+    ms[k] = t;
+    ++k;
+  }
+  return k;
+}
+
+int zfac_last_launch_count(const zfac_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s) {
+  const Layout& L = c->L;
+  char* ws = c->ws;
+  State* st = reinterpret_cast<State*>(ws + L.off_state);
+  double* S = reinterpret_cast<double*>(ws + L.off_S);
+  double* W = reinterpret_cast<double*>(ws + L.off_W);
+  double* T = reinterpret_cast<double*>(ws + L.off_T);
+  double* R = reinterpret_cast<double*>(ws + L.off_R);
+  double* Q = reinterpret_cast<double*>(ws + L.off_Q);
+  double* Z[2] = {reinterpret_cast<double*>(ws + L.off_Z[0]), reinterpret_cast<double*>(ws + L.off_Z[1])};
+  const int tiles = (int)(L.np / F64_BM);
+  const int full = tiles * tiles, tri = tiles * (tiles + 1) / 2;
+  F64Params p{};
+  p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = st;
+  p.stop.st = st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
+  p.stop.num_partials = tri; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+  for (int n = 0; n <= max_iter; ++n) {
+    p.A = W; p.B = S; p.out0 = T; p.out1 = nullptr; p.in0 = nullptr;
+    c->prof.mark(s, EPI_A1 + 16 * n);
+    f64_gemm_kernel<EPI_A1><<<full, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    p.A = W; p.B = T; p.out0 = R; p.stop.n_iter = n;
+    c->prof.mark(s, EPI_A2 + 16 * n);
+    f64_gemm_kernel<EPI_A2><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    c->launches += 2;
+    if (n == max_iter) break;
+    p.A = R; p.B = R; p.in0 = R; p.out0 = Q;
+    c->prof.mark(s, EPI_A4 + 16 * n);
+    f64_gemm_kernel<EPI_A4><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    p.A = Z[n & 1]; p.B = Q; p.in0 = Z[n & 1]; p.out0 = Z[(n + 1) & 1]; p.out1 = W;
+    c->prof.mark(s, EPI_A5 + 16 * n);
+    f64_gemm_kernel<EPI_A5><<<full, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    c->launches += 2;
+  }
+  c->prof.mark(s, 0);
+  ZF_CUDA(cudaGetLastError());
+  return ZFAC_OK;
+}
+
+zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
+                        int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
+                        void* stream) {
+  if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
+  if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
+  if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& L = c->L;
+  char* ws = c->ws;
+  State* st = reinterpret_cast<State*>(ws + L.off_state);
+  c->launches = 0;
+  c->prof.count = 0;
+
+  CopyInArgs ci{};
+  ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np; ci.st = st;
+  ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
+  dim3 gi((unsigned)(L.np / 32), (unsigned)(L.np / 32)), bi(32, 8);
+  if (c->mode == ZFAC_MODE_F64) copy_in_kernel<ZFAC_MODE_F64><<<gi, bi, 0, s>>>(ci);
+  else if (c->mode == ZFAC_MODE_TF32) copy_in_kernel<ZFAC_MODE_TF32><<<gi, bi, 0, s>>>(ci);
+  else copy_in_kernel<ZFAC_MODE_SPLIT16><<<gi, bi, 0, s>>>(ci);
+  c->launches += 1;
+
+  zfac_status rs;
+  if (c->mode == ZFAC_MODE_F64) {
+    rs = refine_f64(c, max_iter, stop, d_err, s);
+  } else {
+    int nl = 0;
+    cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, d_err, s, &nl, &c->prof);
+    c->launches += nl;
+    if (e != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_refine: %s", cudaGetErrorString(e));
+      return ZFAC_E_CUDA;
+    }
+    rs = ZFAC_OK;
+  }
+  if (rs != ZFAC_OK) return rs;
+
+  CopyOutArgs co{};
+  co.Zbuf[0] = ws + L.off_Z[0]; co.Zbuf[1] = ws + L.off_Z[1];
+  co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np; co.st = st; co.d_iters = d_iters; co.d_flags = d_flags;
+  dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
+  if (c->mode == ZFAC_MODE_F64) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
+  else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
+  c->launches += 1;
+  ZF_CUDA(cudaGetLastError());
+  return ZFAC_OK;
+}
+
+zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const void* h_Z0, int64_t ldz0, void* h_Z,
+                             int64_t ldz, int max_iter, zfac_stop stop, int* h_iters, double* h_err, int* h_flags,
+                             void* stream) {
+  if (!c || !h_S || !h_Z0 || !h_Z || !h_iters || !h_err || !h_flags) return ZFAC_E_INVALID;
+  if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0 || max_iter > 4095) return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& L = c->L;
+  char* dS = c->ws + L.off_stage_S;
+  char* dZ = c->ws + L.off_stage_Z;
+  double* dErr = reinterpret_cast<double*>(c->ws + L.off_stage_out);
+  int* dInts = reinterpret_cast<int*>(c->ws + L.off_stage_out + 4096 * sizeof(double));
+  const size_t row = (size_t)c->n * L.elt;
+  ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+  ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+  zfac_status rs = zfac_refine(c, dS, c->n, dZ, c->n, dZ, c->n, max_iter, stop, dInts, dErr, dInts + 1, s);
+  if (rs != ZFAC_OK) return rs;
+  ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
+  int ints[2] = {0, 0};
+  ZF_CUDA(cudaMemcpyAsync(ints, dInts, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
+  ZF_CUDA(cudaStreamSynchronize(s));
+  *h_iters = ints[0]; *h_flags = ints[1];
+  ZF_CUDA(cudaMemcpyAsync(h_err, dErr, (size_t)(ints[0] + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
+  ZF_CUDA(cudaStreamSynchronize(s));
+  return ZFAC_OK;
+}
+
+zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void* stream) {
+  if (!c || !d_out || ld < c->n) return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& L = c->L;
+  char* ws = c->ws;
+  const int n = (int)c->n, np = (int)L.np;
+  dim3 g((unsigned)((n + 255) / 256), (unsigned)n);
+  // the current Z buffer index is only known on the device; read it (peek is a test hook, it may sync)
+  State hst{};
+  ZF_CUDA(cudaStreamSynchronize(s));
+  ZF_CUDA(cudaMemcpy(&hst, ws + L.off_state, sizeof(State), cudaMemcpyDeviceToHost));
+  if (c->mode == ZFAC_MODE_F64 || c->mode == ZFAC_MODE_TF32) {
+    size_t off;
+    switch (which) {
+      case ZFAC_BUF_T: off = L.off_T; break;
+      case ZFAC_BUF_R: off = L.off_R; break;
+      case ZFAC_BUF_Q: off = L.off_Q; break;
+      case ZFAC_BUF_Z: off = L.off_Z[hst.iters & 1]; break;
+      default: return ZFAC_E_INVALID;
+    }
+    if (c->mode == ZFAC_MODE_F64) peek_kernel<double, 0><<<g, 256, 0, s>>>(ws + off, d_out, ld, n, np);
+    else peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + off, d_out, ld, n, np);
+  } else {
+    switch (which) {
+      case ZFAC_BUF_T: peek_kernel<float, 1><<<g, 256, 0, s>>>(ws + L.off_T, d_out, ld, n, np); break;
+      case ZFAC_BUF_R: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
+      case ZFAC_BUF_Q: peek_kernel<float, 2><<<g, 256, 0, s>>>(ws + L.off_Qb, d_out, ld, n, np); break;
+      case ZFAC_BUF_Z: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_Z[0], d_out, ld, n, np); break;
+      default: return ZFAC_E_INVALID;
+    }
+  }
+  ZF_CUDA(cudaGetLastError());
+  return ZFAC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,118 @@
+// Shared device-side pieces of libzfac: the per-call state block, the on-device
+// stopping test (step a3) and small helpers.  No oracle code is shared with this file.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/zfac.h"
+
+namespace zfac {
+
+// Lives at the start of the workspace.  Reset by the first copy-in kernel of every call.
+struct State {
+  int done;                  // set by step a3; every later kernel of the call exits at once
+  int iters;                 // number of Z updates performed so far (= index of the last Err)
+  int flags;                 // ZFAC_R_* bits
+  int pad0;
+  unsigned int arrive[4];    // last-CTA counters (one per use site), self-resetting
+  double zscale;             // reserved
+};
+
+struct StopArgs {
+  State* st;
+  double* partials;          // one FP64 partial sum of squares per output tile
+  int num_partials;
+  double* d_err;             // user array, max_iter + 1 entries
+  int n_iter;                // index n of the residual being evaluated
+  int max_iter;
+  int stop;                  // zfac_stop
+};
+
+// Optional per-kernel timing (zfac_set_profile): an event is recorded on the launching stream
+// before every GEMM kernel and one after the last; tags = step id (1,2,4,5) + 16 * iteration.
+struct Prof {
+  cudaEvent_t* ev = nullptr;
+  int* tags = nullptr;
+  int cap = 0, count = 0;
+  bool on = false;
+  inline void mark(cudaStream_t s, int tag) {
+    if (!on || count >= cap) return;
+    cudaEventRecord(ev[count], s);
+    tags[count] = tag;
+    ++count;
+  }
+};
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Step a3 (Alg. 2, Eq. 38).  Called by ALL threads of the CTA that
+// finished last (blockDim.x <= 1024, multiple of 32).  Sums the per-tile partials in a fixed
+// order (thread-strided, then a fixed shuffle/smem tree), so Err[] is run-to-run deterministic.
+// Readings: strict '>' (Q9); test applied unconditionally as Alg. 2 prints it (Q10);
+// non-finite Err stops with a flag (Q9); Err recorded for the final Z also at max_iter (Q7).
+__device__ inline void stop_test_last_cta(const StopArgs& a, double* smem_red /* >= 32 doubles */) {
+  double s = 0.0;
+  for (int i = threadIdx.x; i < a.num_partials; i += blockDim.x) s += __ldcg(a.partials + i);
+  s = warp_sum(s);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  if (lane == 0) smem_red[wid] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int w = 0; w < nw; ++w) tot += smem_red[w];
+    const double err = sqrt(tot);
+    const int n = a.n_iter;
+    a.d_err[n] = err;
+    State* st = a.st;
+    st->iters = n;
+    int flags = 0, done = 0;
+    if (!isfinite(err)) {
+      flags = ZFAC_R_NONFINITE; done = 1;
+    } else if (a.stop == ZFAC_STOP_PAPER && n > 0) {
+      const double prev = a.d_err[n - 1];
+      if (err > prev * prev * prev) { flags = ZFAC_R_STOPPED; done = 1; }
+    }
+    if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
+    if (done) { st->flags |= flags; __threadfence(); st->done = 1; }
+  }
+}
+
+// Returns true (to every thread of the CTA) if this CTA is the last of `total` to arrive.
+__device__ inline bool arrive_is_last(unsigned int* counter, unsigned int total, int* smem_flag) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned int prev = atomicAdd(counter, 1u);
+    const int last = (prev == total - 1u);
+    if (last) { *counter = 0u; __threadfence(); }
+    *smem_flag = last;
+  }
+  __syncthreads();
+  return *smem_flag != 0;
+}
+
+// Upper-triangle enumeration: t -> (i <= j), t = j (j + 1) / 2 + i.
+__device__ __forceinline__ void tri_decode(int t, int& i, int& j) {
+  int jj = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+  while ((jj + 1) * (jj + 2) / 2 <= t) ++jj;
+  while (jj * (jj + 1) / 2 > t) --jj;
+  j = jj;
+  i = t - jj * (jj + 1) / 2;
+}
+
+// Full-grid rasterisation in bands of `bw` tile-columns so that co-resident CTAs share
+// operand rows/columns in L2.
+__device__ __forceinline__ void band_decode(int t, int tiles_m, int tiles_n, int bw, int& mi, int& ni) {
+  const int per_band = bw * tiles_m;
+  const int band = t / per_band;
+  const int r = t - band * per_band;
+  int nb = tiles_n - band * bw;
+  nb = nb < bw ? nb : bw;
+  mi = r / nb;
+  ni = band * bw + (r - mi * nb);
+}
+
+}  // namespace zfac

@@ -1,0 +1,205 @@
+// Workspace layout and the O(N^2) copy-in / copy-out kernels (steps a0 and a6).
+//
+// Padding (Sec. V.E, :398-400): the library works on internal buffers whose
+// dimension Np is a multiple of the tile size.  The extra rows/columns of S and Z are
+// filled with an IDENTITY block, S_pad = diag(S, I), Z_pad = diag(Z, I), which makes the
+// padded problem exact: R is zero there, no epilogue needs a predicate and ||R||_F is
+// unchanged (zero padding would add Np - N to ||R||_F^2).
+//
+// Operand splitting (Eq. 17-18, :143-149): A ~ A_hi + A_lo.
+//   fp16 pair (residual GEMMs a1, a2):  hi = FP16[a],  lo' = FP16[(a - FP32[hi]) * 2^11]
+//       -- the low half is stored SCALED by 2^11 so that it does not fall into the FP16
+//       subnormal range; the products that contain one lo' are accumulated separately and
+//       weighted by 2^-11 in the epilogue.  Error <= 2^-22 |a| as in PAPER.md:169.
+//   bf16 pair (update GEMMs a4, a5):    hi = BF16[a],  lo = BF16[a - FP32[hi]]
+//       -- 16 significant bits, FP32 exponent range: R and Q shrink towards 0 as the
+//       iteration converges and would underflow FP16.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include "zfac_common.cuh"
+
+namespace zfac {
+
+constexpr float LO_SCALE = 2048.0f;           // 2^11
+constexpr float LO_UNSCALE = 1.0f / 2048.0f;  // 2^-11
+
+__device__ __forceinline__ __half f2h_sat(float a) {
+  unsigned short r;
+  asm("cvt.rn.satfinite.f16.f32 %0, %1;" : "=h"(r) : "f"(a));
+  return __ushort_as_half(r);
+}
+__device__ __forceinline__ void split_f16(float a, __half& hi, __half& lo) {
+  hi = f2h_sat(a);
+  lo = f2h_sat((a - __half2float(hi)) * LO_SCALE);
+}
+__device__ __forceinline__ void split_bf16(float a, __nv_bfloat16& hi, __nv_bfloat16& lo) {
+  hi = __float2bfloat16_rn(a);
+  lo = __float2bfloat16_rn(a - __bfloat162float(hi));
+}
+
+// Round-to-nearest FP32 -> TF32 (low 13 mantissa bits cleared).  The tensor core TRUNCATES FP32
+// operands to TF32, which biases every product towards zero; operand buffers that are only ever
+// read by the tensor core are therefore stored pre-rounded.
+__device__ __forceinline__ float round_tf32(float a) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(a));
+  return __uint_as_float(r);
+}
+
+inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+struct Layout {
+  int64_t n = 0, np = 0;
+  int mode = 0;
+  size_t elt = 0;  // user element size
+  size_t off_state = 0, off_partials = 0, num_partials = 0;
+  size_t off_stage_S = 0, off_stage_Z = 0, off_stage_out = 0;
+  // F64 / TF32: one buffer each of the mode's element type; Z double-buffered
+  size_t off_S = 0, off_W = 0, off_T = 0, off_R = 0, off_Q = 0, off_Z[2] = {0, 0};
+  // SPLIT16: S16/W16/T16 are fp16 [2][Np][Np]; Rb/Qb/Zb[2] bf16 [2][Np][Np]; R and Z(=off_Z[0]) fp32
+  size_t off_Rb = 0, off_Qb = 0, off_Zb[2] = {0, 0};
+  size_t total = 0;
+};
+
+inline int64_t padded_n(int64_t n, int mode) { return round_up(n, mode == ZFAC_MODE_F64 ? 128 : 256); }
+
+inline Layout make_layout(int64_t n, int mode) {
+  Layout L;
+  L.n = n; L.mode = mode; L.np = padded_n(n, mode);
+  L.elt = (mode == ZFAC_MODE_F64) ? 8 : 4;
+  const size_t np2 = (size_t)L.np * (size_t)L.np, n2 = (size_t)n * (size_t)n;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 1023) / 1024 * 1024; return o; };
+  L.off_state = take(sizeof(State));
+  L.num_partials = (size_t)(L.np / 128) * (size_t)(L.np / 128);
+  L.off_partials = take(L.num_partials * sizeof(double));
+  L.off_stage_S = take(n2 * L.elt);
+  L.off_stage_Z = take(n2 * L.elt);
+  L.off_stage_out = take((size_t)4096 * sizeof(double) + 64);
+  if (mode == ZFAC_MODE_SPLIT16) {
+    L.off_S = take(np2 * 4); L.off_W = take(np2 * 4); L.off_T = take(np2 * 4);
+    L.off_R = take(np2 * 4); L.off_Rb = take(np2 * 4); L.off_Qb = take(np2 * 4);
+    L.off_Z[0] = take(np2 * 4); L.off_Z[1] = L.off_Z[0];
+    L.off_Zb[0] = take(np2 * 4); L.off_Zb[1] = take(np2 * 4);
+  } else {
+    L.off_S = take(np2 * L.elt); L.off_W = take(np2 * L.elt); L.off_T = take(np2 * L.elt);
+    L.off_R = take(np2 * L.elt); L.off_Q = take(np2 * L.elt);
+    L.off_Z[0] = take(np2 * L.elt); L.off_Z[1] = take(np2 * L.elt);
+  }
+  L.total = off;
+  return L;
+}
+
+// ------------------------------------------------------------------ copy-in (step a0)
+struct CopyInArgs {
+  const void* S; int64_t lds;
+  const void* Z0; int64_t ldz0;
+  int n, np;
+  State* st;
+  void* oS;            // F64: double[Np][Np]; TF32: float; SPLIT16: half[2][Np][Np]
+  void* oZ;            // F64/TF32: Z[0];  SPLIT16: float Z32
+  void* oW;            // F64/TF32: W;     SPLIT16: half[2][Np][Np]
+  void* oZb;           // SPLIT16: bf16[2][Np][Np] (Zb[0])
+};
+
+// One 32x32 tile per CTA (32 x 8 threads).  Reads S and Z0 tiles (identity padding beyond n),
+// writes S, Z (row-major) and W = Z^T (through a shared-memory transpose).
+template <int MODE>
+__global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
+  using Tin = typename std::conditional<MODE == ZFAC_MODE_F64, double, float>::type;
+  __shared__ Tin tile[32][33];
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) {
+    a.st->done = 0; a.st->iters = 0; a.st->flags = 0;
+    a.st->arrive[0] = a.st->arrive[1] = a.st->arrive[2] = a.st->arrive[3] = 0u;
+  }
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+  const size_t np = (size_t)a.np, np2 = np * np;
+  const Tin* S = static_cast<const Tin*>(a.S);
+  const Tin* Z0 = static_cast<const Tin*>(a.Z0);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = r0 + ty + i * 8, c = c0 + tx;
+    const bool in = (r < a.n && c < a.n);
+    const Tin ident = (r == c) ? Tin(1) : Tin(0);
+    const Tin s = in ? S[(size_t)r * a.lds + c] : ident;
+    const Tin z = in ? Z0[(size_t)r * a.ldz0 + c] : ident;
+    tile[ty + i * 8][tx] = z;
+    const size_t o = (size_t)r * np + c;
+    if (MODE == ZFAC_MODE_SPLIT16) {
+      __half hi, lo; split_f16((float)s, hi, lo);
+      static_cast<__half*>(a.oS)[o] = hi; static_cast<__half*>(a.oS)[np2 + o] = lo;
+      static_cast<float*>(a.oZ)[o] = (float)z;
+      __nv_bfloat16 bh, bl; split_bf16((float)z, bh, bl);
+      static_cast<__nv_bfloat16*>(a.oZb)[o] = bh; static_cast<__nv_bfloat16*>(a.oZb)[np2 + o] = bl;
+    } else if (MODE == ZFAC_MODE_TF32) {
+      static_cast<float*>(a.oS)[o] = round_tf32((float)s);
+      static_cast<float*>(a.oZ)[o] = (float)z;
+    } else {
+      static_cast<Tin*>(a.oS)[o] = s;
+      static_cast<Tin*>(a.oZ)[o] = z;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = c0 + ty + i * 8, c = r0 + tx;      // W[r][c] = Z[c][r]
+    const Tin z = tile[tx][ty + i * 8];
+    const size_t o = (size_t)r * np + c;
+    if (MODE == ZFAC_MODE_SPLIT16) {
+      __half hi, lo; split_f16((float)z, hi, lo);
+      static_cast<__half*>(a.oW)[o] = hi; static_cast<__half*>(a.oW)[np2 + o] = lo;
+    } else if (MODE == ZFAC_MODE_TF32) {
+      static_cast<float*>(a.oW)[o] = round_tf32((float)z);
+    } else {
+      static_cast<Tin*>(a.oW)[o] = z;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ copy-out (step a6)
+struct CopyOutArgs {
+  const void* Zbuf[2];   // internal Z buffers (selected by iters parity; equal in SPLIT16)
+  void* Z; int64_t ldz;
+  int n, np;
+  const State* st;
+  int* d_iters; int* d_flags;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
+  const int iters = a.st->iters;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { *a.d_iters = iters; *a.d_flags = a.st->flags; }
+  const T* src = static_cast<const T*>(a.Zbuf[iters & 1]);
+  T* dst = static_cast<T*>(a.Z);
+  const int c = blockIdx.x * 256 + threadIdx.x;
+  const int r0 = blockIdx.y * 8;
+  if (c >= a.n) return;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int r = r0 + i;
+    if (r < a.n) dst[(size_t)r * a.ldz + c] = src[(size_t)r * a.np + c];
+  }
+}
+
+// ------------------------------------------------------------------ peek (tests)
+// kind 0: plain T buffer; 1: fp16 pair hi + lo' 2^-11; 2: bf16 pair hi + lo
+template <typename T, int KIND>
+__global__ void __launch_bounds__(256) peek_kernel(const void* src, void* out, int64_t ld, int n, int np) {
+  const int c = blockIdx.x * 256 + threadIdx.x, r = blockIdx.y;
+  if (c >= n || r >= n) return;
+  const size_t o = (size_t)r * np + c, np2 = (size_t)np * np;
+  T v;
+  if (KIND == 0) v = static_cast<const T*>(src)[o];
+  else if (KIND == 1) {
+    const __half* h = static_cast<const __half*>(src);
+    v = (T)(__half2float(h[o]) + __half2float(h[np2 + o]) * LO_UNSCALE);
+  } else {
+    const __nv_bfloat16* h = static_cast<const __nv_bfloat16*>(src);
+    v = (T)(__bfloat162float(h[o]) + __bfloat162float(h[np2 + o]));
+  }
+  static_cast<T*>(out)[(size_t)r * ld + c] = v;
+}
+
+}  // namespace zfac

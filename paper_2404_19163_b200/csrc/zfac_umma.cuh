@@ -1,0 +1,558 @@
+// tcgen05 (5th-gen tensor core) GEMM kernels for the SPLIT16 and TF32 modes.
+//
+// One persistent, warp-specialised kernel template serves all four GEMMs of an iteration.
+// As in zfac_f64.cuh every product is brought to  D[m][n] = sum_k A[m][k] B[n][k]  with both
+// operands K-major (row-major storage), by keeping W = Z^T next to Z:
+//   a1  T = (S Z)^T = W S^T    (Eq. 22)     a2  X = Z^T (S Z) = W T^T   (Eq. 26)
+//   a4  P = R R = R R^T        (Eq. 30-32)  a5  Z Q = Z Q^T             (Eq. 13)
+//
+// Roles (192 threads): warp 0 = TMA producer (one lane), warp 1 = TMEM allocator + MMA issuer
+// (one lane issues tcgen05.mma), warps 2-5 = epilogue (tcgen05.ld, fused O(N^2) work, stores).
+// Pipelines: shared-memory ring full/empty mbarriers (TMA <-> MMA) and TMEM full/empty
+// mbarriers (MMA <-> epilogue).  CTA tile 128 x 256, operands staged by TMA in the canonical
+// K-major 128B-swizzle layout, accumulators in TMEM (512 columns).
+//
+// Precision kinds
+//   KIND_F16X2  (a1, a2 of SPLIT16): operands are fp16 pairs (hi, lo' = lo * 2^11), Eq. 17-18.
+//       Three MMA passes per k-step, (l)(l) dropped (Eq. 25, 29):
+//           D_hh += A_hi B_hi          D_x += A_hi B_lo' + A_lo' B_hi
+//       two FP32 accumulators; the epilogue forms D_hh + 2^-11 D_x.
+//   KIND_BF16X2 (a4, a5 of SPLIT16): operands are bf16 pairs (hi, lo); three passes into ONE
+//       accumulator; two accumulator buffers so the epilogue overlaps the next tile.
+//   KIND_TF32   (TF32 mode): FP32 operands read as TF32, one pass, two accumulator buffers.
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include "zfac_common.cuh"
+#include "zfac_io.cuh"
+#include "zfac_f64.cuh"   // EPI_* ids
+
+namespace zfac {
+
+enum { KIND_F16X2 = 0, KIND_BF16X2 = 1, KIND_TF32 = 2 };
+
+constexpr int UM_BM = 128, UM_BN = 256;
+constexpr int UM_THREADS = 192;
+constexpr int UM_ROWB = 128;                     // bytes per operand row per k-block (= swizzle span)
+constexpr int UM_A_BYTES = UM_BM * UM_ROWB;      // 16 KB
+constexpr int UM_B_BYTES = UM_BN * UM_ROWB;      // 32 KB
+constexpr int UM_SMEM_OPERANDS = 192 * 1024;
+constexpr int UM_SMEM_BYTES = UM_SMEM_OPERANDS + 1024 /*align*/ + 256 /*barriers*/;
+constexpr int UM_TMEM_COLS = 512;
+
+template <int KIND> struct KindTraits;
+template <> struct KindTraits<KIND_F16X2> {
+  static constexpr int ARRAYS = 2, STAGES = 2, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 1, FMT = 0;
+};
+template <> struct KindTraits<KIND_BF16X2> {
+  static constexpr int ARRAYS = 2, STAGES = 2, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 2, FMT = 1;
+};
+template <> struct KindTraits<KIND_TF32> {
+  static constexpr int ARRAYS = 1, STAGES = 4, KSTEP_ELEMS = 8, BK_ELEMS = 32, ACC_BUFS = 2, FMT = 2;
+};
+
+struct UmmaParams {
+  CUtensorMap mapA;     // A-operand buffer: [ARRAYS*Np rows][Np cols], box 128B x 128 rows
+  CUtensorMap mapB;     // B-operand buffer, same box
+  int np;               // padded dimension (= K)
+  int macro_tiles;      // Np / 256
+  State* st;
+  StopArgs stop;        // a2 only (partials = one per CTA)
+  // epilogue pointers (which are used depends on EPI / KIND; see the epilogue)
+  float* f32_out;       // a1: T32 (TF32)   a2: R32   a4: Q32 (TF32)   a5: Z32 next
+  const float* f32_in;  // a4: R32          a5: Z32 current
+  void* h_out;          // SPLIT16: a1: T16   a2: Rb   a4: Qb   a5: Zb next   (pairs [2][Np][Np])
+  void* h_out_t;        // SPLIT16: a5: W16 (pair, transposed)                TF32: a5: W32
+};
+
+// ------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// Bounded wait: a pipeline bug traps (launch failure) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  unsigned long long spins = 0;
+  while (true) {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (ok) break;
+    if (++spins > (1ull << 26)) __trap();
+  }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+template <int KIND>
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
+  if (KIND == KIND_TF32) {
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
+  } else {
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
+  }
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// K-major, 128B-swizzle shared-memory matrix descriptor (sm_100 version bit 46).
+__device__ __forceinline__ uint64_t make_sdesc(uint32_t saddr) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// kind::f16 / kind::tf32 instruction descriptor: D = F32, A/B format, both K-major, M = 128, N = 256.
+__host__ __device__ constexpr uint32_t make_idesc(int fmt) {
+  return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(UM_BN >> 3) << 17) | ((uint32_t)(UM_BM >> 4) << 24);
+}
+
+__device__ __forceinline__ uint32_t pack_h2(__half a, __half b) {
+  return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
+}
+__device__ __forceinline__ uint32_t pack_b2(__nv_bfloat16 a, __nv_bfloat16 b) {
+  return (uint32_t)__bfloat16_as_ushort(a) | ((uint32_t)__bfloat16_as_ushort(b) << 16);
+}
+
+// Write 32 consecutive values of one row as a 16-bit pair (hi -> base, lo -> base + plane).
+template <bool F16>
+__device__ __forceinline__ void store_pair_row32(void* base, size_t plane, size_t off, const float (&v)[32]) {
+  uint32_t hi[16], lo[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {
+    if (F16) {
+      __half h0, l0, h1, l1;
+      split_f16(v[2 * j], h0, l0); split_f16(v[2 * j + 1], h1, l1);
+      hi[j] = pack_h2(h0, h1); lo[j] = pack_h2(l0, l1);
+    } else {
+      __nv_bfloat16 h0, l0, h1, l1;
+      split_bf16(v[2 * j], h0, l0); split_bf16(v[2 * j + 1], h1, l1);
+      hi[j] = pack_b2(h0, h1); lo[j] = pack_b2(l0, l1);
+    }
+  }
+  uint16_t* b = static_cast<uint16_t*>(base);
+  uint4* ph = reinterpret_cast<uint4*>(b + off);
+  uint4* pl = reinterpret_cast<uint4*>(b + plane + off);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    ph[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
+    pl[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
+  }
+}
+// Transposed: value j of this lane goes to row (n + j), column m (lanes hold consecutive m).
+template <bool F16>
+__device__ __forceinline__ void store_pair_col32(void* base, size_t plane, size_t off_n0_m, size_t ld, const float (&v)[32]) {
+  uint16_t* b = static_cast<uint16_t*>(base);
+#pragma unroll
+  for (int j = 0; j < 32; ++j) {
+    uint16_t h, l;
+    if (F16) { __half hh, ll; split_f16(v[j], hh, ll); h = __half_as_ushort(hh); l = __half_as_ushort(ll); }
+    else { __nv_bfloat16 hh, ll; split_bf16(v[j], hh, ll); h = __bfloat16_as_ushort(hh); l = __bfloat16_as_ushort(ll); }
+    b[off_n0_m + (size_t)j * ld] = h;
+    b[plane + off_n0_m + (size_t)j * ld] = l;
+  }
+}
+__device__ __forceinline__ void store_f32_row32(float* p, const float (&v)[32]) {
+  float4* q = reinterpret_cast<float4*>(p);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) q[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+}
+__device__ __forceinline__ void load_f32_row32(const float* p, float (&v)[32]) {
+  const float4* q = reinterpret_cast<const float4*>(p);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const float4 t = q[j];
+    v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+  }
+}
+
+// ------------------------------------------------------------------ the kernel
+// MODE_SPLIT: true for the SPLIT16 mode kernels (16-bit pair outputs), false for TF32 mode.
+template <int KIND, int EPI>
+__global__ void __launch_bounds__(UM_THREADS, 1) umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
+  if (*((volatile int*)&p.st->done)) return;       // stop decided earlier in this call
+
+  using KT = KindTraits<KIND>;
+  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4);
+  constexpr int STAGE_BYTES = KT::ARRAYS * (UM_A_BYTES + UM_B_BYTES);
+  static_assert(KT::STAGES * STAGE_BYTES <= UM_SMEM_OPERANDS, "smem");
+  constexpr int KSTEPS = KT::BK_ELEMS / KT::KSTEP_ELEMS;   // 4
+  constexpr uint32_t IDESC = make_idesc(KT::FMT);
+
+  extern __shared__ unsigned char smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + UM_SMEM_OPERANDS;
+  // barrier slots (8 B each): full[0..3], empty[4..7], tmem_full[8..9], tmem_empty[10..11]; tmem ptr at +96
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 32u + 8u * s; };
+  auto tfull_bar = [&](int b) { return bar_base + 64u + 8u * b; };
+  auto tempty_bar = [&](int b) { return bar_base + 80u + 8u * b; };
+  const uint32_t tmem_slot = bar_base + 96u;
+  __shared__ double red[8];
+  __shared__ int last_flag;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int np = p.np;
+  const int KB = np / KT::BK_ELEMS;
+  const int T = p.macro_tiles;
+  const int num_tiles = SYM ? T * (T + 1) : 2 * T * T;     // CTA tiles (two 128-row halves per macro tile)
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int b = 0; b < KT::ACC_BUFS; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 128); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(UM_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
+    const int macro = t >> 1, h = t & 1;
+    int I, J;
+    if (SYM) tri_decode(macro, I, J);
+    else band_decode(macro, T, T, 4, I, J);
+    m0 = I * 256 + h * 128;
+    n0 = J * 256;
+    offdiag = (I != J);
+  };
+
+  double cta_sumsq = 0.0;
+
+  if (warp == 0) {
+    // ===================================================== TMA producer
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+        int m0, n0; bool od; decode(t, m0, n0, od);
+        for (int kb = 0; kb < KB; ++kb) {
+          mbar_wait(empty_bar(stage), phase ^ 1u);
+          mbar_expect_tx(full_bar(stage), STAGE_BYTES);
+          const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          const int kc = kb * KT::BK_ELEMS;
+#pragma unroll
+          for (int a = 0; a < KT::ARRAYS; ++a) {
+            tma_load_2d(sa + a * UM_A_BYTES, &p.mapA, kc, a * np + m0, full_bar(stage));
+            const uint32_t sb = sa + KT::ARRAYS * UM_A_BYTES + a * UM_B_BYTES;
+            tma_load_2d(sb, &p.mapB, kc, a * np + n0, full_bar(stage));
+            tma_load_2d(sb + UM_A_BYTES, &p.mapB, kc, a * np + n0 + 128, full_bar(stage));
+          }
+          if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================================== MMA issuer
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      int buf = 0; uint32_t accphase = 0;
+      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+        mbar_wait(tempty_bar(buf), accphase ^ 1u);
+        tc_fence_after();
+        const uint32_t d0 = tmem_base + (KT::ACC_BUFS == 2 ? buf * 256 : 0);   // D (or D_hh)
+        const uint32_t d1 = tmem_base + 256;                                     // D_x (KIND_F16X2 only)
+        for (int kb = 0; kb < KB; ++kb) {
+          mbar_wait(full_bar(stage), phase);
+          tc_fence_after();
+          const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          const uint64_t a_hi = make_sdesc(sa);
+          const uint64_t a_lo = make_sdesc(sa + UM_A_BYTES);
+          const uint64_t b_hi = make_sdesc(sa + KT::ARRAYS * UM_A_BYTES);
+          const uint64_t b_lo = make_sdesc(sa + KT::ARRAYS * UM_A_BYTES + UM_B_BYTES);
+#pragma unroll
+          for (int k = 0; k < KSTEPS; ++k) {
+            const uint32_t acc = (kb | k) ? 1u : 0u;
+            const uint64_t ko = (uint64_t)(k * 2);            // 32 bytes per k-step, in 16-byte units
+            if (KIND == KIND_F16X2) {
+              tc_mma<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, acc);
+              tc_mma<KIND>(d1, a_lo + ko, b_hi + ko, IDESC, 1u);
+              tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
+            } else if (KIND == KIND_BF16X2) {
+              tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
+              tc_mma<KIND>(d0, a_hi + ko, b_lo + ko, IDESC, 1u);
+              tc_mma<KIND>(d0, a_lo + ko, b_hi + ko, IDESC, 1u);
+            } else {
+              tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
+            }
+          }
+          tc_commit(empty_bar(stage));                         // frees the smem stage when the MMAs retire
+          if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
+        }
+        tc_commit(tfull_bar(buf));                             // accumulator complete
+        if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
+        else accphase ^= 1u;
+      }
+    }
+  } else {
+    // ===================================================== epilogue warps (2..5)
+    const int q = warp & 3;                                    // TMEM lane quarter this warp may read
+    const int row = q * 32 + lane;
+    const size_t ld = (size_t)np, plane = ld * ld;
+    int buf = 0; uint32_t accphase = 0;
+    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+      int m0, n0; bool offdiag; decode(t, m0, n0, offdiag);
+      const int m = m0 + row;
+      mbar_wait(tfull_bar(buf), accphase);
+      tc_fence_after();
+      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (KT::ACC_BUFS == 2 ? buf * 256 : 0);
+      double tile_sumsq = 0.0;
+#pragma unroll 1
+      for (int c = 0; c < UM_BN / 32; ++c) {
+        const int n = n0 + c * 32;
+        float v[32];
+        {
+          uint32_t r[32];
+          tmem_ld32(tbase + c * 32, r);
+          if (KIND == KIND_F16X2) {
+            uint32_t x[32];
+            tmem_ld32(tbase + 256 + c * 32, x);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) + __uint_as_float(x[j]) * LO_UNSCALE;
+          } else {
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+          }
+        }
+        const size_t off = (size_t)m * ld + n;               // (m, n)
+        const size_t offt = (size_t)n * ld + m;              // (n, m)
+        if (EPI == EPI_A1) {                                  // T = (S Z)^T
+          if (KIND == KIND_TF32) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = round_tf32(v[j]);
+            store_f32_row32(p.f32_out + off, v);
+          } else store_pair_row32<true>(p.h_out, plane, off, v);
+        } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            v[j] = ((m == n + j) ? 1.0f : 0.0f) - v[j];
+            tile_sumsq += (double)v[j] * (double)v[j];
+          }
+          store_f32_row32(p.f32_out + off, v);
+          if (KIND != KIND_TF32) store_pair_row32<false>(p.h_out, plane, off, v);
+          if (offdiag) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
+            if (KIND != KIND_TF32) store_pair_col32<false>(p.h_out, plane, offt, ld, v);
+          }
+        } else if (EPI == EPI_A4) {                           // Q = 1/2 R + 3/8 R R, mirror
+          float r32[32];
+          load_f32_row32(p.f32_in + off, r32);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] = 0.5f * r32[j] + 0.375f * v[j];
+          if (KIND == KIND_TF32) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = round_tf32(v[j]);
+            store_f32_row32(p.f32_out + off, v);
+            if (offdiag) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
+            }
+          } else {
+            store_pair_row32<false>(p.h_out, plane, off, v);
+            if (offdiag) store_pair_col32<false>(p.h_out, plane, offt, ld, v);
+          }
+        } else {                                              // a5: Z_next = Z + Z Q, W = Z_next^T
+          float z32[32];
+          load_f32_row32(p.f32_in + off, z32);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] += z32[j];
+          store_f32_row32(p.f32_out + off, v);
+          if (KIND == KIND_TF32) {
+            float* wt = static_cast<float*>(p.h_out_t);
+#pragma unroll
+            for (int j = 0; j < 32; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
+          } else {
+            store_pair_row32<false>(p.h_out, plane, off, v);               // Zb next (bf16 pair)
+            store_pair_col32<true>(p.h_out_t, plane, offt, ld, v);         // W16 (fp16 pair, lo scaled)
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(tempty_bar(buf));                            // 128 arrivals free the accumulator
+      if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
+      if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
+      else accphase ^= 1u;
+    }
+  }
+
+  // ------------------------------------------------------- teardown (+ step a3 for a2)
+  if (EPI == EPI_A2) {
+    const double s = warp_sum(warp >= 2 ? cta_sumsq : 0.0);
+    if (lane == 0) red[warp] = s;
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
+  }
+  if (EPI == EPI_A2) {
+    if (threadIdx.x == 0) p.stop.partials[blockIdx.x] = red[2] + red[3] + red[4] + red[5];
+    if (arrive_is_last(&p.st->arrive[0], gridDim.x, &last_flag)) stop_test_last_cta(p.stop, red);
+  }
+}
+
+// ------------------------------------------------------------------ host side
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct UmmaPlan {
+  Layout L;
+  char* ws = nullptr;
+  int grid = 0;
+  int mode = 0;
+  // tensor maps of every operand buffer (box 128 B x 128 rows, 128B swizzle)
+  CUtensorMap mS, mW, mT, mR, mQ, mZ[2];
+};
+
+inline cudaError_t make_map(PFN_encodeTiled enc, CUtensorMap* m, void* base, CUtensorMapDataType dt, size_t elt,
+                            uint64_t rows, uint64_t cols) {
+  cuuint64_t gdim[2] = {cols, rows};
+  cuuint64_t gstr[1] = {cols * elt};
+  cuuint32_t box[2] = {(cuuint32_t)(UM_ROWB / elt), 128u};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult r = enc(m, dt, 2, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <int KIND, int EPI>
+inline cudaError_t set_smem_attr() {
+  return cudaFuncSetAttribute(umma_gemm_kernel<KIND, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
+}
+
+inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int sm_count) {
+  pl->L = L; pl->ws = ws; pl->grid = sm_count; pl->mode = L.mode;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess) return e;
+  if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+  PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
+  const uint64_t np = (uint64_t)L.np;
+  if (L.mode == ZFAC_MODE_SPLIT16) {
+    const CUtensorMapDataType H = CU_TENSOR_MAP_DATA_TYPE_FLOAT16, B = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+    if ((e = make_map(enc, &pl->mS, ws + L.off_S, H, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mW, ws + L.off_W, H, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mT, ws + L.off_T, H, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mR, ws + L.off_Rb, B, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mQ, ws + L.off_Qb, B, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Zb[0], B, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], B, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_F16X2, EPI_A1>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_F16X2, EPI_A2>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_BF16X2, EPI_A4>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_BF16X2, EPI_A5>()) != cudaSuccess) return e;
+  } else {
+    const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    if ((e = make_map(enc, &pl->mS, ws + L.off_S, F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mW, ws + L.off_W, F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mT, ws + L.off_T, F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mR, ws + L.off_R, F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mQ, ws + L.off_Q, F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Z[0], F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Z[1], F, 4, np, np)) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_TF32, EPI_A1>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_TF32, EPI_A2>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_TF32, EPI_A4>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_TF32, EPI_A5>()) != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, double* d_err, cudaStream_t s, int* launches, Prof* prof) {
+  const Layout& L = pl.L;
+  char* ws = pl.ws;
+  const int T = (int)(L.np / 256);
+  const int full_tiles = 2 * T * T, sym_tiles = T * (T + 1);
+  const int grid_full = full_tiles < pl.grid ? full_tiles : pl.grid;
+  const int grid_sym = sym_tiles < pl.grid ? sym_tiles : pl.grid;
+  UmmaParams p{};
+  p.np = (int)L.np; p.macro_tiles = T;
+  p.st = reinterpret_cast<State*>(ws + L.off_state);
+  p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
+  p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+  float* R32 = reinterpret_cast<float*>(ws + L.off_R);
+  const bool split = (L.mode == ZFAC_MODE_SPLIT16);
+  int nl = 0;
+  for (int n = 0; n <= max_iter; ++n) {
+    // a1: T = W S^T
+    prof->mark(s, EPI_A1 + 16 * n);
+    p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
+    if (split) { p.f32_out = nullptr; p.h_out = ws + L.off_T;
+      umma_gemm_kernel<KIND_F16X2, EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    } else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr;
+      umma_gemm_kernel<KIND_TF32, EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p); }
+    // a2: R = I - W T^T
+    prof->mark(s, EPI_A2 + 16 * n);
+    p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n;
+    if (split) { p.h_out = ws + L.off_Rb;
+      umma_gemm_kernel<KIND_F16X2, EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    } else { p.h_out = nullptr;
+      umma_gemm_kernel<KIND_TF32, EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p); }
+    nl += 2;
+    if (n == max_iter) break;
+    // a4: Q = 1/2 R + 3/8 R R^T
+    prof->mark(s, EPI_A4 + 16 * n);
+    p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
+    if (split) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb;
+      umma_gemm_kernel<KIND_BF16X2, EPI_A4><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    } else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr;
+      umma_gemm_kernel<KIND_TF32, EPI_A4><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p); }
+    // a5: Z_next = Z + Z Q^T ; W = Z_next^T
+    prof->mark(s, EPI_A5 + 16 * n);
+    p.mapA = pl.mZ[n & 1]; p.mapB = pl.mQ;
+    if (split) {
+      float* Z32 = reinterpret_cast<float*>(ws + L.off_Z[0]);       // FP32 master copy, updated in place
+      p.f32_in = Z32; p.f32_out = Z32; p.h_out = ws + L.off_Zb[(n + 1) & 1]; p.h_out_t = ws + L.off_W;
+      umma_gemm_kernel<KIND_BF16X2, EPI_A5><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    } else {
+      p.f32_in = reinterpret_cast<float*>(ws + L.off_Z[n & 1]);
+      p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(n + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
+      umma_gemm_kernel<KIND_TF32, EPI_A5><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    }
+    nl += 2;
+  }
+  prof->mark(s, 0);
+  *launches = nl;
+  return cudaGetLastError();
+}
+
+}  // namespace zfac
