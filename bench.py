@@ -1,0 +1,409 @@
+#!/usr/bin/env python
+"""bench.py -- Z-refinement throughput on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path: one `zfac_refine` call (copy-in, residual and
+update GEMM kernels until the paper's stopping test fires, copy-out) on the N = 8192 warm-start
+workload (BASELINE.json configs[3]).  `value` is FP32-equivalent TFLOP/s with the
+paper's "four multiplications per iteration" convention, (4 + 8 k) N^3 flop for k updates
+(PAPER.md:238), inputs resident in HBM; `e2e` is the same through `zfac_refine_host` with
+pinned HOST buffers (H2D of S and Z0, D2H of Z inside the timed region).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1 (torchrun): N independent replicas, no data-path collective ("replicas only").
+`--impl reference` times the CPU oracle as it stands on a bounded sample of the workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Z-refinement TFLOP/s (FP32-equivalent, (4+8k)N^3 flop) at N=8192, split-FP16, time-to-converged"
+UNIT = "TFLOP/s"
+
+
+def flops_fp32_equiv(n: int, iters: int) -> float:
+    """(k+1) residual evaluations (2 GEMMs) + k updates (2 GEMMs), 2 N^3 each."""
+    return (4.0 + 8.0 * iters) * float(n) ** 3
+
+
+# ----------------------------------------------------------------------------- helpers
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return None
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[5 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return None
+        busy = [s for s, p in zip(sm, pw) if p > 0.5 * max(pw)] or sm
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"bf16_burst": d.get("bf16_tflops"), "bf16_sustained": d.get("bf16_tflops_sustained"),
+                "hbm_gbs": d.get("hbm_gbs"), "source": "measured (MEASURED_PEAKS.json)"}
+    return {"bf16_burst": 1590.0, "bf16_sustained": 1400.0, "hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def torch_gemm_peak(dtype, n, dev, tf32=False, reps=5):
+    """cuBLAS reference rate for a dtype, measured the way MEASURED_PEAKS.json was (burst, best of reps)."""
+    import torch
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = tf32
+    try:
+        a = torch.randn(n, n, device=dev, dtype=dtype)
+        b = torch.randn(n, n, device=dev, dtype=dtype)
+        c = a @ b
+        torch.cuda.synchronize(dev)
+        best = float("inf")
+        for _ in range(reps):
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(); c = a @ b; e1.record(); torch.cuda.synchronize(dev)
+            best = min(best, e0.elapsed_time(e1))
+        del a, b, c
+        return 2.0 * n ** 3 / (best * 1e-3) / 1e12
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+
+
+def build_workload(name, n, dev, rank=0):
+    from paper_2404_19163_b200 import workloads as W
+    if name == "config4":
+        return W.config4(n=n, seed_q=rank, seed_e=1 + rank, device=dev)
+    if name == "config5":
+        return W.config5(n, device=dev, fp32_stored=True)
+    if name == "config2":
+        return W.config2(n)
+    raise ValueError(name)
+
+
+# ----------------------------------------------------------------------------- reference arm (oracle on host cores)
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import torch
+    from oracle import zfac_oracle as O
+    dev = "cuda:0" if torch.cuda.is_available() else None
+    w = build_workload(args.workload, args.n, dev)
+    # bounded sample: the first residual evaluation + Err[0] of the workload (Alg. 2, 4 N_s^3 flop)
+    # on the leading N_s x N_s block, N_s chosen so that one step is ~10-20 s of CPU work
+    a = np.random.default_rng(0).standard_normal((1024, 1024))
+    t0 = time.perf_counter(); a @ a; t1 = time.perf_counter()
+    gfs = 2 * 1024 ** 3 / (t1 - t0) / 1e9
+    ns = args.n
+    while 4.0 * ns ** 3 / (gfs * 1e9) > 20.0 and ns > 1024:
+        ns //= 2
+    S = np.ascontiguousarray(w.S[:ns, :ns]); Z0 = np.ascontiguousarray(w.Z0[:ns, :ns])
+    for _ in range(args.warmup):
+        O.err_fro(O.residual(S, Z0))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e0 = O.err_fro(O.residual(S, Z0))
+    dt = (time.perf_counter() - t0) / args.steps
+    val = 4.0 * ns ** 3 / dt / 1e12
+    cores = os.cpu_count()
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([i.get("num_threads", 1) for i in threadpool_info()] or [cores])
+    except Exception:
+        pass
+    sample = f"first residual evaluation R0 = I - Z0^T(S Z0) and Err[0] on the leading {ns}x{ns} block (4*{ns}^3 flop per step)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}_n{args.n}", "mode": "oracle_fp64", "N": args.n},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "Err0": e0}
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------- our arm
+def time_refine(zf, S, Z0, Zout, max_iter, stop, steps, warmup, dev, profile=False, sampler=None, sync_fn=None):
+    import torch
+    from paper_2404_19163_b200 import binding as zb
+    if sampler:
+        sampler.start()          # covers warm-up + timed region; only samples under load are kept
+    for _ in range(warmup):
+        zf.refine(S, Z0, max_iter=max_iter, stop=stop, out=Zout, sync=False)
+    torch.cuda.synchronize(dev)
+    if profile:
+        zf.set_profile(True)
+    if sync_fn:
+        sync_fn()
+    torch.cuda.synchronize(dev)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        _, d_it, d_err, d_fl = zf.refine(S, Z0, max_iter=max_iter, stop=stop, out=Zout, sync=False)
+    e1.record()
+    torch.cuda.synchronize(dev)
+    if sync_fn:
+        sync_fn()
+    clocks = sampler.stop() if sampler else None
+    ms = e0.elapsed_time(e1) / steps
+    iters = int(d_it.item()); flags = int(d_fl.item())
+    err = d_err[: iters + 1].cpu().numpy()
+    prof = zf.get_profile() if profile else []
+    if profile:
+        zf.set_profile(False)
+    return ms, iters, flags, err, prof, clocks, zf.last_launch_count
+
+
+def kernel_stats(prof, iters):
+    """Average duration (ms) per step id over the kernels that did work (iteration <= iters)."""
+    out = {}
+    for sid, it, ms in prof:
+        if sid == 0:
+            continue
+        if it > iters or (sid in (4, 5) and it >= iters):
+            continue            # early-exit launches after the stop decision
+        out.setdefault(sid, []).append(ms)
+    return {sid: (float(np.mean(v)), len(v)) for sid, v in out.items()}
+
+
+def run_ours(args):
+    import torch
+    from paper_2404_19163_b200 import binding as zb, replicas
+    from paper_2404_19163_b200 import build as zbuild
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (sm_100a); there is no CPU path for --impl ours")
+    rank, local_rank, world = replicas.init("nccl")
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    if not os.path.exists(zb.LIB_PATH):
+        zbuild.build()
+    n = args.n
+    peaks = measured_peaks()
+    w = build_workload(args.workload, n, dev, rank)
+    stop = zb.ZFAC_STOP_PAPER if args.stop == "paper" else zb.ZFAC_STOP_FIXED
+    results = {}
+    primary = None
+
+    def run_mode(mode, with_e2e, with_clock):
+        dt = torch.float64 if mode == "f64" else torch.float32
+        S = torch.from_numpy(w.S).to(dev, dt); Z0 = torch.from_numpy(w.Z0).to(dev, dt)
+        Zout = torch.empty_like(Z0)
+        with zb.Zfac(n, mode, dev) as zf:
+            sampler = ClockSampler(local_rank) if with_clock else None
+            ms, iters, flags, err, prof, clocks, launches = time_refine(
+                zf, S, Z0, Zout, args.max_iter, stop, args.steps, args.warmup, dev, profile=True, sampler=sampler,
+                sync_fn=replicas.barrier)
+            ks = kernel_stats(prof, iters)
+            res = {"ms_per_step": ms, "iters": iters, "flags": flags, "err": [float(x) for x in err],
+                   "launches": launches, "kernel_ms": {f"a{sid}": v[0] for sid, v in sorted(ks.items())},
+                   "tflops_fp32_equiv": flops_fp32_equiv(n, iters) / (ms * 1e-3) / 1e12,
+                   "iters_per_s": (iters / (ms * 1e-3)) if iters else 0.0, "clocks": clocks}
+            if with_e2e:
+                hS = torch.from_numpy(w.S).to(dt).pin_memory(); hZ0 = torch.from_numpy(w.Z0).to(dt).pin_memory()
+                hZ = torch.empty_like(hZ0).pin_memory()
+                for _ in range(max(1, args.warmup // 2)):
+                    zf.refine_host(hS, hZ0, hZ, max_iter=args.max_iter, stop=stop)
+                replicas.barrier(); torch.cuda.synchronize(dev)
+                t0 = time.perf_counter()
+                for _ in range(args.steps):
+                    _, it2, err2, fl2 = zf.refine_host(hS, hZ0, hZ, max_iter=args.max_iter, stop=stop)
+                torch.cuda.synchronize(dev)
+                e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+                res["e2e_ms"] = e2e_ms
+                res["e2e_iters"] = it2
+                res["h2d"] = 2 * n * n * hS.element_size()
+                res["d2h"] = n * n * hS.element_size() + 8 * (it2 + 1) + 8
+                del hS, hZ0, hZ
+            res["Z"] = Zout
+        return res
+
+    primary = run_mode(args.mode, with_e2e=True, with_clock=True)
+    iters = primary["iters"]
+
+    # final invariant ||Z^T S Z - I||_F / sqrt(N) of each mode's Z, evaluated by the library's own FP64 kernels
+    def invariant(Zt):
+        S64 = torch.from_numpy(w.S).to(dev, torch.float64)
+        with zb.Zfac(n, "f64", dev) as zf:
+            _, _, e, _ = zf.refine(S64, Zt.to(torch.float64), max_iter=0, stop=zb.ZFAC_STOP_FIXED)
+        return float(e[0]) / math.sqrt(n)
+
+    extra = {}
+    if rank == 0 and not args.quick:
+        primary["final_residual_per_sqrt_n"] = invariant(primary.pop("Z"))
+        for mode in [m for m in ("f64", "tf32", "split16") if m != args.mode]:
+            r = run_mode(mode, with_e2e=False, with_clock=False)
+            r["final_residual_per_sqrt_n"] = invariant(r.pop("Z"))
+            extra[mode] = r
+        # cuBLAS reference rates per precision, measured in this run the way MEASURED_PEAKS.json was
+        extra["cublas_tflops"] = {"bf16": torch_gemm_peak(torch.bfloat16, 8192, dev),
+                                  "tf32": torch_gemm_peak(torch.float32, 8192, dev, tf32=True),
+                                  "f64": torch_gemm_peak(torch.float64, 8192, dev, reps=3)}
+        # reference point: S^-1/2 through cuSOLVER syevd (torch.linalg.eigh) + scaling + one GEMM
+        try:
+            for dtn, dt in (("f32", torch.float32), ("f64", torch.float64)):
+                Sd = torch.from_numpy(w.S).to(dev, dt)
+                torch.cuda.synchronize(dev); t0 = time.perf_counter()
+                lam, V = torch.linalg.eigh(Sd)
+                Zr = (V / lam.clamp_min(1e-30).sqrt().unsqueeze(0)) @ V.T
+                torch.cuda.synchronize(dev)
+                extra.setdefault("syevd_inv_sqrt_ms", {})[dtn] = (time.perf_counter() - t0) * 1e3
+                del Sd, lam, V, Zr
+        except Exception as ex:  # reference point only
+            extra["syevd_inv_sqrt_ms"] = {"error": str(ex)[:100]}
+    else:
+        primary.pop("Z", None)
+
+    # ---- aggregate over replicas: max time, sum of work
+    units = flops_fp32_equiv(n, iters)
+    t_ms, total_units = replicas.aggregate(primary["ms_per_step"], units, dev)
+    e2e_ms, _ = replicas.aggregate(primary["e2e_ms"], units, dev)
+    value = total_units / (t_ms * 1e-3) / 1e12
+    e2e_value = total_units / (e2e_ms * 1e-3) / 1e12
+
+    # ---- roofline of the dominant kernel: a1 (full split GEMM, 3 MMA passes; a5 costs the same)
+    kms = primary["kernel_ms"]
+    passes = {"split16": 3, "tf32": 1, "f64": 1}[args.mode]
+    roof = None
+    if "a1" in kms:
+        ach = passes * 2.0 * n ** 3 / (kms["a1"] * 1e-3) / 1e12
+        if args.mode == "split16":
+            peak, pk_name = peaks["bf16_sustained"], "bf16_tflops_sustained"
+        elif args.mode == "tf32":
+            peak, pk_name = peaks["bf16_sustained"] * 0.5, "bf16_tflops_sustained x 0.5 (nominal tf32:bf16 ratio)"
+        else:
+            peak, pk_name = extra.get("cublas_tflops", {}).get("f64", 37.0), "cuBLAS dgemm 8192^3 measured in this run"
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            try:
+                traffic = json.load(open(tp)).get(f"{args.mode}_a1_n{n}")
+            except Exception:
+                traffic = None
+        roof = {"bound": "tensor", "kernel": f"umma_gemm_kernel a1 ({args.mode})" if args.mode != "f64" else "f64_gemm_kernel a1",
+                "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": traffic,
+                "peak_source": f"{peaks['source']}: {pk_name}", "frac_of_burst": ach / peaks["bf16_burst"] if args.mode == "split16" else None,
+                "executed_flops_per_launch": passes * 2.0 * n ** 3, "launch_ms": kms["a1"],
+                "all_kernels_ms": kms}
+
+    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N = 1 only
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import zfac_oracle as O
+        ns = min(n, args.cpu_sample_n)
+        S = np.ascontiguousarray(w.S[:ns, :ns]); Z0 = np.ascontiguousarray(w.Z0[:ns, :ns])
+        t0 = time.perf_counter()
+        O.refine(S, Z0, 1, O.STOP_FIXED)          # R0, Err[0], one update, R1, Err[1]: (4 + 8) N^3 flop
+        dt = time.perf_counter() - t0
+        cores = os.cpu_count()
+        try:
+            from threadpoolctl import threadpool_info
+            cores = max([i.get("num_threads", 1) for i in threadpool_info()] or [cores])
+        except Exception:
+            pass
+        cpu = {"value": flops_fp32_equiv(ns, 1) / dt / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"oracle Alg. 2 with one update (R0, Err[0], Z1, R1, Err[1]) on the leading {ns}x{ns} block "
+                         f"of the workload (12*{ns}^3 flop, {dt:.1f} s)"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": {"split16": "f16/bf16 pairs, f32 accumulate", "tf32": "tf32, f32 accumulate", "f64": "f64"}[args.mode],
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "N": n, "stop": args.stop,
+                       "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
+                       "l2": "operands (2.4 GB) exceed L2 (126 MB); no flush needed"},
+            "iters": iters, "iters_per_s": primary["iters_per_s"] * world, "time_to_converged_ms": t_ms,
+            "err_history": primary["err"], "flags": primary["flags"],
+            "final_residual_per_sqrt_n": primary.get("final_residual_per_sqrt_n"),
+            "clocks": primary["clocks"],
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": primary["h2d"],
+                    "d2h_bytes_per_step": primary["d2h"]},
+            "gpu_launches": primary["launches"] * args.steps,
+            "roofline": roof, "cpu_baseline": cpu, "modes": extra,
+        }
+        print(json.dumps(line))
+    replicas.barrier()
+    replicas.shutdown()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=8192)
+    ap.add_argument("--mode", default="split16", choices=["split16", "tf32", "f64"])
+    ap.add_argument("--workload", default="config4", choices=["config4", "config5", "config2"])
+    ap.add_argument("--stop", default="paper", choices=["paper", "fixed"])
+    ap.add_argument("--max-iter", type=int, default=20)
+    ap.add_argument("--cpu-sample-n", type=int, default=8192)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--quick", action="store_true", help="primary mode only (no other modes / reference points)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
