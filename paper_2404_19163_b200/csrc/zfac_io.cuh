@@ -131,8 +131,8 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
       __half hi, lo; split_f16((float)s, hi, lo);
       static_cast<__half*>(a.oS)[o] = hi; static_cast<__half*>(a.oS)[np2 + o] = lo;
       static_cast<float*>(a.oZ)[o] = (float)z;
-      __nv_bfloat16 bh, bl; split_bf16((float)z, bh, bl);
-      static_cast<__nv_bfloat16*>(a.oZb)[o] = bh; static_cast<__nv_bfloat16*>(a.oZb)[np2 + o] = bl;
+      __half zh, zl; split_f16((float)z, zh, zl);
+      static_cast<__half*>(a.oZb)[o] = zh; static_cast<__half*>(a.oZb)[np2 + o] = zl;
     } else if (MODE == ZFAC_MODE_TF32) {
       static_cast<float*>(a.oS)[o] = round_tf32((float)s);
       static_cast<float*>(a.oZ)[o] = (float)z;

@@ -22,6 +22,8 @@
 //   KIND_TF32   (TF32 mode): FP32 operands read as TF32, one pass, two accumulator buffers.
 #pragma once
 #include <cuda.h>
+#include <stdio.h>
+#include <stdlib.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include "zfac_common.cuh"
@@ -33,7 +35,6 @@ namespace zfac {
 enum { KIND_F16X2 = 0, KIND_BF16X2 = 1, KIND_TF32 = 2 };
 
 constexpr int UM_BM = 128, UM_BN = 256;
-constexpr int UM_THREADS = 192;
 constexpr int UM_ROWB = 128;                     // bytes per operand row per k-block (= swizzle span)
 constexpr int UM_A_BYTES = UM_BM * UM_ROWB;      // 16 KB
 constexpr int UM_B_BYTES = UM_BN * UM_ROWB;      // 32 KB
@@ -44,12 +45,15 @@ constexpr int UM_TMEM_COLS = 512;
 template <int KIND> struct KindTraits;
 template <> struct KindTraits<KIND_F16X2> {
   static constexpr int ARRAYS = 2, STAGES = 2, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 1, FMT = 0;
+  static constexpr int EPI_WARPS = 8, SUB = 16, THREADS = 64 + 32 * EPI_WARPS, MAXREG = 192;
 };
 template <> struct KindTraits<KIND_BF16X2> {
   static constexpr int ARRAYS = 2, STAGES = 2, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 2, FMT = 1;
+  static constexpr int EPI_WARPS = 4, SUB = 32, THREADS = 64 + 32 * EPI_WARPS, MAXREG = 255;
 };
 template <> struct KindTraits<KIND_TF32> {
   static constexpr int ARRAYS = 1, STAGES = 4, KSTEP_ELEMS = 8, BK_ELEMS = 32, ACC_BUFS = 2, FMT = 2;
+  static constexpr int EPI_WARPS = 4, SUB = 32, THREADS = 64 + 32 * EPI_WARPS, MAXREG = 255;
 };
 
 struct UmmaParams {
@@ -57,6 +61,7 @@ struct UmmaParams {
   CUtensorMap mapB;     // B-operand buffer, same box
   int np;               // padded dimension (= K)
   int macro_tiles;      // Np / 256
+  int chunk_kb;         // KIND_F16X2: k-blocks (of 64) per promoted accumulation chunk
   State* st;
   StopArgs stop;        // a2 only (partials = one per CTA)
   // epilogue pointers (which are used depends on EPI / KIND; see the epilogue)
@@ -113,7 +118,7 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
   }
 }
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
       "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
@@ -121,6 +126,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
         "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
       : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
@@ -141,12 +153,12 @@ __device__ __forceinline__ uint32_t pack_b2(__nv_bfloat16 a, __nv_bfloat16 b) {
   return (uint32_t)__bfloat16_as_ushort(a) | ((uint32_t)__bfloat16_as_ushort(b) << 16);
 }
 
-// Write 32 consecutive values of one row as a 16-bit pair (hi -> base, lo -> base + plane).
-template <bool F16>
-__device__ __forceinline__ void store_pair_row32(void* base, size_t plane, size_t off, const float (&v)[32]) {
-  uint32_t hi[16], lo[16];
+// Write N consecutive values of one row as a 16-bit pair (hi -> base, lo -> base + plane).
+template <bool F16, int N>
+__device__ __forceinline__ void store_pair_row(void* base, size_t plane, size_t off, const float (&v)[N]) {
+  uint32_t hi[N / 2], lo[N / 2];
 #pragma unroll
-  for (int j = 0; j < 16; ++j) {
+  for (int j = 0; j < N / 2; ++j) {
     if (F16) {
       __half h0, l0, h1, l1;
       split_f16(v[2 * j], h0, l0); split_f16(v[2 * j + 1], h1, l1);
@@ -161,17 +173,17 @@ __device__ __forceinline__ void store_pair_row32(void* base, size_t plane, size_
   uint4* ph = reinterpret_cast<uint4*>(b + off);
   uint4* pl = reinterpret_cast<uint4*>(b + plane + off);
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
+  for (int j = 0; j < N / 8; ++j) {
     ph[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
     pl[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
   }
 }
 // Transposed: value j of this lane goes to row (n + j), column m (lanes hold consecutive m).
-template <bool F16>
-__device__ __forceinline__ void store_pair_col32(void* base, size_t plane, size_t off_n0_m, size_t ld, const float (&v)[32]) {
+template <bool F16, int N>
+__device__ __forceinline__ void store_pair_col(void* base, size_t plane, size_t off_n0_m, size_t ld, const float (&v)[N]) {
   uint16_t* b = static_cast<uint16_t*>(base);
 #pragma unroll
-  for (int j = 0; j < 32; ++j) {
+  for (int j = 0; j < N; ++j) {
     uint16_t h, l;
     if (F16) { __half hh, ll; split_f16(v[j], hh, ll); h = __half_as_ushort(hh); l = __half_as_ushort(ll); }
     else { __nv_bfloat16 hh, ll; split_bf16(v[j], hh, ll); h = __bfloat16_as_ushort(hh); l = __bfloat16_as_ushort(ll); }
@@ -179,54 +191,122 @@ __device__ __forceinline__ void store_pair_col32(void* base, size_t plane, size_
     b[plane + off_n0_m + (size_t)j * ld] = l;
   }
 }
-__device__ __forceinline__ void store_f32_row32(float* p, const float (&v)[32]) {
+template <int N>
+__device__ __forceinline__ void store_f32_row(float* p, const float (&v)[N]) {
   float4* q = reinterpret_cast<float4*>(p);
 #pragma unroll
-  for (int j = 0; j < 8; ++j) q[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+  for (int j = 0; j < N / 4; ++j) q[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
 }
-__device__ __forceinline__ void load_f32_row32(const float* p, float (&v)[32]) {
+template <int N>
+__device__ __forceinline__ void load_f32_row(const float* p, float (&v)[N]) {
   const float4* q = reinterpret_cast<const float4*>(p);
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {
+  for (int j = 0; j < N / 4; ++j) {
     const float4 t = q[j];
     v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
   }
 }
 
+// Fused epilogue for SUB consecutive columns n..n+SUB-1 of row m (v = accumulator values).
+template <int KIND, int EPI, int SUB>
+__device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SUB], int m, int n, bool offdiag,
+                                              double& tile_sumsq) {
+  const size_t ld = (size_t)p.np, plane = ld * ld;
+  const size_t off = (size_t)m * ld + n;               // (m, n)
+  const size_t offt = (size_t)n * ld + m;              // (n, m)
+  if (EPI == EPI_A1) {                                  // T = (S Z)^T
+    if (KIND == KIND_TF32) {
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
+      store_f32_row<SUB>(p.f32_out + off, v);
+    } else store_pair_row<true, SUB>(p.h_out, plane, off, v);
+  } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
+#pragma unroll
+    for (int j = 0; j < SUB; ++j) {
+      v[j] = ((m == n + j) ? 1.0f : 0.0f) - v[j];
+      tile_sumsq += (double)v[j] * (double)v[j];
+    }
+    store_f32_row<SUB>(p.f32_out + off, v);
+    if (KIND != KIND_TF32) store_pair_row<true, SUB>(p.h_out, plane, off, v);
+    if (offdiag) {
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
+      if (KIND != KIND_TF32) store_pair_col<true, SUB>(p.h_out, plane, offt, ld, v);
+    }
+  } else if (EPI == EPI_A4) {                           // Q = 1/2 R + 3/8 R R, mirror
+    float r32[SUB];
+    load_f32_row<SUB>(p.f32_in + off, r32);
+#pragma unroll
+    for (int j = 0; j < SUB; ++j) v[j] = 0.5f * r32[j] + 0.375f * v[j];
+    if (KIND == KIND_TF32) {
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
+      store_f32_row<SUB>(p.f32_out + off, v);
+      if (offdiag) {
+#pragma unroll
+        for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
+      }
+    } else {
+      store_pair_row<true, SUB>(p.h_out, plane, off, v);
+      if (offdiag) store_pair_col<true, SUB>(p.h_out, plane, offt, ld, v);
+    }
+  } else {                                              // a5: Z_next = Z + Z Q, W = Z_next^T
+    float z32[SUB];
+    load_f32_row<SUB>(p.f32_in + off, z32);
+#pragma unroll
+    for (int j = 0; j < SUB; ++j) v[j] += z32[j];
+    store_f32_row<SUB>(p.f32_out + off, v);
+    if (KIND == KIND_TF32) {
+      float* wt = static_cast<float*>(p.h_out_t);
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
+    } else {
+      store_pair_row<true, SUB>(p.h_out, plane, off, v);                // Z16 next (fp16 pair, lo scaled)
+      store_pair_col<true, SUB>(p.h_out_t, plane, offt, ld, v);         // W16 = Z16^T
+    }
+  }
+}
+
 // ------------------------------------------------------------------ the kernel
-// MODE_SPLIT: true for the SPLIT16 mode kernels (16-bit pair outputs), false for TF32 mode.
 template <int KIND, int EPI>
-__global__ void __launch_bounds__(UM_THREADS, 1) umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
+__global__ void __launch_bounds__(KindTraits<KIND>::THREADS, 1) umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   if (*((volatile int*)&p.st->done)) return;       // stop decided earlier in this call
 
   using KT = KindTraits<KIND>;
   constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4);
+  constexpr bool PROMOTE = (KIND == KIND_F16X2);
   constexpr int STAGE_BYTES = KT::ARRAYS * (UM_A_BYTES + UM_B_BYTES);
   static_assert(KT::STAGES * STAGE_BYTES <= UM_SMEM_OPERANDS, "smem");
   constexpr int KSTEPS = KT::BK_ELEMS / KT::KSTEP_ELEMS;   // 4
   constexpr uint32_t IDESC = make_idesc(KT::FMT);
+  constexpr int EPI_THREADS = 32 * KT::EPI_WARPS;
+  constexpr int COLS = UM_BN / (KT::EPI_WARPS / 4);        // columns per epilogue thread
+  constexpr int SUB = KT::SUB;
 
   extern __shared__ unsigned char smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + UM_SMEM_OPERANDS;
-  // barrier slots (8 B each): full[0..3], empty[4..7], tmem_full[8..9], tmem_empty[10..11]; tmem ptr at +96
+  // barrier slots (8 B each): full[0..3], empty[4..7], tfull[8..9], tempty[10..11], hh_full 12, hh_empty 13
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 32u + 8u * s; };
   auto tfull_bar = [&](int b) { return bar_base + 64u + 8u * b; };
   auto tempty_bar = [&](int b) { return bar_base + 80u + 8u * b; };
-  const uint32_t tmem_slot = bar_base + 96u;
-  __shared__ double red[8];
+  const uint32_t hh_full_bar = bar_base + 96u, hh_empty_bar = bar_base + 104u;
+  const uint32_t tmem_slot = bar_base + 112u;
+  __shared__ double red[32];
   __shared__ int last_flag;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int np = p.np;
   const int KB = np / KT::BK_ELEMS;
+  const int CH = p.chunk_kb > 0 ? p.chunk_kb : KB;         // k-blocks per promoted chunk (KIND_F16X2)
   const int T = p.macro_tiles;
   const int num_tiles = SYM ? T * (T + 1) : 2 * T * T;     // CTA tiles (two 128-row halves per macro tile)
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < KT::ACC_BUFS; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 128); }
+    for (int b = 0; b < KT::ACC_BUFS; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), EPI_THREADS); }
+    mbar_init(hh_full_bar, 1); mbar_init(hh_empty_bar, EPI_THREADS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
@@ -280,10 +360,11 @@ __global__ void __launch_bounds__(UM_THREADS, 1) umma_gemm_kernel(const __grid_c
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       int buf = 0; uint32_t accphase = 0;
+      uint32_t chunks = 0;                                     // promoted chunks committed so far (all tiles)
       for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
         mbar_wait(tempty_bar(buf), accphase ^ 1u);
         tc_fence_after();
-        const uint32_t d0 = tmem_base + (KT::ACC_BUFS == 2 ? buf * 256 : 0);   // D (or D_hh)
+        const uint32_t d0 = tmem_base + (KT::ACC_BUFS == 2 ? buf * 256 : 0);   // D (or D_hh chunk)
         const uint32_t d1 = tmem_base + 256;                                     // D_x (KIND_F16X2 only)
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(full_bar(stage), phase);
@@ -293,118 +374,108 @@ __global__ void __launch_bounds__(UM_THREADS, 1) umma_gemm_kernel(const __grid_c
           const uint64_t a_lo = make_sdesc(sa + UM_A_BYTES);
           const uint64_t b_hi = make_sdesc(sa + KT::ARRAYS * UM_A_BYTES);
           const uint64_t b_lo = make_sdesc(sa + KT::ARRAYS * UM_A_BYTES + UM_B_BYTES);
+          if (PROMOTE) {
+            // (h)(h) products first, into the chunk accumulator D_hh; the epilogue warps add every
+            // finished chunk to FP32 registers with round-to-nearest while the 2^11-scaled cross
+            // products of this k-block run on the tensor core.
+            const int kc = kb % CH;
+            if (kc == 0 && chunks > 0) { mbar_wait(hh_empty_bar, (chunks - 1u) & 1u); tc_fence_after(); }
 #pragma unroll
-          for (int k = 0; k < KSTEPS; ++k) {
-            const uint32_t acc = (kb | k) ? 1u : 0u;
-            const uint64_t ko = (uint64_t)(k * 2);            // 32 bytes per k-step, in 16-byte units
-            if (KIND == KIND_F16X2) {
-              tc_mma<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, acc);
+            for (int k = 0; k < KSTEPS; ++k)
+              tc_mma<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (kc | k) ? 1u : 0u);
+            if (kc == CH - 1 || kb == KB - 1) { tc_commit(hh_full_bar); ++chunks; }
+#pragma unroll
+            for (int k = 0; k < KSTEPS; ++k) {
+              const uint64_t ko = (uint64_t)(k * 2);
+              tc_mma<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, (kb | k) ? 1u : 0u);
               tc_mma<KIND>(d1, a_lo + ko, b_hi + ko, IDESC, 1u);
-              tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
-            } else if (KIND == KIND_BF16X2) {
-              tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
-              tc_mma<KIND>(d0, a_hi + ko, b_lo + ko, IDESC, 1u);
-              tc_mma<KIND>(d0, a_lo + ko, b_hi + ko, IDESC, 1u);
-            } else {
-              tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
+            }
+          } else {
+#pragma unroll
+            for (int k = 0; k < KSTEPS; ++k) {
+              const uint32_t acc = (kb | k) ? 1u : 0u;
+              const uint64_t ko = (uint64_t)(k * 2);            // 32 bytes per k-step, in 16-byte units
+              if (KIND == KIND_BF16X2) {
+                tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
+                tc_mma<KIND>(d0, a_hi + ko, b_lo + ko, IDESC, 1u);
+                tc_mma<KIND>(d0, a_lo + ko, b_hi + ko, IDESC, 1u);
+              } else {
+                tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
+              }
             }
           }
           tc_commit(empty_bar(stage));                         // frees the smem stage when the MMAs retire
           if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
         }
-        tc_commit(tfull_bar(buf));                             // accumulator complete
+        tc_commit(tfull_bar(buf));                             // accumulator(s) complete
         if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
         else accphase ^= 1u;
       }
     }
   } else {
-    // ===================================================== epilogue warps (2..5)
+    // ===================================================== epilogue warps (2 .. 2+EPI_WARPS-1)
     const int q = warp & 3;                                    // TMEM lane quarter this warp may read
+    const int g = (warp - 2) >> 2;                             // column group of this warp
     const int row = q * 32 + lane;
-    const size_t ld = (size_t)np, plane = ld * ld;
     int buf = 0; uint32_t accphase = 0;
+    uint32_t chunks = 0;
+    const int nch = (KB + CH - 1) / CH;
     for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
       int m0, n0; bool offdiag; decode(t, m0, n0, offdiag);
       const int m = m0 + row;
-      mbar_wait(tfull_bar(buf), accphase);
-      tc_fence_after();
-      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (KT::ACC_BUFS == 2 ? buf * 256 : 0);
+      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (KT::ACC_BUFS == 2 ? buf * 256 : 0) + g * COLS;
       double tile_sumsq = 0.0;
-#pragma unroll 1
-      for (int c = 0; c < UM_BN / 32; ++c) {
-        const int n = n0 + c * 32;
-        float v[32];
-        {
-          uint32_t r[32];
-          tmem_ld32(tbase + c * 32, r);
-          if (KIND == KIND_F16X2) {
-            uint32_t x[32];
-            tmem_ld32(tbase + 256 + c * 32, x);
+      if (PROMOTE) {
+        float sum[COLS];
+#pragma unroll
+        for (int j = 0; j < COLS; ++j) sum[j] = 0.0f;
+        for (int c = 0; c < nch; ++c) {
+          mbar_wait(hh_full_bar, chunks & 1u);
+          tc_fence_after();
+#pragma unroll
+          for (int i = 0; i < COLS / 32; ++i) {
+            uint32_t r[32];
+            tmem_ld(tbase + i * 32, r);
             tmem_ld_wait();
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) + __uint_as_float(x[j]) * LO_UNSCALE;
-          } else {
-            tmem_ld_wait();
-#pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+            for (int j = 0; j < 32; ++j) sum[i * 32 + j] += __uint_as_float(r[j]);
           }
+          tc_fence_before();
+          mbar_arrive(hh_empty_bar);
+          ++chunks;
         }
-        const size_t off = (size_t)m * ld + n;               // (m, n)
-        const size_t offt = (size_t)n * ld + m;              // (n, m)
-        if (EPI == EPI_A1) {                                  // T = (S Z)^T
-          if (KIND == KIND_TF32) {
+        mbar_wait(tfull_bar(0), accphase);
+        tc_fence_after();
 #pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = round_tf32(v[j]);
-            store_f32_row32(p.f32_out + off, v);
-          } else store_pair_row32<true>(p.h_out, plane, off, v);
-        } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
+        for (int cc = 0; cc < COLS / SUB; ++cc) {
+          float v[SUB];
+          {
+            uint32_t x[SUB];
+            tmem_ld(tbase + 256 + cc * SUB, x);
+            tmem_ld_wait();
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            v[j] = ((m == n + j) ? 1.0f : 0.0f) - v[j];
-            tile_sumsq += (double)v[j] * (double)v[j];
+            for (int j = 0; j < SUB; ++j) v[j] = sum[cc * SUB + j] + __uint_as_float(x[j]) * LO_UNSCALE;
           }
-          store_f32_row32(p.f32_out + off, v);
-          if (KIND != KIND_TF32) store_pair_row32<false>(p.h_out, plane, off, v);
-          if (offdiag) {
+          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + g * COLS + cc * SUB, offdiag, tile_sumsq);
+        }
+      } else {
+        mbar_wait(tfull_bar(buf), accphase);
+        tc_fence_after();
+#pragma unroll 1
+        for (int cc = 0; cc < COLS / SUB; ++cc) {
+          float v[SUB];
+          {
+            uint32_t r[SUB];
+            tmem_ld(tbase + cc * SUB, r);
+            tmem_ld_wait();
 #pragma unroll
-            for (int j = 0; j < 32; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
-            if (KIND != KIND_TF32) store_pair_col32<false>(p.h_out, plane, offt, ld, v);
+            for (int j = 0; j < SUB; ++j) v[j] = __uint_as_float(r[j]);
           }
-        } else if (EPI == EPI_A4) {                           // Q = 1/2 R + 3/8 R R, mirror
-          float r32[32];
-          load_f32_row32(p.f32_in + off, r32);
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] = 0.5f * r32[j] + 0.375f * v[j];
-          if (KIND == KIND_TF32) {
-#pragma unroll
-            for (int j = 0; j < 32; ++j) v[j] = round_tf32(v[j]);
-            store_f32_row32(p.f32_out + off, v);
-            if (offdiag) {
-#pragma unroll
-              for (int j = 0; j < 32; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
-            }
-          } else {
-            store_pair_row32<false>(p.h_out, plane, off, v);
-            if (offdiag) store_pair_col32<false>(p.h_out, plane, offt, ld, v);
-          }
-        } else {                                              // a5: Z_next = Z + Z Q, W = Z_next^T
-          float z32[32];
-          load_f32_row32(p.f32_in + off, z32);
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] += z32[j];
-          store_f32_row32(p.f32_out + off, v);
-          if (KIND == KIND_TF32) {
-            float* wt = static_cast<float*>(p.h_out_t);
-#pragma unroll
-            for (int j = 0; j < 32; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
-          } else {
-            store_pair_row32<false>(p.h_out, plane, off, v);               // Zb next (bf16 pair)
-            store_pair_col32<true>(p.h_out_t, plane, offt, ld, v);         // W16 (fp16 pair, lo scaled)
-          }
+          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + g * COLS + cc * SUB, offdiag, tile_sumsq);
         }
       }
       tc_fence_before();
-      mbar_arrive(tempty_bar(buf));                            // 128 arrivals free the accumulator
+      mbar_arrive(tempty_bar(buf));                            // EPI_THREADS arrivals free the accumulator
       if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
       if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
       else accphase ^= 1u;
@@ -419,11 +490,16 @@ __global__ void __launch_bounds__(UM_THREADS, 1) umma_gemm_kernel(const __grid_c
   tc_fence_before();
   __syncthreads();
   if (warp == 1) {
+    __syncwarp();
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
   }
   if (EPI == EPI_A2) {
-    if (threadIdx.x == 0) p.stop.partials[blockIdx.x] = red[2] + red[3] + red[4] + red[5];
+    if (threadIdx.x == 0) {
+      double tot = 0.0;
+      for (int w = 2; w < 2 + KT::EPI_WARPS; ++w) tot += red[w];
+      p.stop.partials[blockIdx.x] = tot;
+    }
     if (arrive_is_last(&p.st->arrive[0], gridDim.x, &last_flag)) stop_test_last_cta(p.stop, red);
   }
 }
@@ -438,6 +514,7 @@ struct UmmaPlan {
   char* ws = nullptr;
   int grid = 0;
   int mode = 0;
+  int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
   // tensor maps of every operand buffer (box 128 B x 128 rows, 128B swizzle)
   CUtensorMap mS, mW, mT, mR, mQ, mZ[2];
 };
@@ -455,11 +532,24 @@ inline cudaError_t make_map(PFN_encodeTiled enc, CUtensorMap* m, void* base, CUt
 
 template <int KIND, int EPI>
 inline cudaError_t set_smem_attr() {
-  return cudaFuncSetAttribute(umma_gemm_kernel<KIND, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(umma_gemm_kernel<KIND, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  int nb = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, umma_gemm_kernel<KIND, EPI>, KindTraits<KIND>::THREADS, UM_SMEM_BYTES);
+  if (e != cudaSuccess) return e;
+  if (nb < 1) {
+    cudaFuncAttributes fa;
+    cudaFuncGetAttributes(&fa, umma_gemm_kernel<KIND, EPI>);
+    fprintf(stderr, "zfac: kernel<%d,%d> does not fit an SM: regs=%d threads=%d static smem=%zu dyn smem=%d maxThreadsPerBlock=%d\n",
+            KIND, EPI, fa.numRegs, KindTraits<KIND>::THREADS, fa.sharedSizeBytes, UM_SMEM_BYTES, fa.maxThreadsPerBlock);
+    return cudaErrorLaunchOutOfResources;
+  }
+  return cudaSuccess;
 }
 
 inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int sm_count) {
   pl->L = L; pl->ws = ws; pl->grid = sm_count; pl->mode = L.mode;
+  if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knob
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -468,18 +558,18 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
   const uint64_t np = (uint64_t)L.np;
   if (L.mode == ZFAC_MODE_SPLIT16) {
-    const CUtensorMapDataType H = CU_TENSOR_MAP_DATA_TYPE_FLOAT16, B = CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+    const CUtensorMapDataType H = CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
     if ((e = make_map(enc, &pl->mS, ws + L.off_S, H, 2, 2 * np, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mW, ws + L.off_W, H, 2, 2 * np, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mT, ws + L.off_T, H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mR, ws + L.off_Rb, B, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mQ, ws + L.off_Qb, B, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Zb[0], B, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], B, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mR, ws + L.off_Rb, H, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mQ, ws + L.off_Qb, H, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Zb[0], H, 2, 2 * np, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], H, 2, 2 * np, np)) != cudaSuccess) return e;
     if ((e = set_smem_attr<KIND_F16X2, EPI_A1>()) != cudaSuccess) return e;
     if ((e = set_smem_attr<KIND_F16X2, EPI_A2>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_BF16X2, EPI_A4>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_BF16X2, EPI_A5>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_F16X2, EPI_A4>()) != cudaSuccess) return e;
+    if ((e = set_smem_attr<KIND_F16X2, EPI_A5>()) != cudaSuccess) return e;
   } else {
     const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     if ((e = make_map(enc, &pl->mS, ws + L.off_S, F, 4, np, np)) != cudaSuccess) return e;
@@ -505,7 +595,7 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
   const int grid_full = full_tiles < pl.grid ? full_tiles : pl.grid;
   const int grid_sym = sym_tiles < pl.grid ? sym_tiles : pl.grid;
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T;
+  p.np = (int)L.np; p.macro_tiles = T; p.chunk_kb = pl.chunk_kb;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
   p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
@@ -517,36 +607,36 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
     prof->mark(s, EPI_A1 + 16 * n);
     p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
     if (split) { p.f32_out = nullptr; p.h_out = ws + L.off_T;
-      umma_gemm_kernel<KIND_F16X2, EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      umma_gemm_kernel<KIND_F16X2, EPI_A1><<<grid_full, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
     } else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr;
-      umma_gemm_kernel<KIND_TF32, EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p); }
+      umma_gemm_kernel<KIND_TF32, EPI_A1><<<grid_full, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p); }
     // a2: R = I - W T^T
     prof->mark(s, EPI_A2 + 16 * n);
     p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n;
     if (split) { p.h_out = ws + L.off_Rb;
-      umma_gemm_kernel<KIND_F16X2, EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      umma_gemm_kernel<KIND_F16X2, EPI_A2><<<grid_sym, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
     } else { p.h_out = nullptr;
-      umma_gemm_kernel<KIND_TF32, EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p); }
+      umma_gemm_kernel<KIND_TF32, EPI_A2><<<grid_sym, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p); }
     nl += 2;
     if (n == max_iter) break;
     // a4: Q = 1/2 R + 3/8 R R^T
     prof->mark(s, EPI_A4 + 16 * n);
     p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
     if (split) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb;
-      umma_gemm_kernel<KIND_BF16X2, EPI_A4><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      umma_gemm_kernel<KIND_F16X2, EPI_A4><<<grid_sym, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
     } else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr;
-      umma_gemm_kernel<KIND_TF32, EPI_A4><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p); }
+      umma_gemm_kernel<KIND_TF32, EPI_A4><<<grid_sym, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p); }
     // a5: Z_next = Z + Z Q^T ; W = Z_next^T
     prof->mark(s, EPI_A5 + 16 * n);
     p.mapA = pl.mZ[n & 1]; p.mapB = pl.mQ;
     if (split) {
       float* Z32 = reinterpret_cast<float*>(ws + L.off_Z[0]);       // FP32 master copy, updated in place
       p.f32_in = Z32; p.f32_out = Z32; p.h_out = ws + L.off_Zb[(n + 1) & 1]; p.h_out_t = ws + L.off_W;
-      umma_gemm_kernel<KIND_BF16X2, EPI_A5><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      umma_gemm_kernel<KIND_F16X2, EPI_A5><<<grid_full, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
     } else {
       p.f32_in = reinterpret_cast<float*>(ws + L.off_Z[n & 1]);
       p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(n + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
-      umma_gemm_kernel<KIND_TF32, EPI_A5><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      umma_gemm_kernel<KIND_TF32, EPI_A5><<<grid_full, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p);
     }
     nl += 2;
   }

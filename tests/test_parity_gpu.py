@@ -281,6 +281,7 @@ def test_full_size_n8192_bench_configuration_properties():
     rows = rng.integers(0, n, 64)
     cols = rng.integers(0, n, 64)
     Zs = np.einsum("ik,k,ik->i", w.Q[rows], z10, w.Q[cols])
+    Zref = (w.Q * z10[None, :]) @ w.Q.T                 # closed form of the whole iterate (one N^3 product)
     for mode, tol_s, tol_e, err_floor in (("f64", 1e-10, 1e-8, 1e-6), ("split16", 5e-4, 2e-3, 1.0)):
         Z, it, err, fl, _, _ = gpu_refine(w, mode, 10, b.ZFAC_STOP_FIXED)
         assert it == 10 and fl == b.ZFAC_R_MAXITER
@@ -290,6 +291,9 @@ def test_full_size_n8192_bench_configuration_properties():
                 assert err[k] == pytest.approx(errs[k], rel=tol_e), (mode, k)
         samp = np.abs(Z[rows, cols] - Zs).max() / np.abs(Zs).max()
         inv = O.final_residual_per_sqrt_n(w.S, Z)
-        print(f"[n=8192 {mode}] sampled max rel err={samp:.3e} ||Z^T S Z - I||_F/sqrtN={inv:.3e} Err={err[-1]:.3e}")
+        rel = _rel(Z, Zref)
+        print(f"[n=8192 {mode}] rel_F vs closed form={rel:.3e} sampled max rel err={samp:.3e} "
+              f"||Z^T S Z - I||_F/sqrtN={inv:.3e} Err={err[-1]:.3e}")
+        assert rel <= (1e-11 if mode == "f64" else 5e-5)
         assert samp <= tol_s
         assert inv <= (1e-11 if mode == "f64" else 5e-4)
