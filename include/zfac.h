@@ -20,7 +20,7 @@
  *   - matrices are dense, ROW-MAJOR, N x N, leading dimension `ld` in ELEMENTS, ld >= N;
  *     S must be stored in full (both triangles);
  *   - element type is fixed by the mode: double for ZFAC_MODE_F64, float for
- *     ZFAC_MODE_SPLIT16 and ZFAC_MODE_TF32 ("The matrices Z and S are stored in
+ *     ZFAC_MODE_SPLIT16, ZFAC_MODE_HH16 and ZFAC_MODE_TF32 ("The matrices Z and S are stored in
  *     single precision");
  *   - pointers named d_* are DEVICE pointers, h_* are HOST pointers; the caller owns
  *     every buffer including the workspace; the library owns only the small host-side
@@ -45,11 +45,14 @@ typedef struct zfac_ctx zfac_ctx; /* opaque */
 
 /* Precision mode of the four GEMMs of one iteration.
  *  SPLIT16: the paper's (h)(h)+(h)(l)+(l)(h) scheme (Sec. III.A-B, Eq. 17-32): each FP32
- *           operand is split into two 16-bit halves, three tensor-core MMA passes per
- *           product ((l)(l) dropped, Eq. 25/29/32), FP32 accumulation.
- *  TF32   : one tensor-core pass on FP32 operands truncated to TF32, FP32 accumulation.
- *  F64    : the paper's `double` scheme (Table I) on the FP64 tensor pipe. */
-typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2 } zfac_mode;
+ *           operand is split into two FP16 halves (the low half scaled by 2^11), three
+ *           tensor-core MMA passes per product ((l)(l) dropped, Eq. 25/29/32), FP32 accumulation.
+ *  TF32   : one tensor-core pass on FP32 operands rounded to TF32, FP32 accumulation.
+ *  F64    : the paper's `double` scheme (Table I) on the FP64 tensor pipe.
+ *  HH16   : the paper's (h)(h) scheme (Sec. III.C; Table I :211): operands
+ *           rounded to FP16, one tensor-core pass, FP32 accumulation; meant to be followed by
+ *           the refinement step (zfac_refine_refi). */
+typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2, ZFAC_MODE_HH16 = 3 } zfac_mode;
 
 /* Stop rule.  PAPER: Alg. 2's parameter-free test.  FIXED: perform exactly max_iter updates
  * (benchmarks, and parity against the oracle "for the same number of iterations"). */
@@ -67,7 +70,8 @@ typedef enum {
 enum {
   ZFAC_R_STOPPED = 1,  /* the test Err[n] > Err[n-1]^3 fired (converged to the precision floor) */
   ZFAC_R_MAXITER = 2,  /* max_iter updates were performed without the test firing               */
-  ZFAC_R_NONFINITE = 4 /* Err[n] became inf/NaN; iteration stopped                               */
+  ZFAC_R_NONFINITE = 4, /* Err[n] became inf/NaN; iteration stopped                              */
+  ZFAC_R_REFINED = 8    /* zfac_refine_refi: the FP64 refinement updates were applied            */
 };
 
 /* Internal buffers that zfac_peek can copy out (parity tests of the individual steps).
@@ -107,6 +111,32 @@ zfac_status zfac_create(zfac_ctx** ctx, int64_t n, zfac_mode mode, void* d_works
 zfac_status zfac_refine(zfac_ctx* ctx, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0,
                         void* d_Z, int64_t ldz, int max_iter, zfac_stop stop, int* d_iters,
                         double* d_err, int* d_flags, void* stream);
+
+/* Algorithm 3 (PAPER.md:322-341; Sec. IV.B, :308-316): the "+refi" schemes of Table I.
+ *   1. Algorithm 2 in the low-precision mode of `low` (SPLIT16, HH16 or TF32; FP32 S and Z0)
+ *      until its parameter-free test fires (or max_iter updates);
+ *   2. Z is promoted to FP64 and R = I - Z^T S Z is recomputed in FP64 (S promoted exactly);
+ *   3. `refi_steps` (>= 1; the paper uses 1) FP64 updates Z <- Z + Z (1/2 R + 3/8 R R).
+ * `f64` must be a ZFAC_MODE_F64 context of the same n (its own workspace).  d_Z is n x n DOUBLE.
+ * With final_check != 0 the FP64 residual of the returned Z is evaluated too (two more FP64
+ * GEMMs); Alg. 3 as printed stops after the update (final_check = 0).
+ *   d_iters [out] low-precision updates + refi_steps
+ *   d_err   [out] double[max_iter + refi_steps + 2]: Err[0..k] of the low-precision run (k = its
+ *                 stop index), then the FP64 Err before each refinement update, then (final_check)
+ *                 the FP64 Err of the returned Z
+ *   d_flags [out] flags of the low-precision run | ZFAC_R_REFINED
+ * Asynchronous on `stream`, no allocation, no host synchronisation.  Errors: INVALID, CUDA. */
+zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* f64, const void* d_S, int64_t lds, const void* d_Z0,
+                             int64_t ldz0, void* d_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
+                             int* d_iters, double* d_err, int* d_flags, void* stream);
+
+/* Congruence transformation H_perp = Z^T H Z (Eq. 11): what Z is for.  H is
+ * n x n symmetric (full storage), Z n x n (any inverse factor), element type of the context's
+ * mode; the product runs through the same kernels as the residual (T = (H Z)^T, then Z^T (H Z)
+ * with a symmetric-output epilogue: off-diagonal tiles are mirrored).  d_out is n x n, ld ldo.
+ * Asynchronous on `stream`.  Uses the context's workspace: not concurrently with zfac_refine. */
+zfac_status zfac_congruence(zfac_ctx* ctx, const void* d_H, int64_t ldh, const void* d_Z, int64_t ldz,
+                            void* d_out, int64_t ldo, void* stream);
 
 /* Same operation on HOST buffers (pinned memory recommended): copies S and Z0 to the device
  * staging area of the workspace, runs zfac_refine, copies Z, iters, Err[0..max_iter] and flags

@@ -42,7 +42,8 @@ Pins (tests/test_oracle_pins.py): exact-rational brute force at N <= 4; the
 printed error polynomial c,d,e = 5/8,-15/64,9/64 as a matrix
 identity for non-symmetric Z0; Z -> S^-1/2 from a dense eigendecomposition when
 Z0 ∝ I; Z Z^T = S^-1 for non-commuting Z0; cubic order; stop-rule cases;
-scaling / permutation covariances; diagonal S reduces to N scalar recursions.
+scaling / permutation covariances; diagonal S reduces to N scalar recursions;
+`congruence` against the generalized eigenvalues of (H, S) from scipy.linalg.eigh.
 Every function below is pinned; none is "parity unpinned".
 """
 from __future__ import annotations
@@ -156,6 +157,12 @@ def refine_with_refi(S: np.ndarray, Z0: np.ndarray, max_iter: int, low_dtype=np.
         Z = update_delta_form(Z, R)
     err.append(err_fro(residual(S64, Z)))
     return RefineResult(Z, low.iters + refi_steps, np.asarray(err), low.flags)
+
+
+def congruence(H: np.ndarray, Z: np.ndarray) -> np.ndarray:
+    """H_perp = Z^T H Z   (Eq. 11, lines 88-92): the congruence transformation that turns
+    H C = S C eps into the standard problem H_perp C_perp = C_perp eps when Z^T S Z = I."""
+    return Z.T @ (H @ Z)
 
 
 def final_residual_per_sqrt_n(S: np.ndarray, Z: np.ndarray) -> float:

@@ -16,17 +16,18 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libzfac.so")
 
-ZFAC_MODE_SPLIT16, ZFAC_MODE_TF32, ZFAC_MODE_F64 = 0, 1, 2
+ZFAC_MODE_SPLIT16, ZFAC_MODE_TF32, ZFAC_MODE_F64, ZFAC_MODE_HH16 = 0, 1, 2, 3
 ZFAC_STOP_PAPER, ZFAC_STOP_FIXED = 0, 1
 ZFAC_OK, ZFAC_E_INVALID, ZFAC_E_UNSUPPORTED, ZFAC_E_WORKSPACE, ZFAC_E_CUDA = 0, 1, 2, 3, 4
-ZFAC_R_STOPPED, ZFAC_R_MAXITER, ZFAC_R_NONFINITE = 1, 2, 4
+ZFAC_R_STOPPED, ZFAC_R_MAXITER, ZFAC_R_NONFINITE, ZFAC_R_REFINED = 1, 2, 4, 8
 ZFAC_BUF_T, ZFAC_BUF_R, ZFAC_BUF_Q, ZFAC_BUF_Z = 0, 1, 2, 3
 
-MODES = {"split16": ZFAC_MODE_SPLIT16, "tf32": ZFAC_MODE_TF32, "f64": ZFAC_MODE_F64}
+MODES = {"split16": ZFAC_MODE_SPLIT16, "tf32": ZFAC_MODE_TF32, "f64": ZFAC_MODE_F64, "hh16": ZFAC_MODE_HH16}
 
 # symbols include/zfac.h declares (tests check that the library exports every one)
 EXPORTS = [
-    "zfac_workspace_bytes", "zfac_create", "zfac_refine", "zfac_refine_host", "zfac_peek",
+    "zfac_workspace_bytes", "zfac_create", "zfac_refine", "zfac_refine_host", "zfac_refine_refi",
+    "zfac_congruence", "zfac_peek",
     "zfac_last_launch_count", "zfac_padded_n", "zfac_destroy", "zfac_status_string",
     "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile",
 ]
@@ -63,6 +64,10 @@ def lib() -> ctypes.CDLL:
     L.zfac_refine.argtypes = [vp, vp, i64, vp, i64, vp, i64, ci, ci, vp, vp, vp, vp]
     L.zfac_refine_host.restype = ci
     L.zfac_refine_host.argtypes = [vp, vp, i64, vp, i64, vp, i64, ci, ci, vp, vp, vp, vp]
+    L.zfac_refine_refi.restype = ci
+    L.zfac_refine_refi.argtypes = [vp, vp, vp, i64, vp, i64, vp, i64, ci, ci, ci, vp, vp, vp, vp]
+    L.zfac_congruence.restype = ci
+    L.zfac_congruence.argtypes = [vp, vp, i64, vp, i64, vp, i64, vp]
     L.zfac_peek.restype = ci
     L.zfac_peek.argtypes = [vp, ci, vp, i64, vp]
     L.zfac_last_launch_count.restype = ci
@@ -117,6 +122,21 @@ def zfac_refine_host(ctx: int, h_S: int, lds: int, h_Z0: int, ldz0: int, h_Z: in
                                 h_flags, ctypes.c_void_p(stream))
     if st != ZFAC_OK:
         raise ZfacError(st, "zfac_refine_host")
+
+
+def zfac_refine_refi(low: int, f64: int, d_S: int, lds: int, d_Z0: int, ldz0: int, d_Z: int, ldz: int,
+                     max_iter: int, refi_steps: int, final_check: int, d_iters: int, d_err: int, d_flags: int,
+                     stream: int = 0) -> None:
+    st = lib().zfac_refine_refi(low, f64, d_S, lds, d_Z0, ldz0, d_Z, ldz, int(max_iter), int(refi_steps),
+                                int(final_check), d_iters, d_err, d_flags, ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_refine_refi")
+
+
+def zfac_congruence(ctx: int, d_H: int, ldh: int, d_Z: int, ldz: int, d_out: int, ldo: int, stream: int = 0) -> None:
+    st = lib().zfac_congruence(ctx, d_H, ldh, d_Z, ldz, d_out, ldo, ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_congruence")
 
 
 def zfac_peek(ctx: int, which: int, d_out: int, ld: int, stream: int = 0) -> None:
@@ -183,9 +203,10 @@ class Zfac:
         except Exception:
             pass
 
-    def _check(self, t: torch.Tensor, name: str) -> None:
-        if t.dtype != self.dtype or t.dim() != 2 or t.shape[0] != self.n or t.shape[1] != self.n:
-            raise ValueError(f"{name}: expected {self.n}x{self.n} {self.dtype}, got {tuple(t.shape)} {t.dtype}")
+    def _check(self, t: torch.Tensor, name: str, dtype=None) -> None:
+        dtype = dtype or self.dtype
+        if t.dtype != dtype or t.dim() != 2 or t.shape[0] != self.n or t.shape[1] != self.n:
+            raise ValueError(f"{name}: expected {self.n}x{self.n} {dtype}, got {tuple(t.shape)} {t.dtype}")
         if t.stride(1) != 1 or t.stride(0) < self.n:
             raise ValueError(f"{name}: must be row-major with unit column stride")
 
@@ -225,6 +246,35 @@ class Zfac:
                              Z.stride(0), max_iter, stop, ctypes.addressof(iters), err.ctypes.data,
                              ctypes.addressof(flags), stream)
         return Z, iters.value, err[: iters.value + 1], flags.value
+
+    def refine_refi(self, f64: "Zfac", S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, refi_steps: int = 1,
+                    final_check: bool = True, out: Optional[torch.Tensor] = None, sync: bool = True):
+        """Alg. 3: this (low-precision) context until its test fires, then `refi_steps` FP64 updates in `f64`.
+        FP32 device tensors in, FP64 device tensor out: (Z, iters, err[...], flags)."""
+        self._check(S, "S"); self._check(Z0, "Z0")
+        Z = out if out is not None else torch.empty((self.n, self.n), dtype=torch.float64, device=S.device)
+        self._check(Z, "Z", torch.float64)
+        d_iters = torch.zeros(1, dtype=torch.int32, device=S.device)
+        d_flags = torch.zeros(1, dtype=torch.int32, device=S.device)
+        d_err = torch.full((max_iter + refi_steps + 2,), float("nan"), dtype=torch.float64, device=S.device)
+        stream = torch.cuda.current_stream(S.device).cuda_stream
+        zfac_refine_refi(self.ctx, f64.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), Z.data_ptr(),
+                         Z.stride(0), max_iter, refi_steps, int(final_check), d_iters.data_ptr(), d_err.data_ptr(),
+                         d_flags.data_ptr(), stream)
+        if not sync:
+            return Z, d_iters, d_err, d_flags
+        torch.cuda.current_stream(S.device).synchronize()
+        it = int(d_iters.item())
+        return Z, it, d_err[: it + 1 + int(final_check)].cpu().numpy(), int(d_flags.item())
+
+    def congruence(self, H: torch.Tensor, Z: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """H_perp = Z^T H Z (Eq. 11) on device tensors of the mode's element type."""
+        self._check(H, "H"); self._check(Z, "Z")
+        o = out if out is not None else torch.empty((self.n, self.n), dtype=self.dtype, device=H.device)
+        self._check(o, "out")
+        stream = torch.cuda.current_stream(H.device).cuda_stream
+        zfac_congruence(self.ctx, H.data_ptr(), H.stride(0), Z.data_ptr(), Z.stride(0), o.data_ptr(), o.stride(0), stream)
+        return o
 
     def peek(self, which: int) -> torch.Tensor:
         out = torch.empty((self.n, self.n), dtype=self.dtype, device=self.device)

@@ -38,7 +38,9 @@ struct zfac_ctx {
   Prof prof;
 };
 
-static bool valid_mode(int m) { return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_F64; }
+static bool valid_mode(int m) {
+  return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_F64 || m == ZFAC_MODE_HH16;
+}
 
 extern "C" {
 
@@ -83,6 +85,7 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   if (mode == ZFAC_MODE_F64) {
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A1>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A2>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_X3>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A4>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A5>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
   } else {
@@ -137,7 +140,9 @@ int zfac_get_profile(zfac_ctx* c, int* tags, float* ms, int cap) {
 
 int zfac_last_launch_count(const zfac_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
-static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s) {
+// skip_last: Alg. 3 as printed ends after the update, without evaluating the residual of the result.
+static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s,
+                              bool skip_last = false) {
   const Layout& L = c->L;
   char* ws = c->ws;
   State* st = reinterpret_cast<State*>(ws + L.off_state);
@@ -154,6 +159,7 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   p.stop.st = st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = tri; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
   for (int n = 0; n <= max_iter; ++n) {
+    if (n == max_iter && skip_last) break;
     p.A = W; p.B = S; p.out0 = T; p.out1 = nullptr; p.in0 = nullptr;
     c->prof.mark(s, EPI_A1 + 16 * n);
     f64_gemm_kernel<EPI_A1><<<full, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
@@ -175,6 +181,41 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   return ZFAC_OK;
 }
 
+// Step a0: copy S and Z0 (element type float if in_f32, else the mode's own) into the padded buffers.
+static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, bool in_f32,
+                           cudaStream_t s) {
+  const Layout& L = c->L;
+  char* ws = c->ws;
+  CopyInArgs ci{};
+  ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np;
+  ci.st = reinterpret_cast<State*>(ws + L.off_state);
+  ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
+  dim3 gi((unsigned)(L.np / 32), (unsigned)(L.np / 32)), bi(32, 8);
+  switch (c->mode) {
+    case ZFAC_MODE_F64:
+      if (in_f32) copy_in_kernel<ZFAC_MODE_F64, float><<<gi, bi, 0, s>>>(ci);
+      else copy_in_kernel<ZFAC_MODE_F64, double><<<gi, bi, 0, s>>>(ci);
+      break;
+    case ZFAC_MODE_TF32: copy_in_kernel<ZFAC_MODE_TF32, float><<<gi, bi, 0, s>>>(ci); break;
+    case ZFAC_MODE_HH16: copy_in_kernel<ZFAC_MODE_HH16, float><<<gi, bi, 0, s>>>(ci); break;
+    default: copy_in_kernel<ZFAC_MODE_SPLIT16, float><<<gi, bi, 0, s>>>(ci); break;
+  }
+  c->launches += 1;
+}
+
+static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int parity, void* d_Z, int64_t ldz,
+                            int* d_iters, int* d_flags, cudaStream_t s) {
+  const Layout& L = c->L;
+  CopyOutArgs co{};
+  co.Zbuf[0] = b0; co.Zbuf[1] = b1; co.parity = parity;
+  co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np;
+  co.st = reinterpret_cast<State*>(c->ws + L.off_state); co.d_iters = d_iters; co.d_flags = d_flags;
+  dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
+  if (c->mode == ZFAC_MODE_F64) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
+  else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
+  c->launches += 1;
+}
+
 zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
                         int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
                         void* stream) {
@@ -184,18 +225,10 @@ zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;
-  State* st = reinterpret_cast<State*>(ws + L.off_state);
   c->launches = 0;
   c->prof.count = 0;
 
-  CopyInArgs ci{};
-  ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np; ci.st = st;
-  ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
-  dim3 gi((unsigned)(L.np / 32), (unsigned)(L.np / 32)), bi(32, 8);
-  if (c->mode == ZFAC_MODE_F64) copy_in_kernel<ZFAC_MODE_F64><<<gi, bi, 0, s>>>(ci);
-  else if (c->mode == ZFAC_MODE_TF32) copy_in_kernel<ZFAC_MODE_TF32><<<gi, bi, 0, s>>>(ci);
-  else copy_in_kernel<ZFAC_MODE_SPLIT16><<<gi, bi, 0, s>>>(ci);
-  c->launches += 1;
+  launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, s);
 
   zfac_status rs;
   if (c->mode == ZFAC_MODE_F64) {
@@ -212,13 +245,72 @@ zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d
   }
   if (rs != ZFAC_OK) return rs;
 
-  CopyOutArgs co{};
-  co.Zbuf[0] = ws + L.off_Z[0]; co.Zbuf[1] = ws + L.off_Z[1];
-  co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np; co.st = st; co.d_iters = d_iters; co.d_flags = d_flags;
-  dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
-  if (c->mode == ZFAC_MODE_F64) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
-  else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
-  c->launches += 1;
+  launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, s);
+  ZF_CUDA(cudaGetLastError());
+  return ZFAC_OK;
+}
+
+zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* f64, const void* d_S, int64_t lds, const void* d_Z0,
+                             int64_t ldz0, void* d_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
+                             int* d_iters, double* d_err, int* d_flags, void* stream) {
+  if (!low || !f64 || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
+  if (low->mode == ZFAC_MODE_F64 || f64->mode != ZFAC_MODE_F64 || low->n != f64->n) return ZFAC_E_INVALID;
+  if (lds < low->n || ldz0 < low->n || ldz < low->n || max_iter < 0 || refi_steps < 1 || refi_steps > 4000)
+    return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& L = f64->L;
+  // 1. Alg. 2 in low precision; its FP32 result goes to the FP64 context's staging area
+  float* zlow = reinterpret_cast<float*>(f64->ws + L.off_stage_Z);
+  zfac_status rs = zfac_refine(low, d_S, lds, d_Z0, ldz0, zlow, low->n, max_iter, ZFAC_STOP_PAPER, d_iters, d_err,
+                               d_flags, s);
+  if (rs != ZFAC_OK) return rs;
+  // 2. Z = FP64[Z], S promoted exactly; 3. refi_steps FP64 updates (kernels of the F64 mode)
+  f64->launches = 0;
+  f64->prof.count = 0;
+  launch_copy_in(f64, d_S, lds, zlow, f64->n, true, s);
+  double* err64 = reinterpret_cast<double*>(f64->ws + L.off_stage_out);
+  rs = refine_f64(f64, refi_steps, ZFAC_STOP_FIXED, err64, s, final_check == 0);
+  if (rs != ZFAC_OK) return rs;
+  launch_copy_out(f64, f64->ws + L.off_Z[0], f64->ws + L.off_Z[1], refi_steps & 1, d_Z, ldz, nullptr, nullptr, s);
+  refi_merge_kernel<<<1, 32, 0, s>>>(err64, refi_steps + (final_check ? 1 : 0), refi_steps, d_err, d_iters, d_flags);
+  f64->launches += 1;
+  low->launches += f64->launches;
+  ZF_CUDA(cudaGetLastError());
+  return ZFAC_OK;
+}
+
+zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const void* d_Z, int64_t ldz, void* d_out,
+                            int64_t ldo, void* stream) {
+  if (!c || !d_H || !d_Z || !d_out) return ZFAC_E_INVALID;
+  if (ldh < c->n || ldz < c->n || ldo < c->n) return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& L = c->L;
+  char* ws = c->ws;
+  c->launches = 0;
+  c->prof.count = 0;
+  launch_copy_in(c, d_H, ldh, d_Z, ldz, false, s);        // H takes the place of S; W = Z^T
+  if (c->mode == ZFAC_MODE_F64) {
+    double* H = reinterpret_cast<double*>(ws + L.off_S);
+    double* W = reinterpret_cast<double*>(ws + L.off_W);
+    double* T = reinterpret_cast<double*>(ws + L.off_T);
+    const int tiles = (int)(L.np / F64_BM);
+    F64Params p{};
+    p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = reinterpret_cast<State*>(ws + L.off_state);
+    p.A = W; p.B = H; p.out0 = T;
+    f64_gemm_kernel<EPI_A1><<<tiles * tiles, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    p.A = W; p.B = T; p.out0 = reinterpret_cast<double*>(ws + L.off_R);
+    f64_gemm_kernel<EPI_X3><<<tiles * (tiles + 1) / 2, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    c->launches += 2;
+  } else {
+    int nl = 0;
+    cudaError_t e = umma_congruence(c->umma, s, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_congruence: %s", cudaGetErrorString(e));
+      return ZFAC_E_CUDA;
+    }
+  }
+  launch_copy_out(c, ws + L.off_R, ws + L.off_R, 0, d_out, ldo, nullptr, nullptr, s);
   ZF_CUDA(cudaGetLastError());
   return ZFAC_OK;
 }
@@ -271,11 +363,19 @@ zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void
     }
     if (c->mode == ZFAC_MODE_F64) peek_kernel<double, 0><<<g, 256, 0, s>>>(ws + off, d_out, ld, n, np);
     else peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + off, d_out, ld, n, np);
-  } else {
+  } else if (c->mode == ZFAC_MODE_SPLIT16) {
     switch (which) {
       case ZFAC_BUF_T: peek_kernel<float, 1><<<g, 256, 0, s>>>(ws + L.off_T, d_out, ld, n, np); break;
       case ZFAC_BUF_R: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
       case ZFAC_BUF_Q: peek_kernel<float, 1><<<g, 256, 0, s>>>(ws + L.off_Qb, d_out, ld, n, np); break;
+      case ZFAC_BUF_Z: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_Z[0], d_out, ld, n, np); break;
+      default: return ZFAC_E_INVALID;
+    }
+  } else {  // HH16
+    switch (which) {
+      case ZFAC_BUF_T: peek_kernel<float, 2><<<g, 256, 0, s>>>(ws + L.off_T, d_out, ld, n, np); break;
+      case ZFAC_BUF_R: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
+      case ZFAC_BUF_Q: peek_kernel<float, 2><<<g, 256, 0, s>>>(ws + L.off_Qb, d_out, ld, n, np); break;
       case ZFAC_BUF_Z: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_Z[0], d_out, ld, n, np); break;
       default: return ZFAC_E_INVALID;
     }

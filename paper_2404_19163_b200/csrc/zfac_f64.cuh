@@ -24,7 +24,7 @@ constexpr int F64_THREADS = 256;
 constexpr int F64_STAGE_DOUBLES = (F64_BM + F64_BN) * F64_LDS;
 constexpr int F64_SMEM_BYTES = F64_STAGES * F64_STAGE_DOUBLES * 8;
 
-enum { EPI_A1 = 1, EPI_A2 = 2, EPI_A4 = 4, EPI_A5 = 5 };
+enum { EPI_A1 = 1, EPI_A2 = 2, EPI_X3 = 3 /* X = Z^T H Z itself (congruence, Eq. 11) */, EPI_A4 = 4, EPI_A5 = 5 };
 
 struct F64Params {
   const double* A;      // [Np][ld]
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(F64_THREADS, 1) f64_gemm_kernel(const F64Param
   __shared__ double red[32];
   __shared__ int last_flag;
 
-  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4);
+  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3);
   int tm, tn;
   if (SYM) tri_decode((int)blockIdx.x, tm, tn);
   else band_decode((int)blockIdx.x, p.tiles, p.tiles, 8, tm, tn);
@@ -143,6 +143,9 @@ __global__ void __launch_bounds__(F64_THREADS, 1) f64_gemm_kernel(const F64Param
         v0 = (m == n ? 1.0 : 0.0) - v0;              // R = I - X
         v1 = (m == n + 1 ? 1.0 : 0.0) - v1;
         sumsq += v0 * v0 + v1 * v1;
+        *reinterpret_cast<double2*>(p.out0 + m * ld + n) = make_double2(v0, v1);
+        if (tm != tn) { p.out0[(size_t)n * ld + m] = v0; p.out0[(size_t)(n + 1) * ld + m] = v1; }
+      } else if (EPI == EPI_X3) {
         *reinterpret_cast<double2*>(p.out0 + m * ld + n) = make_double2(v0, v1);
         if (tm != tn) { p.out0[(size_t)n * ld + m] = v0; p.out0[(size_t)(n + 1) * ld + m] = v1; }
       } else if (EPI == EPI_A4) {

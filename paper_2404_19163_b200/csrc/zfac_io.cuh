@@ -7,15 +7,15 @@
 // unchanged (zero padding would add Np - N to ||R||_F^2).
 //
 // Operand splitting (Eq. 17-18, :143-149): A ~ A_hi + A_lo.
-//   fp16 pair (residual GEMMs a1, a2):  hi = FP16[a],  lo' = FP16[(a - FP32[hi]) * 2^11]
+//   fp16 pair (SPLIT16, all four GEMMs):  hi = FP16[a],  lo' = FP16[(a - FP32[hi]) * 2^11]
 //       -- the low half is stored SCALED by 2^11 so that it does not fall into the FP16
 //       subnormal range; the products that contain one lo' are accumulated separately and
 //       weighted by 2^-11 in the epilogue.  Error <= 2^-22 |a| as in PAPER.md:169.
-//   bf16 pair (update GEMMs a4, a5):    hi = BF16[a],  lo = BF16[a - FP32[hi]]
-//       -- 16 significant bits, FP32 exponent range: R and Q shrink towards 0 as the
-//       iteration converges and would underflow FP16.
+//   R and Q shrink towards 0 as the iteration converges and their hi half underflows gradually
+//   (fp16 subnormal spacing 2^-24); the remainder, scaled by 2^11, is then below 2^-14 and is
+//   stored to 11 bits, so the ABSOLUTE error of the pair is <= 2^-36 -- far below the FP32
+//   rounding of the sum Z + Z Q that these operands feed.
 #pragma once
-#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include "zfac_common.cuh"
 
@@ -32,10 +32,6 @@ __device__ __forceinline__ __half f2h_sat(float a) {
 __device__ __forceinline__ void split_f16(float a, __half& hi, __half& lo) {
   hi = f2h_sat(a);
   lo = f2h_sat((a - __half2float(hi)) * LO_SCALE);
-}
-__device__ __forceinline__ void split_bf16(float a, __nv_bfloat16& hi, __nv_bfloat16& lo) {
-  hi = __float2bfloat16_rn(a);
-  lo = __float2bfloat16_rn(a - __bfloat162float(hi));
 }
 
 // Round-to-nearest FP32 -> TF32 (low 13 mantissa bits cleared).  The tensor core TRUNCATES FP32
@@ -57,12 +53,14 @@ struct Layout {
   size_t off_stage_S = 0, off_stage_Z = 0, off_stage_out = 0;
   // F64 / TF32: one buffer each of the mode's element type; Z double-buffered
   size_t off_S = 0, off_W = 0, off_T = 0, off_R = 0, off_Q = 0, off_Z[2] = {0, 0};
-  // SPLIT16: S16/W16/T16 are fp16 [2][Np][Np]; Rb/Qb/Zb[2] bf16 [2][Np][Np]; R and Z(=off_Z[0]) fp32
+  // SPLIT16 / HH16: S, W, T, Rb, Qb, Zb[2] are fp16 [planes][Np][Np] (planes = 2: hi, lo'; HH16: 1);
+  // R and the master Z (= off_Z[0]) are fp32
   size_t off_Rb = 0, off_Qb = 0, off_Zb[2] = {0, 0};
   size_t total = 0;
 };
 
 inline int64_t padded_n(int64_t n, int mode) { return round_up(n, mode == ZFAC_MODE_F64 ? 128 : 256); }
+inline bool mode_is_h16(int mode) { return mode == ZFAC_MODE_SPLIT16 || mode == ZFAC_MODE_HH16; }
 
 inline Layout make_layout(int64_t n, int mode) {
   Layout L;
@@ -77,11 +75,12 @@ inline Layout make_layout(int64_t n, int mode) {
   L.off_stage_S = take(n2 * L.elt);
   L.off_stage_Z = take(n2 * L.elt);
   L.off_stage_out = take((size_t)4096 * sizeof(double) + 64);
-  if (mode == ZFAC_MODE_SPLIT16) {
-    L.off_S = take(np2 * 4); L.off_W = take(np2 * 4); L.off_T = take(np2 * 4);
-    L.off_R = take(np2 * 4); L.off_Rb = take(np2 * 4); L.off_Qb = take(np2 * 4);
+  if (mode_is_h16(mode)) {
+    const size_t hb = np2 * (mode == ZFAC_MODE_SPLIT16 ? 4 : 2);     // fp16 planes: (hi, lo') or hi only
+    L.off_S = take(hb); L.off_W = take(hb); L.off_T = take(hb);
+    L.off_R = take(np2 * 4); L.off_Rb = take(hb); L.off_Qb = take(hb);
     L.off_Z[0] = take(np2 * 4); L.off_Z[1] = L.off_Z[0];
-    L.off_Zb[0] = take(np2 * 4); L.off_Zb[1] = take(np2 * 4);
+    L.off_Zb[0] = take(hb); L.off_Zb[1] = take(hb);
   } else {
     L.off_S = take(np2 * L.elt); L.off_W = take(np2 * L.elt); L.off_T = take(np2 * L.elt);
     L.off_R = take(np2 * L.elt); L.off_Q = take(np2 * L.elt);
@@ -100,14 +99,16 @@ struct CopyInArgs {
   void* oS;            // F64: double[Np][Np]; TF32: float; SPLIT16: half[2][Np][Np]
   void* oZ;            // F64/TF32: Z[0];  SPLIT16: float Z32
   void* oW;            // F64/TF32: W;     SPLIT16: half[2][Np][Np]
-  void* oZb;           // SPLIT16: bf16[2][Np][Np] (Zb[0])
+  void* oZb;           // SPLIT16 / HH16: half[planes][Np][Np] (Zb[0])
 };
 
 // One 32x32 tile per CTA (32 x 8 threads).  Reads S and Z0 tiles (identity padding beyond n),
 // writes S, Z (row-major) and W = Z^T (through a shared-memory transpose).
-template <int MODE>
+// Tin = element type of the user's S and Z0: the mode's own type, or float for the FP64
+// refinement step of Alg. 3 ("Z = FP64[Z]"; S is promoted exactly).
+template <int MODE, typename Tin>
 __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
-  using Tin = typename std::conditional<MODE == ZFAC_MODE_F64, double, float>::type;
+  using Tw = typename std::conditional<MODE == ZFAC_MODE_F64, double, float>::type;   // internal element type
   __shared__ Tin tile[32][33];
   if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) {
     a.st->done = 0; a.st->iters = 0; a.st->flags = 0;
@@ -133,12 +134,16 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
       static_cast<float*>(a.oZ)[o] = (float)z;
       __half zh, zl; split_f16((float)z, zh, zl);
       static_cast<__half*>(a.oZb)[o] = zh; static_cast<__half*>(a.oZb)[np2 + o] = zl;
+    } else if (MODE == ZFAC_MODE_HH16) {
+      static_cast<__half*>(a.oS)[o] = f2h_sat((float)s);
+      static_cast<float*>(a.oZ)[o] = (float)z;
+      static_cast<__half*>(a.oZb)[o] = f2h_sat((float)z);
     } else if (MODE == ZFAC_MODE_TF32) {
       static_cast<float*>(a.oS)[o] = round_tf32((float)s);
       static_cast<float*>(a.oZ)[o] = (float)z;
     } else {
-      static_cast<Tin*>(a.oS)[o] = s;
-      static_cast<Tin*>(a.oZ)[o] = z;
+      static_cast<Tw*>(a.oS)[o] = (Tw)s;
+      static_cast<Tw*>(a.oZ)[o] = (Tw)z;
     }
   }
   __syncthreads();
@@ -150,28 +155,31 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
     if (MODE == ZFAC_MODE_SPLIT16) {
       __half hi, lo; split_f16((float)z, hi, lo);
       static_cast<__half*>(a.oW)[o] = hi; static_cast<__half*>(a.oW)[np2 + o] = lo;
+    } else if (MODE == ZFAC_MODE_HH16) {
+      static_cast<__half*>(a.oW)[o] = f2h_sat((float)z);
     } else if (MODE == ZFAC_MODE_TF32) {
       static_cast<float*>(a.oW)[o] = round_tf32((float)z);
     } else {
-      static_cast<Tin*>(a.oW)[o] = z;
+      static_cast<Tw*>(a.oW)[o] = (Tw)z;
     }
   }
 }
 
 // ------------------------------------------------------------------ copy-out (step a6)
 struct CopyOutArgs {
-  const void* Zbuf[2];   // internal Z buffers (selected by iters parity; equal in SPLIT16)
+  const void* Zbuf[2];   // internal Z buffers (selected by iters parity; equal in the 16-bit modes)
   void* Z; int64_t ldz;
   int n, np;
   const State* st;
-  int* d_iters; int* d_flags;
+  int* d_iters; int* d_flags;   // may be null (refinement step, congruence)
+  int parity;                   // -1: buffer = Zbuf[st->iters & 1]; else Zbuf[parity]
 };
 
 template <typename T>
 __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
   const int iters = a.st->iters;
-  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { *a.d_iters = iters; *a.d_flags = a.st->flags; }
-  const T* src = static_cast<const T*>(a.Zbuf[iters & 1]);
+  if (a.d_iters && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { *a.d_iters = iters; *a.d_flags = a.st->flags; }
+  const T* src = static_cast<const T*>(a.Zbuf[a.parity >= 0 ? a.parity : (iters & 1)]);
   T* dst = static_cast<T*>(a.Z);
   const int c = blockIdx.x * 256 + threadIdx.x;
   const int r0 = blockIdx.y * 8;
@@ -183,8 +191,19 @@ __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
   }
 }
 
+// ------------------------------------------------------------------ Alg. 3 bookkeeping
+// Appends the FP64 refinement history to the low-precision one and publishes iters / flags.
+__global__ void refi_merge_kernel(const double* err64, int n64, int refi_steps, double* d_err, int* d_iters, int* d_flags) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    const int k = *d_iters;                       // stop index of the low-precision run
+    for (int i = 0; i < n64; ++i) d_err[k + 1 + i] = err64[i];
+    *d_iters = k + refi_steps;
+    *d_flags |= ZFAC_R_REFINED;
+  }
+}
+
 // ------------------------------------------------------------------ peek (tests)
-// kind 0: plain T buffer; 1: fp16 pair hi + lo' 2^-11; 2: bf16 pair hi + lo
+// kind 0: plain T buffer; 1: fp16 pair hi + lo' 2^-11; 2: fp16 (hi only)
 template <typename T, int KIND>
 __global__ void __launch_bounds__(256) peek_kernel(const void* src, void* out, int64_t ld, int n, int np) {
   const int c = blockIdx.x * 256 + threadIdx.x, r = blockIdx.y;
@@ -196,8 +215,7 @@ __global__ void __launch_bounds__(256) peek_kernel(const void* src, void* out, i
     const __half* h = static_cast<const __half*>(src);
     v = (T)(__half2float(h[o]) + __half2float(h[np2 + o]) * LO_UNSCALE);
   } else {
-    const __nv_bfloat16* h = static_cast<const __nv_bfloat16*>(src);
-    v = (T)(__bfloat162float(h[o]) + __bfloat162float(h[np2 + o]));
+    v = (T)__half2float(static_cast<const __half*>(src)[o]);
   }
   static_cast<T*>(out)[(size_t)r * ld + c] = v;
 }

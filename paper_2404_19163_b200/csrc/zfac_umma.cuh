@@ -1,4 +1,4 @@
-// tcgen05 (5th-gen tensor core) GEMM kernels for the SPLIT16 and TF32 modes.
+// tcgen05 (5th-gen tensor core) GEMM kernels for the SPLIT16, HH16 and TF32 modes.
 //
 // One persistent, warp-specialised kernel template serves all four GEMMs of an iteration.
 // As in zfac_f64.cuh every product is brought to  D[m][n] = sum_k A[m][k] B[n][k]  with both
@@ -6,25 +6,30 @@
 //   a1  T = (S Z)^T = W S^T    (Eq. 22)     a2  X = Z^T (S Z) = W T^T   (Eq. 26)
 //   a4  P = R R = R R^T        (Eq. 30-32)  a5  Z Q = Z Q^T             (Eq. 13)
 //
-// Roles (192 threads): warp 0 = TMA producer (one lane), warp 1 = TMEM allocator + MMA issuer
-// (one lane issues tcgen05.mma), warps 2-5 = epilogue (tcgen05.ld, fused O(N^2) work, stores).
-// Pipelines: shared-memory ring full/empty mbarriers (TMA <-> MMA) and TMEM full/empty
-// mbarriers (MMA <-> epilogue).  CTA tile 128 x 256, operands staged by TMA in the canonical
-// K-major 128B-swizzle layout, accumulators in TMEM (512 columns).
+// CTA pair (cluster of 2, tcgen05 cta_group::2): one 256 x 256 output tile per pair.  CTA r of
+// the pair stages rows [128 r, 128 r + 128) of the A tile and of the B tile (TMA, 128B-swizzle
+// boxes of 128 rows x 128 B, landing on the LEADER's full barrier), the leader's elected thread
+// issues tcgen05.mma with M = 256, N = 256 reading both CTAs' shared memory, and each CTA's
+// TMEM (128 lanes x 512 columns) receives rows [128 r, 128 r + 128) of the accumulators.
+//
+// Roles per CTA (64 + 256 threads): warp 0 = TMA producer (one lane), warp 1 = TMEM allocator +
+// (leader only) MMA issuer, warps 2-9 = epilogue (tcgen05.ld, fused O(N^2) work, stores).
+// Pipelines: shared-memory ring full/empty mbarriers (TMA <-> MMA; "empty" is multicast to both
+// CTAs by tcgen05.commit) and TMEM full/empty mbarriers (MMA <-> the epilogue warps of both CTAs).
 //
 // Precision kinds
-//   KIND_F16X2  (a1, a2 of SPLIT16): operands are fp16 pairs (hi, lo' = lo * 2^11), Eq. 17-18.
-//       Three MMA passes per k-step, (l)(l) dropped (Eq. 25, 29):
+//   KIND_F16X2 (SPLIT16 mode): operands are fp16 pairs (hi, lo' = lo * 2^11), Eq. 17-18.
+//       Three MMA passes per k-step, (l)(l) dropped (Eq. 25, 29, 32):
 //           D_hh += A_hi B_hi          D_x += A_hi B_lo' + A_lo' B_hi
-//       two FP32 accumulators; the epilogue forms D_hh + 2^-11 D_x.
-//   KIND_BF16X2 (a4, a5 of SPLIT16): operands are bf16 pairs (hi, lo); three passes into ONE
-//       accumulator; two accumulator buffers so the epilogue overlaps the next tile.
-//   KIND_TF32   (TF32 mode): FP32 operands read as TF32, one pass, two accumulator buffers.
+//       two FP32 accumulators (256 TMEM columns each); the epilogue forms D_hh + 2^-11 D_x.
+//       D_hh is drained into FP32 registers every chunk_kb k-blocks (promoted accumulation).
+//   KIND_HH16  (HH16 mode, the paper's (h)(h) scheme, Sec. III.C): fp16 operands, one pass,
+//       two accumulator buffers so that the epilogue overlaps the next tile.
+//   KIND_TF32  (TF32 mode): FP32 operands read as TF32, one pass, two accumulator buffers.
 #pragma once
 #include <cuda.h>
 #include <stdio.h>
 #include <stdlib.h>
-#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include "zfac_common.cuh"
 #include "zfac_io.cuh"
@@ -32,56 +37,72 @@
 
 namespace zfac {
 
-enum { KIND_F16X2 = 0, KIND_BF16X2 = 1, KIND_TF32 = 2 };
+enum { KIND_F16X2 = 0, KIND_HH16 = 1, KIND_TF32 = 2 };
 
-constexpr int UM_BM = 128, UM_BN = 256;
+constexpr int UM_TILE = 256;                     // pair tile (M and N)
+constexpr int UM_ROWS = 128;                     // operand rows staged per CTA (of A and of B)
 constexpr int UM_ROWB = 128;                     // bytes per operand row per k-block (= swizzle span)
-constexpr int UM_A_BYTES = UM_BM * UM_ROWB;      // 16 KB
-constexpr int UM_B_BYTES = UM_BN * UM_ROWB;      // 32 KB
+constexpr int UM_BOX_BYTES = UM_ROWS * UM_ROWB;  // 16 KB: one TMA box
 constexpr int UM_SMEM_OPERANDS = 192 * 1024;
 constexpr int UM_SMEM_BYTES = UM_SMEM_OPERANDS + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int UM_TMEM_COLS = 512;
+constexpr int UM_EPI_WARPS = 8;
+constexpr int UM_THREADS = 64 + 32 * UM_EPI_WARPS;
+constexpr int UM_MAX_STAGES = 6;
 
 template <int KIND> struct KindTraits;
 template <> struct KindTraits<KIND_F16X2> {
-  static constexpr int ARRAYS = 2, STAGES = 2, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 1, FMT = 0;
-  static constexpr int EPI_WARPS = 8, SUB = 16, THREADS = 64 + 32 * EPI_WARPS, MAXREG = 192;
+  static constexpr int ARRAYS = 2, STAGES = 3, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 1, FMT = 0, SUB = 16;
 };
-template <> struct KindTraits<KIND_BF16X2> {
-  static constexpr int ARRAYS = 2, STAGES = 2, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 2, FMT = 1;
-  static constexpr int EPI_WARPS = 4, SUB = 32, THREADS = 64 + 32 * EPI_WARPS, MAXREG = 255;
+template <> struct KindTraits<KIND_HH16> {
+  static constexpr int ARRAYS = 1, STAGES = 6, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 2, FMT = 0, SUB = 32;
 };
 template <> struct KindTraits<KIND_TF32> {
-  static constexpr int ARRAYS = 1, STAGES = 4, KSTEP_ELEMS = 8, BK_ELEMS = 32, ACC_BUFS = 2, FMT = 2;
-  static constexpr int EPI_WARPS = 4, SUB = 32, THREADS = 64 + 32 * EPI_WARPS, MAXREG = 255;
+  static constexpr int ARRAYS = 1, STAGES = 6, KSTEP_ELEMS = 8, BK_ELEMS = 32, ACC_BUFS = 2, FMT = 2, SUB = 32;
 };
 
 struct UmmaParams {
-  CUtensorMap mapA;     // A-operand buffer: [ARRAYS*Np rows][Np cols], box 128B x 128 rows
+  CUtensorMap mapA;     // A-operand buffer: [ARRAYS*Np rows][Np cols], box 128 B x 128 rows
   CUtensorMap mapB;     // B-operand buffer, same box
   int np;               // padded dimension (= K)
   int macro_tiles;      // Np / 256
-  int chunk_kb;         // KIND_F16X2: k-blocks (of 64) per promoted accumulation chunk
+  int chunk_kb;         // KIND_F16X2: k-blocks (of 64) per promoted accumulation chunk (0 = whole K)
   State* st;
   StopArgs stop;        // a2 only (partials = one per CTA)
   // epilogue pointers (which are used depends on EPI / KIND; see the epilogue)
   float* f32_out;       // a1: T32 (TF32)   a2: R32   a4: Q32 (TF32)   a5: Z32 next
   const float* f32_in;  // a4: R32          a5: Z32 current
-  void* h_out;          // SPLIT16: a1: T16   a2: Rb   a4: Qb   a5: Zb next   (pairs [2][Np][Np])
-  void* h_out_t;        // SPLIT16: a5: W16 (pair, transposed)                TF32: a5: W32
+  void* h_out;          // 16-bit modes: a1: T16   a2: R16   a4: Q16   a5: Z16 next  ([ARRAYS][Np][Np])
+  void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
 };
 
 // ------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+// arrive on a barrier given by its shared::cluster address (own or peer CTA)
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
 }
 // Bounded wait: a pipeline bug traps (launch failure) instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
@@ -97,24 +118,28 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (++spins > (1ull << 26)) __trap();
   }
 }
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+// TMA load issued by one CTA of the pair into ITS shared memory; the transaction bytes are
+// counted on the barrier `bar_cluster_addr` (the leader CTA's full barrier).
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar_cluster_addr) {
   asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar)
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar_cluster_addr)
       : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+// tcgen05.commit of the pair's MMAs: arrives on the barrier at offset `bar` in BOTH CTAs.
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((uint16_t)3) : "memory");
 }
 template <int KIND>
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
+__device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
   if (KIND == KIND_TF32) {
-    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}"
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
   } else {
-    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+    asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
   }
 }
@@ -141,32 +166,28 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 __device__ __forceinline__ uint64_t make_sdesc(uint32_t saddr) {
   return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
-// kind::f16 / kind::tf32 instruction descriptor: D = F32, A/B format, both K-major, M = 128, N = 256.
+// kind::f16 / kind::tf32 instruction descriptor: D = F32, A/B format, both K-major, M = 256 (pair), N = 256.
 __host__ __device__ constexpr uint32_t make_idesc(int fmt) {
-  return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(UM_BN >> 3) << 17) | ((uint32_t)(UM_BM >> 4) << 24);
+  return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(UM_TILE >> 3) << 17) | ((uint32_t)(UM_TILE >> 4) << 24);
 }
 
 __device__ __forceinline__ uint32_t pack_h2(__half a, __half b) {
   return (uint32_t)__half_as_ushort(a) | ((uint32_t)__half_as_ushort(b) << 16);
 }
-__device__ __forceinline__ uint32_t pack_b2(__nv_bfloat16 a, __nv_bfloat16 b) {
-  return (uint32_t)__bfloat16_as_ushort(a) | ((uint32_t)__bfloat16_as_ushort(b) << 16);
-}
 
-// Write N consecutive values of one row as a 16-bit pair (hi -> base, lo -> base + plane).
-template <bool F16, int N>
-__device__ __forceinline__ void store_pair_row(void* base, size_t plane, size_t off, const float (&v)[N]) {
+// Write N consecutive values of one row in the mode's 16-bit operand format:
+// PAIR: (hi -> base, lo' -> base + plane), Eq. 17-18 with the low half scaled;  else hi = FP16[v] only.
+template <bool PAIR, int N>
+__device__ __forceinline__ void store_h_row(void* base, size_t plane, size_t off, const float (&v)[N]) {
   uint32_t hi[N / 2], lo[N / 2];
 #pragma unroll
   for (int j = 0; j < N / 2; ++j) {
-    if (F16) {
+    if (PAIR) {
       __half h0, l0, h1, l1;
       split_f16(v[2 * j], h0, l0); split_f16(v[2 * j + 1], h1, l1);
       hi[j] = pack_h2(h0, h1); lo[j] = pack_h2(l0, l1);
     } else {
-      __nv_bfloat16 h0, l0, h1, l1;
-      split_bf16(v[2 * j], h0, l0); split_bf16(v[2 * j + 1], h1, l1);
-      hi[j] = pack_b2(h0, h1); lo[j] = pack_b2(l0, l1);
+      hi[j] = pack_h2(f2h_sat(v[2 * j]), f2h_sat(v[2 * j + 1]));
     }
   }
   uint16_t* b = static_cast<uint16_t*>(base);
@@ -175,20 +196,22 @@ __device__ __forceinline__ void store_pair_row(void* base, size_t plane, size_t 
 #pragma unroll
   for (int j = 0; j < N / 8; ++j) {
     ph[j] = make_uint4(hi[4 * j], hi[4 * j + 1], hi[4 * j + 2], hi[4 * j + 3]);
-    pl[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
+    if (PAIR) pl[j] = make_uint4(lo[4 * j], lo[4 * j + 1], lo[4 * j + 2], lo[4 * j + 3]);
   }
 }
 // Transposed: value j of this lane goes to row (n + j), column m (lanes hold consecutive m).
-template <bool F16, int N>
-__device__ __forceinline__ void store_pair_col(void* base, size_t plane, size_t off_n0_m, size_t ld, const float (&v)[N]) {
+template <bool PAIR, int N>
+__device__ __forceinline__ void store_h_col(void* base, size_t plane, size_t off_n0_m, size_t ld, const float (&v)[N]) {
   uint16_t* b = static_cast<uint16_t*>(base);
 #pragma unroll
   for (int j = 0; j < N; ++j) {
-    uint16_t h, l;
-    if (F16) { __half hh, ll; split_f16(v[j], hh, ll); h = __half_as_ushort(hh); l = __half_as_ushort(ll); }
-    else { __nv_bfloat16 hh, ll; split_bf16(v[j], hh, ll); h = __bfloat16_as_ushort(hh); l = __bfloat16_as_ushort(ll); }
-    b[off_n0_m + (size_t)j * ld] = h;
-    b[plane + off_n0_m + (size_t)j * ld] = l;
+    if (PAIR) {
+      __half hh, ll; split_f16(v[j], hh, ll);
+      b[off_n0_m + (size_t)j * ld] = __half_as_ushort(hh);
+      b[plane + off_n0_m + (size_t)j * ld] = __half_as_ushort(ll);
+    } else {
+      b[off_n0_m + (size_t)j * ld] = __half_as_ushort(f2h_sat(v[j]));
+    }
   }
 }
 template <int N>
@@ -211,6 +234,7 @@ __device__ __forceinline__ void load_f32_row(const float* p, float (&v)[N]) {
 template <int KIND, int EPI, int SUB>
 __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SUB], int m, int n, bool offdiag,
                                               double& tile_sumsq) {
+  constexpr bool PAIR = (KIND == KIND_F16X2);
   const size_t ld = (size_t)p.np, plane = ld * ld;
   const size_t off = (size_t)m * ld + n;               // (m, n)
   const size_t offt = (size_t)n * ld + m;              // (n, m)
@@ -219,7 +243,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
       store_f32_row<SUB>(p.f32_out + off, v);
-    } else store_pair_row<true, SUB>(p.h_out, plane, off, v);
+    } else store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
   } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
 #pragma unroll
     for (int j = 0; j < SUB; ++j) {
@@ -227,11 +251,17 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
       tile_sumsq += (double)v[j] * (double)v[j];
     }
     store_f32_row<SUB>(p.f32_out + off, v);
-    if (KIND != KIND_TF32) store_pair_row<true, SUB>(p.h_out, plane, off, v);
+    if (KIND != KIND_TF32) store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
     if (offdiag) {
 #pragma unroll
       for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
-      if (KIND != KIND_TF32) store_pair_col<true, SUB>(p.h_out, plane, offt, ld, v);
+      if (KIND != KIND_TF32) store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
+    }
+  } else if (EPI == EPI_X3) {                           // X = Z^T H Z itself (congruence), mirror
+    store_f32_row<SUB>(p.f32_out + off, v);
+    if (offdiag) {
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
     }
   } else if (EPI == EPI_A4) {                           // Q = 1/2 R + 3/8 R R, mirror
     float r32[SUB];
@@ -247,8 +277,8 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
         for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
       }
     } else {
-      store_pair_row<true, SUB>(p.h_out, plane, off, v);
-      if (offdiag) store_pair_col<true, SUB>(p.h_out, plane, offt, ld, v);
+      store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
+      if (offdiag) store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
     }
   } else {                                              // a5: Z_next = Z + Z Q, W = Z_next^T
     float z32[SUB];
@@ -261,107 +291,109 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
       for (int j = 0; j < SUB; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
     } else {
-      store_pair_row<true, SUB>(p.h_out, plane, off, v);                // Z16 next (fp16 pair, lo scaled)
-      store_pair_col<true, SUB>(p.h_out_t, plane, offt, ld, v);         // W16 = Z16^T
+      store_h_row<PAIR, SUB>(p.h_out, plane, off, v);                // Z16 next
+      store_h_col<PAIR, SUB>(p.h_out_t, plane, offt, ld, v);         // W16 = Z16^T
     }
   }
 }
 
 // ------------------------------------------------------------------ the kernel
 template <int KIND, int EPI>
-__global__ void __launch_bounds__(KindTraits<KIND>::THREADS, 1) umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
-  if (*((volatile int*)&p.st->done)) return;       // stop decided earlier in this call
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(UM_THREADS, 1)
+umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
+  if (*((volatile int*)&p.st->done)) return;       // stop decided earlier in this call (uniform over the grid)
 
   using KT = KindTraits<KIND>;
-  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4);
+  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3);
   constexpr bool PROMOTE = (KIND == KIND_F16X2);
-  constexpr int STAGE_BYTES = KT::ARRAYS * (UM_A_BYTES + UM_B_BYTES);
-  static_assert(KT::STAGES * STAGE_BYTES <= UM_SMEM_OPERANDS, "smem");
-  constexpr int KSTEPS = KT::BK_ELEMS / KT::KSTEP_ELEMS;   // 4
+  constexpr int STAGE_BYTES = KT::ARRAYS * 2 * UM_BOX_BYTES;   // per CTA: A rows + B rows of every array
+  static_assert(KT::STAGES * STAGE_BYTES <= UM_SMEM_OPERANDS && KT::STAGES <= UM_MAX_STAGES, "smem");
+  constexpr int KSTEPS = KT::BK_ELEMS / KT::KSTEP_ELEMS;       // 4
   constexpr uint32_t IDESC = make_idesc(KT::FMT);
-  constexpr int EPI_THREADS = 32 * KT::EPI_WARPS;
-  constexpr int COLS = UM_BN / (KT::EPI_WARPS / 4);        // columns per epilogue thread
+  constexpr int COLS = UM_TILE / (UM_EPI_WARPS / 4);           // columns per epilogue thread (128)
   constexpr int SUB = KT::SUB;
 
   extern __shared__ unsigned char smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + UM_SMEM_OPERANDS;
-  // barrier slots (8 B each): full[0..3], empty[4..7], tfull[8..9], tempty[10..11], hh_full 12, hh_empty 13
+  // barrier slots (8 B each): full[0..5], empty[6..11], tfull[12..13], tempty[14..15], hh_full 16, hh_empty 17
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 32u + 8u * s; };
-  auto tfull_bar = [&](int b) { return bar_base + 64u + 8u * b; };
-  auto tempty_bar = [&](int b) { return bar_base + 80u + 8u * b; };
-  const uint32_t hh_full_bar = bar_base + 96u, hh_empty_bar = bar_base + 104u;
-  const uint32_t tmem_slot = bar_base + 112u;
+  auto empty_bar = [&](int s) { return bar_base + 48u + 8u * s; };
+  auto tfull_bar = [&](int b) { return bar_base + 96u + 8u * b; };
+  auto tempty_bar = [&](int b) { return bar_base + 112u + 8u * b; };
+  const uint32_t hh_full_bar = bar_base + 128u, hh_empty_bar = bar_base + 136u;
+  const uint32_t tmem_slot = bar_base + 144u;
   __shared__ double red[32];
   __shared__ int last_flag;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();                 // 0 = leader (issues the MMAs)
+  const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
   const int np = p.np;
   const int KB = np / KT::BK_ELEMS;
   const int CH = p.chunk_kb > 0 ? p.chunk_kb : KB;         // k-blocks per promoted chunk (KIND_F16X2)
   const int T = p.macro_tiles;
-  const int num_tiles = SYM ? T * (T + 1) : 2 * T * T;     // CTA tiles (two 128-row halves per macro tile)
+  const int num_tiles = SYM ? T * (T + 1) / 2 : T * T;     // 256 x 256 pair tiles
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < KT::ACC_BUFS; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), EPI_THREADS); }
-    mbar_init(hh_full_bar, 1); mbar_init(hh_empty_bar, EPI_THREADS);
+    for (int b = 0; b < KT::ACC_BUFS; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 2 * UM_EPI_WARPS); }
+    mbar_init(hh_full_bar, 1); mbar_init(hh_empty_bar, 2 * UM_EPI_WARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(UM_TMEM_COLS) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(UM_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   }
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();                                      // barrier inits + TMEM allocation visible to the pair
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
-    const int macro = t >> 1, h = t & 1;
     int I, J;
-    if (SYM) tri_decode(macro, I, J);
-    else band_decode(macro, T, T, 4, I, J);
-    m0 = I * 256 + h * 128;
-    n0 = J * 256;
+    if (SYM) tri_decode(t, I, J);
+    else band_decode(t, T, T, 8, I, J);
+    m0 = I * UM_TILE;
+    n0 = J * UM_TILE;
     offdiag = (I != J);
   };
 
   double cta_sumsq = 0.0;
 
   if (warp == 0) {
-    // ===================================================== TMA producer
+    // ===================================================== TMA producer (both CTAs)
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+      const int roff = (int)rank * UM_ROWS;
+      for (int t = pair; t < num_tiles; t += num_pairs) {
         int m0, n0; bool od; decode(t, m0, n0, od);
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1u);
-          mbar_expect_tx(full_bar(stage), STAGE_BYTES);
+          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * STAGE_BYTES);     // both CTAs' boxes
+          const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
           const int kc = kb * KT::BK_ELEMS;
 #pragma unroll
           for (int a = 0; a < KT::ARRAYS; ++a) {
-            tma_load_2d(sa + a * UM_A_BYTES, &p.mapA, kc, a * np + m0, full_bar(stage));
-            const uint32_t sb = sa + KT::ARRAYS * UM_A_BYTES + a * UM_B_BYTES;
-            tma_load_2d(sb, &p.mapB, kc, a * np + n0, full_bar(stage));
-            tma_load_2d(sb + UM_A_BYTES, &p.mapB, kc, a * np + n0 + 128, full_bar(stage));
+            tma_load_2d_pair(sa + a * UM_BOX_BYTES, &p.mapA, kc, a * np + m0 + roff, lead_full);
+            tma_load_2d_pair(sa + (KT::ARRAYS + a) * UM_BOX_BYTES, &p.mapB, kc, a * np + n0 + roff, lead_full);
           }
           if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================================================== MMA issuer
-    if (lane == 0) {
+    // ===================================================== MMA issuer (leader CTA, one lane)
+    if (rank == 0 && lane == 0) {
       int stage = 0; uint32_t phase = 0;
       int buf = 0; uint32_t accphase = 0;
       uint32_t chunks = 0;                                     // promoted chunks committed so far (all tiles)
-      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+      for (int t = pair; t < num_tiles; t += num_pairs) {
         mbar_wait(tempty_bar(buf), accphase ^ 1u);
         tc_fence_after();
         const uint32_t d0 = tmem_base + (KT::ACC_BUFS == 2 ? buf * 256 : 0);   // D (or D_hh chunk)
@@ -371,56 +403,57 @@ __global__ void __launch_bounds__(KindTraits<KIND>::THREADS, 1) umma_gemm_kernel
           tc_fence_after();
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
           const uint64_t a_hi = make_sdesc(sa);
-          const uint64_t a_lo = make_sdesc(sa + UM_A_BYTES);
-          const uint64_t b_hi = make_sdesc(sa + KT::ARRAYS * UM_A_BYTES);
-          const uint64_t b_lo = make_sdesc(sa + KT::ARRAYS * UM_A_BYTES + UM_B_BYTES);
+          const uint64_t a_lo = make_sdesc(sa + UM_BOX_BYTES);
+          const uint64_t b_hi = make_sdesc(sa + KT::ARRAYS * UM_BOX_BYTES);
+          const uint64_t b_lo = make_sdesc(sa + (KT::ARRAYS + 1) * UM_BOX_BYTES);
           if (PROMOTE) {
-            // (h)(h) products first, into the chunk accumulator D_hh; the epilogue warps add every
-            // finished chunk to FP32 registers with round-to-nearest while the 2^11-scaled cross
-            // products of this k-block run on the tensor core.
+            // The (h)(h) products accumulate in D_hh for CH k-blocks at a time; the epilogue warps of both
+            // CTAs add every finished chunk to FP32 registers with round-to-nearest (DESIGN.md "promoted
+            // accumulation").  Issue order hides that drain behind tensor work: the chunk's last k-block
+            // issues (h)(h) first and its 2^11-scaled cross products after the commit, the next chunk's
+            // first k-block issues its cross products BEFORE waiting for the drained accumulator.
             const int kc = kb % CH;
-            if (kc == 0 && chunks > 0) { mbar_wait(hh_empty_bar, (chunks - 1u) & 1u); tc_fence_after(); }
+            const bool first = (kc == 0), last = (kc == CH - 1 || kb == KB - 1);
+            auto issue_cross = [&]() {
+#pragma unroll
+              for (int k = 0; k < KSTEPS; ++k) {
+                const uint64_t ko = (uint64_t)(k * 2);
+                tc_mma_pair<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, (kb | k) ? 1u : 0u);
+                tc_mma_pair<KIND>(d1, a_lo + ko, b_hi + ko, IDESC, 1u);
+              }
+            };
+            if (first) {
+              issue_cross();
+              if (chunks > 0) { mbar_wait(hh_empty_bar, (chunks - 1u) & 1u); tc_fence_after(); }
+            }
 #pragma unroll
             for (int k = 0; k < KSTEPS; ++k)
-              tc_mma<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (kc | k) ? 1u : 0u);
-            if (kc == CH - 1 || kb == KB - 1) { tc_commit(hh_full_bar); ++chunks; }
-#pragma unroll
-            for (int k = 0; k < KSTEPS; ++k) {
-              const uint64_t ko = (uint64_t)(k * 2);
-              tc_mma<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, (kb | k) ? 1u : 0u);
-              tc_mma<KIND>(d1, a_lo + ko, b_hi + ko, IDESC, 1u);
-            }
+              tc_mma_pair<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (kc | k) ? 1u : 0u);
+            if (last) { tc_commit_pair(hh_full_bar); ++chunks; }
+            if (!first) issue_cross();
           } else {
 #pragma unroll
-            for (int k = 0; k < KSTEPS; ++k) {
-              const uint32_t acc = (kb | k) ? 1u : 0u;
-              const uint64_t ko = (uint64_t)(k * 2);            // 32 bytes per k-step, in 16-byte units
-              if (KIND == KIND_BF16X2) {
-                tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
-                tc_mma<KIND>(d0, a_hi + ko, b_lo + ko, IDESC, 1u);
-                tc_mma<KIND>(d0, a_lo + ko, b_hi + ko, IDESC, 1u);
-              } else {
-                tc_mma<KIND>(d0, a_hi + ko, b_hi + ko, IDESC, acc);
-              }
-            }
+            for (int k = 0; k < KSTEPS; ++k)                   // 32 bytes per k-step, in 16-byte units
+              tc_mma_pair<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (kb | k) ? 1u : 0u);
           }
-          tc_commit(empty_bar(stage));                         // frees the smem stage when the MMAs retire
+          tc_commit_pair(empty_bar(stage));                    // frees the smem stage in both CTAs when the MMAs retire
           if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
         }
-        tc_commit(tfull_bar(buf));                             // accumulator(s) complete
+        tc_commit_pair(tfull_bar(buf));                        // accumulator(s) complete, both CTAs
         if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
         else accphase ^= 1u;
       }
     }
   } else {
-    // ===================================================== epilogue warps (2 .. 2+EPI_WARPS-1)
+    // ===================================================== epilogue warps (2 .. 9), both CTAs
     const int q = warp & 3;                                    // TMEM lane quarter this warp may read
-    const int g = (warp - 2) >> 2;                             // column group of this warp
-    const int row = q * 32 + lane;
+    const int g = (warp - 2) >> 2;                             // column half of this warp
+    const int row = (int)rank * UM_ROWS + q * 32 + lane;       // row of the pair tile held by this thread
+    const uint32_t lead_hh_empty = mapa_u32(hh_empty_bar, 0);
     int buf = 0; uint32_t accphase = 0;
     uint32_t chunks = 0;
     const int nch = (KB + CH - 1) / CH;
-    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+    for (int t = pair; t < num_tiles; t += num_pairs) {
       int m0, n0; bool offdiag; decode(t, m0, n0, offdiag);
       const int m = m0 + row;
       const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (KT::ACC_BUFS == 2 ? buf * 256 : 0) + g * COLS;
@@ -441,7 +474,8 @@ __global__ void __launch_bounds__(KindTraits<KIND>::THREADS, 1) umma_gemm_kernel
             for (int j = 0; j < 32; ++j) sum[i * 32 + j] += __uint_as_float(r[j]);
           }
           tc_fence_before();
-          mbar_arrive(hh_empty_bar);
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(lead_hh_empty);
           ++chunks;
         }
         mbar_wait(tfull_bar(0), accphase);
@@ -475,7 +509,8 @@ __global__ void __launch_bounds__(KindTraits<KIND>::THREADS, 1) umma_gemm_kernel
         }
       }
       tc_fence_before();
-      mbar_arrive(tempty_bar(buf));                            // EPI_THREADS arrivals free the accumulator
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty_bar(buf), 0));   // 2 x 8 warp arrivals free the accumulator
       if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
       if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
       else accphase ^= 1u;
@@ -489,15 +524,15 @@ __global__ void __launch_bounds__(KindTraits<KIND>::THREADS, 1) umma_gemm_kernel
   }
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();                                      // no MMA / remote arrive of the pair is in flight any more
   if (warp == 1) {
-    __syncwarp();
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
   }
   if (EPI == EPI_A2) {
     if (threadIdx.x == 0) {
       double tot = 0.0;
-      for (int w = 2; w < 2 + KT::EPI_WARPS; ++w) tot += red[w];
+      for (int w = 2; w < 2 + UM_EPI_WARPS; ++w) tot += red[w];
       p.stop.partials[blockIdx.x] = tot;
     }
     if (arrive_is_last(&p.st->arrive[0], gridDim.x, &last_flag)) stop_test_last_cta(p.stop, red);
@@ -512,7 +547,7 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 struct UmmaPlan {
   Layout L;
   char* ws = nullptr;
-  int grid = 0;
+  int max_pairs = 0;  // CTA pairs that are co-resident on the device (74 on a B200)
   int mode = 0;
   int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
   // tensor maps of every operand buffer (box 128 B x 128 rows, 128B swizzle)
@@ -523,7 +558,7 @@ inline cudaError_t make_map(PFN_encodeTiled enc, CUtensorMap* m, void* base, CUt
                             uint64_t rows, uint64_t cols) {
   cuuint64_t gdim[2] = {cols, rows};
   cuuint64_t gstr[1] = {cols * elt};
-  cuuint32_t box[2] = {(cuuint32_t)(UM_ROWB / elt), 128u};
+  cuuint32_t box[2] = {(cuuint32_t)(UM_ROWB / elt), (cuuint32_t)UM_ROWS};
   cuuint32_t estr[2] = {1u, 1u};
   CUresult r = enc(m, dt, 2, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -531,24 +566,37 @@ inline cudaError_t make_map(PFN_encodeTiled enc, CUtensorMap* m, void* base, CUt
 }
 
 template <int KIND, int EPI>
-inline cudaError_t set_smem_attr() {
+inline cudaError_t prepare_kernel(int* max_pairs) {
   cudaError_t e = cudaFuncSetAttribute(umma_gemm_kernel<KIND, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
   if (e != cudaSuccess) return e;
-  int nb = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, umma_gemm_kernel<KIND, EPI>, KindTraits<KIND>::THREADS, UM_SMEM_BYTES);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(2 * 148); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES;
+  int nc = 0;
+  e = cudaOccupancyMaxActiveClusters(&nc, umma_gemm_kernel<KIND, EPI>, &cfg);
   if (e != cudaSuccess) return e;
-  if (nb < 1) {
+  if (nc < 1) {
     cudaFuncAttributes fa;
     cudaFuncGetAttributes(&fa, umma_gemm_kernel<KIND, EPI>);
-    fprintf(stderr, "zfac: kernel<%d,%d> does not fit an SM: regs=%d threads=%d static smem=%zu dyn smem=%d maxThreadsPerBlock=%d\n",
-            KIND, EPI, fa.numRegs, KindTraits<KIND>::THREADS, fa.sharedSizeBytes, UM_SMEM_BYTES, fa.maxThreadsPerBlock);
+    fprintf(stderr, "zfac: kernel<%d,%d> does not fit an SM pair: regs=%d threads=%d static smem=%zu dyn smem=%d\n",
+            KIND, EPI, fa.numRegs, UM_THREADS, fa.sharedSizeBytes, UM_SMEM_BYTES);
     return cudaErrorLaunchOutOfResources;
   }
+  if (*max_pairs == 0 || nc < *max_pairs) *max_pairs = nc;
   return cudaSuccess;
 }
 
+template <int KIND>
+inline cudaError_t prepare_kind(int* max_pairs) {
+  cudaError_t e;
+  if ((e = prepare_kernel<KIND, EPI_A1>(max_pairs)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_A2>(max_pairs)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_X3>(max_pairs)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_A4>(max_pairs)) != cudaSuccess) return e;
+  return prepare_kernel<KIND, EPI_A5>(max_pairs);
+}
+
 inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int sm_count) {
-  pl->L = L; pl->ws = ws; pl->grid = sm_count; pl->mode = L.mode;
+  pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0;
   if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knob
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -557,19 +605,18 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
   PFN_encodeTiled enc = reinterpret_cast<PFN_encodeTiled>(fn);
   const uint64_t np = (uint64_t)L.np;
-  if (L.mode == ZFAC_MODE_SPLIT16) {
+  if (L.mode == ZFAC_MODE_SPLIT16 || L.mode == ZFAC_MODE_HH16) {
     const CUtensorMapDataType H = CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
-    if ((e = make_map(enc, &pl->mS, ws + L.off_S, H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mW, ws + L.off_W, H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mT, ws + L.off_T, H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mR, ws + L.off_Rb, H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mQ, ws + L.off_Qb, H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Zb[0], H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], H, 2, 2 * np, np)) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_F16X2, EPI_A1>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_F16X2, EPI_A2>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_F16X2, EPI_A4>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_F16X2, EPI_A5>()) != cudaSuccess) return e;
+    const uint64_t rows = (L.mode == ZFAC_MODE_SPLIT16 ? 2 : 1) * np;
+    if ((e = make_map(enc, &pl->mS, ws + L.off_S, H, 2, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mW, ws + L.off_W, H, 2, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mT, ws + L.off_T, H, 2, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mR, ws + L.off_Rb, H, 2, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mQ, ws + L.off_Qb, H, 2, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Zb[0], H, 2, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], H, 2, rows, np)) != cudaSuccess) return e;
+    e = (L.mode == ZFAC_MODE_SPLIT16) ? prepare_kind<KIND_F16X2>(&pl->max_pairs) : prepare_kind<KIND_HH16>(&pl->max_pairs);
+    if (e != cudaSuccess) return e;
   } else {
     const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     if ((e = make_map(enc, &pl->mS, ws + L.off_S, F, 4, np, np)) != cudaSuccess) return e;
@@ -579,69 +626,101 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = make_map(enc, &pl->mQ, ws + L.off_Q, F, 4, np, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Z[0], F, 4, np, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Z[1], F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_TF32, EPI_A1>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_TF32, EPI_A2>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_TF32, EPI_A4>()) != cudaSuccess) return e;
-    if ((e = set_smem_attr<KIND_TF32, EPI_A5>()) != cudaSuccess) return e;
+    if ((e = prepare_kind<KIND_TF32>(&pl->max_pairs)) != cudaSuccess) return e;
   }
+  if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
   return cudaSuccess;
+}
+
+template <int KIND>
+inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) {
+  switch (epi) {
+    case EPI_A1: umma_gemm_kernel<KIND, EPI_A1><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    case EPI_A2: umma_gemm_kernel<KIND, EPI_A2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    case EPI_X3: umma_gemm_kernel<KIND, EPI_X3><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    case EPI_A4: umma_gemm_kernel<KIND, EPI_A4><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    default:     umma_gemm_kernel<KIND, EPI_A5><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+  }
+}
+inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const UmmaParams& p) {
+  if (mode == ZFAC_MODE_SPLIT16) umma_launch<KIND_F16X2>(epi, grid, s, p);
+  else if (mode == ZFAC_MODE_HH16) umma_launch<KIND_HH16>(epi, grid, s, p);
+  else umma_launch<KIND_TF32>(epi, grid, s, p);
 }
 
 inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, double* d_err, cudaStream_t s, int* launches, Prof* prof) {
   const Layout& L = pl.L;
   char* ws = pl.ws;
-  const int T = (int)(L.np / 256);
-  const int full_tiles = 2 * T * T, sym_tiles = T * (T + 1);
-  const int grid_full = full_tiles < pl.grid ? full_tiles : pl.grid;
-  const int grid_sym = sym_tiles < pl.grid ? sym_tiles : pl.grid;
+  const int T = (int)(L.np / UM_TILE);
+  const int full_tiles = T * T, sym_tiles = T * (T + 1) / 2;
+  const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
+  const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T; p.chunk_kb = pl.chunk_kb;
+  p.np = (int)L.np; p.macro_tiles = T;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
   p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
   float* R32 = reinterpret_cast<float*>(ws + L.off_R);
-  const bool split = (L.mode == ZFAC_MODE_SPLIT16);
+  const bool h16 = (L.mode != ZFAC_MODE_TF32);
   int nl = 0;
   for (int n = 0; n <= max_iter; ++n) {
-    // a1: T = W S^T
+    // a1: T = W S^T            (promoted accumulation: T and X are O(1) quantities)
     prof->mark(s, EPI_A1 + 16 * n);
+    p.chunk_kb = pl.chunk_kb;
     p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
-    if (split) { p.f32_out = nullptr; p.h_out = ws + L.off_T;
-      umma_gemm_kernel<KIND_F16X2, EPI_A1><<<grid_full, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
-    } else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr;
-      umma_gemm_kernel<KIND_TF32, EPI_A1><<<grid_full, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p); }
+    if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; }
+    else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; }
+    umma_launch_mode(L.mode, EPI_A1, grid_full, s, p);
     // a2: R = I - W T^T
     prof->mark(s, EPI_A2 + 16 * n);
     p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n;
-    if (split) { p.h_out = ws + L.off_Rb;
-      umma_gemm_kernel<KIND_F16X2, EPI_A2><<<grid_sym, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
-    } else { p.h_out = nullptr;
-      umma_gemm_kernel<KIND_TF32, EPI_A2><<<grid_sym, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p); }
+    p.h_out = h16 ? ws + L.off_Rb : nullptr;
+    umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
     nl += 2;
     if (n == max_iter) break;
-    // a4: Q = 1/2 R + 3/8 R R^T
+    // a4: Q = 1/2 R + 3/8 R R^T   (the product is a correction of size |R|^2: no promotion needed)
     prof->mark(s, EPI_A4 + 16 * n);
+    p.chunk_kb = 0;
     p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
-    if (split) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb;
-      umma_gemm_kernel<KIND_F16X2, EPI_A4><<<grid_sym, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
-    } else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr;
-      umma_gemm_kernel<KIND_TF32, EPI_A4><<<grid_sym, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p); }
+    if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
+    else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr; }
+    umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p);
     // a5: Z_next = Z + Z Q^T ; W = Z_next^T
     prof->mark(s, EPI_A5 + 16 * n);
     p.mapA = pl.mZ[n & 1]; p.mapB = pl.mQ;
-    if (split) {
+    if (h16) {
       float* Z32 = reinterpret_cast<float*>(ws + L.off_Z[0]);       // FP32 master copy, updated in place
       p.f32_in = Z32; p.f32_out = Z32; p.h_out = ws + L.off_Zb[(n + 1) & 1]; p.h_out_t = ws + L.off_W;
-      umma_gemm_kernel<KIND_F16X2, EPI_A5><<<grid_full, KindTraits<KIND_F16X2>::THREADS, UM_SMEM_BYTES, s>>>(p);
     } else {
       p.f32_in = reinterpret_cast<float*>(ws + L.off_Z[n & 1]);
       p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(n + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
-      umma_gemm_kernel<KIND_TF32, EPI_A5><<<grid_full, KindTraits<KIND_TF32>::THREADS, UM_SMEM_BYTES, s>>>(p);
     }
+    umma_launch_mode(L.mode, EPI_A5, grid_full, s, p);
     nl += 2;
   }
   prof->mark(s, 0);
   *launches = nl;
+  return cudaGetLastError();
+}
+
+// Congruence H_perp = Z^T H Z (Eq. 11) with H in the S buffer: T = W H^T, X = W T^T -> R32 buffer.
+inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* launches) {
+  const Layout& L = pl.L;
+  char* ws = pl.ws;
+  const int T = (int)(L.np / UM_TILE);
+  const int full_tiles = T * T, sym_tiles = T * (T + 1) / 2;
+  const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
+  const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
+  UmmaParams p{};
+  p.np = (int)L.np; p.macro_tiles = T; p.chunk_kb = pl.chunk_kb;
+  p.st = reinterpret_cast<State*>(ws + L.off_state);
+  const bool h16 = (L.mode != ZFAC_MODE_TF32);
+  p.mapA = pl.mW; p.mapB = pl.mS;
+  if (h16) p.h_out = ws + L.off_T; else p.f32_out = reinterpret_cast<float*>(ws + L.off_T);
+  umma_launch_mode(L.mode, EPI_A1, grid_full, s, p);
+  p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = reinterpret_cast<float*>(ws + L.off_R); p.h_out = nullptr;
+  umma_launch_mode(L.mode, EPI_X3, grid_sym, s, p);
+  *launches = 2;
   return cudaGetLastError();
 }
 

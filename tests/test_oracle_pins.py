@@ -282,3 +282,22 @@ def test_refi_reaches_fp64_floor():
     before = O.final_residual_per_sqrt_n(w.S, low.Z)
     after = O.final_residual_per_sqrt_n(w.S, res.Z)
     assert after < 1e-11 and after < before * 1e-3
+
+
+def test_congruence_reproduces_generalized_eigenvalues():
+    """PAPER.md Eq. 11 (lines 88-92): with Z^T S Z = I the eigenvalues of H_perp = Z^T H Z are the
+    generalized eigenvalues of H C = S C eps.  Pinned with scipy's generalized symmetric solver;
+    a transposed operand (Z H Z^T) or a dropped factor fails for the non-symmetric Z used here."""
+    import scipy.linalg
+    w = W.random_spd_general(40, seed=21, kappa=50.0, pert=0.2)
+    res = O.refine(w.S, w.Z0, 30, O.STOP_PAPER)
+    assert not np.allclose(res.Z, res.Z.T)
+    rng = np.random.default_rng(5)
+    H = rng.standard_normal((40, 40)); H = 0.5 * (H + H.T)
+    Hp = O.congruence(H, res.Z)
+    assert np.allclose(Hp, Hp.T, atol=1e-12)
+    ev = np.linalg.eigvalsh(0.5 * (Hp + Hp.T))
+    ref = scipy.linalg.eigh(H, w.S, eigvals_only=True)
+    assert np.allclose(ev, ref, rtol=1e-9, atol=1e-9)
+    wrong = res.Z @ H @ res.Z.T
+    assert not np.allclose(np.linalg.eigvalsh(0.5 * (wrong + wrong.T)), ref, rtol=1e-6, atol=1e-6)
