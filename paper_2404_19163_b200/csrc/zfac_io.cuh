@@ -49,7 +49,7 @@ struct Layout {
   int64_t n = 0, np = 0;
   int mode = 0;
   size_t elt = 0;  // user element size
-  size_t off_state = 0, off_partials = 0, num_partials = 0;
+  size_t off_state = 0, off_dbg = 0, off_partials = 0, num_partials = 0;
   size_t off_stage_S = 0, off_stage_Z = 0, off_stage_out = 0;
   // F64 / TF32: one buffer each of the mode's element type; Z double-buffered
   size_t off_S = 0, off_W = 0, off_T = 0, off_R = 0, off_Q = 0, off_Z[2] = {0, 0};
@@ -70,6 +70,7 @@ inline Layout make_layout(int64_t n, int mode) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 1023) / 1024 * 1024; return o; };
   L.off_state = take(sizeof(State));
+  L.off_dbg = take(8 * 148 * 4 * sizeof(unsigned long long));   // -DZFAC_TIMING counters (at a fixed offset: 1024)
   L.num_partials = (size_t)(L.np / 128) * (size_t)(L.np / 128);
   L.off_partials = take(L.num_partials * sizeof(double));
   L.off_stage_S = take(n2 * L.elt);

@@ -74,6 +74,7 @@ struct UmmaParams {
   const float* f32_in;  // a4: R32          a5: Z32 current
   void* h_out;          // 16-bit modes: a1: T16   a2: R16   a4: Q16   a5: Z16 next  ([ARRAYS][Np][Np])
   void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
+  unsigned long long* dbg;  // -DZFAC_TIMING builds only: per-CTA wait-cycle counters of the MMA issuer (else null)
 };
 
 // ------------------------------------------------------------------ PTX wrappers
@@ -100,9 +101,13 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// arrive on a barrier given by its shared::cluster address (own or peer CTA)
+// Arrive on a barrier given by its shared::cluster address (own or peer CTA).  RELAXED: the arrivals of the
+// epilogue warps only tell the MMA issuer that their tcgen05.ld of an accumulator have completed (the values are
+// in registers after tcgen05.wait::ld; tcgen05.fence::before/after_thread_sync order the tensor-memory accesses).
+// No generic-proxy data is published, and a .release.cluster arrive costs a GPU-scope fence
+// (MEMBAR.ALL.GPU + ERRBAR + CGAERRBAR, profiles/r1a_summary.md) on the critical path of every chunk drain.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
 }
 // Bounded wait: a pipeline bug traps (launch failure) instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
@@ -297,6 +302,14 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
   }
 }
 
+// -DZFAC_TIMING: the MMA issuer thread accumulates the cycles it spends in each kind of wait
+// (0 smem-full = TMA starvation, 1 hh_empty = chunk drain, 2 tempty = epilogue, 3 whole role loop).
+#ifdef ZFAC_TIMING
+#define ZF_TWAIT(i, stmt) do { const long long t0_ = clock64(); stmt; twait[i] += clock64() - t0_; } while (0)
+#else
+#define ZF_TWAIT(i, stmt) do { stmt; } while (0)
+#endif
+
 // ------------------------------------------------------------------ the kernel
 template <int KIND, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(UM_THREADS, 1)
@@ -393,13 +406,17 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       int stage = 0; uint32_t phase = 0;
       int buf = 0; uint32_t accphase = 0;
       uint32_t chunks = 0;                                     // promoted chunks committed so far (all tiles)
+#ifdef ZFAC_TIMING
+      long long twait[4] = {0, 0, 0, 0};
+      const long long tstart = clock64();
+#endif
       for (int t = pair; t < num_tiles; t += num_pairs) {
-        mbar_wait(tempty_bar(buf), accphase ^ 1u);
+        ZF_TWAIT(2, mbar_wait(tempty_bar(buf), accphase ^ 1u));
         tc_fence_after();
         const uint32_t d0 = tmem_base + (KT::ACC_BUFS == 2 ? buf * 256 : 0);   // D (or D_hh chunk)
         const uint32_t d1 = tmem_base + 256;                                     // D_x (KIND_F16X2 only)
         for (int kb = 0; kb < KB; ++kb) {
-          mbar_wait(full_bar(stage), phase);
+          ZF_TWAIT(0, mbar_wait(full_bar(stage), phase));
           tc_fence_after();
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
           const uint64_t a_hi = make_sdesc(sa);
@@ -424,7 +441,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
             };
             if (first) {
               issue_cross();
-              if (chunks > 0) { mbar_wait(hh_empty_bar, (chunks - 1u) & 1u); tc_fence_after(); }
+              if (chunks > 0) { ZF_TWAIT(1, mbar_wait(hh_empty_bar, (chunks - 1u) & 1u)); tc_fence_after(); }
             }
 #pragma unroll
             for (int k = 0; k < KSTEPS; ++k)
@@ -443,6 +460,12 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
         if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
         else accphase ^= 1u;
       }
+#ifdef ZFAC_TIMING
+      if (p.dbg) {
+        twait[3] = clock64() - tstart;
+        for (int i = 0; i < 4; ++i) atomicAdd(p.dbg + (size_t)(EPI * 148 + pair) * 4 + i, (unsigned long long)twait[i]);
+      }
+#endif
     }
   } else {
     // ===================================================== epilogue warps (2 .. 9), both CTAs
@@ -658,6 +681,9 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
   UmmaParams p{};
   p.np = (int)L.np; p.macro_tiles = T;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
+#ifdef ZFAC_TIMING
+  p.dbg = reinterpret_cast<unsigned long long*>(ws + L.off_dbg);
+#endif
   p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
   float* R32 = reinterpret_cast<float*>(ws + L.off_R);
