@@ -210,9 +210,18 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
   co.Zbuf[0] = b0; co.Zbuf[1] = b1; co.parity = parity;
   co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np;
   co.st = reinterpret_cast<State*>(c->ws + L.off_state); co.d_iters = d_iters; co.d_flags = d_flags;
-  dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
-  if (c->mode == ZFAC_MODE_F64) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
-  else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
+  const int elt = (int)L.elt;
+  const bool vec16 = ((size_t)c->n * elt) % 16 == 0 && ((size_t)ldz * elt) % 16 == 0 && ((size_t)L.np * elt) % 16 == 0 &&
+                     (reinterpret_cast<uintptr_t>(d_Z) & 15u) == 0 && (reinterpret_cast<uintptr_t>(b0) & 15u) == 0 &&
+                     (reinterpret_cast<uintptr_t>(b1) & 15u) == 0;
+  if (vec16) {
+    dim3 gv((unsigned)(((size_t)c->n * elt / 16 + 255) / 256), (unsigned)((c->n + 7) / 8));
+    copy_out_vec16_kernel<<<gv, 256, 0, s>>>(co, elt);
+  } else {
+    dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
+    if (c->mode == ZFAC_MODE_F64) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
+    else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
+  }
   c->launches += 1;
 }
 

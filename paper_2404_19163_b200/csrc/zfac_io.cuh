@@ -70,7 +70,7 @@ inline Layout make_layout(int64_t n, int mode) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 1023) / 1024 * 1024; return o; };
   L.off_state = take(sizeof(State));
-  L.off_dbg = take(8 * 148 * 4 * sizeof(unsigned long long));   // -DZFAC_TIMING counters (at a fixed offset: 1024)
+  L.off_dbg = take(8 * 148 * 8 * sizeof(unsigned long long));   // -DZFAC_TIMING counters (at a fixed offset: 1024)
   L.num_partials = (size_t)(L.np / 128) * (size_t)(L.np / 128);
   L.off_partials = take(L.num_partials * sizeof(double));
   L.off_stage_S = take(n2 * L.elt);
@@ -190,6 +190,26 @@ __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
     const int r = r0 + i;
     if (r < a.n) dst[(size_t)r * a.ldz + c] = src[(size_t)r * a.np + c];
   }
+}
+
+// 16-byte-vector variant for the aligned case (N * sizeof(T), both pitches and both base pointers multiples of
+// 16 bytes): one uint4 per thread and row, 8 rows per block row.
+__global__ void __launch_bounds__(256) copy_out_vec16_kernel(const CopyOutArgs a, int elt) {
+  const int iters = a.st->iters;
+  if (a.d_iters && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { *a.d_iters = iters; *a.d_flags = a.st->flags; }
+  const char* src = static_cast<const char*>(a.Zbuf[a.parity >= 0 ? a.parity : (iters & 1)]);
+  char* dst = static_cast<char*>(a.Z);
+  const size_t row_bytes = (size_t)a.n * elt, spitch = (size_t)a.np * elt, dpitch = (size_t)a.ldz * elt;
+  const size_t cb = ((size_t)blockIdx.x * 256 + threadIdx.x) * 16;
+  if (cb >= row_bytes) return;
+  const int r0 = blockIdx.y * 8;
+  uint4 v[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i)
+    if (r0 + i < a.n) v[i] = *reinterpret_cast<const uint4*>(src + (size_t)(r0 + i) * spitch + cb);
+#pragma unroll
+  for (int i = 0; i < 8; ++i)
+    if (r0 + i < a.n) *reinterpret_cast<uint4*>(dst + (size_t)(r0 + i) * dpitch + cb) = v[i];
 }
 
 // ------------------------------------------------------------------ Alg. 3 bookkeeping

@@ -6,26 +6,29 @@
 //   a1  T = (S Z)^T = W S^T    (Eq. 22)     a2  X = Z^T (S Z) = W T^T   (Eq. 26)
 //   a4  P = R R = R R^T        (Eq. 30-32)  a5  Z Q = Z Q^T             (Eq. 13)
 //
-// CTA pair (cluster of 2, tcgen05 cta_group::2): one 256 x 256 output tile per pair.  CTA r of
-// the pair stages rows [128 r, 128 r + 128) of the A tile and of the B tile (TMA, 128B-swizzle
-// boxes of 128 rows x 128 B, landing on the LEADER's full barrier), the leader's elected thread
-// issues tcgen05.mma with M = 256, N = 256 reading both CTAs' shared memory, and each CTA's
-// TMEM (128 lanes x 512 columns) receives rows [128 r, 128 r + 128) of the accumulators.
+// CTA pair (cluster of 2, tcgen05 cta_group::2): one 256 x TILE_N output tile per pair.  CTA r of
+// the pair stages rows [128 r, 128 r + 128) of the A tile and rows [TILE_N/2 r, ...) of the B tile
+// (TMA, 128B-swizzle boxes of 64 rows x 128 B, landing on the LEADER's full barrier), the leader's
+// elected thread issues tcgen05.mma with M = 256, N = TILE_N reading both CTAs' shared memory, and
+// each CTA's TMEM (128 lanes x 512 columns) receives rows [128 r, 128 r + 128) of the accumulators.
 //
 // Roles per CTA (64 + 256 threads): warp 0 = TMA producer (one lane), warp 1 = TMEM allocator +
-// (leader only) MMA issuer, warps 2-9 = epilogue (tcgen05.ld, fused O(N^2) work, stores).
+// (leader only) MMA issuer, warps 2-9 = two epilogue groups of 4 warps (tcgen05.ld, fused O(N^2)
+// work, stores).  TMEM holds TWO accumulator sets; tile i of a pair uses set i mod 2 and epilogue
+// group i mod 2, so the epilogue of a tile always overlaps the mainloop of the next one.
 // Pipelines: shared-memory ring full/empty mbarriers (TMA <-> MMA; "empty" is multicast to both
-// CTAs by tcgen05.commit) and TMEM full/empty mbarriers (MMA <-> the epilogue warps of both CTAs).
+// CTAs by tcgen05.commit) and, per accumulator set, TMEM full/empty mbarriers (MMA <-> that set's
+// epilogue group in both CTAs) plus the D_hh chunk hand-over barriers of the promoted accumulation.
 //
 // Precision kinds
 //   KIND_F16X2 (SPLIT16 mode): operands are fp16 pairs (hi, lo' = lo * 2^11), Eq. 17-18.
 //       Three MMA passes per k-step, (l)(l) dropped (Eq. 25, 29, 32):
 //           D_hh += A_hi B_hi          D_x += A_hi B_lo' + A_lo' B_hi
-//       two FP32 accumulators (256 TMEM columns each); the epilogue forms D_hh + 2^-11 D_x.
-//       D_hh is drained into FP32 registers every chunk_kb k-blocks (promoted accumulation).
-//   KIND_HH16  (HH16 mode, the paper's (h)(h) scheme, Sec. III.C): fp16 operands, one pass,
-//       two accumulator buffers so that the epilogue overlaps the next tile.
-//   KIND_TF32  (TF32 mode): FP32 operands read as TF32, one pass, two accumulator buffers.
+//       two FP32 accumulators per set, hence TILE_N = 128 (2 sets x 2 x 128 = 512 TMEM columns); the
+//       epilogue forms D_hh + 2^-11 D_x.  D_hh is drained into FP32 registers every chunk_kb
+//       k-blocks (promoted accumulation).
+//   KIND_HH16  (HH16 mode, the paper's (h)(h) scheme, Sec. III.C): fp16 operands, one pass, TILE_N = 256.
+//   KIND_TF32  (TF32 mode): FP32 operands read as TF32, one pass, TILE_N = 256.
 #pragma once
 #include <cuda.h>
 #include <stdio.h>
@@ -39,34 +42,45 @@ namespace zfac {
 
 enum { KIND_F16X2 = 0, KIND_HH16 = 1, KIND_TF32 = 2 };
 
-constexpr int UM_TILE = 256;                     // pair tile (M and N)
-constexpr int UM_ROWS = 128;                     // operand rows staged per CTA (of A and of B)
+constexpr int UM_TILE_M = 256;                   // pair tile rows: two CTAs x 128 TMEM lanes
+constexpr int UM_MACRO = 256;                    // padding unit and macro tile of the symmetric enumeration
+constexpr int UM_ROWS = 128;                     // A-operand rows staged per CTA
 constexpr int UM_ROWB = 128;                     // bytes per operand row per k-block (= swizzle span)
-constexpr int UM_BOX_BYTES = UM_ROWS * UM_ROWB;  // 16 KB: one TMA box
+constexpr int UM_BOX_ROWS = 64;                  // rows per TMA box
+constexpr int UM_BOX_BYTES = UM_BOX_ROWS * UM_ROWB;  // 8 KB
+constexpr int UM_A_BYTES = UM_ROWS * UM_ROWB;    // 16 KB: A rows of one array, one stage, one CTA
 constexpr int UM_SMEM_OPERANDS = 192 * 1024;
 constexpr int UM_SMEM_BYTES = UM_SMEM_OPERANDS + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int UM_TMEM_COLS = 512;
-constexpr int UM_EPI_WARPS = 8;
+constexpr int UM_EPI_WARPS = 8;                  // two groups of 4 (one warp per TMEM lane quarter), alternating tiles
 constexpr int UM_THREADS = 64 + 32 * UM_EPI_WARPS;
 constexpr int UM_MAX_STAGES = 6;
 
+// TILE_N: columns of the pair tile (= N of one tcgen05.mma; each CTA stages TILE_N / 2 rows of B).
+// SETS: accumulator sets in the 512 TMEM columns.  The one-pass kinds keep two (the epilogue of tile i overlaps
+// the mainloop of tile i + 1, epilogue group i mod 2).  F16X2 needs two FP32 accumulators (D_hh, D_x) per set:
+// at TILE_N = 256 only one set fits, so its epilogue copies the accumulators to registers and releases the
+// tensor memory BEFORE it does the slow global loads / stores.  (TILE_N = 128 with two sets was measured: the
+// operand reads of a 256 x 128 x 16 MMA plus the TMA fill exceed the 128 B/clk shared-memory port, a1 ran 30 %
+// slower -- profiles/r1b_summary.md.)
 template <int KIND> struct KindTraits;
 template <> struct KindTraits<KIND_F16X2> {
-  static constexpr int ARRAYS = 2, STAGES = 3, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 1, FMT = 0, SUB = 16;
+  static constexpr int ARRAYS = 2, TILE_N = 256, SETS = 1, STAGES = 3, KSTEP_ELEMS = 16, BK_ELEMS = 64, FMT = 0, SUB = 16;
 };
 template <> struct KindTraits<KIND_HH16> {
-  static constexpr int ARRAYS = 1, STAGES = 6, KSTEP_ELEMS = 16, BK_ELEMS = 64, ACC_BUFS = 2, FMT = 0, SUB = 32;
+  static constexpr int ARRAYS = 1, TILE_N = 256, SETS = 2, STAGES = 6, KSTEP_ELEMS = 16, BK_ELEMS = 64, FMT = 0, SUB = 32;
 };
 template <> struct KindTraits<KIND_TF32> {
-  static constexpr int ARRAYS = 1, STAGES = 6, KSTEP_ELEMS = 8, BK_ELEMS = 32, ACC_BUFS = 2, FMT = 2, SUB = 32;
+  static constexpr int ARRAYS = 1, TILE_N = 256, SETS = 2, STAGES = 6, KSTEP_ELEMS = 8, BK_ELEMS = 32, FMT = 2, SUB = 32;
 };
 
 struct UmmaParams {
-  CUtensorMap mapA;     // A-operand buffer: [ARRAYS*Np rows][Np cols], box 128 B x 128 rows
+  CUtensorMap mapA;     // A-operand buffer: [ARRAYS*Np rows][Np cols], box 128 B x 64 rows
   CUtensorMap mapB;     // B-operand buffer, same box
   int np;               // padded dimension (= K)
   int macro_tiles;      // Np / 256
   int chunk_kb;         // KIND_F16X2: k-blocks (of 64) per promoted accumulation chunk (0 = whole K)
+  int chunk0_kb;        // KIND_F16X2: k-blocks of the FIRST chunk of a tile (>= chunk_kb; see the MMA issuer)
   State* st;
   StopArgs stop;        // a2 only (partials = one per CTA)
   // epilogue pointers (which are used depends on EPI / KIND; see the epilogue)
@@ -106,8 +120,12 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 // in registers after tcgen05.wait::ld; tcgen05.fence::before/after_thread_sync order the tensor-memory accesses).
 // No generic-proxy data is published, and a .release.cluster arrive costs a GPU-scope fence
 // (MEMBAR.ALL.GPU + ERRBAR + CGAERRBAR, profiles/r1a_summary.md) on the critical path of every chunk drain.
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
-  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
+// Predicated inside the asm (one arrival per warp, lane 0) so that the call site is straight-line code: a
+// compiler barrier in a divergent branch did not keep the epilogue's global loads / stores below the arrive.
+__device__ __forceinline__ void mbar_arrive_cluster_lane0(uint32_t bar_cluster_addr, int lane) {
+  asm volatile(
+      "{\n .reg .pred p;\n setp.eq.s32 p, %1, 0;\n @p mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];\n}"
+      ::"r"(bar_cluster_addr), "r"(lane) : "memory");
 }
 // Bounded wait: a pipeline bug traps (launch failure) instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
@@ -171,9 +189,9 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 __device__ __forceinline__ uint64_t make_sdesc(uint32_t saddr) {
   return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
-// kind::f16 / kind::tf32 instruction descriptor: D = F32, A/B format, both K-major, M = 256 (pair), N = 256.
-__host__ __device__ constexpr uint32_t make_idesc(int fmt) {
-  return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(UM_TILE >> 3) << 17) | ((uint32_t)(UM_TILE >> 4) << 24);
+// kind::f16 / kind::tf32 instruction descriptor: D = F32, A/B format, both K-major, M = 256 (pair), N = n.
+__host__ __device__ constexpr uint32_t make_idesc(int fmt, int n) {
+  return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(UM_TILE_M >> 4) << 24);
 }
 
 __device__ __forceinline__ uint32_t pack_h2(__half a, __half b) {
@@ -318,24 +336,32 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 
   using KT = KindTraits<KIND>;
   constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3);
-  constexpr bool PROMOTE = (KIND == KIND_F16X2);
-  constexpr int STAGE_BYTES = KT::ARRAYS * 2 * UM_BOX_BYTES;   // per CTA: A rows + B rows of every array
+  constexpr bool PAIRK = (KIND == KIND_F16X2);                 // (hi, lo') operand pairs, promoted accumulation
+  constexpr int TN = KT::TILE_N;
+  constexpr int NSPLIT = UM_MACRO / TN;                        // column sub-tiles per 256-wide macro tile
+  constexpr int B_BYTES = (TN / 2) * UM_ROWB;                  // B rows of one array, one stage, one CTA
+  constexpr int STAGE_BYTES = KT::ARRAYS * (UM_A_BYTES + B_BYTES);
+  constexpr int SET_COLS = KT::ARRAYS * TN;                    // TMEM columns of one accumulator set
+  constexpr int SETS = KT::SETS;
+  constexpr int GCOLS = (SETS == 2) ? TN : TN / 2;             // columns per epilogue thread
+  static_assert(SETS * SET_COLS <= UM_TMEM_COLS, "the accumulator sets must fit the tensor memory");
   static_assert(KT::STAGES * STAGE_BYTES <= UM_SMEM_OPERANDS && KT::STAGES <= UM_MAX_STAGES, "smem");
+  static_assert(!PAIRK || (KT::STAGES >= 3 && KT::STAGES <= 4), "promoted issue order: FRONT + BACK + 1 <= STAGES");
   constexpr int KSTEPS = KT::BK_ELEMS / KT::KSTEP_ELEMS;       // 4
-  constexpr uint32_t IDESC = make_idesc(KT::FMT);
-  constexpr int COLS = UM_TILE / (UM_EPI_WARPS / 4);           // columns per epilogue thread (128)
+  constexpr uint32_t IDESC = make_idesc(KT::FMT, TN);
   constexpr int SUB = KT::SUB;
 
   extern __shared__ unsigned char smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t bar_base = smem_base + UM_SMEM_OPERANDS;
-  // barrier slots (8 B each): full[0..5], empty[6..11], tfull[12..13], tempty[14..15], hh_full 16, hh_empty 17
+  // barrier slots (8 B each): full[0..5], empty[6..11], tfull[12..13], tempty[14..15], hh_full[16..17], hh_empty[18..19]
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 48u + 8u * s; };
   auto tfull_bar = [&](int b) { return bar_base + 96u + 8u * b; };
   auto tempty_bar = [&](int b) { return bar_base + 112u + 8u * b; };
-  const uint32_t hh_full_bar = bar_base + 128u, hh_empty_bar = bar_base + 136u;
-  const uint32_t tmem_slot = bar_base + 144u;
+  auto hh_full_bar = [&](int b) { return bar_base + 128u + 8u * b; };
+  auto hh_empty_bar = [&](int b) { return bar_base + 144u + 8u * b; };
+  const uint32_t tmem_slot = bar_base + 160u;
   __shared__ double red[32];
   __shared__ int last_flag;
 
@@ -344,14 +370,19 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
   const int np = p.np;
   const int KB = np / KT::BK_ELEMS;
-  const int CH = p.chunk_kb > 0 ? p.chunk_kb : KB;         // k-blocks per promoted chunk (KIND_F16X2)
+  const int CH = (p.chunk_kb > 0 && p.chunk_kb < KB) ? p.chunk_kb : KB;   // k-blocks per promoted chunk (KIND_F16X2)
+  // first chunk of a tile: at most a quarter of K (its partial sums stay small), never shorter than CH
+  const int CH0 = (CH < KB && p.chunk0_kb > CH && KB / 4 > CH) ? (p.chunk0_kb < KB / 4 ? p.chunk0_kb : KB / 4) : CH;
+  const int NCH = 1 + (KB - CH0 + CH - 1) / CH;                            // chunks per tile
   const int T = p.macro_tiles;
-  const int num_tiles = SYM ? T * (T + 1) / 2 : T * T;     // 256 x 256 pair tiles
+  const int num_tiles = (SYM ? T * (T + 1) / 2 : T * T) * NSPLIT;         // 256 x TN pair tiles
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < KT::ACC_BUFS; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 2 * UM_EPI_WARPS); }
-    mbar_init(hh_full_bar, 1); mbar_init(hh_empty_bar, 2 * UM_EPI_WARPS);
+    for (int b = 0; b < 2; ++b) {                  // arrivals: the warps of both CTAs that read the set
+      mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 2 * UM_EPI_WARPS / SETS);
+      mbar_init(hh_full_bar(b), 1); mbar_init(hh_empty_bar(b), 2 * UM_EPI_WARPS / SETS);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
@@ -369,11 +400,17 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 
   auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
     int I, J;
-    if (SYM) tri_decode(t, I, J);
-    else band_decode(t, T, T, 8, I, J);
-    m0 = I * UM_TILE;
-    n0 = J * UM_TILE;
-    offdiag = (I != J);
+    if (SYM) {
+      const int macro = t / NSPLIT, sub = t - macro * NSPLIT;
+      tri_decode(macro, I, J);
+      n0 = J * UM_MACRO + sub * TN;
+      offdiag = (I != J);
+    } else {
+      band_decode(t, T, T * NSPLIT, 8 * NSPLIT, I, J);
+      n0 = J * TN;
+      offdiag = true;                                      // (unused by the full-output epilogues)
+    }
+    m0 = I * UM_TILE_M;
   };
 
   double cta_sumsq = 0.0;
@@ -382,7 +419,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
     // ===================================================== TMA producer (both CTAs)
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      const int roff = (int)rank * UM_ROWS;
+      const int aoff = (int)rank * UM_ROWS, boff = (int)rank * (TN / 2);
       for (int t = pair; t < num_tiles; t += num_pairs) {
         int m0, n0; bool od; decode(t, m0, n0, od);
         for (int kb = 0; kb < KB; ++kb) {
@@ -390,11 +427,16 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
           if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * STAGE_BYTES);     // both CTAs' boxes
           const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
+          const uint32_t sb = sa + KT::ARRAYS * UM_A_BYTES;
           const int kc = kb * KT::BK_ELEMS;
 #pragma unroll
           for (int a = 0; a < KT::ARRAYS; ++a) {
-            tma_load_2d_pair(sa + a * UM_BOX_BYTES, &p.mapA, kc, a * np + m0 + roff, lead_full);
-            tma_load_2d_pair(sa + (KT::ARRAYS + a) * UM_BOX_BYTES, &p.mapB, kc, a * np + n0 + roff, lead_full);
+#pragma unroll
+            for (int b = 0; b < UM_ROWS / UM_BOX_ROWS; ++b)
+              tma_load_2d_pair(sa + a * UM_A_BYTES + b * UM_BOX_BYTES, &p.mapA, kc, a * np + m0 + aoff + b * UM_BOX_ROWS, lead_full);
+#pragma unroll
+            for (int b = 0; b < TN / 2 / UM_BOX_ROWS; ++b)
+              tma_load_2d_pair(sb + a * B_BYTES + b * UM_BOX_BYTES, &p.mapB, kc, a * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
           }
           if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
         }
@@ -403,93 +445,147 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   } else if (warp == 1) {
     // ===================================================== MMA issuer (leader CTA, one lane)
     if (rank == 0 && lane == 0) {
-      int stage = 0; uint32_t phase = 0;
-      int buf = 0; uint32_t accphase = 0;
-      uint32_t chunks = 0;                                     // promoted chunks committed so far (all tiles)
+      // tile li of this pair uses accumulator set li & 1 and is that set's (li >> 1)-th tile: the phase parities
+      // of the per-set barriers follow from li alone
 #ifdef ZFAC_TIMING
       long long twait[4] = {0, 0, 0, 0};
       const long long tstart = clock64();
 #endif
-      for (int t = pair; t < num_tiles; t += num_pairs) {
-        ZF_TWAIT(2, mbar_wait(tempty_bar(buf), accphase ^ 1u));
-        tc_fence_after();
-        const uint32_t d0 = tmem_base + (KT::ACC_BUFS == 2 ? buf * 256 : 0);   // D (or D_hh chunk)
-        const uint32_t d1 = tmem_base + 256;                                     // D_x (KIND_F16X2 only)
-        for (int kb = 0; kb < KB; ++kb) {
-          ZF_TWAIT(0, mbar_wait(full_bar(stage), phase));
+      if (PAIRK) {
+        // (h)(h) products go to D_hh, the 2^11-scaled cross products (h)(l') + (l')(h) to D_x.  D_hh is handed to
+        // the epilogue warps every CH k-blocks (promoted accumulation).  Issue order of a chunk of
+        // c k-blocks (H = 4 (h)(h) MMAs, C = 8 cross MMAs of one k-block; FRONT = BACK = 1 with 3 stages):
+        //     C0 | wait(D_hh drained) | H0 | H1 C1 ... | H(c-1) | commit(D_hh full) | C(c-1)
+        // so that the cross products of 2 k-blocks (16 MMAs, 2048 cycles) cover the drain of D_hh between chunks.
+        // The FIRST chunk of a tile is CH0 >= CH k-blocks long: while it runs, the epilogue warps still store
+        // the previous tile from registers (they released the tensor memory first), and its partial sums are
+        // small, so the truncation of the FP32 accumulator costs the least there.
+        constexpr int FRONT = (KT::STAGES >= 4) ? 2 : 1, BACK = FRONT;
+        uint32_t it = 0;                                       // k-block sequence number = position in the smem ring
+        int li = 0;
+        for (int t = pair; t < num_tiles; t += num_pairs, ++li) {
+          const int set = (SETS == 2) ? (li & 1) : 0;
+          const uint32_t nuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;   // earlier tiles of this set
+          const uint32_t d0 = tmem_base + set * SET_COLS, d1 = d0 + TN;
+          ZF_TWAIT(2, mbar_wait(tempty_bar(set), (nuse & 1u) ^ 1u));
           tc_fence_after();
-          const uint32_t sa = smem_base + stage * STAGE_BYTES;
-          const uint64_t a_hi = make_sdesc(sa);
-          const uint64_t a_lo = make_sdesc(sa + UM_BOX_BYTES);
-          const uint64_t b_hi = make_sdesc(sa + KT::ARRAYS * UM_BOX_BYTES);
-          const uint64_t b_lo = make_sdesc(sa + (KT::ARRAYS + 1) * UM_BOX_BYTES);
-          if (PROMOTE) {
-            // The (h)(h) products accumulate in D_hh for CH k-blocks at a time; the epilogue warps of both
-            // CTAs add every finished chunk to FP32 registers with round-to-nearest (DESIGN.md "promoted
-            // accumulation").  Issue order hides that drain behind tensor work: the chunk's last k-block
-            // issues (h)(h) first and its 2^11-scaled cross products after the commit, the next chunk's
-            // first k-block issues its cross products BEFORE waiting for the drained accumulator.
-            const int kc = kb % CH;
-            const bool first = (kc == 0), last = (kc == CH - 1 || kb == KB - 1);
-            auto issue_cross = [&]() {
+          uint32_t xacc = 0u;
+          uint32_t hch = nuse * (uint32_t)NCH;                 // chunks committed into this set so far
+          auto ring = [&](int j, uint32_t& st, uint32_t& ph) {
+            const uint32_t x = it + (uint32_t)j;
+            st = x % (uint32_t)KT::STAGES; ph = (x / (uint32_t)KT::STAGES) & 1u;
+          };
+          auto sdescs = [&](int j, uint64_t& a_hi, uint64_t& a_lo, uint64_t& b_hi, uint64_t& b_lo) {
+            uint32_t st, ph; ring(j, st, ph);
+            const uint32_t sa = smem_base + st * STAGE_BYTES;
+            a_hi = make_sdesc(sa); a_lo = make_sdesc(sa + UM_A_BYTES);
+            b_hi = make_sdesc(sa + 2 * UM_A_BYTES); b_lo = make_sdesc(sa + 2 * UM_A_BYTES + B_BYTES);
+          };
+          auto wait_full = [&](int j) {
+            uint32_t st, ph; ring(j, st, ph);
+            ZF_TWAIT(0, mbar_wait(full_bar(st), ph));
+            tc_fence_after();
+          };
+          auto issue_cross = [&](int j) {
+            uint64_t a_hi, a_lo, b_hi, b_lo; sdescs(j, a_hi, a_lo, b_hi, b_lo);
 #pragma unroll
-              for (int k = 0; k < KSTEPS; ++k) {
-                const uint64_t ko = (uint64_t)(k * 2);
-                tc_mma_pair<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, (kb | k) ? 1u : 0u);
-                tc_mma_pair<KIND>(d1, a_lo + ko, b_hi + ko, IDESC, 1u);
-              }
-            };
-            if (first) {
-              issue_cross();
-              if (chunks > 0) { ZF_TWAIT(1, mbar_wait(hh_empty_bar, (chunks - 1u) & 1u)); tc_fence_after(); }
+            for (int k = 0; k < KSTEPS; ++k) {
+              const uint64_t ko = (uint64_t)(k * 2);           // 32 bytes per k-step, in 16-byte units
+              tc_mma_pair<KIND>(d1, a_hi + ko, b_lo + ko, IDESC, xacc);
+              xacc = 1u;
+              tc_mma_pair<KIND>(d1, a_lo + ko, b_hi + ko, IDESC, 1u);
             }
+          };
+          auto issue_hh = [&](int j, bool fresh) {
+            uint64_t a_hi, a_lo, b_hi, b_lo; sdescs(j, a_hi, a_lo, b_hi, b_lo);
 #pragma unroll
             for (int k = 0; k < KSTEPS; ++k)
-              tc_mma_pair<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (kc | k) ? 1u : 0u);
-            if (last) { tc_commit_pair(hh_full_bar); ++chunks; }
-            if (!first) issue_cross();
-          } else {
+              tc_mma_pair<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (fresh && k == 0) ? 0u : 1u);
+          };
+          auto release = [&](int j) {                          // frees the stage in both CTAs when its MMAs retire
+            uint32_t st, ph; ring(j, st, ph);
+            tc_commit_pair(empty_bar(st));
+          };
+          for (int kb0 = 0; kb0 < KB;) {
+            const int want = (kb0 == 0) ? CH0 : CH;
+            const int c = (KB - kb0 < want) ? (KB - kb0) : want;
+            const int f = c < FRONT ? c : FRONT;
+            const int b = (c - f) < BACK ? (c - f) : BACK;
+            for (int j = 0; j < f; ++j) { wait_full(j); issue_cross(j); }
+            ZF_TWAIT(1, mbar_wait(hh_empty_bar(set), (hch & 1u) ^ 1u));
+            tc_fence_after();
+            for (int j = 0; j < f; ++j) { issue_hh(j, j == 0); release(j); }
+            for (int j = f; j < c - b; ++j) { wait_full(j); issue_hh(j, false); issue_cross(j); release(j); }
+            for (int j = c - b; j < c; ++j) { wait_full(j); issue_hh(j, false); }
+            tc_commit_pair(hh_full_bar(set)); ++hch;
+            for (int j = c - b; j < c; ++j) { issue_cross(j); release(j); }
+            it += (uint32_t)c;
+            kb0 += c;
+          }
+          tc_commit_pair(tfull_bar(set));                      // D_x complete, both CTAs
+        }
+      } else {
+        int stage = 0; uint32_t phase = 0;
+        int li = 0;
+        for (int t = pair; t < num_tiles; t += num_pairs, ++li) {
+          const int set = (SETS == 2) ? (li & 1) : 0;
+          const uint32_t nuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;
+          const uint32_t d0 = tmem_base + set * SET_COLS;
+          ZF_TWAIT(2, mbar_wait(tempty_bar(set), (nuse & 1u) ^ 1u));
+          tc_fence_after();
+          for (int kb = 0; kb < KB; ++kb) {
+            ZF_TWAIT(0, mbar_wait(full_bar(stage), phase));
+            tc_fence_after();
+            const uint32_t sa = smem_base + stage * STAGE_BYTES;
+            const uint64_t ad = make_sdesc(sa), bd = make_sdesc(sa + UM_A_BYTES);
 #pragma unroll
             for (int k = 0; k < KSTEPS; ++k)                   // 32 bytes per k-step, in 16-byte units
-              tc_mma_pair<KIND>(d0, a_hi + (uint64_t)(k * 2), b_hi + (uint64_t)(k * 2), IDESC, (kb | k) ? 1u : 0u);
+              tc_mma_pair<KIND>(d0, ad + (uint64_t)(k * 2), bd + (uint64_t)(k * 2), IDESC, (kb | k) ? 1u : 0u);
+            tc_commit_pair(empty_bar(stage));                  // frees the smem stage in both CTAs when the MMAs retire
+            if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
           }
-          tc_commit_pair(empty_bar(stage));                    // frees the smem stage in both CTAs when the MMAs retire
-          if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
+          tc_commit_pair(tfull_bar(set));                      // accumulator complete, both CTAs
         }
-        tc_commit_pair(tfull_bar(buf));                        // accumulator(s) complete, both CTAs
-        if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
-        else accphase ^= 1u;
       }
 #ifdef ZFAC_TIMING
       if (p.dbg) {
         twait[3] = clock64() - tstart;
-        for (int i = 0; i < 4; ++i) atomicAdd(p.dbg + (size_t)(EPI * 148 + pair) * 4 + i, (unsigned long long)twait[i]);
+        for (int i = 0; i < 4; ++i) atomicAdd(p.dbg + (size_t)(EPI * 148 + pair) * 8 + i, (unsigned long long)twait[i]);
       }
 #endif
     }
   } else {
     // ===================================================== epilogue warps (2 .. 9), both CTAs
+    // Group g = warps 2 + 4 g .. 5 + 4 g (one warp per TMEM lane quarter).  SETS == 2: group g owns accumulator
+    // set g, i.e. the tiles with local index li = g (mod 2), all TN columns: its stores overlap the other set's
+    // mainloop.  SETS == 1: both groups work on every tile, group g on columns [g TN/2, (g + 1) TN/2).
     const int q = warp & 3;                                    // TMEM lane quarter this warp may read
-    const int g = (warp - 2) >> 2;                             // column half of this warp
+    const int g = (warp - 2) >> 2;
+    const int set = (SETS == 2) ? g : 0;
+    const int col0 = (SETS == 2) ? 0 : g * GCOLS;              // first column of the tile handled by this thread
     const int row = (int)rank * UM_ROWS + q * 32 + lane;       // row of the pair tile held by this thread
-    const uint32_t lead_hh_empty = mapa_u32(hh_empty_bar, 0);
-    int buf = 0; uint32_t accphase = 0;
-    uint32_t chunks = 0;
-    const int nch = (KB + CH - 1) / CH;
-    for (int t = pair; t < num_tiles; t += num_pairs) {
+    const uint32_t lead_hh_empty = mapa_u32(hh_empty_bar(set), 0), lead_tempty = mapa_u32(tempty_bar(set), 0);
+    const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + set * SET_COLS + col0;
+    int li = 0;
+#ifdef ZFAC_TIMING
+    long long twait[4] = {0, 0, 0, 0};     // 4 wait for MMA (hh_full / tfull), 5 TMEM -> registers, 6 global loads / stores
+#endif
+    for (int t = pair; t < num_tiles; t += num_pairs, ++li) {
+      if (SETS == 2 && (li & 1) != g) continue;
+      const uint32_t tuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;   // tiles this thread has finished
       int m0, n0; bool offdiag; decode(t, m0, n0, offdiag);
       const int m = m0 + row;
-      const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + (KT::ACC_BUFS == 2 ? buf * 256 : 0) + g * COLS;
       double tile_sumsq = 0.0;
-      if (PROMOTE) {
-        float sum[COLS];
+      if (PAIRK) {
+        uint32_t hcnt = tuse * (uint32_t)NCH;                  // chunks drained from this set so far
+        float sum[GCOLS];
 #pragma unroll
-        for (int j = 0; j < COLS; ++j) sum[j] = 0.0f;
-        for (int c = 0; c < nch; ++c) {
-          mbar_wait(hh_full_bar, chunks & 1u);
+        for (int j = 0; j < GCOLS; ++j) sum[j] = 0.0f;
+        for (int c = 0; c < NCH; ++c) {
+          ZF_TWAIT(0, mbar_wait(hh_full_bar(set), hcnt & 1u));
           tc_fence_after();
 #pragma unroll
-          for (int i = 0; i < COLS / 32; ++i) {
+          for (int i = 0; i < GCOLS / 32; ++i) {
             uint32_t r[32];
             tmem_ld(tbase + i * 32, r);
             tmem_ld_wait();
@@ -498,28 +594,48 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
           }
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(lead_hh_empty);
-          ++chunks;
+          mbar_arrive_cluster_lane0(lead_hh_empty, lane);
+          ++hcnt;
         }
-        mbar_wait(tfull_bar(0), accphase);
+        // D_hh + 2^-11 D_x into registers, then hand the tensor memory back BEFORE the global loads / stores:
+        // the next tile's MMAs run while this tile is written out.
+        ZF_TWAIT(0, mbar_wait(tfull_bar(set), tuse & 1u));
         tc_fence_after();
+#ifdef ZFAC_TIMING
+        const long long te0 = clock64();
+#endif
 #pragma unroll
-        for (int cc = 0; cc < COLS / SUB; ++cc) {
-          float v[SUB];
-          {
-            uint32_t x[SUB];
-            tmem_ld(tbase + 256 + cc * SUB, x);
-            tmem_ld_wait();
+        for (int i = 0; i < GCOLS / 32; ++i) {
+          uint32_t x[32];
+          tmem_ld(tbase + TN + i * 32, x);
+          tmem_ld_wait();
 #pragma unroll
-            for (int j = 0; j < SUB; ++j) v[j] = sum[cc * SUB + j] + __uint_as_float(x[j]) * LO_UNSCALE;
-          }
-          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + g * COLS + cc * SUB, offdiag, tile_sumsq);
+          for (int j = 0; j < 32; ++j) sum[i * 32 + j] += __uint_as_float(x[j]) * LO_UNSCALE;
         }
+        tc_fence_before();
+        __syncwarp();
+        mbar_arrive_cluster_lane0(lead_tempty, lane);
+        // ptxas is free to sink a relaxed arrive below the (independent) global loads / stores that follow, which
+        // would give the tensor memory back only after the tile is written; a CTA-scope fence pins it here.
+        asm volatile("fence.acq_rel.cta;" ::: "memory");
+#ifdef ZFAC_TIMING
+        const long long te1 = clock64();
+#endif
+#pragma unroll
+        for (int cc = 0; cc < GCOLS / SUB; ++cc) {
+          float v[SUB];
+#pragma unroll
+          for (int j = 0; j < SUB; ++j) v[j] = sum[cc * SUB + j];
+          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, offdiag, tile_sumsq);
+        }
+#ifdef ZFAC_TIMING
+        twait[1] += te1 - te0; twait[2] += clock64() - te1;
+#endif
       } else {
-        mbar_wait(tfull_bar(buf), accphase);
+        mbar_wait(tfull_bar(set), tuse & 1u);
         tc_fence_after();
 #pragma unroll 1
-        for (int cc = 0; cc < COLS / SUB; ++cc) {
+        for (int cc = 0; cc < GCOLS / SUB; ++cc) {
           float v[SUB];
           {
             uint32_t r[SUB];
@@ -528,16 +644,18 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 #pragma unroll
             for (int j = 0; j < SUB; ++j) v[j] = __uint_as_float(r[j]);
           }
-          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + g * COLS + cc * SUB, offdiag, tile_sumsq);
+          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, offdiag, tile_sumsq);
         }
+        tc_fence_before();
+        __syncwarp();
+        mbar_arrive_cluster_lane0(lead_tempty, lane);            // frees the accumulator set
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive_cluster(mapa_u32(tempty_bar(buf), 0));   // 2 x 8 warp arrivals free the accumulator
       if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
-      if (KT::ACC_BUFS == 2) { buf ^= 1; if (buf == 0) accphase ^= 1u; }
-      else accphase ^= 1u;
     }
+#ifdef ZFAC_TIMING
+    if (p.dbg && rank == 0 && warp == 2 && lane == 0)
+      for (int i = 0; i < 3; ++i) atomicAdd(p.dbg + (size_t)(EPI * 148 + pair) * 8 + 4 + i, (unsigned long long)twait[i]);
+#endif
   }
 
   // ------------------------------------------------------- teardown (+ step a3 for a2)
@@ -573,7 +691,8 @@ struct UmmaPlan {
   int max_pairs = 0;  // CTA pairs that are co-resident on the device (74 on a B200)
   int mode = 0;
   int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
-  // tensor maps of every operand buffer (box 128 B x 128 rows, 128B swizzle)
+  int chunk0_kb = 16; // first chunk of every tile (covers the previous tile's stores; partial sums still small)
+  // tensor maps of every operand buffer (box 128 B x 64 rows, 128B swizzle)
   CUtensorMap mS, mW, mT, mR, mQ, mZ[2];
 };
 
@@ -581,7 +700,7 @@ inline cudaError_t make_map(PFN_encodeTiled enc, CUtensorMap* m, void* base, CUt
                             uint64_t rows, uint64_t cols) {
   cuuint64_t gdim[2] = {cols, rows};
   cuuint64_t gstr[1] = {cols * elt};
-  cuuint32_t box[2] = {(cuuint32_t)(UM_ROWB / elt), (cuuint32_t)UM_ROWS};
+  cuuint32_t box[2] = {(cuuint32_t)(UM_ROWB / elt), (cuuint32_t)UM_BOX_ROWS};
   cuuint32_t estr[2] = {1u, 1u};
   CUresult r = enc(m, dt, 2, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -620,7 +739,8 @@ inline cudaError_t prepare_kind(int* max_pairs) {
 
 inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int sm_count) {
   pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0;
-  if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knob
+  if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knobs
+  if (const char* ck = getenv("ZFAC_CHUNK0_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk0_kb = v; }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -674,8 +794,10 @@ inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const 
 inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, double* d_err, cudaStream_t s, int* launches, Prof* prof) {
   const Layout& L = pl.L;
   char* ws = pl.ws;
-  const int T = (int)(L.np / UM_TILE);
-  const int full_tiles = T * T, sym_tiles = T * (T + 1) / 2;
+  const int T = (int)(L.np / UM_MACRO);
+  const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
+                                 : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
+  const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
   const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
   const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
   UmmaParams p{};
@@ -692,7 +814,7 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
   for (int n = 0; n <= max_iter; ++n) {
     // a1: T = W S^T            (promoted accumulation: T and X are O(1) quantities)
     prof->mark(s, EPI_A1 + 16 * n);
-    p.chunk_kb = pl.chunk_kb;
+    p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
     p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; }
@@ -700,13 +822,14 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
     // a2: R = I - W T^T
     prof->mark(s, EPI_A2 + 16 * n);
     p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n;
+    p.chunk0_kb = 2 * pl.chunk0_kb;           // a2 writes four outputs per element: its stores take twice as long
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
     umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
     nl += 2;
     if (n == max_iter) break;
     // a4: Q = 1/2 R + 3/8 R R^T   (the product is a correction of size |R|^2: no promotion needed)
     prof->mark(s, EPI_A4 + 16 * n);
-    p.chunk_kb = 0;
+    p.chunk_kb = 0; p.chunk0_kb = 0;
     p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr; }
@@ -733,12 +856,14 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
 inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* launches) {
   const Layout& L = pl.L;
   char* ws = pl.ws;
-  const int T = (int)(L.np / UM_TILE);
-  const int full_tiles = T * T, sym_tiles = T * (T + 1) / 2;
+  const int T = (int)(L.np / UM_MACRO);
+  const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
+                                 : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
+  const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
   const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
   const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T; p.chunk_kb = pl.chunk_kb;
+  p.np = (int)L.np; p.macro_tiles = T; p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
   const bool h16 = (L.mode != ZFAC_MODE_TF32);
   p.mapA = pl.mW; p.mapB = pl.mS;

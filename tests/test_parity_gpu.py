@@ -370,3 +370,63 @@ def test_full_size_n8192_bench_configuration_properties():
         assert rel <= (1e-11 if mode == "f64" else 5e-5)
         assert samp <= tol_s
         assert inv <= (1e-11 if mode == "f64" else 5e-4)
+
+
+# ------------------------------------------------------------------ BASELINE configs[2], configs[3] at FULL size
+def test_config3_full_size_n4617_all_modes_and_trace():
+    """BASELINE configs[2] as written: N = 4617 (3^5 * 19: no tile multiple, row pitch not 16-byte aligned),
+    kappa = 1e5, FP32-stored S, Z0 = I / sqrt(lambda_max), all three modes plus the stopping-criterion trace.
+    The oracle (a few 1e13 flop on the host cores) is run for the same number of updates as each GPU run."""
+    b = zb()
+    w = W.config3()
+    assert w.n == 4617
+    nat = O.refine(w.S, w.Z0, 40, O.STOP_PAPER)
+    Z, it, err, fl, _, _ = gpu_refine(w, "f64", 40, b.ZFAC_STOP_PAPER)
+    ref = nat if it == nat.iters else O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+    rel = _rel(Z, ref.Z)
+    print(f"[config3 N=4617 f64] iters={it} (oracle natural stop {nat.iters}) rel={rel:.3e} "
+          f"Err/sqrtN={err[-1] / math.sqrt(w.n):.3e} trace={np.array2string(err, precision=3)}")
+    assert fl == b.ZFAC_R_STOPPED and it == nat.iters == 13          # SURVEY.md §8(c): FP64 stops at n = 13
+    assert rel <= 1e-11
+    assert np.allclose(err[:12], nat.err[:12], rtol=1e-7)
+    Z, it, err, fl, _, _ = gpu_refine(w, "split16", 40, b.ZFAC_STOP_PAPER)
+    ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+    rel = _rel(Z, ref.Z)
+    print(f"[config3 N=4617 split16] iters={it} rel={rel:.3e} (u*kappa floor, DESIGN.md §6) "
+          f"Err/sqrtN={O.final_residual_per_sqrt_n(w.S, Z):.3e} trace={np.array2string(err, precision=3)}")
+    assert fl & b.ZFAC_R_STOPPED and 10 <= it <= 14
+    assert rel <= 5e-3                                               # derived bound at kappa = 1e5 (DESIGN.md §6)
+    for k in range(it + 1):
+        if ref.err[k] > 2.0:                                         # 100 x the SPLIT16 floor of ||R||_F (~2e-2 here)
+            assert err[k] == pytest.approx(ref.err[k], rel=2e-3)
+    Z, it, err, fl, _, _ = gpu_refine(w, "tf32", 40, b.ZFAC_STOP_PAPER)
+    print(f"[config3 N=4617 tf32] iters={it} flags={fl} trace={np.array2string(err, precision=3)}")
+    assert fl != 0 and len(err) == it + 1                            # expected to fail to converge: trace + flags
+
+
+def test_config4_full_size_n8192_bench_workload():
+    """BASELINE configs[3] as bench.py times it: N = 8192 warm start (reading Q-D4), FP32-stored S and Z0,
+    paper stop rule, SPLIT16 and F64, element by element against the oracle run for the same number of updates;
+    plus SPLIT16 followed by the FP64 refinement step (Alg. 3), which is what reaches the tight gate at kappa = 1e5."""
+    b = zb()
+    w = W.config4(n=8192, device=DEV)
+    refs = {}
+    for mode, tol in (("f64", 1e-11), ("split16", 5e-3)):
+        Z, it, err, fl, _, launches = gpu_refine(w, mode, 20, b.ZFAC_STOP_PAPER)
+        if it not in refs:
+            refs[it] = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+        ref = refs[it]
+        rel = _rel(Z, ref.Z)
+        print(f"[config4 N=8192 {mode}] iters={it} rel={rel:.3e} Err={np.array2string(err, precision=3)} "
+              f"oracle Err={np.array2string(ref.err, precision=3)} launches={launches}")
+        assert fl & b.ZFAC_R_STOPPED and 1 <= it <= 3
+        assert rel <= tol
+        assert err[0] == pytest.approx(ref.err[0], rel=1e-9 if mode == "f64" else 2e-3)
+    S, Z0 = _to_dev(w.S, "split16"), _to_dev(w.Z0, "split16")
+    with b.Zfac(w.n, "split16", DEV) as zl, b.Zfac(w.n, "f64", DEV) as zh:
+        Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=20, refi_steps=2, final_check=True)
+    Z = Z.cpu().numpy()
+    inv = O.final_residual_per_sqrt_n(w.S, Z)
+    print(f"[config4 N=8192 split16+refi] iters={it} Err={np.array2string(err, precision=3)} ||Z^T S Z - I||_F/sqrtN={inv:.3e}")
+    assert (fl & b.ZFAC_R_REFINED) and inv < 1e-10
+    assert err[-1] == pytest.approx(inv * math.sqrt(w.n), rel=1e-2, abs=1e-10)
