@@ -357,6 +357,16 @@ def run_ours(args):
                 "peak_source": f"{peaks['source']}: {pk_name}", "frac_of_burst": ach / peaks["bf16_burst"] if args.mode == "split16" else None,
                 "executed_flops_per_launch": passes * 2.0 * n ** 3, "launch_ms": kms["a1"],
                 "all_kernels_ms": kms}
+        if args.mode == "split16":
+            # the contract's denominator for a kernel timed inside a long step is the SUSTAINED figure, which was
+            # taken under 4 s of back-to-back cuBLAS bf16 GEMMs at the power cap; a frac above 1 is not "above
+            # peak": this step mixes in symmetric kernels and O(N^2) epilogues that draw less power, so the chip
+            # holds higher clocks.  frac_of_burst and the same-run cuBLAS rate are the tighter comparison.
+            roof["peak_note"] = ("peak = sustained bf16 (power-capped, 4 s back-to-back GEMM); frac > 1 means the step "
+                                 "throttles less than that reference load, not that the kernel beats the tensor peak; "
+                                 "see frac_of_burst and modes.cublas_tflops.bf16 (same run)")
+            cb = extra.get("cublas_tflops", {}).get("bf16")
+            roof["frac_of_cublas_bf16_same_run"] = (ach / cb) if cb else None
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N = 1 only
     cpu = None

@@ -421,7 +421,17 @@ def test_config4_full_size_n8192_bench_workload():
               f"oracle Err={np.array2string(ref.err, precision=3)} launches={launches}")
         assert fl & b.ZFAC_R_STOPPED and 1 <= it <= 3
         assert rel <= tol
-        assert err[0] == pytest.approx(ref.err[0], rel=1e-9 if mode == "f64" else 2e-3)
+        if mode == "f64":
+            assert err[0] == pytest.approx(ref.err[0], rel=1e-9)
+        else:
+            # DESIGN.md §6 (noise floor of ||R||_F): at kappa = 1e5 the FP32 rounding noise of X = Z^T(SZ) is
+            # ~N u ||z_row|| ||t_row|| ~ 0.03 here, the same size as ||R_0||_F = 0.09 itself, and it is
+            # uncorrelated with R_0: Err[0]^2 = ||R_0||_F^2 + floor^2.  The run stops AT the floor (Eq. 38 fires),
+            # so floor ~ err[it]; it must also stay under the a-priori cap of §6.
+            floor = err[it]
+            assert floor <= 0.1
+            assert abs(err[0] ** 2 - ref.err[0] ** 2) <= (2.0 * floor) ** 2
+            assert err[0] >= ref.err[0] * (1.0 - 2e-3)               # noise can only add
     S, Z0 = _to_dev(w.S, "split16"), _to_dev(w.Z0, "split16")
     with b.Zfac(w.n, "split16", DEV) as zl, b.Zfac(w.n, "f64", DEV) as zh:
         Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=20, refi_steps=2, final_check=True)
