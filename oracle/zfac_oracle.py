@@ -30,6 +30,19 @@ What it computes (PAPER.md = /root/reference/PAPER.md):
   (substitute X = I - R).  The delta-form is the default because it is the one
   BASELINE.json's north_star names; tests pin the two against each other.
 
+  Higher orders m = 3, 4.  The paper does not
+  print the coefficients for m > 2 ("Reference 1 gives a table"); it fixes them by
+  the condition that "the error terms delta^nu = (X_n - I)^nu should vanish up to
+  the highest possible order" after each iteration.  In the
+  residual R = I - X with Z_{n+1} = Z_n p(R_n), X_{n+1} = p(R)(I - R)p(R), so the
+  condition is p(R)^2 (I - R) = I + O(R^{m+1}): p is the degree-m Taylor polynomial
+  of (1 - R)^{-1/2},  c_k = C(2k, k) / 4^k = 1, 1/2, 3/8, 5/16, 35/128  (reading Q18;
+  for m = 2 it is the printed a_k under X = I - R).  The error then obeys
+  R_{n+1} = sum_{k=m+1}^{2m+1} t_k R_n^k with t_k > 0, sum t_k = 1 (for m = 2 the
+  printed 5/8, 15/64, 9/64), so the argument of Sec. IV.A
+   carries over with the exponent nu_max = m + 1:
+  the test is  Err[n] > Err[n-1]^(m+1).
+
 Readings of silent / ambiguous points (repeated in DESIGN.md):
   Q5  the Z returned at the break is the current one (Alg. 2 never rolls back);
   Q6  `iters` = number of Z updates performed = the stop index; Err has iters+1 entries;
@@ -44,6 +57,11 @@ identity for non-symmetric Z0; Z -> S^-1/2 from a dense eigendecomposition when
 Z0 ∝ I; Z Z^T = S^-1 for non-commuting Z0; cubic order; stop-rule cases;
 scaling / permutation covariances; diagonal S reduces to N scalar recursions;
 `congruence` against the generalized eigenvalues of (H, S) from scipy.linalg.eigh.
+Order m = 3, 4 (tests/test_oracle_order_pins.py): the coefficients re-derived in exact
+rationals from the vanishing condition alone; m = 2 mapped onto the printed a_k; the
+tail t_k > 0 with sum 1 and, for m = 2, equal to the printed c, d, e; a scalar
+exact-rational step; the matrix identity R_1 = sum t_k R_0^k for non-symmetric Z0;
+Z -> S^-1/2 from numpy.linalg.eigh; observed order m + 1; the generalised stop test.
 Every function below is pinned; none is "parity unpinned".
 """
 from __future__ import annotations
@@ -102,13 +120,39 @@ def update_x_form(Z: np.ndarray, X: np.ndarray) -> np.ndarray:
     return Z @ P
 
 
+def order_coefficients(m: int) -> list:
+    """c_0..c_m of p(R) = sum c_k R^k, the degree-m Taylor polynomial of (1 - R)^{-1/2}:
+    c_k = C(2k, k) / 4^k  (the vanishing-order condition of PAPER.md:121-123; reading Q18)."""
+    if m < 1:
+        raise ValueError("order m must be >= 1")
+    return [math.comb(2 * k, k) / 4.0 ** k for k in range(m + 1)]
+
+
+def update_order_m(Z: np.ndarray, R: np.ndarray, m: int) -> np.ndarray:
+    """Z_{n+1} = Z_n + Z_n (c_1 R + c_2 R^2 + ... + c_m R^m)   (Eq. 13 / Eq. 16 with general m,
+    PAPER.md:112-131).  The powers of R are formed one by one, R^k = R^{k-1} R, and summed in
+    increasing k: no Horner form, no regrouping."""
+    c = order_coefficients(m)
+    Rk = R
+    Q = c[1] * R
+    for k in range(2, m + 1):
+        Rk = Rk @ R
+        Q = Q + c[k] * Rk
+    return Z + Z @ Q
+
+
 def refine(S: np.ndarray, Z0: np.ndarray, max_iter: int, stop: int = STOP_PAPER,
-           form: str = "delta", dtype=np.float64) -> RefineResult:
+           form: str = "delta", dtype=np.float64, order: int = 2) -> RefineResult:
     """Algorithm 2.  `dtype` exists only so that the paper's
     `single` scheme (Table I) can be emulated in a pin; the oracle
-    proper is FP64."""
+    proper is FP64.  `order` = m of Eq. 13 (2 = the paper's tests; 3, 4 = SURVEY.md §8(f3));
+    the stop test uses the exponent nu_max = m + 1 (Eq. 38)."""
     if max_iter < 0:
         raise ValueError("max_iter must be >= 0")
+    if order < 2 or order > 4:
+        raise ValueError("order must be 2, 3 or 4")
+    if order != 2 and form != "delta":
+        raise ValueError("the X-form is printed for m = 2 only (PAPER.md:303, :451)")
     S = np.asarray(S, dtype=dtype)
     Z = np.array(Z0, dtype=dtype, copy=True)
     n = S.shape[0]
@@ -123,14 +167,16 @@ def refine(S: np.ndarray, Z0: np.ndarray, max_iter: int, stop: int = STOP_PAPER,
         if not math.isfinite(err[it]):
             flags |= R_NONFINITE
             break
-        if stop == STOP_PAPER and it > 0 and err[it] > err[it - 1] ** 3:
+        if stop == STOP_PAPER and it > 0 and err[it] > err[it - 1] ** (order + 1):
             flags |= R_STOPPED
             break
         if it == max_iter:
             flags |= R_MAXITER
             break
         it += 1
-        if form == "delta":
+        if order != 2:
+            Z = update_order_m(Z, R, order)
+        elif form == "delta":
             Z = update_delta_form(Z, R)
         elif form == "x":
             Z = update_x_form(Z, X)
