@@ -68,7 +68,7 @@ typedef enum {
 
 /* Result flags written to *flags together with the outputs. */
 enum {
-  ZFAC_R_STOPPED = 1,  /* the test Err[n] > Err[n-1]^3 fired (converged to the precision floor) */
+  ZFAC_R_STOPPED = 1,  /* the test Err[n] > Err[n-1]^(m+1) fired (m = 2: ^3; converged to the precision floor) */
   ZFAC_R_MAXITER = 2,  /* max_iter updates were performed without the test firing               */
   ZFAC_R_NONFINITE = 4, /* Err[n] became inf/NaN; iteration stopped                              */
   ZFAC_R_REFINED = 8    /* zfac_refine_refi: the FP64 refinement updates were applied            */
@@ -148,6 +148,18 @@ zfac_status zfac_refine_host(zfac_ctx* ctx, const void* h_S, int64_t lds, const 
 /* Copy an internal buffer (top-left n x n block, converted to the mode's element type) to
  * d_out (n x n, ld).  Asynchronous on `stream`.  For tests of the individual steps. */
 zfac_status zfac_peek(zfac_ctx* ctx, zfac_buf which, void* d_out, int64_t ld, void* stream);
+
+/* Order m of the refinement polynomial, Z_{n+1} = Z_n sum_{k=0..m} c_k R_n^k  (Eq. 13 / Eq. 16:
+ * "Reference 1 gives a table with the coefficients a_k for polynomials of order m = 2, 3, 4, 5. For the tests in
+ * this article, we use m = 2").  m = 2 (default; the paper's scheme), 3 or 4; anything else -> ZFAC_E_INVALID and
+ * the context keeps its order.  The coefficients follow from the paper's condition that the error terms vanish to
+ * the highest possible order: c_k = C(2k,k)/4^k = 1, 1/2, 3/8, 5/16, 35/128, and the stop test
+ * becomes Err[n] > Err[n-1]^(m+1) (nu_max = m + 1; Eq. 38).  For m > 2 step a4 is two symmetric
+ * GEMMs, P = R R and Q = 1/2 R + P G with G = 3/8 I + 5/16 R (+ 35/128 P for m = 4), i.e. five kernels per
+ * iteration instead of four.  Host-side state only: takes effect from the next zfac_refine* call on `ctx`;
+ * no device work, no synchronisation.  ZFAC_BUF_Q then holds Q = sum_{k>=1} c_k R^k. */
+zfac_status zfac_set_order(zfac_ctx* ctx, int m);
+int zfac_get_order(const zfac_ctx* ctx);
 
 /* Number of kernels the last zfac_refine / zfac_refine_host call on this context enqueued. */
 int zfac_last_launch_count(const zfac_ctx* ctx);

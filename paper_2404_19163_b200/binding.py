@@ -29,7 +29,7 @@ EXPORTS = [
     "zfac_workspace_bytes", "zfac_create", "zfac_refine", "zfac_refine_host", "zfac_refine_refi",
     "zfac_congruence", "zfac_peek",
     "zfac_last_launch_count", "zfac_padded_n", "zfac_destroy", "zfac_status_string",
-    "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile",
+    "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile", "zfac_set_order", "zfac_get_order",
 ]
 
 _lib: Optional[ctypes.CDLL] = None
@@ -82,6 +82,10 @@ def lib() -> ctypes.CDLL:
     L.zfac_set_profile.argtypes = [vp, ci]
     L.zfac_get_profile.restype = ci
     L.zfac_get_profile.argtypes = [vp, vp, vp, ci]
+    L.zfac_set_order.restype = ci
+    L.zfac_set_order.argtypes = [vp, ci]
+    L.zfac_get_order.restype = ci
+    L.zfac_get_order.argtypes = [vp]
     _lib = L
     return L
 
@@ -147,6 +151,17 @@ def zfac_peek(ctx: int, which: int, d_out: int, ld: int, stream: int = 0) -> Non
 
 def zfac_last_launch_count(ctx: int) -> int:
     return int(lib().zfac_last_launch_count(ctx))
+
+
+def zfac_set_order(ctx: int, m: int) -> None:
+    """Order m of the refinement polynomial (2, 3, 4); see include/zfac.h."""
+    st = lib().zfac_set_order(ctx, int(m))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_set_order")
+
+
+def zfac_get_order(ctx: int) -> int:
+    return int(lib().zfac_get_order(ctx))
 
 
 def zfac_set_profile(ctx: int, enable: bool) -> None:
@@ -285,6 +300,13 @@ class Zfac:
 
     def set_profile(self, enable: bool) -> None:
         zfac_set_profile(self.ctx, enable)
+
+    def set_order(self, m: int) -> None:
+        zfac_set_order(self.ctx, m)
+
+    @property
+    def order(self) -> int:
+        return zfac_get_order(self.ctx)
 
     def get_profile(self):
         return zfac_get_profile(self.ctx)

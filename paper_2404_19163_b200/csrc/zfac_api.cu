@@ -34,6 +34,7 @@ struct zfac_ctx {
   Layout L;
   int launches;
   int sm_count;
+  int order;       // m of Eq. 13 (zfac_set_order): 2 (default), 3, 4
   UmmaPlan umma;   // tensor maps + launch geometry for the tcgen05 modes
   Prof prof;
 };
@@ -81,13 +82,14 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   zfac_ctx* c = new (std::nothrow) zfac_ctx();
   if (!c) return ZFAC_E_INVALID;
   c->n = n; c->np = L.np; c->mode = mode; c->ws = static_cast<char*>(d_workspace); c->ws_bytes = bytes;
-  c->L = L; c->launches = 0; c->sm_count = sms;
+  c->L = L; c->launches = 0; c->sm_count = sms; c->order = 2;
   if (mode == ZFAC_MODE_F64) {
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A1>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A2>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_X3>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A4>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
     ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A5>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_P2>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
   } else {
     cudaError_t e = umma_plan_create(&c->umma, L, c->ws, sms);
     if (e != cudaSuccess) {
@@ -140,6 +142,14 @@ int zfac_get_profile(zfac_ctx* c, int* tags, float* ms, int cap) {
 
 int zfac_last_launch_count(const zfac_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+zfac_status zfac_set_order(zfac_ctx* c, int m) {
+  if (!c || m < 2 || m > 4) return ZFAC_E_INVALID;
+  c->order = m;
+  return ZFAC_OK;
+}
+
+int zfac_get_order(const zfac_ctx* c) { return c ? c->order : 0; }
+
 // skip_last: Alg. 3 as printed ends after the update, without evaluating the residual of the result.
 static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s,
                               bool skip_last = false) {
@@ -158,6 +168,8 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = st;
   p.stop.st = st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = tri; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+  p.stop.order = c->order;
+  p.pc = poly_coef(c->order);
   for (int n = 0; n <= max_iter; ++n) {
     if (n == max_iter && skip_last) break;
     p.A = W; p.B = S; p.out0 = T; p.out1 = nullptr; p.in0 = nullptr;
@@ -168,7 +180,16 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
     f64_gemm_kernel<EPI_A2><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
     c->launches += 2;
     if (n == max_iter) break;
-    p.A = R; p.B = R; p.in0 = R; p.out0 = Q;
+    if (c->order > 2) {
+      // order m > 2: P = R R -> T buffer, G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z buffer a5 overwrites next
+      p.A = R; p.B = R; p.in0 = R; p.out0 = T; p.out1 = Z[(n + 1) & 1];
+      c->prof.mark(s, EPI_P2 + 16 * n);
+      f64_gemm_kernel<EPI_P2><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+      c->launches += 1;
+      p.A = T; p.B = Z[(n + 1) & 1]; p.in0 = R; p.out0 = Q; p.out1 = nullptr;       // Q = 1/2 R + P G
+    } else {
+      p.A = R; p.B = R; p.in0 = R; p.out0 = Q;
+    }
     c->prof.mark(s, EPI_A4 + 16 * n);
     f64_gemm_kernel<EPI_A4><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
     p.A = Z[n & 1]; p.B = Q; p.in0 = Z[n & 1]; p.out0 = Z[(n + 1) & 1]; p.out1 = W;
@@ -244,7 +265,7 @@ zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d
     rs = refine_f64(c, max_iter, stop, d_err, s);
   } else {
     int nl = 0;
-    cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, d_err, s, &nl, &c->prof);
+    cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, c->order, d_err, s, &nl, &c->prof);
     c->launches += nl;
     if (e != cudaSuccess) {
       snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_refine: %s", cudaGetErrorString(e));

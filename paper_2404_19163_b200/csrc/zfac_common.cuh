@@ -25,6 +25,7 @@ struct StopArgs {
   int n_iter;                // index n of the residual being evaluated
   int max_iter;
   int stop;                  // zfac_stop
+  int order;                 // m of Eq. 13 (2, 3, 4): the test's exponent is nu_max = m + 1
 };
 
 // Optional per-kernel timing (zfac_set_profile): an event is recorded on the launching stream
@@ -73,7 +74,9 @@ __device__ inline void stop_test_last_cta(const StopArgs& a, double* smem_red /*
       flags = ZFAC_R_NONFINITE; done = 1;
     } else if (a.stop == ZFAC_STOP_PAPER && n > 0) {
       const double prev = a.d_err[n - 1];
-      if (err > prev * prev * prev) { flags = ZFAC_R_STOPPED; done = 1; }
+      double thr = prev * prev * prev;                         // m = 2: Err[n-1]^3 (Eq. 38)
+      for (int k = 2; k < a.order; ++k) thr *= prev;           // m = 3, 4: Err[n-1]^(m+1)
+      if (err > thr) { flags = ZFAC_R_STOPPED; done = 1; }
     }
     if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
     if (done) { st->flags |= flags; __threadfence(); st->done = 1; }

@@ -24,7 +24,26 @@ constexpr int F64_THREADS = 256;
 constexpr int F64_STAGE_DOUBLES = (F64_BM + F64_BN) * F64_LDS;
 constexpr int F64_SMEM_BYTES = F64_STAGES * F64_STAGE_DOUBLES * 8;
 
-enum { EPI_A1 = 1, EPI_A2 = 2, EPI_X3 = 3 /* X = Z^T H Z itself (congruence, Eq. 11) */, EPI_A4 = 4, EPI_A5 = 5 };
+enum { EPI_A1 = 1, EPI_A2 = 2, EPI_X3 = 3 /* X = Z^T H Z itself (congruence, Eq. 11) */, EPI_A4 = 4, EPI_A5 = 5,
+       EPI_P2 = 6 /* order m > 2: P = R R and G = 3/8 I + 5/16 R (+ 35/128 P), both mirrored */ };
+
+// Polynomial coefficients of step a4 (Eq. 13 / 16 with order m; c_k = C(2k,k)/4^k, zfac.h):
+//   m = 2:  Q = 1/2 R + 3/8 (R R)                                   one symmetric GEMM   (EPI_A4, q_d = 3/8)
+//   m > 2:  P = R R,  G = 3/8 I + 5/16 R + g_p P                     (EPI_P2)
+//           Q = 1/2 R + P G        (P and G commute: symmetric)      (EPI_A4, q_d = 1)
+struct PolyCoef {
+  double q_r;   // EPI_A4: weight of R            (1/2)
+  double q_d;   // EPI_A4: weight of the product  (3/8 for m = 2, 1 for m > 2)
+  double g_i;   // EPI_P2: weight of I in G       (3/8)
+  double g_r;   // EPI_P2: weight of R in G       (5/16)
+  double g_p;   // EPI_P2: weight of P in G       (35/128 for m = 4, 0 for m = 3)
+};
+inline PolyCoef poly_coef(int order) {
+  PolyCoef c;
+  c.q_r = 0.5; c.q_d = (order == 2) ? 0.375 : 1.0;
+  c.g_i = 0.375; c.g_r = 0.3125; c.g_p = (order >= 4) ? 35.0 / 128.0 : 0.0;
+  return c;
+}
 
 struct F64Params {
   const double* A;      // [Np][ld]
@@ -33,9 +52,10 @@ struct F64Params {
   int K;                // = Np
   int tiles;            // Np / 128
   State* st;
-  double* out0;         // a1: T   a2: R   a4: Q   a5: Z_next
-  double* out1;         // a5: W
-  const double* in0;    // a4: R   a5: Z_cur
+  double* out0;         // a1: T   a2: R   a4: Q   a5: Z_next   p2: P
+  double* out1;         // a5: W   p2: G
+  const double* in0;    // a4: R   a5: Z_cur   p2: R
+  PolyCoef pc;          // a4, p2
   StopArgs stop;        // a2 only
 };
 
@@ -62,7 +82,7 @@ __global__ void __launch_bounds__(F64_THREADS, 1) f64_gemm_kernel(const F64Param
   __shared__ double red[32];
   __shared__ int last_flag;
 
-  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3);
+  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3 || EPI == EPI_P2);
   int tm, tn;
   if (SYM) tri_decode((int)blockIdx.x, tm, tn);
   else band_decode((int)blockIdx.x, p.tiles, p.tiles, 8, tm, tn);
@@ -150,10 +170,20 @@ __global__ void __launch_bounds__(F64_THREADS, 1) f64_gemm_kernel(const F64Param
         if (tm != tn) { p.out0[(size_t)n * ld + m] = v0; p.out0[(size_t)(n + 1) * ld + m] = v1; }
       } else if (EPI == EPI_A4) {
         const double2 r = *reinterpret_cast<const double2*>(p.in0 + m * ld + n);
-        v0 = 0.5 * r.x + 0.375 * v0;                 // Q = 1/2 R + 3/8 R R
-        v1 = 0.5 * r.y + 0.375 * v1;
+        v0 = p.pc.q_r * r.x + p.pc.q_d * v0;         // Q = 1/2 R + 3/8 R R   (m > 2: 1/2 R + P G)
+        v1 = p.pc.q_r * r.y + p.pc.q_d * v1;
         *reinterpret_cast<double2*>(p.out0 + m * ld + n) = make_double2(v0, v1);
         if (tm != tn) { p.out0[(size_t)n * ld + m] = v0; p.out0[(size_t)(n + 1) * ld + m] = v1; }
+      } else if (EPI == EPI_P2) {
+        const double2 r = *reinterpret_cast<const double2*>(p.in0 + m * ld + n);
+        const double g0 = (m == n ? p.pc.g_i : 0.0) + p.pc.g_r * r.x + p.pc.g_p * v0;      // G = 3/8 I + 5/16 R + g_p P
+        const double g1 = (m == n + 1 ? p.pc.g_i : 0.0) + p.pc.g_r * r.y + p.pc.g_p * v1;
+        *reinterpret_cast<double2*>(p.out0 + m * ld + n) = make_double2(v0, v1);            // P = R R
+        *reinterpret_cast<double2*>(p.out1 + m * ld + n) = make_double2(g0, g1);
+        if (tm != tn) {
+          p.out0[(size_t)n * ld + m] = v0; p.out0[(size_t)(n + 1) * ld + m] = v1;
+          p.out1[(size_t)n * ld + m] = g0; p.out1[(size_t)(n + 1) * ld + m] = g1;
+        }
       } else {  // EPI_A5
         const double2 z = *reinterpret_cast<const double2*>(p.in0 + m * ld + n);
         v0 += z.x;                                   // Z_next = Z + Z Q

@@ -88,6 +88,9 @@ struct UmmaParams {
   const float* f32_in;  // a4: R32          a5: Z32 current
   void* h_out;          // 16-bit modes: a1: T16   a2: R16   a4: Q16   a5: Z16 next  ([ARRAYS][Np][Np])
   void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
+  void* out2;           // p2 (order m > 2): G operand buffer, same format as the mode's operands
+  float q_r, q_d;       // a4: Q = q_r R + q_d D        (1/2, 3/8; m > 2: 1/2, 1)       see PolyCoef (zfac_f64.cuh)
+  float g_i, g_r, g_p;  // p2: G = g_i I + g_r R + g_p D (3/8, 5/16, 35/128 or 0)
   unsigned long long* dbg;  // -DZFAC_TIMING builds only: per-CTA wait-cycle counters of the MMA issuer (else null)
 };
 
@@ -290,7 +293,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
     float r32[SUB];
     load_f32_row<SUB>(p.f32_in + off, r32);
 #pragma unroll
-    for (int j = 0; j < SUB; ++j) v[j] = 0.5f * r32[j] + 0.375f * v[j];
+    for (int j = 0; j < SUB; ++j) v[j] = p.q_r * r32[j] + p.q_d * v[j];
     if (KIND == KIND_TF32) {
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
@@ -302,6 +305,32 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
     } else {
       store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
       if (offdiag) store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
+    }
+  } else if (EPI == EPI_P2) {                           // order m > 2: P = R R and G = 3/8 I + 5/16 R + g_p P, mirror
+    float g[SUB];
+    {
+      float r32[SUB];
+      load_f32_row<SUB>(p.f32_in + off, r32);
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) g[j] = ((m == n + j) ? p.g_i : 0.0f) + p.g_r * r32[j] + p.g_p * v[j];
+    }
+    if (KIND == KIND_TF32) {
+      float* g32 = static_cast<float*>(p.out2);
+#pragma unroll
+      for (int j = 0; j < SUB; ++j) { v[j] = round_tf32(v[j]); g[j] = round_tf32(g[j]); }
+      store_f32_row<SUB>(p.f32_out + off, v);
+      store_f32_row<SUB>(g32 + off, g);
+      if (offdiag) {
+#pragma unroll
+        for (int j = 0; j < SUB; ++j) { p.f32_out[offt + (size_t)j * ld] = v[j]; g32[offt + (size_t)j * ld] = g[j]; }
+      }
+    } else {
+      store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
+      store_h_row<PAIR, SUB>(p.out2, plane, off, g);
+      if (offdiag) {
+        store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
+        store_h_col<PAIR, SUB>(p.out2, plane, offt, ld, g);
+      }
     }
   } else {                                              // a5: Z_next = Z + Z Q, W = Z_next^T
     float z32[SUB];
@@ -335,7 +364,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   if (*((volatile int*)&p.st->done)) return;       // stop decided earlier in this call (uniform over the grid)
 
   using KT = KindTraits<KIND>;
-  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3);
+  constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3 || EPI == EPI_P2);
   constexpr bool PAIRK = (KIND == KIND_F16X2);                 // (hi, lo') operand pairs, promoted accumulation
   constexpr int TN = KT::TILE_N;
   constexpr int NSPLIT = UM_MACRO / TN;                        // column sub-tiles per 256-wide macro tile
@@ -692,6 +721,8 @@ struct UmmaPlan {
   int mode = 0;
   int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
   int chunk0_kb = 16; // first chunk of every tile (covers the previous tile's stores; partial sums still small)
+  int promote_update = 0;   // tuning knob (ZFAC_PROMOTE_UPDATE=1): promoted accumulation in the update GEMMs (p2, a4, a5)
+                            // too.  Measured to change Err[1] by 1.5e-5 relative only: off.
   // tensor maps of every operand buffer (box 128 B x 64 rows, 128B swizzle)
   CUtensorMap mS, mW, mT, mR, mQ, mZ[2];
 };
@@ -734,6 +765,7 @@ inline cudaError_t prepare_kind(int* max_pairs) {
   if ((e = prepare_kernel<KIND, EPI_A2>(max_pairs)) != cudaSuccess) return e;
   if ((e = prepare_kernel<KIND, EPI_X3>(max_pairs)) != cudaSuccess) return e;
   if ((e = prepare_kernel<KIND, EPI_A4>(max_pairs)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_P2>(max_pairs)) != cudaSuccess) return e;
   return prepare_kernel<KIND, EPI_A5>(max_pairs);
 }
 
@@ -741,6 +773,7 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0;
   if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knobs
   if (const char* ck = getenv("ZFAC_CHUNK0_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk0_kb = v; }
+  if (const char* ck = getenv("ZFAC_PROMOTE_UPDATE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->promote_update = v; }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -782,6 +815,7 @@ inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) 
     case EPI_A2: umma_gemm_kernel<KIND, EPI_A2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
     case EPI_X3: umma_gemm_kernel<KIND, EPI_X3><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
     case EPI_A4: umma_gemm_kernel<KIND, EPI_A4><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    case EPI_P2: umma_gemm_kernel<KIND, EPI_P2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
     default:     umma_gemm_kernel<KIND, EPI_A5><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
   }
 }
@@ -791,7 +825,7 @@ inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const 
   else umma_launch<KIND_TF32>(epi, grid, s, p);
 }
 
-inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, double* d_err, cudaStream_t s, int* launches, Prof* prof) {
+inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof) {
   const Layout& L = pl.L;
   char* ws = pl.ws;
   const int T = (int)(L.np / UM_MACRO);
@@ -808,6 +842,9 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
 #endif
   p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+  p.stop.order = order;
+  const PolyCoef pc = poly_coef(order);
+  p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.g_i = (float)pc.g_i; p.g_r = (float)pc.g_r; p.g_p = (float)pc.g_p;
   float* R32 = reinterpret_cast<float*>(ws + L.off_R);
   const bool h16 = (L.mode != ZFAC_MODE_TF32);
   int nl = 0;
@@ -828,9 +865,23 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, doubl
     nl += 2;
     if (n == max_iter) break;
     // a4: Q = 1/2 R + 3/8 R R^T   (the product is a correction of size |R|^2: no promotion needed)
+    if (pl.promote_update) { p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb; }
+    else { p.chunk_kb = 0; p.chunk0_kb = 0; }
+    if (order > 2) {
+      // order m > 2 (zfac.h, zfac_set_order): P = R R^T -> T buffer (free between a2 and the next a1),
+      // G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z operand buffer a5 is about to overwrite; then Q = 1/2 R + P G^T
+      prof->mark(s, EPI_P2 + 16 * n);
+      p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
+      if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; p.out2 = ws + L.off_Zb[(n + 1) & 1]; }
+      else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; p.out2 = ws + L.off_Z[(n + 1) & 1]; }
+      umma_launch_mode(L.mode, EPI_P2, grid_sym, s, p);
+      nl += 1;
+      p.out2 = nullptr;
+    }
     prof->mark(s, EPI_A4 + 16 * n);
-    p.chunk_kb = 0; p.chunk0_kb = 0;
-    p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
+    if (order > 2) { p.mapA = pl.mT; p.mapB = pl.mZ[(n + 1) & 1]; }
+    else { p.mapA = pl.mR; p.mapB = pl.mR; }
+    p.f32_in = R32;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr; }
     umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p);

@@ -20,6 +20,17 @@ pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-11, "split16": 1e-5, "tf32": 1e-3, "hh16": 1e-3}   # hh16: 11-bit operands like tf32
 DEV = "cuda:0"
+# Absolute noise of the history Err[n] = ||R_n||_F per sqrt(N).  SPLIT16: measured 7e-7 sqrt(N)
+# (||R_gpu - R_ora||_F = 1.05e-5 at N = 257, 1.9e-5 at N = 700, kappa = 20; 70 % of it on the diagonal: ~8 ulp of
+# truncation bias on X_ii ~ 1 inside a promoted chunk), allowed 3x.  F64: none.  TF32 / HH16: covered by rel.
+ERR_ABS = {"f64": 0.0, "split16": 2e-6, "tf32": 0.0, "hh16": 0.0}
+# ... never below 1e-12: F64 forms X ~ I to one ulp, ||R_gpu - R_ora||_F measured <= 7e-14 up to N = 700 (this is also
+# the absolute tolerance pytest.approx applies silently when only `rel` is given; here it is explicit)
+ERR_ABS_MIN = 1e-12
+
+
+def err_abs(mode, n):
+    return max(ERR_ABS_MIN, ERR_ABS[mode] * math.sqrt(n))
 
 
 def zb():
@@ -39,10 +50,13 @@ def _rel(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
-def gpu_refine(w, mode, max_iter, stop, keep=None):
+def gpu_refine(w, mode, max_iter, stop, keep=None, order=2):
     b = zb()
     S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
     with b.Zfac(w.n, mode, DEV) as zf:
+        if order != 2:
+            zf.set_order(order)
+            assert zf.order == order
         Z, iters, err, flags = zf.refine(S, Z0, max_iter=max_iter, stop=stop)
         peeks = {k: zf.peek(k).cpu().double().numpy() for k in (keep or [])}
         launches = zf.last_launch_count
@@ -102,8 +116,99 @@ def test_full_parity_same_iteration_count(mode, n):
     floor = {"f64": 1e-10, "split16": 1e-4, "tf32": 3e-2, "hh16": 3e-2}[mode] * max(1.0, math.sqrt(n))
     for k in range(it + 1):
         if ref.err[k] > floor:
-            assert err[k] == pytest.approx(ref.err[k], rel={"f64": 1e-8, "split16": 1e-3, "tf32": 5e-2, "hh16": 5e-2}[mode])
+            assert err[k] == pytest.approx(ref.err[k], rel={"f64": 1e-8, "split16": 1e-3, "tf32": 5e-2, "hh16": 5e-2}[mode],
+                                           abs=err_abs(mode, n))
     assert launches == 2 + 2 * 41 + 2 * 40                  # statically enqueued sequence
+
+
+# ------------------------------------------------------------------ higher orders m = 3, 4
+def _q_of_order(R, m):
+    """Q = sum_{k=1..m} c_k R^k, powers formed one by one (the oracle's order of operations)."""
+    c = O.order_coefficients(m)
+    Rk, Q = R, c[1] * R
+    for k in range(2, m + 1):
+        Rk = Rk @ R
+        Q = Q + c[k] * Rk
+    return Q
+
+
+@pytest.mark.parametrize("m", [3, 4])
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32", "hh16"])
+@pytest.mark.parametrize("n", [96, 300])
+def test_order_m_steps_against_oracle(mode, n, m):
+    """One update with m = 3, 4: the polynomial Q (two symmetric GEMMs on the GPU, regrouped as 1/2 R + P G)
+    and Z_1 against the oracle's term-by-term sum; non-symmetric Z0."""
+    b = zb()
+    w = W.random_spd_general(n, seed=5, kappa=20.0, pert=0.1, fp32_stored=True)
+    step_tol = {"f64": 1e-13, "split16": 2e-6, "tf32": 2e-3, "hh16": 2e-3}[mode]
+    Z, it, err, fl, pk, launches = gpu_refine(w, mode, 1, b.ZFAC_STOP_FIXED, keep=[b.ZFAC_BUF_Q], order=m)
+    R0 = O.residual(w.S, w.Z0)
+    Z1 = O.update_order_m(w.Z0, R0, m)
+    assert it == 1 and len(err) == 2 and fl == b.ZFAC_R_MAXITER
+    assert launches == 2 + 2 * 2 + 3                                     # copy-in/out, 2 residuals, (p2, a4, a5)
+    assert _rel(pk[b.ZFAC_BUF_Q], _q_of_order(R0, m)) < step_tol * 50
+    assert _rel(Z, Z1) < step_tol * 5
+    # the order is really m: the m = 2 update from the same start is measurably different
+    Z1_m2 = O.update_delta_form(w.Z0, R0)
+    assert _rel(Z, Z1) < 0.2 * _rel(Z1_m2, Z1) or mode in ("tf32", "hh16")
+    assert err[1] == pytest.approx(O.err_fro(O.residual(w.S, Z1)), rel=0.05,
+                                   abs={"f64": 1e-12, "split16": 1e-5, "tf32": 2e-2, "hh16": 2e-2}[mode] * math.sqrt(n))
+    assert not np.allclose(Z, Z.T)
+
+
+@pytest.mark.parametrize("m", [3, 4])
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32", "hh16"])
+@pytest.mark.parametrize("n", [17, 129, 257, 700])
+def test_order_m_full_parity_same_iteration_count(mode, n, m):
+    """Full runs with the generalised stop test Err[n] > Err[n-1]^(m+1), at tile-boundary sizes, against the oracle
+    run for the same number of updates with the same order."""
+    b = zb()
+    w = W.random_spd_general(n, seed=100 + n, kappa=20.0, pert=0.1, fp32_stored=True)
+    Z, it, err, fl, _, launches = gpu_refine(w, mode, 40, b.ZFAC_STOP_PAPER, order=m)
+    assert len(err) == it + 1 and it >= 1 and (fl & b.ZFAC_R_STOPPED)
+    ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED, order=m)
+    rel = _rel(Z, ref.Z)
+    nat = O.refine(w.S, w.Z0, 40, O.STOP_PAPER, order=m).iters
+    _, it2, _, _, _, _ = gpu_refine(w, mode, 40, b.ZFAC_STOP_PAPER)
+    print(f"[{mode} n={n} m={m}] iters={it} (m=2: {it2}; oracle natural stop {nat}) rel={rel:.3e} "
+          f"final Err/sqrtN={O.final_residual_per_sqrt_n(w.S, Z):.3e} launches={launches}")
+    tol = 2.5e-3 if (mode in ("tf32", "hh16") and n < 32) else TOL[mode]
+    assert rel <= tol
+    assert it <= it2                                                     # a higher order never needs more updates
+    floor = {"f64": 1e-10, "split16": 1e-4, "tf32": 3e-2, "hh16": 3e-2}[mode] * max(1.0, math.sqrt(n))
+    for k in range(it + 1):
+        if ref.err[k] > floor:
+            assert err[k] == pytest.approx(ref.err[k], rel={"f64": 1e-8, "split16": 1e-3, "tf32": 5e-2, "hh16": 5e-2}[mode],
+                                           abs=err_abs(mode, n))
+    assert launches == 2 + 2 * 41 + 3 * 40
+
+
+def test_order_m_invalid_and_default():
+    b = zb()
+    with b.Zfac(64, "f64", DEV) as zf:
+        assert zf.order == 2
+        for bad in (0, 1, 5, -3):
+            with pytest.raises(b.ZfacError):
+                zf.set_order(bad)
+            assert zf.order == 2                                         # the context keeps its order
+        zf.set_order(4)
+        assert zf.order == 4
+        zf.set_order(2)
+        assert zf.order == 2
+
+
+@pytest.mark.parametrize("m", [3, 4])
+def test_order_m_config2_n2048(m):
+    """BASELINE configs[1] (N = 2048 banded-decay overlap) with m = 3, 4 in SPLIT16 and F64: several tiles in both
+    directions, symmetric-output schedule with T = 8 macro tiles."""
+    b = zb()
+    w = W.config2(2048)
+    for mode in ("f64", "split16"):
+        Z, it, err, fl, _, _ = gpu_refine(w, mode, 40, b.ZFAC_STOP_PAPER, order=m)
+        ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED, order=m)
+        rel = _rel(Z, ref.Z)
+        print(f"[config2 N=2048 {mode} m={m}] iters={it} rel={rel:.3e} Err={np.array2string(err, precision=3)}")
+        assert (fl & b.ZFAC_R_STOPPED) and rel <= TOL[mode]
 
 
 # ------------------------------------------------------------------ stop rule
