@@ -186,7 +186,8 @@ def zfac_destroy(ctx: int) -> None:
 class Zfac:
     """Owns a torch uint8 workspace tensor and a zfac context for (n, mode) on the current device."""
 
-    def __init__(self, n: int, mode: str | int, device: str | torch.device = "cuda"):
+    def __init__(self, n: int, mode: str | int, device: str | torch.device = "cuda",
+                 workspace: Optional[torch.Tensor] = None):
         if not torch.cuda.is_available():
             raise RuntimeError("zfac needs a CUDA device (sm_100a); there is no CPU path")
         self.n = int(n)
@@ -196,9 +197,15 @@ class Zfac:
         nbytes = zfac_workspace_bytes(self.n, self.mode)
         if nbytes == 0:
             raise ZfacError(ZFAC_E_INVALID, "zfac_workspace_bytes")
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        if workspace is None:
+            workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        elif (workspace.dtype != torch.uint8 or workspace.dim() != 1 or not workspace.is_contiguous()
+              or workspace.device != self.device):
+            # size and 256-byte alignment are the library's to check (ZFAC_E_WORKSPACE)
+            raise ValueError("workspace: expected a contiguous 1-D uint8 tensor on the context's device")
+        self.workspace = workspace                      # caller-owned memory (the C ABI's ownership rule)
         with torch.cuda.device(self.device):
-            self.ctx = zfac_create(self.n, self.mode, self.workspace.data_ptr(), nbytes)
+            self.ctx = zfac_create(self.n, self.mode, self.workspace.data_ptr(), self.workspace.numel())
 
     def close(self) -> None:
         if getattr(self, "ctx", None):

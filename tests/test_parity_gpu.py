@@ -211,6 +211,76 @@ def test_order_m_config2_n2048(m):
         assert (fl & b.ZFAC_R_STOPPED) and rel <= TOL[mode]
 
 
+# ------------------------------------------------------------------ memory discipline (stand-ins for compute-sanitizer)
+# compute-sanitizer is closed on this GPU pool; these tests check what memcheck / initcheck would.
+GUARD = 1 << 20
+
+
+def _guarded_ctx(b, n, mode, fill):
+    """Workspace carved out of a larger buffer: [GUARD sentinel | workspace pre-filled with `fill` | GUARD sentinel]."""
+    nbytes = b.zfac_workspace_bytes(n, b.MODES[mode])
+    big = torch.full((GUARD + nbytes + GUARD,), 0xA5, dtype=torch.uint8, device=DEV)
+    assert big.data_ptr() % 256 == 0
+    ws = big[GUARD:GUARD + nbytes]
+    ws.fill_(fill)
+    return big, b.Zfac(n, mode, DEV, workspace=ws), nbytes
+
+
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32", "hh16"])
+@pytest.mark.parametrize("n", [129, 300, 4617 // 9])
+def test_no_write_outside_workspace_or_user_buffers(mode, n):
+    """Out-of-bounds WRITES: sentinel bands around the workspace and around a user Z with ld > n must survive
+    refine (orders 2 and 4), congruence and the host entry point.  n is never a tile multiple, so every kernel
+    works on padded tiles whose tails lie next to those bands."""
+    b = zb()
+    w = W.random_spd_general(n, seed=7, kappa=20.0, pert=0.1, fp32_stored=True)
+    S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
+    ld = n + 5
+    Zbig = torch.full((n + 2, ld), -777.0, dtype=_dt(mode), device=DEV)       # guard row above and below, 5 guard columns
+    Zv = Zbig[1:n + 1, :n]
+    big, zf, nbytes = _guarded_ctx(b, n, mode, 0x00)
+    with zf:
+        for m in (2, 4):
+            zf.set_order(m)
+            _, it, err, fl = zf.refine(S, Z0, max_iter=8, stop=b.ZFAC_STOP_PAPER, out=Zv)
+            assert fl & b.ZFAC_R_STOPPED
+        zf.set_order(2)
+        zf.congruence(S, Zv.contiguous())
+        hS, hZ0 = S.cpu().pin_memory(), Z0.cpu().pin_memory()
+        hZ = torch.empty_like(hZ0).pin_memory()
+        zf.refine_host(hS, hZ0, hZ, max_iter=2, stop=b.ZFAC_STOP_FIXED)
+        torch.cuda.synchronize()
+    assert bool((big[:GUARD] == 0xA5).all()) and bool((big[GUARD + nbytes:] == 0xA5).all())
+    assert bool((Zbig[0] == -777.0).all()) and bool((Zbig[n + 1] == -777.0).all()) and bool((Zbig[:, n:] == -777.0).all())
+    assert bool(torch.isfinite(Zv).all())
+
+
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32", "hh16"])
+@pytest.mark.parametrize("m", [2, 3])
+def test_result_independent_of_stale_workspace_contents(mode, m):
+    """Uninitialised READS: the same call on a workspace pre-filled with 0x00 and with 0xFF (NaN in fp16, fp32 and
+    fp64 alike) must give bit-identical Z, Err[] and flags -- any read of a byte the call did not write first would
+    differ or turn into NaN.  The second context re-uses the 0xFF memory after a first call, too (warm workspace)."""
+    b = zb()
+    n = 300
+    w = W.random_spd_general(n, seed=9, kappa=20.0, pert=0.1, fp32_stored=True)
+    S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
+    out = []
+    for fill in (0x00, 0xFF):
+        big, zf, _ = _guarded_ctx(b, n, mode, fill)
+        with zf:
+            zf.set_order(m)
+            for _ in range(2):
+                Z, it, err, fl = zf.refine(S, Z0, max_iter=10, stop=b.ZFAC_STOP_PAPER)
+                out.append((Z.clone(), it, err.copy(), fl))
+    Zr, itr, errr, flr = out[0]
+    assert bool(torch.isfinite(Zr).all()) and (flr & b.ZFAC_R_STOPPED)
+    for Z, it, err, fl in out[1:]:
+        assert it == itr and fl == flr
+        assert np.array_equal(err, errr)
+        assert torch.equal(Z, Zr)
+
+
 # ------------------------------------------------------------------ stop rule
 @pytest.mark.parametrize("mode", ["f64", "split16", "tf32"])
 def test_stop_rule_cases(mode):
