@@ -57,6 +57,8 @@ identity for non-symmetric Z0; Z -> S^-1/2 from a dense eigendecomposition when
 Z0 ∝ I; Z Z^T = S^-1 for non-commuting Z0; cubic order; stop-rule cases;
 scaling / permutation covariances; diagonal S reduces to N scalar recursions;
 `congruence` against the generalized eigenvalues of (H, S) from scipy.linalg.eigh.
+`spectral_closed_form` (N scalar recursions for Z0 = alpha I): against the matrix iteration of `refine` at N = 64
+and 256 (the two routes share only the coefficients), and against z -> lam^-1/2.
 Order m = 3, 4 (tests/test_oracle_order_pins.py): the coefficients re-derived in exact
 rationals from the vanishing condition alone; m = 2 mapped onto the printed a_k; the
 tail t_k > 0 with sum 1 and, for m = 2, equal to the printed c, d, e; a scalar
@@ -184,6 +186,43 @@ def refine(S: np.ndarray, Z0: np.ndarray, max_iter: int, stop: int = STOP_PAPER,
             raise ValueError(form)
         X = triple_product(S, Z)
     return RefineResult(Z, it, np.asarray(err, dtype=np.float64), flags)
+
+
+class SpectralResult(NamedTuple):
+    z: np.ndarray        # z_n per eigenvalue: Z_n = Q diag(z_n) Q^T
+    err: np.ndarray      # Err[0..iters] = (sum_i r_{n,i}^2)^(1/2)
+
+
+def spectral_closed_form(lam: np.ndarray, alpha: float, iters: int, order: int = 2) -> SpectralResult:
+    """The refinement for the special start Z0 = alpha I, written per eigenvalue.
+
+    With S = Q diag(lam) Q^T and Z0 = alpha I, every Z_n is a polynomial in S: Z_n = Q diag(z_n) Q^T, and
+    Eq. 13 / Eq. 16 decouple into N independent scalar recursions
+
+        r_i = 1 - lam_i z_i^2,      z_i <- z_i (1 + c_1 r_i + ... + c_m r_i^m),
+
+    with Err[n] = ||R_n||_F = (sum_i r_{n,i}^2)^(1/2) because Q is orthogonal.  No matrix is
+    formed: this is the parity reference at sizes where the matrix iteration is too slow (N = 16384), after ONE
+    N^3 reconstruction Q diag(z) Q^T by the caller.  Runs exactly `iters` updates (no stop test).  Exact only when
+    `lam` are the eigenvalues of the S actually used: for FP32-stored S they are perturbed by ~6e-8 ||S||."""
+    if order < 2 or order > 4:
+        raise ValueError("order must be 2, 3 or 4")
+    lam = np.asarray(lam, dtype=np.float64)
+    c = order_coefficients(order)
+    z = np.full(lam.shape, float(alpha), dtype=np.float64)
+    err = []
+    for n in range(iters + 1):
+        r = 1.0 - lam * z * z
+        err.append(math.sqrt(float(np.sum(r * r))))
+        if n == iters:
+            break
+        rk = r
+        q = c[1] * r
+        for k in range(2, order + 1):
+            rk = rk * r
+            q = q + c[k] * rk
+        z = z + z * q
+    return SpectralResult(z, np.asarray(err, dtype=np.float64))
 
 
 def refine_with_refi(S: np.ndarray, Z0: np.ndarray, max_iter: int, low_dtype=np.float32,
