@@ -177,6 +177,70 @@ def run_reference(args):
     return 0
 
 
+# ----------------------------------------------------------------------------- N sweep (BASELINE.json configs[4])
+def executed_tensor_flops(np_, updates, passes):
+    """Tensor flops one call EXECUTES on padded dimension Np: full GEMMs 2 Np^3 (a1 x (k+1), a5 x k),
+    symmetric ones Np^2 (Np + 256) (a2 x (k+1), a4 x k: upper triangle of 256-wide macro tiles), times the passes."""
+    full = 2.0 * np_ ** 3
+    sym = float(np_) ** 2 * (np_ + 256)
+    return passes * ((updates + 1) * (full + sym) + updates * (sym + full))
+
+
+def run_sweep(args, dev, peaks):
+    """configs[4]: N in {1024 .. 16384}, lambda in [1e-3, 1], Z0 = I/sqrt(lambda_max), FIXED 10 updates, per mode:
+    ms per call (median), FP32-equivalent TFLOP/s = (4 + 80) N^3 / t, executed tensor TFLOP/s and its fraction of the
+    mode's peak, next to S^-1/2 through cuSOLVER syevd (torch.linalg.eigh + scaling + one GEMM)."""
+    import torch
+    from paper_2404_19163_b200 import binding as zb, workloads as W
+    out = []
+    f64_peak = torch_gemm_peak(torch.float64, 8192, dev, reps=3)
+    peak_of = {"split16": peaks["bf16_burst"], "hh16": peaks["bf16_burst"], "tf32": peaks["bf16_burst"] * 0.5, "f64": f64_peak}
+    passes_of = {"split16": 3, "hh16": 1, "tf32": 1, "f64": 1}
+    for n in [int(x) for x in args.sweep_n.split(",")]:
+        w = W.config5(n, device=dev, fp32_stored=True)
+        row = {"N": n, "updates": 10, "modes": {}}
+        for mode in ("split16", "hh16", "tf32", "f64"):
+            dt = torch.float64 if mode == "f64" else torch.float32
+            S = torch.from_numpy(w.S).to(dev, dt); Z0 = torch.from_numpy(w.Z0).to(dev, dt)
+            Zout = torch.empty_like(Z0)
+            with zb.Zfac(n, mode, dev) as zf:
+                np_ = zb.zfac_padded_n(n, zb.MODES[mode])
+                for _ in range(2):
+                    zf.refine(S, Z0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=Zout, sync=False)
+                torch.cuda.synchronize(dev)
+                reps = 3 if (mode == "f64" and n >= 8192) else (7 if n >= 8192 else 25)
+                ts = []
+                for _ in range(reps):
+                    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    _, d_it, d_err, d_fl = zf.refine(S, Z0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=Zout, sync=False)
+                    e1.record(); torch.cuda.synchronize(dev)
+                    ts.append(e0.elapsed_time(e1))
+                ms = float(np.median(ts))
+                ex = executed_tensor_flops(np_, 10, passes_of[mode]) / (ms * 1e-3) / 1e12
+                row["modes"][mode] = {"ms_per_call": ms, "ms_best": float(min(ts)), "reps": reps, "N_padded": int(np_),
+                                      "tflops_fp32_equiv": flops_fp32_equiv(n, 10) / (ms * 1e-3) / 1e12,
+                                      "iters_per_s": 10.0 / (ms * 1e-3), "executed_tensor_tflops": ex,
+                                      "frac_of_peak": ex / peak_of[mode], "err_last": float(d_err[10].item())}
+            del S, Z0, Zout
+        for dtn, dt in (("f32", torch.float32), ("f64", torch.float64)):
+            try:
+                Sd = torch.from_numpy(w.S).to(dev, dt)
+                torch.cuda.synchronize(dev); t0 = time.perf_counter()
+                lam, V = torch.linalg.eigh(Sd)
+                Zr = (V / lam.clamp_min(1e-30).sqrt().unsqueeze(0)) @ V.T
+                torch.cuda.synchronize(dev)
+                row.setdefault("syevd_inv_sqrt_ms", {})[dtn] = (time.perf_counter() - t0) * 1e3
+                del Sd, lam, V, Zr
+            except Exception as ex_:  # reference point only
+                row.setdefault("syevd_inv_sqrt_ms", {})[dtn] = f"error: {str(ex_)[:80]}"
+        torch.cuda.empty_cache()
+        out.append(row)
+    return {"rows": out, "peaks_tflops": peak_of,
+            "peak_note": "split16/hh16: MEASURED_PEAKS bf16 burst (each call is timed alone); tf32: that x 0.5 (nominal ratio); "
+                         "f64: cuBLAS dgemm 8192^3 measured in this run"}
+
+
 # ----------------------------------------------------------------------------- our arm
 def time_refine(zf, S, Z0, Zout, max_iter, stop, steps, warmup, dev, profile=False, sampler=None, sync_fn=None):
     import torch
@@ -336,6 +400,9 @@ def run_ours(args):
             extra["syevd_inv_sqrt_ms"] = {"error": str(ex)[:100]}
     else:
         primary.pop("Z", None)
+    if rank == 0 and args.sweep:
+        torch.cuda.empty_cache()
+        extra["sweep"] = run_sweep(args, dev, peaks)
 
     # ---- aggregate over replicas: max time, sum of work
     units = flops_fp32_equiv(n, iters)
@@ -439,6 +506,9 @@ def main():
     ap.add_argument("--cpu-sample-n", type=int, default=8192)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick", action="store_true", help="primary mode only (no other modes / reference points)")
+    ap.add_argument("--sweep", action="store_true",
+                    help="also run the N sweep of BASELINE.json configs[4] (all modes, 10 fixed updates, syevd reference)")
+    ap.add_argument("--sweep-n", default="1024,2048,4096,8192,16384")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
