@@ -223,6 +223,30 @@ def run_sweep(args, dev, peaks):
                                       "iters_per_s": 10.0 / (ms * 1e-3), "executed_tensor_tflops": ex,
                                       "frac_of_peak": ex / peak_of[mode], "err_last": float(d_err[10].item())}
             del S, Z0, Zout
+        if n <= args.sweep_batch_max_n:
+            # many small problems at once: B contexts on B streams, no kernel change
+            row["concurrent"] = {}
+            for mode in ("split16", "f64"):
+                dt = torch.float64 if mode == "f64" else torch.float32
+                S = torch.from_numpy(w.S).to(dev, dt); Z0 = torch.from_numpy(w.Z0).to(dev, dt)
+                for B in (4, 8, 16):
+                    with zb.ZfacBatch(n, mode, B, dev) as zbatch:
+                        outs = [torch.empty_like(Z0) for _ in range(B)]
+                        zbatch.refine(S, Z0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=outs, sync=False); zbatch.wait()
+                        reps = 8
+                        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        for _ in range(reps):
+                            zbatch.refine(S, Z0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=outs, sync=False)
+                        cur = torch.cuda.current_stream(dev)
+                        for st in zbatch.streams:
+                            cur.wait_stream(st)
+                        e1.record(); torch.cuda.synchronize(dev)
+                        ms = e0.elapsed_time(e1) / (reps * B)
+                    row["concurrent"][f"{mode}_B{B}"] = {
+                        "ms_per_problem": ms, "tflops_fp32_equiv_aggregate": flops_fp32_equiv(n, 10) / (ms * 1e-3) / 1e12,
+                        "speedup_vs_alone": row["modes"][mode]["ms_per_call"] / ms}
+                del S, Z0
         for dtn, dt in (("f32", torch.float32), ("f64", torch.float64)):
             try:
                 Sd = torch.from_numpy(w.S).to(dev, dt)
@@ -509,6 +533,8 @@ def main():
     ap.add_argument("--sweep", action="store_true",
                     help="also run the N sweep of BASELINE.json configs[4] (all modes, 10 fixed updates, syevd reference)")
     ap.add_argument("--sweep-n", default="1024,2048,4096,8192,16384")
+    ap.add_argument("--sweep-batch-max-n", type=int, default=2048,
+                    help="sweep: also time B = 4, 8, 16 concurrent problems (ZfacBatch) for N up to this")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

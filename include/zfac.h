@@ -149,6 +149,13 @@ zfac_status zfac_refine_host(zfac_ctx* ctx, const void* h_S, int64_t lds, const 
  * d_out (n x n, ld).  Asynchronous on `stream`.  For tests of the individual steps. */
 zfac_status zfac_peek(zfac_ctx* ctx, zfac_buf which, void* d_out, int64_t ld, void* stream);
 
+/* Concurrency.  Contexts share no state (each owns its workspace and tensor maps; the last-error string is
+ * thread-local): calls on DIFFERENT contexts may be issued from different host threads and / or on different streams
+ * and run concurrently on the device; results are bit-identical to running them one after another.  This is the way
+ * to refine many small problems at once (the graph-partitioned sub-problems of PAPER.md:98): at n <= 1024 one
+ * problem's kernels cover 20-32 of the 148 SMs and 5-7 problems co-reside (profiles/r1c_sweep.md: 4.4-7.5x).
+ * Calls on the SAME context must not overlap (they share the workspace); issue them on one stream. */
+
 /* Order m of the refinement polynomial, Z_{n+1} = Z_n sum_{k=0..m} c_k R_n^k  (Eq. 13 / Eq. 16:
  * "Reference 1 gives a table with the coefficients a_k for polynomials of order m = 2, 3, 4, 5. For the tests in
  * this article, we use m = 2").  m = 2 (default; the paper's scheme), 3 or 4; anything else -> ZFAC_E_INVALID and

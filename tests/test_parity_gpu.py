@@ -211,6 +211,35 @@ def test_order_m_config2_n2048(m):
         assert (fl & b.ZFAC_R_STOPPED) and rel <= TOL[mode]
 
 
+# ------------------------------------------------------------------ concurrent small problems (batched small N)
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32"])
+def test_concurrent_contexts_on_streams_match_sequential_runs_bitwise(mode):
+    """ZfacBatch: B different problems, one context and one stream each, running concurrently.  Contexts share no
+    state, so every result must be BIT-identical to the same problem run alone (hidden shared state in the library
+    -- a static buffer, a shared tensor map, a common stop flag -- would show here), and match the oracle."""
+    b = zb()
+    n, B = 300, 6
+    ws = [W.random_spd_general(n, seed=40 + i, kappa=10.0 + 5 * i, pert=0.05 + 0.02 * i, fp32_stored=True) for i in range(B)]
+    Ss = [_to_dev(w.S, mode) for w in ws]
+    Z0s = [_to_dev(w.Z0, mode) for w in ws]
+    alone = []
+    for S, Z0 in zip(Ss, Z0s):
+        with b.Zfac(n, mode, DEV) as zf:
+            Z, it, err, fl = zf.refine(S, Z0, max_iter=20, stop=b.ZFAC_STOP_PAPER)
+            alone.append((Z.clone(), it, err.copy(), fl))
+    with b.ZfacBatch(n, mode, B, DEV) as zbatch:
+        for _ in range(3):                                               # repeated: warm workspaces, interleavings differ
+            res = zbatch.refine(Ss, Z0s, max_iter=20, stop=b.ZFAC_STOP_PAPER)
+            for (Z, it, err, fl), (Za, ita, erra, fla) in zip(res, alone):
+                assert it == ita and fl == fla and np.array_equal(err, erra)
+                assert torch.equal(Z, Za)
+    for i in range(1, B):                                                # the problems really differ from one another
+        assert not torch.equal(alone[i][0], alone[0][0]) and alone[i][2][0] != alone[0][2][0]
+    for w, (Z, it, err, fl) in zip(ws, alone):
+        ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+        assert _rel(Z.cpu().double().numpy(), ref.Z) <= TOL[mode]
+
+
 # ------------------------------------------------------------------ memory discipline (stand-ins for compute-sanitizer)
 # compute-sanitizer is closed on this GPU pool (DESIGN.md §6a); these tests check what memcheck / initcheck would.
 GUARD = 1 << 20
