@@ -271,11 +271,17 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
       store_f32_row<SUB>(p.f32_out + off, v);
     } else store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
   } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
+    // sum of squares: FP32 inside this group of SUB (16 / 32) columns, FP64 across groups, tiles and CTAs.  One DFMA
+    // plus one conversion per ELEMENT was 13 % of all warp samples of a2 (a quarter of its non-waiting time,
+    // profiles/r1b_summary.md §4); the entries of R carry ~6e-8 relative noise themselves, a 16-term FP32 partial
+    // sum adds <= 1e-6 relative per group, random in sign; the order is fixed, so Err[] stays run-to-run deterministic.
+    float ss = 0.0f;
 #pragma unroll
     for (int j = 0; j < SUB; ++j) {
       v[j] = ((m == n + j) ? 1.0f : 0.0f) - v[j];
-      tile_sumsq += (double)v[j] * (double)v[j];
+      ss = fmaf(v[j], v[j], ss);
     }
+    tile_sumsq += (double)ss;
     store_f32_row<SUB>(p.f32_out + off, v);
     if (KIND != KIND_TF32) store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
     if (offdiag) {
