@@ -811,6 +811,8 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = prepare_kind<KIND_TF32>(&pl->max_pairs)) != cudaSuccess) return e;
   }
   if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
+  // tuning knob: run on fewer CTA pairs (the power-cap experiment of profiles/r1c_sweep.md)
+  if (const char* ck = getenv("ZFAC_MAX_PAIRS")) { int v = atoi(ck); if (v >= 1 && v < pl->max_pairs) pl->max_pairs = v; }
   return cudaSuccess;
 }
 
