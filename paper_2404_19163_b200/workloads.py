@@ -250,15 +250,26 @@ def config4(n: int = 8192, eps: float = 1e-3, seed_q: int = 0, seed_e: int = 1, 
 # the paper's own synthetic workload (Eq. 39 / Eq. 40)
 # --------------------------------------------------------------------------
 
-def paper_eq39(n: int, gamma: float = 0.5) -> tuple[np.ndarray, np.ndarray, np.ndarray]:
+def paper_eq39(n: int, gamma: float = 0.5, device=None) -> tuple[np.ndarray, np.ndarray, np.ndarray]:
     """S~_ij = exp(-|i-j|/2) sin(i+1), 1<=i,j<=N (Eq. 39), read
     as symmetrised (S~ + S~^T)/2 because the printed form is not symmetric although
     the text calls it symmetric; S = S~ + (gamma - eps_1) I,
     gamma = 0.5 (PAPER.md:350).  Returns (S, eigenvalues, eigenvectors) -- the
-    eigendecomposition is the paper's own route to S^-1/2 for Z0."""
+    eigendecomposition is the paper's own route to S^-1/2 for Z0.
+    With `device` (and N >= 4096) the two eigendecompositions of the CONSTRUCTION run in FP64 through
+    torch.linalg on that device (minutes on the host at N = 16384); none of the method's arithmetic is here."""
     i = np.arange(1, n + 1, dtype=np.float64)
     St = np.exp(-np.abs(i[:, None] - i[None, :]) / 2.0) * np.sin(i + 1.0)[:, None]
     St = 0.5 * (St + St.T)
+    if _use_torch(device) and n >= 4096:
+        import torch
+        eps1 = float(torch.linalg.eigvalsh(torch.from_numpy(St).to(device))[0].item())
+        S = St + (gamma - eps1) * np.eye(n)
+        S = np.ascontiguousarray(0.5 * (S + S.T))
+        wt, Vt = torch.linalg.eigh(torch.from_numpy(S).to(device))
+        w, V = wt.cpu().numpy(), np.ascontiguousarray(Vt.cpu().numpy())
+        del wt, Vt
+        return S, w, V
     eps1 = float(np.linalg.eigvalsh(St)[0])
     S = St + (gamma - eps1) * np.eye(n)
     S = np.ascontiguousarray(0.5 * (S + S.T))
@@ -266,10 +277,10 @@ def paper_eq39(n: int, gamma: float = 0.5) -> tuple[np.ndarray, np.ndarray, np.n
     return S, w, V
 
 
-def paper_workload(n: int, alpha: float = 0.005, seed: int = 0, *, fp32_stored: bool = True) -> Workload:
+def paper_workload(n: int, alpha: float = 0.005, seed: int = 0, *, fp32_stored: bool = True, device=None) -> Workload:
     """Eq. 39 overlap with Z0 = S^-1/2 + alpha U (Eq. 40): NON-symmetric start."""
-    S, w, V = paper_eq39(n)
-    Sinvh = (V / np.sqrt(w)[None, :]) @ V.T
+    S, w, V = paper_eq39(n, device=device)
+    Sinvh = spectral_matrix(V, 1.0 / np.sqrt(w), device)
     Z0 = Sinvh + alpha * uniform_perturbation(n, seed)
     if fp32_stored:
         S = round_fp32(S)

@@ -8,6 +8,7 @@ SURVEY.md §8(c) "Tolerance feasibility") the test asserts the de
 and prints the measured value.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -623,6 +624,39 @@ def test_config5_n16384_against_spectral_closed_form():
     for k in range(11):
         if cf.err[k] > 1.0:
             assert err[k] == pytest.approx(cf.err[k], rel=5e-3), k
+
+
+def test_paper_eq39_workload_n16384_printed_stop_index_and_full_oracle_parity():
+    """The paper's own benchmark at its largest size (Eq. 39 / 40; Fig. 1): N = 16384, symmetrised
+    Eq. 39 overlap (reading Q14), NON-symmetric start Z0 = S^-1/2 + 0.005 U, split scheme, the paper's stop rule.
+    (i) The stop index the paper PRINTS: "for N = 16384, ratios of both norms exceed 1 at iteration number 4"
+    ("it takes 5" X evaluations) -- tests/golden/paper_stop_index.txt.
+    (ii) Element by element against the FULL matrix oracle run for the same 4 updates ((4 + 32) N^3 = 1.6e14 flop on
+    the host cores): this overlap is well conditioned (kappa ~ 8), so SPLIT16 is held to the north_star gate 1e-5 itself;
+    F64 is covered at this size by the config-5 test.  A transposed operand anywhere would show: Z is not symmetric."""
+    b = zb()
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "paper_stop_index.txt"))
+            if l.strip() and not l.startswith("#")]
+    n, alpha, stop_index = next((int(r[0]), float(r[1]), int(r[2])) for r in rows if int(r[0]) == 16384)
+    w = W.paper_workload(n, alpha=alpha, seed=0, fp32_stored=True, device=DEV)
+    assert np.linalg.norm(w.Z0 - w.Z0.T) / np.linalg.norm(w.Z0) > 1e-3
+    Z, it, err, fl, _, launches = gpu_refine(w, "split16", 20, b.ZFAC_STOP_PAPER)
+    print(f"[paper Eq. 39 N=16384 split16] iters={it} (printed stop index {stop_index}) flags={fl} "
+          f"Err={np.array2string(err, precision=4)}")
+    assert (fl & b.ZFAC_R_STOPPED) and it == stop_index and len(err) == stop_index + 1
+    for k in range(1, it):
+        assert err[k] <= err[k - 1] ** 3                                 # Eq. 38 holds until the printed index ...
+    assert err[it] > err[it - 1] ** 3                                    # ... and is violated there
+    ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+    rel = _rel(Z, ref.Z)
+    inv = O.final_residual_per_sqrt_n(w.S, Z)
+    print(f"[paper Eq. 39 N=16384 split16] rel vs oracle={rel:.3e} ||Z^T S Z - I||_F/sqrtN={inv:.3e} "
+          f"oracle Err={np.array2string(ref.err, precision=4)}")
+    assert rel <= TOL["split16"]
+    for k in range(it + 1):
+        if ref.err[k] > 1e-4 * math.sqrt(n):
+            assert err[k] == pytest.approx(ref.err[k], rel=1e-3, abs=err_abs("split16", n))
+    assert not np.allclose(Z, Z.T, rtol=0, atol=1e-6)
 
 
 # ------------------------------------------------------------------ BASELINE configs[2], configs[3] at FULL size
