@@ -149,7 +149,9 @@ def run_reference(args):
     t0 = time.perf_counter(); a @ a; t1 = time.perf_counter()
     gfs = 2 * 1024 ** 3 / (t1 - t0) / 1e9
     ns = args.n
-    while 4.0 * ns ** 3 / (gfs * 1e9) > 20.0 and ns > 1024:
+    # one step <= ~20 s AND the whole --steps K --warmup W run <= ~150 s of CPU work
+    per_step = min(20.0, 150.0 / max(1, args.steps + args.warmup))
+    while 4.0 * ns ** 3 / (gfs * 1e9) > per_step and ns > 256:
         ns //= 2
     S = np.ascontiguousarray(w.S[:ns, :ns]); Z0 = np.ascontiguousarray(w.Z0[:ns, :ns])
     for _ in range(args.warmup):
@@ -496,7 +498,7 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": {"split16": "f16/bf16 pairs, f32 accumulate", "tf32": "tf32, f32 accumulate", "f64": "f64"}[args.mode],
+            "dtype": {"split16": "f16 (hi + scaled-lo pairs), f32 accumulate", "tf32": "tf32, f32 accumulate", "f64": "f64"}[args.mode],
             "data": "synthetic",
             "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "N": n, "stop": args.stop,
                        "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
