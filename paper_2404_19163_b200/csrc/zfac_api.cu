@@ -11,6 +11,7 @@
 #include "zfac_io.cuh"
 #include "zfac_f64.cuh"
 #include "zfac_umma.cuh"
+#include "zfac_f64_tma.cuh"
 
 using namespace zfac;
 
@@ -36,6 +37,7 @@ struct zfac_ctx {
   int sm_count;
   int order;       // m of Eq. 13 (zfac_set_order): 2 (default), 3, 4
   UmmaPlan umma;   // tensor maps + launch geometry for the tcgen05 modes
+  F64Plan f64p;    // tensor maps of the FP64 buffers (ZFAC_MODE_F64)
   Prof prof;
 };
 
@@ -84,12 +86,18 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   c->n = n; c->np = L.np; c->mode = mode; c->ws = static_cast<char*>(d_workspace); c->ws_bytes = bytes;
   c->L = L; c->launches = 0; c->sm_count = sms; c->order = 2;
   if (mode == ZFAC_MODE_F64) {
-    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A1>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
-    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A2>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
-    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_X3>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
-    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A4>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
-    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_A5>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
-    ZF_CUDA(cudaFuncSetAttribute(f64_gemm_kernel<EPI_P2>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64_SMEM_BYTES));
+    cudaError_t e = f64_plan_create(&c->f64p, L, c->ws);
+    if (e == cudaSuccess) e = f64_tma_prepare<EPI_A1>();
+    if (e == cudaSuccess) e = f64_tma_prepare<EPI_A2>();
+    if (e == cudaSuccess) e = f64_tma_prepare<EPI_X3>();
+    if (e == cudaSuccess) e = f64_tma_prepare<EPI_A4>();
+    if (e == cudaSuccess) e = f64_tma_prepare<EPI_A5>();
+    if (e == cudaSuccess) e = f64_tma_prepare<EPI_P2>();
+    if (e != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "f64_plan_create: %s", cudaGetErrorString(e));
+      delete c;
+      return ZFAC_E_CUDA;
+    }
   } else {
     cudaError_t e = umma_plan_create(&c->umma, L, c->ws, sms);
     if (e != cudaSuccess) {
@@ -164,7 +172,9 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   double* Z[2] = {reinterpret_cast<double*>(ws + L.off_Z[0]), reinterpret_cast<double*>(ws + L.off_Z[1])};
   const int tiles = (int)(L.np / F64_BM);
   const int full = tiles * tiles, tri = tiles * (tiles + 1) / 2;
-  F64Params p{};
+  const F64Plan& fp = c->f64p;
+  F64TParams P{};
+  F64Params& p = P.q;
   p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = st;
   p.stop.st = st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
   p.stop.num_partials = tri; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
@@ -172,29 +182,29 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   p.pc = poly_coef(c->order);
   for (int n = 0; n <= max_iter; ++n) {
     if (n == max_iter && skip_last) break;
-    p.A = W; p.B = S; p.out0 = T; p.out1 = nullptr; p.in0 = nullptr;
+    P.mapA = fp.mW; P.mapB = fp.mS; p.out0 = T; p.out1 = nullptr; p.in0 = nullptr;          // a1: T = W S^T
     c->prof.mark(s, EPI_A1 + 16 * n);
-    f64_gemm_kernel<EPI_A1><<<full, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
-    p.A = W; p.B = T; p.out0 = R; p.stop.n_iter = n;
+    f64_tma_launch(EPI_A1, full, s, P);
+    P.mapA = fp.mW; P.mapB = fp.mT; p.out0 = R; p.stop.n_iter = n;                           // a2: R = I - W T^T
     c->prof.mark(s, EPI_A2 + 16 * n);
-    f64_gemm_kernel<EPI_A2><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    f64_tma_launch(EPI_A2, tri, s, P);
     c->launches += 2;
     if (n == max_iter) break;
     if (c->order > 2) {
       // order m > 2: P = R R -> T buffer, G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z buffer a5 overwrites next
-      p.A = R; p.B = R; p.in0 = R; p.out0 = T; p.out1 = Z[(n + 1) & 1];
+      P.mapA = fp.mR; P.mapB = fp.mR; p.in0 = R; p.out0 = T; p.out1 = Z[(n + 1) & 1];
       c->prof.mark(s, EPI_P2 + 16 * n);
-      f64_gemm_kernel<EPI_P2><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+      f64_tma_launch(EPI_P2, tri, s, P);
       c->launches += 1;
-      p.A = T; p.B = Z[(n + 1) & 1]; p.in0 = R; p.out0 = Q; p.out1 = nullptr;       // Q = 1/2 R + P G
+      P.mapA = fp.mT; P.mapB = fp.mZ[(n + 1) & 1]; p.in0 = R; p.out0 = Q; p.out1 = nullptr;  // Q = 1/2 R + P G
     } else {
-      p.A = R; p.B = R; p.in0 = R; p.out0 = Q;
+      P.mapA = fp.mR; P.mapB = fp.mR; p.in0 = R; p.out0 = Q;
     }
     c->prof.mark(s, EPI_A4 + 16 * n);
-    f64_gemm_kernel<EPI_A4><<<tri, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
-    p.A = Z[n & 1]; p.B = Q; p.in0 = Z[n & 1]; p.out0 = Z[(n + 1) & 1]; p.out1 = W;
+    f64_tma_launch(EPI_A4, tri, s, P);
+    P.mapA = fp.mZ[n & 1]; P.mapB = fp.mQ; p.in0 = Z[n & 1]; p.out0 = Z[(n + 1) & 1]; p.out1 = W;   // a5
     c->prof.mark(s, EPI_A5 + 16 * n);
-    f64_gemm_kernel<EPI_A5><<<full, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    f64_tma_launch(EPI_A5, full, s, P);
     c->launches += 2;
   }
   c->prof.mark(s, 0);
@@ -324,12 +334,13 @@ zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const voi
     double* W = reinterpret_cast<double*>(ws + L.off_W);
     double* T = reinterpret_cast<double*>(ws + L.off_T);
     const int tiles = (int)(L.np / F64_BM);
-    F64Params p{};
+    F64TParams P{};
+    F64Params& p = P.q;
     p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = reinterpret_cast<State*>(ws + L.off_state);
-    p.A = W; p.B = H; p.out0 = T;
-    f64_gemm_kernel<EPI_A1><<<tiles * tiles, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
-    p.A = W; p.B = T; p.out0 = reinterpret_cast<double*>(ws + L.off_R);
-    f64_gemm_kernel<EPI_X3><<<tiles * (tiles + 1) / 2, F64_THREADS, F64_SMEM_BYTES, s>>>(p);
+    P.mapA = c->f64p.mW; P.mapB = c->f64p.mS; p.out0 = T;                                   // H sits in the S buffer
+    f64_tma_launch(EPI_A1, tiles * tiles, s, P);
+    P.mapA = c->f64p.mW; P.mapB = c->f64p.mT; p.out0 = reinterpret_cast<double*>(ws + L.off_R);
+    f64_tma_launch(EPI_X3, tiles * (tiles + 1) / 2, s, P);
     c->launches += 2;
   } else {
     int nl = 0;
