@@ -448,7 +448,10 @@ def run_ours(args):
         elif args.mode == "tf32":
             peak, pk_name = peaks["bf16_sustained"] * 0.5, "bf16_tflops_sustained x 0.5 (nominal tf32:bf16 ratio)"
         else:
-            peak, pk_name = extra.get("cublas_tflops", {}).get("f64", 37.0), "cuBLAS dgemm 8192^3 measured in this run"
+            f64_peak = extra.get("cublas_tflops", {}).get("f64")
+            if f64_peak is None:                              # --quick: the reference rates were skipped; this one is needed
+                f64_peak = torch_gemm_peak(torch.float64, 8192, dev, reps=3)
+            peak, pk_name = f64_peak, "cuBLAS dgemm 8192^3 measured in this run"
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):

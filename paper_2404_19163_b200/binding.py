@@ -387,3 +387,38 @@ class ZfacBatch:
         for st in self.streams:
             cur.wait_stream(st)
         cur.synchronize()
+
+
+class ZfacGraph:
+    """One `zfac_refine` call captured into a CUDA graph (include/zfac.h, "CUDA graphs") and replayed.
+
+    The graph works on the tensors given here: write new S / Z0 contents INTO them (`S.copy_(...)`) and call
+    `replay()`.  Marshalling only: capture uses torch's graph API around the same C-ABI call `Zfac.refine` makes."""
+
+    def __init__(self, zf: Zfac, S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, stop: int = ZFAC_STOP_PAPER,
+                 out: Optional[torch.Tensor] = None):
+        zf._check(S, "S"); zf._check(Z0, "Z0")
+        self.zf, self.S, self.Z0, self.max_iter = zf, S, Z0, int(max_iter)
+        self.Z = out if out is not None else torch.empty((zf.n, zf.n), dtype=zf.dtype, device=S.device)
+        zf._check(self.Z, "Z")
+        self.d_iters = torch.zeros(1, dtype=torch.int32, device=S.device)
+        self.d_flags = torch.zeros(1, dtype=torch.int32, device=S.device)
+        self.d_err = torch.full((self.max_iter + 1,), float("nan"), dtype=torch.float64, device=S.device)
+        zf.set_profile(False)
+        side = torch.cuda.Stream(S.device)
+        side.wait_stream(torch.cuda.current_stream(S.device))
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=side):
+            zfac_refine(zf.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), self.Z.data_ptr(),
+                        self.Z.stride(0), self.max_iter, stop, self.d_iters.data_ptr(), self.d_err.data_ptr(),
+                        self.d_flags.data_ptr(), torch.cuda.current_stream(S.device).cuda_stream)
+        torch.cuda.current_stream(S.device).wait_stream(side)
+
+    def replay(self, sync: bool = True):
+        """Launch the captured call on the current stream.  sync=True: (Z, iters, err[0..iters], flags)."""
+        self.graph.replay()
+        if not sync:
+            return self.Z, self.d_iters, self.d_err, self.d_flags
+        torch.cuda.current_stream(self.S.device).synchronize()
+        it = int(self.d_iters.item())
+        return self.Z, it, self.d_err[: it + 1].cpu().numpy(), int(self.d_flags.item())

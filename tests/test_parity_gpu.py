@@ -241,6 +241,34 @@ def test_concurrent_contexts_on_streams_match_sequential_runs_bitwise(mode):
         assert _rel(Z.cpu().double().numpy(), ref.Z) <= TOL[mode]
 
 
+# ------------------------------------------------------------------ CUDA-graph capture (include/zfac.h, "CUDA graphs")
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32"])
+def test_refine_is_graph_capturable_and_replays_bitwise(mode):
+    """zfac_refine enqueues kernels only (no allocation, no host sync): it captures into a CUDA graph, and replays
+    are bit-identical to direct calls -- also after NEW inputs have been written into the captured buffers, with a
+    different stop index (the stop decision is taken on the device at replay time, not baked into the graph)."""
+    b = zb()
+    n = 300
+    w1 = W.random_spd_general(n, seed=21, kappa=20.0, pert=0.1, fp32_stored=True)
+    w2 = W.random_spd_general(n, seed=22, kappa=200.0, pert=0.02, fp32_stored=True)
+    S, Z0 = _to_dev(w1.S, mode), _to_dev(w1.Z0, mode)
+    with b.Zfac(n, mode, DEV) as zf:
+        zg = b.ZfacGraph(zf, S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+        seen = []
+        for w in (w1, w2, w1):
+            S.copy_(_to_dev(w.S, mode)); Z0.copy_(_to_dev(w.Z0, mode))
+            Zd, itd, errd, fld = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+            Zd = Zd.clone()
+            zg.Z.zero_()
+            Zr, itr, errr, flr = zg.replay()
+            assert itr == itd and flr == fld and np.array_equal(errr, errd)
+            assert torch.equal(Zr, Zd)
+            seen.append((itd, float(errd[0])))
+        assert seen[0] == seen[2] and seen[0][1] != seen[1][1]           # replays follow the inputs
+        ref = O.refine(w1.S, w1.Z0, seen[2][0], O.STOP_FIXED)
+        assert _rel(zg.Z.cpu().double().numpy(), ref.Z) <= TOL[mode]
+
+
 # ------------------------------------------------------------------ memory discipline (stand-ins for compute-sanitizer)
 # compute-sanitizer is closed on this GPU pool (DESIGN.md §6a); these tests check what memcheck / initcheck would.
 GUARD = 1 << 20
