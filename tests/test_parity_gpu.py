@@ -654,6 +654,41 @@ def test_config5_n16384_against_spectral_closed_form():
             assert err[k] == pytest.approx(cf.err[k], rel=5e-3), k
 
 
+@pytest.mark.skipif(os.environ.get("ZFAC_TEST_HUGE") != "1",
+                    reason="opt-in (ZFAC_TEST_HUGE=1): ~6 min and ~60 GB of host memory; result recorded in DESIGN.md §6b")
+def test_maximum_size_n32768_offsets_beyond_4gb():
+    """Maximum sizes: N = 32768, SPLIT16.  One FP32 matrix is 4.3 GB and the workspace 43 GB, so every byte offset in
+    the kernels, the copy-in / copy-out and the TMA maps crosses 2^31 and 2^32 -- a 32-bit offset anywhere would pass
+    every smaller test (at N = 16384 a matrix is 1.07 GB).  Config-5 recipe (lambda in [1e-3, 1], Z0 = I/sqrt(lambda_max)),
+    9 fixed updates (converged: the closed form's Err[8] is 2e-7); reference = the oracle's spectral closed form + one
+    host reconstruction; plus the oracle's invariant.
+    Rows and columns from all four corners are compared separately, so a wrap-around cannot hide in a norm."""
+    b = zb()
+    n, k = 32768, 9
+    w = W.config5(n, device=DEV, fp32_stored=True)
+    cf = O.spectral_closed_form(w.lam, w.alpha, k)
+    Z, it, err, fl, _, _ = gpu_refine(w, "split16", k, b.ZFAC_STOP_FIXED)
+    assert it == k and fl == b.ZFAC_R_MAXITER
+    Zref = (w.Q * cf.z) @ w.Q.T
+    rel = _rel(Z, Zref)
+    print(f"[config5 N=32768 split16, {k} updates] rel vs closed form={rel:.3e} Err={np.array2string(err, precision=4)} "
+          f"closed form={np.array2string(cf.err, precision=4)}")
+    assert rel <= 4.0 * 2.0 ** -24 * 1e3                                 # the u kappa bound of the N = 16384 test
+    for name, sl in (("top-left", (slice(0, 512), slice(0, 512))), ("top-right", (slice(0, 512), slice(n - 512, n))),
+                     ("bottom-left", (slice(n - 512, n), slice(0, 512))), ("bottom-right", (slice(n - 512, n), slice(n - 512, n))),
+                     ("centre", (slice(n // 2 - 256, n // 2 + 256), slice(n // 2 - 256, n // 2 + 256)))):
+        blk = np.linalg.norm(Z[sl] - Zref[sl]) / np.linalg.norm(Zref[sl])
+        print(f"    block {name}: rel {blk:.3e}")
+        assert blk <= 1e-3, name
+    for kk in range(k + 1):
+        if cf.err[kk] > 1.0:
+            assert err[kk] == pytest.approx(cf.err[kk], rel=5e-3), kk
+    del Zref
+    inv = O.final_residual_per_sqrt_n(w.S, Z)
+    print(f"    ||Z^T S Z - I||_F/sqrtN (oracle, FP64) = {inv:.3e} (reported Err[{k}]/sqrtN = {err[k] / math.sqrt(n):.3e})")
+    assert inv <= 1e-4                                                   # N = 16384: 2.0e-5
+
+
 def test_paper_eq39_workload_n16384_printed_stop_index_and_full_oracle_parity():
     """The paper's own benchmark at its largest size (Eq. 39 / 40; Fig. 1): N = 16384, symmetrised
     Eq. 39 overlap (reading Q14), NON-symmetric start Z0 = S^-1/2 + 0.005 U, split scheme, the paper's stop rule.
