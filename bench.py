@@ -180,12 +180,25 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------- N sweep (BASELINE.json configs[4])
-def executed_tensor_flops(np_, updates, passes):
+def hh_square_bound():
+    """SPLIT16: step a4 of an update taken from Err[n] <= this bound runs ONE pass instead of three (DESIGN.md §5,
+    "One pass for the second-order product"; same default and environment knobs as zfac_umma.cuh)."""
+    if os.environ.get("ZFAC_HH_SQUARE", "1") == "0":
+        return -1.0
+    return float(os.environ.get("ZFAC_HH_SQUARE_ERR", "0.1"))
+
+
+def executed_tensor_flops(np_, updates, passes, err=None):
     """Tensor flops one call EXECUTES on padded dimension Np: full GEMMs 2 Np^3 (a1 x (k+1), a5 x k),
-    symmetric ones Np^2 (Np + 256) (a2 x (k+1), a4 x k: upper triangle of 256-wide macro tiles), times the passes."""
+    symmetric ones Np^2 (Np + 256) (a2 x (k+1), a4 x k: upper triangle of 256-wide macro tiles), times the passes.
+    `err` (SPLIT16): the Err[] history of the call -- a4 of update n counts one pass where Err[n] <= hh_square_bound()."""
     full = 2.0 * np_ ** 3
     sym = float(np_) ** 2 * (np_ + 256)
-    return passes * ((updates + 1) * (full + sym) + updates * (sym + full))
+    a4_passes = float(passes * updates)
+    if passes == 3 and err is not None:
+        b = hh_square_bound()
+        a4_passes = float(sum(1 if (float(err[n]) <= b) else 3 for n in range(updates)))
+    return passes * ((updates + 1) * (full + sym) + updates * full) + a4_passes * sym
 
 
 def run_sweep(args, dev, peaks):
@@ -219,7 +232,8 @@ def run_sweep(args, dev, peaks):
                     e1.record(); torch.cuda.synchronize(dev)
                     ts.append(e0.elapsed_time(e1))
                 ms = float(np.median(ts))
-                ex = executed_tensor_flops(np_, 10, passes_of[mode]) / (ms * 1e-3) / 1e12
+                hist = d_err[:11].cpu().numpy() if mode == "split16" else None
+                ex = executed_tensor_flops(np_, 10, passes_of[mode], hist) / (ms * 1e-3) / 1e12
                 row["modes"][mode] = {"ms_per_call": ms, "ms_best": float(min(ts)), "reps": reps, "N_padded": int(np_),
                                       "tflops_fp32_equiv": flops_fp32_equiv(n, 10) / (ms * 1e-3) / 1e12,
                                       "iters_per_s": 10.0 / (ms * 1e-3), "executed_tensor_tflops": ex,

@@ -89,6 +89,8 @@ struct UmmaParams {
   void* h_out;          // 16-bit modes: a1: T16   a2: R16   a4: Q16   a5: Z16 next  ([ARRAYS][Np][Np])
   void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
   void* out2;           // p2 (order m > 2): G operand buffer, same format as the mode's operands
+  int hh_only;          // KIND_F16X2: 1 = this launch MAY use the (h)(h) pass only (D_x neither written nor read) ...
+  double hh_err_max;    // ... and does so iff Err[n] = stop.d_err[stop.n_iter] <= hh_err_max (decided on the device)
   float q_r, q_d;       // a4: Q = q_r R + q_d D        (1/2, 3/8; m > 2: 1/2, 1)       see PolyCoef (zfac_f64.cuh)
   float g_i, g_r, g_p;  // p2: G = g_i I + g_r R + g_p D (3/8, 5/16, 35/128 or 0)
   unsigned long long* dbg;  // -DZFAC_TIMING builds only: per-CTA wait-cycle counters of the MMA issuer (else null)
@@ -411,6 +413,9 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int NCH = 1 + (KB - CH0 + CH - 1) / CH;                            // chunks per tile
   const int T = p.macro_tiles;
   const int num_tiles = (SYM ? T * (T + 1) / 2 : T * T) * NSPLIT;         // 256 x TN pair tiles
+  // One pass for a second-order product (a4 / p2, KIND_F16X2): taken by every thread of the grid from the Err[n] that
+  // a2 of this iteration wrote (a completed kernel: visible), so issuer and epilogues of both CTAs agree.
+  const bool hh_only = PAIRK && p.hh_only && (__ldcg(p.stop.d_err + p.stop.n_iter) <= p.hh_err_max);
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
@@ -522,6 +527,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
             tc_fence_after();
           };
           auto issue_cross = [&](int j) {
+            if (hh_only) return;                               // second-order product (a4 / p2): (h)(h) pass only
             uint64_t a_hi, a_lo, b_hi, b_lo; sdescs(j, a_hi, a_lo, b_hi, b_lo);
 #pragma unroll
             for (int k = 0; k < KSTEPS; ++k) {
@@ -639,13 +645,15 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 #ifdef ZFAC_TIMING
         const long long te0 = clock64();
 #endif
+        if (!hh_only) {
 #pragma unroll
-        for (int i = 0; i < GCOLS / 32; ++i) {
-          uint32_t x[32];
-          tmem_ld(tbase + TN + i * 32, x);
-          tmem_ld_wait();
+          for (int i = 0; i < GCOLS / 32; ++i) {
+            uint32_t x[32];
+            tmem_ld(tbase + TN + i * 32, x);
+            tmem_ld_wait();
 #pragma unroll
-          for (int j = 0; j < 32; ++j) sum[i * 32 + j] += __uint_as_float(x[j]) * LO_UNSCALE;
+            for (int j = 0; j < 32; ++j) sum[i * 32 + j] += __uint_as_float(x[j]) * LO_UNSCALE;
+          }
         }
         tc_fence_before();
         __syncwarp();
@@ -727,6 +735,9 @@ struct UmmaPlan {
   int mode = 0;
   int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
   int chunk0_kb = 16; // first chunk of every tile (covers the previous tile's stores; partial sums still small)
+  int hh_square = 1;        // SPLIT16: the second-order products of step a4 (R R; P G for m > 2) use the (h)(h) pass only
+  double hh_err_max = 0.1;  // ... for updates taken from Err[n] <= this (DESIGN.md §5 "One pass for the second-order
+                            // product"); ZFAC_HH_SQUARE=0 restores three passes everywhere, ZFAC_HH_SQUARE_ERR sets the bound
   int promote_update = 0;   // tuning knob (ZFAC_PROMOTE_UPDATE=1): promoted accumulation in the update GEMMs (p2, a4, a5)
                             // too.  Measured to change Err[1] by 1.5e-5 relative only: off.
   // tensor maps of every operand buffer (box 128 B x 64 rows, 128B swizzle)
@@ -779,6 +790,8 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0;
   if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knobs
   if (const char* ck = getenv("ZFAC_CHUNK0_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk0_kb = v; }
+  if (const char* ck = getenv("ZFAC_HH_SQUARE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->hh_square = v; }
+  if (const char* ck = getenv("ZFAC_HH_SQUARE_ERR")) { double v = atof(ck); if (v >= 0.0) pl->hh_err_max = v; }
   if (const char* ck = getenv("ZFAC_PROMOTE_UPDATE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->promote_update = v; }
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -875,6 +888,8 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
     // a4: Q = 1/2 R + 3/8 R R^T   (the product is a correction of size |R|^2: no promotion needed)
     if (pl.promote_update) { p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb; }
     else { p.chunk_kb = 0; p.chunk0_kb = 0; }
+    p.hh_only = (L.mode == ZFAC_MODE_SPLIT16 && pl.hh_square) ? 1 : 0;      // p2 and a4 only; a5 below needs all passes
+    p.hh_err_max = pl.hh_err_max;
     if (order > 2) {
       // order m > 2 (zfac.h, zfac_set_order): P = R R^T -> T buffer (free between a2 and the next a1),
       // G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z operand buffer a5 is about to overwrite; then Q = 1/2 R + P G^T
@@ -893,7 +908,8 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr; }
     umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p);
-    // a5: Z_next = Z + Z Q^T ; W = Z_next^T
+    // a5: Z_next = Z + Z Q^T ; W = Z_next^T   (first order in R: all three passes)
+    p.hh_only = 0;
     prof->mark(s, EPI_A5 + 16 * n);
     p.mapA = pl.mZ[n & 1]; p.mapB = pl.mQ;
     if (h16) {

@@ -241,6 +241,35 @@ def test_concurrent_contexts_on_streams_match_sequential_runs_bitwise(mode):
         assert _rel(Z.cpu().double().numpy(), ref.Z) <= TOL[mode]
 
 
+# ------------------------------------------------------------------ one pass for the second-order product
+@pytest.mark.parametrize("case", ["config2_n2048", "general_n700"])
+def test_one_pass_square_below_the_err_bound_does_not_change_z(case, monkeypatch):
+    """SPLIT16 runs a4's product R R with the (h)(h) pass only for updates taken from Err[n] <= 0.1.  A/B against three
+    passes everywhere (ZFAC_HH_SQUARE=0; the knobs are read when a context is created): same stop index, Z agrees with
+    the oracle equally well (the bound is where the surviving rotation 9e-5 Err^3 drops below 2^-23), and the two
+    results differ by less than the gate -- while WITHOUT the bound (ZFAC_HH_SQUARE_ERR=1e9) Z is measurably worse."""
+    b = zb()
+    w = W.config2(2048) if case == "config2_n2048" else W.random_spd_general(700, seed=800, kappa=20.0, pert=0.1, fp32_stored=True)
+    out = {}
+    for name, env in (("three", {"ZFAC_HH_SQUARE": "0"}), ("default", {}), ("unbounded", {"ZFAC_HH_SQUARE_ERR": "1e9"})):
+        for k in ("ZFAC_HH_SQUARE", "ZFAC_HH_SQUARE_ERR"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        Z, it, err, fl, _, _ = gpu_refine(w, "split16", 40, b.ZFAC_STOP_PAPER)
+        out[name] = (Z, it, err)
+    it = out["three"][1]
+    assert out["default"][1] == it and (out["default"][2][:-1] <= 0.1).any()      # the bound really applied somewhere
+    ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+    r3, rd = _rel(out["three"][0], ref.Z), _rel(out["default"][0], ref.Z)
+    ru = _rel(out["unbounded"][0], O.refine(w.S, w.Z0, out["unbounded"][1], O.STOP_FIXED).Z)
+    print(f"[{case}] rel vs oracle: three passes {r3:.3e}, default bound {rd:.3e}, unbounded {ru:.3e}")
+    assert rd <= TOL["split16"] and rd <= 1.05 * r3 + 1e-8
+    assert _rel(out["default"][0], out["three"][0]) <= 2e-7
+    if case == "config2_n2048":
+        assert ru > 10.0 * rd                                                     # the bound is what protects Z
+
+
 # ------------------------------------------------------------------ CUDA-graph capture (include/zfac.h, "CUDA graphs")
 @pytest.mark.parametrize("mode", ["f64", "split16", "tf32"])
 def test_refine_is_graph_capturable_and_replays_bitwise(mode):
