@@ -52,8 +52,9 @@ typedef struct zfac_ctx zfac_ctx; /* opaque */
  *  HH16   : the paper's (h)(h) scheme (Sec. III.C; Table I :211): operands
  *           rounded to FP16, one tensor-core pass, FP32 accumulation; meant to be followed by
  *           the refinement step (zfac_refine_refi).
- *           In SPLIT16 the second-order product of step a4 (R R) runs its (h)(h) pass only when the update is taken
- *           from Err[n] <= 0.1 (decided on the device); the effect on Z is below FP32 resolution. */
+ * Note on SPLIT16: the second-order product of step a4 (R R in Q = 1/2 R + 3/8 R R) runs its (h)(h) pass only when
+ * the update is taken from Err[n] <= 0.1 (decided on the device from the Err[n] just computed); the effect on Z is
+ * below FP32 resolution, every other product always runs all three passes. */
 typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2, ZFAC_MODE_HH16 = 3 } zfac_mode;
 
 /* Stop rule.  PAPER: Alg. 2's parameter-free test.  FIXED: perform exactly max_iter updates
