@@ -89,6 +89,7 @@ struct UmmaParams {
   void* h_out;          // 16-bit modes: a1: T16   a2: R16   a4: Q16   a5: Z16 next  ([ARRAYS][Np][Np])
   void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
   void* out2;           // p2 (order m > 2): G operand buffer, same format as the mode's operands
+  int band;             // full outputs: tile columns per rasterisation band (L2 reuse of the B column blocks)
   int hh_only;          // KIND_F16X2: 1 = this launch MAY use the (h)(h) pass only (D_x neither written nor read) ...
   double hh_err_max;    // ... and does so iff Err[n] = stop.d_err[stop.n_iter] <= hh_err_max (decided on the device)
   float q_r, q_d;       // a4: Q = q_r R + q_d D        (1/2, 3/8; m > 2: 1/2, 1)       see PolyCoef (zfac_f64.cuh)
@@ -446,7 +447,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       n0 = J * UM_MACRO + sub * TN;
       offdiag = (I != J);
     } else {
-      band_decode(t, T, T * NSPLIT, 8 * NSPLIT, I, J);
+      band_decode(t, T, T * NSPLIT, p.band * NSPLIT, I, J);
       n0 = J * TN;
       offdiag = true;                                      // (unused by the full-output epilogues)
     }
@@ -735,6 +736,7 @@ struct UmmaPlan {
   int mode = 0;
   int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
   int chunk0_kb = 16; // first chunk of every tile (covers the previous tile's stores; partial sums still small)
+  int band = 8;             // rasterisation band width of the full GEMMs, in tile columns (tuning knob ZFAC_BAND)
   int hh_square = 1;        // SPLIT16: the second-order products of step a4 (R R; P G for m > 2) use the (h)(h) pass only
   double hh_err_max = 0.1;  // ... for updates taken from Err[n] <= this (DESIGN.md §5 "One pass for the second-order
                             // product"); ZFAC_HH_SQUARE=0 restores three passes everywhere, ZFAC_HH_SQUARE_ERR sets the bound
@@ -790,6 +792,7 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0;
   if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knobs
   if (const char* ck = getenv("ZFAC_CHUNK0_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk0_kb = v; }
+  if (const char* ck = getenv("ZFAC_BAND")) { int v = atoi(ck); if (v >= 1 && v <= 4096) pl->band = v; }
   if (const char* ck = getenv("ZFAC_HH_SQUARE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->hh_square = v; }
   if (const char* ck = getenv("ZFAC_HH_SQUARE_ERR")) { double v = atof(ck); if (v >= 0.0) pl->hh_err_max = v; }
   if (const char* ck = getenv("ZFAC_PROMOTE_UPDATE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->promote_update = v; }
@@ -856,7 +859,7 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
   const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
   const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T;
+  p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
 #ifdef ZFAC_TIMING
   p.dbg = reinterpret_cast<unsigned long long*>(ws + L.off_dbg);
@@ -938,7 +941,7 @@ inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* laun
   const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
   const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T; p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
+  p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band; p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
   const bool h16 = (L.mode != ZFAC_MODE_TF32);
   p.mapA = pl.mW; p.mapB = pl.mS;
