@@ -38,6 +38,8 @@ struct zfac_ctx {
   int order;       // m of Eq. 13 (zfac_set_order): 2 (default), 3, 4
   UmmaPlan umma;   // tensor maps + launch geometry for the tcgen05 modes
   F64Plan f64p;    // tensor maps of the FP64 buffers (ZFAC_MODE_F64)
+  cudaStream_t side = nullptr;                 // zfac_refine_host: stream of the speculative copy-out (created lazily)
+  cudaEvent_t ev_a5 = nullptr, ev_copy = nullptr;
   Prof prof;
 };
 
@@ -112,6 +114,9 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
 
 zfac_status zfac_destroy(zfac_ctx* ctx) {
   if (ctx) {
+    if (ctx->ev_a5) cudaEventDestroy(ctx->ev_a5);
+    if (ctx->ev_copy) cudaEventDestroy(ctx->ev_copy);
+    if (ctx->side) cudaStreamDestroy(ctx->side);
     for (int i = 0; i < ctx->prof.cap; ++i) cudaEventDestroy(ctx->prof.ev[i]);
     delete[] ctx->prof.ev;
     delete[] ctx->prof.tags;
@@ -160,12 +165,11 @@ int zfac_get_order(const zfac_ctx* c) { return c ? c->order : 0; }
 
 // skip_last: Alg. 3 as printed ends after the update, without evaluating the residual of the result.
 static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s,
-                              bool skip_last = false) {
+                              bool skip_last = false, const IterHook* hook = nullptr) {
   const Layout& L = c->L;
   char* ws = c->ws;
   State* st = reinterpret_cast<State*>(ws + L.off_state);
-  double* S = reinterpret_cast<double*>(ws + L.off_S);
-  double* W = reinterpret_cast<double*>(ws + L.off_W);
+  double* W = reinterpret_cast<double*>(ws + L.off_W);          // epilogue pointers; the operands go through tensor maps
   double* T = reinterpret_cast<double*>(ws + L.off_T);
   double* R = reinterpret_cast<double*>(ws + L.off_R);
   double* Q = reinterpret_cast<double*>(ws + L.off_Q);
@@ -205,6 +209,7 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
     P.mapA = fp.mZ[n & 1]; P.mapB = fp.mQ; p.in0 = Z[n & 1]; p.out0 = Z[(n + 1) & 1]; p.out1 = W;   // a5
     c->prof.mark(s, EPI_A5 + 16 * n);
     f64_tma_launch(EPI_A5, full, s, P);
+    if (hook) hook->after_a5(hook->self, n, s);
     c->launches += 2;
   }
   c->prof.mark(s, 0);
@@ -256,9 +261,9 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
   c->launches += 1;
 }
 
-zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
-                        int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
-                        void* stream) {
+static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
+                               int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
+                               void* stream, const IterHook* hook) {
   if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
   if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
   if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
@@ -272,10 +277,10 @@ zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d
 
   zfac_status rs;
   if (c->mode == ZFAC_MODE_F64) {
-    rs = refine_f64(c, max_iter, stop, d_err, s);
+    rs = refine_f64(c, max_iter, stop, d_err, s, false, hook);
   } else {
     int nl = 0;
-    cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, c->order, d_err, s, &nl, &c->prof);
+    cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, c->order, d_err, s, &nl, &c->prof, hook);
     c->launches += nl;
     if (e != cudaSuccess) {
       snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_refine: %s", cudaGetErrorString(e));
@@ -288,6 +293,37 @@ zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d
   launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, s);
   ZF_CUDA(cudaGetLastError());
   return ZFAC_OK;
+}
+
+zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
+                        int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
+                        void* stream) {
+  return refine_impl(c, d_S, lds, d_Z0, ldz0, d_Z, ldz, max_iter, stop, d_iters, d_err, d_flags, stream, nullptr);
+}
+
+// zfac_refine_host, pinned h_Z: the download of Z starts right after the FIRST update (a5 of iteration 0 always runs when
+// max_iter >= 1) on a side stream, with the copy engine, straight from the internal buffer.  If that update turns out
+// to be the only one -- the warm-start case -- the download has overlapped the final residual evaluation (a1 + a2), which
+// the caller would otherwise wait for before the download even starts.  If more updates ran it is superseded by the
+// normal download at the end; PCIe and the copy engine were idle anyway, so it cost nothing on the critical path.
+// (A device-predicated copy KERNEL after every a5 was built and measured first: SM stores into mapped host memory reach
+// ~31 GB/s where the copy engine reaches 54; it made the call slower.  DESIGN.md §7.)
+struct HostOverlap {
+  zfac_ctx* c;
+  void* h_Z;
+  int64_t ldz;
+};
+static void host_after_a5(void* self, int n, cudaStream_t s) {
+  if (n != 0) return;
+  HostOverlap* h = static_cast<HostOverlap*>(self);
+  zfac_ctx* c = h->c;
+  const Layout& L = c->L;
+  const char* src = c->ws + L.off_Z[1];           // Z_1: buffer 1 (F64 / TF32); the 16-bit modes update one FP32 master in place
+  cudaEventRecord(c->ev_a5, s);
+  cudaStreamWaitEvent(c->side, c->ev_a5, 0);
+  cudaMemcpy2DAsync(h->h_Z, (size_t)h->ldz * L.elt, src, (size_t)L.np * L.elt, (size_t)c->n * L.elt, (size_t)c->n,
+                    cudaMemcpyDeviceToHost, c->side);
+  cudaEventRecord(c->ev_copy, c->side);
 }
 
 zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* f64, const void* d_S, int64_t lds, const void* d_Z0,
@@ -330,8 +366,6 @@ zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const voi
   c->prof.count = 0;
   launch_copy_in(c, d_H, ldh, d_Z, ldz, false, s);        // H takes the place of S; W = Z^T
   if (c->mode == ZFAC_MODE_F64) {
-    double* H = reinterpret_cast<double*>(ws + L.off_S);
-    double* W = reinterpret_cast<double*>(ws + L.off_W);
     double* T = reinterpret_cast<double*>(ws + L.off_T);
     const int tiles = (int)(L.np / F64_BM);
     F64TParams P{};
@@ -370,13 +404,36 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   const size_t row = (size_t)c->n * L.elt;
   ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
   ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
-  zfac_status rs = zfac_refine(c, dS, c->n, dZ, c->n, dZ, c->n, max_iter, stop, dInts, dErr, dInts + 1, s);
+  // overlapped download: needs a pinned (device-visible) h_Z and at least one possible update
+  bool z_dev = false;                             // early download possible: pinned h_Z (an async copy from pageable memory
+  {                                               // is staged and may block) and at least one possible update
+    cudaPointerAttributes pa{};
+    const char* off = getenv("ZFAC_HOST_OVERLAP");
+    if (max_iter >= 1 && !(off && off[0] == '0') && cudaPointerGetAttributes(&pa, h_Z) == cudaSuccess &&
+        pa.type == cudaMemoryTypeHost)
+      z_dev = true;
+    (void)cudaGetLastError();
+  }
+  HostOverlap ho{c, h_Z, ldz};
+  IterHook hook{host_after_a5, &ho};
+  if (z_dev) {
+    if (!c->side) {
+      ZF_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+      ZF_CUDA(cudaEventCreateWithFlags(&c->ev_a5, cudaEventDisableTiming));
+      ZF_CUDA(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
+    }
+  }
+  zfac_status rs = refine_impl(c, dS, c->n, dZ, c->n, dZ, c->n, max_iter, stop, dInts, dErr, dInts + 1, s,
+                               z_dev ? &hook : nullptr);
   if (rs != ZFAC_OK) return rs;
-  ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
+  if (z_dev) ZF_CUDA(cudaStreamWaitEvent(s, c->ev_copy, 0));   // the early download is complete (and can no longer land late)
+  else ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
   int ints[2] = {0, 0};
   ZF_CUDA(cudaMemcpyAsync(ints, dInts, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaStreamSynchronize(s));
   *h_iters = ints[0]; *h_flags = ints[1];
+  if (z_dev && ints[0] != 1)       // the early download holds Z_1: final only if exactly one update ran
+    ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaMemcpyAsync(h_err, dErr, (size_t)(ints[0] + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaStreamSynchronize(s));
   return ZFAC_OK;

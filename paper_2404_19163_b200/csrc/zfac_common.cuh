@@ -43,6 +43,13 @@ struct Prof {
   }
 };
 
+// Host-side hook after step a5 of every statically enqueued iteration (zfac_refine_host starts the download of Z
+// after the first update through it).
+struct IterHook {
+  void (*after_a5)(void* self, int n, cudaStream_t s);
+  void* self;
+};
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -849,7 +849,8 @@ inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const 
   else umma_launch<KIND_TF32>(epi, grid, s, p);
 }
 
-inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof) {
+inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof,
+                               const IterHook* hook = nullptr) {
   const Layout& L = pl.L;
   char* ws = pl.ws;
   const int T = (int)(L.np / UM_MACRO);
@@ -923,6 +924,7 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
       p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(n + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
     }
     umma_launch_mode(L.mode, EPI_A5, grid_full, s, p);
+    if (hook) hook->after_a5(hook->self, n, s);
     nl += 2;
   }
   prof->mark(s, 0);

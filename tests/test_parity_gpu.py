@@ -472,6 +472,54 @@ def test_host_buffer_entry_point(mode):
     assert _rel(Z.double().numpy(), ref.Z) <= TOL[mode]
 
 
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32"])
+def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise(mode, monkeypatch):
+    """zfac_refine_host with a PINNED Z starts the download of Z right after the first update, on a side stream
+    (final if that update is the only one, superseded by the normal download otherwise); with a pageable Z, or
+    ZFAC_HOST_OVERLAP=0, there is one cudaMemcpy at the end.  All three must return exactly what zfac_refine returns for
+    the same inputs -- with ld > n, where the guard columns of the caller's buffer must stay untouched; with a start that
+    needs several updates (the early download is stale); with one that needs exactly one (it is the result); and with
+    a non-finite start (no update runs: Z = Z0 comes back)."""
+    b = zb()
+    n = 260
+    w = W.random_spd_general(n, seed=12, kappa=15.0, pert=0.1, fp32_stored=True)
+    dt = _dt(mode)
+    Sd, Z0d = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
+    with b.Zfac(n, mode, DEV) as zf:
+        Zref, itref, errref, flref = zf.refine(Sd, Z0d, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        Zref = Zref.cpu()
+        assert itref >= 2
+        for pinned, overlap in ((True, "1"), (False, "1"), (True, "0")):
+            monkeypatch.setenv("ZFAC_HOST_OVERLAP", overlap)
+            S = torch.from_numpy(w.S).to(dt); Z0 = torch.from_numpy(w.Z0).to(dt)
+            Zbig = torch.full((n, n + 7), -5.0, dtype=dt)
+            if pinned:
+                S, Z0, Zbig = S.pin_memory(), Z0.pin_memory(), Zbig.pin_memory()
+            Z = Zbig[:, :n]
+            _, it, err, fl = zf.refine_host(S, Z0, Z, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+            assert it == itref and fl == flref and np.array_equal(err, errref), (pinned, overlap)
+            assert torch.equal(Z, Zref), (pinned, overlap)
+            assert bool((Zbig[:, n:] == -5.0).all())
+        # exactly one update: a converged start (the stop test fires at n = 1) -- the early download IS the result
+        lam, V = np.linalg.eigh(w.S)
+        Zc = W.round_fp32((V / np.sqrt(lam)) @ V.T)
+        Zc_d = _to_dev(Zc, mode)
+        Zr1, it1, err1, fl1 = zf.refine(Sd, Zc_d, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        assert it1 == 1
+        S = torch.from_numpy(w.S).to(dt).pin_memory(); Z0 = torch.from_numpy(Zc).to(dt).pin_memory()
+        Z = torch.zeros(n, n, dtype=dt).pin_memory()
+        _, it, err, fl = zf.refine_host(S, Z0, Z, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        assert it == 1 and fl == fl1 and np.array_equal(err, err1) and torch.equal(Z, Zr1.cpu())
+        # non-finite start: Err[0] = NaN stops at n = 0, no a5 runs, the caller gets Z0 back
+        monkeypatch.setenv("ZFAC_HOST_OVERLAP", "1")
+        Z0bad = torch.from_numpy(w.Z0).to(dt).clone(); Z0bad[3, 4] = float("nan")
+        S = torch.from_numpy(w.S).to(dt).pin_memory(); Z0bad = Z0bad.pin_memory()
+        Z = torch.zeros(n, n, dtype=dt).pin_memory()
+        _, it, err, fl = zf.refine_host(S, Z0bad, Z, max_iter=5, stop=b.ZFAC_STOP_PAPER)
+        assert it == 0 and (fl & b.ZFAC_R_NONFINITE) and len(err) == 1
+        assert torch.equal(torch.nan_to_num(Z, nan=-1.0), torch.nan_to_num(Z0bad, nan=-1.0))
+
+
 # ------------------------------------------------------------------ Alg. 3 ("+refi") and the congruence transformation
 @pytest.mark.parametrize("low", ["split16", "hh16", "tf32"])
 @pytest.mark.parametrize("n", [130, 300])
