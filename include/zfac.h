@@ -143,7 +143,8 @@ zfac_status zfac_congruence(zfac_ctx* ctx, const void* d_H, int64_t ldh, const v
 
 /* Same operation on HOST buffers (pinned memory recommended): copies S and Z0 to the device
  * staging area of the workspace, runs zfac_refine, copies Z, iters, Err[0..max_iter] and flags
- * back, and synchronises `stream` before returning.  This is the end-to-end call bench.py times.  * With a PINNED h_Z and max_iter >= 1 the download of Z starts right after the first update, on an internal side stream:
+ * back, and synchronises `stream` before returning.  This is the end-to-end call bench.py times.
+ * With a PINNED h_Z and max_iter >= 1 the download of Z starts right after the first update, on an internal side stream:
  * if that update is the only one (a warm start) it has overlapped the final residual evaluation; otherwise the normal
  * download at the end supersedes it (measured, N = 8192 SPLIT16 warm start: 24.7 -> 20.9 ms per call; three-update HH16 run:
  * unchanged).  Results are bit-identical either way; ZFAC_HOST_OVERLAP=0 disables it. */
