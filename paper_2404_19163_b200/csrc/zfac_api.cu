@@ -226,7 +226,7 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
   ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np;
   ci.st = reinterpret_cast<State*>(ws + L.off_state);
   ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
-  dim3 gi((unsigned)(L.np / 32), (unsigned)(L.np / 32)), bi(32, 8);
+  dim3 gi((unsigned)(L.np / CI_TC), (unsigned)(L.np / CI_TR)), bi(256);
   switch (c->mode) {
     case ZFAC_MODE_F64:
       if (in_f32) copy_in_kernel<ZFAC_MODE_F64, float><<<gi, bi, 0, s>>>(ci);

@@ -103,65 +103,109 @@ struct CopyInArgs {
   void* oZb;           // SPLIT16 / HH16: half[planes][Np][Np] (Zb[0])
 };
 
-// One 32x32 tile per CTA (32 x 8 threads).  Reads S and Z0 tiles (identity padding beyond n),
-// writes S, Z (row-major) and W = Z^T (through a shared-memory transpose).
-// Tin = element type of the user's S and Z0: the mode's own type, or float for the FP64
-// refinement step of Alg. 3 ("Z = FP64[Z]"; S is promoted exactly).
+// One tile of CI_TR = 32 rows x CI_TC = 64 columns per CTA (256 threads).  Phase 1: coalesced loads of the S and Z0
+// tiles (identity padding beyond n; the user's leading dimension need not be aligned) into shared memory.  Phase 2: every
+// thread takes 8 consecutive columns of one row and writes S, Z (and the 16-bit operand planes) with 16-byte stores.
+// Phase 3: every thread takes 8 consecutive ROWS of one column of the Z tile -- a conflict-free column read of the
+// 65-wide tile -- and writes 8 consecutive elements of a row of W = Z^T, again as 16-byte stores.  (The first version
+// wrote one element per thread, 2-byte stores to the fp16 planes: transaction-bound, i.e. as slow as the SM clock,
+// which is 1.2-1.3 GHz inside a sustained run.)
+// Tin = element type of the user's S and Z0: the mode's own type, or float for the FP64 refinement step of Alg. 3
+// ("Z = FP64[Z]"; S is promoted exactly).
+constexpr int CI_TR = 32, CI_TC = 64, CI_PITCH = CI_TC + 1;
+
+template <int MODE>
+__device__ __forceinline__ void ci_store8(void* buf, size_t np2, size_t o, const float (&v)[8], bool operand) {
+  // 8 consecutive FP32 values -> the mode's representation at element offset o (o is a multiple of 8).
+  // operand = true: a buffer only the tensor core reads (S, W; Zb): fp16 plane(s) / TF32-rounded FP32.
+  if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) {
+    uint32_t hi[4], lo[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (MODE == ZFAC_MODE_SPLIT16) {
+        __half h0, l0, h1, l1;
+        split_f16(v[2 * j], h0, l0); split_f16(v[2 * j + 1], h1, l1);
+        hi[j] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
+        lo[j] = (uint32_t)__half_as_ushort(l0) | ((uint32_t)__half_as_ushort(l1) << 16);
+      } else {
+        hi[j] = (uint32_t)__half_as_ushort(f2h_sat(v[2 * j])) | ((uint32_t)__half_as_ushort(f2h_sat(v[2 * j + 1])) << 16);
+      }
+    }
+    __half* b = static_cast<__half*>(buf);
+    *reinterpret_cast<uint4*>(b + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    if (MODE == ZFAC_MODE_SPLIT16) *reinterpret_cast<uint4*>(b + np2 + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+  } else {                                   // TF32 operand buffers: FP32, rounded to nearest TF32
+    float* b = static_cast<float*>(buf);
+    (void)operand;
+    *reinterpret_cast<float4*>(b + o) = make_float4(round_tf32(v[0]), round_tf32(v[1]), round_tf32(v[2]), round_tf32(v[3]));
+    *reinterpret_cast<float4*>(b + o + 4) = make_float4(round_tf32(v[4]), round_tf32(v[5]), round_tf32(v[6]), round_tf32(v[7]));
+  }
+}
+
 template <int MODE, typename Tin>
 __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
   using Tw = typename std::conditional<MODE == ZFAC_MODE_F64, double, float>::type;   // internal element type
-  __shared__ Tin tile[32][33];
-  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) {
+  __shared__ Tin sS[CI_TR * CI_PITCH];
+  __shared__ Tin sZ[CI_TR * CI_PITCH];
+  const int t = threadIdx.x;
+  if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
     a.st->done = 0; a.st->iters = 0; a.st->flags = 0;
     a.st->arrive[0] = a.st->arrive[1] = a.st->arrive[2] = a.st->arrive[3] = 0u;
   }
-  const int tx = threadIdx.x, ty = threadIdx.y;
-  const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+  const int c0 = blockIdx.x * CI_TC, r0 = blockIdx.y * CI_TR;
   const size_t np = (size_t)a.np, np2 = np * np;
   const Tin* S = static_cast<const Tin*>(a.S);
   const Tin* Z0 = static_cast<const Tin*>(a.Z0);
+  // ---- phase 1: coalesced loads (64 consecutive columns per row), identity padding
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int r = r0 + ty + i * 8, c = c0 + tx;
+  for (int i = 0; i < CI_TR * CI_TC / 256; ++i) {
+    const int idx = t + 256 * i, lr = idx / CI_TC, lc = idx - lr * CI_TC;
+    const int r = r0 + lr, c = c0 + lc;
     const bool in = (r < a.n && c < a.n);
     const Tin ident = (r == c) ? Tin(1) : Tin(0);
-    const Tin s = in ? S[(size_t)r * a.lds + c] : ident;
-    const Tin z = in ? Z0[(size_t)r * a.ldz0 + c] : ident;
-    tile[ty + i * 8][tx] = z;
-    const size_t o = (size_t)r * np + c;
-    if (MODE == ZFAC_MODE_SPLIT16) {
-      __half hi, lo; split_f16((float)s, hi, lo);
-      static_cast<__half*>(a.oS)[o] = hi; static_cast<__half*>(a.oS)[np2 + o] = lo;
-      static_cast<float*>(a.oZ)[o] = (float)z;
-      __half zh, zl; split_f16((float)z, zh, zl);
-      static_cast<__half*>(a.oZb)[o] = zh; static_cast<__half*>(a.oZb)[np2 + o] = zl;
-    } else if (MODE == ZFAC_MODE_HH16) {
-      static_cast<__half*>(a.oS)[o] = f2h_sat((float)s);
-      static_cast<float*>(a.oZ)[o] = (float)z;
-      static_cast<__half*>(a.oZb)[o] = f2h_sat((float)z);
-    } else if (MODE == ZFAC_MODE_TF32) {
-      static_cast<float*>(a.oS)[o] = round_tf32((float)s);
-      static_cast<float*>(a.oZ)[o] = (float)z;
-    } else {
-      static_cast<Tw*>(a.oS)[o] = (Tw)s;
-      static_cast<Tw*>(a.oZ)[o] = (Tw)z;
-    }
+    sS[lr * CI_PITCH + lc] = in ? S[(size_t)r * a.lds + c] : ident;
+    sZ[lr * CI_PITCH + lc] = in ? Z0[(size_t)r * a.ldz0 + c] : ident;
   }
   __syncthreads();
+  // ---- phase 2: S and Z, 8 consecutive columns of one row per thread
+  {
+    const int lr = t >> 3, lc = (t & 7) * 8;
+    const size_t o = (size_t)(r0 + lr) * np + (size_t)(c0 + lc);
+    if (MODE == ZFAC_MODE_F64) {
+      Tw* oS = static_cast<Tw*>(a.oS); Tw* oZ = static_cast<Tw*>(a.oZ);
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int r = c0 + ty + i * 8, c = r0 + tx;      // W[r][c] = Z[c][r]
-    const Tin z = tile[tx][ty + i * 8];
-    const size_t o = (size_t)r * np + c;
-    if (MODE == ZFAC_MODE_SPLIT16) {
-      __half hi, lo; split_f16((float)z, hi, lo);
-      static_cast<__half*>(a.oW)[o] = hi; static_cast<__half*>(a.oW)[np2 + o] = lo;
-    } else if (MODE == ZFAC_MODE_HH16) {
-      static_cast<__half*>(a.oW)[o] = f2h_sat((float)z);
-    } else if (MODE == ZFAC_MODE_TF32) {
-      static_cast<float*>(a.oW)[o] = round_tf32((float)z);
+      for (int j = 0; j < 8; j += 2) {
+        *reinterpret_cast<double2*>(reinterpret_cast<double*>(oS) + o + j) =
+            make_double2((double)sS[lr * CI_PITCH + lc + j], (double)sS[lr * CI_PITCH + lc + j + 1]);
+        *reinterpret_cast<double2*>(reinterpret_cast<double*>(oZ) + o + j) =
+            make_double2((double)sZ[lr * CI_PITCH + lc + j], (double)sZ[lr * CI_PITCH + lc + j + 1]);
+      }
     } else {
-      static_cast<Tw*>(a.oW)[o] = (Tw)z;
+      float vs[8], vz[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { vs[j] = (float)sS[lr * CI_PITCH + lc + j]; vz[j] = (float)sZ[lr * CI_PITCH + lc + j]; }
+      ci_store8<MODE>(a.oS, np2, o, vs, true);
+      float* z32 = static_cast<float*>(a.oZ);                       // FP32 Z (the master copy in the 16-bit modes): not rounded
+      *reinterpret_cast<float4*>(z32 + o) = make_float4(vz[0], vz[1], vz[2], vz[3]);
+      *reinterpret_cast<float4*>(z32 + o + 4) = make_float4(vz[4], vz[5], vz[6], vz[7]);
+      if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true);
+    }
+  }
+  // ---- phase 3: W = Z^T, 8 consecutive rows of one column of the tile per thread -> 8 consecutive elements of a row of W
+  {
+    const int wr = t >> 2, wc = (t & 3) * 8;                        // W tile: CI_TC rows x CI_TR columns
+    const size_t o = (size_t)(c0 + wr) * np + (size_t)(r0 + wc);
+    if (MODE == ZFAC_MODE_F64) {
+      double* oW = static_cast<double*>(a.oW);
+#pragma unroll
+      for (int j = 0; j < 8; j += 2)
+        *reinterpret_cast<double2*>(oW + o + j) =
+            make_double2((double)sZ[(wc + j) * CI_PITCH + wr], (double)sZ[(wc + j + 1) * CI_PITCH + wr]);
+    } else {
+      float vw[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) vw[j] = (float)sZ[(wc + j) * CI_PITCH + wr];
+      ci_store8<MODE>(a.oW, np2, o, vw, true);
     }
   }
 }
