@@ -467,10 +467,13 @@ def run_ours(args):
                 f64_peak = torch_gemm_peak(torch.float64, 8192, dev, reps=3)
             peak, pk_name = f64_peak, "cuBLAS dgemm 8192^3 measured in this run"
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")          # per-launch DRAM bytes from the committed ncu captures
         if os.path.exists(tp):
             try:
-                traffic = json.load(open(tp)).get(f"{args.mode}_a1_n{n}")
+                for ln in open(tp):
+                    f = ln.strip().split(",")
+                    if len(f) == 2 and f[0] == f"{args.mode}_a1_n{n}":
+                        traffic = int(f[1])
             except Exception:
                 traffic = None
         roof = {"bound": "tensor", "kernel": f"umma_gemm_kernel a1 ({args.mode})" if args.mode != "f64" else "f64_gemm_kernel a1",
