@@ -58,7 +58,8 @@ Z0 ∝ I; Z Z^T = S^-1 for non-commuting Z0; cubic order; stop-rule cases;
 scaling / permutation covariances; diagonal S reduces to N scalar recursions;
 `congruence` against the generalized eigenvalues of (H, S) from scipy.linalg.eigh.
 `spectral_closed_form` (N scalar recursions for Z0 = alpha I): against the matrix iteration of `refine` at N = 64
-and 256 (the two routes share only the coefficients), and against z -> lam^-1/2.
+and 256 (the two routes share only the coefficients), against z -> lam^-1/2, against 50-digit `decimal` arithmetic,
+and against the Err tables SURVEY.md §8(c) prints from an independent 80-bit computation.
 Order m = 3, 4 (tests/test_oracle_order_pins.py): the coefficients re-derived in exact
 rationals from the vanishing condition alone; m = 2 mapped onto the printed a_k; the
 tail t_k > 0 with sum 1 and, for m = 2, equal to the printed c, d, e; a scalar

@@ -57,6 +57,53 @@ def test_against_the_surveys_80_bit_tables():
     assert rows == 3
 
 
+def _decimal_history(n, lo, hi, updates, digits=50):
+    """The same N scalar recursions in `decimal` arithmetic at `digits` significant digits (test-local, no numpy):
+    lam_i = lo (hi/lo)^(i/(N-1)), z_0 = 1/sqrt(hi), r = 1 - lam z^2, z <- z (1 + r/2 + 3 r^2/8)."""
+    import decimal
+    D = decimal.Decimal
+    with decimal.localcontext() as ctx:
+        ctx.prec = digits
+        ratio = D(hi) / D(lo)
+        lam = [D(lo) * ratio ** (D(i) / D(n - 1)) for i in range(n)]
+        z = [D(1) / D(hi).sqrt()] * n
+        out = []
+        for k in range(updates + 1):
+            r = [D(1) - l * zi * zi for l, zi in zip(lam, z)]
+            out.append(float(sum(x * x for x in r).sqrt()))
+            z = [zi * (D(1) + x / 2 + D(3) * x * x / 8) for zi, x in zip(z, r)]
+        return [float(l) for l in lam], out
+
+
+def test_against_50_digit_decimal_arithmetic_and_provenance_of_the_stored_table():
+    """Brute force in extended precision (pin list): the FP64 closed form agrees with 50-digit
+    decimal arithmetic to FP64 rounding, and every value of the stored table (golden/survey_closed_form_err.txt, the
+    surveyor's 80-bit numbers) is reproduced by that decimal computation to its 7 printed digits -- so the fixture's
+    content is checkable inside the repository, not taken on trust."""
+    for line in open(os.path.join(GOLDEN, "survey_closed_form_err.txt")):
+        f = line.split("#")[0].split()
+        if not f or int(f[1]) > 1000:                  # the N = 256 row in full; the large rows below on a prefix
+            continue
+        n, lo, hi = int(f[1]), f[2], f[3]
+        want = [float(x) for x in f[4:]]
+        lam, dec = _decimal_history(n, lo, hi, len(want) + 1)
+        for i, v in enumerate(want):
+            assert dec[i] == pytest.approx(v, rel=2e-6), (f[0], i)
+        cf = O.spectral_closed_form(np.array(lam), 1.0 / math.sqrt(float(hi)), len(want) + 1)
+        for i in range(len(want) + 2):
+            if dec[i] > 1e-9:
+                assert cf.err[i] == pytest.approx(dec[i], rel=1e-11), i
+        assert dec[len(want)] < 1e-5 and dec[len(want) + 1] < 1e-15      # 5.7e-7, then below FP64 resolution
+    # the two large rows: first four entries (4617 / 8192 recursions x 4 updates in decimal is still a second or two)
+    for line in open(os.path.join(GOLDEN, "survey_closed_form_err.txt")):
+        f = line.split("#")[0].split()
+        if not f or int(f[1]) <= 1000:
+            continue
+        _, dec = _decimal_history(int(f[1]), f[2], f[3], 3, digits=30)
+        for i in range(4):
+            assert dec[i] == pytest.approx(float(f[4 + i]), rel=2e-6), (f[0], i)
+
+
 def test_argument_checks():
     with pytest.raises(ValueError):
         O.spectral_closed_form(np.ones(4), 1.0, 3, order=5)
