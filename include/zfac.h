@@ -172,6 +172,21 @@ zfac_status zfac_peek(zfac_ctx* ctx, zfac_buf which, void* d_out, int64_t ld, vo
  * launch rate is the limit, a replay is 15-30 % faster than the direct call (n = 300: 0.65 -> 0.46 ms, n = 1024: 1.45 ->
  * 1.23 ms for max_iter = 20), and the host thread is free (2 us per replay instead of 0.6-10 ms of enqueueing). */
 
+/* The whole call as ONE CUDA graph with a WHILE node: copy-in, first residual, WHILE (not stopped) { update, residual,
+ * update, residual }, copy-out.  The stop test (Alg. 2, Eq. 38) of every residual sets the loop condition on
+ * the device, so the graph runs exactly as many iterations as the refinement needs: none of the 2 + 4 max_iter
+ * statically enqueued launches of zfac_refine that return at once after the stop exist here (zfac_refine with
+ * max_iter = 20 and one update: 84 launches, 76 of them such returns).  Same arguments, same results (bit-identical) and
+ * the same restrictions as zfac_refine; the graph is bound to these buffers (write new inputs into them) and to the
+ * context's order at creation time.  zfac_graph_launch is asynchronous on `stream`; launches of one graph, and of graphs
+ * and calls that share a context, must not overlap.  Destroy graphs before their context. */
+typedef struct zfac_graph zfac_graph; /* opaque */
+zfac_status zfac_graph_create(zfac_ctx* ctx, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0,
+                              void* d_Z, int64_t ldz, int max_iter, zfac_stop stop, int* d_iters,
+                              double* d_err, int* d_flags, zfac_graph** graph);
+zfac_status zfac_graph_launch(zfac_graph* graph, void* stream);
+zfac_status zfac_graph_destroy(zfac_graph* graph);
+
 /* Order m of the refinement polynomial, Z_{n+1} = Z_n sum_{k=0..m} c_k R_n^k  (Eq. 13 / Eq. 16:
  * "Reference 1 gives a table with the coefficients a_k for polynomials of order m = 2, 3, 4, 5. For the tests in
  * this article, we use m = 2").  m = 2 (default; the paper's scheme), 3 or 4; anything else -> ZFAC_E_INVALID and

@@ -30,6 +30,7 @@ EXPORTS = [
     "zfac_congruence", "zfac_peek",
     "zfac_last_launch_count", "zfac_padded_n", "zfac_destroy", "zfac_status_string",
     "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile", "zfac_set_order", "zfac_get_order",
+    "zfac_graph_create", "zfac_graph_launch", "zfac_graph_destroy",
 ]
 
 _lib: Optional[ctypes.CDLL] = None
@@ -82,6 +83,12 @@ def lib() -> ctypes.CDLL:
     L.zfac_set_profile.argtypes = [vp, ci]
     L.zfac_get_profile.restype = ci
     L.zfac_get_profile.argtypes = [vp, vp, vp, ci]
+    L.zfac_graph_create.restype = ci
+    L.zfac_graph_create.argtypes = [vp, vp, i64, vp, i64, vp, i64, ci, ci, vp, vp, vp, ctypes.POINTER(vp)]
+    L.zfac_graph_launch.restype = ci
+    L.zfac_graph_launch.argtypes = [vp, vp]
+    L.zfac_graph_destroy.restype = ci
+    L.zfac_graph_destroy.argtypes = [vp]
     L.zfac_set_order.restype = ci
     L.zfac_set_order.argtypes = [vp, ci]
     L.zfac_get_order.restype = ci
@@ -151,6 +158,26 @@ def zfac_peek(ctx: int, which: int, d_out: int, ld: int, stream: int = 0) -> Non
 
 def zfac_last_launch_count(ctx: int) -> int:
     return int(lib().zfac_last_launch_count(ctx))
+
+
+def zfac_graph_create(ctx: int, d_S: int, lds: int, d_Z0: int, ldz0: int, d_Z: int, ldz: int, max_iter: int,
+                      stop: int, d_iters: int, d_err: int, d_flags: int) -> int:
+    g = ctypes.c_void_p()
+    st = lib().zfac_graph_create(ctx, d_S, lds, d_Z0, ldz0, d_Z, ldz, int(max_iter), int(stop), d_iters, d_err, d_flags,
+                                 ctypes.byref(g))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_graph_create")
+    return g.value
+
+
+def zfac_graph_launch(graph: int, stream: int = 0) -> None:
+    st = lib().zfac_graph_launch(graph, stream)
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_graph_launch")
+
+
+def zfac_graph_destroy(graph: int) -> None:
+    lib().zfac_graph_destroy(graph)
 
 
 def zfac_set_order(ctx: int, m: int) -> None:
@@ -422,3 +449,50 @@ class ZfacGraph:
         torch.cuda.current_stream(self.S.device).synchronize()
         it = int(self.d_iters.item())
         return self.Z, it, self.d_err[: it + 1].cpu().numpy(), int(self.d_flags.item())
+
+
+class ZfacLoopGraph:
+    """The call as the library's own CUDA graph with a WHILE node (include/zfac.h, zfac_graph_*): it runs exactly as
+    many iterations as the stop test allows -- no statically enqueued launches after the stop.  Bound to the tensors
+    given here: write new S / Z0 contents INTO them and call `launch()`.  Marshalling only."""
+
+    def __init__(self, zf: Zfac, S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, stop: int = ZFAC_STOP_PAPER,
+                 out: Optional[torch.Tensor] = None):
+        zf._check(S, "S"); zf._check(Z0, "Z0")
+        self.zf, self.S, self.Z0, self.max_iter = zf, S, Z0, int(max_iter)
+        self.Z = out if out is not None else torch.empty((zf.n, zf.n), dtype=zf.dtype, device=S.device)
+        zf._check(self.Z, "Z")
+        self.d_iters = torch.zeros(1, dtype=torch.int32, device=S.device)
+        self.d_flags = torch.zeros(1, dtype=torch.int32, device=S.device)
+        self.d_err = torch.full((self.max_iter + 1,), float("nan"), dtype=torch.float64, device=S.device)
+        with torch.cuda.device(S.device):
+            self.graph = zfac_graph_create(zf.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0),
+                                           self.Z.data_ptr(), self.Z.stride(0), self.max_iter, stop,
+                                           self.d_iters.data_ptr(), self.d_err.data_ptr(), self.d_flags.data_ptr())
+
+    def close(self) -> None:
+        if getattr(self, "graph", None):
+            zfac_graph_destroy(self.graph)
+            self.graph = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def launch(self, sync: bool = True):
+        """Launch on the current stream.  sync=True: (Z, iters, err[0..iters], flags)."""
+        zfac_graph_launch(self.graph, torch.cuda.current_stream(self.S.device).cuda_stream)
+        if not sync:
+            return self.Z, self.d_iters, self.d_err, self.d_flags
+        torch.cuda.current_stream(self.S.device).synchronize()
+        it = int(self.d_iters.item())
+        return self.Z, it, self.d_err[: it + 1].cpu().numpy(), int(self.d_flags.item())
+

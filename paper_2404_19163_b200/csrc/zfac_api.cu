@@ -163,54 +163,75 @@ zfac_status zfac_set_order(zfac_ctx* c, int m) {
 
 int zfac_get_order(const zfac_ctx* c) { return c ? c->order : 0; }
 
-// skip_last: Alg. 3 as printed ends after the update, without evaluating the residual of the result.
-static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s,
-                              bool skip_last = false, const IterHook* hook = nullptr) {
-  const Layout& L = c->L;
-  char* ws = c->ws;
-  State* st = reinterpret_cast<State*>(ws + L.off_state);
-  double* W = reinterpret_cast<double*>(ws + L.off_W);          // epilogue pointers; the operands go through tensor maps
-  double* T = reinterpret_cast<double*>(ws + L.off_T);
-  double* R = reinterpret_cast<double*>(ws + L.off_R);
-  double* Q = reinterpret_cast<double*>(ws + L.off_Q);
-  double* Z[2] = {reinterpret_cast<double*>(ws + L.off_Z[0]), reinterpret_cast<double*>(ws + L.off_Z[1])};
-  const int tiles = (int)(L.np / F64_BM);
-  const int full = tiles * tiles, tri = tiles * (tiles + 1) / 2;
-  const F64Plan& fp = c->f64p;
+// FP64 mode: the two halves of one iteration (see UmmaSeq in zfac_umma.cuh for the contract of n_stop / par).
+struct F64Seq {
+  zfac_ctx* c;
   F64TParams P{};
-  F64Params& p = P.q;
-  p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = st;
-  p.stop.st = st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
-  p.stop.num_partials = tri; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
-  p.stop.order = c->order;
-  p.pc = poly_coef(c->order);
-  for (int n = 0; n <= max_iter; ++n) {
-    if (n == max_iter && skip_last) break;
+  int full = 0, tri = 0;
+  double *W, *T, *R, *Q, *Z[2];
+
+  F64Seq(zfac_ctx* c_, int max_iter, zfac_stop stop, double* d_err, unsigned long long cond) : c(c_) {
+    const Layout& L = c->L;
+    char* ws = c->ws;
+    State* st = reinterpret_cast<State*>(ws + L.off_state);
+    W = reinterpret_cast<double*>(ws + L.off_W);          // epilogue pointers; the operands go through tensor maps
+    T = reinterpret_cast<double*>(ws + L.off_T);
+    R = reinterpret_cast<double*>(ws + L.off_R);
+    Q = reinterpret_cast<double*>(ws + L.off_Q);
+    Z[0] = reinterpret_cast<double*>(ws + L.off_Z[0]); Z[1] = reinterpret_cast<double*>(ws + L.off_Z[1]);
+    const int tiles = (int)(L.np / F64_BM);
+    full = tiles * tiles; tri = tiles * (tiles + 1) / 2;
+    F64Params& p = P.q;
+    p.ld = (int)L.np; p.K = (int)L.np; p.tiles = tiles; p.st = st;
+    p.stop.st = st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
+    p.stop.num_partials = tri; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+    p.stop.order = c->order; p.stop.cond = cond;
+    p.pc = poly_coef(c->order);
+  }
+  void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+    const F64Plan& fp = c->f64p;
+    F64Params& p = P.q;
     P.mapA = fp.mW; P.mapB = fp.mS; p.out0 = T; p.out1 = nullptr; p.in0 = nullptr;          // a1: T = W S^T
-    c->prof.mark(s, EPI_A1 + 16 * n);
+    if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
     f64_tma_launch(EPI_A1, full, s, P);
-    P.mapA = fp.mW; P.mapB = fp.mT; p.out0 = R; p.stop.n_iter = n;                           // a2: R = I - W T^T
-    c->prof.mark(s, EPI_A2 + 16 * n);
+    P.mapA = fp.mW; P.mapB = fp.mT; p.out0 = R; p.stop.n_iter = n_stop;                      // a2: R = I - W T^T
+    if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
     f64_tma_launch(EPI_A2, tri, s, P);
     c->launches += 2;
-    if (n == max_iter) break;
+  }
+  void update(int par, int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+    const F64Plan& fp = c->f64p;
+    F64Params& p = P.q;
+    p.stop.n_iter = n_stop;
     if (c->order > 2) {
       // order m > 2: P = R R -> T buffer, G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z buffer a5 overwrites next
-      P.mapA = fp.mR; P.mapB = fp.mR; p.in0 = R; p.out0 = T; p.out1 = Z[(n + 1) & 1];
-      c->prof.mark(s, EPI_P2 + 16 * n);
+      P.mapA = fp.mR; P.mapB = fp.mR; p.in0 = R; p.out0 = T; p.out1 = Z[(par + 1) & 1];
+      if (prof) prof->mark(s, EPI_P2 + 16 * tagn);
       f64_tma_launch(EPI_P2, tri, s, P);
       c->launches += 1;
-      P.mapA = fp.mT; P.mapB = fp.mZ[(n + 1) & 1]; p.in0 = R; p.out0 = Q; p.out1 = nullptr;  // Q = 1/2 R + P G
+      P.mapA = fp.mT; P.mapB = fp.mZ[(par + 1) & 1]; p.in0 = R; p.out0 = Q; p.out1 = nullptr;  // Q = 1/2 R + P G
     } else {
       P.mapA = fp.mR; P.mapB = fp.mR; p.in0 = R; p.out0 = Q;
     }
-    c->prof.mark(s, EPI_A4 + 16 * n);
+    if (prof) prof->mark(s, EPI_A4 + 16 * tagn);
     f64_tma_launch(EPI_A4, tri, s, P);
-    P.mapA = fp.mZ[n & 1]; P.mapB = fp.mQ; p.in0 = Z[n & 1]; p.out0 = Z[(n + 1) & 1]; p.out1 = W;   // a5
-    c->prof.mark(s, EPI_A5 + 16 * n);
+    P.mapA = fp.mZ[par]; P.mapB = fp.mQ; p.in0 = Z[par]; p.out0 = Z[(par + 1) & 1]; p.out1 = W;   // a5
+    if (prof) prof->mark(s, EPI_A5 + 16 * tagn);
     f64_tma_launch(EPI_A5, full, s, P);
-    if (hook) hook->after_a5(hook->self, n, s);
     c->launches += 2;
+  }
+};
+
+// skip_last: Alg. 3 as printed ends after the update, without evaluating the residual of the result.
+static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s,
+                              bool skip_last = false, const IterHook* hook = nullptr) {
+  F64Seq q(c, max_iter, stop, d_err, 0ull);
+  for (int n = 0; n <= max_iter; ++n) {
+    if (n == max_iter && skip_last) break;
+    q.residual(n, n, s, &c->prof);
+    if (n == max_iter) break;
+    q.update(n & 1, n, n, s, &c->prof);
+    if (hook) hook->after_a5(hook->self, n, s);
   }
   c->prof.mark(s, 0);
   ZF_CUDA(cudaGetLastError());
@@ -436,6 +457,110 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
     ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaMemcpyAsync(h_err, dErr, (size_t)(ints[0] + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaStreamSynchronize(s));
+  return ZFAC_OK;
+}
+
+// ------------------------------------------------------------------ zfac_graph: the call as a CUDA graph with a WHILE node
+struct zfac_graph {
+  zfac_ctx* c = nullptr;
+  cudaGraph_t g = nullptr;
+  cudaGraphExec_t ex = nullptr;
+};
+
+extern "C++" {
+template <class Seq>
+static void enqueue_loop_body(Seq& q, cudaStream_t s) {
+  // two iterations (the Z operand buffers alternate with the parity of n); indices come from the device (n_stop = -1).
+  // If the stop test fires in the first half, the second half's kernels return at once (State::done).
+  q.update(0, -1, 0, s, nullptr); q.residual(-1, 0, s, nullptr);
+  q.update(1, -1, 0, s, nullptr); q.residual(-1, 0, s, nullptr);
+}
+}
+
+zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
+                              int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
+                              zfac_graph** out) {
+  if (!out) return ZFAC_E_INVALID;
+  *out = nullptr;
+  if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
+  if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
+  if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
+  const Layout& L = c->L;
+  char* ws = c->ws;
+  zfac_graph* zg = new (std::nothrow) zfac_graph();
+  if (!zg) return ZFAC_E_INVALID;
+  zg->c = c;
+  cudaStream_t cs = nullptr, bs = nullptr;
+  zfac_status rs = ZFAC_OK;
+  bool capturing = false;
+  auto fail = [&](const char* what, cudaError_t e) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "zfac_graph_create: %s: %s", what, cudaGetErrorString(e));
+    rs = ZFAC_E_CUDA;
+  };
+  cudaError_t e;
+  do {
+    if ((e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking)) != cudaSuccess) { fail("stream", e); break; }
+    if ((e = cudaStreamCreateWithFlags(&bs, cudaStreamNonBlocking)) != cudaSuccess) { fail("stream", e); break; }
+    if ((e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeRelaxed)) != cudaSuccess) { fail("begin capture", e); break; }
+    capturing = true;
+    cudaStreamCaptureStatus cst; unsigned long long cid = 0; cudaGraph_t g = nullptr;
+    const cudaGraphNode_t* deps = nullptr; size_t ndeps = 0;
+    if ((e = cudaStreamGetCaptureInfo_v2(cs, &cst, &cid, &g, &deps, &ndeps)) != cudaSuccess) { fail("capture info", e); break; }
+    cudaGraphConditionalHandle h;
+    if ((e = cudaGraphConditionalHandleCreate(&h, g, 1, cudaGraphCondAssignDefault)) != cudaSuccess) { fail("conditional handle", e); break; }
+    // root: copy-in, first residual (its stop test already sets the condition: max_iter = 0 or a non-finite Err[0] skip the loop)
+    const int saved_launches = c->launches;
+    launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, cs);
+    cudaGraphNodeParams np = {};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
+    cudaGraphNode_t wnode = nullptr;
+    auto splice_loop = [&]() -> bool {
+      if ((e = cudaStreamGetCaptureInfo_v2(cs, &cst, &cid, &g, &deps, &ndeps)) != cudaSuccess) { fail("capture info", e); return false; }
+      if ((e = cudaGraphAddNode(&wnode, g, deps, ndeps, &np)) != cudaSuccess) { fail("while node", e); return false; }
+      if ((e = cudaStreamUpdateCaptureDependencies(cs, &wnode, 1, cudaStreamSetCaptureDependencies)) != cudaSuccess) { fail("capture deps", e); return false; }
+      if ((e = cudaStreamBeginCaptureToGraph(bs, np.conditional.phGraph_out[0], nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed)) != cudaSuccess) { fail("body capture", e); return false; }
+      return true;
+    };
+    bool ok = true;
+    if (c->mode == ZFAC_MODE_F64) {
+      F64Seq q(c, max_iter, stop, d_err, (unsigned long long)h);
+      q.residual(0, 0, cs, nullptr);
+      if ((ok = splice_loop())) enqueue_loop_body(q, bs);
+    } else {
+      UmmaSeq q(c->umma, max_iter, (int)stop, c->order, d_err, (unsigned long long)h);
+      q.residual(0, 0, cs, nullptr);
+      if ((ok = splice_loop())) enqueue_loop_body(q, bs);
+    }
+    if (!ok) break;
+    if ((e = cudaStreamEndCapture(bs, nullptr)) != cudaSuccess) { fail("end body capture", e); break; }
+    launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, cs);
+    c->launches = saved_launches;
+    capturing = false;
+    if ((e = cudaStreamEndCapture(cs, &zg->g)) != cudaSuccess) { fail("end capture", e); break; }
+    if ((e = cudaGetLastError()) != cudaSuccess) { fail("launch during capture", e); break; }
+    if ((e = cudaGraphInstantiate(&zg->ex, zg->g, 0)) != cudaSuccess) { fail("instantiate", e); break; }
+  } while (false);
+  if (capturing) { cudaGraph_t junk = nullptr; cudaStreamEndCapture(cs, &junk); if (junk) cudaGraphDestroy(junk); }
+  if (cs) cudaStreamDestroy(cs);
+  if (bs) cudaStreamDestroy(bs);
+  if (rs != ZFAC_OK) { zfac_graph_destroy(zg); return rs; }
+  *out = zg;
+  return ZFAC_OK;
+}
+
+zfac_status zfac_graph_launch(zfac_graph* zg, void* stream) {
+  if (!zg || !zg->ex) return ZFAC_E_INVALID;
+  ZF_CUDA(cudaGraphLaunch(zg->ex, static_cast<cudaStream_t>(stream)));
+  return ZFAC_OK;
+}
+
+zfac_status zfac_graph_destroy(zfac_graph* zg) {
+  if (zg) {
+    if (zg->ex) cudaGraphExecDestroy(zg->ex);
+    if (zg->g) cudaGraphDestroy(zg->g);
+    delete zg;
+  }
   return ZFAC_OK;
 }
 

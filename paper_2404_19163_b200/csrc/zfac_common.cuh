@@ -26,7 +26,11 @@ struct StopArgs {
   int max_iter;
   int stop;                  // zfac_stop
   int order;                 // m of Eq. 13 (2, 3, 4): the test's exponent is nu_max = m + 1
+  unsigned long long cond;   // zfac_graph_*: handle of the WHILE node's condition, set to "not done" by the stop test (0: none)
 };
+// n_iter < 0 (inside the loop body of a zfac_graph, whose kernel parameters are fixed): the index comes from the device,
+// State::iters = index of the last Err written, so the residual being evaluated is iters + 1.
+__device__ __forceinline__ int stop_index(const StopArgs& a) { return a.n_iter >= 0 ? a.n_iter : a.st->iters + 1; }
 
 // Optional per-kernel timing (zfac_set_profile): an event is recorded on the launching stream
 // before every GEMM kernel and one after the last; tags = step id (1,2,4,5) + 16 * iteration.
@@ -72,7 +76,7 @@ __device__ inline void stop_test_last_cta(const StopArgs& a, double* smem_red /*
     double tot = 0.0;
     for (int w = 0; w < nw; ++w) tot += smem_red[w];
     const double err = sqrt(tot);
-    const int n = a.n_iter;
+    const int n = stop_index(a);
     a.d_err[n] = err;
     State* st = a.st;
     st->iters = n;
@@ -87,6 +91,7 @@ __device__ inline void stop_test_last_cta(const StopArgs& a, double* smem_red /*
     }
     if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
     if (done) { st->flags |= flags; __threadfence(); st->done = 1; }
+    if (a.cond) cudaGraphSetConditional((cudaGraphConditionalHandle)a.cond, done ? 0u : 1u);   // another pass of the loop?
   }
 }
 

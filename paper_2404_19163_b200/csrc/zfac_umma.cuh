@@ -416,7 +416,9 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int num_tiles = (SYM ? T * (T + 1) / 2 : T * T) * NSPLIT;         // 256 x TN pair tiles
   // One pass for a second-order product (a4 / p2, KIND_F16X2): taken by every thread of the grid from the Err[n] that
   // a2 of this iteration wrote (a completed kernel: visible), so issuer and epilogues of both CTAs agree.
-  const bool hh_only = PAIRK && p.hh_only && (__ldcg(p.stop.d_err + p.stop.n_iter) <= p.hh_err_max);
+  // (n_iter < 0, loop body of a zfac_graph: the update is taken from the last residual written, State::iters)
+  const bool hh_only = PAIRK && p.hh_only &&
+                       (__ldcg(p.stop.d_err + (p.stop.n_iter >= 0 ? p.stop.n_iter : p.st->iters)) <= p.hh_err_max);
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
@@ -849,46 +851,68 @@ inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const 
   else umma_launch<KIND_TF32>(epi, grid, s, p);
 }
 
-inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof,
-                               const IterHook* hook = nullptr) {
-  const Layout& L = pl.L;
-  char* ws = pl.ws;
-  const int T = (int)(L.np / UM_MACRO);
-  const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
-                                 : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
-  const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
-  const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
-  const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
+// The two halves of one iteration as the host enqueues them.  The only dependence on the iteration index n is (i) the
+// index of the Err[] entry a2 writes and a4 reads -- `n_stop`, or -1 = "take it from State::iters on the device" -- and
+// (ii) the parity of n, which selects the Z operand buffers.  zfac_refine loops over (residual, update); a zfac_graph
+// puts update(0), residual, update(1), residual into the body of a WHILE node (fixed kernel parameters, hence the
+// parity-unrolled body and the device-side index).
+struct UmmaSeq {
+  const UmmaPlan& pl;
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band;
-  p.st = reinterpret_cast<State*>(ws + L.off_state);
+  int grid_full = 0, grid_sym = 0, order = 2, nl = 0;
+  bool h16 = false;
+  float* R32 = nullptr;
+
+  UmmaSeq(const UmmaPlan& pl_, int max_iter, int stop, int order_, double* d_err, unsigned long long cond) : pl(pl_) {
+    const Layout& L = pl.L;
+    char* ws = pl.ws;
+    const int T = (int)(L.np / UM_MACRO);
+    const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
+                                   : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
+    const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
+    grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
+    grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
+    order = order_;
+    p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band;
+    p.st = reinterpret_cast<State*>(ws + L.off_state);
 #ifdef ZFAC_TIMING
-  p.dbg = reinterpret_cast<unsigned long long*>(ws + L.off_dbg);
+    p.dbg = reinterpret_cast<unsigned long long*>(ws + L.off_dbg);
 #endif
-  p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
-  p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
-  p.stop.order = order;
-  const PolyCoef pc = poly_coef(order);
-  p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.g_i = (float)pc.g_i; p.g_r = (float)pc.g_r; p.g_p = (float)pc.g_p;
-  float* R32 = reinterpret_cast<float*>(ws + L.off_R);
-  const bool h16 = (L.mode != ZFAC_MODE_TF32);
-  int nl = 0;
-  for (int n = 0; n <= max_iter; ++n) {
+    p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
+    p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+    p.stop.order = order; p.stop.cond = cond;
+    const PolyCoef pc = poly_coef(order);
+    p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.g_i = (float)pc.g_i; p.g_r = (float)pc.g_r; p.g_p = (float)pc.g_p;
+    R32 = reinterpret_cast<float*>(ws + L.off_R);
+    h16 = (L.mode != ZFAC_MODE_TF32);
+  }
+
+  // a1 + a2 (+ a3): residual number n_stop (-1: device-side index)
+  void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+    const Layout& L = pl.L;
+    char* ws = pl.ws;
     // a1: T = W S^T            (promoted accumulation: T and X are O(1) quantities)
-    prof->mark(s, EPI_A1 + 16 * n);
+    if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
+    p.hh_only = 0;
     p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
     p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; }
     umma_launch_mode(L.mode, EPI_A1, grid_full, s, p);
     // a2: R = I - W T^T
-    prof->mark(s, EPI_A2 + 16 * n);
-    p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n;
+    if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
+    p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n_stop;
     p.chunk0_kb = 2 * pl.chunk0_kb;           // a2 writes four outputs per element: its stores take twice as long
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
     umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
     nl += 2;
-    if (n == max_iter) break;
+  }
+
+  // (p2,) a4, a5: update number n with n & 1 = par, taken from residual n_stop (-1: device-side index)
+  void update(int par, int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+    const Layout& L = pl.L;
+    char* ws = pl.ws;
+    p.stop.n_iter = n_stop;
     // a4: Q = 1/2 R + 3/8 R R^T   (the product is a correction of size |R|^2: no promotion needed)
     if (pl.promote_update) { p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb; }
     else { p.chunk_kb = 0; p.chunk0_kb = 0; }
@@ -897,16 +921,16 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
     if (order > 2) {
       // order m > 2 (zfac.h, zfac_set_order): P = R R^T -> T buffer (free between a2 and the next a1),
       // G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z operand buffer a5 is about to overwrite; then Q = 1/2 R + P G^T
-      prof->mark(s, EPI_P2 + 16 * n);
+      if (prof) prof->mark(s, EPI_P2 + 16 * tagn);
       p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
-      if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; p.out2 = ws + L.off_Zb[(n + 1) & 1]; }
-      else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; p.out2 = ws + L.off_Z[(n + 1) & 1]; }
+      if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; p.out2 = ws + L.off_Zb[(par + 1) & 1]; }
+      else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; p.out2 = ws + L.off_Z[(par + 1) & 1]; }
       umma_launch_mode(L.mode, EPI_P2, grid_sym, s, p);
       nl += 1;
       p.out2 = nullptr;
     }
-    prof->mark(s, EPI_A4 + 16 * n);
-    if (order > 2) { p.mapA = pl.mT; p.mapB = pl.mZ[(n + 1) & 1]; }
+    if (prof) prof->mark(s, EPI_A4 + 16 * tagn);
+    if (order > 2) { p.mapA = pl.mT; p.mapB = pl.mZ[(par + 1) & 1]; }
     else { p.mapA = pl.mR; p.mapB = pl.mR; }
     p.f32_in = R32;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
@@ -914,21 +938,31 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
     umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p);
     // a5: Z_next = Z + Z Q^T ; W = Z_next^T   (first order in R: all three passes)
     p.hh_only = 0;
-    prof->mark(s, EPI_A5 + 16 * n);
-    p.mapA = pl.mZ[n & 1]; p.mapB = pl.mQ;
+    if (prof) prof->mark(s, EPI_A5 + 16 * tagn);
+    p.mapA = pl.mZ[par]; p.mapB = pl.mQ;
     if (h16) {
       float* Z32 = reinterpret_cast<float*>(ws + L.off_Z[0]);       // FP32 master copy, updated in place
-      p.f32_in = Z32; p.f32_out = Z32; p.h_out = ws + L.off_Zb[(n + 1) & 1]; p.h_out_t = ws + L.off_W;
+      p.f32_in = Z32; p.f32_out = Z32; p.h_out = ws + L.off_Zb[(par + 1) & 1]; p.h_out_t = ws + L.off_W;
     } else {
-      p.f32_in = reinterpret_cast<float*>(ws + L.off_Z[n & 1]);
-      p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(n + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
+      p.f32_in = reinterpret_cast<float*>(ws + L.off_Z[par]);
+      p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(par + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
     }
     umma_launch_mode(L.mode, EPI_A5, grid_full, s, p);
-    if (hook) hook->after_a5(hook->self, n, s);
     nl += 2;
   }
+};
+
+inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof,
+                               const IterHook* hook = nullptr) {
+  UmmaSeq q(pl, max_iter, stop, order, d_err, 0ull);
+  for (int n = 0; n <= max_iter; ++n) {
+    q.residual(n, n, s, prof);
+    if (n == max_iter) break;
+    q.update(n & 1, n, n, s, prof);
+    if (hook) hook->after_a5(hook->self, n, s);
+  }
   prof->mark(s, 0);
-  *launches = nl;
+  *launches = q.nl;
   return cudaGetLastError();
 }
 

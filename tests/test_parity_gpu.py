@@ -298,6 +298,36 @@ def test_refine_is_graph_capturable_and_replays_bitwise(mode):
         assert _rel(zg.Z.cpu().double().numpy(), ref.Z) <= TOL[mode]
 
 
+@pytest.mark.parametrize("m", [2, 4])
+@pytest.mark.parametrize("mode", ["f64", "split16", "tf32", "hh16"])
+def test_while_graph_runs_exactly_the_needed_iterations_bitwise(mode, m):
+    """zfac_graph_*: the call as one CUDA graph with a WHILE node whose condition the stop test sets on the device.
+    Launches must be bit-identical to zfac_refine -- for new inputs written into the bound buffers (different stop
+    indices, odd and even: the loop body is unrolled over the parity of n), for max_iter = 0 (the loop must not run) and
+    for a max_iter smaller than the natural stop (MAXITER inside the loop)."""
+    b = zb()
+    n = 300
+    ws = [W.random_spd_general(n, seed=21, kappa=20.0, pert=0.1, fp32_stored=True),
+          W.random_spd_general(n, seed=22, kappa=200.0, pert=0.02, fp32_stored=True),
+          W.spectral_workload(n, 0.05, 1.0, seed=2, fp32_stored=True)]
+    S, Z0 = _to_dev(ws[0].S, mode), _to_dev(ws[0].Z0, mode)
+    with b.Zfac(n, mode, DEV) as zf:
+        zf.set_order(m)
+        seen = set()
+        for max_iter, stop in ((25, b.ZFAC_STOP_PAPER), (0, b.ZFAC_STOP_PAPER), (2, b.ZFAC_STOP_FIXED), (3, b.ZFAC_STOP_FIXED)):
+            with b.ZfacLoopGraph(zf, S, Z0, max_iter=max_iter, stop=stop) as lg:
+                for w in ws + ws[:1]:
+                    S.copy_(_to_dev(w.S, mode)); Z0.copy_(_to_dev(w.Z0, mode))
+                    Zd, itd, errd, fld = zf.refine(S, Z0, max_iter=max_iter, stop=stop)
+                    Zd = Zd.clone()
+                    lg.Z.fill_(-3.0)
+                    Zg, itg, errg, flg = lg.launch()
+                    assert itg == itd and flg == fld and np.array_equal(errg, errd), (max_iter, w.name)
+                    assert torch.equal(Zg, Zd), (max_iter, w.name)
+                    seen.add(itd)
+        assert 0 in seen and any(i % 2 == 1 for i in seen) and any(i % 2 == 0 and i > 0 for i in seen)
+
+
 # ------------------------------------------------------------------ memory discipline (stand-ins for compute-sanitizer)
 # compute-sanitizer is closed on this GPU pool (DESIGN.md §6a); these tests check what memcheck / initcheck would.
 GUARD = 1 << 20
