@@ -387,6 +387,24 @@ def run_ours(args):
                    "tflops_fp32_equiv": flops_fp32_equiv(n, iters) / (ms * 1e-3) / 1e12,
                    "iters_per_s": (iters / (ms * 1e-3)) if iters else 0.0, "clocks": clocks}
             if with_e2e:
+                # the same steps through the library's WHILE-node graph (zfac_graph_*): no launches after the stop
+                try:
+                    with zb.ZfacLoopGraph(zf, S, Z0, max_iter=args.max_iter, stop=stop, out=Zout) as lg:
+                        for _ in range(args.warmup):
+                            lg.launch(sync=False)
+                        torch.cuda.synchronize(dev)
+                        g0 = torch.cuda.Event(enable_timing=True); g1 = torch.cuda.Event(enable_timing=True)
+                        g0.record()
+                        for _ in range(args.steps):
+                            lg.launch(sync=False)
+                        g1.record(); torch.cuda.synchronize(dev)
+                        gms = g0.elapsed_time(g1) / args.steps
+                        git = int(lg.d_iters.item())
+                    res["while_graph"] = {"ms_per_step": gms, "iters": git,
+                                          "value": flops_fp32_equiv(n, git) / (gms * 1e-3) / 1e12, "unit": UNIT,
+                                          "note": "zfac_graph_launch: CUDA graph with a WHILE node, same workload and steps"}
+                except Exception as ex:                       # informational figure only
+                    res["while_graph"] = {"error": str(ex)[:120]}
                 hS = torch.from_numpy(w.S).to(dt).pin_memory(); hZ0 = torch.from_numpy(w.Z0).to(dt).pin_memory()
                 hZ = torch.empty_like(hZ0).pin_memory()
                 for _ in range(max(1, args.warmup // 2)):
@@ -530,6 +548,7 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": primary["h2d"],
                     "d2h_bytes_per_step": primary["d2h"]},
             "gpu_launches": primary["launches"] * args.steps,
+            "while_graph": primary.get("while_graph"),
             "roofline": roof, "cpu_baseline": cpu, "modes": extra,
         }
         print(json.dumps(line))
