@@ -440,6 +440,39 @@ def run_ours(args):
             r = run_mode(mode, with_e2e=False, with_clock=False)
             r["final_residual_per_sqrt_n"] = invariant(r.pop("Z"))
             extra[mode] = r
+        # iterations / s (BASELINE.json's metric names it for split-FP16 and FP64 at N = 8192): SURVEY.md §8(d)'s difference
+        # quotient over fixed-count runs, t_iter = (t(k2) - t(k1)) / (k2 - k1), which cancels copy-in, copy-out and the
+        # first residual.  One iteration = a4, a5, a1, a2 = 8 N^3 flop in the paper's convention.
+        # Config 5 (cold start, lambda in [1e-3, 1]) so that every counted update does real work.
+        try:
+            from paper_2404_19163_b200 import workloads as W5
+            w5 = W5.config5(n, device=dev, fp32_stored=True)
+            rate = {}
+            for mode, (k1, k2, reps) in (("split16", (2, 10, 8)), ("f64", (1, 3, 2))):
+                dt = torch.float64 if mode == "f64" else torch.float32
+                S5 = torch.from_numpy(w5.S).to(dev, dt); Z5 = torch.from_numpy(w5.Z0).to(dev, dt); O5 = torch.empty_like(Z5)
+                with zb.Zfac(n, mode, dev) as zf:
+                    ts = {}
+                    for k in (k1, k2):
+                        for _ in range(2):
+                            zf.refine(S5, Z5, max_iter=k, stop=zb.ZFAC_STOP_FIXED, out=O5, sync=False)
+                        torch.cuda.synchronize(dev)
+                        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        for _ in range(reps):
+                            zf.refine(S5, Z5, max_iter=k, stop=zb.ZFAC_STOP_FIXED, out=O5, sync=False)
+                        e1.record(); torch.cuda.synchronize(dev)
+                        ts[k] = e0.elapsed_time(e1) / reps
+                t_it = (ts[k2] - ts[k1]) / (k2 - k1)
+                rate[mode] = {"ms_per_iteration": t_it, "iters_per_s": 1e3 / t_it,
+                              "tflops_fp32_equiv": 8.0 * float(n) ** 3 / (t_it * 1e-3) / 1e12,
+                              "k1": k1, "k2": k2, "ms_k1": ts[k1], "ms_k2": ts[k2]}
+                del S5, Z5, O5
+            rate["workload"] = f"config5_n{n} (cold start, kappa 1e3), ZFAC_STOP_FIXED"
+            extra["iteration_rate"] = rate
+            del w5
+        except Exception as ex:                                   # secondary figure
+            extra["iteration_rate"] = {"error": str(ex)[:120]}
         # cuBLAS reference rates per precision, measured in this run the way MEASURED_PEAKS.json was
         extra["cublas_tflops"] = {"bf16": torch_gemm_peak(torch.bfloat16, 8192, dev),
                                   "tf32": torch_gemm_peak(torch.float32, 8192, dev, tf32=True),
