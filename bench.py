@@ -504,11 +504,11 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel: a1 (full split GEMM, 3 MMA passes; a5 costs the same)
     kms = primary["kernel_ms"]
-    passes = {"split16": 3, "tf32": 1, "f64": 1}[args.mode]
+    passes = {"split16": 3, "tf32": 1, "f64": 1, "hh16": 1}[args.mode]
     roof = None
     if "a1" in kms:
         ach = passes * 2.0 * n ** 3 / (kms["a1"] * 1e-3) / 1e12
-        if args.mode == "split16":
+        if args.mode in ("split16", "hh16"):
             peak, pk_name = peaks["bf16_sustained"], "bf16_tflops_sustained"
         elif args.mode == "tf32":
             peak, pk_name = peaks["bf16_sustained"] * 0.5, "bf16_tflops_sustained x 0.5 (nominal tf32:bf16 ratio)"
@@ -569,7 +569,8 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": {"split16": "f16 (hi + scaled-lo pairs), f32 accumulate", "tf32": "tf32, f32 accumulate", "f64": "f64"}[args.mode],
+            "dtype": {"split16": "f16 (hi + scaled-lo pairs), f32 accumulate", "tf32": "tf32, f32 accumulate", "f64": "f64",
+                      "hh16": "f16 (one pass), f32 accumulate"}[args.mode],
             "data": "synthetic",
             "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "N": n, "stop": args.stop,
                        "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
@@ -597,7 +598,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=8192)
-    ap.add_argument("--mode", default="split16", choices=["split16", "tf32", "f64"])
+    ap.add_argument("--mode", default="split16", choices=["split16", "tf32", "f64", "hh16"])
     ap.add_argument("--workload", default="config4", choices=["config4", "config5", "config2"])
     ap.add_argument("--stop", default="paper", choices=["paper", "fixed"])
     ap.add_argument("--max-iter", type=int, default=20)

@@ -467,13 +467,16 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
         int m0, n0; bool od; decode(t, m0, n0, od);
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1u);
-          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * STAGE_BYTES);     // both CTAs' boxes
+          // one-pass launch of the pair kind (hh_only): the lo' planes are never read -- do not load them
+          const int narr = hh_only ? 1 : KT::ARRAYS;
+          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * (uint32_t)narr * (UM_A_BYTES + B_BYTES));   // both CTAs' boxes
           const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
           const uint32_t sa = smem_base + stage * STAGE_BYTES;
           const uint32_t sb = sa + KT::ARRAYS * UM_A_BYTES;
           const int kc = kb * KT::BK_ELEMS;
 #pragma unroll
           for (int a = 0; a < KT::ARRAYS; ++a) {
+            if (a >= narr) break;
 #pragma unroll
             for (int b = 0; b < UM_ROWS / UM_BOX_ROWS; ++b)
               tma_load_2d_pair(sa + a * UM_A_BYTES + b * UM_BOX_BYTES, &p.mapA, kc, a * np + m0 + aoff + b * UM_BOX_ROWS, lead_full);
