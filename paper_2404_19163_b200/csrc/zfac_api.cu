@@ -589,7 +589,7 @@ zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void
   } else if (c->mode == ZFAC_MODE_SPLIT16) {
     switch (which) {
       case ZFAC_BUF_T: peek_kernel<float, 1><<<g, 256, 0, s>>>(ws + L.off_T, d_out, ld, n, np); break;
-      case ZFAC_BUF_R: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
+      case ZFAC_BUF_R: peek_kernel<float, 3><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
       case ZFAC_BUF_Q: peek_kernel<float, 1><<<g, 256, 0, s>>>(ws + L.off_Qb, d_out, ld, n, np); break;
       case ZFAC_BUF_Z: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_Z[0], d_out, ld, n, np); break;
       default: return ZFAC_E_INVALID;
@@ -597,7 +597,7 @@ zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void
   } else {  // HH16
     switch (which) {
       case ZFAC_BUF_T: peek_kernel<float, 2><<<g, 256, 0, s>>>(ws + L.off_T, d_out, ld, n, np); break;
-      case ZFAC_BUF_R: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
+      case ZFAC_BUF_R: peek_kernel<float, 3><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np); break;
       case ZFAC_BUF_Q: peek_kernel<float, 2><<<g, 256, 0, s>>>(ws + L.off_Qb, d_out, ld, n, np); break;
       case ZFAC_BUF_Z: peek_kernel<float, 0><<<g, 256, 0, s>>>(ws + L.off_Z[0], d_out, ld, n, np); break;
       default: return ZFAC_E_INVALID;

@@ -268,14 +268,15 @@ __global__ void refi_merge_kernel(const double* err64, int n64, int refi_steps, 
 }
 
 // ------------------------------------------------------------------ peek (tests)
-// kind 0: plain T buffer; 1: fp16 pair hi + lo' 2^-11; 2: fp16 (hi only)
+// kind 0: plain T buffer; 1: fp16 pair hi + lo' 2^-11; 2: fp16 (hi only); 3: plain T buffer of a SYMMETRIC matrix of
+// which only the upper triangle of tiles is stored (the FP32 R of the 16-bit modes): element (r, c), r > c, is (c, r)
 template <typename T, int KIND>
 __global__ void __launch_bounds__(256) peek_kernel(const void* src, void* out, int64_t ld, int n, int np) {
   const int c = blockIdx.x * 256 + threadIdx.x, r = blockIdx.y;
   if (c >= n || r >= n) return;
-  const size_t o = (size_t)r * np + c, np2 = (size_t)np * np;
+  const size_t o = (KIND == 3 && r > c) ? (size_t)c * np + r : (size_t)r * np + c, np2 = (size_t)np * np;
   T v;
-  if (KIND == 0) v = static_cast<const T*>(src)[o];
+  if (KIND == 0 || KIND == 3) v = static_cast<const T*>(src)[o];
   else if (KIND == 1) {
     const __half* h = static_cast<const __half*>(src);
     v = (T)(__half2float(h[o]) + __half2float(h[np2 + o]) * LO_UNSCALE);

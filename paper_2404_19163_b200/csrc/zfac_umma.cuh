@@ -288,9 +288,15 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
     store_f32_row<SUB>(p.f32_out + off, v);
     if (KIND != KIND_TF32) store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
     if (offdiag) {
+      // mirror: the operand of a4 needs the whole matrix -- the fp16 plane(s), or in TF32 mode the FP32 buffer itself.
+      // The FP32 copy of the 16-bit modes is read by a4's / p2's epilogue only, at upper-triangle tiles: its lower
+      // triangle is never written (zfac_peek reads the upper one).
+      if (KIND == KIND_TF32) {
 #pragma unroll
-      for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
-      if (KIND != KIND_TF32) store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
+        for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
+      } else {
+        store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
+      }
     }
   } else if (EPI == EPI_X3) {                           // X = Z^T H Z itself (congruence), mirror
     store_f32_row<SUB>(p.f32_out + off, v);
