@@ -360,7 +360,12 @@ def run_ours(args):
     from paper_2404_19163_b200 import build as zbuild
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (sm_100a); there is no CPU path for --impl ours")
-    rank, local_rank, world = replicas.init("nccl")
+    # ZFAC_BENCH_BACKEND=gloo: rendezvous over gloo, ranks mapped onto the visible GPUs modulo their count -- a check of
+    # the N > 1 control flow on a one-GPU box (replicas share no kernel-level dependency); never a reported number
+    backend = os.environ.get("ZFAC_BENCH_BACKEND", "nccl")
+    rank, local_rank, world = replicas.init(backend)
+    if backend != "nccl":
+        local_rank %= torch.cuda.device_count()
     dev = torch.device(f"cuda:{local_rank}")
     torch.cuda.set_device(dev)
     if not os.path.exists(zb.LIB_PATH):
@@ -380,7 +385,7 @@ def run_ours(args):
             sampler = ClockSampler(local_rank) if with_clock else None
             ms, iters, flags, err, prof, clocks, launches, ms_prof = time_refine(
                 zf, S, Z0, Zout, args.max_iter, stop, args.steps, args.warmup, dev, profile=True, sampler=sampler,
-                sync_fn=replicas.barrier)
+                sync_fn=replicas.barrier if with_e2e else None)   # the primary mode runs on every rank; the others on rank 0 only
             ks = kernel_stats(prof, iters)
             res = {"ms_per_step": ms, "ms_per_step_profiled": ms_prof, "iters": iters, "flags": flags, "err": [float(x) for x in err],
                    "launches": launches, "kernel_ms": {f"a{sid}": v[0] for sid, v in sorted(ks.items())},
@@ -436,9 +441,16 @@ def run_ours(args):
     extra = {}
     if rank == 0 and not args.quick:
         primary["final_residual_per_sqrt_n"] = invariant(primary.pop("Z"))
+    else:
+        primary.pop("Z", None)
+    if rank == 0 and world == 1 and not args.quick:      # single-GPU diagnostics; at N > 1 the other ranks would idle in the all-reduce
         for mode in [m for m in ("f64", "tf32", "split16") if m != args.mode]:
             r = run_mode(mode, with_e2e=False, with_clock=False)
             r["final_residual_per_sqrt_n"] = invariant(r.pop("Z"))
+            if r["flags"] & zb.ZFAC_R_NONFINITE:
+                r["note"] = ("ZFAC_R_NONFINITE: this mode's operand rounding times the workload's condition number puts "
+                             "||R_0||_2 above 1, outside the method's convergence region (DESIGN.md §2 Q10: TF32 at "
+                             "kappa = 1e5); the timing stands, the result is flagged, not usable")
             extra[mode] = r
         # iterations / s (BASELINE.json's metric names it for split-FP16 and FP64 at N = 8192): SURVEY.md §8(d)'s difference
         # quotient over fixed-count runs, t_iter = (t(k2) - t(k1)) / (k2 - k1), which cancels copy-in, copy-out and the
@@ -489,8 +501,6 @@ def run_ours(args):
                 del Sd, lam, V, Zr
         except Exception as ex:  # reference point only
             extra["syevd_inv_sqrt_ms"] = {"error": str(ex)[:100]}
-    else:
-        primary.pop("Z", None)
     if rank == 0 and args.sweep:
         torch.cuda.empty_cache()
         extra["sweep"] = run_sweep(args, dev, peaks)

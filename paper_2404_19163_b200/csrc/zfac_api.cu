@@ -129,10 +129,18 @@ zfac_status zfac_set_profile(zfac_ctx* c, int enable) {
   if (!c) return ZFAC_E_INVALID;
   if (enable && c->prof.cap == 0) {
     const int cap = 1024;
-    c->prof.ev = new (std::nothrow) cudaEvent_t[cap];
-    c->prof.tags = new (std::nothrow) int[cap];
+    if (!c->prof.ev) c->prof.ev = new (std::nothrow) cudaEvent_t[cap];
+    if (!c->prof.tags) c->prof.tags = new (std::nothrow) int[cap];
     if (!c->prof.ev || !c->prof.tags) return ZFAC_E_INVALID;
-    for (int i = 0; i < cap; ++i) ZF_CUDA(cudaEventCreate(&c->prof.ev[i]));
+    int made = 0;
+    for (; made < cap; ++made)
+      if (cudaEventCreate(&c->prof.ev[made]) != cudaSuccess) break;
+    if (made < cap) {                       // all or nothing: zfac_destroy only sees prof.cap events
+      for (int i = 0; i < made; ++i) cudaEventDestroy(c->prof.ev[i]);
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "zfac_set_profile: cudaEventCreate failed after %d events", made);
+      (void)cudaGetLastError();
+      return ZFAC_E_CUDA;
+    }
     c->prof.cap = cap;
   }
   c->prof.on = enable != 0;

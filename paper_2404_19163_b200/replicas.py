@@ -38,6 +38,8 @@ def aggregate(elapsed_ms: float, units: float, device: str | torch.device = "cpu
     independent replicas is sum(units) / max(time)."""
     if not dist.is_initialized():
         return float(elapsed_ms), float(units)
+    if dist.get_backend() == "gloo":
+        device = "cpu"
     t = torch.tensor([elapsed_ms], dtype=torch.float64, device=device)
     u = torch.tensor([units], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
