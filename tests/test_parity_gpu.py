@@ -452,6 +452,56 @@ def test_leading_dimension_and_aliasing(mode):
     assert _rel(Zbig[:, :n].cpu().double().numpy(), ref.Z) <= TOL[mode]
 
 
+@pytest.mark.parametrize("case", range(32))
+def test_seeded_random_shapes_strides_modes_orders(case):
+    """Seeded random sweep over what the fixed cases hold constant: N anywhere in 1..640 (not only tile boundaries),
+    three DIFFERENT, mostly unaligned leading dimensions for S, Z0 and Z (odd FP32 pitches take the scalar copy paths),
+    mode, order m, stop rule, update count, conditioning and size of the start's perturbation.  NaN guards around every
+    user buffer; element-wise parity against the oracle run for the same number of updates."""
+    b = zb()
+    rng = np.random.default_rng([2404, 19163, case])
+    mode = ["f64", "split16", "tf32", "hh16"][case % 4]           # every mode gets 8 cases
+    n = int(rng.integers(1, 641)) if case >= 4 else [1, 3, 640, 513][case]
+    m = int(rng.integers(2, 5))
+    lds, ldz0, ldz = (n + int(rng.integers(0, 38)) for _ in range(3))
+    paper_stop = bool(rng.integers(0, 2))
+    k = 40 if paper_stop else int(rng.integers(0, 6))
+    kappa = float(10.0 ** rng.uniform(0.3, 1.3 if mode in ("tf32", "hh16") else 1.7))   # 11-bit operands: gate 1e-3 needs kappa <~ 20
+    pert = float(rng.uniform(0.02, 0.12))
+    w = W.random_spd_general(n, seed=int(rng.integers(0, 2 ** 31)), kappa=kappa, pert=pert, fp32_stored=True)
+    dt = _dt(mode)
+    bufs = []
+    for ld in (lds, ldz0, ldz):
+        bufs.append(torch.full((n + 2, ld), float("nan"), dtype=dt, device=DEV))     # guard rows above and below
+    Sb, Z0b, Zb = bufs
+    Sb[1:n + 1, :n] = _to_dev(w.S, mode)
+    Z0b[1:n + 1, :n] = _to_dev(w.Z0, mode)
+    with b.Zfac(n, mode, DEV) as zf:
+        if m != 2:
+            zf.set_order(m)
+        out, it, err, fl = zf.refine(Sb[1:n + 1, :n], Z0b[1:n + 1, :n], max_iter=k,
+                                     stop=b.ZFAC_STOP_PAPER if paper_stop else b.ZFAC_STOP_FIXED, out=Zb[1:n + 1, :n])
+    assert torch.isnan(Zb[0]).all() and torch.isnan(Zb[n + 1]).all() and torch.isnan(Zb[1:n + 1, n:]).all()
+    assert torch.equal(Sb[1:n + 1, :n], _to_dev(w.S, mode)) and torch.equal(Z0b[1:n + 1, :n], _to_dev(w.Z0, mode))
+    assert len(err) == it + 1
+    if paper_stop:
+        assert (fl & b.ZFAC_R_STOPPED) or (it == 40 and err[-1] <= 1e-300)
+    else:
+        assert it == k and fl == b.ZFAC_R_MAXITER
+    ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED, order=m)
+    Z = Zb[1:n + 1, :n].cpu().double().numpy()
+    rel = _rel(Z, ref.Z)
+    print(f"[case {case}: {mode} n={n} m={m} ld=({lds},{ldz0},{ldz}) {'paper' if paper_stop else 'fixed'} k={k} "
+          f"kappa={kappa:.1f} pert={pert:.3f}] iters={it} rel={rel:.3e}")
+    tol = 2.5e-3 if (mode in ("tf32", "hh16") and n < 32) else TOL[mode]
+    assert rel <= tol
+    floor = {"f64": 1e-10, "split16": 1e-4, "tf32": 3e-2, "hh16": 3e-2}[mode] * max(1.0, math.sqrt(n))
+    for j in range(it + 1):
+        if ref.err[j] > floor:
+            assert err[j] == pytest.approx(ref.err[j], rel={"f64": 1e-8, "split16": 1e-3, "tf32": 5e-2, "hh16": 5e-2}[mode],
+                                           abs=err_abs(mode, n))
+
+
 def test_invalid_arguments_and_no_fallback():
     b = zb()
     assert b.zfac_workspace_bytes(0, b.ZFAC_MODE_F64) == 0
