@@ -673,6 +673,81 @@ def test_congruence_against_oracle(mode, n):
     assert rel <= {"f64": 1e-13, "split16": 2e-6, "tf32": 2e-3, "hh16": 2e-3}[mode]
 
 
+@pytest.mark.parametrize("case", range(24))
+def test_seeded_random_other_entry_points(case):
+    """The same kind of seeded sweep through the remaining entry points, each with random N and distinct unaligned
+    leading dimensions: zfac_refine_host (pinned and pageable), zfac_congruence, zfac_refine_refi, zfac_graph_*."""
+    b = zb()
+    rng = np.random.default_rng([19163, 2404, case])
+    entry = ["host", "congruence", "refi", "graph"][case % 4]
+    mode = ["split16", "f64", "tf32", "hh16"][(case // 4) % 4]
+    if entry == "refi" and mode == "f64":
+        mode = "split16"                                   # the low-precision stage of Alg. 3 is never F64
+    n = int(rng.integers(1, 601))
+    m = int(rng.integers(2, 5)) if entry in ("host", "graph") else 2
+    lda, ldb, ldc = (n + int(rng.integers(0, 30)) for _ in range(3))
+    kappa = float(10.0 ** rng.uniform(0.3, 1.3))
+    w = W.random_spd_general(n, seed=int(rng.integers(0, 2 ** 31)), kappa=kappa, pert=float(rng.uniform(0.03, 0.12)),
+                             fp32_stored=True)
+    dt = _dt(mode)
+    tol = 2.5e-3 if (mode in ("tf32", "hh16") and n < 32) else TOL[mode]
+    tag = f"[case {case}: {entry} {mode} n={n} m={m} ld=({lda},{ldb},{ldc}) kappa={kappa:.1f}]"
+
+    def strided(a, ld, host=False, pin=False):
+        t = torch.full((n, ld), float("nan"), dtype=dt, device="cpu" if host else DEV)
+        if pin:
+            t = t.pin_memory()
+        if a is not None:
+            t[:, :n] = torch.from_numpy(np.ascontiguousarray(a)).to(dt)
+        return t
+
+    if entry == "host":
+        pin = bool(rng.integers(0, 2))
+        Sb, Z0b, Zb = strided(w.S, lda, True, pin), strided(w.Z0, ldb, True, pin), strided(None, ldc, True, pin)
+        with b.Zfac(n, mode, DEV) as zf:
+            if m != 2:
+                zf.set_order(m)
+            _, it, err, fl = zf.refine_host(Sb[:, :n], Z0b[:, :n], Zb[:, :n], max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        assert torch.isnan(Zb[:, n:]).all() and len(err) == it + 1
+        ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED, order=m)
+        rel = _rel(Zb[:, :n].double().numpy(), ref.Z)
+    elif entry == "congruence":
+        H = rng.standard_normal((n, n)); H = W.round_fp32(0.5 * (H + H.T))
+        Hb, Zin, Ob = strided(H, lda), strided(w.Z0, ldb), strided(None, ldc)
+        with b.Zfac(n, mode, DEV) as zf:
+            zf.congruence(Hb[:, :n], Zin[:, :n], out=Ob[:, :n])
+            torch.cuda.synchronize()
+        assert torch.isnan(Ob[:, n:]).all()
+        rel = _rel(Ob[:, :n].cpu().double().numpy(), O.congruence(H, w.Z0))
+        tol = {"f64": 1e-13, "split16": 2e-6, "tf32": 2e-3, "hh16": 2e-3}[mode]
+        if mode in ("tf32", "hh16") and n < 32:
+            tol = 5e-3
+    elif entry == "refi":
+        steps = int(rng.integers(1, 3))
+        Sb, Z0b = strided(w.S, lda), strided(w.Z0, ldb)
+        with b.Zfac(n, mode, DEV) as zl, b.Zfac(n, "f64", DEV) as zh:
+            Z, it, err, fl = zl.refine_refi(zh, Sb[:, :n], Z0b[:, :n], max_iter=0, refi_steps=steps, final_check=True)
+        ref = O.refine(w.S, w.Z0, steps, O.STOP_FIXED)
+        assert it == steps and (fl & b.ZFAC_R_REFINED) and len(err) == steps + 2
+        rel = _rel(Z.cpu().numpy(), ref.Z)
+        tol = 1e-11
+    else:
+        Sb, Z0b, Zb = strided(w.S, lda), strided(w.Z0, ldb), strided(None, ldc)
+        with b.Zfac(n, mode, DEV) as zf:
+            if m != 2:
+                zf.set_order(m)
+            with b.ZfacLoopGraph(zf, Sb[:, :n], Z0b[:, :n], max_iter=30, stop=b.ZFAC_STOP_PAPER, out=Zb[:, :n]) as lg:
+                lg.launch(sync=True)
+                it = int(lg.d_iters.item())
+                lg.launch(sync=True)                        # a second launch of the same graph: same answer
+                assert int(lg.d_iters.item()) == it
+        assert torch.isnan(Zb[:, n:]).all() and it >= 1
+        ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED, order=m)
+        rel = _rel(Zb[:, :n].cpu().double().numpy(), ref.Z)
+    print(f"{tag} rel={rel:.3e}")
+    assert rel <= tol
+
+
 # ------------------------------------------------------------------ BASELINE configs at (near) full size
 def test_config2_n2048_all_modes():
     """BASELINE configs[1]: N=2048 banded-decay overlap, FP32 stored, all three modes."""
