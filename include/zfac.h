@@ -147,7 +147,13 @@ zfac_status zfac_congruence(zfac_ctx* ctx, const void* d_H, int64_t ldh, const v
  * With a PINNED h_Z and max_iter >= 1 the download of Z starts right after the first update, on an internal side stream:
  * if that update is the only one (a warm start) it has overlapped the final residual evaluation; otherwise the normal
  * download at the end supersedes it (measured, N = 8192 SPLIT16 warm start: 24.7 -> 20.9 ms per call; three-update HH16 run:
- * unchanged).  Results are bit-identical either way; ZFAC_HOST_OVERLAP=0 disables it. */
+ * unchanged).  Results are bit-identical either way; ZFAC_HOST_OVERLAP=0 disables it.
+ * With PINNED h_S and h_Z0, a tensor-core mode (not ZFAC_MODE_F64) and a padded dimension of at least 1024, the UPLOAD
+ * is overlapped as well: Z0 goes first, then S in up to 8 chunks of whole 256-row blocks on the side stream; rows
+ * [r0, r1) of S are all that step a1 needs for columns [r0, r1) of T = (S Z)^T, so each chunk is converted (step a0,
+ * S only) and multiplied (a1 restricted to that band of tiles) while the next chunk is still on the bus.  The bands
+ * are disjoint sets of whole tiles: bit-identical to the single launch (measured, same workload: 20.7 -> 18.6 ms per
+ * call; 8 + 7 extra launches).  ZFAC_HOST_UPLOAD_OVERLAP=0 disables it.  Pageable buffers take the plain path. */
 zfac_status zfac_refine_host(zfac_ctx* ctx, const void* h_S, int64_t lds, const void* h_Z0,
                              int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, zfac_stop stop,
                              int* h_iters, double* h_err, int* h_flags, void* stream);

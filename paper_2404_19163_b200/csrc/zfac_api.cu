@@ -38,8 +38,10 @@ struct zfac_ctx {
   int order;       // m of Eq. 13 (zfac_set_order): 2 (default), 3, 4
   UmmaPlan umma;   // tensor maps + launch geometry for the tcgen05 modes
   F64Plan f64p;    // tensor maps of the FP64 buffers (ZFAC_MODE_F64)
-  cudaStream_t side = nullptr;                 // zfac_refine_host: stream of the speculative copy-out (created lazily)
+  cudaStream_t side = nullptr;                 // zfac_refine_host: stream of the chunked upload and the early download (lazy)
   cudaEvent_t ev_a5 = nullptr, ev_copy = nullptr;
+  static constexpr int UP_CHUNKS = 8;            // zfac_refine_host: S is uploaded in at most this many row chunks
+  cudaEvent_t ev_begin = nullptr, ev_up[1 + UP_CHUNKS] = {};
   Prof prof;
 };
 
@@ -116,6 +118,8 @@ zfac_status zfac_destroy(zfac_ctx* ctx) {
   if (ctx) {
     if (ctx->ev_a5) cudaEventDestroy(ctx->ev_a5);
     if (ctx->ev_copy) cudaEventDestroy(ctx->ev_copy);
+    if (ctx->ev_begin) cudaEventDestroy(ctx->ev_begin);
+    for (cudaEvent_t e : ctx->ev_up) if (e) cudaEventDestroy(e);
     if (ctx->side) cudaStreamDestroy(ctx->side);
     for (int i = 0; i < ctx->prof.cap; ++i) cudaEventDestroy(ctx->prof.ev[i]);
     delete[] ctx->prof.ev;
@@ -239,7 +243,7 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
     q.residual(n, n, s, &c->prof);
     if (n == max_iter) break;
     q.update(n & 1, n, n, s, &c->prof);
-    if (hook) hook->after_a5(hook->self, n, s);
+    if (hook && hook->after_a5) hook->after_a5(hook->self, n, s);
   }
   c->prof.mark(s, 0);
   ZF_CUDA(cudaGetLastError());
@@ -247,15 +251,17 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
 }
 
 // Step a0: copy S and Z0 (element type float if in_f32, else the mode's own) into the padded buffers.
+// what: 1 = S only, 2 = Z0 (W, State reset) only, 3 = both; tile rows [ty0, ty0 + tyn) of CI_TR rows each (tyn = 0: all).
 static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, bool in_f32,
-                           cudaStream_t s) {
+                           cudaStream_t s, int what = 3, int ty0 = 0, int tyn = 0) {
   const Layout& L = c->L;
   char* ws = c->ws;
   CopyInArgs ci{};
   ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np;
   ci.st = reinterpret_cast<State*>(ws + L.off_state);
   ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
-  dim3 gi((unsigned)(L.np / CI_TC), (unsigned)(L.np / CI_TR)), bi(256);
+  ci.what = what; ci.ty0 = ty0;
+  dim3 gi((unsigned)(L.np / CI_TC), (unsigned)(tyn > 0 ? tyn : L.np / CI_TR)), bi(256);
   switch (c->mode) {
     case ZFAC_MODE_F64:
       if (in_f32) copy_in_kernel<ZFAC_MODE_F64, float><<<gi, bi, 0, s>>>(ci);
@@ -292,7 +298,7 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
 
 static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
                                int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
-                               void* stream, const IterHook* hook) {
+                               void* stream, const IterHook* hook, int copy_what = 3) {
   if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
   if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
   if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
@@ -302,7 +308,7 @@ static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const 
   c->launches = 0;
   c->prof.count = 0;
 
-  launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, s);
+  launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, s, copy_what);     // copy_what = 2: the hook's first_a1 brings S in
 
   zfac_status rs;
   if (c->mode == ZFAC_MODE_F64) {
@@ -341,7 +347,32 @@ struct HostOverlap {
   zfac_ctx* c;
   void* h_Z;
   int64_t ldz;
+  const void* dS = nullptr;   // staged S (dense n x n), arriving in `chunks` row chunks; chunk k is complete at ev_up[1 + k]
+  int chunks = 0;
 };
+
+// Upload overlap (tcgen05 modes, pinned h_S): Z0 is uploaded first, then S in row chunks of whole macro-tile rows on
+// the side stream.  Rows [r0, r1) of S are all step a1 needs for the columns [r0, r1) of T = W S^T, so the main stream
+// converts each chunk (copy-in, S only) and runs a1 on that band while the next chunk is still on the bus; only the
+// last band's a1 is exposed.  Bands are disjoint sets of whole tiles: bit-identical to the one-launch a1.
+static void host_chunk_rows(const zfac_ctx* c, int chunks, int k, int* mc0, int* mcn) {
+  const int T = (int)(c->L.np / UM_MACRO);
+  *mc0 = (int)((int64_t)T * k / chunks);
+  *mcn = (int)((int64_t)T * (k + 1) / chunks) - *mc0;
+}
+static bool host_first_a1(void* self, void* seq, cudaStream_t s) {
+  HostOverlap* h = static_cast<HostOverlap*>(self);
+  if (h->chunks <= 0) return false;
+  zfac_ctx* c = h->c;
+  UmmaSeq* q = static_cast<UmmaSeq*>(seq);
+  for (int k = 0; k < h->chunks; ++k) {
+    int mc0, mcn; host_chunk_rows(c, h->chunks, k, &mc0, &mcn);
+    cudaStreamWaitEvent(s, c->ev_up[1 + k], 0);
+    launch_copy_in(c, h->dS, c->n, nullptr, c->n, false, s, 1, mc0 * (UM_MACRO / CI_TR), mcn * (UM_MACRO / CI_TR));
+    q->a1(mc0, mcn, s);
+  }
+  return true;
+}
 static void host_after_a5(void* self, int n, cudaStream_t s) {
   if (n != 0) return;
   HostOverlap* h = static_cast<HostOverlap*>(self);
@@ -431,8 +462,42 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   double* dErr = reinterpret_cast<double*>(c->ws + L.off_stage_out);
   int* dInts = reinterpret_cast<int*>(c->ws + L.off_stage_out + 4096 * sizeof(double));
   const size_t row = (size_t)c->n * L.elt;
-  ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
-  ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+  // upload overlap (see host_first_a1): tcgen05 modes, pinned h_S and h_Z0, at least 4 macro-tile rows
+  int chunks = 0;
+  if (c->mode != ZFAC_MODE_F64 && L.np / UM_MACRO >= 4) {
+    cudaPointerAttributes pS{}, pZ{};
+    const char* off = getenv("ZFAC_HOST_UPLOAD_OVERLAP");
+    if (!(off && off[0] == '0') && cudaPointerGetAttributes(&pS, h_S) == cudaSuccess && pS.type == cudaMemoryTypeHost &&
+        cudaPointerGetAttributes(&pZ, h_Z0) == cudaSuccess && pZ.type == cudaMemoryTypeHost) {
+      const int T = (int)(L.np / UM_MACRO);
+      chunks = T < zfac_ctx::UP_CHUNKS ? T : zfac_ctx::UP_CHUNKS;
+    }
+    (void)cudaGetLastError();
+  }
+  if (chunks > 0) {
+    if (!c->side) ZF_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+    if (!c->ev_begin) {
+      ZF_CUDA(cudaEventCreateWithFlags(&c->ev_begin, cudaEventDisableTiming));
+      for (cudaEvent_t& e : c->ev_up) ZF_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    ZF_CUDA(cudaEventRecord(c->ev_begin, s));                    // the uploads keep their place in the caller's stream order
+    ZF_CUDA(cudaStreamWaitEvent(c->side, c->ev_begin, 0));
+    ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, c->side));
+    ZF_CUDA(cudaEventRecord(c->ev_up[0], c->side));
+    for (int k = 0; k < chunks; ++k) {
+      int mc0, mcn; host_chunk_rows(c, chunks, k, &mc0, &mcn);
+      const int64_t r0 = (int64_t)mc0 * UM_MACRO < c->n ? (int64_t)mc0 * UM_MACRO : c->n;
+      const int64_t r1 = (int64_t)(mc0 + mcn) * UM_MACRO < c->n ? (int64_t)(mc0 + mcn) * UM_MACRO : c->n;
+      if (r1 > r0)
+        ZF_CUDA(cudaMemcpy2DAsync(dS + (size_t)r0 * row, row, static_cast<const char*>(h_S) + (size_t)r0 * lds * L.elt,
+                                  (size_t)lds * L.elt, row, (size_t)(r1 - r0), cudaMemcpyHostToDevice, c->side));
+      ZF_CUDA(cudaEventRecord(c->ev_up[1 + k], c->side));
+    }
+    ZF_CUDA(cudaStreamWaitEvent(s, c->ev_up[0], 0));            // Z0 is there: copy-in of Z0 (W, operand planes) can start
+  } else {
+    ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+    ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+  }
   // overlapped download: needs a pinned (device-visible) h_Z and at least one possible update
   bool z_dev = false;                             // early download possible: pinned h_Z (an async copy from pageable memory
   {                                               // is staged and may block) and at least one possible update
@@ -444,16 +509,16 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
     (void)cudaGetLastError();
   }
   HostOverlap ho{c, h_Z, ldz};
-  IterHook hook{host_after_a5, &ho};
+  ho.dS = dS; ho.chunks = chunks;
+  IterHook hook{z_dev ? host_after_a5 : nullptr, &ho};
+  if (chunks > 0) hook.first_a1 = host_first_a1;
   if (z_dev) {
-    if (!c->side) {
-      ZF_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
-      ZF_CUDA(cudaEventCreateWithFlags(&c->ev_a5, cudaEventDisableTiming));
-      ZF_CUDA(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
-    }
+    if (!c->side) ZF_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+    if (!c->ev_a5) ZF_CUDA(cudaEventCreateWithFlags(&c->ev_a5, cudaEventDisableTiming));
+    if (!c->ev_copy) ZF_CUDA(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
   }
   zfac_status rs = refine_impl(c, dS, c->n, dZ, c->n, dZ, c->n, max_iter, stop, dInts, dErr, dInts + 1, s,
-                               z_dev ? &hook : nullptr);
+                               (z_dev || chunks > 0) ? &hook : nullptr, chunks > 0 ? 2 : 3);
   if (rs != ZFAC_OK) return rs;
   if (z_dev) ZF_CUDA(cudaStreamWaitEvent(s, c->ev_copy, 0));   // the early download is complete (and can no longer land late)
   else ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));

@@ -52,6 +52,9 @@ struct Prof {
 struct IterHook {
   void (*after_a5)(void* self, int n, cudaStream_t s);
   void* self;
+  // tcgen05 modes: called once before the first residual with the sequencer (a zfac::UmmaSeq*); returns true if it has
+  // enqueued the copy-in of S and step a1 itself (zfac_refine_host: band by band behind the upload of S)
+  bool (*first_a1)(void* self, void* seq, cudaStream_t s) = nullptr;
 };
 
 __device__ __forceinline__ double warp_sum(double v) {

@@ -101,6 +101,8 @@ struct CopyInArgs {
   void* oZ;            // F64/TF32: Z[0];  SPLIT16: float Z32
   void* oW;            // F64/TF32: W;     SPLIT16: half[2][Np][Np]
   void* oZb;           // SPLIT16 / HH16: half[planes][Np][Np] (Zb[0])
+  int what;            // bit 0: S, bit 1: Z0 (and W, State reset); 0 is read as 3 (both)
+  int ty0;             // first tile row of this launch (grid.y counts from it): row chunks of S for zfac_refine_host
 };
 
 // One tile of CI_TR = 32 rows x CI_TC = 64 columns per CTA (256 threads).  Phase 1: coalesced loads of the S and Z0
@@ -148,11 +150,12 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
   __shared__ Tin sS[CI_TR * CI_PITCH];
   __shared__ Tin sZ[CI_TR * CI_PITCH];
   const int t = threadIdx.x;
-  if (blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
+  const bool doS = (a.what == 0) || (a.what & 1), doZ = (a.what == 0) || (a.what & 2);
+  if (doZ && blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
     a.st->done = 0; a.st->iters = 0; a.st->flags = 0;
     a.st->arrive[0] = a.st->arrive[1] = a.st->arrive[2] = a.st->arrive[3] = 0u;
   }
-  const int c0 = blockIdx.x * CI_TC, r0 = blockIdx.y * CI_TR;
+  const int c0 = blockIdx.x * CI_TC, r0 = ((int)blockIdx.y + a.ty0) * CI_TR;
   const size_t np = (size_t)a.np, np2 = np * np;
   const Tin* S = static_cast<const Tin*>(a.S);
   const Tin* Z0 = static_cast<const Tin*>(a.Z0);
@@ -163,8 +166,8 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
     const int r = r0 + lr, c = c0 + lc;
     const bool in = (r < a.n && c < a.n);
     const Tin ident = (r == c) ? Tin(1) : Tin(0);
-    sS[lr * CI_PITCH + lc] = in ? S[(size_t)r * a.lds + c] : ident;
-    sZ[lr * CI_PITCH + lc] = in ? Z0[(size_t)r * a.ldz0 + c] : ident;
+    if (doS) sS[lr * CI_PITCH + lc] = in ? S[(size_t)r * a.lds + c] : ident;
+    if (doZ) sZ[lr * CI_PITCH + lc] = in ? Z0[(size_t)r * a.ldz0 + c] : ident;
   }
   __syncthreads();
   // ---- phase 2: S and Z, 8 consecutive columns of one row per thread
@@ -175,24 +178,31 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
       Tw* oS = static_cast<Tw*>(a.oS); Tw* oZ = static_cast<Tw*>(a.oZ);
 #pragma unroll
       for (int j = 0; j < 8; j += 2) {
-        *reinterpret_cast<double2*>(reinterpret_cast<double*>(oS) + o + j) =
+        if (doS) *reinterpret_cast<double2*>(reinterpret_cast<double*>(oS) + o + j) =
             make_double2((double)sS[lr * CI_PITCH + lc + j], (double)sS[lr * CI_PITCH + lc + j + 1]);
-        *reinterpret_cast<double2*>(reinterpret_cast<double*>(oZ) + o + j) =
+        if (doZ) *reinterpret_cast<double2*>(reinterpret_cast<double*>(oZ) + o + j) =
             make_double2((double)sZ[lr * CI_PITCH + lc + j], (double)sZ[lr * CI_PITCH + lc + j + 1]);
       }
     } else {
-      float vs[8], vz[8];
+      if (doS) {
+        float vs[8];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) { vs[j] = (float)sS[lr * CI_PITCH + lc + j]; vz[j] = (float)sZ[lr * CI_PITCH + lc + j]; }
-      ci_store8<MODE>(a.oS, np2, o, vs, true);
-      float* z32 = static_cast<float*>(a.oZ);                       // FP32 Z (the master copy in the 16-bit modes): not rounded
-      *reinterpret_cast<float4*>(z32 + o) = make_float4(vz[0], vz[1], vz[2], vz[3]);
-      *reinterpret_cast<float4*>(z32 + o + 4) = make_float4(vz[4], vz[5], vz[6], vz[7]);
-      if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true);
+        for (int j = 0; j < 8; ++j) vs[j] = (float)sS[lr * CI_PITCH + lc + j];
+        ci_store8<MODE>(a.oS, np2, o, vs, true);
+      }
+      if (doZ) {
+        float vz[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) vz[j] = (float)sZ[lr * CI_PITCH + lc + j];
+        float* z32 = static_cast<float*>(a.oZ);                     // FP32 Z (the master copy in the 16-bit modes): not rounded
+        *reinterpret_cast<float4*>(z32 + o) = make_float4(vz[0], vz[1], vz[2], vz[3]);
+        *reinterpret_cast<float4*>(z32 + o + 4) = make_float4(vz[4], vz[5], vz[6], vz[7]);
+        if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true);
+      }
     }
   }
   // ---- phase 3: W = Z^T, 8 consecutive rows of one column of the tile per thread -> 8 consecutive elements of a row of W
-  {
+  if (doZ) {
     const int wr = t >> 2, wc = (t & 3) * 8;                        // W tile: CI_TC rows x CI_TR columns
     const size_t o = (size_t)(c0 + wr) * np + (size_t)(r0 + wc);
     if (MODE == ZFAC_MODE_F64) {

@@ -90,6 +90,8 @@ struct UmmaParams {
   void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
   void* out2;           // p2 (order m > 2): G operand buffer, same format as the mode's operands
   int band;             // full outputs: tile columns per rasterisation band (L2 reuse of the B column blocks)
+  int joff, jcols;      // full outputs: this launch covers tile columns [joff, joff + jcols) only (jcols = 0: all) --
+                        // zfac_refine_host runs a1 band by band while the row chunks of S are still arriving
   int hh_only;          // KIND_F16X2: 1 = this launch MAY use the (h)(h) pass only (D_x neither written nor read) ...
   double hh_err_max;    // ... and does so iff Err[n] = stop.d_err[stop.n_iter] <= hh_err_max (decided on the device)
   float q_r, q_d;       // a4: Q = q_r R + q_d D        (1/2, 3/8; m > 2: 1/2, 1)       see PolyCoef (zfac_f64.cuh)
@@ -419,7 +421,8 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int CH0 = (CH < KB && p.chunk0_kb > CH && KB / 4 > CH) ? (p.chunk0_kb < KB / 4 ? p.chunk0_kb : KB / 4) : CH;
   const int NCH = 1 + (KB - CH0 + CH - 1) / CH;                            // chunks per tile
   const int T = p.macro_tiles;
-  const int num_tiles = (SYM ? T * (T + 1) / 2 : T * T) * NSPLIT;         // 256 x TN pair tiles
+  const int JC = (!SYM && p.jcols > 0) ? p.jcols : T * NSPLIT;             // tile columns of this launch
+  const int num_tiles = SYM ? T * (T + 1) / 2 * NSPLIT : T * JC;          // 256 x TN pair tiles
   // One pass for a second-order product (a4 / p2, KIND_F16X2): taken by every thread of the grid from the Err[n] that
   // a2 of this iteration wrote (a completed kernel: visible), so issuer and epilogues of both CTAs agree.
   // (n_iter < 0, loop body of a zfac_graph: the update is taken from the last residual written, State::iters)
@@ -455,7 +458,8 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       n0 = J * UM_MACRO + sub * TN;
       offdiag = (I != J);
     } else {
-      band_decode(t, T, T * NSPLIT, p.band * NSPLIT, I, J);
+      band_decode(t, T, JC, p.band * NSPLIT, I, J);
+      J += p.joff;
       n0 = J * TN;
       offdiag = true;                                      // (unused by the full-output epilogues)
     }
@@ -882,6 +886,7 @@ struct UmmaSeq {
     grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
     grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
     order = order_;
+    nsplit_ = nsplit;
     p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band;
     p.st = reinterpret_cast<State*>(ws + L.off_state);
 #ifdef ZFAC_TIMING
@@ -896,25 +901,45 @@ struct UmmaSeq {
     h16 = (L.mode != ZFAC_MODE_TF32);
   }
 
-  // a1 + a2 (+ a3): residual number n_stop (-1: device-side index)
-  void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+  int nsplit_ = 1;
+
+  // a1 restricted to the macro-tile columns [mc0, mc0 + mcn) of T, i.e. to the rows [256 mc0, 256 (mc0 + mcn)) of S
+  // (mcn = 0: all of T).  Tiles do not overlap between bands, so a banded a1 is bit-identical to the full launch.
+  void a1(int mc0, int mcn, cudaStream_t s) {
     const Layout& L = pl.L;
     char* ws = pl.ws;
-    // a1: T = W S^T            (promoted accumulation: T and X are O(1) quantities, see DESIGN.md §5)
-    if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
     p.hh_only = 0;
     p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
     p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; }
-    umma_launch_mode(L.mode, EPI_A1, grid_full, s, p);
+    int grid = grid_full;
+    if (mcn > 0) {
+      p.joff = mc0 * nsplit_; p.jcols = mcn * nsplit_;
+      const int tiles = p.macro_tiles * p.jcols;
+      grid = 2 * (tiles < pl.max_pairs ? tiles : pl.max_pairs);
+    }
+    umma_launch_mode(L.mode, EPI_A1, grid, s, p);
+    p.joff = 0; p.jcols = 0;
+    nl += 1;
+  }
+
+  // a1 + a2 (+ a3): residual number n_stop (-1: device-side index); skip_a1: a1 was already enqueued band by band
+  void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof, bool skip_a1 = false) {
+    const Layout& L = pl.L;
+    char* ws = pl.ws;
+    // a1: T = W S^T            (promoted accumulation: T and X are O(1) quantities, see DESIGN.md §5)
+    if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
+    if (!skip_a1) a1(0, 0, s);
+    p.hh_only = 0; p.f32_in = nullptr; p.h_out_t = nullptr;
+    p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
     // a2: R = I - W T^T
     if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
     p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n_stop;
     p.chunk0_kb = 2 * pl.chunk0_kb;           // a2 writes four outputs per element: its stores take twice as long
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
     umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
-    nl += 2;
+    nl += 1;
   }
 
   // (p2,) a4, a5: update number n with n & 1 = par, taken from residual n_stop (-1: device-side index)
@@ -964,11 +989,12 @@ struct UmmaSeq {
 inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof,
                                const IterHook* hook = nullptr) {
   UmmaSeq q(pl, max_iter, stop, order, d_err, 0ull);
+  const bool banded = hook && hook->first_a1 && hook->first_a1(hook->self, &q, s);   // copy-in of S + a1, band by band
   for (int n = 0; n <= max_iter; ++n) {
-    q.residual(n, n, s, prof);
+    q.residual(n, n, s, prof, banded && n == 0);
     if (n == max_iter) break;
     q.update(n & 1, n, n, s, prof);
-    if (hook) hook->after_a5(hook->self, n, s);
+    if (hook && hook->after_a5) hook->after_a5(hook->self, n, s);
   }
   prof->mark(s, 0);
   *launches = q.nl;

@@ -600,6 +600,44 @@ def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise
         assert torch.equal(torch.nan_to_num(Z, nan=-1.0), torch.nan_to_num(Z0bad, nan=-1.0))
 
 
+@pytest.mark.parametrize("mode,n,pad", [("split16", 1000, 0), ("split16", 1500, 13), ("tf32", 1111, 5), ("hh16", 2048, 0),
+                                        ("split16", 2309, 3)])
+def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mode, n, pad, monkeypatch):
+    """zfac_refine_host with pinned S and Z0 (tensor-core modes, padded dimension >= 1024) uploads S in row chunks on a
+    side stream and runs copy-in + a1 band by band behind them (include/zfac.h).  The bands are disjoint sets of whole
+    tiles, so the call must return exactly what zfac_refine returns -- with the overlap on, off, with pageable inputs
+    (plain path), with ld > n, with max_iter = 0 (the banded a1 is the only a1), and on a second call of the same
+    context (events and side stream reused); 8 + 7 extra launches say the banded path really ran."""
+    b = zb()
+    w = W.random_spd_general(n, seed=n, kappa=15.0, pert=0.1, fp32_stored=True)
+    dt = _dt(mode)
+    Sd, Z0d = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
+    chunks = min(8, -(-n // 256))
+
+    def host(t, pin):
+        big = torch.full((n, n + pad), float("nan"), dtype=dt)
+        big[:, :n] = torch.from_numpy(t).to(dt)
+        return big.pin_memory() if pin else big
+
+    with b.Zfac(n, mode, DEV) as zf:
+        for max_iter in (30, 0):
+            Zref, itref, errref, flref = zf.refine(Sd, Z0d, max_iter=max_iter, stop=b.ZFAC_STOP_PAPER)
+            base = zf.last_launch_count
+            Zref = Zref.cpu()
+            for pin, overlap, reps in ((True, "1", 2), (True, "0", 1), (False, "1", 1)):
+                monkeypatch.setenv("ZFAC_HOST_UPLOAD_OVERLAP", overlap)
+                S, Z0 = host(w.S, pin), host(w.Z0, pin)
+                Zbig = torch.full((n, n + pad), -5.0, dtype=dt)
+                Zbig = Zbig.pin_memory() if pin else Zbig
+                for _ in range(reps):
+                    _, it, err, fl = zf.refine_host(S[:, :n], Z0[:, :n], Zbig[:, :n], max_iter=max_iter, stop=b.ZFAC_STOP_PAPER)
+                    assert it == itref and fl == flref and np.array_equal(err, errref), (max_iter, pin, overlap)
+                    assert torch.equal(Zbig[:, :n], Zref), (max_iter, pin, overlap)
+                    assert bool((Zbig[:, n:] == -5.0).all())
+                    banded = pin and overlap == "1"
+                    assert zf.last_launch_count == base + ((chunks - 1) + chunks if banded else 0), (max_iter, pin, overlap)
+
+
 # ------------------------------------------------------------------ Alg. 3 ("+refi") and the congruence transformation
 @pytest.mark.parametrize("low", ["split16", "hh16", "tf32"])
 @pytest.mark.parametrize("n", [130, 300])
