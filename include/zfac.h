@@ -153,7 +153,9 @@ zfac_status zfac_congruence(zfac_ctx* ctx, const void* d_H, int64_t ldh, const v
  * [r0, r1) of S are all that step a1 needs for columns [r0, r1) of T = (S Z)^T, so each chunk is converted (step a0,
  * S only) and multiplied (a1 restricted to that band of tiles) while the next chunk is still on the bus.  The bands
  * are disjoint sets of whole tiles: bit-identical to the single launch (measured, same workload: 20.7 -> 18.6 ms per
- * call; 8 + 7 extra launches).  ZFAC_HOST_UPLOAD_OVERLAP=0 disables it.  Pageable buffers take the plain path. */
+ * call; 8 + 7 extra launches).  ZFAC_HOST_UPLOAD_OVERLAP=0 disables it.  Pageable buffers take the plain path.
+ * In those modes the first update's a5 also runs in two row bands (pinned h_Z), each band's rows of Z downloaded as soon
+ * as they are final: 18.6 -> 17.9 ms; one extra launch; ZFAC_HOST_A5_BANDS=1 disables it. */
 zfac_status zfac_refine_host(zfac_ctx* ctx, const void* h_S, int64_t lds, const void* h_Z0,
                              int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, zfac_stop stop,
                              int* h_iters, double* h_err, int* h_flags, void* stream);

@@ -55,6 +55,10 @@ struct IterHook {
   // tcgen05 modes: called once before the first residual with the sequencer (a zfac::UmmaSeq*); returns true if it has
   // enqueued the copy-in of S and step a1 itself (zfac_refine_host: band by band behind the upload of S)
   bool (*first_a1)(void* self, void* seq, cudaStream_t s) = nullptr;
+  // tcgen05 modes, first update only: a5_bands > 1 runs a5 in that many row bands and calls after_a5_band after each
+  // (rows [r0, r1) of the padded Z_1 are final; last = the whole of Z_1 is) INSTEAD of after_a5(0)
+  int a5_bands = 1;
+  void (*after_a5_band)(void* self, int r0, int r1, bool last, cudaStream_t s) = nullptr;
 };
 
 __device__ __forceinline__ double warp_sum(double v) {

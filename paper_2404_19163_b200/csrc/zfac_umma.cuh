@@ -90,6 +90,8 @@ struct UmmaParams {
   void* h_out_t;        // 16-bit modes: a5: W16 (transposed)                         TF32: a5: W32
   void* out2;           // p2 (order m > 2): G operand buffer, same format as the mode's operands
   int band;             // full outputs: tile columns per rasterisation band (L2 reuse of the B column blocks)
+  int ioff, irows;      // full outputs: ... and tile rows [ioff, ioff + irows) only (irows = 0: all): a5 in row bands, so
+                        // that zfac_refine_host can start downloading the finished rows of Z
   int joff, jcols;      // full outputs: this launch covers tile columns [joff, joff + jcols) only (jcols = 0: all) --
                         // zfac_refine_host runs a1 band by band while the row chunks of S are still arriving
   int hh_only;          // KIND_F16X2: 1 = this launch MAY use the (h)(h) pass only (D_x neither written nor read) ...
@@ -422,7 +424,8 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int NCH = 1 + (KB - CH0 + CH - 1) / CH;                            // chunks per tile
   const int T = p.macro_tiles;
   const int JC = (!SYM && p.jcols > 0) ? p.jcols : T * NSPLIT;             // tile columns of this launch
-  const int num_tiles = SYM ? T * (T + 1) / 2 * NSPLIT : T * JC;          // 256 x TN pair tiles
+  const int TI = (!SYM && p.irows > 0) ? p.irows : T;                      // tile rows of this launch
+  const int num_tiles = SYM ? T * (T + 1) / 2 * NSPLIT : TI * JC;         // 256 x TN pair tiles
   // One pass for a second-order product (a4 / p2, KIND_F16X2): taken by every thread of the grid from the Err[n] that
   // a2 of this iteration wrote (a completed kernel: visible), so issuer and epilogues of both CTAs agree.
   // (n_iter < 0, loop body of a zfac_graph: the update is taken from the last residual written, State::iters)
@@ -458,7 +461,8 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       n0 = J * UM_MACRO + sub * TN;
       offdiag = (I != J);
     } else {
-      band_decode(t, T, JC, p.band * NSPLIT, I, J);
+      band_decode(t, TI, JC, p.band * NSPLIT, I, J);
+      I += p.ioff;
       J += p.joff;
       n0 = J * TN;
       offdiag = true;                                      // (unused by the full-output epilogues)
@@ -943,7 +947,9 @@ struct UmmaSeq {
   }
 
   // (p2,) a4, a5: update number n with n & 1 = par, taken from residual n_stop (-1: device-side index)
-  void update(int par, int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+  // hook + bands > 1: a5 runs in `bands` launches over whole macro-tile rows; after each, hook->after_a5_band is told
+  // which rows of Z_next are final (disjoint whole tiles: bit-identical to the single launch)
+  void update(int par, int n_stop, int tagn, cudaStream_t s, Prof* prof, const IterHook* hook = nullptr, int bands = 1) {
     const Layout& L = pl.L;
     char* ws = pl.ws;
     p.stop.n_iter = n_stop;
@@ -981,6 +987,19 @@ struct UmmaSeq {
       p.f32_in = reinterpret_cast<float*>(ws + L.off_Z[par]);
       p.f32_out = reinterpret_cast<float*>(ws + L.off_Z[(par + 1) & 1]); p.h_out = nullptr; p.h_out_t = ws + L.off_W;
     }
+    if (hook && bands > 1 && hook->after_a5_band) {
+      const int T = p.macro_tiles;
+      for (int b = 0; b < bands; ++b) {
+        const int i0 = (int)((long long)T * b / bands), i1 = (int)((long long)T * (b + 1) / bands);
+        p.ioff = i0; p.irows = i1 - i0;
+        const int tiles = p.irows * T * nsplit_;
+        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.max_pairs ? tiles : pl.max_pairs), s, p);
+        hook->after_a5_band(hook->self, i0 * UM_MACRO, i1 * UM_MACRO, b == bands - 1, s);
+      }
+      p.ioff = 0; p.irows = 0;
+      nl += 1 + bands;
+      return;
+    }
     umma_launch_mode(L.mode, EPI_A5, grid_full, s, p);
     nl += 2;
   }
@@ -993,8 +1012,9 @@ inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int o
   for (int n = 0; n <= max_iter; ++n) {
     q.residual(n, n, s, prof, banded && n == 0);
     if (n == max_iter) break;
-    q.update(n & 1, n, n, s, prof);
-    if (hook && hook->after_a5) hook->after_a5(hook->self, n, s);
+    const bool a5_banded = (n == 0 && hook && hook->a5_bands > 1 && hook->after_a5_band);
+    q.update(n & 1, n, n, s, prof, hook, a5_banded ? hook->a5_bands : 1);
+    if (hook && hook->after_a5 && !a5_banded) hook->after_a5(hook->self, n, s);
   }
   prof->mark(s, 0);
   *launches = q.nl;

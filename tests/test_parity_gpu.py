@@ -607,7 +607,8 @@ def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mo
     side stream and runs copy-in + a1 band by band behind them (include/zfac.h).  The bands are disjoint sets of whole
     tiles, so the call must return exactly what zfac_refine returns -- with the overlap on, off, with pageable inputs
     (plain path), with ld > n, with max_iter = 0 (the banded a1 is the only a1), and on a second call of the same
-    context (events and side stream reused); 8 + 7 extra launches say the banded path really ran."""
+    context (events and side stream reused); the launch counts say the banded paths really ran.  With a pinned Z the
+    first a5 runs in two row bands and each band's rows are downloaded as soon as they are final."""
     b = zb()
     w = W.random_spd_general(n, seed=n, kappa=15.0, pert=0.1, fp32_stored=True)
     dt = _dt(mode)
@@ -635,7 +636,22 @@ def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mo
                     assert torch.equal(Zbig[:, :n], Zref), (max_iter, pin, overlap)
                     assert bool((Zbig[:, n:] == -5.0).all())
                     banded = pin and overlap == "1"
-                    assert zf.last_launch_count == base + ((chunks - 1) + chunks if banded else 0), (max_iter, pin, overlap)
+                    a5_bands = pin and max_iter >= 1          # pinned h_Z: the first a5 runs in two row bands (early download)
+                    assert zf.last_launch_count == base + ((chunks - 1) + chunks if banded else 0) + (1 if a5_bands else 0), \
+                        (max_iter, pin, overlap)
+        # exactly one update (a converged start): the rows downloaded band by band behind the first a5 ARE the result
+        monkeypatch.setenv("ZFAC_HOST_UPLOAD_OVERLAP", "1")
+        lam, V = np.linalg.eigh(w.S)
+        Zc = W.round_fp32((V / np.sqrt(lam)) @ V.T)
+        Zr1, it1, err1, fl1 = zf.refine(Sd, _to_dev(Zc, mode), max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        if it1 == 1:
+            S, Z0 = host(w.S, True), host(Zc, True)
+            Zbig = torch.full((n, n + pad), -5.0, dtype=dt).pin_memory()
+            _, it, err, fl = zf.refine_host(S[:, :n], Z0[:, :n], Zbig[:, :n], max_iter=30, stop=b.ZFAC_STOP_PAPER)
+            assert it == 1 and fl == fl1 and np.array_equal(err, err1) and torch.equal(Zbig[:, :n], Zr1.cpu())
+            assert bool((Zbig[:, n:] == -5.0).all())
+        else:
+            assert mode in ("tf32", "hh16")                   # 11-bit operands: the FP32-rounded exact factor is not at their floor
 
 
 # ------------------------------------------------------------------ Alg. 3 ("+refi") and the congruence transformation
