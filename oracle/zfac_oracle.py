@@ -65,6 +65,11 @@ rationals from the vanishing condition alone; m = 2 mapped onto the printed a_k;
 tail t_k > 0 with sum 1 and, for m = 2, equal to the printed c, d, e; a scalar
 exact-rational step; the matrix identity R_1 = sum t_k R_0^k for non-symmetric Z0;
 Z -> S^-1/2 from numpy.linalg.eigh; observed order m + 1; the generalised stop test.
+`refine_with_refi` / `update_mixed` (Alg. 3; tests/test_oracle_refi_pins.py): the err[] layout entry by entry
+against norms formed directly from the returned low-precision Z; a float32 refinement of a float16 run lands at
+the level of a pure float32 run (PAPER.md:374); a float64 refinement reaches the FP64 floor (PAPER.md:392);
+the mixed update leaves u_update ||R|| in the next residual and two mixed steps reach the FP64 floor, while a
+run whose MASTER is float32 cannot; update_dtype = float64 reproduces the plain update bit for bit.
 Every function below is pinned; none is "parity unpinned".
 """
 from __future__ import annotations
@@ -226,22 +231,51 @@ def spectral_closed_form(lam: np.ndarray, alpha: float, iters: int, order: int =
     return SpectralResult(z, np.asarray(err, dtype=np.float64))
 
 
+def update_mixed(Z: np.ndarray, R: np.ndarray, update_dtype) -> np.ndarray:
+    """Z_{n+1} = Z_n + D with the correction D = Z_n (1/2 R + 3/8 R R) (Eq. 16 form of Eq. 13, m = 2) evaluated
+    in `update_dtype` from the operands rounded to it, and ADDED to the master Z in Z's own precision.  This is
+    step 3 of Sec. IV.B when only the residual of step 2 is recomputed in the enhanced
+    precision: D is a correction of relative size ||R||, so its rounding error u_update ||R|| is what is left
+    of the update in the next residual (reading Q-R2)."""
+    Ru = np.asarray(R, dtype=update_dtype)
+    Zu = np.asarray(Z, dtype=update_dtype)
+    Q = 0.5 * Ru + 0.375 * (Ru @ Ru)
+    D = Zu @ Q
+    return Z + np.asarray(D, dtype=Z.dtype)
+
+
 def refine_with_refi(S: np.ndarray, Z0: np.ndarray, max_iter: int, low_dtype=np.float32,
-                     refi_steps: int = 1) -> RefineResult:
-    """Algorithm 3: run Alg. 2 in a lower precision until the
-    test fires, then promote Z, recompute X in FP64 and apply `refi_steps`
-    FP64 updates (Sec. IV.B).  err[] is the low-precision
-    history followed by the FP64 Err before each refinement update and after
-    the last one."""
+                     refi_steps: int = 1, refi_dtype=np.float64, update_dtype=None,
+                     final_check: bool = True) -> RefineResult:
+    """Algorithm 3 (Sec. IV.B):
+      1. Alg. 2 in the lower precision `low_dtype` until the test of Eq. 38 fires (or max_iter updates);
+      2. "Z = FP32[Z] or FP64[Z]": Z is converted to the enhanced precision `refi_dtype`
+         (float32 = the paper's single-precision refinement; float64)
+         and X = Z^T S Z is recomputed in it (S converted to it as well);
+      3. Z_{n+1} is computed in the enhanced precision -- or, with `update_dtype` given, its correction
+         Z (1/2 R + 3/8 R R) alone is evaluated in `update_dtype` and added to the `refi_dtype` master
+         (`update_mixed`).
+    Steps 2-3 are repeated `refi_steps` times ("Typically we would only do one extra refinement step,
+    although we could continue").
+
+    err[] layout (k = stop index of the low-precision run):
+        err[0..k]               the low-precision history, Err[n] = ||R_n||_F in `low_dtype`
+        err[k+1 .. k+refi_steps] the enhanced-precision Err evaluated BEFORE each refinement update
+        err[k+refi_steps+1]      (final_check only) the enhanced-precision Err of the returned Z;
+                                 Alg. 3 as printed ends after the update (final_check = False).
+    iters = k + refi_steps; flags are those of the low-precision run."""
+    if refi_steps < 1:
+        raise ValueError("refi_steps must be >= 1")
     low = refine(S, Z0, max_iter, STOP_PAPER, dtype=low_dtype)
-    S64 = np.asarray(S, dtype=np.float64)
-    Z = np.asarray(low.Z, dtype=np.float64)
+    Sr = np.asarray(S, dtype=refi_dtype)
+    Z = np.asarray(low.Z, dtype=refi_dtype)
     err = list(low.err)
     for _ in range(refi_steps):
-        R = residual(S64, Z)
+        R = residual(Sr, Z)
         err.append(err_fro(R))
-        Z = update_delta_form(Z, R)
-    err.append(err_fro(residual(S64, Z)))
+        Z = update_delta_form(Z, R) if update_dtype is None else update_mixed(Z, R, update_dtype)
+    if final_check:
+        err.append(err_fro(residual(Sr, Z)))
     return RefineResult(Z, low.iters + refi_steps, np.asarray(err), low.flags)
 
 
