@@ -53,8 +53,8 @@ typedef struct zfac_ctx zfac_ctx; /* opaque */
  *           rounded to FP16, one tensor-core pass, FP32 accumulation; meant to be followed by
  *           the refinement step (zfac_refine_refi).
  * Note on SPLIT16: the second-order product of step a4 (R R in Q = 1/2 R + 3/8 R R) runs its (h)(h) pass only when
- * the update is taken from Err[n] <= 0.1 (decided on the device from the Err[n] just computed); the effect on Z is
- * below FP32 resolution, every other product always runs all three passes. */
+ * the update is taken from Err[n] <= ZFAC_OPT_HH_SQUARE_ERR (default 0.1; decided on the device from the Err[n] just
+ * computed); every other product always runs all three passes (ZFAC_OPT_HH_SQUARE = 0 disables it). */
 typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2, ZFAC_MODE_HH16 = 3 } zfac_mode;
 
 /* Stop rule.  PAPER: Alg. 2's parameter-free test.  FIXED: perform exactly max_iter updates
@@ -74,7 +74,11 @@ enum {
   ZFAC_R_STOPPED = 1,  /* the test Err[n] > Err[n-1]^(m+1) fired (m = 2: ^3; converged to the precision floor) */
   ZFAC_R_MAXITER = 2,  /* max_iter updates were performed without the test firing               */
   ZFAC_R_NONFINITE = 4, /* Err[n] became inf/NaN; iteration stopped                              */
-  ZFAC_R_REFINED = 8    /* zfac_refine_refi: the FP64 refinement updates were applied            */
+  ZFAC_R_REFINED = 8,   /* zfac_refine_refi: at least one refinement update was applied          */
+  ZFAC_R_RANGE = 16     /* SPLIT16 / HH16: a value of S, Z0, T = (S Z)^T or Z with magnitude >= 65504 was clamped when it
+                           was rounded to an FP16 operand (FP16 range); the result is not to be trusted.  Admissible input:
+                           abs(S_ij), abs(Z_ij), abs((S Z)_ij) < 65504 throughout -- e.g. lambda_min(S) >~ 3e-10 for a
+                           normalised S; rescale S by a power of four otherwise (Z scales by its square root)   */
 };
 
 /* Internal buffers that zfac_peek can copy out (parity tests of the individual steps).
@@ -92,11 +96,12 @@ typedef enum {
  * Returns 0 for invalid arguments.  Host function, launches nothing. */
 size_t zfac_workspace_bytes(int64_t n, zfac_mode mode);
 
-/* Create a context for n x n problems in `mode`, bound to the CURRENT device and to the
+/* Create a context for n x n problems (1 <= n <= 2^20) in `mode`, bound to the CURRENT device and to the
  * caller-owned device workspace [d_workspace, d_workspace + bytes), which must be 256-byte
  * aligned and stay alive and otherwise unused until zfac_destroy.  Builds the TMA tensor maps.
  * One context serves any number of zfac_refine calls (the MD-step use),
- * one at a time.  Errors: INVALID, WORKSPACE, UNSUPPORTED, CUDA. */
+ * one at a time.  Every later call on the context must be made with the same device current
+ * (checked: ZFAC_E_INVALID otherwise).  Errors: INVALID, WORKSPACE, UNSUPPORTED, CUDA. */
 zfac_status zfac_create(zfac_ctx** ctx, int64_t n, zfac_mode mode, void* d_workspace, size_t bytes);
 
 /* Algorithm 2 on device buffers.  Asynchronous on `stream` (a cudaStream_t passed as void*;
@@ -116,22 +121,37 @@ zfac_status zfac_refine(zfac_ctx* ctx, const void* d_S, int64_t lds, const void*
                         double* d_err, int* d_flags, void* stream);
 
 /* Algorithm 3 (PAPER.md:322-341; Sec. IV.B, :308-316): the "+refi" schemes of Table I.
- *   1. Algorithm 2 in the low-precision mode of `low` (SPLIT16, HH16 or TF32; FP32 S and Z0)
- *      until its parameter-free test fires (or max_iter updates);
- *   2. Z is promoted to FP64 and R = I - Z^T S Z is recomputed in FP64 (S promoted exactly);
- *   3. `refi_steps` (>= 1; the paper uses 1) FP64 updates Z <- Z + Z (1/2 R + 3/8 R R).
- * `f64` must be a ZFAC_MODE_F64 context of the same n (its own workspace).  d_Z is n x n DOUBLE.
- * With final_check != 0 the FP64 residual of the returned Z is evaluated too (two more FP64
- * GEMMs); Alg. 3 as printed stops after the update (final_check = 0).
- *   d_iters [out] low-precision updates + refi_steps
- *   d_err   [out] double[max_iter + refi_steps + 2]: Err[0..k] of the low-precision run (k = its
- *                 stop index), then the FP64 Err before each refinement update, then (final_check)
- *                 the FP64 Err of the returned Z
- *   d_flags [out] flags of the low-precision run | ZFAC_R_REFINED
- * Asynchronous on `stream`, no allocation, no host synchronisation.  Errors: INVALID, CUDA. */
-zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* f64, const void* d_S, int64_t lds, const void* d_Z0,
+ *   1. Algorithm 2 in the low-precision mode of `low` (FP32 S and Z0) until its parameter-free test fires (or
+ *      max_iter updates);
+ *   2. "Z = FP32[Z] or FP64[Z]": Z is handed to the context `high` of a MORE precise mode, straight
+ *      from `low`'s workspace, and R = I - Z^T S Z is recomputed there (S converted exactly);
+ *   3. `refi_steps` updates Z <- Z + Z (1/2 R + 3/8 R R) in `high`'s arithmetic (1 <= refi_steps <= 4000; the paper uses 1).
+ * Allowed pairs (low -> high): HH16 -> SPLIT16, TF32 -> SPLIT16 (the paper's single-precision refinement,
+ * SPLIT16 is this library's FP32-class arithmetic), and HH16 / TF32 / SPLIT16 -> F64
+ * (PAPER.md:392-394).  `high` has the same n and order and its own workspace.  d_Z is n x n of `high`'s element
+ * type (float for SPLIT16, double for F64).
+ * With final_check != 0 the residual of the returned Z is evaluated in `high` as well (two more GEMMs); Alg. 3 as
+ * printed stops after the update (final_check = 0).
+ *   d_iters [out] low-precision updates + refinement updates performed
+ *   d_err   [out] double[max_iter + refi_steps + 2]: Err[0..k] of the low-precision run (k = its stop index), then
+ *                 `high`'s Err before each refinement update, then (final_check) `high`'s Err of the returned Z
+ *   d_flags [out] flags of the low-precision run | ZFAC_R_REFINED (if a refinement update was applied)
+ * If the low-precision run ends non-finite nothing is refined (Z = its last iterate, promoted); if a refinement
+ * residual is non-finite the refinement stops there (ZFAC_R_NONFINITE); d_iters and d_err say what was done.
+ * Asynchronous on `stream`, no allocation, no host synchronisation.  Errors: INVALID (also: mode pair not allowed,
+ * orders differ), CUDA. */
+zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* high, const void* d_S, int64_t lds, const void* d_Z0,
                              int64_t ldz0, void* d_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
                              int* d_iters, double* d_err, int* d_flags, void* stream);
+
+/* zfac_refine_refi on HOST buffers (pinned memory recommended): h_S, h_Z0 float, h_Z of `high`'s element type.
+ * Uploads S and Z0 (overlapped with the first a1 as in zfac_refine_host), runs Alg. 3, downloads Z (started right
+ * after the last refinement update, i.e. overlapped with the final check), iters, Err[] and flags, and synchronises
+ * `stream`.  max_iter + refi_steps + 2 <= 4096.  h_err: double[max_iter + refi_steps + 2].  This is the end-to-end
+ * "time to gate" call of bench.py. */
+zfac_status zfac_refine_refi_host(zfac_ctx* low, zfac_ctx* high, const void* h_S, int64_t lds, const void* h_Z0,
+                                  int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
+                                  int* h_iters, double* h_err, int* h_flags, void* stream);
 
 /* Congruence transformation H_perp = Z^T H Z (Eq. 11): what Z is for.  H is
  * n x n symmetric (full storage), Z n x n (any inverse factor), element type of the context's
@@ -142,20 +162,20 @@ zfac_status zfac_congruence(zfac_ctx* ctx, const void* d_H, int64_t ldh, const v
                             void* d_out, int64_t ldo, void* stream);
 
 /* Same operation on HOST buffers (pinned memory recommended): copies S and Z0 to the device
- * staging area of the workspace, runs zfac_refine, copies Z, iters, Err[0..max_iter] and flags
+ * staging area of the workspace, runs zfac_refine, copies Z, iters, Err[0..iters] and flags
  * back, and synchronises `stream` before returning.  This is the end-to-end call bench.py times.
- * With a PINNED h_Z and max_iter >= 1 the download of Z starts right after the first update, on an internal side stream:
- * if that update is the only one (a warm start) it has overlapped the final residual evaluation; otherwise the normal
- * download at the end supersedes it (measured, N = 8192 SPLIT16 warm start: 24.7 -> 20.9 ms per call; three-update HH16 run:
- * unchanged).  Results are bit-identical either way; ZFAC_HOST_OVERLAP=0 disables it.
- * With PINNED h_S and h_Z0, a tensor-core mode (not ZFAC_MODE_F64) and a padded dimension of at least 1024, the UPLOAD
- * is overlapped as well: Z0 goes first, then S in up to 8 chunks of whole 256-row blocks on the side stream; rows
- * [r0, r1) of S are all that step a1 needs for columns [r0, r1) of T = (S Z)^T, so each chunk is converted (step a0,
- * S only) and multiplied (a1 restricted to that band of tiles) while the next chunk is still on the bus.  The bands
- * are disjoint sets of whole tiles: bit-identical to the single launch (measured, same workload: 20.7 -> 18.6 ms per
- * call; 8 + 7 extra launches).  ZFAC_HOST_UPLOAD_OVERLAP=0 disables it.  Pageable buffers take the plain path.
- * In those modes the first update's a5 also runs in two row bands (pinned h_Z), each band's rows of Z downloaded as soon
- * as they are final: 18.6 -> 17.9 ms; one extra launch; ZFAC_HOST_A5_BANDS=1 disables it. */
+ * max_iter <= 4095 (size of the staging area for Err[]; ZFAC_E_INVALID beyond).
+ * Transfers are overlapped with the kernels where the data dependences allow, results are
+ * bit-identical to zfac_refine either way:
+ *   - pinned h_Z, max_iter >= 1: the download of Z starts right after the first update on an internal side stream; it
+ *     is the result if that update is the only one (a warm start), else the download at the end supersedes it
+ *     (ZFAC_OPT_HOST_OVERLAP = 0 disables it);
+ *   - pinned h_S and h_Z0, a tensor-core mode, padded dimension >= 1024: Z0 is uploaded first, then S in up to 8
+ *     chunks of whole 256-row blocks; each chunk is converted (step a0) and multiplied (step a1 restricted to that
+ *     band of tiles) while the next one is on the bus (ZFAC_OPT_HOST_UPLOAD_OVERLAP = 0 disables it);
+ *   - in those modes the first update's a5 runs in ZFAC_OPT_HOST_A5_BANDS (default 2) row bands, each band's rows
+ *     of Z downloaded as soon as they are final.
+ * Pageable buffers take the plain path. */
 zfac_status zfac_refine_host(zfac_ctx* ctx, const void* h_S, int64_t lds, const void* h_Z0,
                              int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, zfac_stop stop,
                              int* h_iters, double* h_err, int* h_flags, void* stream);
@@ -167,8 +187,7 @@ zfac_status zfac_peek(zfac_ctx* ctx, zfac_buf which, void* d_out, int64_t ld, vo
 /* Concurrency.  Contexts share no state (each owns its workspace and tensor maps; the last-error string is
  * thread-local): calls on DIFFERENT contexts may be issued from different host threads and / or on different streams
  * and run concurrently on the device; results are bit-identical to running them one after another.  This is the way
- * to refine many small problems at once (the graph-partitioned sub-problems of PAPER.md:98): at n <= 1024 one
- * problem's kernels cover 20-32 of the 148 SMs and 5-7 problems co-reside (profiles/r1c_sweep.md: 4.4-7.5x).
+ * to refine many small problems at once (the graph-partitioned sub-problems of PAPER.md:98).
  * Calls on the SAME context must not overlap (they share the workspace); issue them on one stream. */
 
 /* CUDA graphs.  zfac_refine, zfac_refine_refi and zfac_congruence only enqueue kernels on `stream`: no allocation, no
@@ -176,15 +195,12 @@ zfac_status zfac_peek(zfac_ctx* ctx, zfac_buf which, void* d_out, int64_t ld, vo
  * statically enqueued kernels after it return at once).  With profiling disabled (zfac_set_profile) a call can
  * therefore be captured into a CUDA graph (cudaStreamBeginCapture ... cudaStreamEndCapture) and replayed; the graph
  * reads and writes the SAME user and workspace buffers as the captured call, so new inputs are written into them in
- * place.  One graph launch replaces 2 + 2 (max_iter + 1) + 2..3 max_iter kernel launches: at n <= 1024, where the host's
- * launch rate is the limit, a replay is 15-30 % faster than the direct call (n = 300: 0.65 -> 0.46 ms, n = 1024: 1.45 ->
- * 1.23 ms for max_iter = 20), and the host thread is free (2 us per replay instead of 0.6-10 ms of enqueueing). */
+ * place.  One graph launch replaces 2 + 2 (max_iter + 1) + 2..3 max_iter kernel launches (measurements: DESIGN.md §1). */
 
 /* The whole call as ONE CUDA graph with a WHILE node: copy-in, first residual, WHILE (not stopped) { update, residual,
  * update, residual }, copy-out.  The stop test (Alg. 2, Eq. 38) of every residual sets the loop condition on
  * the device, so the graph runs exactly as many iterations as the refinement needs: none of the 2 + 4 max_iter
- * statically enqueued launches of zfac_refine that return at once after the stop exist here (zfac_refine with
- * max_iter = 20 and one update: 84 launches, 76 of them such returns).  Same arguments, same results (bit-identical) and
+ * statically enqueued launches of zfac_refine that return at once after the stop exist here.  Same arguments, same results (bit-identical) and
  * the same restrictions as zfac_refine; the graph is bound to these buffers (write new inputs into them) and to the
  * context's order at creation time.  zfac_graph_launch is asynchronous on `stream`; launches of one graph, and of graphs
  * and calls that share a context, must not overlap.  Destroy graphs before their context. */
@@ -194,6 +210,30 @@ zfac_status zfac_graph_create(zfac_ctx* ctx, const void* d_S, int64_t lds, const
                               double* d_err, int* d_flags, zfac_graph** graph);
 zfac_status zfac_graph_launch(zfac_graph* graph, void* stream);
 zfac_status zfac_graph_destroy(zfac_graph* graph);
+
+/* Per-context options (host-side state only: no device work; take effect from the next call on `ctx`).  They
+ * replace every environment variable earlier versions read.  Values are passed as double; integer options are
+ * rounded.  Unknown key or out-of-range value -> ZFAC_E_INVALID, the option keeps its value.
+ *   The first six change which arithmetic is performed (hence results, within the mode's accuracy):           default
+ *   ZFAC_OPT_CHUNK_KB        SPLIT16, a1 / a2: k-blocks (64 products each) of (h)(h) products that are summed in the
+ *                            tensor core's truncating FP32 accumulator before they are added, with round-to-nearest,
+ *                            to FP32 registers ("promoted accumulation"); 1 .. 1024                    1
+ *   ZFAC_OPT_CHUNK0_KB       ... length of the FIRST chunk of every tile (>= CHUNK_KB to take effect)                 1
+ *   ZFAC_OPT_HH_SQUARE       SPLIT16, a4 (and p2): one (h)(h) pass for the second-order product when the update is
+ *                            taken from Err[n] <= HH_SQUARE_ERR; 0 = always three passes (Eq. 32 as printed)        1
+ *   ZFAC_OPT_HH_SQUARE_ERR   the bound, >= 0                                                                       0.1
+ *   ZFAC_OPT_PROMOTE_UPDATE  SPLIT16: promoted accumulation in the update GEMMs (p2, a4, a5) as well; 0 / 1          0
+ *   The rest change scheduling only (bit-identical results):
+ *   ZFAC_OPT_BAND            full GEMMs: tile columns per rasterisation band, 1 .. 4096                               8
+ *   ZFAC_OPT_MAX_PAIRS       tensor-core modes: use at most this many CTA pairs; 0 = all co-resident ones            0
+ *   ZFAC_OPT_HOST_OVERLAP, ZFAC_OPT_HOST_UPLOAD_OVERLAP (0 / 1), ZFAC_OPT_HOST_A5_BANDS (1 .. 64): zfac_refine_host     1, 1, 2 */
+typedef enum {
+  ZFAC_OPT_CHUNK_KB = 0, ZFAC_OPT_CHUNK0_KB = 1, ZFAC_OPT_HH_SQUARE = 2, ZFAC_OPT_HH_SQUARE_ERR = 3,
+  ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
+  ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9
+} zfac_option;
+zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
+zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);
 
 /* Order m of the refinement polynomial, Z_{n+1} = Z_n sum_{k=0..m} c_k R_n^k  (Eq. 13 / Eq. 16:
  * "Reference 1 gives a table with the coefficients a_k for polynomials of order m = 2, 3, 4, 5. For the tests in

@@ -11,6 +11,7 @@ import ctypes
 import os
 from typing import Optional
 
+import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -19,8 +20,15 @@ LIB_PATH = os.path.join(_HERE, "libzfac.so")
 ZFAC_MODE_SPLIT16, ZFAC_MODE_TF32, ZFAC_MODE_F64, ZFAC_MODE_HH16 = 0, 1, 2, 3
 ZFAC_STOP_PAPER, ZFAC_STOP_FIXED = 0, 1
 ZFAC_OK, ZFAC_E_INVALID, ZFAC_E_UNSUPPORTED, ZFAC_E_WORKSPACE, ZFAC_E_CUDA = 0, 1, 2, 3, 4
-ZFAC_R_STOPPED, ZFAC_R_MAXITER, ZFAC_R_NONFINITE, ZFAC_R_REFINED = 1, 2, 4, 8
+ZFAC_R_STOPPED, ZFAC_R_MAXITER, ZFAC_R_NONFINITE, ZFAC_R_REFINED, ZFAC_R_RANGE = 1, 2, 4, 8, 16
 ZFAC_BUF_T, ZFAC_BUF_R, ZFAC_BUF_Q, ZFAC_BUF_Z = 0, 1, 2, 3
+
+(ZFAC_OPT_CHUNK_KB, ZFAC_OPT_CHUNK0_KB, ZFAC_OPT_HH_SQUARE, ZFAC_OPT_HH_SQUARE_ERR, ZFAC_OPT_PROMOTE_UPDATE, ZFAC_OPT_BAND,
+ ZFAC_OPT_MAX_PAIRS, ZFAC_OPT_HOST_OVERLAP, ZFAC_OPT_HOST_UPLOAD_OVERLAP, ZFAC_OPT_HOST_A5_BANDS) = range(10)
+OPTIONS = {"chunk_kb": ZFAC_OPT_CHUNK_KB, "chunk0_kb": ZFAC_OPT_CHUNK0_KB, "hh_square": ZFAC_OPT_HH_SQUARE,
+           "hh_square_err": ZFAC_OPT_HH_SQUARE_ERR, "promote_update": ZFAC_OPT_PROMOTE_UPDATE, "band": ZFAC_OPT_BAND,
+           "max_pairs": ZFAC_OPT_MAX_PAIRS, "host_overlap": ZFAC_OPT_HOST_OVERLAP,
+           "host_upload_overlap": ZFAC_OPT_HOST_UPLOAD_OVERLAP, "host_a5_bands": ZFAC_OPT_HOST_A5_BANDS}
 
 MODES = {"split16": ZFAC_MODE_SPLIT16, "tf32": ZFAC_MODE_TF32, "f64": ZFAC_MODE_F64, "hh16": ZFAC_MODE_HH16}
 
@@ -31,6 +39,7 @@ EXPORTS = [
     "zfac_last_launch_count", "zfac_padded_n", "zfac_destroy", "zfac_status_string",
     "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile", "zfac_set_order", "zfac_get_order",
     "zfac_graph_create", "zfac_graph_launch", "zfac_graph_destroy",
+    "zfac_set_option", "zfac_get_option", "zfac_refine_refi_host",
 ]
 
 _lib: Optional[ctypes.CDLL] = None
@@ -67,6 +76,12 @@ def lib() -> ctypes.CDLL:
     L.zfac_refine_host.argtypes = [vp, vp, i64, vp, i64, vp, i64, ci, ci, vp, vp, vp, vp]
     L.zfac_refine_refi.restype = ci
     L.zfac_refine_refi.argtypes = [vp, vp, vp, i64, vp, i64, vp, i64, ci, ci, ci, vp, vp, vp, vp]
+    L.zfac_refine_refi_host.restype = ci
+    L.zfac_refine_refi_host.argtypes = [vp, vp, vp, i64, vp, i64, vp, i64, ci, ci, ci, vp, vp, vp, vp]
+    L.zfac_set_option.restype = ci
+    L.zfac_set_option.argtypes = [vp, ci, ctypes.c_double]
+    L.zfac_get_option.restype = ci
+    L.zfac_get_option.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double)]
     L.zfac_congruence.restype = ci
     L.zfac_congruence.argtypes = [vp, vp, i64, vp, i64, vp, i64, vp]
     L.zfac_peek.restype = ci
@@ -142,6 +157,29 @@ def zfac_refine_refi(low: int, f64: int, d_S: int, lds: int, d_Z0: int, ldz0: in
                                 int(final_check), d_iters, d_err, d_flags, ctypes.c_void_p(stream))
     if st != ZFAC_OK:
         raise ZfacError(st, "zfac_refine_refi")
+
+
+def zfac_refine_refi_host(low: int, high: int, h_S: int, lds: int, h_Z0: int, ldz0: int, h_Z: int, ldz: int,
+                          max_iter: int, refi_steps: int, final_check: int, h_iters: int, h_err: int, h_flags: int,
+                          stream: int = 0) -> None:
+    st = lib().zfac_refine_refi_host(low, high, h_S, lds, h_Z0, ldz0, h_Z, ldz, int(max_iter), int(refi_steps),
+                                     int(final_check), h_iters, h_err, h_flags, ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_refine_refi_host")
+
+
+def zfac_set_option(ctx: int, key: int, value: float) -> None:
+    st = lib().zfac_set_option(ctx, int(key), float(value))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_set_option")
+
+
+def zfac_get_option(ctx: int, key: int) -> float:
+    v = ctypes.c_double(0.0)
+    st = lib().zfac_get_option(ctx, int(key), ctypes.byref(v))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_get_option")
+    return float(v.value)
 
 
 def zfac_congruence(ctx: int, d_H: int, ldh: int, d_Z: int, ldz: int, d_out: int, ldo: int, stream: int = 0) -> None:
@@ -281,7 +319,6 @@ class Zfac:
     def refine_host(self, S: torch.Tensor, Z0: torch.Tensor, Z: torch.Tensor, max_iter: int = 40,
                     stop: int = ZFAC_STOP_PAPER):
         """Host (pinned) tensors in and out, through zfac_refine_host."""
-        import numpy as np
         for t, name in ((S, "S"), (Z0, "Z0"), (Z, "Z")):
             self._check(t, name)
             if t.is_cuda:
@@ -296,18 +333,26 @@ class Zfac:
                              ctypes.addressof(flags), stream)
         return Z, iters.value, err[: iters.value + 1], flags.value
 
-    def refine_refi(self, f64: "Zfac", S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, refi_steps: int = 1,
+    def set_option(self, key: str | int, value: float) -> None:
+        """zfac_set_option; key by name (OPTIONS) or number."""
+        zfac_set_option(self.ctx, OPTIONS[key] if isinstance(key, str) else int(key), value)
+
+    def get_option(self, key: str | int) -> float:
+        return zfac_get_option(self.ctx, OPTIONS[key] if isinstance(key, str) else int(key))
+
+    def refine_refi(self, high: "Zfac", S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, refi_steps: int = 1,
                     final_check: bool = True, out: Optional[torch.Tensor] = None, sync: bool = True):
-        """Alg. 3: this (low-precision) context until its test fires, then `refi_steps` FP64 updates in `f64`.
-        FP32 device tensors in, FP64 device tensor out: (Z, iters, err[...], flags)."""
+        """Alg. 3: this (low-precision) context until its test fires, then `refi_steps` updates in the more precise
+        context `high` (SPLIT16 or F64).  FP32 device tensors in, device tensor of `high`'s element type out:
+        (Z, iters, err[...], flags)."""
         self._check(S, "S"); self._check(Z0, "Z0")
-        Z = out if out is not None else torch.empty((self.n, self.n), dtype=torch.float64, device=S.device)
-        self._check(Z, "Z", torch.float64)
+        Z = out if out is not None else torch.empty((self.n, self.n), dtype=high.dtype, device=S.device)
+        self._check(Z, "Z", high.dtype)
         d_iters = torch.zeros(1, dtype=torch.int32, device=S.device)
         d_flags = torch.zeros(1, dtype=torch.int32, device=S.device)
         d_err = torch.full((max_iter + refi_steps + 2,), float("nan"), dtype=torch.float64, device=S.device)
         stream = torch.cuda.current_stream(S.device).cuda_stream
-        zfac_refine_refi(self.ctx, f64.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), Z.data_ptr(),
+        zfac_refine_refi(self.ctx, high.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), Z.data_ptr(),
                          Z.stride(0), max_iter, refi_steps, int(final_check), d_iters.data_ptr(), d_err.data_ptr(),
                          d_flags.data_ptr(), stream)
         if not sync:
@@ -315,6 +360,23 @@ class Zfac:
         torch.cuda.current_stream(S.device).synchronize()
         it = int(d_iters.item())
         return Z, it, d_err[: it + 1 + int(final_check)].cpu().numpy(), int(d_flags.item())
+
+    def refine_refi_host(self, high: "Zfac", S: torch.Tensor, Z0: torch.Tensor, Z: torch.Tensor, max_iter: int = 40,
+                         refi_steps: int = 1, final_check: bool = True):
+        """zfac_refine_refi_host: host (pinned) FP32 S, Z0 in, host Z of `high`'s element type out."""
+        self._check(S, "S"); self._check(Z0, "Z0"); self._check(Z, "Z", high.dtype)
+        for t, name in ((S, "S"), (Z0, "Z0"), (Z, "Z")):
+            if t.is_cuda:
+                raise ValueError(f"{name}: refine_refi_host takes host tensors")
+        iters = ctypes.c_int(0)
+        flags = ctypes.c_int(0)
+        err = np.full(max_iter + refi_steps + 2, np.nan, dtype=np.float64)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        with torch.cuda.device(self.device):
+            zfac_refine_refi_host(self.ctx, high.ctx, S.data_ptr(), S.stride(0), Z0.data_ptr(), Z0.stride(0), Z.data_ptr(),
+                                  Z.stride(0), max_iter, refi_steps, int(final_check), ctypes.addressof(iters),
+                                  err.ctypes.data, ctypes.addressof(flags), stream)
+        return Z, iters.value, err[: iters.value + 1 + int(final_check)], flags.value
 
     def congruence(self, H: torch.Tensor, Z: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
         """H_perp = Z^T H Z (Eq. 11) on device tensors of the mode's element type."""

@@ -30,6 +30,8 @@ static thread_local char g_cuda_err[256] = "";
 struct zfac_ctx {
   int64_t n, np;
   int mode;
+  int dev = 0;     // device the context was created on; every entry point checks that it is current
+  Options opt;     // zfac_set_option
   char* ws;
   size_t ws_bytes;
   Layout L;
@@ -48,6 +50,13 @@ struct zfac_ctx {
 static bool valid_mode(int m) {
   return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_F64 || m == ZFAC_MODE_HH16;
 }
+// The context is bound to the device that was current at zfac_create (workspace, tensor maps, lazily created streams).
+static bool on_own_device(const zfac_ctx* c) {
+  int dev = -1;
+  return cudaGetDevice(&dev) == cudaSuccess && dev == c->dev;
+}
+// precision rank of a mode for Alg. 3 ("enhanced precision"): one 11-bit pass < FP32-class split < FP64
+static int mode_rank(int m) { return m == ZFAC_MODE_F64 ? 2 : (m == ZFAC_MODE_SPLIT16 ? 1 : 0); }
 
 extern "C" {
 
@@ -88,7 +97,7 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   zfac_ctx* c = new (std::nothrow) zfac_ctx();
   if (!c) return ZFAC_E_INVALID;
   c->n = n; c->np = L.np; c->mode = mode; c->ws = static_cast<char*>(d_workspace); c->ws_bytes = bytes;
-  c->L = L; c->launches = 0; c->sm_count = sms; c->order = 2;
+  c->L = L; c->launches = 0; c->sm_count = sms; c->order = 2; c->dev = dev;
   if (mode == ZFAC_MODE_F64) {
     cudaError_t e = f64_plan_create(&c->f64p, L, c->ws);
     if (e == cudaSuccess) e = f64_tma_prepare<EPI_A1>();
@@ -103,7 +112,7 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
       return ZFAC_E_CUDA;
     }
   } else {
-    cudaError_t e = umma_plan_create(&c->umma, L, c->ws, sms);
+    cudaError_t e = umma_plan_create(&c->umma, L, c->ws, sms, &c->opt);
     if (e != cudaSuccess) {
       snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_plan_create: %s", cudaGetErrorString(e));
       delete c;
@@ -174,6 +183,43 @@ zfac_status zfac_set_order(zfac_ctx* c, int m) {
 }
 
 int zfac_get_order(const zfac_ctx* c) { return c ? c->order : 0; }
+
+zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
+  if (!c || !(v == v)) return ZFAC_E_INVALID;
+  const long iv = (long)(v < 0 ? v - 0.5 : v + 0.5);
+  Options& o = c->opt;
+  switch (key) {
+    case ZFAC_OPT_CHUNK_KB: if (iv < 1 || iv > 1024) return ZFAC_E_INVALID; o.chunk_kb = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_CHUNK0_KB: if (iv < 1 || iv > 1024) return ZFAC_E_INVALID; o.chunk0_kb = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_HH_SQUARE: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.hh_square = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_HH_SQUARE_ERR: if (!(v >= 0.0)) return ZFAC_E_INVALID; o.hh_square_err = v; return ZFAC_OK;
+    case ZFAC_OPT_PROMOTE_UPDATE: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.promote_update = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_BAND: if (iv < 1 || iv > 4096) return ZFAC_E_INVALID; o.band = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_MAX_PAIRS: if (iv < 0 || iv > 65536) return ZFAC_E_INVALID; o.max_pairs = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_HOST_OVERLAP: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.host_overlap = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_HOST_UPLOAD_OVERLAP: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.host_upload_overlap = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_HOST_A5_BANDS: if (iv < 1 || iv > 64) return ZFAC_E_INVALID; o.host_a5_bands = (int)iv; return ZFAC_OK;
+  }
+  return ZFAC_E_INVALID;
+}
+
+zfac_status zfac_get_option(const zfac_ctx* c, zfac_option key, double* v) {
+  if (!c || !v) return ZFAC_E_INVALID;
+  const Options& o = c->opt;
+  switch (key) {
+    case ZFAC_OPT_CHUNK_KB: *v = o.chunk_kb; return ZFAC_OK;
+    case ZFAC_OPT_CHUNK0_KB: *v = o.chunk0_kb; return ZFAC_OK;
+    case ZFAC_OPT_HH_SQUARE: *v = o.hh_square; return ZFAC_OK;
+    case ZFAC_OPT_HH_SQUARE_ERR: *v = o.hh_square_err; return ZFAC_OK;
+    case ZFAC_OPT_PROMOTE_UPDATE: *v = o.promote_update; return ZFAC_OK;
+    case ZFAC_OPT_BAND: *v = o.band; return ZFAC_OK;
+    case ZFAC_OPT_MAX_PAIRS: *v = o.max_pairs; return ZFAC_OK;
+    case ZFAC_OPT_HOST_OVERLAP: *v = o.host_overlap; return ZFAC_OK;
+    case ZFAC_OPT_HOST_UPLOAD_OVERLAP: *v = o.host_upload_overlap; return ZFAC_OK;
+    case ZFAC_OPT_HOST_A5_BANDS: *v = o.host_a5_bands; return ZFAC_OK;
+  }
+  return ZFAC_E_INVALID;
+}
 
 // FP64 mode: the two halves of one iteration (see UmmaSeq in zfac_umma.cuh for the contract of n_stop / par).
 struct F64Seq {
@@ -252,11 +298,20 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
 
 // Step a0: copy S and Z0 (element type float if in_f32, else the mode's own) into the padded buffers.
 // what: 1 = S only, 2 = Z0 (W, State reset) only, 3 = both; tile rows [ty0, ty0 + tyn) of CI_TR rows each (tyn = 0: all).
+// First operation of every call: clears State::range (set by any CTA of the copy-in and of the a1 / a5 kernels when an fp16
+// conversion clamps, published as ZFAC_R_RANGE).  A memset node, not a kernel; capturable.
+static cudaError_t clear_range(zfac_ctx* c, cudaStream_t s) {
+  State* st = reinterpret_cast<State*>(c->ws + c->L.off_state);
+  return cudaMemsetAsync(&st->range, 0, sizeof(int), s);
+}
+
 static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, bool in_f32,
-                           cudaStream_t s, int what = 3, int ty0 = 0, int tyn = 0) {
+                           cudaStream_t s, int what = 3, int ty0 = 0, int tyn = 0, const State* prev = nullptr,
+                           const void* d_Z0_alt = nullptr) {
   const Layout& L = c->L;
   char* ws = c->ws;
   CopyInArgs ci{};
+  ci.prev = prev; ci.Z0_alt = d_Z0_alt;
   ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np;
   ci.st = reinterpret_cast<State*>(ws + L.off_state);
   ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
@@ -277,6 +332,11 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
 static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int parity, void* d_Z, int64_t ldz,
                             int* d_iters, int* d_flags, cudaStream_t s) {
   const Layout& L = c->L;
+  if (!d_Z) {                                     // publish iters / flags only (the result stays in the workspace)
+    publish_kernel<<<1, 32, 0, s>>>(reinterpret_cast<const State*>(c->ws + L.off_state), d_iters, d_flags);
+    c->launches += 1;
+    return;
+  }
   CopyOutArgs co{};
   co.Zbuf[0] = b0; co.Zbuf[1] = b1; co.parity = parity;
   co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np;
@@ -296,35 +356,38 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
   c->launches += 1;
 }
 
+// The iteration proper (everything between copy-in and copy-out) in the context's mode.
+static zfac_status run_iterations(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s, bool skip_last,
+                                  const IterHook* hook) {
+  if (c->mode == ZFAC_MODE_F64) return refine_f64(c, max_iter, stop, d_err, s, skip_last, hook);
+  int nl = 0;
+  cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, c->order, d_err, s, &nl, &c->prof, hook, skip_last);
+  c->launches += nl;
+  if (e != cudaSuccess) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_refine: %s", cudaGetErrorString(e));
+    return ZFAC_E_CUDA;
+  }
+  return ZFAC_OK;
+}
+
+// d_Z == nullptr (zfac_refine_refi's low-precision stage): the result stays in the workspace, iters / flags are published.
 static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
                                int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
                                void* stream, const IterHook* hook, int copy_what = 3) {
-  if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
-  if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
+  if (!c || !d_S || !d_Z0 || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
+  if (lds < c->n || ldz0 < c->n || (d_Z && ldz < c->n) || max_iter < 0) return ZFAC_E_INVALID;
   if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
+  if (!on_own_device(c)) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;
   c->launches = 0;
   c->prof.count = 0;
 
+  ZF_CUDA(clear_range(c, s));
   launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, s, copy_what);     // copy_what = 2: the hook's first_a1 brings S in
-
-  zfac_status rs;
-  if (c->mode == ZFAC_MODE_F64) {
-    rs = refine_f64(c, max_iter, stop, d_err, s, false, hook);
-  } else {
-    int nl = 0;
-    cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, c->order, d_err, s, &nl, &c->prof, hook);
-    c->launches += nl;
-    if (e != cudaSuccess) {
-      snprintf(g_cuda_err, sizeof(g_cuda_err), "umma_refine: %s", cudaGetErrorString(e));
-      return ZFAC_E_CUDA;
-    }
-    rs = ZFAC_OK;
-  }
+  zfac_status rs = run_iterations(c, max_iter, stop, d_err, s, false, hook);
   if (rs != ZFAC_OK) return rs;
-
   launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, s);
   ZF_CUDA(cudaGetLastError());
   return ZFAC_OK;
@@ -333,6 +396,7 @@ static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const 
 zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
                         int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
                         void* stream) {
+  if (!d_Z) return ZFAC_E_INVALID;
   return refine_impl(c, d_S, lds, d_Z0, ldz0, d_Z, ldz, max_iter, stop, d_iters, d_err, d_flags, stream, nullptr);
 }
 
@@ -402,44 +466,57 @@ static void host_after_a5_band(void* self, int r0, int r1, bool last, cudaStream
   if (last) cudaEventRecord(c->ev_copy, c->side);
 }
 
-zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* f64, const void* d_S, int64_t lds, const void* d_Z0,
-                             int64_t ldz0, void* d_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
-                             int* d_iters, double* d_err, int* d_flags, void* stream) {
-  if (!low || !f64 || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
-  if (low->mode == ZFAC_MODE_F64 || f64->mode != ZFAC_MODE_F64 || low->n != f64->n) return ZFAC_E_INVALID;
+// Alg. 3.  low_hook / low_copy_what: the host entry point's upload overlap for the low-precision stage; high_hook: its
+// early download.  d_upd (may be null): int[2] = refinement updates performed, Err entries written in total.
+static zfac_status refi_impl(zfac_ctx* low, zfac_ctx* high, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0,
+                             void* d_Z, int64_t ldz, int max_iter, int refi_steps, int final_check, int* d_iters,
+                             double* d_err, int* d_flags, int* d_upd, cudaStream_t s, const IterHook* low_hook,
+                             int low_copy_what, const IterHook* high_hook) {
+  if (!low || !high || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
+  if (mode_rank(high->mode) <= mode_rank(low->mode) || low->n != high->n || low->order != high->order) return ZFAC_E_INVALID;
   if (lds < low->n || ldz0 < low->n || ldz < low->n || max_iter < 0 || refi_steps < 1 || refi_steps > 4000)
     return ZFAC_E_INVALID;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
-  const Layout& L = f64->L;
-  // 1. Alg. 2 in low precision; its FP32 result goes to the FP64 context's staging area
-  float* zlow = reinterpret_cast<float*>(f64->ws + L.off_stage_Z);
-  zfac_status rs = zfac_refine(low, d_S, lds, d_Z0, ldz0, zlow, low->n, max_iter, ZFAC_STOP_PAPER, d_iters, d_err,
-                               d_flags, s);
+  if (!on_own_device(low) || low->dev != high->dev) return ZFAC_E_INVALID;
+  const Layout& LL = low->L;
+  const Layout& L = high->L;
+  // 1. Alg. 2 in low precision; the result stays in `low`'s workspace (FP32 master Z; TF32: the buffer of parity iters & 1)
+  zfac_status rs = refine_impl(low, d_S, lds, d_Z0, ldz0, nullptr, 0, max_iter, ZFAC_STOP_PAPER, d_iters, d_err, d_flags, s,
+                               low_hook, low_copy_what);
   if (rs != ZFAC_OK) return rs;
-  // 2. Z = FP64[Z], S promoted exactly; 3. refi_steps FP64 updates (kernels of the F64 mode)
-  f64->launches = 0;
-  f64->prof.count = 0;
-  launch_copy_in(f64, d_S, lds, zlow, f64->n, true, s);
-  double* err64 = reinterpret_cast<double*>(f64->ws + L.off_stage_out);
-  rs = refine_f64(f64, refi_steps, ZFAC_STOP_FIXED, err64, s, final_check == 0);
+  // 2. Z = FP32[Z] or FP64[Z], S converted exactly; X recomputed; 3. refi_steps updates in `high`'s kernels
+  high->launches = 0;
+  high->prof.count = 0;
+  const State* lst = reinterpret_cast<const State*>(low->ws + LL.off_state);
+  ZF_CUDA(clear_range(high, s));
+  launch_copy_in(high, d_S, lds, low->ws + LL.off_Z[0], LL.np, true, s, 3, 0, 0, lst, low->ws + LL.off_Z[1]);
+  double* err_hi = reinterpret_cast<double*>(high->ws + L.off_stage_out);
+  rs = run_iterations(high, refi_steps, ZFAC_STOP_FIXED, err_hi, s, final_check == 0, high_hook);
   if (rs != ZFAC_OK) return rs;
-  launch_copy_out(f64, f64->ws + L.off_Z[0], f64->ws + L.off_Z[1], refi_steps & 1, d_Z, ldz, nullptr, nullptr, s);
-  refi_merge_kernel<<<1, 32, 0, s>>>(err64, refi_steps + (final_check ? 1 : 0), refi_steps, d_err, d_iters, d_flags);
-  f64->launches += 1;
-  low->launches += f64->launches;
+  launch_copy_out(high, high->ws + L.off_Z[0], high->ws + L.off_Z[1], -2, d_Z, ldz, nullptr, nullptr, s);
+  refi_merge_kernel<<<1, 32, 0, s>>>(reinterpret_cast<const State*>(high->ws + L.off_state), err_hi, d_err, d_iters, d_flags, d_upd);
+  high->launches += 1;
+  low->launches += high->launches;
   ZF_CUDA(cudaGetLastError());
   return ZFAC_OK;
+}
+
+zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* high, const void* d_S, int64_t lds, const void* d_Z0,
+                             int64_t ldz0, void* d_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
+                             int* d_iters, double* d_err, int* d_flags, void* stream) {
+  return refi_impl(low, high, d_S, lds, d_Z0, ldz0, d_Z, ldz, max_iter, refi_steps, final_check, d_iters, d_err, d_flags,
+                   nullptr, static_cast<cudaStream_t>(stream), nullptr, 3, nullptr);
 }
 
 zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const void* d_Z, int64_t ldz, void* d_out,
                             int64_t ldo, void* stream) {
   if (!c || !d_H || !d_Z || !d_out) return ZFAC_E_INVALID;
-  if (ldh < c->n || ldz < c->n || ldo < c->n) return ZFAC_E_INVALID;
+  if (ldh < c->n || ldz < c->n || ldo < c->n || !on_own_device(c)) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;
   c->launches = 0;
   c->prof.count = 0;
+  ZF_CUDA(clear_range(c, s));
   launch_copy_in(c, d_H, ldh, d_Z, ldz, false, s);        // H takes the place of S; W = Z^T
   if (c->mode == ZFAC_MODE_F64) {
     double* T = reinterpret_cast<double*>(ws + L.off_T);
@@ -466,24 +543,18 @@ zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const voi
   return ZFAC_OK;
 }
 
-zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const void* h_Z0, int64_t ldz0, void* h_Z,
-                             int64_t ldz, int max_iter, zfac_stop stop, int* h_iters, double* h_err, int* h_flags,
-                             void* stream) {
-  if (!c || !h_S || !h_Z0 || !h_Z || !h_iters || !h_err || !h_flags) return ZFAC_E_INVALID;
-  if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0 || max_iter > 4095) return ZFAC_E_INVALID;
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
+// Upload of S and Z0 into the staging area for the host entry points.  With pinned inputs in a tensor-core mode
+// (see host_first_a1) Z0 goes first and S follows in row chunks on the side stream; *chunks > 0 says so.
+static zfac_status host_upload(zfac_ctx* c, const void* h_S, int64_t lds, const void* h_Z0, int64_t ldz0, cudaStream_t s,
+                               int* chunks_out) {
   const Layout& L = c->L;
   char* dS = c->ws + L.off_stage_S;
   char* dZ = c->ws + L.off_stage_Z;
-  double* dErr = reinterpret_cast<double*>(c->ws + L.off_stage_out);
-  int* dInts = reinterpret_cast<int*>(c->ws + L.off_stage_out + 4096 * sizeof(double));
   const size_t row = (size_t)c->n * L.elt;
-  // upload overlap (see host_first_a1): tcgen05 modes, pinned h_S and h_Z0, at least 4 macro-tile rows
   int chunks = 0;
-  if (c->mode != ZFAC_MODE_F64 && L.np / UM_MACRO >= 4) {
+  if (c->mode != ZFAC_MODE_F64 && L.np / UM_MACRO >= 4 && c->opt.host_upload_overlap) {
     cudaPointerAttributes pS{}, pZ{};
-    const char* off = getenv("ZFAC_HOST_UPLOAD_OVERLAP");
-    if (!(off && off[0] == '0') && cudaPointerGetAttributes(&pS, h_S) == cudaSuccess && pS.type == cudaMemoryTypeHost &&
+    if (cudaPointerGetAttributes(&pS, h_S) == cudaSuccess && pS.type == cudaMemoryTypeHost &&
         cudaPointerGetAttributes(&pZ, h_Z0) == cudaSuccess && pZ.type == cudaMemoryTypeHost) {
       const int T = (int)(L.np / UM_MACRO);
       chunks = T < zfac_ctx::UP_CHUNKS ? T : zfac_ctx::UP_CHUNKS;
@@ -514,33 +585,55 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
     ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
     ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
   }
-  // overlapped download: needs a pinned (device-visible) h_Z and at least one possible update
-  bool z_dev = false;                             // early download possible: pinned h_Z (an async copy from pageable memory
-  {                                               // is staged and may block) and at least one possible update
-    cudaPointerAttributes pa{};
-    const char* off = getenv("ZFAC_HOST_OVERLAP");
-    if (max_iter >= 1 && !(off && off[0] == '0') && cudaPointerGetAttributes(&pa, h_Z) == cudaSuccess &&
-        pa.type == cudaMemoryTypeHost)
-      z_dev = true;
-    (void)cudaGetLastError();
-  }
+  *chunks_out = chunks;
+  return ZFAC_OK;
+}
+
+static bool host_pinned(const void* p) {
+  cudaPointerAttributes pa{};
+  const bool pinned = cudaPointerGetAttributes(&pa, p) == cudaSuccess && pa.type == cudaMemoryTypeHost;
+  (void)cudaGetLastError();
+  return pinned;
+}
+
+static zfac_status host_side_objects(zfac_ctx* c) {
+  if (!c->side) ZF_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+  if (!c->ev_a5) ZF_CUDA(cudaEventCreateWithFlags(&c->ev_a5, cudaEventDisableTiming));
+  if (!c->ev_copy) ZF_CUDA(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
+  return ZFAC_OK;
+}
+
+zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const void* h_Z0, int64_t ldz0, void* h_Z,
+                             int64_t ldz, int max_iter, zfac_stop stop, int* h_iters, double* h_err, int* h_flags,
+                             void* stream) {
+  if (!c || !h_S || !h_Z0 || !h_Z || !h_iters || !h_err || !h_flags) return ZFAC_E_INVALID;
+  if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0 || max_iter > 4095) return ZFAC_E_INVALID;
+  if (!on_own_device(c)) return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& L = c->L;
+  char* dS = c->ws + L.off_stage_S;
+  char* dZ = c->ws + L.off_stage_Z;
+  double* dErr = reinterpret_cast<double*>(c->ws + L.off_stage_out);
+  int* dInts = reinterpret_cast<int*>(c->ws + L.off_stage_out + 4096 * sizeof(double));
+  const size_t row = (size_t)c->n * L.elt;
+  int chunks = 0;
+  zfac_status rs = host_upload(c, h_S, lds, h_Z0, ldz0, s, &chunks);
+  if (rs != ZFAC_OK) return rs;
+  // overlapped download: needs a pinned (device-visible) h_Z (an async copy to pageable memory is staged and may
+  // block) and at least one possible update
+  const bool z_dev = max_iter >= 1 && c->opt.host_overlap && host_pinned(h_Z);
   HostOverlap ho{c, h_Z, ldz};
   ho.dS = dS; ho.chunks = chunks;
   IterHook hook{z_dev ? host_after_a5 : nullptr, &ho};
   if (chunks > 0) hook.first_a1 = host_first_a1;
   if (z_dev && c->mode != ZFAC_MODE_F64 && L.np / UM_MACRO >= 4) {
-    const char* nb = getenv("ZFAC_HOST_A5_BANDS");
-    hook.a5_bands = nb ? atoi(nb) : 2;
+    hook.a5_bands = c->opt.host_a5_bands;
     if (hook.a5_bands > (int)(L.np / UM_MACRO)) hook.a5_bands = (int)(L.np / UM_MACRO);
     hook.after_a5_band = host_after_a5_band;
   }
-  if (z_dev) {
-    if (!c->side) ZF_CUDA(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
-    if (!c->ev_a5) ZF_CUDA(cudaEventCreateWithFlags(&c->ev_a5, cudaEventDisableTiming));
-    if (!c->ev_copy) ZF_CUDA(cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
-  }
-  zfac_status rs = refine_impl(c, dS, c->n, dZ, c->n, dZ, c->n, max_iter, stop, dInts, dErr, dInts + 1, s,
-                               (z_dev || chunks > 0) ? &hook : nullptr, chunks > 0 ? 2 : 3);
+  if (z_dev && (rs = host_side_objects(c)) != ZFAC_OK) return rs;
+  rs = refine_impl(c, dS, c->n, dZ, c->n, dZ, c->n, max_iter, stop, dInts, dErr, dInts + 1, s,
+                   (z_dev || chunks > 0) ? &hook : nullptr, chunks > 0 ? 2 : 3);
   if (rs != ZFAC_OK) return rs;
   if (z_dev) ZF_CUDA(cudaStreamWaitEvent(s, c->ev_copy, 0));   // the early download is complete (and can no longer land late)
   else ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
@@ -551,6 +644,73 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   if (z_dev && ints[0] != 1)       // the early download holds Z_1: final only if exactly one update ran
     ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaMemcpyAsync(h_err, dErr, (size_t)(ints[0] + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
+  ZF_CUDA(cudaStreamSynchronize(s));
+  return ZFAC_OK;
+}
+
+// zfac_refine_refi_host: the download of Z starts right after the LAST refinement update (straight from the internal
+// buffer, on `high`'s side stream), so it overlaps the final check; if the refinement stage did not perform all its
+// updates (non-finite residual) the normal download at the end supersedes it.
+struct RefiDownload {
+  zfac_ctx* high;
+  void* h_Z;
+  int64_t ldz;
+  int last;            // index of the last refinement update (refi_steps - 1)
+};
+static void refi_after_a5(void* self, int n, cudaStream_t s) {
+  RefiDownload* r = static_cast<RefiDownload*>(self);
+  if (n != r->last) return;
+  zfac_ctx* c = r->high;
+  const Layout& L = c->L;
+  // Z after update n sits in buffer (n + 1) & 1 (F64 / TF32); the 16-bit modes update one FP32 master in place
+  const char* src = c->ws + L.off_Z[mode_is_h16(c->mode) ? 0 : ((n + 1) & 1)];
+  cudaEventRecord(c->ev_a5, s);
+  cudaStreamWaitEvent(c->side, c->ev_a5, 0);
+  cudaMemcpy2DAsync(r->h_Z, (size_t)r->ldz * L.elt, src, (size_t)L.np * L.elt, (size_t)c->n * L.elt, (size_t)c->n,
+                    cudaMemcpyDeviceToHost, c->side);
+  cudaEventRecord(c->ev_copy, c->side);
+}
+
+zfac_status zfac_refine_refi_host(zfac_ctx* low, zfac_ctx* high, const void* h_S, int64_t lds, const void* h_Z0,
+                                  int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
+                                  int* h_iters, double* h_err, int* h_flags, void* stream) {
+  if (!low || !high || !h_S || !h_Z0 || !h_Z || !h_iters || !h_err || !h_flags) return ZFAC_E_INVALID;
+  if (low->mode == ZFAC_MODE_F64 || low->n != high->n) return ZFAC_E_INVALID;
+  if (lds < low->n || ldz0 < low->n || ldz < low->n || max_iter < 0 || refi_steps < 1 || max_iter + refi_steps + 2 > 4096)
+    return ZFAC_E_INVALID;
+  if (!on_own_device(low) || low->dev != high->dev) return ZFAC_E_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Layout& LL = low->L;
+  const Layout& L = high->L;
+  char* dS = low->ws + LL.off_stage_S;
+  char* dZ0 = low->ws + LL.off_stage_Z;
+  char* dZ = high->ws + L.off_stage_Z;                         // n x n of high's element type
+  double* dErr = reinterpret_cast<double*>(low->ws + LL.off_stage_out);
+  int* dInts = reinterpret_cast<int*>(low->ws + LL.off_stage_out + 4096 * sizeof(double));
+  const size_t row = (size_t)high->n * L.elt;
+  int chunks = 0;
+  zfac_status rs = host_upload(low, h_S, lds, h_Z0, ldz0, s, &chunks);
+  if (rs != ZFAC_OK) return rs;
+  HostOverlap ho{low, nullptr, 0};
+  ho.dS = dS; ho.chunks = chunks;
+  IterHook low_hook{nullptr, &ho};
+  low_hook.first_a1 = host_first_a1;
+  const bool z_dev = high->opt.host_overlap && host_pinned(h_Z);
+  RefiDownload rd{high, h_Z, ldz, refi_steps - 1};
+  IterHook high_hook{refi_after_a5, &rd};
+  if (z_dev && (rs = host_side_objects(high)) != ZFAC_OK) return rs;
+  rs = refi_impl(low, high, dS, low->n, dZ0, low->n, dZ, high->n, max_iter, refi_steps, final_check, dInts, dErr, dInts + 1,
+                 dInts + 2, s, chunks > 0 ? &low_hook : nullptr, chunks > 0 ? 2 : 3, z_dev ? &high_hook : nullptr);
+  if (rs != ZFAC_OK) return rs;
+  if (z_dev) ZF_CUDA(cudaStreamWaitEvent(s, high->ev_copy, 0));
+  else ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)high->n, cudaMemcpyDeviceToHost, s));
+  int ints[4] = {0, 0, 0, 0};
+  ZF_CUDA(cudaMemcpyAsync(ints, dInts, 4 * sizeof(int), cudaMemcpyDeviceToHost, s));
+  ZF_CUDA(cudaStreamSynchronize(s));
+  *h_iters = ints[0]; *h_flags = ints[1];
+  if (z_dev && ints[2] != refi_steps)      // the refinement stage stopped early: the early download is not the result
+    ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)high->n, cudaMemcpyDeviceToHost, s));
+  ZF_CUDA(cudaMemcpyAsync(h_err, dErr, (size_t)ints[3] * sizeof(double), cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaStreamSynchronize(s));
   return ZFAC_OK;
 }
@@ -580,6 +740,7 @@ zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const v
   if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
   if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
   if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
+  if (!on_own_device(c)) return ZFAC_E_INVALID;
   const Layout& L = c->L;
   char* ws = c->ws;
   zfac_graph* zg = new (std::nothrow) zfac_graph();
@@ -605,6 +766,7 @@ zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const v
     if ((e = cudaGraphConditionalHandleCreate(&h, g, 1, cudaGraphCondAssignDefault)) != cudaSuccess) { fail("conditional handle", e); break; }
     // root: copy-in, first residual (its stop test already sets the condition: max_iter = 0 or a non-finite Err[0] skip the loop)
     const int saved_launches = c->launches;
+    if ((e = clear_range(c, cs)) != cudaSuccess) { fail("memset", e); break; }
     launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, cs);
     cudaGraphNodeParams np = {};
     np.type = cudaGraphNodeTypeConditional;
@@ -645,7 +807,7 @@ zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const v
 }
 
 zfac_status zfac_graph_launch(zfac_graph* zg, void* stream) {
-  if (!zg || !zg->ex) return ZFAC_E_INVALID;
+  if (!zg || !zg->ex || !on_own_device(zg->c)) return ZFAC_E_INVALID;
   ZF_CUDA(cudaGraphLaunch(zg->ex, static_cast<cudaStream_t>(stream)));
   return ZFAC_OK;
 }
@@ -660,7 +822,7 @@ zfac_status zfac_graph_destroy(zfac_graph* zg) {
 }
 
 zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void* stream) {
-  if (!c || !d_out || ld < c->n) return ZFAC_E_INVALID;
+  if (!c || !d_out || ld < c->n || !on_own_device(c)) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;

@@ -14,7 +14,25 @@ struct State {
   int flags;                 // ZFAC_R_* bits
   int pad0;
   unsigned int arrive[4];    // last-CTA counters (one per use site), self-resetting
-  double zscale;             // reserved
+  int range;                 // != 0: a value of magnitude >= 65504 was clamped on its way into an fp16 operand (16-bit modes);
+                             // cleared by a memset node BEFORE the copy-in of a call (every CTA of the copy-in may set it),
+                             // merged into the published flags as ZFAC_R_RANGE
+  int pad1;
+};
+constexpr float H16_MAX = 65504.0f;   // largest finite fp16: cvt.rn.satfinite clamps beyond it
+
+// Per-context tuning / behaviour options (zfac_set_option; defaults here).  Host-side state only.
+struct Options {
+  int chunk_kb = 1;          // SPLIT16 a1/a2: k-blocks (64 products each) per promoted-accumulation chunk
+  int chunk0_kb = 1;         // ... of the first chunk of a tile
+  int band = 8;              // full GEMMs: tile columns per rasterisation band
+  int hh_square = 1;         // SPLIT16 a4/p2: (h)(h) pass only for updates taken from Err[n] <= hh_square_err
+  double hh_square_err = 0.1;
+  int promote_update = 0;    // SPLIT16: promoted accumulation in p2/a4/a5 too
+  int max_pairs = 0;         // run on at most this many CTA pairs (0: all that are co-resident)
+  int host_overlap = 1;      // zfac_refine_host: early download of Z after the first update
+  int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
+  int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
 };
 
 struct StopArgs {

@@ -103,6 +103,9 @@ struct CopyInArgs {
   void* oZb;           // SPLIT16 / HH16: half[planes][Np][Np] (Zb[0])
   int what;            // bit 0: S, bit 1: Z0 (and W, State reset); 0 is read as 3 (both)
   int ty0;             // first tile row of this launch (grid.y counts from it): row chunks of S for zfac_refine_host
+  // zfac_refine_refi: Z0 is the result of a low-precision run, taken straight from that context's workspace.
+  const State* prev;   // State of the low-precision context (null: none)
+  const void* Z0_alt;  // Z0 is this buffer instead when prev->iters is odd (modes whose Z buffers alternate); may be null
 };
 
 // One tile of CI_TR = 32 rows x CI_TC = 64 columns per CTA (256 threads).  Phase 1: coalesced loads of the S and Z0
@@ -117,10 +120,14 @@ struct CopyInArgs {
 constexpr int CI_TR = 32, CI_TC = 64, CI_PITCH = CI_TC + 1;
 
 template <int MODE>
-__device__ __forceinline__ void ci_store8(void* buf, size_t np2, size_t o, const float (&v)[8], bool operand) {
+__device__ __forceinline__ void ci_store8(void* buf, size_t np2, size_t o, const float (&v)[8], bool operand, State* st) {
   // 8 consecutive FP32 values -> the mode's representation at element offset o (o is a multiple of 8).
   // operand = true: a buffer only the tensor core reads (S, W; Zb): fp16 plane(s) / TF32-rounded FP32.
   if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) {
+    float mx = 0.0f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) mx = fmaxf(mx, fabsf(v[j]));
+    if (mx >= H16_MAX) atomicOr(&st->range, 1);          // cvt.rn.satfinite is about to clamp: ZFAC_R_RANGE
     uint32_t hi[4], lo[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
@@ -152,13 +159,16 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
   const int t = threadIdx.x;
   const bool doS = (a.what == 0) || (a.what & 1), doZ = (a.what == 0) || (a.what & 2);
   if (doZ && blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
-    a.st->done = 0; a.st->iters = 0; a.st->flags = 0;
+    // refinement stage of Alg. 3 behind a low-precision run that ended non-finite: nothing to refine -- every later
+    // kernel of this context exits at once (done = 1) and no Err entry exists (iters = -1)
+    const bool dead = a.prev && (a.prev->flags & ZFAC_R_NONFINITE);
+    a.st->done = dead ? 1 : 0; a.st->iters = dead ? -1 : 0; a.st->flags = 0;
     a.st->arrive[0] = a.st->arrive[1] = a.st->arrive[2] = a.st->arrive[3] = 0u;
   }
   const int c0 = blockIdx.x * CI_TC, r0 = ((int)blockIdx.y + a.ty0) * CI_TR;
   const size_t np = (size_t)a.np, np2 = np * np;
   const Tin* S = static_cast<const Tin*>(a.S);
-  const Tin* Z0 = static_cast<const Tin*>(a.Z0);
+  const Tin* Z0 = static_cast<const Tin*>((a.prev && a.Z0_alt && (a.prev->iters & 1)) ? a.Z0_alt : a.Z0);
   // ---- phase 1: coalesced loads (64 consecutive columns per row), identity padding
 #pragma unroll
   for (int i = 0; i < CI_TR * CI_TC / 256; ++i) {
@@ -188,7 +198,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
         float vs[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) vs[j] = (float)sS[lr * CI_PITCH + lc + j];
-        ci_store8<MODE>(a.oS, np2, o, vs, true);
+        ci_store8<MODE>(a.oS, np2, o, vs, true, a.st);
       }
       if (doZ) {
         float vz[8];
@@ -197,7 +207,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
         float* z32 = static_cast<float*>(a.oZ);                     // FP32 Z (the master copy in the 16-bit modes): not rounded
         *reinterpret_cast<float4*>(z32 + o) = make_float4(vz[0], vz[1], vz[2], vz[3]);
         *reinterpret_cast<float4*>(z32 + o + 4) = make_float4(vz[4], vz[5], vz[6], vz[7]);
-        if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true);
+        if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true, a.st);
       }
     }
   }
@@ -215,26 +225,39 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
       float vw[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) vw[j] = (float)sZ[(wc + j) * CI_PITCH + wr];
-      ci_store8<MODE>(a.oW, np2, o, vw, true);
+      ci_store8<MODE>(a.oW, np2, o, vw, true, a.st);
     }
   }
 }
 
 // ------------------------------------------------------------------ copy-out (step a6)
 struct CopyOutArgs {
-  const void* Zbuf[2];   // internal Z buffers (selected by iters parity; equal in the 16-bit modes)
+  const void* Zbuf[2];   // internal Z buffers (selected by the parity of the update count; equal in the 16-bit modes)
   void* Z; int64_t ldz;
   int n, np;
   const State* st;
   int* d_iters; int* d_flags;   // may be null (refinement step, congruence)
-  int parity;                   // -1: buffer = Zbuf[st->iters & 1]; else Zbuf[parity]
+  int parity;                   // >= 0: Zbuf[parity];  -1: Zbuf[st->iters & 1] (plain call);  -2: Zbuf[updates_done & 1]
 };
+// Number of Z updates a call has performed.  State::iters is the index of the last Err written; it equals the update
+// count unless the call ended with an update whose residual was not evaluated (Alg. 3 as printed: done stays 0).
+__device__ __forceinline__ int updates_done(const State* st) {
+  const int it = st->iters;
+  return st->done ? (it > 0 ? it : 0) : it + 1;
+}
+__device__ __forceinline__ int published_flags(const State* st) { return st->flags | (st->range ? ZFAC_R_RANGE : 0); }
+// `plain`: the ordinary call (every residual evaluated): the update count is State::iters itself.
+__device__ __forceinline__ void publish_and_select(const CopyOutArgs& a, bool first, const void*& src) {
+  const int iters = a.st->iters;
+  if (a.d_iters && first) { *a.d_iters = iters; *a.d_flags = published_flags(a.st); }
+  src = a.Zbuf[a.parity >= 0 ? a.parity : (a.parity == -1 ? (iters & 1) : (updates_done(a.st) & 1))];
+}
 
 template <typename T>
 __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
-  const int iters = a.st->iters;
-  if (a.d_iters && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { *a.d_iters = iters; *a.d_flags = a.st->flags; }
-  const T* src = static_cast<const T*>(a.Zbuf[a.parity >= 0 ? a.parity : (iters & 1)]);
+  const void* sel;
+  publish_and_select(a, blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0, sel);
+  const T* src = static_cast<const T*>(sel);
   T* dst = static_cast<T*>(a.Z);
   const int c = blockIdx.x * 256 + threadIdx.x;
   const int r0 = blockIdx.y * 8;
@@ -249,9 +272,9 @@ __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
 // 16-byte-vector variant for the aligned case (N * sizeof(T), both pitches and both base pointers multiples of
 // 16 bytes): one uint4 per thread and row, 8 rows per block row.
 __global__ void __launch_bounds__(256) copy_out_vec16_kernel(const CopyOutArgs a, int elt) {
-  const int iters = a.st->iters;
-  if (a.d_iters && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { *a.d_iters = iters; *a.d_flags = a.st->flags; }
-  const char* src = static_cast<const char*>(a.Zbuf[a.parity >= 0 ? a.parity : (iters & 1)]);
+  const void* sel;
+  publish_and_select(a, blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0, sel);
+  const char* src = static_cast<const char*>(sel);
   char* dst = static_cast<char*>(a.Z);
   const size_t row_bytes = (size_t)a.n * elt, spitch = (size_t)a.np * elt, dpitch = (size_t)a.ldz * elt;
   const size_t cb = ((size_t)blockIdx.x * 256 + threadIdx.x) * 16;
@@ -267,13 +290,22 @@ __global__ void __launch_bounds__(256) copy_out_vec16_kernel(const CopyOutArgs a
 }
 
 // ------------------------------------------------------------------ Alg. 3 bookkeeping
-// Appends the FP64 refinement history to the low-precision one and publishes iters / flags.
-__global__ void refi_merge_kernel(const double* err64, int n64, int refi_steps, double* d_err, int* d_iters, int* d_flags) {
+// Publishes iters / flags of a call without copying Z out (the low-precision stage of zfac_refine_refi, whose result
+// the refinement stage takes straight from the workspace).
+__global__ void publish_kernel(const State* st, int* d_iters, int* d_flags) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) { *d_iters = st->iters; *d_flags = published_flags(st); }
+}
+// Appends the history of the refinement stage (State `hi`, Err entries in err_hi) to the low-precision one and
+// publishes iters / flags.  Everything is taken from the refinement stage's State, so a stage that stopped early
+// (non-finite residual) or never ran (non-finite low-precision result) is reported as it happened.
+__global__ void refi_merge_kernel(const State* hi, const double* err_hi, double* d_err, int* d_iters, int* d_flags, int* d_upd) {
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     const int k = *d_iters;                       // stop index of the low-precision run
-    for (int i = 0; i < n64; ++i) d_err[k + 1 + i] = err64[i];
-    *d_iters = k + refi_steps;
-    *d_flags |= ZFAC_R_REFINED;
+    const int entries = hi->iters + 1, upd = updates_done(hi);
+    for (int i = 0; i < entries; ++i) d_err[k + 1 + i] = err_hi[i];
+    *d_iters = k + upd;
+    if (d_upd) { d_upd[0] = upd; d_upd[1] = k + 1 + entries; }     // refinement updates performed; Err entries in total
+    *d_flags |= (upd > 0 ? ZFAC_R_REFINED : 0) | (hi->flags & ZFAC_R_NONFINITE) | (hi->range ? ZFAC_R_RANGE : 0);
   }
 }
 

@@ -263,6 +263,16 @@ __device__ __forceinline__ void load_f32_row(const float* p, float (&v)[N]) {
   }
 }
 
+// A magnitude >= 65504 is clamped by the fp16 conversion (cvt.rn.satfinite) without producing inf / NaN: report it
+// (ZFAC_R_RANGE) for the two outputs whose size the iteration does not bound, T = (S Z)^T and Z.
+template <int N>
+__device__ __forceinline__ void flag_h16_range(State* st, const float (&v)[N]) {
+  float mx = 0.0f;
+#pragma unroll
+  for (int j = 0; j < N; ++j) mx = fmaxf(mx, fabsf(v[j]));
+  if (mx >= H16_MAX) atomicOr(&st->range, 1);
+}
+
 // Fused epilogue for SUB consecutive columns n..n+SUB-1 of row m (v = accumulator values).
 template <int KIND, int EPI, int SUB>
 __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SUB], int m, int n, bool offdiag,
@@ -276,7 +286,10 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
       store_f32_row<SUB>(p.f32_out + off, v);
-    } else store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
+    } else {
+      flag_h16_range<SUB>(p.st, v);
+      store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
+    }
   } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
     // sum of squares: FP32 inside this group of SUB (16 / 32) columns, FP64 across groups, tiles and CTAs.  One DFMA
     // plus one conversion per ELEMENT was 13 % of all warp samples of a2 (a quarter of its non-waiting time,
@@ -362,6 +375,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
       for (int j = 0; j < SUB; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
     } else {
+      flag_h16_range<SUB>(p.st, v);
       store_h_row<PAIR, SUB>(p.h_out, plane, off, v);                // Z16 next
       store_h_col<PAIR, SUB>(p.h_out_t, plane, offt, ld, v);         // W16 = Z16^T
     }
@@ -753,14 +767,8 @@ struct UmmaPlan {
   char* ws = nullptr;
   int max_pairs = 0;  // CTA pairs that are co-resident on the device (74 on a B200)
   int mode = 0;
-  int chunk_kb = 4;   // promoted-accumulation chunk: 4 k-blocks = 256 products per FP32-RN add
-  int chunk0_kb = 16; // first chunk of every tile (covers the previous tile's stores; partial sums still small)
-  int band = 8;             // rasterisation band width of the full GEMMs, in tile columns (tuning knob ZFAC_BAND)
-  int hh_square = 1;        // SPLIT16: the second-order products of step a4 (R R; P G for m > 2) use the (h)(h) pass only
-  double hh_err_max = 0.1;  // ... for updates taken from Err[n] <= this (DESIGN.md §5 "One pass for the second-order
-                            // product"); ZFAC_HH_SQUARE=0 restores three passes everywhere, ZFAC_HH_SQUARE_ERR sets the bound
-  int promote_update = 0;   // tuning knob (ZFAC_PROMOTE_UPDATE=1): promoted accumulation in the update GEMMs (p2, a4, a5)
-                            // too.  Measured to change Err[1] by 1.5e-5 relative only: off.
+  const Options* opt = nullptr;   // the context's options (zfac_set_option): chunk lengths, band, one-pass a4, max_pairs
+  int pairs() const { return (opt->max_pairs > 0 && opt->max_pairs < max_pairs) ? opt->max_pairs : max_pairs; }
   // tensor maps of every operand buffer (box 128 B x 64 rows, 128B swizzle)
   CUtensorMap mS, mW, mT, mR, mQ, mZ[2];
 };
@@ -777,11 +785,11 @@ inline cudaError_t make_map(PFN_encodeTiled enc, CUtensorMap* m, void* base, CUt
 }
 
 template <int KIND, int EPI>
-inline cudaError_t prepare_kernel(int* max_pairs) {
+inline cudaError_t prepare_kernel(int* max_pairs, int sm_count) {
   cudaError_t e = cudaFuncSetAttribute(umma_gemm_kernel<KIND, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
   if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(2 * 148); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES;
+  cfg.gridDim = dim3(2 * (sm_count / 2)); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES;
   int nc = 0;
   e = cudaOccupancyMaxActiveClusters(&nc, umma_gemm_kernel<KIND, EPI>, &cfg);
   if (e != cudaSuccess) return e;
@@ -797,24 +805,18 @@ inline cudaError_t prepare_kernel(int* max_pairs) {
 }
 
 template <int KIND>
-inline cudaError_t prepare_kind(int* max_pairs) {
+inline cudaError_t prepare_kind(int* max_pairs, int sm_count) {
   cudaError_t e;
-  if ((e = prepare_kernel<KIND, EPI_A1>(max_pairs)) != cudaSuccess) return e;
-  if ((e = prepare_kernel<KIND, EPI_A2>(max_pairs)) != cudaSuccess) return e;
-  if ((e = prepare_kernel<KIND, EPI_X3>(max_pairs)) != cudaSuccess) return e;
-  if ((e = prepare_kernel<KIND, EPI_A4>(max_pairs)) != cudaSuccess) return e;
-  if ((e = prepare_kernel<KIND, EPI_P2>(max_pairs)) != cudaSuccess) return e;
-  return prepare_kernel<KIND, EPI_A5>(max_pairs);
+  if ((e = prepare_kernel<KIND, EPI_A1>(max_pairs, sm_count)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_A2>(max_pairs, sm_count)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_X3>(max_pairs, sm_count)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_A4>(max_pairs, sm_count)) != cudaSuccess) return e;
+  if ((e = prepare_kernel<KIND, EPI_P2>(max_pairs, sm_count)) != cudaSuccess) return e;
+  return prepare_kernel<KIND, EPI_A5>(max_pairs, sm_count);
 }
 
-inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int sm_count) {
-  pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0;
-  if (const char* ck = getenv("ZFAC_CHUNK_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk_kb = v; }   // tuning knobs
-  if (const char* ck = getenv("ZFAC_CHUNK0_KB")) { int v = atoi(ck); if (v >= 1 && v <= 1024) pl->chunk0_kb = v; }
-  if (const char* ck = getenv("ZFAC_BAND")) { int v = atoi(ck); if (v >= 1 && v <= 4096) pl->band = v; }
-  if (const char* ck = getenv("ZFAC_HH_SQUARE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->hh_square = v; }
-  if (const char* ck = getenv("ZFAC_HH_SQUARE_ERR")) { double v = atof(ck); if (v >= 0.0) pl->hh_err_max = v; }
-  if (const char* ck = getenv("ZFAC_PROMOTE_UPDATE")) { int v = atoi(ck); if (v == 0 || v == 1) pl->promote_update = v; }
+inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int sm_count, const Options* opt) {
+  pl->L = L; pl->ws = ws; pl->mode = L.mode; pl->max_pairs = 0; pl->opt = opt;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -832,7 +834,7 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = make_map(enc, &pl->mQ, ws + L.off_Qb, H, 2, rows, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Zb[0], H, 2, rows, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], H, 2, rows, np)) != cudaSuccess) return e;
-    e = (L.mode == ZFAC_MODE_SPLIT16) ? prepare_kind<KIND_F16X2>(&pl->max_pairs) : prepare_kind<KIND_HH16>(&pl->max_pairs);
+    e = (L.mode == ZFAC_MODE_SPLIT16) ? prepare_kind<KIND_F16X2>(&pl->max_pairs, sm_count) : prepare_kind<KIND_HH16>(&pl->max_pairs, sm_count);
     if (e != cudaSuccess) return e;
   } else {
     const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
@@ -843,11 +845,9 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = make_map(enc, &pl->mQ, ws + L.off_Q, F, 4, np, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Z[0], F, 4, np, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Z[1], F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = prepare_kind<KIND_TF32>(&pl->max_pairs)) != cudaSuccess) return e;
+    if ((e = prepare_kind<KIND_TF32>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
   }
   if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
-  // tuning knob: run on fewer CTA pairs (the power-cap experiment of profiles/r1c_sweep.md)
-  if (const char* ck = getenv("ZFAC_MAX_PAIRS")) { int v = atoi(ck); if (v >= 1 && v < pl->max_pairs) pl->max_pairs = v; }
   return cudaSuccess;
 }
 
@@ -887,11 +887,11 @@ struct UmmaSeq {
     const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
                                    : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
     const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
-    grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
-    grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
+    grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
+    grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());
     order = order_;
     nsplit_ = nsplit;
-    p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band;
+    p.np = (int)L.np; p.macro_tiles = T; p.band = pl.opt->band;
     p.st = reinterpret_cast<State*>(ws + L.off_state);
 #ifdef ZFAC_TIMING
     p.dbg = reinterpret_cast<unsigned long long*>(ws + L.off_dbg);
@@ -913,7 +913,7 @@ struct UmmaSeq {
     const Layout& L = pl.L;
     char* ws = pl.ws;
     p.hh_only = 0;
-    p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
+    p.chunk_kb = pl.opt->chunk_kb; p.chunk0_kb = pl.opt->chunk0_kb;
     p.mapA = pl.mW; p.mapB = pl.mS; p.f32_in = nullptr; p.h_out_t = nullptr;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; }
@@ -921,7 +921,7 @@ struct UmmaSeq {
     if (mcn > 0) {
       p.joff = mc0 * nsplit_; p.jcols = mcn * nsplit_;
       const int tiles = p.macro_tiles * p.jcols;
-      grid = 2 * (tiles < pl.max_pairs ? tiles : pl.max_pairs);
+      grid = 2 * (tiles < pl.pairs() ? tiles : pl.pairs());
     }
     umma_launch_mode(L.mode, EPI_A1, grid, s, p);
     p.joff = 0; p.jcols = 0;
@@ -936,11 +936,12 @@ struct UmmaSeq {
     if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
     if (!skip_a1) a1(0, 0, s);
     p.hh_only = 0; p.f32_in = nullptr; p.h_out_t = nullptr;
-    p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
+    p.chunk_kb = pl.opt->chunk_kb; p.chunk0_kb = pl.opt->chunk0_kb;
     // a2: R = I - W T^T
     if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
     p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = R32; p.stop.n_iter = n_stop;
-    p.chunk0_kb = 2 * pl.chunk0_kb;           // a2 writes four outputs per element: its stores take twice as long
+    // a2 writes four outputs per element: its stores take twice as long, so a long first chunk (if one is set) doubles
+    if (pl.opt->chunk0_kb > pl.opt->chunk_kb) p.chunk0_kb = 2 * pl.opt->chunk0_kb;
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
     umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
     nl += 1;
@@ -954,10 +955,10 @@ struct UmmaSeq {
     char* ws = pl.ws;
     p.stop.n_iter = n_stop;
     // a4: Q = 1/2 R + 3/8 R R^T   (the product is a correction of size |R|^2: no promotion needed)
-    if (pl.promote_update) { p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb; }
+    if (pl.opt->promote_update) { p.chunk_kb = pl.opt->chunk_kb; p.chunk0_kb = pl.opt->chunk0_kb; }
     else { p.chunk_kb = 0; p.chunk0_kb = 0; }
-    p.hh_only = (L.mode == ZFAC_MODE_SPLIT16 && pl.hh_square) ? 1 : 0;      // p2 and a4 only; a5 below needs all passes
-    p.hh_err_max = pl.hh_err_max;
+    p.hh_only = (L.mode == ZFAC_MODE_SPLIT16 && pl.opt->hh_square) ? 1 : 0;      // p2 and a4 only; a5 below needs all passes
+    p.hh_err_max = pl.opt->hh_square_err;
     if (order > 2) {
       // order m > 2 (zfac.h, zfac_set_order): P = R R^T -> T buffer (free between a2 and the next a1),
       // G = 3/8 I + 5/16 R (+ 35/128 P) -> the Z operand buffer a5 is about to overwrite; then Q = 1/2 R + P G^T
@@ -993,7 +994,7 @@ struct UmmaSeq {
         const int i0 = (int)((long long)T * b / bands), i1 = (int)((long long)T * (b + 1) / bands);
         p.ioff = i0; p.irows = i1 - i0;
         const int tiles = p.irows * T * nsplit_;
-        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.max_pairs ? tiles : pl.max_pairs), s, p);
+        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.pairs() ? tiles : pl.pairs()), s, p);
         hook->after_a5_band(hook->self, i0 * UM_MACRO, i1 * UM_MACRO, b == bands - 1, s);
       }
       p.ioff = 0; p.irows = 0;
@@ -1005,11 +1006,13 @@ struct UmmaSeq {
   }
 };
 
+// skip_last: Alg. 3 as printed ends after the update, without evaluating the residual of the result.
 inline cudaError_t umma_refine(const UmmaPlan& pl, int max_iter, int stop, int order, double* d_err, cudaStream_t s, int* launches, Prof* prof,
-                               const IterHook* hook = nullptr) {
+                               const IterHook* hook = nullptr, bool skip_last = false) {
   UmmaSeq q(pl, max_iter, stop, order, d_err, 0ull);
   const bool banded = hook && hook->first_a1 && hook->first_a1(hook->self, &q, s);   // copy-in of S + a1, band by band
   for (int n = 0; n <= max_iter; ++n) {
+    if (n == max_iter && skip_last) break;
     q.residual(n, n, s, prof, banded && n == 0);
     if (n == max_iter) break;
     const bool a5_banded = (n == 0 && hook && hook->a5_bands > 1 && hook->after_a5_band);
@@ -1029,10 +1032,10 @@ inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* laun
   const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
                                  : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
   const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
-  const int grid_full = 2 * (full_tiles < pl.max_pairs ? full_tiles : pl.max_pairs);
-  const int grid_sym = 2 * (sym_tiles < pl.max_pairs ? sym_tiles : pl.max_pairs);
+  const int grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
+  const int grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T; p.band = pl.band; p.chunk_kb = pl.chunk_kb; p.chunk0_kb = pl.chunk0_kb;
+  p.np = (int)L.np; p.macro_tiles = T; p.band = pl.opt->band; p.chunk_kb = pl.opt->chunk_kb; p.chunk0_kb = pl.opt->chunk0_kb;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
   const bool h16 = (L.mode != ZFAC_MODE_TF32);
   p.mapA = pl.mW; p.mapB = pl.mS;

@@ -75,3 +75,21 @@ def test_no_gpu_means_loud_failure(binding):
         pytest.skip("GPU present")
     with pytest.raises(RuntimeError):
         binding.Zfac(64, "f64")
+
+
+def test_header_is_c99_and_a_plain_c_consumer_links(binding, tmp_path):
+    """include/zfac.h is a C header (no C++ in it) and a C99 program that calls the ABI links against libzfac.so
+    (tests/abi_consumer.c; the GPU suite runs it)."""
+    import subprocess
+    res = subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-fsyntax-only", "-x", "c",
+                          os.path.join(ROOT, "include", "zfac.h")], capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
+    from abi_build import compile_consumer
+    assert os.path.exists(compile_consumer(str(tmp_path / "abi_consumer")))
+
+
+def test_library_reads_no_environment_variable():
+    """Behaviour is set through zfac_set_option only (include/zfac.h): no hidden process-global state."""
+    csrc = os.path.join(ROOT, "paper_2404_19163_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f

@@ -28,6 +28,12 @@ ERR_ABS = {"f64": 0.0, "split16": 2e-6, "tf32": 0.0, "hh16": 0.0}
 # ... never below 1e-12: F64 forms X ~ I to one ulp, ||R_gpu - R_ora||_F measured <= 7e-14 up to N = 700 (this is also
 # the absolute tolerance pytest.approx applies silently when only `rel` is given; here it is explicit)
 ERR_ABS_MIN = 1e-12
+# KNOWN FLOOR (not a widened gate): SPLIT16 accumulates in FP32; its error of Z is ~u kappa (with a native
+# FP32 control on the same GPU).  Where kappa N puts that floor above the north_star gate 1e-5, the raw SPLIT16 run is
+# held to the floor named here and the GATE itself is asserted on the path that can meet it: SPLIT16 + the refinement
+# step of Alg. 3 (test_config4_full_size_n8192_bench_workload, test_time_to_gate_paths_config5_n8192).
+FLOOR_CONFIG5_N8192 = 5e-5        # kappa = 1e3, N = 8192: measured 4.4e-5 (native FP32: 5.0e-5)
+FLOOR_KAPPA_1E5 = 5e-3            # kappa = 1e5 (configs 3, 4): measured 2.4e-4 .. 3.8e-4 (native FP32: 3.6e-4)
 
 
 def err_abs(mode, n):
@@ -51,10 +57,13 @@ def _rel(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
-def gpu_refine(w, mode, max_iter, stop, keep=None, order=2):
+def gpu_refine(w, mode, max_iter, stop, keep=None, order=2, options=None):
     b = zb()
     S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
     with b.Zfac(w.n, mode, DEV) as zf:
+        for k, v in (options or {}).items():
+            zf.set_option(k, v)
+            assert zf.get_option(k) == pytest.approx(v)
         if order != 2:
             zf.set_order(order)
             assert zf.order == order
@@ -243,20 +252,17 @@ def test_concurrent_contexts_on_streams_match_sequential_runs_bitwise(mode):
 
 # ------------------------------------------------------------------ one pass for the second-order product
 @pytest.mark.parametrize("case", ["config2_n2048", "general_n700"])
-def test_one_pass_square_below_the_err_bound_does_not_change_z(case, monkeypatch):
+def test_one_pass_square_below_the_err_bound_does_not_change_z(case):
     """SPLIT16 runs a4's product R R with the (h)(h) pass only for updates taken from Err[n] <= 0.1.  A/B against three
-    passes everywhere (ZFAC_HH_SQUARE=0; the knobs are read when a context is created): same stop index, Z agrees with
+    passes everywhere (zfac_set_option ZFAC_OPT_HH_SQUARE = 0): same stop index, Z agrees with
     the oracle equally well (the bound is where the surviving rotation 9e-5 Err^3 drops below 2^-23), and the two
-    results differ by less than the gate -- while WITHOUT the bound (ZFAC_HH_SQUARE_ERR=1e9) Z is measurably worse."""
+    results differ by less than the gate -- while WITHOUT the bound (ZFAC_OPT_HH_SQUARE_ERR = 1e9) Z is measurably
+    worse.  (The headline workload, config 4 at N = 8192, has its own A/B in the full-size test below.)"""
     b = zb()
     w = W.config2(2048) if case == "config2_n2048" else W.random_spd_general(700, seed=800, kappa=20.0, pert=0.1, fp32_stored=True)
     out = {}
-    for name, env in (("three", {"ZFAC_HH_SQUARE": "0"}), ("default", {}), ("unbounded", {"ZFAC_HH_SQUARE_ERR": "1e9"})):
-        for k in ("ZFAC_HH_SQUARE", "ZFAC_HH_SQUARE_ERR"):
-            monkeypatch.delenv(k, raising=False)
-        for k, v in env.items():
-            monkeypatch.setenv(k, v)
-        Z, it, err, fl, _, _ = gpu_refine(w, "split16", 40, b.ZFAC_STOP_PAPER)
+    for name, opts in (("three", {"hh_square": 0}), ("default", {}), ("unbounded", {"hh_square_err": 1e9})):
+        Z, it, err, fl, _, _ = gpu_refine(w, "split16", 40, b.ZFAC_STOP_PAPER, options=opts)
         out[name] = (Z, it, err)
     it = out["three"][1]
     assert out["default"][1] == it and (out["default"][2][:-1] <= 0.1).any()      # the bound really applied somewhere
@@ -553,10 +559,10 @@ def test_host_buffer_entry_point(mode):
 
 
 @pytest.mark.parametrize("mode", ["f64", "split16", "tf32"])
-def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise(mode, monkeypatch):
+def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise(mode):
     """zfac_refine_host with a PINNED Z starts the download of Z right after the first update, on a side stream
     (final if that update is the only one, superseded by the normal download otherwise); with a pageable Z, or
-    ZFAC_HOST_OVERLAP=0, there is one cudaMemcpy at the end.  All three must return exactly what zfac_refine returns for
+    ZFAC_OPT_HOST_OVERLAP = 0, there is one cudaMemcpy at the end.  All three must return exactly what zfac_refine returns for
     the same inputs -- with ld > n, where the guard columns of the caller's buffer must stay untouched; with a start that
     needs several updates (the early download is stale); with one that needs exactly one (it is the result); and with
     a non-finite start (no update runs: Z = Z0 comes back)."""
@@ -569,8 +575,8 @@ def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise
         Zref, itref, errref, flref = zf.refine(Sd, Z0d, max_iter=30, stop=b.ZFAC_STOP_PAPER)
         Zref = Zref.cpu()
         assert itref >= 2
-        for pinned, overlap in ((True, "1"), (False, "1"), (True, "0")):
-            monkeypatch.setenv("ZFAC_HOST_OVERLAP", overlap)
+        for pinned, overlap in ((True, 1), (False, 1), (True, 0)):
+            zf.set_option("host_overlap", overlap)
             S = torch.from_numpy(w.S).to(dt); Z0 = torch.from_numpy(w.Z0).to(dt)
             Zbig = torch.full((n, n + 7), -5.0, dtype=dt)
             if pinned:
@@ -591,7 +597,7 @@ def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise
         _, it, err, fl = zf.refine_host(S, Z0, Z, max_iter=30, stop=b.ZFAC_STOP_PAPER)
         assert it == 1 and fl == fl1 and np.array_equal(err, err1) and torch.equal(Z, Zr1.cpu())
         # non-finite start: Err[0] = NaN stops at n = 0, no a5 runs, the caller gets Z0 back
-        monkeypatch.setenv("ZFAC_HOST_OVERLAP", "1")
+        zf.set_option("host_overlap", 1)
         Z0bad = torch.from_numpy(w.Z0).to(dt).clone(); Z0bad[3, 4] = float("nan")
         S = torch.from_numpy(w.S).to(dt).pin_memory(); Z0bad = Z0bad.pin_memory()
         Z = torch.zeros(n, n, dtype=dt).pin_memory()
@@ -602,7 +608,7 @@ def test_host_entry_point_overlapped_download_matches_device_entry_point_bitwise
 
 @pytest.mark.parametrize("mode,n,pad", [("split16", 1000, 0), ("split16", 1500, 13), ("tf32", 1111, 5), ("hh16", 2048, 0),
                                         ("split16", 2309, 3)])
-def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mode, n, pad, monkeypatch):
+def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mode, n, pad):
     """zfac_refine_host with pinned S and Z0 (tensor-core modes, padded dimension >= 1024) uploads S in row chunks on a
     side stream and runs copy-in + a1 band by band behind them (include/zfac.h).  The bands are disjoint sets of whole
     tiles, so the call must return exactly what zfac_refine returns -- with the overlap on, off, with pageable inputs
@@ -625,8 +631,8 @@ def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mo
             Zref, itref, errref, flref = zf.refine(Sd, Z0d, max_iter=max_iter, stop=b.ZFAC_STOP_PAPER)
             base = zf.last_launch_count
             Zref = Zref.cpu()
-            for pin, overlap, reps in ((True, "1", 2), (True, "0", 1), (False, "1", 1)):
-                monkeypatch.setenv("ZFAC_HOST_UPLOAD_OVERLAP", overlap)
+            for pin, overlap, reps in ((True, 1, 2), (True, 0, 1), (False, 1, 1)):
+                zf.set_option("host_upload_overlap", overlap)
                 S, Z0 = host(w.S, pin), host(w.Z0, pin)
                 Zbig = torch.full((n, n + pad), -5.0, dtype=dt)
                 Zbig = Zbig.pin_memory() if pin else Zbig
@@ -635,12 +641,12 @@ def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mo
                     assert it == itref and fl == flref and np.array_equal(err, errref), (max_iter, pin, overlap)
                     assert torch.equal(Zbig[:, :n], Zref), (max_iter, pin, overlap)
                     assert bool((Zbig[:, n:] == -5.0).all())
-                    banded = pin and overlap == "1"
+                    banded = pin and overlap == 1
                     a5_bands = pin and max_iter >= 1          # pinned h_Z: the first a5 runs in two row bands (early download)
                     assert zf.last_launch_count == base + ((chunks - 1) + chunks if banded else 0) + (1 if a5_bands else 0), \
                         (max_iter, pin, overlap)
         # exactly one update (a converged start): the rows downloaded band by band behind the first a5 ARE the result
-        monkeypatch.setenv("ZFAC_HOST_UPLOAD_OVERLAP", "1")
+        zf.set_option("host_upload_overlap", 1)
         lam, V = np.linalg.eigh(w.S)
         Zc = W.round_fp32((V / np.sqrt(lam)) @ V.T)
         Zr1, it1, err1, fl1 = zf.refine(Sd, _to_dev(Zc, mode), max_iter=30, stop=b.ZFAC_STOP_PAPER)
@@ -652,6 +658,193 @@ def test_host_entry_point_overlapped_upload_is_bitwise_the_device_entry_point(mo
             assert bool((Zbig[:, n:] == -5.0).all())
         else:
             assert mode in ("tf32", "hh16")                   # 11-bit operands: the FP32-rounded exact factor is not at their floor
+
+
+
+# ------------------------------------------------------------------ options, range flag, C consumer (boundary)
+def test_options_api_defaults_and_validation():
+    b = zb()
+    with b.Zfac(64, "split16", DEV) as zf:
+        defaults = {"chunk_kb": 1, "chunk0_kb": 1, "hh_square": 1, "hh_square_err": 0.1, "promote_update": 0, "band": 8,
+                    "max_pairs": 0, "host_overlap": 1, "host_upload_overlap": 1, "host_a5_bands": 2}
+        for k, v in defaults.items():
+            assert zf.get_option(k) == pytest.approx(v), k
+        for k, bad in (("chunk_kb", 0), ("chunk_kb", 5000), ("hh_square", 2), ("hh_square_err", -1.0), ("band", 0),
+                       ("host_a5_bands", 0), ("max_pairs", -1), (99, 1.0), ("chunk_kb", float("nan"))):
+            with pytest.raises(b.ZfacError) as e:
+                zf.set_option(k, bad)
+            assert e.value.status == b.ZFAC_E_INVALID
+        for k, v in defaults.items():
+            assert zf.get_option(k) == pytest.approx(v), k              # a rejected value changes nothing
+        zf.set_option("max_pairs", 3); zf.set_option("band", 2)          # scheduling-only options: bit-identical results
+        w = W.random_spd_general(600, seed=3, kappa=20.0, pert=0.1, fp32_stored=True)
+    base = gpu_refine(w, "split16", 30, b.ZFAC_STOP_PAPER)
+    alt = gpu_refine(w, "split16", 30, b.ZFAC_STOP_PAPER, options={"max_pairs": 3, "band": 2})
+    assert np.array_equal(base[0], alt[0]) and np.array_equal(base[2], alt[2]) and base[1] == alt[1]
+
+
+@pytest.mark.parametrize("mode", ["split16", "hh16", "tf32", "f64"])
+def test_fp16_range_overflow_is_flagged_not_silent(mode):
+    """The 16-bit modes clamp magnitudes >= 65504 on the way into an FP16 operand (cvt.rn.satfinite): no inf / NaN
+    appears, so ZFAC_R_NONFINITE cannot fire -- ZFAC_R_RANGE must (include/zfac.h).  S = c S_0 with c = 2.5e-10 puts
+    Z ~ S^-1/2 at ~6e4 lambda^-1/2: Z0 = I / sqrt(lambda_max) = 6.3e4 is still representable, the iterates are not, so
+    the flag comes from step a5's epilogue; with c = 1e-10 Z0 itself is out of range and the copy-in flags it.
+    TF32 and F64 have the FP32 / FP64 exponent range and must not flag."""
+    b = zb()
+    n = 300
+    base = W.spectral_workload(n, 0.1, 1.0, seed=4)
+    for c, where in ((2.5e-10, "a5"), (1e-10, "copy-in")):
+        S = W.round_fp32(base.S * c)
+        Z0 = W.round_fp32(np.eye(n) / math.sqrt(c * 1.01))
+        w = W.Workload(f"range_{where}", n, S, Z0, fp32_stored=True)
+        Z, it, err, fl, _, _ = gpu_refine(w, mode, 12, b.ZFAC_STOP_PAPER)
+        print(f"[range {mode} {where}] iters={it} flags={fl} max|Z|={np.abs(Z).max():.3e}")
+        if mode in ("split16", "hh16"):
+            assert fl & b.ZFAC_R_RANGE, where
+        else:
+            assert not (fl & b.ZFAC_R_RANGE)
+            assert np.abs(Z).max() > 65504.0
+    # ... and an ordinary problem never carries the flag (every other test of this file compares flags exactly)
+    w = W.random_spd_general(n, seed=9, kappa=20.0, pert=0.1, fp32_stored=True)
+    assert not (gpu_refine(w, mode, 30, b.ZFAC_STOP_PAPER)[3] & b.ZFAC_R_RANGE)
+
+
+def test_plain_c_consumer_runs_through_the_abi(tmp_path):
+    """tests/abi_consumer.c: a C99 program (no Python, no torch) that allocates with cudaMalloc, calls zfac_create /
+    zfac_refine / zfac_destroy in F64 and SPLIT16 and checks ||Z^T S Z - I||_F / sqrt(N) with plain loops."""
+    import subprocess
+    from abi_build import compile_consumer
+    exe = compile_consumer(str(tmp_path / "abi_consumer"))
+    res = subprocess.run([exe], capture_output=True, text=True, timeout=300)
+    print(res.stdout, res.stderr)
+    assert res.returncode == 0 and "abi_consumer: OK" in res.stdout
+
+
+# ------------------------------------------------------------------ Alg. 3 into an FP32-class mode: (h)(h) + refi (PAPER.md:240-244)
+@pytest.mark.parametrize("low", ["hh16", "tf32"])
+@pytest.mark.parametrize("n", [130, 300, 1100])
+def test_refi_into_split16_step_is_the_split16_iteration_bitwise(low, n):
+    """Alg. 3 steps 2-3 in isolation, refinement in SPLIT16 (the paper's single-precision refinement, "FP32[Z]",
+    PAPER.md:338): with max_iter = 0 the low-precision stage performs no update, Z = Z0 is handed over inside the
+    workspace, and the SPLIT16 stage must be, bit for bit, a SPLIT16 run of `steps` fixed updates from the same
+    inputs -- and match the FP64 oracle to the SPLIT16 gate."""
+    b = zb()
+    w = W.random_spd_general(n, seed=60 + n, kappa=30.0, pert=0.1, fp32_stored=True)
+    S, Z0 = _to_dev(w.S, low), _to_dev(w.Z0, low)
+    for steps, final_check in ((1, True), (2, True), (2, False)):
+        with b.Zfac(n, low, DEV) as zl, b.Zfac(n, "split16", DEV) as zh:
+            Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=0, refi_steps=steps, final_check=final_check)
+            assert Z.dtype == torch.float32
+            Zd, itd, errd, fld = zh.refine(S, Z0, max_iter=steps, stop=b.ZFAC_STOP_FIXED)
+        assert it == steps and (fl & b.ZFAC_R_REFINED) and (fl & b.ZFAC_R_MAXITER)
+        assert torch.equal(Z, Zd)
+        assert len(err) == 1 + steps + int(final_check)
+        assert np.array_equal(err[1:], errd[: steps + int(final_check)])
+        ref = O.refine(w.S, w.Z0, steps, O.STOP_FIXED)
+        assert _rel(Z.cpu().double().numpy(), ref.Z) <= TOL["split16"]
+
+
+@pytest.mark.parametrize("low,case", [("hh16", "paper_eq39"), ("tf32", "paper_eq39"), ("hh16", "config2")])
+def test_hh_plus_single_refinement_reaches_the_split16_level(low, case):
+    """The paper's fastest scheme, (h)(h) + refi with a single-precision refinement (PAPER.md:240-244, Fig. 2, :374:
+    "the 2-norm error drops to the same level as that of the single method"): HH16 (or TF32) to its stop, then two
+    SPLIT16 updates.  Z is not unique (rounding in the low-precision stage rotates it: any Z U is a factor), so what is
+    compared is what is unique -- the residual of the returned Z (oracle-evaluated) against the one a SPLIT16-only run
+    reaches, and Z Z^T against the oracle's Alg. 3 with the same refinement precision."""
+    b = zb()
+    w = W.paper_workload(1100, alpha=0.005) if case == "paper_eq39" else W.config2(2048)
+    S, Z0 = _to_dev(w.S, low), _to_dev(w.Z0, low)
+    with b.Zfac(w.n, low, DEV) as zl, b.Zfac(w.n, "split16", DEV) as zh:
+        Zlow, klow, errlow, fllow = zl.refine(S, Z0, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        Zlow = Zlow.cpu().double().numpy()
+        Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=30, refi_steps=2, final_check=True)
+        Zs, its, errs, fls = zh.refine(S, Z0, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+    Z = Z.cpu().double().numpy(); Zs = Zs.cpu().double().numpy()
+    r_low, r_refi, r_split = (O.final_residual_per_sqrt_n(w.S, z) for z in (Zlow, Z, Zs))
+    print(f"[{low}+refi(split16) {case}] low iters={klow} residual/sqrtN: {low} {r_low:.3e} -> refined {r_refi:.3e} "
+          f"(split16 alone, {its} updates: {r_split:.3e}) err={np.array2string(err, precision=3)}")
+    assert it == klow + 2 and (fl & b.ZFAC_R_REFINED) and len(err) == it + 2
+    assert np.array_equal(err[: klow + 1], errlow)
+    assert r_low > 20.0 * r_split                       # the one-pass run is far from the single level ...
+    assert r_refi < 3.0 * r_split                       # ... two SPLIT16 updates bring it there (PAPER.md:374)
+    ora = O.refine_with_refi(w.S, w.Z0, 30, low_dtype=np.float32, refi_steps=2, refi_dtype=np.float32)
+    assert _rel(Z @ Z.T, ora.Z.astype(np.float64) @ ora.Z.astype(np.float64).T) < 2e-5
+
+
+def test_refi_edge_cases_nonfinite_mismatch_and_pairs():
+    b = zb()
+    n = 200
+    w = W.random_spd_general(n, seed=77, kappa=30.0, pert=0.1, fp32_stored=True)
+    S, Z0 = _to_dev(w.S, "split16"), _to_dev(w.Z0, "split16")
+    with b.Zfac(n, "split16", DEV) as zs, b.Zfac(n, "f64", DEV) as zf, b.Zfac(n, "hh16", DEV) as zh, \
+            b.Zfac(n, "tf32", DEV) as zt:
+        # pairs: the second context must be MORE precise; same n; same order
+        for lo, hi in ((zs, zh), (zs, zs), (zh, zt), (zs, zt)):
+            with pytest.raises(b.ZfacError) as e:
+                lo.refine_refi(hi, S, Z0, max_iter=5)
+            assert e.value.status == b.ZFAC_E_INVALID
+        zf.set_order(3)
+        with pytest.raises(b.ZfacError) as e:
+            zs.refine_refi(zf, S, Z0, max_iter=5)
+        assert e.value.status == b.ZFAC_E_INVALID
+        zf.set_order(2)
+        # a refinement AFTER a stale one: first a normal call, so that the FP64 workspace holds a finished run ...
+        Zg, itg, errg, flg = zs.refine_refi(zf, S, Z0, max_iter=20, refi_steps=2, final_check=True)
+        assert (flg & b.ZFAC_R_REFINED) and not (flg & b.ZFAC_R_NONFINITE)
+        # ... then a non-finite start: the low-precision run stops at n = 0, nothing is refined, nothing stale leaks
+        Zbad = Z0.clone(); Zbad[5, 7] = float("nan")
+        Z, it, err, fl = zs.refine_refi(zf, S, Zbad, max_iter=20, refi_steps=2, final_check=True)
+        assert it == 0 and (fl & b.ZFAC_R_NONFINITE) and not (fl & b.ZFAC_R_REFINED)
+        assert math.isnan(err[0])
+        Zr = Z.cpu().numpy()
+        assert np.isnan(Zr[5, 7]) and np.array_equal(np.nan_to_num(Zr, nan=0.0), np.nan_to_num(Zbad.cpu().double().numpy(), nan=0.0))
+        # TF32 -> F64: the low-precision result sits in the buffer of parity iters & 1; both parities must be handed over
+        seen = set()
+        for mi in (1, 2, 3):
+            Z, it, err, fl = zt.refine_refi(zf, S, Z0, max_iter=mi, refi_steps=1, final_check=False)
+            k = it - 1                                   # updates of the TF32 stage (its paper test may fire before max_iter)
+            Zt, kt, _, _ = zt.refine(S, Z0, max_iter=k, stop=b.ZFAC_STOP_FIXED)
+            assert kt == k
+            # one exact FP64 update of the TF32 iterate: reproduce it with the oracle's step from that iterate
+            Zt64 = Zt.cpu().double().numpy()
+            ref = O.update_delta_form(Zt64, O.residual(w.S, Zt64))
+            assert _rel(Z.cpu().numpy(), ref) <= 1e-11, mi
+            seen.add(k & 1)
+        assert seen == {0, 1}
+
+
+@pytest.mark.parametrize("low,high,n", [("split16", "f64", 300), ("hh16", "split16", 1100), ("split16", "f64", 1100),
+                                        ("tf32", "f64", 520)])
+def test_refi_host_entry_point_matches_the_device_entry_point_bitwise(low, high, n):
+    """zfac_refine_refi_host: upload (chunked and overlapped with a1 for n_pad >= 1024), Alg. 3, download of Z started
+    after the last refinement update.  Must return exactly what zfac_refine_refi returns -- pinned and pageable,
+    with and without the final check, with ld > n on the host side."""
+    b = zb()
+    w = W.random_spd_general(n, seed=n + 5, kappa=40.0, pert=0.1, fp32_stored=True)
+    S, Z0 = _to_dev(w.S, low), _to_dev(w.Z0, low)
+    hdt = _dt(high)
+    with b.Zfac(n, low, DEV) as zl, b.Zfac(n, high, DEV) as zh:
+        for steps, fc in ((1, True), (2, False)):
+            Zd, itd, errd, fld = zl.refine_refi(zh, S, Z0, max_iter=30, refi_steps=steps, final_check=fc)
+            Zd = Zd.cpu()
+            for pin in (True, False):
+                hS = torch.full((n, n + 3), float("nan"), dtype=torch.float32); hS[:, :n] = torch.from_numpy(w.S).float()
+                hZ0 = torch.from_numpy(w.Z0).float().contiguous()
+                hZ = torch.full((n, n + 5), -7.0, dtype=hdt)
+                if pin:
+                    hS, hZ0, hZ = hS.pin_memory(), hZ0.pin_memory(), hZ.pin_memory()
+                _, it, err, fl = zl.refine_refi_host(zh, hS[:, :n], hZ0, hZ[:, :n], max_iter=30, refi_steps=steps, final_check=fc)
+                assert it == itd and fl == fld and np.array_equal(err, errd), (steps, fc, pin)
+                assert torch.equal(hZ[:, :n], Zd), (steps, fc, pin)
+                assert bool((hZ[:, n:] == -7.0).all())
+        # a non-finite refinement residual cannot be provoked from finite inputs; the early-download fallback is covered by
+        # the non-finite START: no refinement update runs, the early download is skipped / superseded
+        hZ0 = torch.from_numpy(w.Z0).float().contiguous(); hZ0[1, 2] = float("nan")
+        hS = torch.from_numpy(w.S).float().contiguous().pin_memory(); hZ0 = hZ0.pin_memory()
+        hZ = torch.zeros(n, n, dtype=hdt).pin_memory()
+        _, it, err, fl = zl.refine_refi_host(zh, hS, hZ0, hZ, max_iter=30, refi_steps=2, final_check=True)
+        assert it == 0 and (fl & b.ZFAC_R_NONFINITE) and not (fl & b.ZFAC_R_REFINED)
+        assert torch.equal(torch.nan_to_num(hZ, nan=-1.0), torch.nan_to_num(hZ0.to(hdt), nan=-1.0))
 
 
 # ------------------------------------------------------------------ Alg. 3 ("+refi") and the congruence transformation
@@ -833,7 +1026,7 @@ def test_config3_shape_n1155_illconditioned_trace():
     ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
     rel = _rel(Z, ref.Z)
     print(f"[config3/4 split16] iters={it} rel={rel:.3e} err={np.array2string(err, precision=3)}")
-    assert fl & b.ZFAC_R_STOPPED and rel <= 5e-3
+    assert fl & b.ZFAC_R_STOPPED and rel <= FLOOR_KAPPA_1E5
     Z, it, err, fl, _, _ = gpu_refine(w, "tf32", 40, b.ZFAC_STOP_PAPER)
     print(f"[config3/4 tf32] iters={it} flags={fl} err={np.array2string(err, precision=3)}")
     assert fl != 0 and len(err) == it + 1
@@ -849,7 +1042,7 @@ def test_config4_warm_start_n2048(mode):
     rel = _rel(Z, ref.Z)
     print(f"[config4 n=2048 {mode}] iters={it} rel={rel:.3e} err={np.array2string(err, precision=3)}")
     assert fl & b.ZFAC_R_STOPPED and 1 <= it <= 4
-    assert rel <= (1e-11 if mode == "f64" else 5e-3)
+    assert rel <= (1e-11 if mode == "f64" else FLOOR_KAPPA_1E5)
 
 
 def test_full_size_n8192_bench_configuration_properties():
@@ -886,9 +1079,12 @@ def test_full_size_n8192_bench_configuration_properties():
         rel = _rel(Z, Zref)
         print(f"[n=8192 {mode}] rel_F vs closed form={rel:.3e} sampled max rel err={samp:.3e} "
               f"||Z^T S Z - I||_F/sqrtN={inv:.3e} Err={err[-1]:.3e}")
-        assert rel <= (1e-11 if mode == "f64" else 5e-5)
+        assert rel <= (1e-11 if mode == "f64" else FLOOR_CONFIG5_N8192)
         assert samp <= tol_s
         assert inv <= (1e-11 if mode == "f64" else 5e-4)
+        # the history is honest at the floor: the reported Err[last] is the true residual of the returned Z to within
+        # 1.5x (SPLIT16: one-k-block promoted chunks; with 4 / 16 k-blocks it under-reported 5.4x here)
+        assert inv / 1.5 <= err[-1] / math.sqrt(n) <= inv * 1.5, (mode, err[-1] / math.sqrt(n), inv)
 
 
 def test_config5_n16384_against_spectral_closed_form():
@@ -1049,7 +1245,7 @@ def test_config3_full_size_n4617_all_modes_and_trace():
     print(f"[config3 N=4617 split16] iters={it} rel={rel:.3e} (u*kappa floor, DESIGN.md §6) "
           f"Err/sqrtN={O.final_residual_per_sqrt_n(w.S, Z):.3e} trace={np.array2string(err, precision=3)}")
     assert fl & b.ZFAC_R_STOPPED and 10 <= it <= 14
-    assert rel <= 5e-3                                               # derived bound at kappa = 1e5
+    assert rel <= FLOOR_KAPPA_1E5                                    # known floor at kappa = 1e5
     for k in range(it + 1):
         if ref.err[k] > 2.0:                                         # 100 x the SPLIT16 floor of ||R||_F (~2e-2 here)
             assert err[k] == pytest.approx(ref.err[k], rel=2e-3)
@@ -1065,7 +1261,7 @@ def test_config4_full_size_n8192_bench_workload():
     b = zb()
     w = W.config4(n=8192, device=DEV)
     refs = {}
-    for mode, tol in (("f64", 1e-11), ("split16", 5e-3)):
+    for mode, tol in (("f64", 1e-11), ("split16", FLOOR_KAPPA_1E5)):
         Z, it, err, fl, _, launches = gpu_refine(w, mode, 20, b.ZFAC_STOP_PAPER)
         if it not in refs:
             refs[it] = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
@@ -1086,11 +1282,28 @@ def test_config4_full_size_n8192_bench_workload():
             assert floor <= 0.1
             assert abs(err[0] ** 2 - ref.err[0] ** 2) <= (2.0 * floor) ** 2
             assert err[0] >= ref.err[0] * (1.0 - 2e-3)               # noise can only add
+    # ---- the one-pass a4 on THIS workload: Err[0] = 0.097 is below the bound 0.1, so the headline's a4 runs
+    # the (h)(h) pass only.  Control: three passes (Eq. 32 as printed, ZFAC_OPT_HH_SQUARE = 0).  Same stop index, and Z
+    # must not move by more than 1e-6 relative (measured: see the print) -- else the bound does not hold at kappa = 1e5.
+    Z1, it1, err1, _, _, _ = gpu_refine(w, "split16", 20, b.ZFAC_STOP_PAPER)
+    Z3, it3, err3, _, _, _ = gpu_refine(w, "split16", 20, b.ZFAC_STOP_PAPER, options={"hh_square": 0})
+    moved = _rel(Z1, Z3)
+    r1, r3 = _rel(Z1, refs[it1].Z), _rel(Z3, refs[it3].Z) if it3 in refs else float("nan")
+    print(f"[config4 N=8192 split16] one-pass a4 vs three passes: Z moves by {moved:.3e} relative; rel vs oracle {r1:.3e} / {r3:.3e}; "
+          f"Err {np.array2string(err1, precision=5)} / {np.array2string(err3, precision=5)}")
+    assert err1[0] <= 0.1 and it1 == it3
+    assert moved <= 1e-6
+    # ---- the GATE (1e-5) on the path that can meet it at kappa = 1e5: SPLIT16 to its stop + the refinement step of Alg. 3
     S, Z0 = _to_dev(w.S, "split16"), _to_dev(w.Z0, "split16")
     with b.Zfac(w.n, "split16", DEV) as zl, b.Zfac(w.n, "f64", DEV) as zh:
         Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=20, refi_steps=2, final_check=True)
     Z = Z.cpu().numpy()
     inv = O.final_residual_per_sqrt_n(w.S, Z)
-    print(f"[config4 N=8192 split16+refi] iters={it} Err={np.array2string(err, precision=3)} ||Z^T S Z - I||_F/sqrtN={inv:.3e}")
+    if it not in refs:
+        refs[it] = O.refine(w.S, w.Z0, it, O.STOP_FIXED)                 # the FP64 oracle, same total number of updates
+    rel = _rel(Z, refs[it].Z)
+    print(f"[config4 N=8192 split16+refi] iters={it} Err={np.array2string(err, precision=3)} ||Z^T S Z - I||_F/sqrtN={inv:.3e} "
+          f"rel vs oracle ({it} updates)={rel:.3e}")
     assert (fl & b.ZFAC_R_REFINED) and inv < 1e-10
+    assert rel <= TOL["split16"]                                         # north_star's split gate, met
     assert err[-1] == pytest.approx(inv * math.sqrt(w.n), rel=1e-2, abs=1e-10)
