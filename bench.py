@@ -683,24 +683,28 @@ def run_ours(args):
             cb = extra.get("cublas_tflops", {}).get("bf16")
             roof["frac_of_cublas_bf16_same_run"] = (ach / cb) if cb else None
 
-    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0 at N = 1 only
+    # ---- CPU baseline: the oracle as it stands, rank 0 at N = 1 only.  Its first update step (R0, Err[0], Z1, R1, Err[1]) was
+    # timed while the oracle's iterates were computed for the parity figures (same functions, same inputs, nothing tuned).
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import zfac_oracle as O
-        ns = min(n, args.cpu_sample_n)
-        S = np.ascontiguousarray(w.S[:ns, :ns]); Z0 = np.ascontiguousarray(w.Z0[:ns, :ns])
-        t0 = time.perf_counter()
-        O.refine(S, Z0, 1, O.STOP_FIXED)          # R0, Err[0], one update, R1, Err[1]: (4 + 8) N^3 flop
-        dt = time.perf_counter() - t0
         cores = os.cpu_count()
         try:
             from threadpoolctl import threadpool_info
             cores = max([i.get("num_threads", 1) for i in threadpool_info()] or [cores])
         except Exception:
             pass
+        if ora is not None:
+            ns, dt = n, ora["t_first"]
+        else:                                                 # --quick: no parity run; time the same sample here
+            ns = min(n, args.cpu_sample_n)
+            S = np.ascontiguousarray(w.S[:ns, :ns]); Z0 = np.ascontiguousarray(w.Z0[:ns, :ns])
+            t0 = time.perf_counter()
+            O.refine(S, Z0, 1, O.STOP_FIXED)
+            dt = time.perf_counter() - t0
         cpu = {"value": flops_fp32_equiv(ns, 1) / dt / 1e12, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"oracle Alg. 2 with one update (R0, Err[0], Z1, R1, Err[1]) on the leading {ns}x{ns} block "
-                         f"of the workload (12*{ns}^3 flop, {dt:.1f} s)"}
+               "sample": f"oracle Alg. 2 with one update (R0, Err[0], Z1, R1, Err[1]) on the {ns}x{ns} workload "
+                         f"(12*{ns}^3 flop, {dt:.1f} s)"}
 
     if rank == 0:
         line = {
@@ -715,6 +719,13 @@ def run_ours(args):
             "iters": iters, "iters_per_s": primary["iters_per_s"] * world, "time_to_converged_ms": t_ms,
             "err_history": primary["err"], "flags": primary["flags"],
             "final_residual_per_sqrt_n": primary.get("final_residual_per_sqrt_n"),
+            "final_residual_evaluated_by": "oracle (FP64, CPU)" if primary.get("final_residual_per_sqrt_n") is not None else None,
+            # `value` times Alg. 2 in the primary mode as the paper prints it; whether that result meets the mode's gate on
+            # this workload is stated here, and the paths that DO meet the gates are timed under `time_to_gate`
+            "gate": GATES[args.mode], "rel_vs_oracle": (parity.get(args.mode) or {}).get("rel_vs_oracle"),
+            "gate_met": (parity.get(args.mode) or {}).get("meets_gate"),
+            "time_to_gate": time_to_gate, "parity": parity or None,
+            "iteration_rate": extra.get("iteration_rate"), "sustained": sustained,
             "clocks": primary["clocks"],
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": primary["h2d"],
                     "d2h_bytes_per_step": primary["d2h"]},
