@@ -128,6 +128,19 @@ def update_x_form(Z: np.ndarray, X: np.ndarray) -> np.ndarray:
     return Z @ P
 
 
+def update_mixed(Z: np.ndarray, R: np.ndarray, update_dtype) -> np.ndarray:
+    """Z_{n+1} = Z_n + D with the correction D = Z_n (1/2 R + 3/8 R R) (Eq. 16 form of Eq. 13, m = 2) evaluated
+    in `update_dtype` from the operands rounded to it, and ADDED to the master Z in Z's own precision.  This is
+    step 3 of Sec. IV.B (PAPER.md:314-316) when only the residual of step 2 is recomputed in the enhanced
+    precision: D is a correction of relative size ||R||, so its rounding error u_update ||R|| is what is left
+    of the update in the next residual (DESIGN.md reading Q-R2)."""
+    Ru = np.asarray(R, dtype=update_dtype)
+    Zu = np.asarray(Z, dtype=update_dtype)
+    Q = 0.5 * Ru + 0.375 * (Ru @ Ru)
+    D = Zu @ Q
+    return Z + np.asarray(D, dtype=Z.dtype)
+
+
 def order_coefficients(m: int) -> list:
     """c_0..c_m of p(R) = sum c_k R^k, the degree-m Taylor polynomial of (1 - R)^{-1/2}:
     c_k = C(2k, k) / 4^k  (the vanishing-order condition of PAPER.md:121-123; reading Q18)."""
@@ -150,17 +163,21 @@ def update_order_m(Z: np.ndarray, R: np.ndarray, m: int) -> np.ndarray:
 
 
 def refine(S: np.ndarray, Z0: np.ndarray, max_iter: int, stop: int = STOP_PAPER,
-           form: str = "delta", dtype=np.float64, order: int = 2) -> RefineResult:
+           form: str = "delta", dtype=np.float64, order: int = 2, update_dtype=None) -> RefineResult:
     """Algorithm 2.  `dtype` exists only so that the paper's
     `single` scheme (Table I) can be emulated in a pin; the oracle
     proper is FP64.  `order` = m of Eq. 13 (2 = the paper's tests; 3, 4 = SURVEY.md §8(f3));
-    the stop test uses the exponent nu_max = m + 1 (Eq. 38)."""
+    the stop test uses the exponent nu_max = m + 1 (Eq. 38).
+    `update_dtype` (m = 2 only): the correction of every update is evaluated in that precision and added to the
+    `dtype` master (`update_mixed`): Alg. 2 with the enhanced-precision residual of Sec. IV.B in EVERY iteration."""
     if max_iter < 0:
         raise ValueError("max_iter must be >= 0")
     if order < 2 or order > 4:
         raise ValueError("order must be 2, 3 or 4")
     if order != 2 and form != "delta":
         raise ValueError("the X-form is printed for m = 2 only (PAPER.md:303, :451)")
+    if update_dtype is not None and (order != 2 or form != "delta"):
+        raise ValueError("the mixed update is defined for m = 2 in the delta form")
     S = np.asarray(S, dtype=dtype)
     Z = np.array(Z0, dtype=dtype, copy=True)
     n = S.shape[0]
@@ -184,6 +201,8 @@ def refine(S: np.ndarray, Z0: np.ndarray, max_iter: int, stop: int = STOP_PAPER,
         it += 1
         if order != 2:
             Z = update_order_m(Z, R, order)
+        elif update_dtype is not None:
+            Z = update_mixed(Z, R, update_dtype)
         elif form == "delta":
             Z = update_delta_form(Z, R)
         elif form == "x":
@@ -229,19 +248,6 @@ def spectral_closed_form(lam: np.ndarray, alpha: float, iters: int, order: int =
             q = q + c[k] * rk
         z = z + z * q
     return SpectralResult(z, np.asarray(err, dtype=np.float64))
-
-
-def update_mixed(Z: np.ndarray, R: np.ndarray, update_dtype) -> np.ndarray:
-    """Z_{n+1} = Z_n + D with the correction D = Z_n (1/2 R + 3/8 R R) (Eq. 16 form of Eq. 13, m = 2) evaluated
-    in `update_dtype` from the operands rounded to it, and ADDED to the master Z in Z's own precision.  This is
-    step 3 of Sec. IV.B (PAPER.md:314-316) when only the residual of step 2 is recomputed in the enhanced
-    precision: D is a correction of relative size ||R||, so its rounding error u_update ||R|| is what is left
-    of the update in the next residual (DESIGN.md reading Q-R2)."""
-    Ru = np.asarray(R, dtype=update_dtype)
-    Zu = np.asarray(Z, dtype=update_dtype)
-    Q = 0.5 * Ru + 0.375 * (Ru @ Ru)
-    D = Zu @ Q
-    return Z + np.asarray(D, dtype=Z.dtype)
 
 
 def refine_with_refi(S: np.ndarray, Z0: np.ndarray, max_iter: int, low_dtype=np.float32,

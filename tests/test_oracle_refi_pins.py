@@ -127,3 +127,26 @@ def test_mixed_update_leaves_u_times_r_and_two_steps_reach_the_fp64_floor():
     k = mixed.iters - 2
     assert mixed.err[k + 1] == full.err[k + 1]
     assert mixed.err[k + 2] < 1e-4 * mixed.err[k + 1]
+
+
+def test_alg2_with_mixed_update_converges_to_the_fp64_floor_one_iteration_late_at_most():
+    """`refine(..., update_dtype=float32)`: FP64 residual, float32 correction, in every iteration of Alg. 2.  The
+    rounding of the correction leaves u ||R_n|| behind (pinned above), which is below the cubic term until
+    ||R_n||^2 ~ u: the run tracks the FP64 run entry by entry down to Err ~ 1e-4, reaches the FP64 floor, and needs
+    at most one update more.  A float32 MASTER (dtype = float32) stalls ~1e5 higher."""
+    w = W.random_spd_general(40, 31, kappa=1e3, pert=0.1, fp32_stored=True)
+    full = O.refine(w.S, w.Z0, 40, O.STOP_PAPER)
+    mixed = O.refine(w.S, w.Z0, 40, O.STOP_PAPER, update_dtype=np.float32)
+    single = O.refine(w.S, w.Z0, 40, O.STOP_PAPER, dtype=np.float32)
+    assert full.iters <= mixed.iters <= full.iters + 1
+    for k in range(min(full.iters, mixed.iters)):
+        if full.err[k] > 1e-4:
+            assert mixed.err[k] == pytest.approx(full.err[k], rel=1e-4)
+    fm, ff, fs = (_fro_residual(w.S, r.Z) / math.sqrt(w.n) for r in (mixed, full, single))
+    assert fm < 1e-12 and ff < 1e-12 and fs > 1e3 * fm
+    same = O.refine(w.S, w.Z0, 40, O.STOP_PAPER, update_dtype=np.float64)
+    assert same.iters == full.iters and np.array_equal(same.Z, full.Z) and np.array_equal(same.err, full.err)
+    # both are the inverse factor reached from the same start: the rotation the float32 correction adds is ~u ||R_0||
+    assert np.linalg.norm(mixed.Z - full.Z) / np.linalg.norm(full.Z) < 1e-6
+    with pytest.raises(ValueError):
+        O.refine(w.S, w.Z0, 5, order=3, update_dtype=np.float32)
