@@ -54,8 +54,20 @@ typedef struct zfac_ctx zfac_ctx; /* opaque */
  *           the refinement step (zfac_refine_refi).
  * Note on SPLIT16: the second-order product of step a4 (R R in Q = 1/2 R + 3/8 R R) runs its (h)(h) pass only when
  * the update is taken from Err[n] <= ZFAC_OPT_HH_SQUARE_ERR (default 0.1; decided on the device from the Err[n] just
- * computed); every other product always runs all three passes (ZFAC_OPT_HH_SQUARE = 0 disables it). */
-typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2, ZFAC_MODE_HH16 = 3 } zfac_mode;
+ * computed); every other product always runs all three passes (ZFAC_OPT_HH_SQUARE = 0 disables it).
+ *  F64_MIXED, F64_I8: FP64-master modes built for the refinement stage of Alg. 3 but complete modes of
+ *           their own (element type double).  What needs FP64-level accuracy in an iteration is the RESIDUAL
+ *           R = I - Z^T (S Z); the update Z + Z (1/2 R + 3/8 R R) is a correction of relative size ||R||, evaluated here
+ *           with the SPLIT16 tensor-core passes on the FP32 parts of Z and R and ADDED to the FP64 master (its rounding
+ *           leaves ~2^-22 ||R|| in the next residual; oracle: update_mixed).  The residual is computed
+ *             F64_MIXED: on the FP64 tensor pipe (the kernels of ZFAC_MODE_F64);
+ *             F64_I8   : on the INT8 tensor cores -- each FP64 operand row is cut, error-free, into ZFAC_OPT_I8_SLICES
+ *                        int8 slices of 7 bits under one exponent per row, all slice products with i + j < slices are
+ *                        accumulated exactly in INT32 and summed in FP64 (Ozaki scheme): ~2^(-7 slices) relative to the
+ *                        row maxima, i.e. FP64-equivalent for 8 slices.  n <= 32768.
+ *           Order m = 2 only; zfac_congruence is not available in these two modes. */
+typedef enum { ZFAC_MODE_SPLIT16 = 0, ZFAC_MODE_TF32 = 1, ZFAC_MODE_F64 = 2, ZFAC_MODE_HH16 = 3,
+               ZFAC_MODE_F64_MIXED = 4, ZFAC_MODE_F64_I8 = 5 } zfac_mode;
 
 /* Stop rule.  PAPER: Alg. 2's parameter-free test.  FIXED: perform exactly max_iter updates
  * (benchmarks, and parity against the oracle "for the same number of iterations"). */
@@ -127,9 +139,9 @@ zfac_status zfac_refine(zfac_ctx* ctx, const void* d_S, int64_t lds, const void*
  *      from `low`'s workspace, and R = I - Z^T S Z is recomputed there (S converted exactly);
  *   3. `refi_steps` updates Z <- Z + Z (1/2 R + 3/8 R R) in `high`'s arithmetic (1 <= refi_steps <= 4000; the paper uses 1).
  * Allowed pairs (low -> high): HH16 -> SPLIT16, TF32 -> SPLIT16 (the paper's single-precision refinement,
- * SPLIT16 is this library's FP32-class arithmetic), and HH16 / TF32 / SPLIT16 -> F64
- * (PAPER.md:392-394).  `high` has the same n and order and its own workspace.  d_Z is n x n of `high`'s element
- * type (float for SPLIT16, double for F64).
+ * SPLIT16 is this library's FP32-class arithmetic), and HH16 / TF32 / SPLIT16 -> F64,
+ * F64_MIXED or F64_I8 (double-precision refinement).  `high` has the same n and order and its own workspace.  d_Z is n x n of `high`'s element
+ * type (float for SPLIT16, double for F64 / F64_MIXED / F64_I8).
  * With final_check != 0 the residual of the returned Z is evaluated in `high` as well (two more GEMMs); Alg. 3 as
  * printed stops after the update (final_check = 0).
  *   d_iters [out] low-precision updates + refinement updates performed
@@ -214,7 +226,7 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
 /* Per-context options (host-side state only: no device work; take effect from the next call on `ctx`).  They
  * replace every environment variable earlier versions read.  Values are passed as double; integer options are
  * rounded.  Unknown key or out-of-range value -> ZFAC_E_INVALID, the option keeps its value.
- *   The first six change which arithmetic is performed (hence results, within the mode's accuracy):           default
+ *   The first group changes which arithmetic is performed (hence results, within the mode's accuracy):           default
  *   ZFAC_OPT_CHUNK_KB        SPLIT16, a1 / a2: k-blocks (64 products each) of (h)(h) products that are summed in the
  *                            tensor core's truncating FP32 accumulator before they are added, with round-to-nearest,
  *                            to FP32 registers ("promoted accumulation"); 1 .. 1024                    1
@@ -223,6 +235,7 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *                            taken from Err[n] <= HH_SQUARE_ERR; 0 = always three passes (Eq. 32 as printed)        1
  *   ZFAC_OPT_HH_SQUARE_ERR   the bound, >= 0                                                                       0.1
  *   ZFAC_OPT_PROMOTE_UPDATE  SPLIT16: promoted accumulation in the update GEMMs (p2, a4, a5) as well; 0 / 1          0
+ *   ZFAC_OPT_I8_SLICES       F64_I8: int8 slices per operand row = orders i + j kept, 2 .. 8 (7 bits each)              8
  *   The rest change scheduling only (bit-identical results):
  *   ZFAC_OPT_BAND            full GEMMs: tile columns per rasterisation band, 1 .. 4096                               8
  *   ZFAC_OPT_MAX_PAIRS       tensor-core modes: use at most this many CTA pairs; 0 = all co-resident ones            0
@@ -230,7 +243,7 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
 typedef enum {
   ZFAC_OPT_CHUNK_KB = 0, ZFAC_OPT_CHUNK0_KB = 1, ZFAC_OPT_HH_SQUARE = 2, ZFAC_OPT_HH_SQUARE_ERR = 3,
   ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
-  ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9
+  ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10
 } zfac_option;
 zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
 zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);
@@ -238,7 +251,7 @@ zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value)
 /* Order m of the refinement polynomial, Z_{n+1} = Z_n sum_{k=0..m} c_k R_n^k  (Eq. 13 / Eq. 16:
  * "Reference 1 gives a table with the coefficients a_k for polynomials of order m = 2, 3, 4, 5. For the tests in
  * this article, we use m = 2").  m = 2 (default; the paper's scheme), 3 or 4; anything else -> ZFAC_E_INVALID and
- * the context keeps its order.  The coefficients follow from the paper's condition that the error terms vanish to
+ * the context keeps its order (F64_MIXED / F64_I8: m = 2 only).  The coefficients follow from the paper's condition that the error terms vanish to
  * the highest possible order: c_k = C(2k,k)/4^k = 1, 1/2, 3/8, 5/16, 35/128, and the stop test
  * becomes Err[n] > Err[n-1]^(m+1) (nu_max = m + 1; Eq. 38).  For m > 2 step a4 is two symmetric
  * GEMMs, P = R R and Q = 1/2 R + P G with G = 3/8 I + 5/16 R (+ 35/128 P for m = 4), i.e. five kernels per

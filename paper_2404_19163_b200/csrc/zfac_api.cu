@@ -12,6 +12,7 @@
 #include "zfac_f64.cuh"
 #include "zfac_umma.cuh"
 #include "zfac_f64_tma.cuh"
+#include "zfac_mix.cuh"
 
 using namespace zfac;
 
@@ -40,6 +41,7 @@ struct zfac_ctx {
   int order;       // m of Eq. 13 (zfac_set_order): 2 (default), 3, 4
   UmmaPlan umma;   // tensor maps + launch geometry for the tcgen05 modes
   F64Plan f64p;    // tensor maps of the FP64 buffers (ZFAC_MODE_F64)
+  MixPlan mix;     // FP64-master modes (ZFAC_MODE_F64_MIXED, ZFAC_MODE_F64_I8)
   cudaStream_t side = nullptr;                 // zfac_refine_host: stream of the chunked upload and the early download (lazy)
   cudaEvent_t ev_a5 = nullptr, ev_copy = nullptr;
   static constexpr int UP_CHUNKS = 8;            // zfac_refine_host: S is uploaded in at most this many row chunks
@@ -48,20 +50,22 @@ struct zfac_ctx {
 };
 
 static bool valid_mode(int m) {
-  return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_F64 || m == ZFAC_MODE_HH16;
+  return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_F64 || m == ZFAC_MODE_HH16 ||
+         m == ZFAC_MODE_F64_MIXED || m == ZFAC_MODE_F64_I8;
 }
+static bool mode_is_umma(int m) { return m == ZFAC_MODE_SPLIT16 || m == ZFAC_MODE_TF32 || m == ZFAC_MODE_HH16; }
 // The context is bound to the device that was current at zfac_create (workspace, tensor maps, lazily created streams).
 static bool on_own_device(const zfac_ctx* c) {
   int dev = -1;
   return cudaGetDevice(&dev) == cudaSuccess && dev == c->dev;
 }
 // precision rank of a mode for Alg. 3 ("enhanced precision"): one 11-bit pass < FP32-class split < FP64
-static int mode_rank(int m) { return m == ZFAC_MODE_F64 ? 2 : (m == ZFAC_MODE_SPLIT16 ? 1 : 0); }
+static int mode_rank(int m) { return mode_is_f64_elt(m) ? 2 : (m == ZFAC_MODE_SPLIT16 ? 1 : 0); }
 
 extern "C" {
 
 size_t zfac_workspace_bytes(int64_t n, zfac_mode mode) {
-  if (n <= 0 || n > (1 << 20) || !valid_mode(mode)) return 0;
+  if (n <= 0 || n > (1 << 20) || !valid_mode(mode) || (mode == ZFAC_MODE_F64_I8 && n > 32768)) return 0;
   return make_layout(n, mode).total;
 }
 
@@ -87,6 +91,7 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   if (!out) return ZFAC_E_INVALID;
   *out = nullptr;
   if (n <= 0 || n > (1 << 20) || !valid_mode(mode)) return ZFAC_E_INVALID;
+  if (mode == ZFAC_MODE_F64_I8 && n > 32768) return ZFAC_E_INVALID;      // INT32 accumulation: 8 slice pairs x 2^12 x K < 2^31
   Layout L = make_layout(n, mode);
   if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || bytes < L.total) return ZFAC_E_WORKSPACE;
   int dev = 0, major = 0, sms = 0;
@@ -108,6 +113,13 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
     if (e == cudaSuccess) e = f64_tma_prepare<EPI_P2>();
     if (e != cudaSuccess) {
       snprintf(g_cuda_err, sizeof(g_cuda_err), "f64_plan_create: %s", cudaGetErrorString(e));
+      delete c;
+      return ZFAC_E_CUDA;
+    }
+  } else if (mode_is_mix(mode)) {
+    cudaError_t e = mix_plan_create(&c->mix, L, c->ws, sms, &c->opt);
+    if (e != cudaSuccess) {
+      snprintf(g_cuda_err, sizeof(g_cuda_err), "mix_plan_create: %s", cudaGetErrorString(e));
       delete c;
       return ZFAC_E_CUDA;
     }
@@ -177,7 +189,7 @@ int zfac_get_profile(zfac_ctx* c, int* tags, float* ms, int cap) {
 int zfac_last_launch_count(const zfac_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 zfac_status zfac_set_order(zfac_ctx* c, int m) {
-  if (!c || m < 2 || m > 4) return ZFAC_E_INVALID;
+  if (!c || m < 2 || m > 4 || (mode_is_mix(c->mode) && m != 2)) return ZFAC_E_INVALID;
   c->order = m;
   return ZFAC_OK;
 }
@@ -199,6 +211,7 @@ zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
     case ZFAC_OPT_HOST_OVERLAP: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.host_overlap = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_HOST_UPLOAD_OVERLAP: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.host_upload_overlap = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_HOST_A5_BANDS: if (iv < 1 || iv > 64) return ZFAC_E_INVALID; o.host_a5_bands = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_I8_SLICES: if (iv < 2 || iv > I8_MAX_SLICES) return ZFAC_E_INVALID; o.i8_slices = (int)iv; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }
@@ -217,6 +230,7 @@ zfac_status zfac_get_option(const zfac_ctx* c, zfac_option key, double* v) {
     case ZFAC_OPT_HOST_OVERLAP: *v = o.host_overlap; return ZFAC_OK;
     case ZFAC_OPT_HOST_UPLOAD_OVERLAP: *v = o.host_upload_overlap; return ZFAC_OK;
     case ZFAC_OPT_HOST_A5_BANDS: *v = o.host_a5_bands; return ZFAC_OK;
+    case ZFAC_OPT_I8_SLICES: *v = o.i8_slices; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }
@@ -296,6 +310,23 @@ static zfac_status refine_f64(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   return ZFAC_OK;
 }
 
+// FP64-master modes: same loop, MixSeq's halves.
+static zfac_status refine_mix(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s, bool skip_last,
+                              const IterHook* hook) {
+  MixSeq q(c->mix, max_iter, (int)stop, d_err, 0ull);
+  for (int n = 0; n <= max_iter; ++n) {
+    if (n == max_iter && skip_last) break;
+    q.residual(n, n, s, &c->prof);
+    if (n == max_iter) break;
+    q.update(n & 1, n, n, s, &c->prof);
+    if (hook && hook->after_a5) hook->after_a5(hook->self, n, s);
+  }
+  c->prof.mark(s, 0);
+  c->launches += q.nl;
+  ZF_CUDA(cudaGetLastError());
+  return ZFAC_OK;
+}
+
 // Step a0: copy S and Z0 (element type float if in_f32, else the mode's own) into the padded buffers.
 // what: 1 = S only, 2 = Z0 (W, State reset) only, 3 = both; tile rows [ty0, ty0 + tyn) of CI_TR rows each (tyn = 0: all).
 // First operation of every call: clears State::range (set by any CTA of the copy-in and of the a1 / a5 kernels when an fp16
@@ -317,6 +348,27 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
   ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
   ci.what = what; ci.ty0 = ty0;
   dim3 gi((unsigned)(L.np / CI_TC), (unsigned)(tyn > 0 ? tyn : L.np / CI_TR)), bi(256);
+  if (mode_is_mix(c->mode)) {
+    // FP64 master Z (+ S, W in FP64 for the DMMA engine), then the FP32 operand pair of Z; I8 engine: int8 slices of S and W
+    const bool i8 = (c->mode == ZFAC_MODE_F64_I8);
+    ci.what = i8 ? (2 | 4) : 3;
+    if (in_f32) copy_in_kernel<ZFAC_MODE_F64, float><<<gi, bi, 0, s>>>(ci);
+    else copy_in_kernel<ZFAC_MODE_F64, double><<<gi, bi, 0, s>>>(ci);
+    const size_t np2 = (size_t)L.np * (size_t)L.np;
+    z_planes_kernel<<<(unsigned)((np2 / 8 + 255) / 256), 256, 0, s>>>(reinterpret_cast<const double*>(ws + L.off_Z[0]),
+                                                                    reinterpret_cast<__half*>(ws + L.off_Zb[0]), np2, ci.st);
+    c->launches += 2;
+    if (i8) {
+      int* eS = reinterpret_cast<int*>(ws + L.off_exp);
+      int8_t* S8 = reinterpret_cast<int8_t*>(ws + L.off_S8);
+      if (in_f32) slice_rows_kernel<float><<<(unsigned)L.np, 256, 0, s>>>(static_cast<const float*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
+      else slice_rows_kernel<double><<<(unsigned)L.np, 256, 0, s>>>(static_cast<const double*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
+      MixSeq q(c->mix, 0, 0, nullptr, 0ull);
+      q.w_slices(s);
+      c->launches += 1 + q.nl;
+    }
+    return;
+  }
   switch (c->mode) {
     case ZFAC_MODE_F64:
       if (in_f32) copy_in_kernel<ZFAC_MODE_F64, float><<<gi, bi, 0, s>>>(ci);
@@ -350,7 +402,7 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
     copy_out_vec16_kernel<<<gv, 256, 0, s>>>(co, elt);
   } else {
     dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
-    if (c->mode == ZFAC_MODE_F64) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
+    if (mode_is_f64_elt(c->mode)) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
     else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
   }
   c->launches += 1;
@@ -360,6 +412,7 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
 static zfac_status run_iterations(zfac_ctx* c, int max_iter, zfac_stop stop, double* d_err, cudaStream_t s, bool skip_last,
                                   const IterHook* hook) {
   if (c->mode == ZFAC_MODE_F64) return refine_f64(c, max_iter, stop, d_err, s, skip_last, hook);
+  if (mode_is_mix(c->mode)) return refine_mix(c, max_iter, stop, d_err, s, skip_last, hook);
   int nl = 0;
   cudaError_t e = umma_refine(c->umma, max_iter, (int)stop, c->order, d_err, s, &nl, &c->prof, hook, skip_last);
   c->launches += nl;
@@ -510,7 +563,7 @@ zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* high, const void* d_S, int
 zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const void* d_Z, int64_t ldz, void* d_out,
                             int64_t ldo, void* stream) {
   if (!c || !d_H || !d_Z || !d_out) return ZFAC_E_INVALID;
-  if (ldh < c->n || ldz < c->n || ldo < c->n || !on_own_device(c)) return ZFAC_E_INVALID;
+  if (ldh < c->n || ldz < c->n || ldo < c->n || !on_own_device(c) || mode_is_mix(c->mode)) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;
@@ -552,7 +605,7 @@ static zfac_status host_upload(zfac_ctx* c, const void* h_S, int64_t lds, const 
   char* dZ = c->ws + L.off_stage_Z;
   const size_t row = (size_t)c->n * L.elt;
   int chunks = 0;
-  if (c->mode != ZFAC_MODE_F64 && L.np / UM_MACRO >= 4 && c->opt.host_upload_overlap) {
+  if (mode_is_umma(c->mode) && L.np / UM_MACRO >= 4 && c->opt.host_upload_overlap) {
     cudaPointerAttributes pS{}, pZ{};
     if (cudaPointerGetAttributes(&pS, h_S) == cudaSuccess && pS.type == cudaMemoryTypeHost &&
         cudaPointerGetAttributes(&pZ, h_Z0) == cudaSuccess && pZ.type == cudaMemoryTypeHost) {
@@ -626,7 +679,7 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   ho.dS = dS; ho.chunks = chunks;
   IterHook hook{z_dev ? host_after_a5 : nullptr, &ho};
   if (chunks > 0) hook.first_a1 = host_first_a1;
-  if (z_dev && c->mode != ZFAC_MODE_F64 && L.np / UM_MACRO >= 4) {
+  if (z_dev && mode_is_umma(c->mode) && L.np / UM_MACRO >= 4) {
     hook.a5_bands = c->opt.host_a5_bands;
     if (hook.a5_bands > (int)(L.np / UM_MACRO)) hook.a5_bands = (int)(L.np / UM_MACRO);
     hook.after_a5_band = host_after_a5_band;
@@ -675,7 +728,7 @@ zfac_status zfac_refine_refi_host(zfac_ctx* low, zfac_ctx* high, const void* h_S
                                   int64_t ldz0, void* h_Z, int64_t ldz, int max_iter, int refi_steps, int final_check,
                                   int* h_iters, double* h_err, int* h_flags, void* stream) {
   if (!low || !high || !h_S || !h_Z0 || !h_Z || !h_iters || !h_err || !h_flags) return ZFAC_E_INVALID;
-  if (low->mode == ZFAC_MODE_F64 || low->n != high->n) return ZFAC_E_INVALID;
+  if (!mode_is_umma(low->mode) || low->n != high->n) return ZFAC_E_INVALID;
   if (lds < low->n || ldz0 < low->n || ldz < low->n || max_iter < 0 || refi_steps < 1 || max_iter + refi_steps + 2 > 4096)
     return ZFAC_E_INVALID;
   if (!on_own_device(low) || low->dev != high->dev) return ZFAC_E_INVALID;
@@ -784,6 +837,10 @@ zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const v
       F64Seq q(c, max_iter, stop, d_err, (unsigned long long)h);
       q.residual(0, 0, cs, nullptr);
       if ((ok = splice_loop())) enqueue_loop_body(q, bs);
+    } else if (mode_is_mix(c->mode)) {
+      MixSeq q(c->mix, max_iter, (int)stop, d_err, (unsigned long long)h);
+      q.residual(0, 0, cs, nullptr);
+      if ((ok = splice_loop())) enqueue_loop_body(q, bs);
     } else {
       UmmaSeq q(c->umma, max_iter, (int)stop, c->order, d_err, (unsigned long long)h);
       q.residual(0, 0, cs, nullptr);
@@ -832,7 +889,17 @@ zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void
   State hst{};
   ZF_CUDA(cudaStreamSynchronize(s));
   ZF_CUDA(cudaMemcpy(&hst, ws + L.off_state, sizeof(State), cudaMemcpyDeviceToHost));
-  if (c->mode == ZFAC_MODE_F64 || c->mode == ZFAC_MODE_TF32) {
+  if (mode_is_mix(c->mode)) {
+    switch (which) {
+      case ZFAC_BUF_T: peek_kernel<double, 0><<<g, 256, 0, s>>>(ws + L.off_T, d_out, ld, n, np); break;
+      case ZFAC_BUF_R:
+        if (c->mode == ZFAC_MODE_F64_MIXED) peek_kernel<double, 0><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np);
+        else peek_kernel<double, 4><<<g, 256, 0, s>>>(ws + L.off_R, d_out, ld, n, np);
+        break;
+      case ZFAC_BUF_Z: peek_kernel<double, 0><<<g, 256, 0, s>>>(ws + L.off_Z[0], d_out, ld, n, np); break;
+      default: return ZFAC_E_INVALID;               // Q exists only as the scaled operand pair in these modes
+    }
+  } else if (c->mode == ZFAC_MODE_F64 || c->mode == ZFAC_MODE_TF32) {
     size_t off;
     switch (which) {
       case ZFAC_BUF_T: off = L.off_T; break;

@@ -14,9 +14,13 @@ struct State {
   int flags;                 // ZFAC_R_* bits
   int pad0;
   unsigned int arrive[4];    // last-CTA counters (one per use site), self-resetting
-  int range;                 // != 0: a value of magnitude >= 65504 was clamped on its way into an fp16 operand (16-bit modes);
+  int range;                 // bit 0: a value of magnitude >= 65504 was clamped on its way into an fp16 operand (16-bit modes;
+                             // bit 1: F64_I8 met a non-finite operand while slicing -> the next Err is NaN);
                              // cleared by a memset node BEFORE the copy-in of a call (every CTA of the copy-in may set it),
                              // merged into the published flags as ZFAC_R_RANGE
+  // FP64-master modes (zfac_mix.cuh): R is handed to the FP32-class update GEMMs scaled by a power of two, R~ = rscale R,
+  // chosen from ||R||_F by r_split_kernel so that the fp16 operand pairs of R~ and Q~ neither overflow nor underflow
+  float rscale, rinv;        // rscale and 1 / rscale
   int pad1;
 };
 constexpr float H16_MAX = 65504.0f;   // largest finite fp16: cvt.rn.satfinite clamps beyond it
@@ -33,6 +37,7 @@ struct Options {
   int host_overlap = 1;      // zfac_refine_host: early download of Z after the first update
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
+  int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
 };
 
 struct StopArgs {

@@ -19,7 +19,8 @@ constexpr int F64_BM = 128, F64_BN = 128, F64_BK = 16;   // CTA tile; 8 warps x 
 constexpr int F64_THREADS = 256;
 
 enum { EPI_A1 = 1, EPI_A2 = 2, EPI_X3 = 3 /* X = Z^T H Z itself (congruence, Eq. 11) */, EPI_A4 = 4, EPI_A5 = 5,
-       EPI_P2 = 6 /* order m > 2: P = R R and G = 3/8 I + 5/16 R (+ 35/128 P), both mirrored */ };
+       EPI_P2 = 6 /* order m > 2: P = R R and G = 3/8 I + 5/16 R (+ 35/128 P), both mirrored */,
+       EPI_A5X = 7 /* FP64-master modes: Z64 += (Z Q~) / rscale, next FP32 operand pair of Z, optional W64 = Z^T */ };
 
 // Polynomial coefficients of step a4 (Eq. 13 / 16 with order m; c_k = C(2k,k)/4^k, zfac.h):
 //   m = 2:  Q = 1/2 R + 3/8 (R R)                                   one symmetric GEMM   (EPI_A4, q_d = 3/8)

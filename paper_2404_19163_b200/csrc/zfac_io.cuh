@@ -56,16 +56,21 @@ struct Layout {
   // SPLIT16 / HH16: S, W, T, Rb, Qb, Zb[2] are fp16 [planes][Np][Np] (planes = 2: hi, lo'; HH16: 1);
   // R and the master Z (= off_Z[0]) are fp32
   size_t off_Rb = 0, off_Qb = 0, off_Zb[2] = {0, 0};
+  // FP64-master modes (zfac_mix.cuh): S, W, T (F64_MIXED), Z in FP64; R in FP64 (F64_MIXED) or FP32 (F64_I8) at off_R;
+  // R~ (FP32) at off_R32; fp16 pairs Rb, Qb, Zb[2]; F64_I8: int8 slices of S, W, T, row exponents, partial-sum scratch
+  size_t off_R32 = 0, off_S8 = 0, off_W8 = 0, off_T8 = 0, off_exp = 0, off_scratch = 0;
   size_t total = 0;
 };
 
 inline int64_t padded_n(int64_t n, int mode) { return round_up(n, mode == ZFAC_MODE_F64 ? 128 : 256); }
 inline bool mode_is_h16(int mode) { return mode == ZFAC_MODE_SPLIT16 || mode == ZFAC_MODE_HH16; }
+inline bool mode_is_mix(int mode) { return mode == ZFAC_MODE_F64_MIXED || mode == ZFAC_MODE_F64_I8; }
+inline bool mode_is_f64_elt(int mode) { return mode == ZFAC_MODE_F64 || mode_is_mix(mode); }
 
 inline Layout make_layout(int64_t n, int mode) {
   Layout L;
   L.n = n; L.mode = mode; L.np = padded_n(n, mode);
-  L.elt = (mode == ZFAC_MODE_F64) ? 8 : 4;
+  L.elt = mode_is_f64_elt(mode) ? 8 : 4;
   const size_t np2 = (size_t)L.np * (size_t)L.np, n2 = (size_t)n * (size_t)n;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 1023) / 1024 * 1024; return o; };
@@ -76,7 +81,21 @@ inline Layout make_layout(int64_t n, int mode) {
   L.off_stage_S = take(n2 * L.elt);
   L.off_stage_Z = take(n2 * L.elt);
   L.off_stage_out = take((size_t)4096 * sizeof(double) + 64);
-  if (mode_is_h16(mode)) {
+  if (mode_is_mix(mode)) {
+    const size_t hb = np2 * 4;                                        // fp16 pair planes
+    L.off_T = take(np2 * 8);
+    L.off_Z[0] = take(np2 * 8); L.off_Z[1] = L.off_Z[0];              // FP64 master, updated in place
+    L.off_R32 = take(np2 * 4); L.off_Rb = take(hb); L.off_Qb = take(hb);
+    L.off_Zb[0] = take(hb); L.off_Zb[1] = take(hb);
+    if (mode == ZFAC_MODE_F64_MIXED) {
+      L.off_S = take(np2 * 8); L.off_W = take(np2 * 8); L.off_R = take(np2 * 8);
+    } else {
+      L.off_R = take(np2 * 4);
+      L.off_S8 = take(np2 * 8); L.off_W8 = take(np2 * 8); L.off_T8 = take(np2 * 8);      // 8 slices of Np^2 int8 each
+      L.off_exp = take(3 * (size_t)L.np * sizeof(int));
+      L.off_scratch = take((size_t)192 * 128 * 256 * sizeof(double));
+    }
+  } else if (mode_is_h16(mode)) {
     const size_t hb = np2 * (mode == ZFAC_MODE_SPLIT16 ? 4 : 2);     // fp16 planes: (hi, lo') or hi only
     L.off_S = take(hb); L.off_W = take(hb); L.off_T = take(hb);
     L.off_R = take(np2 * 4); L.off_Rb = take(hb); L.off_Qb = take(hb);
@@ -101,7 +120,7 @@ struct CopyInArgs {
   void* oZ;            // F64/TF32: Z[0];  SPLIT16: float Z32
   void* oW;            // F64/TF32: W;     SPLIT16: half[2][Np][Np]
   void* oZb;           // SPLIT16 / HH16: half[planes][Np][Np] (Zb[0])
-  int what;            // bit 0: S, bit 1: Z0 (and W, State reset); 0 is read as 3 (both)
+  int what;            // bit 0: S, bit 1: Z0 (and W, State reset); 0 is read as 3 (both); bit 2: no W (F64_I8: sliced later)
   int ty0;             // first tile row of this launch (grid.y counts from it): row chunks of S for zfac_refine_host
   // zfac_refine_refi: Z0 is the result of a low-precision run, taken straight from that context's workspace.
   const State* prev;   // State of the low-precision context (null: none)
@@ -157,7 +176,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
   __shared__ Tin sS[CI_TR * CI_PITCH];
   __shared__ Tin sZ[CI_TR * CI_PITCH];
   const int t = threadIdx.x;
-  const bool doS = (a.what == 0) || (a.what & 1), doZ = (a.what == 0) || (a.what & 2);
+  const bool doS = (a.what == 0) || (a.what & 1), doZ = (a.what == 0) || (a.what & 2), doW = doZ && !(a.what & 4);
   if (doZ && blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
     // refinement stage of Alg. 3 behind a low-precision run that ended non-finite: nothing to refine -- every later
     // kernel of this context exits at once (done = 1) and no Err entry exists (iters = -1)
@@ -212,7 +231,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
     }
   }
   // ---- phase 3: W = Z^T, 8 consecutive rows of one column of the tile per thread -> 8 consecutive elements of a row of W
-  if (doZ) {
+  if (doW) {
     const int wr = t >> 2, wc = (t & 3) * 8;                        // W tile: CI_TC rows x CI_TR columns
     const size_t o = (size_t)(c0 + wr) * np + (size_t)(r0 + wc);
     if (MODE == ZFAC_MODE_F64) {
@@ -245,7 +264,7 @@ __device__ __forceinline__ int updates_done(const State* st) {
   const int it = st->iters;
   return st->done ? (it > 0 ? it : 0) : it + 1;
 }
-__device__ __forceinline__ int published_flags(const State* st) { return st->flags | (st->range ? ZFAC_R_RANGE : 0); }
+__device__ __forceinline__ int published_flags(const State* st) { return st->flags | ((st->range & 1) ? ZFAC_R_RANGE : 0); }
 // `plain`: the ordinary call (every residual evaluated): the update count is State::iters itself.
 __device__ __forceinline__ void publish_and_select(const CopyOutArgs& a, bool first, const void*& src) {
   const int iters = a.st->iters;
@@ -305,13 +324,14 @@ __global__ void refi_merge_kernel(const State* hi, const double* err_hi, double*
     for (int i = 0; i < entries; ++i) d_err[k + 1 + i] = err_hi[i];
     *d_iters = k + upd;
     if (d_upd) { d_upd[0] = upd; d_upd[1] = k + 1 + entries; }     // refinement updates performed; Err entries in total
-    *d_flags |= (upd > 0 ? ZFAC_R_REFINED : 0) | (hi->flags & ZFAC_R_NONFINITE) | (hi->range ? ZFAC_R_RANGE : 0);
+    *d_flags |= (upd > 0 ? ZFAC_R_REFINED : 0) | (hi->flags & ZFAC_R_NONFINITE) | ((hi->range & 1) ? ZFAC_R_RANGE : 0);
   }
 }
 
 // ------------------------------------------------------------------ peek (tests)
 // kind 0: plain T buffer; 1: fp16 pair hi + lo' 2^-11; 2: fp16 (hi only); 3: plain T buffer of a SYMMETRIC matrix of
-// which only the upper triangle of tiles is stored (the FP32 R of the 16-bit modes): element (r, c), r > c, is (c, r)
+// which only the upper triangle of tiles is stored (the FP32 R of the 16-bit modes): element (r, c), r > c, is (c, r);
+// 4: plain FLOAT buffer read into T (the FP32 R of ZFAC_MODE_F64_I8)
 template <typename T, int KIND>
 __global__ void __launch_bounds__(256) peek_kernel(const void* src, void* out, int64_t ld, int n, int np) {
   const int c = blockIdx.x * 256 + threadIdx.x, r = blockIdx.y;
@@ -319,6 +339,7 @@ __global__ void __launch_bounds__(256) peek_kernel(const void* src, void* out, i
   const size_t o = (KIND == 3 && r > c) ? (size_t)c * np + r : (size_t)r * np + c, np2 = (size_t)np * np;
   T v;
   if (KIND == 0 || KIND == 3) v = static_cast<const T*>(src)[o];
+  else if (KIND == 4) v = (T) static_cast<const float*>(src)[o];
   else if (KIND == 1) {
     const __half* h = static_cast<const __half*>(src);
     v = (T)(__half2float(h[o]) + __half2float(h[np2 + o]) * LO_UNSCALE);

@@ -98,6 +98,9 @@ struct UmmaParams {
   double hh_err_max;    // ... and does so iff Err[n] = stop.d_err[stop.n_iter] <= hh_err_max (decided on the device)
   float q_r, q_d;       // a4: Q = q_r R + q_d D        (1/2, 3/8; m > 2: 1/2, 1)       see PolyCoef (zfac_f64.cuh)
   float g_i, g_r, g_p;  // p2: G = g_i I + g_r R + g_p D (3/8, 5/16, 35/128 or 0)
+  int scaled;           // FP64-master modes: a4 works on R~ = rscale R (State::rscale): Q~ = q_r R~ + (q_d / rscale) R~ R~
+  double* z64;          // a5x: FP64 master Z, updated in place: Z64 += D / rscale
+  double* w64t;         // a5x: FP64 W = Z^T (DMMA residual engine) or null
   unsigned long long* dbg;  // -DZFAC_TIMING builds only: per-CTA wait-cycle counters of the MMA issuer (else null)
 };
 
@@ -324,8 +327,9 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
   } else if (EPI == EPI_A4) {                           // Q = 1/2 R + 3/8 R R, mirror
     float r32[SUB];
     load_f32_row<SUB>(p.f32_in + off, r32);
+    const float qd = p.scaled ? p.q_d * p.st->rinv : p.q_d;            // scaled operands: D = R~ R~ = rscale^2 R R
 #pragma unroll
-    for (int j = 0; j < SUB; ++j) v[j] = p.q_r * r32[j] + p.q_d * v[j];
+    for (int j = 0; j < SUB; ++j) v[j] = p.q_r * r32[j] + qd * v[j];
     if (KIND == KIND_TF32) {
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
@@ -363,6 +367,22 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
         store_h_col<PAIR, SUB>(p.h_out, plane, offt, ld, v);
         store_h_col<PAIR, SUB>(p.out2, plane, offt, ld, g);
       }
+    }
+  } else if (EPI == EPI_A5X) {                          // FP64 master: Z64 += (Z Q~) / rscale; next operand pair; W64 = Z^T
+    if (KIND == KIND_F16X2) {
+      const double rinv = (double)p.st->rinv;
+      double* zp = p.z64 + off;
+      float z32[SUB];
+#pragma unroll
+      for (int j = 0; j < SUB; j += 2) {
+        double2 z = *reinterpret_cast<const double2*>(zp + j);
+        z.x += (double)v[j] * rinv; z.y += (double)v[j + 1] * rinv;
+        *reinterpret_cast<double2*>(zp + j) = z;
+        if (p.w64t) { p.w64t[offt + (size_t)j * ld] = z.x; p.w64t[offt + (size_t)(j + 1) * ld] = z.y; }
+        z32[j] = (float)z.x; z32[j + 1] = (float)z.y;
+      }
+      flag_h16_range<SUB>(p.st, z32);
+      store_h_row<PAIR, SUB>(p.h_out, plane, off, z32);                // FP32[Z64] as the next update's A operand
     }
   } else {                                              // a5: Z_next = Z + Z Q, W = Z_next^T
     float z32[SUB];
@@ -859,6 +879,9 @@ inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) 
     case EPI_X3: umma_gemm_kernel<KIND, EPI_X3><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
     case EPI_A4: umma_gemm_kernel<KIND, EPI_A4><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
     case EPI_P2: umma_gemm_kernel<KIND, EPI_P2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    case EPI_A5X:
+      if (KIND == KIND_F16X2) umma_gemm_kernel<KIND_F16X2, EPI_A5X><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      break;
     default:     umma_gemm_kernel<KIND, EPI_A5><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
   }
 }

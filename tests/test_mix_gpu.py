@@ -1,0 +1,195 @@
+"""GPU parity of the FP64-master modes (include/zfac.h: ZFAC_MODE_F64_MIXED, ZFAC_MODE_F64_I8) against the oracle.
+
+Both modes compute the residual to the FP64 level (F64_MIXED on the FP64 tensor pipe, F64_I8 from error-free int8 slices
+on the INT8 tensor cores) and evaluate the update's correction in FP32-class arithmetic, added to the FP64 master.  The
+oracle of that iteration is `O.refine(..., update_dtype=float32)` / `O.update_mixed` (pinned in
+tests/test_oracle_refi_pins.py); against the all-FP64 oracle the result differs by the rounding of the correction,
+~2^-22 ||R_0|| (a rotation of Z: any Z U is an inverse factor), so Z is held to 1e-6 there and what is unique -- the
+invariant ||Z^T S Z - I||_F / sqrt(N) and Z Z^T = S^-1 -- to the FP64 level."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import zfac_oracle as O
+from paper_2404_19163_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+MIX = ["f64mix", "f64i8"]
+
+
+def zb():
+    from paper_2404_19163_b200 import binding
+    return binding
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def _dev(a, dt=torch.float64):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(DEV, dt)
+
+
+def run(w, mode, max_iter, stop, keep=(), options=None):
+    b = zb()
+    S, Z0 = _dev(w.S), _dev(w.Z0)
+    with b.Zfac(w.n, mode, DEV) as zf:
+        for k, v in (options or {}).items():
+            zf.set_option(k, v)
+        Z, it, err, fl = zf.refine(S, Z0, max_iter=max_iter, stop=stop)
+        pk = {k: zf.peek(k).cpu().numpy() for k in keep}
+        launches = zf.last_launch_count
+    return Z.cpu().numpy(), it, err, fl, pk, launches
+
+
+@pytest.mark.parametrize("mode", MIX)
+@pytest.mark.parametrize("n", [96, 300, 700])
+def test_residual_and_one_update_against_oracle(mode, n):
+    """a1, a2, a3 to the FP64 level; one update against the oracle's mixed update."""
+    b = zb()
+    w = W.random_spd_general(n, seed=5 + n, kappa=200.0, pert=0.1, fp32_stored=False)
+    Z, it, err, fl, pk, _ = run(w, mode, 0, b.ZFAC_STOP_FIXED, keep=[b.ZFAC_BUF_T, b.ZFAC_BUF_R, b.ZFAC_BUF_Z])
+    A = w.S @ w.Z0
+    R0 = O.residual(w.S, w.Z0)
+    assert it == 0 and fl == b.ZFAC_R_MAXITER and len(err) == 1
+    assert _rel(pk[b.ZFAC_BUF_T], A.T) < 1e-13                            # a1: T = (S Z)^T
+    # a2: R = I - Z^T S Z; X ~ I is formed to ~1e-15 absolute, F64_I8 then stores R rounded to FP32 (6e-8 relative)
+    tol_r = 1e-13 * math.sqrt(n) + (1e-7 * np.linalg.norm(R0) if mode == "f64i8" else 0.0)
+    assert np.linalg.norm(pk[b.ZFAC_BUF_R] - R0) < tol_r
+    assert err[0] == pytest.approx(O.err_fro(R0), rel=1e-7 if mode == "f64i8" else 1e-10)
+    assert np.array_equal(Z, w.Z0) and np.array_equal(pk[b.ZFAC_BUF_Z], w.Z0)
+    Z, it, err, fl, _, _ = run(w, mode, 1, b.ZFAC_STOP_FIXED)
+    Zm = O.update_mixed(w.Z0, R0, np.float32)
+    Zx = O.update_delta_form(w.Z0, R0)
+    q = np.linalg.norm(0.5 * R0 + 0.375 * R0 @ R0, 2)
+    print(f"[{mode} n={n}] one update: rel vs mixed oracle {_rel(Z, Zm):.2e}, vs FP64 oracle {_rel(Z, Zx):.2e} (||Q||_2 = {q:.2e})")
+    assert it == 1 and len(err) == 2
+    assert _rel(Z, Zx) < 4.0 * 2.0 ** -22 * q                             # the correction is FP32-class, the master FP64
+    assert _rel(Z, Zm) < 4.0 * 2.0 ** -22 * q
+    assert err[1] == pytest.approx(O.err_fro(O.residual(w.S, Z)), rel=1e-6, abs=1e-13 * math.sqrt(n))
+    assert not np.allclose(Z, Z.T)
+
+
+@pytest.mark.parametrize("mode", MIX)
+@pytest.mark.parametrize("n", [1, 2, 17, 127, 128, 129, 255, 256, 257, 383, 700, 1100])
+def test_full_run_reaches_the_fp64_level(mode, n):
+    b = zb()
+    w = W.random_spd_general(n, seed=300 + n, kappa=50.0, pert=0.1, fp32_stored=False)
+    Z, it, err, fl, _, launches = run(w, mode, 40, b.ZFAC_STOP_PAPER)
+    nat = O.refine(w.S, w.Z0, 40, O.STOP_PAPER)
+    assert len(err) == it + 1
+    if not (fl & b.ZFAC_R_STOPPED):
+        assert fl == b.ZFAC_R_MAXITER and it == 40 and err[-1] <= 1e-300
+        return
+    ref = O.refine(w.S, w.Z0, it, O.STOP_FIXED)
+    mix = O.refine(w.S, w.Z0, it, O.STOP_FIXED, update_dtype=np.float32)
+    inv = O.final_residual_per_sqrt_n(w.S, Z)
+    print(f"[{mode} n={n}] iters={it} (FP64 oracle stops at {nat.iters}) rel vs FP64 oracle {_rel(Z, ref.Z):.2e}, vs mixed oracle "
+          f"{_rel(Z, mix.Z):.2e}; ||Z^T S Z - I||_F/sqrtN = {inv:.2e}; Err={np.array2string(err, precision=2)}")
+    assert nat.iters <= it <= nat.iters + 2
+    assert inv < 1e-12 * max(1.0, math.sqrt(n))
+    assert _rel(Z, ref.Z) < 1e-6 and _rel(Z, mix.Z) < 1e-6
+    assert _rel(Z @ Z.T, ref.Z @ ref.Z.T) < 1e-11
+    for k in range(it + 1):
+        if ref.err[k] > 1e-4:
+            assert err[k] == pytest.approx(ref.err[k], rel=1e-4)
+    assert err[it] == pytest.approx(O.err_fro(O.residual(w.S, Z)), rel=1e-2, abs=1e-13 * math.sqrt(n) + 1e-15)
+
+
+@pytest.mark.parametrize("mode", MIX)
+def test_ill_conditioned_kappa_1e5_and_unaligned_ld(mode):
+    """kappa = 1e5 (the Ag561 stand-in of configs 3 / 4): the FP64-level residual is what makes the run converge where
+    SPLIT16 stalls at ~1e-2; ld > n on every buffer."""
+    b = zb()
+    n = 770
+    w = W.nonsymmetric_start(W.config3(n=n), alpha=2e-4)
+    S64 = np.asarray(w.S, np.float64); Z64 = np.asarray(w.Z0, np.float64)
+    Sb = torch.full((n, n + 3), float("nan"), dtype=torch.float64, device=DEV); Sb[:, :n] = _dev(S64)
+    Zb0 = torch.full((n, n + 1), float("nan"), dtype=torch.float64, device=DEV); Zb0[:, :n] = _dev(Z64)
+    out = torch.full((n, n + 5), -3.0, dtype=torch.float64, device=DEV)
+    with b.Zfac(n, mode, DEV) as zf:
+        Z, it, err, fl = zf.refine(Sb[:, :n], Zb0[:, :n], max_iter=40, stop=b.ZFAC_STOP_PAPER, out=out[:, :n])
+    Z = Z.cpu().numpy()
+    assert bool((out[:, n:] == -3.0).all())
+    ref = O.refine(S64, Z64, it, O.STOP_FIXED)
+    inv = O.final_residual_per_sqrt_n(S64, Z)
+    print(f"[{mode} kappa=1e5 n={n}] iters={it} rel vs FP64 oracle {_rel(Z, ref.Z):.2e}; invariant {inv:.2e}; Err={np.array2string(err, precision=2)}")
+    assert fl & b.ZFAC_R_STOPPED
+    assert inv < 1e-10
+    assert _rel(Z, ref.Z) < 1e-6
+
+
+@pytest.mark.parametrize("high", MIX)
+@pytest.mark.parametrize("low", ["split16", "hh16"])
+def test_refi_into_the_fp64_master_modes(low, high):
+    """Alg. 3 with the new refinement stage: low precision to its stop, then refinement steps whose residual is FP64-level.
+    With max_iter = 0 the stage starts from FP64[Z0] and must match the oracle's mixed refinement steps."""
+    b = zb()
+    n = 520
+    w = W.random_spd_general(n, seed=91, kappa=300.0, pert=0.1, fp32_stored=True)
+    S, Z0 = _dev(w.S, torch.float32), _dev(w.Z0, torch.float32)
+    with b.Zfac(n, low, DEV) as zl, b.Zfac(n, high, DEV) as zh:
+        Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=0, refi_steps=2, final_check=True)
+        assert Z.dtype == torch.float64 and it == 2 and (fl & b.ZFAC_R_REFINED) and len(err) == 4
+        ora = O.refine(w.S, w.Z0, 2, O.STOP_FIXED, update_dtype=np.float32)
+        assert _rel(Z.cpu().numpy(), ora.Z) < 1e-6
+        assert err[1] == pytest.approx(ora.err[0], rel=1e-9)            # FP64[Z0]: the same residual
+        assert np.allclose(err[1:], ora.err, rtol=2e-2, atol=1e-12)     # later ones carry the (different) FP32 roundings of the correction
+        Z, it, err, fl = zl.refine_refi(zh, S, Z0, max_iter=30, refi_steps=2, final_check=True)
+    Z = Z.cpu().numpy()
+    k = it - 2
+    inv = O.final_residual_per_sqrt_n(w.S, Z)
+    print(f"[{low} -> {high}] low iters={k} Err={np.array2string(err, precision=2)} invariant={inv:.2e}")
+    assert (fl & b.ZFAC_R_REFINED) and len(err) == it + 2 and inv < 1e-11
+    assert err[-1] == pytest.approx(inv * math.sqrt(n), rel=1e-2, abs=1e-12)
+    full = O.refine_with_refi(w.S, w.Z0, 30, low_dtype=np.float32, refi_steps=2, update_dtype=np.float32)
+    assert _rel(Z @ Z.T, full.Z @ full.Z.T) < 1e-9
+
+
+def test_i8_slice_count_sets_the_accuracy_and_nonfinite_input_is_reported():
+    """ZFAC_OPT_I8_SLICES: s slices keep 7 s bits relative to the row maxima, so the floor of the residual scales like
+    2^(-7 s); 8 slices are FP64-equivalent.  A NaN in the input cannot be sliced: it must still surface as
+    ZFAC_R_NONFINITE (the other modes get that from the arithmetic itself)."""
+    b = zb()
+    n = 300
+    w = W.random_spd_general(n, seed=17, kappa=100.0, pert=0.1, fp32_stored=False)
+    floors = {}
+    for s_ in (4, 6, 8):
+        Z, it, err, fl, _, _ = run(w, "f64i8", 40, b.ZFAC_STOP_PAPER, options={"i8_slices": s_})
+        floors[s_] = O.final_residual_per_sqrt_n(w.S, Z)
+        assert fl & b.ZFAC_R_STOPPED
+    print("[f64i8] invariant by slice count:", {k: f"{v:.2e}" for k, v in floors.items()})
+    assert floors[8] < 1e-12 and floors[6] < 3e-9 and floors[4] < 3e-5
+    assert floors[4] > 1e3 * floors[8]
+    for mode in MIX:
+        wb = W.Workload("nan", n, w.S, w.Z0.copy(), fp32_stored=False)
+        wb.Z0[3, 4] = float("nan")
+        Z, it, err, fl, _, _ = run(wb, mode, 10, b.ZFAC_STOP_PAPER)
+        assert it == 0 and (fl & b.ZFAC_R_NONFINITE) and math.isnan(err[0]), mode
+        ws = W.Workload("nanS", n, w.S.copy(), w.Z0, fp32_stored=False)
+        ws.S[7, 7] = float("inf")
+        Z, it, err, fl, _, _ = run(ws, mode, 10, b.ZFAC_STOP_PAPER)
+        assert it == 0 and (fl & b.ZFAC_R_NONFINITE), mode
+
+
+@pytest.mark.parametrize("mode", MIX)
+def test_while_graph_and_determinism(mode):
+    b = zb()
+    n = 300
+    w = W.random_spd_general(n, seed=23, kappa=40.0, pert=0.1, fp32_stored=False)
+    S, Z0 = _dev(w.S), _dev(w.Z0)
+    with b.Zfac(n, mode, DEV) as zf:
+        Zd, itd, errd, fld = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+        Zd = Zd.clone()
+        Z2, it2, err2, fl2 = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+        assert torch.equal(Zd, Z2) and np.array_equal(errd, err2)               # run-to-run determinism
+        with b.ZfacLoopGraph(zf, S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER) as lg:
+            Zg, itg, errg, flg = lg.launch()
+            assert itg == itd and flg == fld and np.array_equal(errg, errd) and torch.equal(Zg, Zd)
+        with pytest.raises(b.ZfacError):
+            zf.set_order(3)
+        with pytest.raises(b.ZfacError):
+            zf.congruence(S, Z0)
