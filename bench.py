@@ -30,8 +30,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# Alg. 3 paths timed for `time_to_gate`: (name, low-precision mode, refinement mode, refinement updates)
-REFI_PATHS = [("split16+refi_f64", "split16", "f64", 1)]
+# Paths timed for `time_to_gate` on the FP32-stored workload.  ("refi", name, low mode, refinement mode, refinement updates):
+# Alg. 3; ("mode", name, mode): Alg. 2 in a double-element mode fed with the FP32-stored S, Z0 (ZFAC_OPT_INPUT_F32).
+GATE_PATHS = [("mode", "f64i8", "f64i8"), ("mode", "f64mix", "f64mix"), ("refi", "split16+refi_f64i8", "split16", "f64i8", 2),
+              ("refi", "split16+refi_f64", "split16", "f64", 1)]
 
 METRIC = "Z-refinement TFLOP/s (FP32-equivalent, (4+8k)N^3 flop) at N=8192, split-FP16, time-to-converged"
 UNIT = "TFLOP/s"
@@ -283,7 +285,8 @@ def run_sweep(args, dev, peaks):
 
 
 # ----------------------------------------------------------------------------- parity and time-to-gate (oracle side)
-GATES = {"f64": 1e-11, "split16": 1e-5, "tf32": 1e-3, "hh16": 1e-3}      # north_star: ||Z - Z_ora||_F / ||Z_ora||_F
+F64_MODES = ("f64", "f64mix", "f64i8")
+GATES = {"f64": 1e-11, "split16": 1e-5, "tf32": 1e-3, "hh16": 1e-3, "f64mix": 1e-6, "f64i8": 1e-6}      # north_star: ||Z - Z_ora||_F / ||Z_ora||_F
 RESIDUAL_GATE = 1e-10       # ||Z^T S Z - I||_F / sqrt(N) of a "converged to FP64 level" result (~1e-11 after refinement)
 
 
@@ -406,7 +409,7 @@ def run_ours(args):
     primary = None
 
     def run_mode(mode, with_e2e, with_clock):
-        dt = torch.float64 if mode == "f64" else torch.float32
+        dt = torch.float64 if mode in F64_MODES else torch.float32
         S = torch.from_numpy(w.S).to(dev, dt); Z0 = torch.from_numpy(w.Z0).to(dev, dt)
         Zout = torch.empty_like(Z0)
         with zb.Zfac(n, mode, dev) as zf:
@@ -464,7 +467,7 @@ def run_ours(args):
     # --steps the caller passed); no profiling events inside
     sustained = None
     if diag:
-        dtp = torch.float64 if args.mode == "f64" else torch.float32
+        dtp = torch.float64 if args.mode in F64_MODES else torch.float32
         Sd = torch.from_numpy(w.S).to(dev, dtp); Zd = torch.from_numpy(w.Z0).to(dev, dtp); Zo = torch.empty_like(Zd)
         with zb.Zfac(n, args.mode, dev) as zf:
             per = max(1, int(2000.0 / max(primary["ms_per_step"], 1e-3)) + 1)
@@ -532,41 +535,58 @@ def run_ours(args):
         # run for the same total number of updates AND the FP64-level invariant <= 1e-10.
         try:
             ttg = {}
-            for pname, low, high, steps in REFI_PATHS:
-                if high not in zb.MODES:
-                    continue
+            for path in GATE_PATHS:
+                kind, pname = path[0], path[1]
                 S32 = torch.from_numpy(w.S).to(dev, torch.float32); Z32 = torch.from_numpy(w.Z0).to(dev, torch.float32)
-                hdt = torch.float32 if high == "split16" else torch.float64
-                Zr = torch.empty((n, n), dtype=hdt, device=dev)
-                with zb.Zfac(n, low, dev) as zl, zb.Zfac(n, high, dev) as zh:
+                hS = torch.from_numpy(w.S).to(torch.float32).pin_memory(); hZ0 = torch.from_numpy(w.Z0).to(torch.float32).pin_memory()
+                if kind == "refi":
+                    low, high, steps = path[2], path[3], path[4]
+                    hdt = torch.float32 if high == "split16" else torch.float64
+                    ctxs = (zb.Zfac(n, low, dev), zb.Zfac(n, high, dev))
+                    zl, zh = ctxs
+                    Zr = torch.empty((n, n), dtype=hdt, device=dev); hZ = torch.empty((n, n), dtype=hdt).pin_memory()
+                    call = lambda: zl.refine_refi(zh, S32, Z32, max_iter=args.max_iter, refi_steps=steps, final_check=True, out=Zr, sync=False)
+                    host = lambda: zl.refine_refi_host(zh, hS, hZ0, hZ, max_iter=args.max_iter, refi_steps=steps, final_check=True)
+                    info = {"low": low, "high": high, "refi_steps": steps, "final_check": True}
+                    extra_entries = 2
+                else:
+                    mode = path[2]
+                    hdt = torch.float64
+                    ctxs = (zb.Zfac(n, mode, dev),)
+                    zl = ctxs[0]
+                    zl.set_option("input_f32", 1)
+                    Zr = torch.empty((n, n), dtype=hdt, device=dev); hZ = torch.empty((n, n), dtype=hdt).pin_memory()
+                    call = lambda: zl.refine(S32, Z32, max_iter=args.max_iter, stop=zb.ZFAC_STOP_PAPER, out=Zr, sync=False)
+                    host = lambda: zl.refine_host(hS, hZ0, hZ, max_iter=args.max_iter, stop=zb.ZFAC_STOP_PAPER)
+                    info = {"mode": mode, "inputs": "float (ZFAC_OPT_INPUT_F32)"}
+                    extra_entries = 1
+                try:
                     for _ in range(2):
-                        zl.refine_refi(zh, S32, Z32, max_iter=args.max_iter, refi_steps=steps, final_check=True, out=Zr, sync=False)
+                        call()
                     torch.cuda.synchronize(dev)
                     ts = []
                     for _ in range(5):
                         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
                         e0.record()
-                        _, d_it, d_err, d_fl = zl.refine_refi(zh, S32, Z32, max_iter=args.max_iter, refi_steps=steps,
-                                                             final_check=True, out=Zr, sync=False)
+                        _, d_it, d_err, d_fl = call()
                         e1.record(); torch.cuda.synchronize(dev)
                         ts.append(e0.elapsed_time(e1))
                     its = int(d_it.item())
-                    hist = [float(x) for x in d_err[: its + 2].cpu().numpy()]
-                    hS = torch.from_numpy(w.S).to(torch.float32).pin_memory(); hZ0 = torch.from_numpy(w.Z0).to(torch.float32).pin_memory()
-                    hZ = torch.empty((n, n), dtype=hdt).pin_memory()
-                    zl.refine_refi_host(zh, hS, hZ0, hZ, max_iter=args.max_iter, refi_steps=steps, final_check=True)
+                    hist = [float(x) for x in d_err[: its + extra_entries].cpu().numpy()]
+                    launches = zl.last_launch_count
+                    host()
                     t0 = time.perf_counter()
                     for _ in range(3):
-                        zl.refine_refi_host(zh, hS, hZ0, hZ, max_iter=args.max_iter, refi_steps=steps, final_check=True)
+                        host()
                     e2e = (time.perf_counter() - t0) * 1e3 / 3
                     same = bool(torch.equal(hZ, Zr.cpu()))
-                    launches = zl.last_launch_count
-                res = judge(pname, Zr, its, "split16" if high != "split16" else "split16",
-                            {"ms": float(np.median(ts)), "ms_best": float(min(ts)), "e2e_ms": e2e, "e2e_bitwise_equal_device": same,
+                finally:
+                    for cx in ctxs:
+                        cx.close()
+                info.update({"ms": float(np.median(ts)), "ms_best": float(min(ts)), "e2e_ms": e2e, "e2e_bitwise_equal_device": same,
                              "h2d_bytes": 2 * n * n * 4, "d2h_bytes": n * n * hZ.element_size(), "launches": launches,
-                             "low": low, "high": high, "refi_steps": steps, "final_check": True, "err_history": hist,
-                             "flags": int(d_fl.item())})
-                ttg[pname] = res
+                             "err_history": hist, "flags": int(d_fl.item())})
+                ttg[pname] = judge(pname, Zr, its, "split16", info)
                 del S32, Z32, Zr, hS, hZ0, hZ
                 torch.cuda.empty_cache()
             if "f64" in extra and "f64" in parity:
@@ -641,12 +661,16 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel: a1 (full split GEMM, 3 MMA passes; a5 costs the same)
     kms = primary["kernel_ms"]
-    passes = {"split16": 3, "tf32": 1, "f64": 1, "hh16": 1}[args.mode]
+    passes = {"split16": 3, "tf32": 1, "f64": 1, "hh16": 1, "f64mix": 1, "f64i8": 36}[args.mode]
     roof = None
     if "a1" in kms:
         ach = passes * 2.0 * n ** 3 / (kms["a1"] * 1e-3) / 1e12
         if args.mode in ("split16", "hh16"):
             peak, pk_name = peaks["bf16_sustained"], "bf16_tflops_sustained"
+        elif args.mode == "f64i8":
+            # int8 tensor peak: no measured figure in MEASURED_PEAKS.json; the guide's nominal ratio int8 : bf16 = 2
+            # (4.5 POP/s : 2.25 PFLOP/s dense) applied to the measured bf16 figure
+            peak, pk_name = peaks["bf16_sustained"] * 2.0, "bf16_tflops_sustained x 2 (nominal int8:bf16 ratio); executed int8 ops of 36 slice products"
         elif args.mode == "tf32":
             peak, pk_name = peaks["bf16_sustained"] * 0.5, "bf16_tflops_sustained x 0.5 (nominal tf32:bf16 ratio)"
         else:
@@ -664,7 +688,9 @@ def run_ours(args):
                         traffic = int(f[1])
             except Exception:
                 traffic = None
-        roof = {"bound": "tensor", "kernel": f"umma_gemm_kernel a1 ({args.mode})" if args.mode != "f64" else "f64_gemm_kernel a1",
+        kname = {"f64": "f64_tma_gemm_kernel a1", "f64mix": "f64_tma_gemm_kernel a1", "f64i8": "i8_gemm_kernel a1 (36 int8 slice products)"}.get(
+            args.mode, f"umma_gemm_kernel a1 ({args.mode})")
+        roof = {"bound": "tensor", "kernel": kname,
                 "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": traffic,
                 "peak_source": f"{peaks['source']}: {pk_name}", "frac_of_burst": ach / peaks["bf16_burst"] if args.mode == "split16" else None,
                 "executed_flops_per_launch": passes * 2.0 * n ** 3, "launch_ms": kms["a1"],
@@ -711,7 +737,8 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": {"split16": "f16 (hi + scaled-lo pairs), f32 accumulate", "tf32": "tf32, f32 accumulate", "f64": "f64",
-                      "hh16": "f16 (one pass), f32 accumulate"}[args.mode],
+                      "hh16": "f16 (one pass), f32 accumulate", "f64mix": "f64 residual, f16-pair update into an f64 master",
+                      "f64i8": "int8 slices (exact int32 accumulate) for the f64-level residual, f16-pair update into an f64 master"}[args.mode],
             "data": "synthetic",
             "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "N": n, "stop": args.stop,
                        "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
@@ -746,7 +773,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=8192)
-    ap.add_argument("--mode", default="split16", choices=["split16", "tf32", "f64", "hh16"])
+    ap.add_argument("--mode", default="split16", choices=["split16", "tf32", "f64", "hh16", "f64mix", "f64i8"])
     ap.add_argument("--workload", default="config4", choices=["config4", "config5", "config2"])
     ap.add_argument("--stop", default="paper", choices=["paper", "fixed"])
     ap.add_argument("--max-iter", type=int, default=20)

@@ -24,12 +24,13 @@ ZFAC_R_STOPPED, ZFAC_R_MAXITER, ZFAC_R_NONFINITE, ZFAC_R_REFINED, ZFAC_R_RANGE =
 ZFAC_BUF_T, ZFAC_BUF_R, ZFAC_BUF_Q, ZFAC_BUF_Z = 0, 1, 2, 3
 
 (ZFAC_OPT_CHUNK_KB, ZFAC_OPT_CHUNK0_KB, ZFAC_OPT_HH_SQUARE, ZFAC_OPT_HH_SQUARE_ERR, ZFAC_OPT_PROMOTE_UPDATE, ZFAC_OPT_BAND,
- ZFAC_OPT_MAX_PAIRS, ZFAC_OPT_HOST_OVERLAP, ZFAC_OPT_HOST_UPLOAD_OVERLAP, ZFAC_OPT_HOST_A5_BANDS, ZFAC_OPT_I8_SLICES) = range(11)
+ ZFAC_OPT_MAX_PAIRS, ZFAC_OPT_HOST_OVERLAP, ZFAC_OPT_HOST_UPLOAD_OVERLAP, ZFAC_OPT_HOST_A5_BANDS, ZFAC_OPT_I8_SLICES,
+ ZFAC_OPT_INPUT_F32) = range(12)
 OPTIONS = {"chunk_kb": ZFAC_OPT_CHUNK_KB, "chunk0_kb": ZFAC_OPT_CHUNK0_KB, "hh_square": ZFAC_OPT_HH_SQUARE,
            "hh_square_err": ZFAC_OPT_HH_SQUARE_ERR, "promote_update": ZFAC_OPT_PROMOTE_UPDATE, "band": ZFAC_OPT_BAND,
            "max_pairs": ZFAC_OPT_MAX_PAIRS, "host_overlap": ZFAC_OPT_HOST_OVERLAP,
            "host_upload_overlap": ZFAC_OPT_HOST_UPLOAD_OVERLAP, "host_a5_bands": ZFAC_OPT_HOST_A5_BANDS,
-           "i8_slices": ZFAC_OPT_I8_SLICES}
+           "i8_slices": ZFAC_OPT_I8_SLICES, "input_f32": ZFAC_OPT_INPUT_F32}
 
 MODES = {"split16": ZFAC_MODE_SPLIT16, "tf32": ZFAC_MODE_TF32, "f64": ZFAC_MODE_F64, "hh16": ZFAC_MODE_HH16,
          "f64mix": ZFAC_MODE_F64_MIXED, "f64i8": ZFAC_MODE_F64_I8}
@@ -261,6 +262,7 @@ class Zfac:
         self.n = int(n)
         self.mode = MODES[mode] if isinstance(mode, str) else int(mode)
         self.dtype = torch.float64 if self.mode in F64_ELT_MODES else torch.float32
+        self.in_dtype = self.dtype                      # element type of S and Z0 (float with ZFAC_OPT_INPUT_F32)
         self.device = torch.device(device)
         nbytes = zfac_workspace_bytes(self.n, self.mode)
         if nbytes == 0:
@@ -304,7 +306,7 @@ class Zfac:
                out: Optional[torch.Tensor] = None, sync: bool = True):
         """Device tensors in, device tensors out: (Z, iters, err[0..iters], flags).
         With sync=False returns the raw device tensors (Z, d_iters, d_err, d_flags)."""
-        self._check(S, "S"); self._check(Z0, "Z0")
+        self._check(S, "S", self.in_dtype); self._check(Z0, "Z0", self.in_dtype)
         Z = out if out is not None else torch.empty((self.n, self.n), dtype=self.dtype, device=S.device)
         self._check(Z, "Z")
         d_iters = torch.zeros(1, dtype=torch.int32, device=S.device)
@@ -322,8 +324,8 @@ class Zfac:
     def refine_host(self, S: torch.Tensor, Z0: torch.Tensor, Z: torch.Tensor, max_iter: int = 40,
                     stop: int = ZFAC_STOP_PAPER):
         """Host (pinned) tensors in and out, through zfac_refine_host."""
-        for t, name in ((S, "S"), (Z0, "Z0"), (Z, "Z")):
-            self._check(t, name)
+        for t, name, dt in ((S, "S", self.in_dtype), (Z0, "Z0", self.in_dtype), (Z, "Z", self.dtype)):
+            self._check(t, name, dt)
             if t.is_cuda:
                 raise ValueError(f"{name}: refine_host takes host tensors")
         iters = ctypes.c_int(0)
@@ -338,7 +340,10 @@ class Zfac:
 
     def set_option(self, key: str | int, value: float) -> None:
         """zfac_set_option; key by name (OPTIONS) or number."""
-        zfac_set_option(self.ctx, OPTIONS[key] if isinstance(key, str) else int(key), value)
+        k = OPTIONS[key] if isinstance(key, str) else int(key)
+        zfac_set_option(self.ctx, k, value)
+        if k == ZFAC_OPT_INPUT_F32:
+            self.in_dtype = torch.float32 if int(value) else self.dtype
 
     def get_option(self, key: str | int) -> float:
         return zfac_get_option(self.ctx, OPTIONS[key] if isinstance(key, str) else int(key))

@@ -212,6 +212,9 @@ zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
     case ZFAC_OPT_HOST_UPLOAD_OVERLAP: if (iv != 0 && iv != 1) return ZFAC_E_INVALID; o.host_upload_overlap = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_HOST_A5_BANDS: if (iv < 1 || iv > 64) return ZFAC_E_INVALID; o.host_a5_bands = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_I8_SLICES: if (iv < 2 || iv > I8_MAX_SLICES) return ZFAC_E_INVALID; o.i8_slices = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_INPUT_F32:
+      if ((iv != 0 && iv != 1) || (iv == 1 && !mode_is_f64_elt(c->mode))) return ZFAC_E_INVALID;
+      o.input_f32 = (int)iv; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }
@@ -231,6 +234,7 @@ zfac_status zfac_get_option(const zfac_ctx* c, zfac_option key, double* v) {
     case ZFAC_OPT_HOST_UPLOAD_OVERLAP: *v = o.host_upload_overlap; return ZFAC_OK;
     case ZFAC_OPT_HOST_A5_BANDS: *v = o.host_a5_bands; return ZFAC_OK;
     case ZFAC_OPT_I8_SLICES: *v = o.i8_slices; return ZFAC_OK;
+    case ZFAC_OPT_INPUT_F32: *v = o.input_f32; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }
@@ -438,7 +442,7 @@ static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const 
   c->prof.count = 0;
 
   ZF_CUDA(clear_range(c, s));
-  launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, s, copy_what);     // copy_what = 2: the hook's first_a1 brings S in
+  launch_copy_in(c, d_S, lds, d_Z0, ldz0, c->opt.input_f32 != 0, s, copy_what);     // copy_what = 2: the hook's first_a1 brings S in
   zfac_status rs = run_iterations(c, max_iter, stop, d_err, s, false, hook);
   if (rs != ZFAC_OK) return rs;
   launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, s);
@@ -603,7 +607,8 @@ static zfac_status host_upload(zfac_ctx* c, const void* h_S, int64_t lds, const 
   const Layout& L = c->L;
   char* dS = c->ws + L.off_stage_S;
   char* dZ = c->ws + L.off_stage_Z;
-  const size_t row = (size_t)c->n * L.elt;
+  const size_t elt = (mode_is_f64_elt(c->mode) && c->opt.input_f32) ? 4 : L.elt;      // element size of the INPUTS
+  const size_t row = (size_t)c->n * elt;
   int chunks = 0;
   if (mode_is_umma(c->mode) && L.np / UM_MACRO >= 4 && c->opt.host_upload_overlap) {
     cudaPointerAttributes pS{}, pZ{};
@@ -622,21 +627,21 @@ static zfac_status host_upload(zfac_ctx* c, const void* h_S, int64_t lds, const 
     }
     ZF_CUDA(cudaEventRecord(c->ev_begin, s));                    // the uploads keep their place in the caller's stream order
     ZF_CUDA(cudaStreamWaitEvent(c->side, c->ev_begin, 0));
-    ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, c->side));
+    ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * elt, row, (size_t)c->n, cudaMemcpyHostToDevice, c->side));
     ZF_CUDA(cudaEventRecord(c->ev_up[0], c->side));
     for (int k = 0; k < chunks; ++k) {
       int mc0, mcn; host_chunk_rows(c, chunks, k, &mc0, &mcn);
       const int64_t r0 = (int64_t)mc0 * UM_MACRO < c->n ? (int64_t)mc0 * UM_MACRO : c->n;
       const int64_t r1 = (int64_t)(mc0 + mcn) * UM_MACRO < c->n ? (int64_t)(mc0 + mcn) * UM_MACRO : c->n;
       if (r1 > r0)
-        ZF_CUDA(cudaMemcpy2DAsync(dS + (size_t)r0 * row, row, static_cast<const char*>(h_S) + (size_t)r0 * lds * L.elt,
-                                  (size_t)lds * L.elt, row, (size_t)(r1 - r0), cudaMemcpyHostToDevice, c->side));
+        ZF_CUDA(cudaMemcpy2DAsync(dS + (size_t)r0 * row, row, static_cast<const char*>(h_S) + (size_t)r0 * lds * elt,
+                                  (size_t)lds * elt, row, (size_t)(r1 - r0), cudaMemcpyHostToDevice, c->side));
       ZF_CUDA(cudaEventRecord(c->ev_up[1 + k], c->side));
     }
     ZF_CUDA(cudaStreamWaitEvent(s, c->ev_up[0], 0));            // Z0 is there: copy-in of Z0 (W, operand planes) can start
   } else {
-    ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
-    ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * L.elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+    ZF_CUDA(cudaMemcpy2DAsync(dS, row, h_S, (size_t)lds * elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
+    ZF_CUDA(cudaMemcpy2DAsync(dZ, row, h_Z0, (size_t)ldz0 * elt, row, (size_t)c->n, cudaMemcpyHostToDevice, s));
   }
   *chunks_out = chunks;
   return ZFAC_OK;
@@ -820,7 +825,7 @@ zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const v
     // root: copy-in, first residual (its stop test already sets the condition: max_iter = 0 or a non-finite Err[0] skip the loop)
     const int saved_launches = c->launches;
     if ((e = clear_range(c, cs)) != cudaSuccess) { fail("memset", e); break; }
-    launch_copy_in(c, d_S, lds, d_Z0, ldz0, false, cs);
+    launch_copy_in(c, d_S, lds, d_Z0, ldz0, c->opt.input_f32 != 0, cs);
     cudaGraphNodeParams np = {};
     np.type = cudaGraphNodeTypeConditional;
     np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;

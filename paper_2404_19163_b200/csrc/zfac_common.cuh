@@ -38,6 +38,7 @@ struct Options {
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
+  int input_f32 = 0;         // double-element modes: S and Z0 are float (promoted exactly), Z is returned as double
 };
 
 struct StopArgs {
