@@ -338,9 +338,9 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
         }
       }
     }
-  } else {
-    // ===================================================== epilogue warps 2 .. 9: thread = (row, 128-column half)
-    const int q = warp & 3, g = (warp - 2) >> 2;
+  } else if (warp >= UM_EPI_WARP0) {
+    // ===================================================== epilogue warps 4 .. 11: thread = (row, 128-column half)
+    const int q = warp & 3, g = (warp - UM_EPI_WARP0) >> 2;
     const int rowl = q * 32 + lane;                            // row of this CTA's 128-row half tile
     const uint32_t lead_tempty0 = mapa_u32(tempty_bar(0), 0), lead_tempty1 = mapa_u32(tempty_bar(1), 0);
     double* slab = p.scratch + (size_t)blockIdx.x * (128 * 256);
@@ -403,7 +403,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
 
   // ------------------------------------------------------- teardown (+ step a3 for a2)
   if (EPI == EPI_A2) {
-    const double s = warp_sum(warp >= 2 ? cta_sumsq : 0.0);
+    const double s = warp_sum(warp >= UM_EPI_WARP0 ? cta_sumsq : 0.0);
     if (lane == 0) red[warp] = s;
   }
   tc_fence_before();
@@ -416,7 +416,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
   if (EPI == EPI_A2) {
     if (threadIdx.x == 0) {
       double tot = 0.0;
-      for (int w = 2; w < 2 + UM_EPI_WARPS; ++w) tot += red[w];
+      for (int w = UM_EPI_WARP0; w < UM_EPI_WARP0 + UM_EPI_WARPS; ++w) tot += red[w];
       if (*((volatile int*)&p.st->range) & 2) tot = nan("");   // a non-finite operand was met while slicing
       p.stop.partials[blockIdx.x] = tot;
     }

@@ -53,7 +53,17 @@ constexpr int UM_SMEM_OPERANDS = 192 * 1024;
 constexpr int UM_SMEM_BYTES = UM_SMEM_OPERANDS + 1024 /*align*/ + 256 /*barriers*/;
 constexpr int UM_TMEM_COLS = 512;
 constexpr int UM_EPI_WARPS = 8;                  // two groups of 4 (one warp per TMEM lane quarter), alternating tiles
-constexpr int UM_THREADS = 64 + 32 * UM_EPI_WARPS;
+constexpr int UM_EPI_WARP0 = 4;                  // first epilogue warp: warps 0-3 form the control warpgroup (producer, issuer, 2 idle)
+constexpr int UM_THREADS = 32 * (UM_EPI_WARP0 + UM_EPI_WARPS);     // 384 = three warpgroups
+// Register budget (setmaxnreg works on whole warpgroups): the kernel is launched with 65536 / 384 -> 168 registers per
+// thread; the control warpgroup (one lane each runs TMA issue / MMA issue) gives most of its share to the two epilogue
+// warpgroups, whose SPLIT16 threads hold a 128-column FP32 running sum: 128 x 64 + 256 x 216 <= 384 x 168.
+constexpr int UM_REGS_CONTROL = 64, UM_REGS_EPILOGUE = 216;
+#ifndef ZFAC_DRAIN_W
+#define ZFAC_DRAIN_W 32
+#endif
+template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 constexpr int UM_MAX_STAGES = 6;
 
 // TILE_N: columns of the pair tile (= N of one tcgen05.mma; each CTA stages TILE_N / 2 rows of B).
@@ -194,6 +204,21 @@ __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[16]) {
       "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
       : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
         "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&r)[64]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x64.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,"
+      "%32,%33,%34,%35,%36,%37,%38,%39,%40,%41,%42,%43,%44,%45,%46,%47,%48,%49,%50,%51,%52,%53,%54,%55,%56,%57,%58,%59,%60,%61,%62,%63}, [%64];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31]), "=r"(r[32]),
+        "=r"(r[33]), "=r"(r[34]), "=r"(r[35]), "=r"(r[36]), "=r"(r[37]), "=r"(r[38]), "=r"(r[39]), "=r"(r[40]),
+        "=r"(r[41]), "=r"(r[42]), "=r"(r[43]), "=r"(r[44]), "=r"(r[45]), "=r"(r[46]), "=r"(r[47]), "=r"(r[48]),
+        "=r"(r[49]), "=r"(r[50]), "=r"(r[51]), "=r"(r[52]), "=r"(r[53]), "=r"(r[54]), "=r"(r[55]), "=r"(r[56]),
+        "=r"(r[57]), "=r"(r[58]), "=r"(r[59]), "=r"(r[60]), "=r"(r[61]), "=r"(r[62]), "=r"(r[63])
       : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
@@ -466,26 +491,23 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const bool hh_only = PAIRK && p.hh_only &&
                        (__ldcg(p.stop.d_err + (p.stop.n_iter >= 0 ? p.stop.n_iter : p.st->iters)) <= p.hh_err_max);
 
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < 2; ++b) {                  // arrivals: the warps of both CTAs that read the set
-      mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 2 * UM_EPI_WARPS / SETS);
-      mbar_init(hh_full_bar(b), 1); mbar_init(hh_empty_bar(b), 2 * UM_EPI_WARPS / SETS);
-    }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
-  }
-  if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(UM_TMEM_COLS) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-  }
-  tc_fence_before();
-  __syncthreads();
-  cluster_sync_all();                                      // barrier inits + TMEM allocation visible to the pair
-  tc_fence_after();
-  uint32_t tmem_base;
-  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  // The two register regimes (setmaxnreg) are two disjoint regions of the kernel: everything a role executes, including
+  // its side of the two pair-wide synchronisations, sits inside its own branch (ptxas allocates registers per region
+  // only when no path joins them again before the role code).
+  auto pair_sync_in = [&]() -> uint32_t {                  // barrier inits + TMEM allocation visible to the pair
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    tc_fence_after();
+    uint32_t tb;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tb) : "r"(tmem_slot));
+    return tb;
+  };
+  auto pair_sync_out = [&]() {                             // no MMA / remote arrive of the pair is in flight any more
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+  };
 
   auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
     int I, J;
@@ -504,8 +526,23 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
     m0 = I * UM_TILE_M;
   };
 
-  double cta_sumsq = 0.0;
-
+  if (warp < UM_EPI_WARP0) {
+  reg_dealloc<UM_REGS_CONTROL>();
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < KT::STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int b = 0; b < 2; ++b) {                  // arrivals: the warps of both CTAs that read the set
+      mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 2 * UM_EPI_WARPS / SETS);
+      mbar_init(hh_full_bar(b), 1); mbar_init(hh_empty_bar(b), 2 * UM_EPI_WARPS / SETS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(UM_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+  const uint32_t tmem_base = pair_sync_in();
   if (warp == 0) {
     // ===================================================== TMA producer (both CTAs)
     if (lane == 0) {
@@ -649,13 +686,22 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       }
 #endif
     }
+  }
+  pair_sync_out();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
+  }
   } else {
-    // ===================================================== epilogue warps (2 .. 9), both CTAs
-    // Group g = warps 2 + 4 g .. 5 + 4 g (one warp per TMEM lane quarter).  SETS == 2: group g owns accumulator
+    reg_alloc<UM_REGS_EPILOGUE>();
+    const uint32_t tmem_base = pair_sync_in();
+    double cta_sumsq = 0.0;
+    // ===================================================== epilogue warps (4 .. 11), both CTAs
+    // Group g = warps 4 + 4 g .. 7 + 4 g (one warp per TMEM lane quarter).  SETS == 2: group g owns accumulator
     // set g, i.e. the tiles with local index li = g (mod 2), all TN columns: its stores overlap the other set's
     // mainloop.  SETS == 1: both groups work on every tile, group g on columns [g TN/2, (g + 1) TN/2).
     const int q = warp & 3;                                    // TMEM lane quarter this warp may read
-    const int g = (warp - 2) >> 2;
+    const int g = (warp - UM_EPI_WARP0) >> 2;
     const int set = (SETS == 2) ? g : 0;
     const int col0 = (SETS == 2) ? 0 : g * GCOLS;              // first column of the tile handled by this thread
     const int row = (int)rank * UM_ROWS + q * 32 + lane;       // row of the pair tile held by this thread
@@ -679,17 +725,22 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
         for (int c = 0; c < NCH; ++c) {
           ZF_TWAIT(0, mbar_wait(hh_full_bar(set), hcnt & 1u));
           tc_fence_after();
+          // DRAIN_W columns per tcgen05.ld; the chunk is handed back (arrive) as soon as its last columns are in registers,
+          // BEFORE they are added: the drain is on the critical path of the next chunk's (h)(h) MMAs
+          constexpr int DRAIN_W = ZFAC_DRAIN_W;
 #pragma unroll
-          for (int i = 0; i < GCOLS / 32; ++i) {
-            uint32_t r[32];
-            tmem_ld(tbase + i * 32, r);
+          for (int i = 0; i < GCOLS / DRAIN_W; ++i) {
+            uint32_t r[DRAIN_W];
+            tmem_ld(tbase + i * DRAIN_W, r);
             tmem_ld_wait();
+            if (i == GCOLS / DRAIN_W - 1) {
+              tc_fence_before();
+              __syncwarp();
+              mbar_arrive_cluster_lane0(lead_hh_empty, lane);
+            }
 #pragma unroll
-            for (int j = 0; j < 32; ++j) sum[i * 32 + j] += __uint_as_float(r[j]);
+            for (int j = 0; j < DRAIN_W; ++j) sum[i * DRAIN_W + j] += __uint_as_float(r[j]);
           }
-          tc_fence_before();
-          __syncwarp();
-          mbar_arrive_cluster_lane0(lead_hh_empty, lane);
           ++hcnt;
         }
         // D_hh + 2^-11 D_x into registers, then hand the tensor memory back BEFORE the global loads / stores:
@@ -750,27 +801,21 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
     }
 #ifdef ZFAC_TIMING
-    if (p.dbg && rank == 0 && warp == 2 && lane == 0)
+    if (p.dbg && rank == 0 && warp == UM_EPI_WARP0 && lane == 0)
       for (int i = 0; i < 3; ++i) atomicAdd(p.dbg + (size_t)(EPI * 148 + pair) * 8 + 4 + i, (unsigned long long)twait[i]);
 #endif
+    if (EPI == EPI_A2) {
+      const double s = warp_sum(cta_sumsq);
+      if (lane == 0) red[warp] = s;
+    }
+    pair_sync_out();
   }
 
-  // ------------------------------------------------------- teardown (+ step a3 for a2)
-  if (EPI == EPI_A2) {
-    const double s = warp_sum(warp >= 2 ? cta_sumsq : 0.0);
-    if (lane == 0) red[warp] = s;
-  }
-  tc_fence_before();
-  __syncthreads();
-  cluster_sync_all();                                      // no MMA / remote arrive of the pair is in flight any more
-  if (warp == 1) {
-    tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
-  }
+  // ------------------------------------------------------- step a3 for a2 (all threads)
   if (EPI == EPI_A2) {
     if (threadIdx.x == 0) {
       double tot = 0.0;
-      for (int w = 2; w < 2 + UM_EPI_WARPS; ++w) tot += red[w];
+      for (int w = UM_EPI_WARP0; w < UM_EPI_WARP0 + UM_EPI_WARPS; ++w) tot += red[w];
       p.stop.partials[blockIdx.x] = tot;
     }
     if (arrive_is_last(&p.st->arrive[0], gridDim.x, &last_flag)) stop_test_last_cta(p.stop, red);
