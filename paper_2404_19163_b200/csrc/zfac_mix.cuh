@@ -220,8 +220,8 @@ __host__ __device__ constexpr uint32_t make_idesc_i8(int n) {
   return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(UM_TILE_M >> 4) << 24);
 }
 
-constexpr int I8_STAGES = 6;
-constexpr int I8_STAGE_BYTES = 2 * UM_A_BYTES;      // A rows + B rows of one CTA, one k-block: 32 KB
+constexpr int I8_STAGES = 4;
+constexpr int I8_STAGE_BYTES = 3 * UM_A_BYTES;      // A_i, B_(d-i), B_(d-1-i) rows of one CTA, one k-block: 48 KB
 
 template <int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(UM_THREADS, 1)
@@ -253,7 +253,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < I8_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(tfull_bar(b), 1); mbar_init(tempty_bar(b), 2 * UM_EPI_WARPS); }
+    mbar_init(tfull_bar(0), 1); mbar_init(tempty_bar(0), 2 * UM_EPI_WARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapB)) : "memory");
@@ -285,20 +285,22 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
       const int aoff = (int)rank * UM_ROWS, boff = (int)rank * (TN / 2);
       for (int t = pair; t < num_tiles; t += num_pairs) {
         int m0, n0; bool od; decode(t, m0, n0, od);
-        for (int d = ORD - 1; d >= 0; --d)
+        for (int d = ORD - 1; d >= 0; d -= 2)                // sweep over the orders (d, d - 1)
           for (int i = 0; i <= d; ++i) {
-            const int j = d - i;
-            if (i >= p.sa || j >= p.sb) continue;
+            const int j1 = d - i, j2 = d - 1 - i;             // B slices for order d and order d - 1
+            const bool v1 = (i < p.sa && j1 < p.sb), v2 = (i < p.sa && j2 >= 0 && j2 < p.sb);
+            if (!v1 && !v2) continue;
             for (int kb = 0; kb < KB; ++kb) {
               mbar_wait(empty_bar(stage), phase ^ 1u);
-              if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * I8_STAGE_BYTES);
+              if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * (uint32_t)UM_A_BYTES * (1u + (v1 ? 1u : 0u) + (v2 ? 1u : 0u)));
               const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
-              const uint32_t sa = smem_base + stage * I8_STAGE_BYTES, sb = sa + UM_A_BYTES;
+              const uint32_t sa = smem_base + stage * I8_STAGE_BYTES, sb1 = sa + UM_A_BYTES, sb2 = sb1 + UM_A_BYTES;
               const int kc = kb * 128;
 #pragma unroll
               for (int b = 0; b < UM_ROWS / UM_BOX_ROWS; ++b) {
                 tma_load_2d_pair(sa + b * UM_BOX_BYTES, &p.mapA, kc, i * np + m0 + aoff + b * UM_BOX_ROWS, lead_full);
-                tma_load_2d_pair(sb + b * UM_BOX_BYTES, &p.mapB, kc, j * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                if (v1) tma_load_2d_pair(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                if (v2) tma_load_2d_pair(sb2 + b * UM_BOX_BYTES, &p.mapB, kc, j2 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
               }
               if (++stage == I8_STAGES) { stage = 0; phase ^= 1u; }
             }
@@ -309,32 +311,32 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
     // ===================================================== MMA issuer (leader CTA, one lane)
     if (rank == 0 && lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      uint32_t seq = 0;                                      // orders finished by this pair: accumulator = seq & 1
+      uint32_t seq = 0;                                      // sweeps finished by this pair
       for (int t = pair; t < num_tiles; t += num_pairs) {
-        for (int d = ORD - 1; d >= 0; --d, ++seq) {
-          const uint32_t set = seq & 1u, nuse = seq >> 1;
-          const uint32_t d0 = tmem_base + set * TN;
-          mbar_wait(tempty_bar(set), (nuse & 1u) ^ 1u);
+        for (int d = ORD - 1; d >= 0; d -= 2, ++seq) {
+          const uint32_t dA = tmem_base, dB = tmem_base + TN;  // order d -> columns [0, 256), order d - 1 -> [256, 512)
+          mbar_wait(tempty_bar(0), (seq & 1u) ^ 1u);          // both accumulators drained
           tc_fence_after();
-          uint32_t acc = 0u;
+          uint32_t acc1 = 0u, acc2 = 0u;
           for (int i = 0; i <= d; ++i) {
-            const int j = d - i;
-            if (i >= p.sa || j >= p.sb) continue;
+            const int j1 = d - i, j2 = d - 1 - i;
+            const bool v1 = (i < p.sa && j1 < p.sb), v2 = (i < p.sa && j2 >= 0 && j2 < p.sb);
+            if (!v1 && !v2) continue;
             for (int kb = 0; kb < KB; ++kb) {
               mbar_wait(full_bar(stage), phase);
               tc_fence_after();
               const uint32_t sa = smem_base + stage * I8_STAGE_BYTES;
-              const uint64_t ad = make_sdesc(sa), bd = make_sdesc(sa + UM_A_BYTES);
+              const uint64_t ad = make_sdesc(sa), b1 = make_sdesc(sa + UM_A_BYTES), b2 = make_sdesc(sa + 2 * UM_A_BYTES);
 #pragma unroll
               for (int k = 0; k < 4; ++k) {                  // K = 32 int8 = 32 bytes per MMA, in 16-byte units
-                tc_mma_pair_i8(d0, ad + (uint64_t)(k * 2), bd + (uint64_t)(k * 2), IDESC, acc);
-                acc = 1u;
+                if (v1) { tc_mma_pair_i8(dA, ad + (uint64_t)(k * 2), b1 + (uint64_t)(k * 2), IDESC, acc1); acc1 = 1u; }
+                if (v2) { tc_mma_pair_i8(dB, ad + (uint64_t)(k * 2), b2 + (uint64_t)(k * 2), IDESC, acc2); acc2 = 1u; }
               }
               tc_commit_pair(empty_bar(stage));
               if (++stage == I8_STAGES) { stage = 0; phase ^= 1u; }
             }
           }
-          tc_commit_pair(tfull_bar(set));                    // order d complete in both CTAs
+          tc_commit_pair(tfull_bar(0));                      // orders d and d - 1 complete in both CTAs
         }
       }
     }
@@ -342,7 +344,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
     // ===================================================== epilogue warps 4 .. 11: thread = (row, 128-column half)
     const int q = warp & 3, g = (warp - UM_EPI_WARP0) >> 2;
     const int rowl = q * 32 + lane;                            // row of this CTA's 128-row half tile
-    const uint32_t lead_tempty0 = mapa_u32(tempty_bar(0), 0), lead_tempty1 = mapa_u32(tempty_bar(1), 0);
+    const uint32_t lead_tempty = mapa_u32(tempty_bar(0), 0);
     double* slab = p.scratch + (size_t)blockIdx.x * (128 * 256);
     uint32_t seq = 0;
     for (int t = pair; t < num_tiles; t += num_pairs) {
@@ -350,40 +352,43 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
       const int m = m0 + (int)rank * UM_ROWS + rowl;
       const int eA = p.expA[m];
       double tile_sumsq = 0.0;
-      for (int d = ORD - 1; d >= 0; --d, ++seq) {
-        const uint32_t set = seq & 1u;
-        mbar_wait(tfull_bar(set), (seq >> 1) & 1u);
+      for (int d = ORD - 1; d >= 0; d -= 2, ++seq) {
+        mbar_wait(tfull_bar(0), seq & 1u);
         tc_fence_after();
-        const double wgt = ldexp(1.0, -7 * d);
-        const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + set * TN + g * 128;
+        const bool two = (d >= 1);                             // the sweep carries order d - 1 as well
+        const bool first = (d == ORD - 1), last = (d <= 1);
+        const double w1 = ldexp(1.0, -7 * d), w2 = ldexp(1.0, -7 * (d - 1));
+        const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + g * 128;
 #pragma unroll 1
         for (int c = 0; c < 4; ++c) {
-          uint32_t r[32];
-          tmem_ld(tbase + c * 32, r);
+          uint32_t r1[32], r2[32];
+          tmem_ld(tbase + c * 32, r1);
+          if (two) tmem_ld(tbase + TN + c * 32, r2);
           tmem_ld_wait();
-          if (c == 3) {                                        // accumulator read out: hand it back before the arithmetic
+          if (c == 3) {                                        // accumulators read out: hand them back before the arithmetic
             tc_fence_before();
             __syncwarp();
-            mbar_arrive_cluster_lane0(set ? lead_tempty1 : lead_tempty0, lane);
+            mbar_arrive_cluster_lane0(lead_tempty, lane);
             asm volatile("fence.acq_rel.cta;" ::: "memory");
           }
           const int col0 = g * 128 + c * 32;
           double* sl = slab + (size_t)col0 * 128 + rowl;     // element (row, col) at (col * 128 + row): coalesced per column
-          if (d > 0) {
+          if (!last) {
 #pragma unroll
             for (int j = 0; j < 32; ++j) {
-              double v = (double)(int)r[j] * wgt;
-              if (d < ORD - 1) v += sl[(size_t)j * 128];
+              double v = (double)(int)r1[j] * w1 + (double)(int)r2[j] * w2;
+              if (!first) v += sl[(size_t)j * 128];
               sl[(size_t)j * 128] = v;
             }
           } else {
-            // d = 0: the sum is complete -> scale by the row / column exponents and apply the fused epilogue
+            // last sweep: the sum is complete -> scale by the row / column exponents and apply the fused epilogue
             const size_t ld = (size_t)np;
             const int n = n0 + col0;
 #pragma unroll
             for (int j = 0; j < 32; ++j) {
-              double v = (double)(int)r[j];
-              if (ORD > 1) v += sl[(size_t)j * 128];
+              double v = (double)(int)r1[j] * w1;
+              if (two) v += (double)(int)r2[j] * w2;
+              if (!first) v += sl[(size_t)j * 128];
               v = ldexp(v, eA + p.expB[n + j] - 12);
               if (EPI == EPI_A1) {
                 p.out64[(size_t)m * ld + n + j] = v;
@@ -529,7 +534,9 @@ struct MixSeq {
       nl += 2;
     } else {
       I8Params p{};
-      p.np = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band;
+      // rasterisation band of the full GEMM: half the width of the fp16 kernels' (their operand rows are twice as long in
+      // bytes per slice pass here; measured 2 / 4 / 8 / 16 / 32 columns: 11.9 / 11.85 / 12.3 / 12.9 / 14.1 ms at N = 8192)
+      p.np = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band > 1 ? pl.opt->band / 2 : 1;
       p.sa = p.sb = p.orders = pl.opt->i8_slices;
       p.scratch = reinterpret_cast<double*>(ws + L.off_scratch);
       p.st = st; p.stop = stop; p.stop.num_partials = grid_sym;
