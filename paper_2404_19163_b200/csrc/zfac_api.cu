@@ -322,6 +322,7 @@ static zfac_status refine_mix(zfac_ctx* c, int max_iter, zfac_stop stop, double*
     if (n == max_iter && skip_last) break;
     q.residual(n, n, s, &c->prof);
     if (n == max_iter) break;
+    if (hook && hook->before_update) hook->before_update(hook->self, n, s);
     q.update(n & 1, n, n, s, &c->prof);
     if (hook && hook->after_a5) hook->after_a5(hook->self, n, s);
   }
@@ -470,6 +471,8 @@ struct HostOverlap {
   int64_t ldz;
   const void* dS = nullptr;   // staged S (dense n x n), arriving in `chunks` row chunks; chunk k is complete at ev_up[1 + k]
   int chunks = 0;
+  int early = 1;              // early downloads: after the updates 0 .. early - 1 (2 in the FP64-master modes, whose
+                              // iteration is longer than the download; 1 elsewhere)
 };
 
 // Upload overlap (tcgen05 modes, pinned h_S): Z0 is uploaded first, then S in row chunks of whole macro-tile rows on
@@ -494,12 +497,17 @@ static bool host_first_a1(void* self, void* seq, cudaStream_t s) {
   }
   return true;
 }
-static void host_after_a5(void* self, int n, cudaStream_t s) {
-  if (n != 0) return;
+static void host_before_update(void* self, int n, cudaStream_t s) {
   HostOverlap* h = static_cast<HostOverlap*>(self);
+  if (n >= 1 && n <= h->early) cudaStreamWaitEvent(s, h->c->ev_copy, 0);      // the download of Z_n has left the master buffer
+}
+static void host_after_a5(void* self, int n, cudaStream_t s) {
+  HostOverlap* h = static_cast<HostOverlap*>(self);
+  if (n >= h->early) return;
   zfac_ctx* c = h->c;
   const Layout& L = c->L;
-  const char* src = c->ws + L.off_Z[1];           // Z_1: buffer 1 (F64 / TF32); the 16-bit modes update one FP32 master in place
+  // Z_{n+1}: buffer (n + 1) & 1 (F64 / TF32); the 16-bit and the FP64-master modes update one master in place
+  const char* src = c->ws + L.off_Z[(n + 1) & 1];
   cudaEventRecord(c->ev_a5, s);
   cudaStreamWaitEvent(c->side, c->ev_a5, 0);
   cudaMemcpy2DAsync(h->h_Z, (size_t)h->ldz * L.elt, src, (size_t)L.np * L.elt, (size_t)c->n * L.elt, (size_t)c->n,
@@ -684,6 +692,12 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   ho.dS = dS; ho.chunks = chunks;
   IterHook hook{z_dev ? host_after_a5 : nullptr, &ho};
   if (chunks > 0) hook.first_a1 = host_first_a1;
+  if (z_dev && mode_is_mix(c->mode) && max_iter >= 2) {
+    // one update of these modes (a full FP64-level residual) outlasts the download: the results of the first TWO updates
+    // are sent early, each behind its update; the master is updated in place, so update n + 1 waits for the download of Z_n
+    ho.early = 2;
+    hook.before_update = host_before_update;
+  }
   if (z_dev && mode_is_umma(c->mode) && L.np / UM_MACRO >= 4) {
     hook.a5_bands = c->opt.host_a5_bands;
     if (hook.a5_bands > (int)(L.np / UM_MACRO)) hook.a5_bands = (int)(L.np / UM_MACRO);
@@ -699,7 +713,10 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   ZF_CUDA(cudaMemcpyAsync(ints, dInts, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaStreamSynchronize(s));
   *h_iters = ints[0]; *h_flags = ints[1];
-  if (z_dev && ints[0] != 1)       // the early download holds Z_1: final only if exactly one update ran
+  // the early downloads hold Z_1 (.. Z_early): final if no later update ran.  In-place masters stay what they were once the
+  // iteration has stopped, so the last early download is also right when FEWER updates ran (it re-sent the final Z).
+  const bool early_final = (ho.early == 1) ? (ints[0] == 1) : (ints[0] >= 1 && ints[0] <= ho.early);
+  if (z_dev && !early_final)
     ZF_CUDA(cudaMemcpy2DAsync(h_Z, (size_t)ldz * L.elt, dZ, row, row, (size_t)c->n, cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaMemcpyAsync(h_err, dErr, (size_t)(ints[0] + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
   ZF_CUDA(cudaStreamSynchronize(s));

@@ -83,6 +83,9 @@ struct IterHook {
   // (rows [r0, r1) of the padded Z_1 are final; last = the whole of Z_1 is) INSTEAD of after_a5(0)
   int a5_bands = 1;
   void (*after_a5_band)(void* self, int r0, int r1, bool last, cudaStream_t s) = nullptr;
+  // double-element modes: called before the update n is enqueued (an early download of the in-place FP64 master must have
+  // finished before step a5 overwrites it)
+  void (*before_update)(void* self, int n, cudaStream_t s) = nullptr;
 };
 
 __device__ __forceinline__ double warp_sum(double v) {

@@ -193,3 +193,48 @@ def test_while_graph_and_determinism(mode):
             zf.set_order(3)
         with pytest.raises(b.ZfacError):
             zf.congruence(S, Z0)
+
+
+@pytest.mark.parametrize("mode", MIX)
+def test_host_entry_point_and_float_inputs_match_the_device_entry_point_bitwise(mode):
+    """zfac_refine_host in the FP64-master modes: the results of the first TWO updates are downloaded early, each behind
+    its update (the master is updated in place: update n + 1 waits for the download of Z_n); whichever of them is the
+    last update performed is the result, else the download at the end.  Runs that stop after 1, 2 and >= 3 updates,
+    pinned and pageable, double and float (ZFAC_OPT_INPUT_F32) inputs, ld > n."""
+    b = zb()
+    n = 300
+    w = W.random_spd_general(n, seed=55, kappa=30.0, pert=0.1, fp32_stored=True)
+    lam, V = np.linalg.eigh(w.S)
+    Zex = (V / np.sqrt(lam)) @ V.T
+    G = np.random.default_rng(3).standard_normal((n, n)) / math.sqrt(n)
+    starts = {"exact (1 update)": Zex, "close (2 updates)": W.round_fp32(Zex @ (np.eye(n) + 1e-3 * G)), "far (>= 3 updates)": w.Z0}
+    seen = set()
+    with b.Zfac(n, mode, DEV) as zf:
+        for f32 in (0, 1):
+            zf.set_option("input_f32", f32)
+            idt = torch.float32 if f32 else torch.float64
+            for name, Z0 in starts.items():
+                Sd, Zd = _dev(w.S, idt), _dev(Z0, idt)
+                Zref, itref, errref, flref = zf.refine(Sd, Zd, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+                Zref = Zref.cpu()
+                seen.add(min(itref, 3))
+                for pin in (True, False):
+                    hS = torch.full((n, n + 2), float("nan"), dtype=idt); hS[:, :n] = torch.from_numpy(w.S).to(idt)
+                    hZ0 = torch.from_numpy(np.ascontiguousarray(Z0)).to(idt)
+                    hZ = torch.full((n, n + 3), -2.0, dtype=torch.float64)
+                    if pin:
+                        hS, hZ0, hZ = hS.pin_memory(), hZ0.pin_memory(), hZ.pin_memory()
+                    _, it, err, fl = zf.refine_host(hS[:, :n], hZ0, hZ[:, :n], max_iter=30, stop=b.ZFAC_STOP_PAPER)
+                    assert it == itref and fl == flref and np.array_equal(err, errref), (name, f32, pin)
+                    assert torch.equal(hZ[:, :n], Zref), (name, f32, pin)
+                    assert bool((hZ[:, n:] == -2.0).all())
+        # float inputs promoted exactly: the same FP32-stored problem given as double gives the same bits
+        zf.set_option("input_f32", 0)
+        Za = zf.refine(_dev(w.S), _dev(w.Z0), max_iter=30, stop=b.ZFAC_STOP_PAPER)[0].clone()
+        zf.set_option("input_f32", 1)
+        Zb_ = zf.refine(_dev(w.S, torch.float32), _dev(w.Z0, torch.float32), max_iter=30, stop=b.ZFAC_STOP_PAPER)[0]
+        assert torch.equal(Za, Zb_)
+    assert seen == {1, 2, 3}
+    with b.Zfac(n, "split16", DEV) as zs:
+        with pytest.raises(b.ZfacError):
+            zs.set_option("input_f32", 1)
