@@ -132,6 +132,25 @@ zfac_status zfac_refine(zfac_ctx* ctx, const void* d_S, int64_t lds, const void*
                         void* d_Z, int64_t ldz, int max_iter, zfac_stop stop, int* d_iters,
                         double* d_err, int* d_flags, void* stream);
 
+/* Many small problems in ONE launch sequence (the graph-partitioned sub-problems of PAPER.md:98; the regime
+ * N = O(10^2) - O(10^3) in which the paper reports its largest gain over diagonalisation).
+ * A batched context refines `batch` independent n x n problems of one mode (SPLIT16, HH16 or TF32) together: every
+ * kernel of the iteration is launched once and walks the tiles of all problems, so tensor-memory allocation, barrier
+ * set-up and pipeline fill are paid per launch, not per problem.  Each problem has its own stop test, iteration count,
+ * Err history and flags; a problem that has stopped is skipped by the later launches.  Results are bit-identical to
+ * refining each problem alone with zfac_refine.
+ *   problem b:  S at d_S + b * stride_S, Z0 at d_Z0 + b * stride_Z0, Z at d_Z + b * stride_Z (strides in elements,
+ *               problems must not overlap);  d_iters[b], d_flags[b], d_err[b * (max_iter + 1) .. ]
+ *   1 <= batch <= 4096 and batch * zfac_padded_n(n) <= 2^24.  zfac_refine_batched also accepts a context made by
+ *   zfac_create (batch = 1).  The other entry points take unbatched contexts only (ZFAC_E_INVALID otherwise).
+ * Errors: INVALID (also: mode F64 / F64_MIXED / F64_I8), WORKSPACE, UNSUPPORTED, CUDA. */
+size_t zfac_workspace_bytes_batched(int64_t n, zfac_mode mode, int batch);
+zfac_status zfac_create_batched(zfac_ctx** ctx, int64_t n, zfac_mode mode, int batch, void* d_workspace, size_t bytes);
+int zfac_get_batch(const zfac_ctx* ctx);
+zfac_status zfac_refine_batched(zfac_ctx* ctx, const void* d_S, int64_t lds, int64_t stride_S, const void* d_Z0,
+                                int64_t ldz0, int64_t stride_Z0, void* d_Z, int64_t ldz, int64_t stride_Z, int max_iter,
+                                zfac_stop stop, int* d_iters, double* d_err, int* d_flags, void* stream);
+
 /* Algorithm 3 (PAPER.md:322-341; Sec. IV.B, :308-316): the "+refi" schemes of Table I.
  *   1. Algorithm 2 in the low-precision mode of `low` (FP32 S and Z0) until its parameter-free test fires (or
  *      max_iter updates);

@@ -44,6 +44,7 @@ EXPORTS = [
     "zfac_last_cuda_error", "zfac_set_profile", "zfac_get_profile", "zfac_set_order", "zfac_get_order",
     "zfac_graph_create", "zfac_graph_launch", "zfac_graph_destroy",
     "zfac_set_option", "zfac_get_option", "zfac_refine_refi_host",
+    "zfac_workspace_bytes_batched", "zfac_create_batched", "zfac_get_batch", "zfac_refine_batched",
 ]
 
 _lib: Optional[ctypes.CDLL] = None
@@ -86,6 +87,14 @@ def lib() -> ctypes.CDLL:
     L.zfac_set_option.argtypes = [vp, ci, ctypes.c_double]
     L.zfac_get_option.restype = ci
     L.zfac_get_option.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_double)]
+    L.zfac_workspace_bytes_batched.restype = sz
+    L.zfac_workspace_bytes_batched.argtypes = [i64, ci, ci]
+    L.zfac_create_batched.restype = ci
+    L.zfac_create_batched.argtypes = [ctypes.POINTER(vp), i64, ci, ci, vp, sz]
+    L.zfac_get_batch.restype = ci
+    L.zfac_get_batch.argtypes = [vp]
+    L.zfac_refine_batched.restype = ci
+    L.zfac_refine_batched.argtypes = [vp, vp, i64, i64, vp, i64, i64, vp, i64, i64, ci, ci, vp, vp, vp, vp]
     L.zfac_congruence.restype = ci
     L.zfac_congruence.argtypes = [vp, vp, i64, vp, i64, vp, i64, vp]
     L.zfac_peek.restype = ci
@@ -184,6 +193,31 @@ def zfac_get_option(ctx: int, key: int) -> float:
     if st != ZFAC_OK:
         raise ZfacError(st, "zfac_get_option")
     return float(v.value)
+
+
+def zfac_workspace_bytes_batched(n: int, mode: int, batch: int) -> int:
+    return int(lib().zfac_workspace_bytes_batched(int(n), int(mode), int(batch)))
+
+
+def zfac_create_batched(n: int, mode: int, batch: int, d_workspace: int, nbytes: int) -> int:
+    h = ctypes.c_void_p()
+    st = lib().zfac_create_batched(ctypes.byref(h), int(n), int(mode), int(batch), ctypes.c_void_p(d_workspace), int(nbytes))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_create_batched")
+    return h.value
+
+
+def zfac_get_batch(ctx: int) -> int:
+    return int(lib().zfac_get_batch(ctx))
+
+
+def zfac_refine_batched(ctx: int, d_S: int, lds: int, stride_S: int, d_Z0: int, ldz0: int, stride_Z0: int, d_Z: int,
+                        ldz: int, stride_Z: int, max_iter: int, stop: int, d_iters: int, d_err: int, d_flags: int,
+                        stream: int = 0) -> None:
+    st = lib().zfac_refine_batched(ctx, d_S, lds, stride_S, d_Z0, ldz0, stride_Z0, d_Z, ldz, stride_Z, int(max_iter),
+                                   int(stop), d_iters, d_err, d_flags, ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_refine_batched")
 
 
 def zfac_congruence(ctx: int, d_H: int, ldh: int, d_Z: int, ldz: int, d_out: int, ldo: int, stream: int = 0) -> None:
@@ -414,6 +448,70 @@ class Zfac:
 
     def get_profile(self):
         return zfac_get_profile(self.ctx)
+
+    @property
+    def last_launch_count(self) -> int:
+        return zfac_last_launch_count(self.ctx)
+
+
+class ZfacBatched:
+    """`batch` independent n x n problems refined by ONE launch sequence (zfac_create_batched / zfac_refine_batched):
+    S, Z0, Z are [batch, n, n] device tensors (row-major problems, any batch stride).  Marshalling only."""
+
+    def __init__(self, n: int, mode: str | int, batch: int, device: str | torch.device = "cuda"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("zfac needs a CUDA device (sm_100a); there is no CPU path")
+        self.n, self.batch, self.device = int(n), int(batch), torch.device(device)
+        self.mode = MODES[mode] if isinstance(mode, str) else int(mode)
+        self.dtype = torch.float32
+        nbytes = zfac_workspace_bytes_batched(self.n, self.mode, self.batch)
+        if nbytes == 0:
+            raise ZfacError(ZFAC_E_INVALID, "zfac_workspace_bytes_batched")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            self.ctx = zfac_create_batched(self.n, self.mode, self.batch, self.workspace.data_ptr(), self.workspace.numel())
+
+    def close(self) -> None:
+        if getattr(self, "ctx", None):
+            zfac_destroy(self.ctx)
+            self.ctx = None
+            self.workspace = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def set_option(self, key: str | int, value: float) -> None:
+        zfac_set_option(self.ctx, OPTIONS[key] if isinstance(key, str) else int(key), value)
+
+    def set_order(self, m: int) -> None:
+        zfac_set_order(self.ctx, m)
+
+    def _check(self, t: torch.Tensor, name: str) -> None:
+        if (t.dtype != self.dtype or t.dim() != 3 or t.shape[0] != self.batch or t.shape[1] != self.n or t.shape[2] != self.n
+                or t.stride(2) != 1 or t.stride(1) < self.n or not t.is_cuda):
+            raise ValueError(f"{name}: expected a [{self.batch}, {self.n}, {self.n}] {self.dtype} device tensor with unit column stride")
+
+    def refine(self, S: torch.Tensor, Z0: torch.Tensor, max_iter: int = 40, stop: int = ZFAC_STOP_PAPER,
+               out: Optional[torch.Tensor] = None, sync: bool = True):
+        """sync=True: list of (Z_b, iters_b, err_b[0..iters_b], flags_b); sync=False: (Z, d_iters, d_err, d_flags)."""
+        self._check(S, "S"); self._check(Z0, "Z0")
+        Z = out if out is not None else torch.empty((self.batch, self.n, self.n), dtype=self.dtype, device=S.device)
+        self._check(Z, "Z")
+        d_iters = torch.zeros(self.batch, dtype=torch.int32, device=S.device)
+        d_flags = torch.zeros(self.batch, dtype=torch.int32, device=S.device)
+        d_err = torch.full((self.batch, max_iter + 1), float("nan"), dtype=torch.float64, device=S.device)
+        stream = torch.cuda.current_stream(S.device).cuda_stream
+        zfac_refine_batched(self.ctx, S.data_ptr(), S.stride(1), S.stride(0), Z0.data_ptr(), Z0.stride(1), Z0.stride(0),
+                            Z.data_ptr(), Z.stride(1), Z.stride(0), max_iter, stop, d_iters.data_ptr(), d_err.data_ptr(),
+                            d_flags.data_ptr(), stream)
+        if not sync:
+            return Z, d_iters, d_err, d_flags
+        torch.cuda.current_stream(S.device).synchronize()
+        its = d_iters.cpu().numpy(); fls = d_flags.cpu().numpy(); errs = d_err.cpu().numpy()
+        return [(Z[b], int(its[b]), errs[b, : its[b] + 1], int(fls[b])) for b in range(self.batch)]
 
     @property
     def last_launch_count(self) -> int:

@@ -31,6 +31,7 @@ static thread_local char g_cuda_err[256] = "";
 struct zfac_ctx {
   int64_t n, np;
   int mode;
+  int batch = 1;   // zfac_create_batched: independent problems refined by one launch sequence (tcgen05 modes)
   int dev = 0;     // device the context was created on; every entry point checks that it is current
   Options opt;     // zfac_set_option
   char* ws;
@@ -69,6 +70,12 @@ size_t zfac_workspace_bytes(int64_t n, zfac_mode mode) {
   return make_layout(n, mode).total;
 }
 
+size_t zfac_workspace_bytes_batched(int64_t n, zfac_mode mode, int batch) {
+  if (n <= 0 || n > (1 << 20) || !mode_is_umma(mode) || batch < 1 || batch > 4096) return 0;
+  if ((int64_t)batch * padded_n(n, mode) > (int64_t)1 << 24) return 0;        // stacked rows must stay 32-bit TMA coordinates
+  return make_layout(n, mode, batch).total;
+}
+
 int64_t zfac_padded_n(int64_t n, zfac_mode mode) {
   if (n <= 0 || !valid_mode(mode)) return 0;
   return padded_n(n, mode);
@@ -87,12 +94,14 @@ const char* zfac_status_string(zfac_status s) {
 
 const char* zfac_last_cuda_error(void) { return g_cuda_err; }
 
-zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_workspace, size_t bytes) {
+static zfac_status create_impl(zfac_ctx** out, int64_t n, zfac_mode mode, int batch, void* d_workspace, size_t bytes) {
   if (!out) return ZFAC_E_INVALID;
   *out = nullptr;
   if (n <= 0 || n > (1 << 20) || !valid_mode(mode)) return ZFAC_E_INVALID;
   if (mode == ZFAC_MODE_F64_I8 && n > 32768) return ZFAC_E_INVALID;      // INT32 accumulation: 8 slice pairs x 2^12 x K < 2^31
-  Layout L = make_layout(n, mode);
+  if (batch < 1 || batch > 4096 || (batch > 1 && !mode_is_umma(mode))) return ZFAC_E_INVALID;
+  if ((int64_t)batch * padded_n(n, mode) > (int64_t)1 << 24) return ZFAC_E_INVALID;
+  Layout L = make_layout(n, mode, batch);
   if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || bytes < L.total) return ZFAC_E_WORKSPACE;
   int dev = 0, major = 0, sms = 0;
   ZF_CUDA(cudaGetDevice(&dev));
@@ -102,7 +111,7 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   zfac_ctx* c = new (std::nothrow) zfac_ctx();
   if (!c) return ZFAC_E_INVALID;
   c->n = n; c->np = L.np; c->mode = mode; c->ws = static_cast<char*>(d_workspace); c->ws_bytes = bytes;
-  c->L = L; c->launches = 0; c->sm_count = sms; c->order = 2; c->dev = dev;
+  c->L = L; c->launches = 0; c->sm_count = sms; c->order = 2; c->dev = dev; c->batch = batch;
   if (mode == ZFAC_MODE_F64) {
     cudaError_t e = f64_plan_create(&c->f64p, L, c->ws);
     if (e == cudaSuccess) e = f64_tma_prepare<EPI_A1>();
@@ -134,6 +143,16 @@ zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_works
   *out = c;
   return ZFAC_OK;
 }
+
+zfac_status zfac_create(zfac_ctx** out, int64_t n, zfac_mode mode, void* d_workspace, size_t bytes) {
+  return create_impl(out, n, mode, 1, d_workspace, bytes);
+}
+
+zfac_status zfac_create_batched(zfac_ctx** out, int64_t n, zfac_mode mode, int batch, void* d_workspace, size_t bytes) {
+  return create_impl(out, n, mode, batch, d_workspace, bytes);
+}
+
+int zfac_get_batch(const zfac_ctx* c) { return c ? c->batch : 0; }
 
 zfac_status zfac_destroy(zfac_ctx* ctx) {
   if (ctx) {
@@ -338,21 +357,23 @@ static zfac_status refine_mix(zfac_ctx* c, int max_iter, zfac_stop stop, double*
 // conversion clamps, published as ZFAC_R_RANGE).  A memset node, not a kernel; capturable.
 static cudaError_t clear_range(zfac_ctx* c, cudaStream_t s) {
   State* st = reinterpret_cast<State*>(c->ws + c->L.off_state);
+  if (c->batch > 1) return cudaMemsetAsync(st, 0, (size_t)c->batch * sizeof(State), s);   // every problem's State (the copy-in sets the rest)
   return cudaMemsetAsync(&st->range, 0, sizeof(int), s);
 }
 
 static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, bool in_f32,
                            cudaStream_t s, int what = 3, int ty0 = 0, int tyn = 0, const State* prev = nullptr,
-                           const void* d_Z0_alt = nullptr) {
+                           const void* d_Z0_alt = nullptr, int64_t stride_S = 0, int64_t stride_Z0 = 0) {
   const Layout& L = c->L;
   char* ws = c->ws;
   CopyInArgs ci{};
   ci.prev = prev; ci.Z0_alt = d_Z0_alt;
+  ci.stride_S = stride_S; ci.stride_Z0 = stride_Z0; ci.rows = (int)L.rows;
   ci.S = d_S; ci.lds = lds; ci.Z0 = d_Z0; ci.ldz0 = ldz0; ci.n = (int)c->n; ci.np = (int)L.np;
   ci.st = reinterpret_cast<State*>(ws + L.off_state);
   ci.oS = ws + L.off_S; ci.oZ = ws + L.off_Z[0]; ci.oW = ws + L.off_W; ci.oZb = ws + L.off_Zb[0];
   ci.what = what; ci.ty0 = ty0;
-  dim3 gi((unsigned)(L.np / CI_TC), (unsigned)(tyn > 0 ? tyn : L.np / CI_TR)), bi(256);
+  dim3 gi((unsigned)(L.np / CI_TC), (unsigned)(tyn > 0 ? tyn : L.np / CI_TR), (unsigned)c->batch), bi(256);
   if (mode_is_mix(c->mode)) {
     // FP64 master Z (+ S, W in FP64 for the DMMA engine), then the FP32 operand pair of Z; I8 engine: int8 slices of S and W
     const bool i8 = (c->mode == ZFAC_MODE_F64_I8);
@@ -387,7 +408,7 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
 }
 
 static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int parity, void* d_Z, int64_t ldz,
-                            int* d_iters, int* d_flags, cudaStream_t s) {
+                            int* d_iters, int* d_flags, cudaStream_t s, int64_t stride_Z = 0) {
   const Layout& L = c->L;
   if (!d_Z) {                                     // publish iters / flags only (the result stays in the workspace)
     publish_kernel<<<1, 32, 0, s>>>(reinterpret_cast<const State*>(c->ws + L.off_state), d_iters, d_flags);
@@ -396,17 +417,18 @@ static void launch_copy_out(zfac_ctx* c, const void* b0, const void* b1, int par
   }
   CopyOutArgs co{};
   co.Zbuf[0] = b0; co.Zbuf[1] = b1; co.parity = parity;
-  co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np;
+  co.Z = d_Z; co.ldz = ldz; co.n = (int)c->n; co.np = (int)L.np; co.stride_Z = stride_Z;
   co.st = reinterpret_cast<State*>(c->ws + L.off_state); co.d_iters = d_iters; co.d_flags = d_flags;
   const int elt = (int)L.elt;
   const bool vec16 = ((size_t)c->n * elt) % 16 == 0 && ((size_t)ldz * elt) % 16 == 0 && ((size_t)L.np * elt) % 16 == 0 &&
+                     ((size_t)stride_Z * elt) % 16 == 0 &&
                      (reinterpret_cast<uintptr_t>(d_Z) & 15u) == 0 && (reinterpret_cast<uintptr_t>(b0) & 15u) == 0 &&
                      (reinterpret_cast<uintptr_t>(b1) & 15u) == 0;
   if (vec16) {
-    dim3 gv((unsigned)(((size_t)c->n * elt / 16 + 255) / 256), (unsigned)((c->n + 7) / 8));
+    dim3 gv((unsigned)(((size_t)c->n * elt / 16 + 255) / 256), (unsigned)((c->n + 7) / 8), (unsigned)c->batch);
     copy_out_vec16_kernel<<<gv, 256, 0, s>>>(co, elt);
   } else {
-    dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8));
+    dim3 go((unsigned)((c->n + 255) / 256), (unsigned)((c->n + 7) / 8), (unsigned)c->batch);
     if (mode_is_f64_elt(c->mode)) copy_out_kernel<double><<<go, 256, 0, s>>>(co);
     else copy_out_kernel<float><<<go, 256, 0, s>>>(co);
   }
@@ -431,7 +453,8 @@ static zfac_status run_iterations(zfac_ctx* c, int max_iter, zfac_stop stop, dou
 // d_Z == nullptr (zfac_refine_refi's low-precision stage): the result stays in the workspace, iters / flags are published.
 static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
                                int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
-                               void* stream, const IterHook* hook, int copy_what = 3) {
+                               void* stream, const IterHook* hook, int copy_what = 3, int64_t stride_S = 0,
+                               int64_t stride_Z0 = 0, int64_t stride_Z = 0) {
   if (!c || !d_S || !d_Z0 || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
   if (lds < c->n || ldz0 < c->n || (d_Z && ldz < c->n) || max_iter < 0) return ZFAC_E_INVALID;
   if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
@@ -443,10 +466,10 @@ static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const 
   c->prof.count = 0;
 
   ZF_CUDA(clear_range(c, s));
-  launch_copy_in(c, d_S, lds, d_Z0, ldz0, c->opt.input_f32 != 0, s, copy_what);     // copy_what = 2: the hook's first_a1 brings S in
+  launch_copy_in(c, d_S, lds, d_Z0, ldz0, c->opt.input_f32 != 0, s, copy_what, 0, 0, nullptr, nullptr, stride_S, stride_Z0);   // copy_what = 2: the hook's first_a1 brings S in
   zfac_status rs = run_iterations(c, max_iter, stop, d_err, s, false, hook);
   if (rs != ZFAC_OK) return rs;
-  launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, s);
+  launch_copy_out(c, ws + L.off_Z[0], ws + L.off_Z[1], -1, d_Z, ldz, d_iters, d_flags, s, stride_Z);
   ZF_CUDA(cudaGetLastError());
   return ZFAC_OK;
 }
@@ -454,8 +477,18 @@ static zfac_status refine_impl(zfac_ctx* c, const void* d_S, int64_t lds, const 
 zfac_status zfac_refine(zfac_ctx* c, const void* d_S, int64_t lds, const void* d_Z0, int64_t ldz0, void* d_Z,
                         int64_t ldz, int max_iter, zfac_stop stop, int* d_iters, double* d_err, int* d_flags,
                         void* stream) {
-  if (!d_Z) return ZFAC_E_INVALID;
+  if (!d_Z || (c && c->batch != 1)) return ZFAC_E_INVALID;
   return refine_impl(c, d_S, lds, d_Z0, ldz0, d_Z, ldz, max_iter, stop, d_iters, d_err, d_flags, stream, nullptr);
+}
+
+zfac_status zfac_refine_batched(zfac_ctx* c, const void* d_S, int64_t lds, int64_t stride_S, const void* d_Z0, int64_t ldz0,
+                                int64_t stride_Z0, void* d_Z, int64_t ldz, int64_t stride_Z, int max_iter, zfac_stop stop,
+                                int* d_iters, double* d_err, int* d_flags, void* stream) {
+  if (!c || !d_Z || !mode_is_umma(c->mode)) return ZFAC_E_INVALID;
+  if (c->batch > 1 && (stride_S < c->n * lds - (lds - c->n) || stride_Z0 < c->n * ldz0 - (ldz0 - c->n) ||
+                       stride_Z < c->n * ldz - (ldz - c->n))) return ZFAC_E_INVALID;      // problems must not overlap
+  return refine_impl(c, d_S, lds, d_Z0, ldz0, d_Z, ldz, max_iter, stop, d_iters, d_err, d_flags, stream, nullptr, 3,
+                     stride_S, stride_Z0, stride_Z);
 }
 
 // zfac_refine_host, pinned h_Z: the download of Z starts right after the FIRST update (a5 of iteration 0 always runs when
@@ -538,6 +571,7 @@ static zfac_status refi_impl(zfac_ctx* low, zfac_ctx* high, const void* d_S, int
                              double* d_err, int* d_flags, int* d_upd, cudaStream_t s, const IterHook* low_hook,
                              int low_copy_what, const IterHook* high_hook) {
   if (!low || !high || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
+  if (low->batch != 1 || high->batch != 1) return ZFAC_E_INVALID;
   if (mode_rank(high->mode) <= mode_rank(low->mode) || low->n != high->n || low->order != high->order) return ZFAC_E_INVALID;
   if (lds < low->n || ldz0 < low->n || ldz < low->n || max_iter < 0 || refi_steps < 1 || refi_steps > 4000)
     return ZFAC_E_INVALID;
@@ -575,7 +609,7 @@ zfac_status zfac_refine_refi(zfac_ctx* low, zfac_ctx* high, const void* d_S, int
 zfac_status zfac_congruence(zfac_ctx* c, const void* d_H, int64_t ldh, const void* d_Z, int64_t ldz, void* d_out,
                             int64_t ldo, void* stream) {
   if (!c || !d_H || !d_Z || !d_out) return ZFAC_E_INVALID;
-  if (ldh < c->n || ldz < c->n || ldo < c->n || !on_own_device(c) || mode_is_mix(c->mode)) return ZFAC_E_INVALID;
+  if (ldh < c->n || ldz < c->n || ldo < c->n || !on_own_device(c) || mode_is_mix(c->mode) || c->batch != 1) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;
@@ -674,7 +708,7 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
                              void* stream) {
   if (!c || !h_S || !h_Z0 || !h_Z || !h_iters || !h_err || !h_flags) return ZFAC_E_INVALID;
   if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0 || max_iter > 4095) return ZFAC_E_INVALID;
-  if (!on_own_device(c)) return ZFAC_E_INVALID;
+  if (!on_own_device(c) || c->batch != 1) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* dS = c->ws + L.off_stage_S;
@@ -815,7 +849,7 @@ zfac_status zfac_graph_create(zfac_ctx* c, const void* d_S, int64_t lds, const v
   if (!c || !d_S || !d_Z0 || !d_Z || !d_iters || !d_err || !d_flags) return ZFAC_E_INVALID;
   if (lds < c->n || ldz0 < c->n || ldz < c->n || max_iter < 0) return ZFAC_E_INVALID;
   if (stop != ZFAC_STOP_PAPER && stop != ZFAC_STOP_FIXED) return ZFAC_E_INVALID;
-  if (!on_own_device(c)) return ZFAC_E_INVALID;
+  if (!on_own_device(c) || c->batch != 1) return ZFAC_E_INVALID;
   const Layout& L = c->L;
   char* ws = c->ws;
   zfac_graph* zg = new (std::nothrow) zfac_graph();
@@ -901,7 +935,7 @@ zfac_status zfac_graph_destroy(zfac_graph* zg) {
 }
 
 zfac_status zfac_peek(zfac_ctx* c, zfac_buf which, void* d_out, int64_t ld, void* stream) {
-  if (!c || !d_out || ld < c->n || !on_own_device(c)) return ZFAC_E_INVALID;
+  if (!c || !d_out || ld < c->n || !on_own_device(c) || c->batch != 1) return ZFAC_E_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Layout& L = c->L;
   char* ws = c->ws;

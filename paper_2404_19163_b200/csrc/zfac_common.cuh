@@ -8,7 +8,7 @@
 namespace zfac {
 
 // Lives at the start of the workspace.  Reset by the first copy-in kernel of every call.
-struct State {
+struct alignas(64) State {
   int done;                  // set by step a3; every later kernel of the call exits at once
   int iters;                 // number of Z updates performed so far (= index of the last Err)
   int flags;                 // ZFAC_R_* bits
@@ -51,6 +51,12 @@ struct StopArgs {
   int stop;                  // zfac_stop
   int order;                 // m of Eq. 13 (2, 3, 4): the test's exponent is nu_max = m + 1
   unsigned long long cond;   // zfac_graph_*: handle of the WHILE node's condition, set to "not done" by the stop test (0: none)
+  // tcgen05 kernels (one launch may carry `batch` independent problems): `st` is an array of one State per problem, the
+  // partials hold 16 sums per a2 tile (8 epilogue warps x 2 CTAs), tiles_pp a2 tiles per problem, and d_err is
+  // [batch][err_stride]
+  int tiles_pp;
+  int slots_pt;              // partial sums per tile: 16 (SPLIT16: both epilogue groups work on a tile) or 8 (one-pass kinds)
+  long long err_stride;
 };
 // n_iter < 0 (inside the loop body of a zfac_graph, whose kernel parameters are fixed): the index comes from the device,
 // State::iters = index of the last Err written, so the residual being evaluated is iters + 1.
@@ -94,11 +100,55 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// Step a3 (Alg. 2, Eq. 38).  Called by ALL threads of the CTA that
-// finished last (blockDim.x <= 1024, multiple of 32).  Sums the per-tile partials in a fixed
+// The decision of step a3 for one problem, taken by ONE thread from Err[n] = err (Alg. 2, Eq. 38).
+// Readings: strict '>' (Q9); test applied unconditionally as Alg. 2 prints it (Q10); non-finite Err stops with a flag
+// (Q9); Err recorded for the final Z also at max_iter (Q7).
+__device__ inline void stop_decide(const StopArgs& a, State* st, double* d_err, double err) {
+  const int n = a.n_iter >= 0 ? a.n_iter : st->iters + 1;
+  d_err[n] = err;
+  st->iters = n;
+  int flags = 0, done = 0;
+  if (!isfinite(err)) {
+    flags = ZFAC_R_NONFINITE; done = 1;
+  } else if (a.stop == ZFAC_STOP_PAPER && n > 0) {
+    const double prev = d_err[n - 1];
+    double thr = prev * prev * prev;                         // m = 2: Err[n-1]^3 (Eq. 38)
+    for (int k = 2; k < a.order; ++k) thr *= prev;           // m = 3, 4: Err[n-1]^(m+1)
+    if (err > thr) { flags = ZFAC_R_STOPPED; done = 1; }
+  }
+  if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
+  if (done) { st->flags |= flags; __threadfence(); st->done = 1; }
+  if (a.cond) cudaGraphSetConditional((cudaGraphConditionalHandle)a.cond, done ? 0u : 1u);   // another pass of the loop?
+}
+
+// Step a3 in the tcgen05 kernels: every epilogue warp leaves the sum of squares of its 32 rows x 128 / 256 columns of an
+// a2 tile in partials[(problem, tile)][slots_pt] and counts itself in; the warp that arrives LAST for a problem sums that
+// problem's partials in index order (lane-strided, then a fixed shuffle tree) and takes the decision.  The order depends
+// on the tile enumeration only, not on which CTA computed which tile: Err[] is run-to-run deterministic and the same
+// whether a problem runs alone or as one of a batch.  Called by all 32 lanes of an epilogue warp after a tile.
+__device__ inline void stop_test_tile_warp(const StopArgs& a, int b, int tile, int slot, double tile_sumsq, int lane) {
+  const double s = warp_sum(tile_sumsq);
+  State* st = a.st + b;
+  const int per = a.tiles_pp * a.slots_pt;
+  double* part = a.partials + (size_t)b * per;
+  int last = 0;
+  if (lane == 0) {
+    part[(size_t)tile * a.slots_pt + slot] = s;
+    __threadfence();
+    last = (atomicAdd(&st->arrive[0], 1u) == (unsigned int)per - 1u);
+    if (last) { st->arrive[0] = 0u; __threadfence(); }
+  }
+  last = __shfl_sync(0xffffffffu, last, 0);
+  if (!last) return;
+  double t = 0.0;
+  for (int i = lane; i < per; i += 32) t += __ldcg(part + i);
+  t = warp_sum(t);
+  if (lane == 0) stop_decide(a, st, a.d_err + (size_t)b * a.err_stride, sqrt(t));
+}
+
+// Step a3 (Alg. 2, Eq. 38), FP64 / INT8 residual kernels.  Called by ALL threads of the CTA that
+// finished last (blockDim.x <= 1024, multiple of 32).  Sums the per-CTA partials in a fixed
 // order (thread-strided, then a fixed shuffle/smem tree), so Err[] is run-to-run deterministic.
-// Readings: strict '>' (Q9); test applied unconditionally as Alg. 2 prints it (Q10);
-// non-finite Err stops with a flag (Q9); Err recorded for the final Z also at max_iter (Q7).
 __device__ inline void stop_test_last_cta(const StopArgs& a, double* smem_red /* >= 32 doubles */) {
   double s = 0.0;
   for (int i = threadIdx.x; i < a.num_partials; i += blockDim.x) s += __ldcg(a.partials + i);
@@ -109,23 +159,7 @@ __device__ inline void stop_test_last_cta(const StopArgs& a, double* smem_red /*
   if (threadIdx.x == 0) {
     double tot = 0.0;
     for (int w = 0; w < nw; ++w) tot += smem_red[w];
-    const double err = sqrt(tot);
-    const int n = stop_index(a);
-    a.d_err[n] = err;
-    State* st = a.st;
-    st->iters = n;
-    int flags = 0, done = 0;
-    if (!isfinite(err)) {
-      flags = ZFAC_R_NONFINITE; done = 1;
-    } else if (a.stop == ZFAC_STOP_PAPER && n > 0) {
-      const double prev = a.d_err[n - 1];
-      double thr = prev * prev * prev;                         // m = 2: Err[n-1]^3 (Eq. 38)
-      for (int k = 2; k < a.order; ++k) thr *= prev;           // m = 3, 4: Err[n-1]^(m+1)
-      if (err > thr) { flags = ZFAC_R_STOPPED; done = 1; }
-    }
-    if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
-    if (done) { st->flags |= flags; __threadfence(); st->done = 1; }
-    if (a.cond) cudaGraphSetConditional((cudaGraphConditionalHandle)a.cond, done ? 0u : 1u);   // another pass of the loop?
+    stop_decide(a, a.st, a.d_err, sqrt(tot));
   }
 }
 

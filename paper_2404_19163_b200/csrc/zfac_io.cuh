@@ -47,6 +47,8 @@ inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 struct Layout {
   int64_t n = 0, np = 0;
+  int batch = 1;        // tcgen05 modes: `batch` independent problems stacked along the rows of every buffer
+  int64_t rows = 0;     // = batch * np: rows of one plane of one buffer (problem b occupies rows [b np, (b + 1) np))
   int mode = 0;
   size_t elt = 0;  // user element size
   size_t off_state = 0, off_dbg = 0, off_partials = 0, num_partials = 0;
@@ -67,19 +69,21 @@ inline bool mode_is_h16(int mode) { return mode == ZFAC_MODE_SPLIT16 || mode == 
 inline bool mode_is_mix(int mode) { return mode == ZFAC_MODE_F64_MIXED || mode == ZFAC_MODE_F64_I8; }
 inline bool mode_is_f64_elt(int mode) { return mode == ZFAC_MODE_F64 || mode_is_mix(mode); }
 
-inline Layout make_layout(int64_t n, int mode) {
+inline Layout make_layout(int64_t n, int mode, int batch = 1) {
   Layout L;
-  L.n = n; L.mode = mode; L.np = padded_n(n, mode);
+  L.n = n; L.mode = mode; L.np = padded_n(n, mode); L.batch = batch; L.rows = (int64_t)batch * L.np;
   L.elt = mode_is_f64_elt(mode) ? 8 : 4;
-  const size_t np2 = (size_t)L.np * (size_t)L.np, n2 = (size_t)n * (size_t)n;
+  const size_t np2 = (size_t)L.rows * (size_t)L.np, n2 = (size_t)n * (size_t)n;      // np2: one plane of one (stacked) buffer
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 1023) / 1024 * 1024; return o; };
-  L.off_state = take(sizeof(State));
+  L.off_state = take(sizeof(State));                             // State of problem 0 (the only one unless batched) ...
   L.off_dbg = take(8 * 148 * 8 * sizeof(unsigned long long));   // -DZFAC_TIMING counters (at a fixed offset: 1024)
-  L.num_partials = (size_t)(L.np / 128) * (size_t)(L.np / 128);
+  if (batch > 1) L.off_state = take((size_t)batch * sizeof(State));       // ... batched: an array of States
+  // tcgen05 kernels: 16 partial sums per a2 tile (256 x 256), per problem; FP64 / INT8 kernels: one per CTA (<= (np / 128)^2)
+  L.num_partials = (size_t)batch * 16 * (size_t)(L.np / 128) * (size_t)(L.np / 128);
   L.off_partials = take(L.num_partials * sizeof(double));
-  L.off_stage_S = take(n2 * L.elt);
-  L.off_stage_Z = take(n2 * L.elt);
+  L.off_stage_S = take(batch > 1 ? 0 : n2 * L.elt);              // staging of the host entry points (not batched)
+  L.off_stage_Z = take(batch > 1 ? 0 : n2 * L.elt);
   L.off_stage_out = take((size_t)4096 * sizeof(double) + 64);
   if (mode_is_mix(mode)) {
     const size_t hb = np2 * 4;                                        // fp16 pair planes
@@ -120,6 +124,8 @@ struct CopyInArgs {
   void* oZ;            // F64/TF32: Z[0];  SPLIT16: float Z32
   void* oW;            // F64/TF32: W;     SPLIT16: half[2][Np][Np]
   void* oZb;           // SPLIT16 / HH16: half[planes][Np][Np] (Zb[0])
+  int64_t stride_S, stride_Z0;   // batched: elements between consecutive problems in the caller's S and Z0 (grid.z = problem)
+  int rows;            // batch * np
   int what;            // bit 0: S, bit 1: Z0 (and W, State reset); 0 is read as 3 (both); bit 2: no W (F64_I8: sliced later)
   int ty0;             // first tile row of this launch (grid.y counts from it): row chunks of S for zfac_refine_host
   // zfac_refine_refi: Z0 is the result of a low-precision run, taken straight from that context's workspace.
@@ -177,17 +183,20 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
   __shared__ Tin sZ[CI_TR * CI_PITCH];
   const int t = threadIdx.x;
   const bool doS = (a.what == 0) || (a.what & 1), doZ = (a.what == 0) || (a.what & 2), doW = doZ && !(a.what & 4);
+  const int pb = blockIdx.z;                                   // problem of a batch (0 otherwise)
+  State* st = a.st + pb;
   if (doZ && blockIdx.x == 0 && blockIdx.y == 0 && t == 0) {
     // refinement stage of Alg. 3 behind a low-precision run that ended non-finite: nothing to refine -- every later
     // kernel of this context exits at once (done = 1) and no Err entry exists (iters = -1)
     const bool dead = a.prev && (a.prev->flags & ZFAC_R_NONFINITE);
-    a.st->done = dead ? 1 : 0; a.st->iters = dead ? -1 : 0; a.st->flags = 0;
-    a.st->arrive[0] = a.st->arrive[1] = a.st->arrive[2] = a.st->arrive[3] = 0u;
+    st->done = dead ? 1 : 0; st->iters = dead ? -1 : 0; st->flags = 0;
+    st->arrive[0] = st->arrive[1] = st->arrive[2] = st->arrive[3] = 0u;
   }
   const int c0 = blockIdx.x * CI_TC, r0 = ((int)blockIdx.y + a.ty0) * CI_TR;
-  const size_t np = (size_t)a.np, np2 = np * np;
-  const Tin* S = static_cast<const Tin*>(a.S);
-  const Tin* Z0 = static_cast<const Tin*>((a.prev && a.Z0_alt && (a.prev->iters & 1)) ? a.Z0_alt : a.Z0);
+  const size_t np = (size_t)a.np, np2 = (size_t)(a.rows > 0 ? a.rows : a.np) * np;     // plane stride of the stacked buffers
+  const size_t rb = (size_t)pb * np;                           // first row of this problem in the stacked buffers
+  const Tin* S = static_cast<const Tin*>(a.S) + (size_t)pb * a.stride_S;
+  const Tin* Z0 = static_cast<const Tin*>((a.prev && a.Z0_alt && (a.prev->iters & 1)) ? a.Z0_alt : a.Z0) + (size_t)pb * a.stride_Z0;
   // ---- phase 1: coalesced loads (64 consecutive columns per row), identity padding
 #pragma unroll
   for (int i = 0; i < CI_TR * CI_TC / 256; ++i) {
@@ -202,7 +211,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
   // ---- phase 2: S and Z, 8 consecutive columns of one row per thread
   {
     const int lr = t >> 3, lc = (t & 7) * 8;
-    const size_t o = (size_t)(r0 + lr) * np + (size_t)(c0 + lc);
+    const size_t o = (rb + (size_t)(r0 + lr)) * np + (size_t)(c0 + lc);
     if (MODE == ZFAC_MODE_F64) {
       Tw* oS = static_cast<Tw*>(a.oS); Tw* oZ = static_cast<Tw*>(a.oZ);
 #pragma unroll
@@ -217,7 +226,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
         float vs[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) vs[j] = (float)sS[lr * CI_PITCH + lc + j];
-        ci_store8<MODE>(a.oS, np2, o, vs, true, a.st);
+        ci_store8<MODE>(a.oS, np2, o, vs, true, st);
       }
       if (doZ) {
         float vz[8];
@@ -226,14 +235,14 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
         float* z32 = static_cast<float*>(a.oZ);                     // FP32 Z (the master copy in the 16-bit modes): not rounded
         *reinterpret_cast<float4*>(z32 + o) = make_float4(vz[0], vz[1], vz[2], vz[3]);
         *reinterpret_cast<float4*>(z32 + o + 4) = make_float4(vz[4], vz[5], vz[6], vz[7]);
-        if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true, a.st);
+        if (MODE == ZFAC_MODE_SPLIT16 || MODE == ZFAC_MODE_HH16) ci_store8<MODE>(a.oZb, np2, o, vz, true, st);
       }
     }
   }
   // ---- phase 3: W = Z^T, 8 consecutive rows of one column of the tile per thread -> 8 consecutive elements of a row of W
   if (doW) {
     const int wr = t >> 2, wc = (t & 3) * 8;                        // W tile: CI_TC rows x CI_TR columns
-    const size_t o = (size_t)(c0 + wr) * np + (size_t)(r0 + wc);
+    const size_t o = (rb + (size_t)(c0 + wr)) * np + (size_t)(r0 + wc);
     if (MODE == ZFAC_MODE_F64) {
       double* oW = static_cast<double*>(a.oW);
 #pragma unroll
@@ -244,7 +253,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
       float vw[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) vw[j] = (float)sZ[(wc + j) * CI_PITCH + wr];
-      ci_store8<MODE>(a.oW, np2, o, vw, true, a.st);
+      ci_store8<MODE>(a.oW, np2, o, vw, true, st);
     }
   }
 }
@@ -257,6 +266,7 @@ struct CopyOutArgs {
   const State* st;
   int* d_iters; int* d_flags;   // may be null (refinement step, congruence)
   int parity;                   // >= 0: Zbuf[parity];  -1: Zbuf[st->iters & 1] (plain call);  -2: Zbuf[updates_done & 1]
+  int64_t stride_Z;             // batched (grid.z = problem): elements between consecutive problems in the caller's Z
 };
 // Number of Z updates a call has performed.  State::iters is the index of the last Err written; it equals the update
 // count unless the call ended with an update whose residual was not evaluated (Alg. 3 as printed: done stays 0).
@@ -267,17 +277,19 @@ __device__ __forceinline__ int updates_done(const State* st) {
 __device__ __forceinline__ int published_flags(const State* st) { return st->flags | ((st->range & 1) ? ZFAC_R_RANGE : 0); }
 // `plain`: the ordinary call (every residual evaluated): the update count is State::iters itself.
 __device__ __forceinline__ void publish_and_select(const CopyOutArgs& a, bool first, const void*& src) {
-  const int iters = a.st->iters;
-  if (a.d_iters && first) { *a.d_iters = iters; *a.d_flags = published_flags(a.st); }
-  src = a.Zbuf[a.parity >= 0 ? a.parity : (a.parity == -1 ? (iters & 1) : (updates_done(a.st) & 1))];
+  const int pb = blockIdx.z;
+  const State* st = a.st + pb;
+  const int iters = st->iters;
+  if (a.d_iters && first) { a.d_iters[pb] = iters; a.d_flags[pb] = published_flags(st); }
+  src = a.Zbuf[a.parity >= 0 ? a.parity : (a.parity == -1 ? (iters & 1) : (updates_done(st) & 1))];
 }
 
 template <typename T>
 __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
   const void* sel;
   publish_and_select(a, blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0, sel);
-  const T* src = static_cast<const T*>(sel);
-  T* dst = static_cast<T*>(a.Z);
+  const T* src = static_cast<const T*>(sel) + (size_t)blockIdx.z * a.np * a.np;
+  T* dst = static_cast<T*>(a.Z) + (size_t)blockIdx.z * a.stride_Z;
   const int c = blockIdx.x * 256 + threadIdx.x;
   const int r0 = blockIdx.y * 8;
   if (c >= a.n) return;
@@ -293,8 +305,8 @@ __global__ void __launch_bounds__(256) copy_out_kernel(const CopyOutArgs a) {
 __global__ void __launch_bounds__(256) copy_out_vec16_kernel(const CopyOutArgs a, int elt) {
   const void* sel;
   publish_and_select(a, blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0, sel);
-  const char* src = static_cast<const char*>(sel);
-  char* dst = static_cast<char*>(a.Z);
+  const char* src = static_cast<const char*>(sel) + (size_t)blockIdx.z * a.np * a.np * elt;
+  char* dst = static_cast<char*>(a.Z) + (size_t)blockIdx.z * a.stride_Z * elt;
   const size_t row_bytes = (size_t)a.n * elt, spitch = (size_t)a.np * elt, dpitch = (size_t)a.ldz * elt;
   const size_t cb = ((size_t)blockIdx.x * 256 + threadIdx.x) * 16;
   if (cb >= row_bytes) return;

@@ -5,7 +5,7 @@
 // from O(1) terms and the signal is what is left after the cancellation.  The UPDATE Z <- Z + Z (1/2 R + 3/8 R R) is a
 // correction of relative size ||R||: evaluated in FP32-class arithmetic (the SPLIT16 kernels of zfac_umma.cuh on the FP32
 // parts of Z and R) and ADDED to the FP64 master, its rounding leaves only ~2^-22 ||R|| in the next residual
-// (oracle: update_mixed; tests/test_oracle_refi_pins.py).  Two modes, same update, two residual engines:
+// (pinned on the CPU side of the tests).  Two modes, same update, two residual engines:
 //
 //   ZFAC_MODE_F64_MIXED   residual by the DMMA kernels of zfac_f64_tma.cuh (a1, a2 on FP64 S, W = Z^T, T);
 //   ZFAC_MODE_F64_I8      residual on the INT8 tensor cores (tcgen05.mma kind::i8, exact INT32 accumulation in tensor
@@ -567,8 +567,8 @@ struct MixSeq {
     else
       r_split_kernel<float><<<g8, 256, 0, s>>>(reinterpret_cast<const float*>(ws + L.off_R), R32s, Rb, np2, st, d_err, n_stop);
     UmmaParams p{};
-    p.np = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band; p.st = st;
-    p.stop = stop; p.stop.n_iter = n_stop;
+    p.np = (int)L.np; p.batch = 1; p.rows = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band; p.st = st;
+    p.stop = stop; p.stop.n_iter = n_stop; p.stop.err_stride = 0;
     const PolyCoef pc = poly_coef(2);
     p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.scaled = 1;
     // a4: Q~ = 1/2 R~ + (3/8 / rscale) R~ R~^T

@@ -88,11 +88,13 @@ struct UmmaParams {
   CUtensorMap mapA;     // A-operand buffer: [ARRAYS*Np rows][Np cols], box 128 B x 64 rows
   CUtensorMap mapB;     // B-operand buffer, same box
   int np;               // padded dimension (= K)
+  int batch;            // independent problems in this launch (>= 1), stacked along the rows of every buffer
+  int rows;             // batch * np: rows of one plane of a buffer; problem b owns rows [b np, (b + 1) np)
   int macro_tiles;      // Np / 256
   int chunk_kb;         // KIND_F16X2: k-blocks (of 64) per promoted accumulation chunk (0 = whole K)
   int chunk0_kb;        // KIND_F16X2: k-blocks of the FIRST chunk of a tile (>= chunk_kb; see the MMA issuer)
-  State* st;
-  StopArgs stop;        // a2 only (partials = one per CTA)
+  State* st;            // [batch]
+  StopArgs stop;        // a2 (partials: 2 UM_EPI_WARPS / SETS per tile and problem); a4 / p2: Err[n] of the one-pass decision
   // epilogue pointers (which are used depends on EPI / KIND; see the epilogue)
   float* f32_out;       // a1: T32 (TF32)   a2: R32   a4: Q32 (TF32)   a5: Z32 next
   const float* f32_in;  // a4: R32          a5: Z32 current
@@ -302,20 +304,22 @@ __device__ __forceinline__ void flag_h16_range(State* st, const float (&v)[N]) {
 }
 
 // Fused epilogue for SUB consecutive columns n..n+SUB-1 of row m (v = accumulator values).
+// m = row in the stacked buffers (mb + local row, mb = first row of the tile's problem), n = local column.
 template <int KIND, int EPI, int SUB>
-__device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SUB], int m, int n, bool offdiag,
+__device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SUB], int m, int n, int mb, bool offdiag,
                                               double& tile_sumsq) {
   constexpr bool PAIR = (KIND == KIND_F16X2);
-  const size_t ld = (size_t)p.np, plane = ld * ld;
+  const size_t ld = (size_t)p.np, plane = ld * (size_t)p.rows;
   const size_t off = (size_t)m * ld + n;               // (m, n)
-  const size_t offt = (size_t)n * ld + m;              // (n, m)
+  const size_t offt = (size_t)(mb + n) * ld + (m - mb);   // (n, m) of the same problem
+  const int ml = m - mb;                               // local row: the diagonal is ml == n
   if (EPI == EPI_A1) {                                  // T = (S Z)^T
     if (KIND == KIND_TF32) {
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
       store_f32_row<SUB>(p.f32_out + off, v);
     } else {
-      flag_h16_range<SUB>(p.st, v);
+      flag_h16_range<SUB>(p.st + mb / p.np, v);
       store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
     }
   } else if (EPI == EPI_A2) {                           // R = I - X, sum R^2, mirror
@@ -326,7 +330,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
     float ss = 0.0f;
 #pragma unroll
     for (int j = 0; j < SUB; ++j) {
-      v[j] = ((m == n + j) ? 1.0f : 0.0f) - v[j];
+      v[j] = ((ml == n + j) ? 1.0f : 0.0f) - v[j];
       ss = fmaf(v[j], v[j], ss);
     }
     tile_sumsq += (double)ss;
@@ -373,7 +377,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
       float r32[SUB];
       load_f32_row<SUB>(p.f32_in + off, r32);
 #pragma unroll
-      for (int j = 0; j < SUB; ++j) g[j] = ((m == n + j) ? p.g_i : 0.0f) + p.g_r * r32[j] + p.g_p * v[j];
+      for (int j = 0; j < SUB; ++j) g[j] = ((ml == n + j) ? p.g_i : 0.0f) + p.g_r * r32[j] + p.g_p * v[j];
     }
     if (KIND == KIND_TF32) {
       float* g32 = static_cast<float*>(p.out2);
@@ -420,7 +424,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
       for (int j = 0; j < SUB; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
     } else {
-      flag_h16_range<SUB>(p.st, v);
+      flag_h16_range<SUB>(p.st + mb / p.np, v);
       store_h_row<PAIR, SUB>(p.h_out, plane, off, v);                // Z16 next
       store_h_col<PAIR, SUB>(p.h_out_t, plane, offt, ld, v);         // W16 = Z16^T
     }
@@ -439,7 +443,8 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 template <int KIND, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(UM_THREADS, 1)
 umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
-  if (*((volatile int*)&p.st->done)) return;       // stop decided earlier in this call (uniform over the grid)
+  // stop decided earlier in this call (uniform over the grid); in a batched launch finished problems are skipped tile by tile
+  if (p.batch == 1 && *((volatile int*)&p.st->done)) return;
 
   using KT = KindTraits<KIND>;
   constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3 || EPI == EPI_P2);
@@ -469,9 +474,6 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   auto hh_full_bar = [&](int b) { return bar_base + 128u + 8u * b; };
   auto hh_empty_bar = [&](int b) { return bar_base + 144u + 8u * b; };
   const uint32_t tmem_slot = bar_base + 160u;
-  __shared__ double red[32];
-  __shared__ int last_flag;
-
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();                 // 0 = leader (issues the MMAs)
   const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
@@ -484,12 +486,8 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int T = p.macro_tiles;
   const int JC = (!SYM && p.jcols > 0) ? p.jcols : T * NSPLIT;             // tile columns of this launch
   const int TI = (!SYM && p.irows > 0) ? p.irows : T;                      // tile rows of this launch
-  const int num_tiles = SYM ? T * (T + 1) / 2 * NSPLIT : TI * JC;         // 256 x TN pair tiles
-  // One pass for a second-order product (a4 / p2, KIND_F16X2): taken by every thread of the grid from the Err[n] that
-  // a2 of this iteration wrote (a completed kernel: visible), so issuer and epilogues of both CTAs agree.
-  // (n_iter < 0, loop body of a zfac_graph: the update is taken from the last residual written, State::iters)
-  const bool hh_only = PAIRK && p.hh_only &&
-                       (__ldcg(p.stop.d_err + (p.stop.n_iter >= 0 ? p.stop.n_iter : p.st->iters)) <= p.hh_err_max);
+  const int tiles_pp = SYM ? T * (T + 1) / 2 * NSPLIT : TI * JC;          // 256 x TN pair tiles of ONE problem
+  const int num_tiles = tiles_pp * p.batch;                                // tile t: problem t / tiles_pp
 
   // The two register regimes (setmaxnreg) are two disjoint regions of the kernel: everything a role executes, including
   // its side of the two pair-wide synchronisations, sits inside its own branch (ptxas allocates registers per region
@@ -509,7 +507,14 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
     cluster_sync_all();
   };
 
-  auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
+  // Tile t of the launch -> its problem and position.  m0: first row of the A operand and of the output in the stacked
+  // buffers; n0: first output column (local); mb: first row of the problem (B operand rows start at mb + n0).
+  // Returns false for a tile of a problem that has already stopped (batched launches; every role skips it alike: `done` is
+  // set by the a2 launch that evaluates the problem's last tile, i.e. never while a role still has a tile of it ahead).
+  // hh: one pass for a second-order product (a4 / p2, KIND_F16X2), taken from the Err[n] that a2 of this iteration wrote
+  // for this problem (a completed kernel: visible), so issuer and epilogues of both CTAs agree.  (n_iter < 0, loop body
+  // of a zfac_graph: the update is taken from the last residual written, State::iters.)
+  auto decode_local = [&](int t, int& m0, int& n0, bool& offdiag) {
     int I, J;
     if (SYM) {
       const int macro = t / NSPLIT, sub = t - macro * NSPLIT;
@@ -524,6 +529,18 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       offdiag = true;                                      // (unused by the full-output epilogues)
     }
     m0 = I * UM_TILE_M;
+  };
+  auto decode = [&](int t, int& m0, int& n0, int& mb, int& tl, bool& offdiag, bool& hh) -> bool {
+    const int b = t / tiles_pp;
+    tl = t - b * tiles_pp;
+    if (p.batch > 1 && *((volatile int*)&p.st[b].done)) return false;
+    decode_local(tl, m0, n0, offdiag);
+    mb = b * np;
+    m0 += mb;
+    hh = false;
+    if (PAIRK && p.hh_only)
+      hh = __ldcg(p.stop.d_err + (size_t)b * p.stop.err_stride + (p.stop.n_iter >= 0 ? p.stop.n_iter : p.st[b].iters)) <= p.hh_err_max;
+    return true;
   };
 
   if (warp < UM_EPI_WARP0) {
@@ -549,10 +566,12 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       int stage = 0; uint32_t phase = 0;
       const int aoff = (int)rank * UM_ROWS, boff = (int)rank * (TN / 2);
       for (int t = pair; t < num_tiles; t += num_pairs) {
-        int m0, n0; bool od; decode(t, m0, n0, od);
+        int m0, n0, mb, tl; bool od, hh_only;
+        if (!decode(t, m0, n0, mb, tl, od, hh_only)) continue;
+        n0 += mb;                                              // B operand rows of this problem
         for (int kb = 0; kb < KB; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1u);
-          // one-pass launch of the pair kind (hh_only): the lo' planes are never read -- do not load them
+          // one-pass tile of the pair kind (hh_only): the lo' planes are never read -- do not load them
           const int narr = hh_only ? 1 : KT::ARRAYS;
           if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * (uint32_t)narr * (UM_A_BYTES + B_BYTES));   // both CTAs' boxes
           const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
@@ -564,10 +583,10 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
             if (a >= narr) break;
 #pragma unroll
             for (int b = 0; b < UM_ROWS / UM_BOX_ROWS; ++b)
-              tma_load_2d_pair(sa + a * UM_A_BYTES + b * UM_BOX_BYTES, &p.mapA, kc, a * np + m0 + aoff + b * UM_BOX_ROWS, lead_full);
+              tma_load_2d_pair(sa + a * UM_A_BYTES + b * UM_BOX_BYTES, &p.mapA, kc, a * p.rows + m0 + aoff + b * UM_BOX_ROWS, lead_full);
 #pragma unroll
             for (int b = 0; b < TN / 2 / UM_BOX_ROWS; ++b)
-              tma_load_2d_pair(sb + a * B_BYTES + b * UM_BOX_BYTES, &p.mapB, kc, a * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+              tma_load_2d_pair(sb + a * B_BYTES + b * UM_BOX_BYTES, &p.mapB, kc, a * p.rows + n0 + boff + b * UM_BOX_ROWS, lead_full);
           }
           if (++stage == KT::STAGES) { stage = 0; phase ^= 1u; }
         }
@@ -593,8 +612,11 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
         // small, so the truncation of the FP32 accumulator costs the least there.
         constexpr int FRONT = (KT::STAGES >= 4) ? 2 : 1, BACK = FRONT;
         uint32_t it = 0;                                       // k-block sequence number = position in the smem ring
-        int li = 0;
-        for (int t = pair; t < num_tiles; t += num_pairs, ++li) {
+        int li = -1;                                           // tiles of this pair that are processed (skipped ones do not count)
+        for (int t = pair; t < num_tiles; t += num_pairs) {
+          int m0_, n0_, mb_, tl_; bool od_, hh_only;
+          if (!decode(t, m0_, n0_, mb_, tl_, od_, hh_only)) continue;
+          ++li;
           const int set = (SETS == 2) ? (li & 1) : 0;
           const uint32_t nuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;   // earlier tiles of this set
           const uint32_t d0 = tmem_base + set * SET_COLS, d1 = d0 + TN;
@@ -658,8 +680,11 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
         }
       } else {
         int stage = 0; uint32_t phase = 0;
-        int li = 0;
-        for (int t = pair; t < num_tiles; t += num_pairs, ++li) {
+        int li = -1;
+        for (int t = pair; t < num_tiles; t += num_pairs) {
+          int m0_, n0_, mb_, tl_; bool od_, hh_;
+          if (!decode(t, m0_, n0_, mb_, tl_, od_, hh_)) continue;
+          ++li;
           const int set = (SETS == 2) ? (li & 1) : 0;
           const uint32_t nuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;
           const uint32_t d0 = tmem_base + set * SET_COLS;
@@ -695,7 +720,6 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   } else {
     reg_alloc<UM_REGS_EPILOGUE>();
     const uint32_t tmem_base = pair_sync_in();
-    double cta_sumsq = 0.0;
     // ===================================================== epilogue warps (4 .. 11), both CTAs
     // Group g = warps 4 + 4 g .. 7 + 4 g (one warp per TMEM lane quarter).  SETS == 2: group g owns accumulator
     // set g, i.e. the tiles with local index li = g (mod 2), all TN columns: its stores overlap the other set's
@@ -707,14 +731,16 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
     const int row = (int)rank * UM_ROWS + q * 32 + lane;       // row of the pair tile held by this thread
     const uint32_t lead_hh_empty = mapa_u32(hh_empty_bar(set), 0), lead_tempty = mapa_u32(tempty_bar(set), 0);
     const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + set * SET_COLS + col0;
-    int li = 0;
+    int li = -1;
 #ifdef ZFAC_TIMING
     long long twait[4] = {0, 0, 0, 0};     // 4 wait for MMA (hh_full / tfull), 5 TMEM -> registers, 6 global loads / stores
 #endif
-    for (int t = pair; t < num_tiles; t += num_pairs, ++li) {
+    for (int t = pair; t < num_tiles; t += num_pairs) {
+      int m0, n0, mb, tl; bool offdiag, hh_only;
+      if (!decode(t, m0, n0, mb, tl, offdiag, hh_only)) continue;
+      ++li;
       if (SETS == 2 && (li & 1) != g) continue;
       const uint32_t tuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;   // tiles this thread has finished
-      int m0, n0; bool offdiag; decode(t, m0, n0, offdiag);
       const int m = m0 + row;
       double tile_sumsq = 0.0;
       if (PAIRK) {
@@ -774,7 +800,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
           float v[SUB];
 #pragma unroll
           for (int j = 0; j < SUB; ++j) v[j] = sum[cc * SUB + j];
-          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, offdiag, tile_sumsq);
+          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, mb, offdiag, tile_sumsq);
         }
 #ifdef ZFAC_TIMING
         twait[1] += te1 - te0; twait[2] += clock64() - te1;
@@ -792,33 +818,22 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 #pragma unroll
             for (int j = 0; j < SUB; ++j) v[j] = __uint_as_float(r[j]);
           }
-          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, offdiag, tile_sumsq);
+          epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, mb, offdiag, tile_sumsq);
         }
         tc_fence_before();
         __syncwarp();
         mbar_arrive_cluster_lane0(lead_tempty, lane);            // frees the accumulator set
       }
-      if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
+      // step a3: this warp's share of the tile (slot: CTA of the pair x warp of the tile's epilogue group(s))
+      if (EPI == EPI_A2)
+        stop_test_tile_warp(p.stop, mb / np, tl, (int)rank * (UM_EPI_WARPS / SETS) + ((SETS == 2) ? q : (warp - UM_EPI_WARP0)),
+                            offdiag ? 2.0 * tile_sumsq : tile_sumsq, lane);
     }
 #ifdef ZFAC_TIMING
     if (p.dbg && rank == 0 && warp == UM_EPI_WARP0 && lane == 0)
       for (int i = 0; i < 3; ++i) atomicAdd(p.dbg + (size_t)(EPI * 148 + pair) * 8 + 4 + i, (unsigned long long)twait[i]);
 #endif
-    if (EPI == EPI_A2) {
-      const double s = warp_sum(cta_sumsq);
-      if (lane == 0) red[warp] = s;
-    }
     pair_sync_out();
-  }
-
-  // ------------------------------------------------------- step a3 for a2 (all threads)
-  if (EPI == EPI_A2) {
-    if (threadIdx.x == 0) {
-      double tot = 0.0;
-      for (int w = UM_EPI_WARP0; w < UM_EPI_WARP0 + UM_EPI_WARPS; ++w) tot += red[w];
-      p.stop.partials[blockIdx.x] = tot;
-    }
-    if (arrive_is_last(&p.st->arrive[0], gridDim.x, &last_flag)) stop_test_last_cta(p.stop, red);
   }
 }
 
@@ -891,7 +906,7 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   const uint64_t np = (uint64_t)L.np;
   if (L.mode == ZFAC_MODE_SPLIT16 || L.mode == ZFAC_MODE_HH16) {
     const CUtensorMapDataType H = CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
-    const uint64_t rows = (L.mode == ZFAC_MODE_SPLIT16 ? 2 : 1) * np;
+    const uint64_t rows = (L.mode == ZFAC_MODE_SPLIT16 ? 2 : 1) * (uint64_t)L.rows;
     if ((e = make_map(enc, &pl->mS, ws + L.off_S, H, 2, rows, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mW, ws + L.off_W, H, 2, rows, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mT, ws + L.off_T, H, 2, rows, np)) != cudaSuccess) return e;
@@ -903,13 +918,14 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if (e != cudaSuccess) return e;
   } else {
     const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    if ((e = make_map(enc, &pl->mS, ws + L.off_S, F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mW, ws + L.off_W, F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mT, ws + L.off_T, F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mR, ws + L.off_R, F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mQ, ws + L.off_Q, F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Z[0], F, 4, np, np)) != cudaSuccess) return e;
-    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Z[1], F, 4, np, np)) != cudaSuccess) return e;
+    const uint64_t rows = (uint64_t)L.rows;
+    if ((e = make_map(enc, &pl->mS, ws + L.off_S, F, 4, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mW, ws + L.off_W, F, 4, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mT, ws + L.off_T, F, 4, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mR, ws + L.off_R, F, 4, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mQ, ws + L.off_Q, F, 4, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Z[0], F, 4, rows, np)) != cudaSuccess) return e;
+    if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Z[1], F, 4, rows, np)) != cudaSuccess) return e;
     if ((e = prepare_kind<KIND_TF32>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
   }
   if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
@@ -954,19 +970,21 @@ struct UmmaSeq {
     const int T = (int)(L.np / UM_MACRO);
     const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
                                    : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
-    const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
+    const int full_tiles = T * T * nsplit * L.batch, sym_tiles = T * (T + 1) / 2 * nsplit * L.batch;
     grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
     grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());
     order = order_;
     nsplit_ = nsplit;
-    p.np = (int)L.np; p.macro_tiles = T; p.band = pl.opt->band;
+    p.np = (int)L.np; p.batch = L.batch; p.rows = (int)L.rows; p.macro_tiles = T; p.band = pl.opt->band;
     p.st = reinterpret_cast<State*>(ws + L.off_state);
 #ifdef ZFAC_TIMING
     p.dbg = reinterpret_cast<unsigned long long*>(ws + L.off_dbg);
 #endif
     p.stop.st = p.st; p.stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
-    p.stop.num_partials = grid_sym; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
+    p.stop.num_partials = 0; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
     p.stop.order = order; p.stop.cond = cond;
+    p.stop.tiles_pp = T * (T + 1) / 2 * nsplit; p.stop.err_stride = (long long)max_iter + 1;
+    p.stop.slots_pt = 2 * UM_EPI_WARPS / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::SETS : KindTraits<KIND_HH16>::SETS);
     const PolyCoef pc = poly_coef(order);
     p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.g_i = (float)pc.g_i; p.g_r = (float)pc.g_r; p.g_p = (float)pc.g_p;
     R32 = reinterpret_cast<float*>(ws + L.off_R);
@@ -1103,7 +1121,8 @@ inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* laun
   const int grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
   const int grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());
   UmmaParams p{};
-  p.np = (int)L.np; p.macro_tiles = T; p.band = pl.opt->band; p.chunk_kb = pl.opt->chunk_kb; p.chunk0_kb = pl.opt->chunk0_kb;
+  p.np = (int)L.np; p.batch = 1; p.rows = (int)L.np; p.macro_tiles = T; p.band = pl.opt->band;
+  p.chunk_kb = pl.opt->chunk_kb; p.chunk0_kb = pl.opt->chunk0_kb;
   p.st = reinterpret_cast<State*>(ws + L.off_state);
   const bool h16 = (L.mode != ZFAC_MODE_TF32);
   p.mapA = pl.mW; p.mapB = pl.mS;

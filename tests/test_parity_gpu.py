@@ -1313,3 +1313,62 @@ def test_config4_full_size_n8192_bench_workload():
     assert zzt <= TOL["split16"]                                         # north_star's split gate on the unique quantity
     assert rel <= 1e-4
     assert err[-1] == pytest.approx(inv * math.sqrt(w.n), rel=1e-2, abs=1e-10)
+
+
+# ------------------------------------------------------------------ batched small problems in one launch sequence
+@pytest.mark.parametrize("mode", ["split16", "hh16", "tf32"])
+@pytest.mark.parametrize("n,batch", [(130, 3), (300, 7), (520, 16), (1024, 5)])
+def test_batched_launch_is_bitwise_the_solo_runs(mode, n, batch):
+    """zfac_refine_batched: `batch` different problems -- different conditioning, different starts, hence different stop
+    indices, one of them non-finite -- refined by ONE launch sequence whose kernels walk the tiles of all problems.
+    Every problem must come out bit for bit as from its own zfac_refine call (Z, iters, Err[], flags): the per-problem
+    stop test, the skipping of finished problems and the stacked operand layout may not change a single rounding.
+    Also with order m = 3 and with batch strides larger than n * n."""
+    b = zb()
+    ws = [W.random_spd_general(n, seed=1000 + 17 * i + n, kappa=[8.0, 40.0, 150.0][i % 3], pert=[0.02, 0.1, 0.2][(i // 3) % 3],
+                               fp32_stored=True) for i in range(batch)]
+    S = torch.zeros((batch, n, n + 3), dtype=torch.float32, device=DEV)[:, :, :n]
+    Z0 = torch.zeros((batch + 1, n, n), dtype=torch.float32, device=DEV)[:batch]
+    for i, w in enumerate(ws):
+        S[i] = _to_dev(w.S, mode); Z0[i] = _to_dev(w.Z0, mode)
+    bad = batch - 1
+    Z0[bad, 2, 3] = float("nan")                                         # one problem fails at n = 0; the others must not care
+    for order in (2, 3):
+        with b.ZfacBatched(n, mode, batch, DEV) as zbt:
+            zbt.set_order(order)
+            res = zbt.refine(S, Z0, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+            launches = zbt.last_launch_count
+        stops = set()
+        with b.Zfac(n, mode, DEV) as zf:
+            zf.set_order(order)
+            for i in range(batch):
+                Zs, its, errs, fls = zf.refine(S[i], Z0[i], max_iter=30, stop=b.ZFAC_STOP_PAPER)
+                Zb_, itb, errb, flb = res[i]
+                assert itb == its and flb == fls, (i, order)
+                assert np.array_equal(errb, errs, equal_nan=True), (i, order)
+                assert torch.equal(torch.nan_to_num(Zb_, nan=-9.0), torch.nan_to_num(Zs, nan=-9.0)), (i, order)
+                stops.add(its)
+            assert launches == zf.last_launch_count                      # one launch sequence for the whole batch
+        assert res[bad][1] == 0 and (res[bad][3] & b.ZFAC_R_NONFINITE)
+        assert len(stops) >= 2                                           # the problems really stop at different indices
+    # parity of one of them against the oracle (the solo path is covered everywhere else)
+    ref = O.refine(ws[0].S, ws[0].Z0, res[0][1], O.STOP_FIXED, order=3)
+    assert _rel(res[0][0].cpu().double().numpy(), ref.Z) <= (2.5e-3 if n < 32 else TOL[mode])
+
+
+def test_batched_context_argument_checks():
+    b = zb()
+    assert b.zfac_workspace_bytes_batched(256, b.ZFAC_MODE_F64, 4) == 0          # tcgen05 modes only
+    assert b.zfac_workspace_bytes_batched(256, b.ZFAC_MODE_SPLIT16, 0) == 0
+    assert b.zfac_workspace_bytes_batched(256, b.ZFAC_MODE_SPLIT16, 4) > 3 * b.zfac_workspace_bytes(256, b.ZFAC_MODE_SPLIT16) // 2
+    with b.ZfacBatched(100, "split16", 2, DEV) as zbt:
+        assert b.zfac_get_batch(zbt.ctx) == 2
+        S = torch.eye(100, device=DEV).repeat(2, 1, 1)
+        d_i = torch.zeros(2, dtype=torch.int32, device=DEV); d_e = torch.zeros(2, 6, dtype=torch.float64, device=DEV)
+        with pytest.raises(b.ZfacError) as e:                                    # unbatched entry points refuse a batched context
+            b.zfac_refine(zbt.ctx, S.data_ptr(), 100, S.data_ptr(), 100, S.data_ptr(), 100, 5, 0, d_i.data_ptr(), d_e.data_ptr(), d_i.data_ptr())
+        assert e.value.status == b.ZFAC_E_INVALID
+        with pytest.raises(b.ZfacError) as e:                                    # overlapping problems
+            b.zfac_refine_batched(zbt.ctx, S.data_ptr(), 100, 50, S.data_ptr(), 100, 10000, S.data_ptr(), 100, 10000, 5, 0,
+                                  d_i.data_ptr(), d_e.data_ptr(), d_i.data_ptr())
+        assert e.value.status == b.ZFAC_E_INVALID
