@@ -266,6 +266,30 @@ def run_sweep(args, dev, peaks):
                         "ms_per_problem": ms, "tflops_fp32_equiv_aggregate": flops_fp32_equiv(n, 10) / (ms * 1e-3) / 1e12,
                         "speedup_vs_alone": row["modes"][mode]["ms_per_call"] / ms}
                 del S, Z0
+            # ... and as ONE launch sequence over all problems (zfac_refine_batched): B problems stacked in one context
+            row["batched"] = {}
+            for mode in ("split16", "hh16"):
+                S1 = torch.from_numpy(w.S).to(dev, torch.float32); Z1 = torch.from_numpy(w.Z0).to(dev, torch.float32)
+                for B in (16, 64):
+                    if n * n * B * 48 > 40e9:
+                        continue
+                    Sb = S1.repeat(B, 1, 1).contiguous(); Zb0 = Z1.repeat(B, 1, 1).contiguous(); Ob = torch.empty_like(Zb0)
+                    with zb.ZfacBatched(n, mode, B, dev) as zt:
+                        for _ in range(2):
+                            zt.refine(Sb, Zb0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=Ob, sync=False)
+                        torch.cuda.synchronize(dev)
+                        reps = 8
+                        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        for _ in range(reps):
+                            zt.refine(Sb, Zb0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=Ob, sync=False)
+                        e1.record(); torch.cuda.synchronize(dev)
+                        ms = e0.elapsed_time(e1) / (reps * B)
+                    row["batched"][f"{mode}_B{B}"] = {
+                        "ms_per_problem": ms, "tflops_fp32_equiv_aggregate": flops_fp32_equiv(n, 10) / (ms * 1e-3) / 1e12,
+                        "speedup_vs_alone": row["modes"][mode]["ms_per_call"] / ms}
+                    del Sb, Zb0, Ob
+                del S1, Z1
         for dtn, dt in (("f32", torch.float32), ("f64", torch.float64)):
             try:
                 Sd = torch.from_numpy(w.S).to(dev, dt)
