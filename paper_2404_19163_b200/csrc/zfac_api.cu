@@ -387,8 +387,8 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
     if (i8) {
       int* eS = reinterpret_cast<int*>(ws + L.off_exp);
       int8_t* S8 = reinterpret_cast<int8_t*>(ws + L.off_S8);
-      if (in_f32) slice_rows_kernel<float><<<(unsigned)L.np, 256, 0, s>>>(static_cast<const float*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
-      else slice_rows_kernel<double><<<(unsigned)L.np, 256, 0, s>>>(static_cast<const double*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
+      if (in_f32) slice_rows_kernel<float><<<small_grid((size_t)L.np), 256, 0, s>>>(static_cast<const float*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
+      else slice_rows_kernel<double><<<small_grid((size_t)L.np), 256, 0, s>>>(static_cast<const double*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
       MixSeq q(c->mix, 0, 0, nullptr, 0ull);
       q.w_slices(s);
       c->launches += 1 + q.nl;

@@ -39,23 +39,27 @@ __global__ void __launch_bounds__(256) r_split_kernel(const Tin* __restrict__ R,
   if (*((volatile int*)&st->done)) return;
   const double sc = pick_rscale(d_err[n_iter >= 0 ? n_iter : st->iters]);
   if (blockIdx.x == 0 && threadIdx.x == 0) { st->rscale = (float)sc; st->rinv = (float)(1.0 / sc); }
-  const size_t o = ((size_t)blockIdx.x * 256 + threadIdx.x) * 8;
-  if (o >= np2) return;
-  float v[8];
+  // grid-stride over groups of 8 elements: the grid is a few CTAs per SM, so that the statically enqueued launches after
+  // the stop return in microseconds (a grid of Np^2 / 2048 CTAs that all exit at once still took 80 us at N = 8192)
+  for (size_t o = ((size_t)blockIdx.x * 256 + threadIdx.x) * 8; o < np2; o += (size_t)gridDim.x * 256 * 8) {
+    float v[8];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) v[j] = (float)((double)R[o + j] * sc);
-  *reinterpret_cast<float4*>(R32s + o) = make_float4(v[0], v[1], v[2], v[3]);
-  *reinterpret_cast<float4*>(R32s + o + 4) = make_float4(v[4], v[5], v[6], v[7]);
-  uint32_t hi[4], lo[4];
+    for (int j = 0; j < 8; ++j) v[j] = (float)((double)R[o + j] * sc);
+    *reinterpret_cast<float4*>(R32s + o) = make_float4(v[0], v[1], v[2], v[3]);
+    *reinterpret_cast<float4*>(R32s + o + 4) = make_float4(v[4], v[5], v[6], v[7]);
+    uint32_t hi[4], lo[4];
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    __half h0, l0, h1, l1;
-    split_f16(v[2 * j], h0, l0); split_f16(v[2 * j + 1], h1, l1);
-    hi[j] = pack_h2(h0, h1); lo[j] = pack_h2(l0, l1);
+    for (int j = 0; j < 4; ++j) {
+      __half h0, l0, h1, l1;
+      split_f16(v[2 * j], h0, l0); split_f16(v[2 * j + 1], h1, l1);
+      hi[j] = pack_h2(h0, h1); lo[j] = pack_h2(l0, l1);
+    }
+    *reinterpret_cast<uint4*>(Rb + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(Rb + np2 + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
   }
-  *reinterpret_cast<uint4*>(Rb + o) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-  *reinterpret_cast<uint4*>(Rb + np2 + o) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
 }
+// Grid of the O(N^2) helper kernels: enough CTAs to fill the device, few enough to exit at once.
+inline unsigned small_grid(size_t work_items, unsigned cap = 148 * 8) { return (unsigned)(work_items < cap ? (work_items ? work_items : 1) : cap); }
 
 // FP32[Z64] as the (hi, lo') operand pair of the first update (later ones are written by a5x's epilogue).
 __global__ void __launch_bounds__(256) z_planes_kernel(const double* __restrict__ Z, __half* __restrict__ Zb, size_t np2, State* st) {
@@ -122,7 +126,8 @@ __global__ void __launch_bounds__(256) slice_rows_kernel(const Tin* __restrict__
   if (*((volatile int*)&st->done)) return;
   __shared__ double red[8];
   __shared__ int e_sh;
-  const int r = blockIdx.x, t = threadIdx.x;
+  const int t = threadIdx.x;
+  for (int r = blockIdx.x; r < np; r += gridDim.x) {
   double mx = 0.0;
   if (r < n) {
     for (int c = t; c < n; c += 256) mx = fmax(mx, fabs((double)src[(size_t)r * ld + c]));
@@ -151,6 +156,8 @@ __global__ void __launch_bounds__(256) slice_rows_kernel(const Tin* __restrict__
     }
     slice16(a, e, slices, out, plane, (size_t)r * np + c0, st);
   }
+  __syncthreads();                                             // red / e_sh are reused by the next row
+  }
 }
 
 // W = Z^T: the rows of W are the COLUMNS of Z.  Column maxima first (one CTA per 32 columns) ...
@@ -173,7 +180,9 @@ __global__ void __launch_bounds__(256) slice_transpose_kernel(const double* __re
                                                               const int* __restrict__ exps, State* st) {
   if (*((volatile int*)&st->done)) return;
   __shared__ double tile[64][65];
-  const int r0 = blockIdx.y * 64, c0 = blockIdx.x * 64, t = threadIdx.x;
+  const int t = threadIdx.x, tn = np / 64;
+  for (int tt = blockIdx.x; tt < tn * tn; tt += gridDim.x) {
+  const int r0 = (tt / tn) * 64, c0 = (tt % tn) * 64;
 #pragma unroll
   for (int i = 0; i < 16; ++i) {
     const int idx = t + 256 * i, lr = idx >> 6, lc = idx & 63;
@@ -185,6 +194,8 @@ __global__ void __launch_bounds__(256) slice_transpose_kernel(const double* __re
 #pragma unroll
   for (int j = 0; j < 16; ++j) a[j] = tile[kc + j][wc];
   slice16(a, exps[c0 + wc], slices, out, (size_t)np * np, (size_t)(c0 + wc) * np + r0 + kc, st);
+  __syncthreads();
+  }
 }
 
 // ------------------------------------------------------------------ the INT8 GEMM (Ozaki scheme on tcgen05)
@@ -546,7 +557,7 @@ struct MixSeq {
       p.mapA = pl.mW8; p.mapB = pl.mS8; p.expA = eW; p.expB = eS; p.out64 = reinterpret_cast<double*>(ws + L.off_T);
       if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
       i8_gemm_kernel<EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
-      slice_rows_kernel<double><<<(unsigned)L.np, 256, 0, s>>>(p.out64, L.np, (int)L.np, (int)L.np, p.orders,
+      slice_rows_kernel<double><<<small_grid((size_t)L.np), 256, 0, s>>>(p.out64, L.np, (int)L.np, (int)L.np, p.orders,
                                                                  reinterpret_cast<int8_t*>(ws + L.off_T8), eT, st);
       // a2: R = I - W T^T (FP32 out, both triangles), sum R^2, stop test
       p.mapA = pl.mW8; p.mapB = pl.mT8; p.expA = eW; p.expB = eT; p.out64 = nullptr; p.out32 = reinterpret_cast<float*>(ws + L.off_R);
@@ -559,7 +570,7 @@ struct MixSeq {
   void update(int par, int n_stop, int tagn, cudaStream_t s, Prof* prof, const IterHook* = nullptr, int = 1) {
     const Layout& L = pl.L;
     char* ws = pl.ws;
-    const unsigned g8 = (unsigned)((np2 / 8 + 255) / 256);
+    const unsigned g8 = small_grid((np2 / 8 + 255) / 256);
     __half* Rb = reinterpret_cast<__half*>(ws + L.off_Rb);
     if (prof) prof->mark(s, EPI_A4 + 16 * tagn);
     if (L.mode == ZFAC_MODE_F64_MIXED)
@@ -593,8 +604,7 @@ struct MixSeq {
     int* eW = reinterpret_cast<int*>(ws + L.off_exp) + L.np;
     const double* Z = reinterpret_cast<const double*>(ws + L.off_Z[0]);
     colmax_kernel<<<(unsigned)(L.np / 32), 256, 0, s>>>(Z, (int)L.np, eW, st);
-    dim3 g((unsigned)(L.np / 64), (unsigned)(L.np / 64));
-    slice_transpose_kernel<<<g, 256, 0, s>>>(Z, (int)L.np, pl.opt->i8_slices, reinterpret_cast<int8_t*>(ws + L.off_W8), eW, st);
+    slice_transpose_kernel<<<small_grid((size_t)(L.np / 64) * (size_t)(L.np / 64)), 256, 0, s>>>(Z, (int)L.np, pl.opt->i8_slices, reinterpret_cast<int8_t*>(ws + L.off_W8), eW, st);
     nl += 2;
   }
 };
