@@ -290,6 +290,44 @@ def run_sweep(args, dev, peaks):
                         "speedup_vs_alone": row["modes"][mode]["ms_per_call"] / ms}
                     del Sb, Zb0, Ob
                 del S1, Z1
+        # The paper's fastest scheme, (h)(h) + refi with a single-precision refinement (Fig. 3), and
+        # its relatives: the low-precision mode to ITS stop (paper rule), then refinement updates in the more precise mode;
+        # next to each mode alone run to its own stop.  Residuals evaluated by the oracle (N <= 8192).
+        if not args.sweep_no_refi:
+            from oracle import zfac_oracle as O
+            S32 = torch.from_numpy(w.S).to(dev, torch.float32); Z32 = torch.from_numpy(w.Z0).to(dev, torch.float32)
+            row["stop_rule_paths"] = {}
+            specs = [("hh16", None, 0), ("hh16", "split16", 1), ("hh16", "split16", 2), ("tf32", "split16", 2),
+                     ("split16", None, 0), ("split16", "f64i8", 1)]
+            for low, high, steps in specs:
+                name = low if high is None else f"{low}+{steps}x{high}"
+                try:
+                    hdt = torch.float64 if high in F64_MODES else torch.float32
+                    Zr = torch.empty((n, n), dtype=hdt, device=dev)
+                    zl = zb.Zfac(n, low, dev); zh = zb.Zfac(n, high, dev) if high else None
+                    try:
+                        if high:
+                            call = lambda: zl.refine_refi(zh, S32, Z32, max_iter=40, refi_steps=steps, final_check=False, out=Zr, sync=False)
+                        else:
+                            call = lambda: zl.refine(S32, Z32, max_iter=40, stop=zb.ZFAC_STOP_PAPER, out=Zr, sync=False)
+                        call(); torch.cuda.synchronize(dev)
+                        ts = []
+                        for _ in range(3 if n >= 8192 else 7):
+                            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                            e0.record(); _, d_it, d_err, d_fl = call(); e1.record(); torch.cuda.synchronize(dev)
+                            ts.append(e0.elapsed_time(e1))
+                    finally:
+                        zl.close()
+                        if zh:
+                            zh.close()
+                    ent = {"ms": float(np.median(ts)), "updates": int(d_it.item()), "flags": int(d_fl.item())}
+                    if n <= 8192:
+                        ent["residual_per_sqrt_n_oracle"] = O.final_residual_per_sqrt_n(w.S, Zr.cpu().double().numpy())
+                    row["stop_rule_paths"][name] = ent
+                    del Zr
+                except Exception as ex_:
+                    row["stop_rule_paths"][name] = {"error": str(ex_)[:100]}
+            del S32, Z32
         for dtn, dt in (("f32", torch.float32), ("f64", torch.float64)):
             try:
                 Sd = torch.from_numpy(w.S).to(dev, dt)
@@ -807,6 +845,7 @@ def main():
     ap.add_argument("--sweep", action="store_true",
                     help="also run the N sweep of BASELINE.json configs[4] (all modes, 10 fixed updates, syevd reference)")
     ap.add_argument("--sweep-n", default="1024,2048,4096,8192,16384")
+    ap.add_argument("--sweep-no-refi", action="store_true", help="sweep: skip the stop-rule / Alg. 3 paths")
     ap.add_argument("--sweep-batch-max-n", type=int, default=2048,
                     help="sweep: also time B = 4, 8, 16 concurrent problems (ZfacBatch) for N up to this")
     args = ap.parse_args()
