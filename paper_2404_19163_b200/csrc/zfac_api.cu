@@ -293,6 +293,7 @@ struct F64Seq {
     if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
     f64_tma_launch(EPI_A2, tri, s, P);
     c->launches += 2;
+    if (p.stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(p.st, p.stop.cond);       // zfac_graph_*: loop condition
   }
   void update(int par, int n_stop, int tagn, cudaStream_t s, Prof* prof) {
     const F64Plan& fp = c->f64p;

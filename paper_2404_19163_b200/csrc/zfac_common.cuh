@@ -50,7 +50,7 @@ struct StopArgs {
   int max_iter;
   int stop;                  // zfac_stop
   int order;                 // m of Eq. 13 (2, 3, 4): the test's exponent is nu_max = m + 1
-  unsigned long long cond;   // zfac_graph_*: handle of the WHILE node's condition, set to "not done" by the stop test (0: none)
+  unsigned long long cond;   // zfac_graph_*: handle of the WHILE node's condition (0: none); set by graph_cond_kernel after a2
   // tcgen05 kernels (one launch may carry `batch` independent problems): `st` is an array of one State per problem, the
   // partials hold 16 sums per a2 tile (8 epilogue warps x 2 CTAs), tiles_pp a2 tiles per problem, and d_err is
   // [batch][err_stride]
@@ -118,7 +118,13 @@ __device__ inline void stop_decide(const StopArgs& a, State* st, double* d_err, 
   }
   if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
   if (done) { st->flags |= flags; __threadfence(); st->done = 1; }
-  if (a.cond) cudaGraphSetConditional((cudaGraphConditionalHandle)a.cond, done ? 0u : 1u);   // another pass of the loop?
+}
+
+// zfac_graph_*: the WHILE node's condition (another pass of the loop?) is set by this one-thread kernel right after every a2.
+// It is a kernel of its own because cudaGraphSetConditional is a device-runtime CALL: a call anywhere in a kernel makes
+// ptxas ignore setmaxnreg there (the a2 kernels ran all warps at the 168-register launch cap and spilled).
+__global__ void graph_cond_kernel(const State* st, unsigned long long cond) {
+  cudaGraphSetConditional((cudaGraphConditionalHandle)cond, st->done ? 0u : 1u);
 }
 
 // Step a3 in the tcgen05 kernels: every epilogue warp leaves the sum of squares of its 32 rows x 128 / 256 columns of an

@@ -543,6 +543,7 @@ struct MixSeq {
       if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
       f64_tma_launch(EPI_A2, tiles * (tiles + 1) / 2, s, P);
       nl += 2;
+      if (stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(st, stop.cond);
     } else {
       I8Params p{};
       // rasterisation band of the full GEMM: half the width of the fp16 kernels' (their operand rows are twice as long in
@@ -564,6 +565,7 @@ struct MixSeq {
       if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
       i8_gemm_kernel<EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
       nl += 3;
+      if (stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(st, stop.cond);
     }
   }
 

@@ -1031,6 +1031,7 @@ struct UmmaSeq {
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
     umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
     nl += 1;
+    if (p.stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(p.st, p.stop.cond);       // zfac_graph_*: loop condition
   }
 
   // (p2,) a4, a5: update number n with n & 1 = par, taken from residual n_stop (-1: device-side index)
