@@ -257,6 +257,10 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *   ZFAC_OPT_I8_SLICES       F64_I8: int8 slices per operand row = orders i + j kept, 2 .. 8 (7 bits each)              8
  *   ZFAC_OPT_INPUT_F32       F64, F64_MIXED, F64_I8: S and Z0 are given as FLOAT ("FP32 stored" inputs, promoted exactly);
  *                            Z is still returned as double; 0 / 1                                                   0
+ *   ZFAC_OPT_EXTRA_UPDATE    F64_MIXED, F64_I8 with ZFAC_STOP_PAPER: when the test fires, perform ONE more update (flag
+ *                            ZFAC_R_REFINED) and stop after its residual.  The FP32-class correction of these modes makes the
+ *                            test also fire when Err has only reached ~2^-22 sqrt(kappa) Err[n-1], one update short of the
+ *                            FP64 floor (cold starts); this is Alg. 3's single refinement step, built in; 0 / 1               0
  *   The rest change scheduling only (bit-identical results):
  *   ZFAC_OPT_BAND            full GEMMs: tile columns per rasterisation band, 1 .. 4096                               8
  *   ZFAC_OPT_MAX_PAIRS       tensor-core modes: use at most this many CTA pairs; 0 = all co-resident ones            0
@@ -264,7 +268,8 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
 typedef enum {
   ZFAC_OPT_CHUNK_KB = 0, ZFAC_OPT_CHUNK0_KB = 1, ZFAC_OPT_HH_SQUARE = 2, ZFAC_OPT_HH_SQUARE_ERR = 3,
   ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
-  ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10, ZFAC_OPT_INPUT_F32 = 11
+  ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10, ZFAC_OPT_INPUT_F32 = 11,
+  ZFAC_OPT_EXTRA_UPDATE = 12
 } zfac_option;
 zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
 zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);

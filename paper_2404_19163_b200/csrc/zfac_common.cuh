@@ -38,6 +38,7 @@ struct Options {
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
+  int extra_update = 0;      // FP64-master modes: one more update after the paper's test has fired (see stop_decide)
   int input_f32 = 0;         // double-element modes: S and Z0 are float (promoted exactly), Z is returned as double
 };
 
@@ -54,6 +55,7 @@ struct StopArgs {
   // tcgen05 kernels (one launch may carry `batch` independent problems): `st` is an array of one State per problem, the
   // partials hold 16 sums per a2 tile (8 epilogue warps x 2 CTAs), tiles_pp a2 tiles per problem, and d_err is
   // [batch][err_stride]
+  int extra;                 // FP64-master modes, ZFAC_OPT_EXTRA_UPDATE: when the test fires, perform ONE more update, then stop
   int tiles_pp;
   int slots_pt;              // partial sums per tile: 16 (SPLIT16: both epilogue groups work on a tile) or 8 (one-pass kinds)
   long long err_stride;
@@ -115,6 +117,14 @@ __device__ inline void stop_decide(const StopArgs& a, State* st, double* d_err, 
     double thr = prev * prev * prev;                         // m = 2: Err[n-1]^3 (Eq. 38)
     for (int k = 2; k < a.order; ++k) thr *= prev;           // m = 3, 4: Err[n-1]^(m+1)
     if (err > thr) { flags = ZFAC_R_STOPPED; done = 1; }
+    // ZFAC_OPT_EXTRA_UPDATE (FP64-master modes): the correction of these modes is FP32-class, so the test also fires when the
+    // residual has merely reached ~u32 sqrt(kappa) Err[n-1], one update short of the FP64 floor.  Like the refinement step of
+    // Alg. 3 ("Typically we would only do one extra refinement step"), the first firing is answered by ONE
+    // more update (marked ZFAC_R_REFINED); the evaluation after it ends the run.
+    if (a.extra) {
+      if (st->flags & ZFAC_R_REFINED) { flags = ZFAC_R_STOPPED; done = 1; }
+      else if (done) { st->flags |= ZFAC_R_REFINED; flags = 0; done = 0; }
+    }
   }
   if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
   if (done) { st->flags |= flags; __threadfence(); st->done = 1; }

@@ -521,7 +521,7 @@ struct MixSeq {
     grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());
     st = reinterpret_cast<State*>(ws + L.off_state);
     stop.st = st; stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
-    stop.d_err = d_err; stop.max_iter = max_iter; stop.stop = stop_rule; stop.order = 2; stop.cond = cond;
+    stop.d_err = d_err; stop.max_iter = max_iter; stop.stop = stop_rule; stop.order = 2; stop.cond = cond; stop.extra = pl.opt->extra_update;
     R32s = reinterpret_cast<float*>(ws + L.off_R32);
     np2 = (size_t)L.np * (size_t)L.np;
   }

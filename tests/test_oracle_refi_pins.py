@@ -150,3 +150,22 @@ def test_alg2_with_mixed_update_converges_to_the_fp64_floor_one_iteration_late_a
     assert np.linalg.norm(mixed.Z - full.Z) / np.linalg.norm(full.Z) < 1e-6
     with pytest.raises(ValueError):
         O.refine(w.S, w.Z0, 5, order=3, update_dtype=np.float32)
+
+
+def test_mixed_update_makes_the_papers_test_fire_one_update_short_of_the_fp64_floor_on_a_cold_start():
+    """What ZFAC_OPT_EXTRA_UPDATE (include/zfac.h) is for, on the oracle's own model of the FP64-master update.  From a
+    cold start at kappa = 1e5 the last cubic step goes from Err ~ 3e-4 to the u ||R|| sqrt(kappa)-class term the float32
+    correction leaves (pinned above), which is ABOVE Err^3: the test of Alg. 2 fires there, one update before
+    the all-FP64 run stops, with an invariant ~1e2-1e3 times the FP64 floor.  One more mixed update -- Alg. 3's single
+    refinement step -- lands on the floor."""
+    w = W.spectral_workload(300, 1e-5, 1.0, seed=0)
+    full = O.refine(w.S, w.Z0, 40, O.STOP_PAPER)
+    mixed = O.refine(w.S, w.Z0, 40, O.STOP_PAPER, update_dtype=np.float32)
+    assert mixed.iters == full.iters - 1 and (mixed.flags & O.R_STOPPED)
+    k = mixed.iters
+    assert mixed.err[k] > mixed.err[k - 1] ** 3                          # the test fired ...
+    assert mixed.err[k] < 1e-4 * mixed.err[k - 1]                        # ... on a residual that had just dropped 1e4-fold
+    f_m, f_f = (_fro_residual(w.S, r.Z) / math.sqrt(w.n) for r in (mixed, full))
+    assert f_m > 50.0 * f_f and f_m < 1e-8
+    Z1 = O.update_mixed(mixed.Z, O.residual(w.S, mixed.Z), np.float32)
+    assert _fro_residual(w.S, Z1) / math.sqrt(w.n) < 3.0 * f_f

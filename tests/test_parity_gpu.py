@@ -31,7 +31,8 @@ ERR_ABS_MIN = 1e-12
 # KNOWN FLOOR (not a widened gate): SPLIT16 accumulates in FP32; its error of Z is ~u kappa (with a native
 # FP32 control on the same GPU).  Where kappa N puts that floor above the north_star gate 1e-5, the raw SPLIT16 run is
 # held to the floor named here and the GATE itself is asserted on the path that can meet it: SPLIT16 + the refinement
-# step of Alg. 3 (test_config4_full_size_n8192_bench_workload, test_time_to_gate_paths_config5_n8192).
+# step of Alg. 3 and the FP64-master modes (test_config4_full_size_n8192_bench_workload here;
+# tests/test_mix_gpu.py: test_time_to_gate_path_config4_n8192_f64i8_float_inputs, test_config3_full_size_n4617_f64i8_...).
 FLOOR_CONFIG5_N8192 = 5e-5        # kappa = 1e3, N = 8192: measured 4.4e-5 (native FP32: 5.0e-5)
 FLOOR_KAPPA_1E5 = 5e-3            # kappa = 1e5 (configs 3, 4): measured 2.4e-4 .. 3.8e-4 (native FP32: 3.6e-4)
 
