@@ -87,6 +87,7 @@ enum {
   ZFAC_R_MAXITER = 2,  /* max_iter updates were performed without the test firing               */
   ZFAC_R_NONFINITE = 4, /* Err[n] became inf/NaN; iteration stopped                              */
   ZFAC_R_REFINED = 8,   /* zfac_refine_refi: at least one refinement update was applied          */
+  ZFAC_R_NOCHECK = 32,  /* ZFAC_OPT_FINAL_CHECK = 0: the residual of the last update was not evaluated (Err[iters] is NaN) */
   ZFAC_R_RANGE = 16     /* SPLIT16 / HH16: a value of S, Z0, T = (S Z)^T or Z with magnitude >= 65504 was clamped when it
                            was rounded to an FP16 operand (FP16 range); the result is not to be trusted.  Admissible input:
                            abs(S_ij), abs(Z_ij), abs((S Z)_ij) < 65504 throughout -- e.g. lambda_min(S) >~ 3e-10 for a
@@ -261,6 +262,12 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *                            ZFAC_R_REFINED) and stop after its residual.  The FP32-class correction of these modes makes the
  *                            test also fire when Err has only reached ~2^-22 sqrt(kappa) Err[n-1], one update short of the
  *                            FP64 floor (cold starts); this is Alg. 3's single refinement step, built in; 0 / 1               0
+ *   ZFAC_OPT_FINAL_CHECK     F64_MIXED, F64_I8 with ZFAC_STOP_PAPER: 1 = Alg. 2 as printed, every update is followed by its
+ *                            residual.  0 = a residual whose stop decision is known beforehand is not evaluated: the one
+ *                            after an update taken from Err[n]^3 < 2^-53 sqrt(N) (the test is bound to fire), or, with
+ *                            ZFAC_OPT_EXTRA_UPDATE, the one after the extra update.  Same Z, bit for bit, and same iteration
+ *                            count as with 1 whenever that run ends by the test; Err[iters] = NaN, flag ZFAC_R_NOCHECK;
+ *                            saves one residual (a1 + a2) per call; 0 / 1                                              1
  *   The rest change scheduling only (bit-identical results):
  *   ZFAC_OPT_BAND            full GEMMs: tile columns per rasterisation band, 1 .. 4096                               8
  *   ZFAC_OPT_MAX_PAIRS       tensor-core modes: use at most this many CTA pairs; 0 = all co-resident ones            0
@@ -269,7 +276,7 @@ typedef enum {
   ZFAC_OPT_CHUNK_KB = 0, ZFAC_OPT_CHUNK0_KB = 1, ZFAC_OPT_HH_SQUARE = 2, ZFAC_OPT_HH_SQUARE_ERR = 3,
   ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
   ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10, ZFAC_OPT_INPUT_F32 = 11,
-  ZFAC_OPT_EXTRA_UPDATE = 12
+  ZFAC_OPT_EXTRA_UPDATE = 12, ZFAC_OPT_FINAL_CHECK = 13
 } zfac_option;
 zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
 zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);

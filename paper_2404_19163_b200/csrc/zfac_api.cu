@@ -234,6 +234,9 @@ zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
     case ZFAC_OPT_INPUT_F32:
       if ((iv != 0 && iv != 1) || (iv == 1 && !mode_is_f64_elt(c->mode))) return ZFAC_E_INVALID;
       o.input_f32 = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_FINAL_CHECK:
+      if ((iv != 0 && iv != 1) || (iv == 0 && !mode_is_mix(c->mode))) return ZFAC_E_INVALID;
+      o.final_check = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_EXTRA_UPDATE:
       if ((iv != 0 && iv != 1) || (iv == 1 && !mode_is_mix(c->mode))) return ZFAC_E_INVALID;
       o.extra_update = (int)iv; return ZFAC_OK;
@@ -258,6 +261,7 @@ zfac_status zfac_get_option(const zfac_ctx* c, zfac_option key, double* v) {
     case ZFAC_OPT_I8_SLICES: *v = o.i8_slices; return ZFAC_OK;
     case ZFAC_OPT_INPUT_F32: *v = o.input_f32; return ZFAC_OK;
     case ZFAC_OPT_EXTRA_UPDATE: *v = o.extra_update; return ZFAC_OK;
+    case ZFAC_OPT_FINAL_CHECK: *v = o.final_check; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }

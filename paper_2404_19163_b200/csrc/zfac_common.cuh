@@ -12,7 +12,7 @@ struct alignas(64) State {
   int done;                  // set by step a3; every later kernel of the call exits at once
   int iters;                 // number of Z updates performed so far (= index of the last Err)
   int flags;                 // ZFAC_R_* bits
-  int pad0;
+  int last;                  // ZFAC_OPT_FINAL_CHECK = 0: the update now in flight is the last one, its residual is not evaluated
   unsigned int arrive[4];    // last-CTA counters (one per use site), self-resetting
   int range;                 // bit 0: a value of magnitude >= 65504 was clamped on its way into an fp16 operand (16-bit modes;
                              // bit 1: F64_I8 met a non-finite operand while slicing -> the next Err is NaN);
@@ -38,6 +38,7 @@ struct Options {
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
+  int final_check = 1;       // FP64-master modes: 0 = skip a residual evaluation whose outcome is known beforehand (see stop_decide)
   int extra_update = 0;      // FP64-master modes: one more update after the paper's test has fired (see stop_decide)
   int input_f32 = 0;         // double-element modes: S and Z0 are float (promoted exactly), Z is returned as double
 };
@@ -56,6 +57,8 @@ struct StopArgs {
   // partials hold 16 sums per a2 tile (8 epilogue warps x 2 CTAs), tiles_pp a2 tiles per problem, and d_err is
   // [batch][err_stride]
   int extra;                 // FP64-master modes, ZFAC_OPT_EXTRA_UPDATE: when the test fires, perform ONE more update, then stop
+  int nocheck;               // FP64-master modes, ZFAC_OPT_FINAL_CHECK = 0 (see stop_decide)
+  double floor;              // ... the smallest Err worth iterating towards: 2^-53 sqrt(N)
   int tiles_pp;
   int slots_pt;              // partial sums per tile: 16 (SPLIT16: both epilogue groups work on a tile) or 8 (one-pass kinds)
   long long err_stride;
@@ -127,7 +130,28 @@ __device__ inline void stop_decide(const StopArgs& a, State* st, double* d_err, 
     }
   }
   if (!done && n == a.max_iter) { flags = ZFAC_R_MAXITER; done = 1; }
+  // ZFAC_OPT_FINAL_CHECK = 0 (FP64-master modes, paper's rule): an evaluation whose outcome is known beforehand is not made.
+  // That is the one after the extra update above (it ends the run whatever it finds), and, without that option, the one
+  // after an update taken from Err[n]^3 < 2^-53 sqrt(N): the next Err cannot pass the test unless it is below anything the
+  // arithmetic resolves, in which case there is nothing left to iterate for either.  The update in flight is then the last
+  // (State::last); finish_kernel, at the head of the next residual, counts it and ends the run.
+  if (!done && a.nocheck && a.stop == ZFAC_STOP_PAPER) {
+    if (a.extra ? (st->flags & ZFAC_R_REFINED) != 0 : (err * err * err < a.floor)) st->last = 1;
+  }
   if (done) { st->flags |= flags; __threadfence(); st->done = 1; }
+}
+
+// ZFAC_OPT_FINAL_CHECK = 0: first launch of every residual of the FP64-master modes.  If the update just performed was marked
+// as the last one, count it, leave NaN in its Err entry and end the run: the residual kernels behind return at once.
+__global__ void finish_kernel(State* st, double* d_err) {
+  if (st->done || !st->last) return;
+  const int n = st->iters + 1;
+  st->iters = n;
+  d_err[n] = nan("");
+  st->flags |= ZFAC_R_STOPPED | ZFAC_R_NOCHECK;
+  st->last = 0;
+  __threadfence();
+  st->done = 1;
 }
 
 // zfac_graph_*: the WHILE node's condition (another pass of the loop?) is set by this one-thread kernel right after every a2.

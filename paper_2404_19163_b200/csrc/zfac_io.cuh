@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) copy_in_kernel(const CopyInArgs a) {
     // refinement stage of Alg. 3 behind a low-precision run that ended non-finite: nothing to refine -- every later
     // kernel of this context exits at once (done = 1) and no Err entry exists (iters = -1)
     const bool dead = a.prev && (a.prev->flags & ZFAC_R_NONFINITE);
-    st->done = dead ? 1 : 0; st->iters = dead ? -1 : 0; st->flags = 0;
+    st->done = dead ? 1 : 0; st->iters = dead ? -1 : 0; st->flags = 0; st->last = 0;
     st->arrive[0] = st->arrive[1] = st->arrive[2] = st->arrive[3] = 0u;
   }
   const int c0 = blockIdx.x * CI_TC, r0 = ((int)blockIdx.y + a.ty0) * CI_TR;

@@ -522,6 +522,7 @@ struct MixSeq {
     st = reinterpret_cast<State*>(ws + L.off_state);
     stop.st = st; stop.partials = reinterpret_cast<double*>(ws + L.off_partials);
     stop.d_err = d_err; stop.max_iter = max_iter; stop.stop = stop_rule; stop.order = 2; stop.cond = cond; stop.extra = pl.opt->extra_update;
+    stop.nocheck = pl.opt->final_check ? 0 : 1; stop.floor = ldexp(1.0, -53) * sqrt((double)L.n);
     R32s = reinterpret_cast<float*>(ws + L.off_R32);
     np2 = (size_t)L.np * (size_t)L.np;
   }
@@ -530,6 +531,7 @@ struct MixSeq {
     const Layout& L = pl.L;
     char* ws = pl.ws;
     stop.n_iter = n_stop;
+    if (stop.nocheck && stop.stop == ZFAC_STOP_PAPER) { finish_kernel<<<1, 1, 0, s>>>(st, d_err); ++nl; }
     if (L.mode == ZFAC_MODE_F64_MIXED) {
       const int tiles = (int)(L.np / F64_BM);
       F64TParams P{};

@@ -6,6 +6,7 @@ oracle of that iteration is `O.refine(..., update_dtype=float32)` / `O.update_mi
 tests/test_oracle_refi_pins.py); against the all-FP64 oracle the result differs by the rounding of the correction,
 ~2^-22 ||R_0|| (a rotation of Z: any Z U is an inverse factor), so Z is held to 1e-6 there and what is unique -- the
 invariant ||Z^T S Z - I||_F / sqrt(N) and Z Z^T = S^-1 -- to the FP64 level."""
+import dataclasses
 import math
 
 import numpy as np
@@ -341,3 +342,63 @@ def test_extra_update_option_is_one_more_update_after_the_first_firing(mode):
         with pytest.raises(Exception):
             zf.set_option("extra_update", 1)
         assert zf.get_option("extra_update") == 0
+
+
+@pytest.mark.parametrize("mode", MIX)
+def test_final_check_option_skips_only_evaluations_whose_outcome_is_known(mode):
+    """ZFAC_OPT_FINAL_CHECK = 0 (include/zfac.h).  (i) Warm start: the run ends by the test in both settings, with the same
+    number of updates and the same Z bit for bit; the history is the same up to the last evaluated entry, Err[iters] is NaN,
+    the flag ZFAC_R_NOCHECK is set (the skipped residual's kernels are still enqueued, they return at once).  The update that was not
+    checked is the oracle's: Z against the oracle run for `iters` updates.  (ii) Cold start at kappa = 1e5: the last
+    evaluated Err before the firing is 3e-4, its cube is far above 2^-53 sqrt(N): nothing is foregone, the run is the
+    default run.  (iii) With ZFAC_OPT_EXTRA_UPDATE the evaluation after the extra update is the one skipped.  (iv) The WHILE
+    graph and the host entry point follow.  (v) Refused outside the FP64-master modes."""
+    b = zb()
+    n = 300
+    w = W.random_spd_general(n, seed=91, kappa=100.0, pert=0.02, fp32_stored=False)
+    lam, V = np.linalg.eigh(w.S)
+    G = np.random.default_rng(3).standard_normal((n, n)) / math.sqrt(n)
+    w = dataclasses.replace(w, Z0=np.ascontiguousarray(((V / np.sqrt(lam)) @ V.T) @ (np.eye(n) + 1e-3 * G)))     # Err: 2e-2, 7e-8, floor
+    Zd, itd, errd, fld, _, ld = run(w, mode, 30, b.ZFAC_STOP_PAPER)
+    Zn, itn, errn, fln, _, ln = run(w, mode, 30, b.ZFAC_STOP_PAPER, options={"final_check": 0})
+    print(f"[{mode} final_check=0] iters {itd} / {itn}, launches {ld} / {ln}, Err {errd} / {errn}")
+    assert fld == b.ZFAC_R_STOPPED and fln == (b.ZFAC_R_STOPPED | b.ZFAC_R_NOCHECK)
+    assert itn == itd and np.array_equal(Zn, Zd)
+    assert len(errn) == itd + 1 and np.array_equal(errn[:itd], errd[:itd]) and np.isnan(errn[itd])
+    assert errd[itd - 1] ** 3 < 2.0 ** -53 * math.sqrt(n)                 # why the last evaluation was foregone
+    ref = O.refine(w.S, w.Z0, itn, O.STOP_FIXED)
+    assert _rel(Zn, ref.Z) < 1e-8 and O.final_residual_per_sqrt_n(w.S, Zn) < 1e-12
+    # (ii) cold start: nothing foregone
+    wc = W.spectral_workload(300, 1e-5, 1.0, seed=0)
+    Zc, itc, errc, flc, _, _ = run(wc, mode, 40, b.ZFAC_STOP_PAPER)
+    Zc0, itc0, errc0, flc0, _, _ = run(wc, mode, 40, b.ZFAC_STOP_PAPER, options={"final_check": 0})
+    assert itc0 == itc and flc0 == flc and np.array_equal(Zc0, Zc) and np.array_equal(errc0, errc)
+    # (iii) with the extra update
+    Ze, ite, erre, fle, _, _ = run(wc, mode, 40, b.ZFAC_STOP_PAPER, options={"extra_update": 1})
+    Zx, itx, errx, flx, _, _ = run(wc, mode, 40, b.ZFAC_STOP_PAPER, options={"extra_update": 1, "final_check": 0})
+    assert itx == ite == itc + 1 and np.array_equal(Zx, Ze)
+    assert flx == (fle | b.ZFAC_R_NOCHECK) and (fle & b.ZFAC_R_REFINED)
+    assert np.array_equal(errx[:ite], erre[:ite]) and np.isnan(errx[ite])
+    # max_iter still bounds the run: the foregone update is not performed beyond it
+    Zm, itm, errm, flm, _, _ = run(w, mode, itd - 1, b.ZFAC_STOP_PAPER, options={"final_check": 0})
+    assert itm == itd - 1 and (flm & b.ZFAC_R_MAXITER) and not (flm & b.ZFAC_R_NOCHECK) and np.array_equal(errm, errd[:itd])
+    # (iv) graph and host entry
+    S, Z0 = _dev(w.S), _dev(w.Z0)
+    with b.Zfac(n, mode, DEV) as zf:
+        zf.set_option("final_check", 0)
+        with b.ZfacLoopGraph(zf, S, Z0, max_iter=30, stop=b.ZFAC_STOP_PAPER) as lg:
+            Zg, itg, errg, flg = lg.launch()
+            assert itg == itn and flg == fln and np.array_equal(Zg.cpu().numpy(), Zn) and np.isnan(errg[itg])
+        hS = torch.from_numpy(w.S).pin_memory(); hZ0 = torch.from_numpy(np.ascontiguousarray(w.Z0)).pin_memory()
+        hZ = torch.empty((n, n), dtype=torch.float64).pin_memory()
+        _, ith, errh, flh = zf.refine_host(hS, hZ0, hZ, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        assert ith == itn and flh == fln and np.array_equal(hZ.numpy(), Zn)
+        # a later call with the option back on is the default run again (State::last does not leak)
+        zf.set_option("final_check", 1)
+        Z1, it1, err1, fl1 = zf.refine(S, Z0, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        assert it1 == itd and fl1 == fld and np.array_equal(err1, errd) and np.array_equal(Z1.cpu().numpy(), Zd)
+    # (v)
+    with b.Zfac(256, "f64", DEV) as zf:
+        with pytest.raises(b.ZfacError):
+            zf.set_option("final_check", 0)
+        zf.set_option("final_check", 1)
