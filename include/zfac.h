@@ -86,12 +86,13 @@ enum {
   ZFAC_R_STOPPED = 1,  /* the test Err[n] > Err[n-1]^(m+1) fired (m = 2: ^3; converged to the precision floor) */
   ZFAC_R_MAXITER = 2,  /* max_iter updates were performed without the test firing               */
   ZFAC_R_NONFINITE = 4, /* Err[n] became inf/NaN; iteration stopped                              */
-  ZFAC_R_REFINED = 8,   /* zfac_refine_refi: at least one refinement update was applied          */
-  ZFAC_R_NOCHECK = 32,  /* ZFAC_OPT_FINAL_CHECK = 0: the residual of the last update was not evaluated (Err[iters] is NaN) */
-  ZFAC_R_RANGE = 16     /* SPLIT16 / HH16: a value of S, Z0, T = (S Z)^T or Z with magnitude >= 65504 was clamped when it
+  ZFAC_R_REFINED = 8,   /* zfac_refine_refi: at least one refinement update was applied; ZFAC_OPT_EXTRA_UPDATE: the extra
+                           update was taken                                                      */
+  ZFAC_R_RANGE = 16,    /* SPLIT16 / HH16: a value of S, Z0, T = (S Z)^T or Z with magnitude >= 65504 was clamped when it
                            was rounded to an FP16 operand (FP16 range); the result is not to be trusted.  Admissible input:
                            abs(S_ij), abs(Z_ij), abs((S Z)_ij) < 65504 throughout -- e.g. lambda_min(S) >~ 3e-10 for a
                            normalised S; rescale S by a power of four otherwise (Z scales by its square root)   */
+  ZFAC_R_NOCHECK = 32   /* ZFAC_OPT_FINAL_CHECK = 0: the residual of the last update was not evaluated (Err[iters] is NaN) */
 };
 
 /* Internal buffers that zfac_peek can copy out (parity tests of the individual steps).
