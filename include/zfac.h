@@ -317,6 +317,33 @@ const char* zfac_status_string(zfac_status s);
 /* Last CUDA error string recorded on this thread by a ZFAC_E_CUDA return ("" if none). */
 const char* zfac_last_cuda_error(void);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * An entry point that ALLOCATES NOTHING (no context, no workspace, no cudaMalloc / cudaFree / stream or event creation):
+ * for callers that cannot allocate -- code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ *
+ *   *d_err = || I - Z^T (S Z) ||_F        (Err of Alg. 2 for a GIVEN Z: Eq. 22-29; FP64 throughout)
+ *
+ * -- the check a consumer makes on a Z it holds (is it still an inverse factor of this S, or must it be refined?).
+ * It is the variant of the library's steps a1, a2, a3 whose scratch (T = S Z, the per-CTA partial sums, the arrival
+ * counter) lives in a file-scope device array of libzfac.so instead of a caller workspace: 8 MiB + 32 KiB + 256 B, held
+ * by every GPU that loads the library until the process exits.
+ *   d_S, d_Z [in]  device, double, row-major, n x n, leading dimensions lds, ldz >= n (elements); not modified
+ *   n              1 .. ZFAC_NOALLOC_MAX_N; larger n is REJECTED with ZFAC_E_INVALID (zfac_noalloc_last_error() says why):
+ *                  use zfac_create / zfac_refine (max_iter = 0) with a workspace there
+ *   d_err    [out] device, one double; valid once the work enqueued on `stream` has completed
+ *   stream         a cudaStream_t passed as void* (NULL = default stream); the call is asynchronous: one 4-byte memset
+ *                  + two kernels on `stream`
+ * The result is run-to-run deterministic (partial sums added in index order).  ALL calls on a device share the one scratch
+ * array: it keeps the last call's contents (nothing in it needs to survive; the counter is cleared at the head of every
+ * call), and two calls that OVERLAP on the GPU -- different streams without an event between them -- RACE on it and give
+ * wrong results.  Serialise them.  Calls on different devices do not interact.
+ * Returns ZFAC_OK, ZFAC_E_INVALID (null pointer, n < 1, n > ZFAC_NOALLOC_MAX_N, ld < n) or ZFAC_E_CUDA; the reason of
+ * the last failure on this thread is in zfac_noalloc_last_error() ("" after a success). */
+#define ZFAC_NOALLOC_MAX_N 1024
+zfac_status zfac_residual_norm_noalloc(const double* d_S, int64_t lds, const double* d_Z, int64_t ldz, int64_t n,
+                                       double* d_err, void* stream);
+const char* zfac_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

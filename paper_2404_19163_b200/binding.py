@@ -45,6 +45,7 @@ EXPORTS = [
     "zfac_graph_create", "zfac_graph_launch", "zfac_graph_destroy",
     "zfac_set_option", "zfac_get_option", "zfac_refine_refi_host",
     "zfac_workspace_bytes_batched", "zfac_create_batched", "zfac_get_batch", "zfac_refine_batched",
+    "zfac_residual_norm_noalloc", "zfac_noalloc_last_error",
 ]
 
 _lib: Optional[ctypes.CDLL] = None
@@ -73,6 +74,10 @@ def lib() -> ctypes.CDLL:
     L.zfac_workspace_bytes.argtypes = [i64, ci]
     L.zfac_padded_n.restype = i64
     L.zfac_padded_n.argtypes = [i64, ci]
+    L.zfac_residual_norm_noalloc.restype = ci
+    L.zfac_residual_norm_noalloc.argtypes = [vp, i64, vp, i64, i64, vp, vp]
+    L.zfac_noalloc_last_error.restype = ctypes.c_char_p
+    L.zfac_noalloc_last_error.argtypes = []
     L.zfac_create.restype = ci
     L.zfac_create.argtypes = [ctypes.POINTER(vp), i64, ci, vp, sz]
     L.zfac_refine.restype = ci
@@ -136,6 +141,22 @@ def zfac_workspace_bytes(n: int, mode: int) -> int:
 
 def zfac_padded_n(n: int, mode: int) -> int:
     return int(lib().zfac_padded_n(int(n), int(mode)))
+
+
+ZFAC_NOALLOC_MAX_N = 1024
+
+
+def zfac_noalloc_last_error() -> str:
+    return lib().zfac_noalloc_last_error().decode()
+
+
+def zfac_residual_norm_noalloc(d_S: int, lds: int, d_Z: int, ldz: int, n: int, d_err: int, stream: int = 0) -> None:
+    """Err = ||I - Z^T S Z||_F (FP64) into *d_err; allocates nothing (scratch is a static device array of the library;
+    n <= ZFAC_NOALLOC_MAX_N; overlapping calls race).  Raises ZfacError with the library's reason on failure."""
+    st = lib().zfac_residual_norm_noalloc(ctypes.c_void_p(d_S), int(lds), ctypes.c_void_p(d_Z), int(ldz), int(n),
+                                          ctypes.c_void_p(d_err), ctypes.c_void_p(stream))
+    if st != ZFAC_OK:
+        raise ZfacError(st, "zfac_residual_norm_noalloc: " + zfac_noalloc_last_error())
 
 
 def zfac_create(n: int, mode: int, d_workspace: int, nbytes: int) -> int:

@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libzfac.so")
-SOURCES = ["zfac_api.cu"]
+SOURCES = ["zfac_api.cu", "zfac_noalloc.cu"]
 HEADERS = ["zfac_common.cuh", "zfac_io.cuh", "zfac_f64.cuh", "zfac_umma.cuh", "zfac_f64_tma.cuh", "zfac_mix.cuh"]
 
 NVCC_FLAGS = [
