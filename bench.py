@@ -529,6 +529,10 @@ def run_ours(args):
         S = torch.from_numpy(w.S).to(dev, dt); Z0 = torch.from_numpy(w.Z0).to(dev, dt)
         Zout = torch.empty_like(Z0)
         with zb.Zfac(n, mode, dev) as zf:
+            if mode == args.mode:
+                for kv in args.option:                          # --option key=value: zfac_set_option on the primary mode's context
+                    k, v = kv.split("=", 1)
+                    zf.set_option(k, float(v))
             sampler = ClockSampler(local_rank) if with_clock else None
             ms, iters, flags, err, prof, clocks, launches, ms_prof = time_refine(
                 zf, S, Z0, Zout, args.max_iter, stop, args.steps, args.warmup, dev, profile=True, sampler=sampler,
@@ -862,7 +866,7 @@ def run_ours(args):
                       "hh16": "f16 (one pass), f32 accumulate", "f64mix": "f64 residual, f16-pair update into an f64 master",
                       "f64i8": "int8 slices (exact int32 accumulate) for the f64-level residual, f16-pair update into an f64 master"}[args.mode],
             "data": "synthetic",
-            "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "N": n, "stop": args.stop,
+            "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "options": args.option or None, "N": n, "stop": args.stop,
                        "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
                        "l2": "operands (2.4 GB) exceed L2 (126 MB); no flush needed"},
             "iters": iters, "iters_per_s": primary["iters_per_s"] * world, "time_to_converged_ms": t_ms,
@@ -899,6 +903,8 @@ def main():
     ap.add_argument("--workload", default="config4", choices=["config4", "config5", "config2"])
     ap.add_argument("--stop", default="paper", choices=["paper", "fixed"])
     ap.add_argument("--max-iter", type=int, default=20)
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=VALUE",
+                    help="zfac_set_option on the primary mode's context (binding.OPTIONS names), e.g. --option i8_cluster=1; repeatable")
     ap.add_argument("--cpu-sample-n", type=int, default=8192)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick", action="store_true", help="primary mode only (no other modes / reference points)")

@@ -234,6 +234,9 @@ zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
     case ZFAC_OPT_INPUT_F32:
       if ((iv != 0 && iv != 1) || (iv == 1 && !mode_is_f64_elt(c->mode))) return ZFAC_E_INVALID;
       o.input_f32 = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_I8_CLUSTER:
+      if ((iv != 0 && iv != 1) || (iv == 1 && c->mode != ZFAC_MODE_F64_I8)) return ZFAC_E_INVALID;
+      o.i8_cluster = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_FINAL_CHECK:
       if ((iv != 0 && iv != 1) || (iv == 0 && !mode_is_mix(c->mode))) return ZFAC_E_INVALID;
       o.final_check = (int)iv; return ZFAC_OK;
@@ -262,6 +265,7 @@ zfac_status zfac_get_option(const zfac_ctx* c, zfac_option key, double* v) {
     case ZFAC_OPT_INPUT_F32: *v = o.input_f32; return ZFAC_OK;
     case ZFAC_OPT_EXTRA_UPDATE: *v = o.extra_update; return ZFAC_OK;
     case ZFAC_OPT_FINAL_CHECK: *v = o.final_check; return ZFAC_OK;
+    case ZFAC_OPT_I8_CLUSTER: *v = o.i8_cluster; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }

@@ -37,6 +37,7 @@ struct Options {
   int host_overlap = 1;      // zfac_refine_host: early download of Z after the first update
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
+  int i8_cluster = 0;        // F64_I8 a1: clusters of two CTA pairs sharing the B slices by TMA multicast (scheduling only)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
   int final_check = 1;       // FP64-master modes: 0 = skip a residual evaluation whose outcome is known beforehand (see stop_decide)
   int extra_update = 0;      // FP64-master modes: one more update after the paper's test has fired (see stop_decide)

@@ -234,9 +234,30 @@ __host__ __device__ constexpr uint32_t make_idesc_i8(int n) {
 constexpr int I8_STAGES = 4;
 constexpr int I8_STAGE_BYTES = 3 * UM_A_BYTES;      // A_i, B_(d-i), B_(d-1-i) rows of one CTA, one k-block: 48 KB
 
-template <int EPI>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(UM_THREADS, 1)
+// tcgen05.commit of the pair's MMAs arriving on the barrier at offset `bar` in every CTA of `mask` (cluster ranks)
+__device__ __forceinline__ void tc_commit_mask(uint32_t bar, uint32_t mask) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((uint16_t)mask) : "memory");
+}
+// TMA load by one CTA into the SAME shared-memory offset of every CTA of `mask`; each destination counts the bytes on the
+// barrier at offset `bar` of ITS pair's leader (the address is this CTA's own with the peer bit, bit 24, cleared).
+__device__ __forceinline__ void tma_load_2d_pair_mc(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar, uint32_t mask) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%2, %3}], [%4], %5;"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(bar & 0xFEFFFFFFu), "h"((uint16_t)mask)
+      : "memory");
+}
+
+// CP = CTA pairs per cluster.  CP = 1: every pair on its own.  CP = 2 (full outputs, an even number of tile rows): a cluster
+// of two pairs works on the tiles (2 I', J) and (2 I' + 1, J); they use the same rows of B, so each B box is fetched from L2
+// ONCE and delivered to both pairs by TMA multicast (pair 0's CTAs fetch the B slice of order d, pair 1's the one of order
+// d - 1): 2/3 of a stage's bytes are shared, the L2 -> SM traffic falls by a third.  The two pairs then move in lockstep, a
+// stage at a time: a stage is refilled when BOTH pairs have released it (every MMA leader commits to the empty barriers of all
+// four CTAs).  Same arithmetic per tile: bit-identical results.
+template <int EPI, int CP = 1>
+__global__ void __cluster_dims__(2 * CP, 1, 1) __launch_bounds__(UM_THREADS, 1)
 i8_gemm_kernel(const __grid_constant__ I8Params p) {
+  static_assert(CP == 1 || EPI == EPI_A1, "clusters of two pairs: full outputs only");
   if (*((volatile int*)&p.st->done)) return;
   constexpr bool SYM = (EPI == EPI_A2);
   constexpr int TN = 256;
@@ -254,16 +275,20 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
   __shared__ int last_flag;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();
-  const int pair = blockIdx.x >> 1, num_pairs = gridDim.x >> 1;
+  const uint32_t crank = cluster_ctarank();                  // 0 .. 2 CP - 1
+  const uint32_t rank = crank & 1u;                          // within the pair: 0 = leader (issues the MMAs)
+  const uint32_t lead = crank & ~1u;                         // cluster rank of this pair's leader
+  const int pp = (int)(crank >> 1);                          // pair within the cluster
+  // unit of work distribution: the cluster.  CP = 2: one "tile" of the loops below is a 512 x 256 super tile
+  const int pair = (int)blockIdx.x / (2 * CP), num_pairs = (int)gridDim.x / (2 * CP);
   const int np = p.np;
   const int KB = np / 128;                                   // k-blocks of 128 int8
   const int T = p.macro_tiles;
-  const int num_tiles = SYM ? T * (T + 1) / 2 : T * T;
+  const int num_tiles = SYM ? T * (T + 1) / 2 : (T / CP) * T;
   const int ORD = p.orders;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < I8_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < I8_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), CP); }
     mbar_init(tfull_bar(0), 1); mbar_init(tempty_bar(0), 2 * UM_EPI_WARPS);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&p.mapA)) : "memory");
@@ -283,7 +308,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
   auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
     int I, J;
     if (SYM) { tri_decode(t, I, J); offdiag = (I != J); }
-    else { band_decode(t, T, T, p.band, I, J); offdiag = true; }
+    else { band_decode(t, T / CP, T, p.band, I, J); I = I * CP + pp; offdiag = true; }
     m0 = I * UM_TILE_M; n0 = J * TN;
   };
 
@@ -304,14 +329,21 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
             for (int kb = 0; kb < KB; ++kb) {
               mbar_wait(empty_bar(stage), phase ^ 1u);
               if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * (uint32_t)UM_A_BYTES * (1u + (v1 ? 1u : 0u) + (v2 ? 1u : 0u)));
-              const uint32_t lead_full = mapa_u32(full_bar(stage), 0);
+              const uint32_t lead_full = mapa_u32(full_bar(stage), lead);
               const uint32_t sa = smem_base + stage * I8_STAGE_BYTES, sb1 = sa + UM_A_BYTES, sb2 = sb1 + UM_A_BYTES;
               const int kc = kb * 128;
+              const uint32_t mc = (1u << rank) | (1u << (rank + 2u));   // CP = 2: the CTAs of both pairs that hold this half of B
 #pragma unroll
               for (int b = 0; b < UM_ROWS / UM_BOX_ROWS; ++b) {
                 tma_load_2d_pair(sa + b * UM_BOX_BYTES, &p.mapA, kc, i * np + m0 + aoff + b * UM_BOX_ROWS, lead_full);
-                if (v1) tma_load_2d_pair(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
-                if (v2) tma_load_2d_pair(sb2 + b * UM_BOX_BYTES, &p.mapB, kc, j2 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                if (CP == 1) {
+                  if (v1) tma_load_2d_pair(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                  if (v2) tma_load_2d_pair(sb2 + b * UM_BOX_BYTES, &p.mapB, kc, j2 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                } else if (pp == 0) {
+                  if (v1) tma_load_2d_pair_mc(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, full_bar(stage), mc);
+                } else {
+                  if (v2) tma_load_2d_pair_mc(sb2 + b * UM_BOX_BYTES, &p.mapB, kc, j2 * np + n0 + boff + b * UM_BOX_ROWS, full_bar(stage), mc);
+                }
               }
               if (++stage == I8_STAGES) { stage = 0; phase ^= 1u; }
             }
@@ -343,11 +375,11 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
                 if (v1) { tc_mma_pair_i8(dA, ad + (uint64_t)(k * 2), b1 + (uint64_t)(k * 2), IDESC, acc1); acc1 = 1u; }
                 if (v2) { tc_mma_pair_i8(dB, ad + (uint64_t)(k * 2), b2 + (uint64_t)(k * 2), IDESC, acc2); acc2 = 1u; }
               }
-              tc_commit_pair(empty_bar(stage));
+              tc_commit_mask(empty_bar(stage), (1u << (2 * CP)) - 1u);      // every CTA of the cluster: its stage is free
               if (++stage == I8_STAGES) { stage = 0; phase ^= 1u; }
             }
           }
-          tc_commit_pair(tfull_bar(0));                      // orders d and d - 1 complete in both CTAs
+          tc_commit_mask(tfull_bar(0), 3u << lead);           // orders d and d - 1 complete in both CTAs of the pair
         }
       }
     }
@@ -355,7 +387,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
     // ===================================================== epilogue warps 4 .. 11: thread = (row, 128-column half)
     const int q = warp & 3, g = (warp - UM_EPI_WARP0) >> 2;
     const int rowl = q * 32 + lane;                            // row of this CTA's 128-row half tile
-    const uint32_t lead_tempty = mapa_u32(tempty_bar(0), 0);
+    const uint32_t lead_tempty = mapa_u32(tempty_bar(0), lead);
     double* slab = p.scratch + (size_t)blockIdx.x * (128 * 256);
     uint32_t seq = 0;
     for (int t = pair; t < num_tiles; t += num_pairs) {
@@ -446,6 +478,7 @@ struct MixPlan {
   char* ws = nullptr;
   int mode = 0;
   int max_pairs = 0;
+  int max_quads = 0;                    // I8 engine: co-resident clusters of two pairs (i8_gemm_kernel<EPI_A1, 2>)
   const Options* opt = nullptr;
   F64Plan f64;                          // DMMA engine: S, W, T, R (FP64)
   CUtensorMap mR, mQ, mZ[2];            // fp16 pair planes of R~, Q~, FP32[Z] (update GEMMs)
@@ -453,14 +486,14 @@ struct MixPlan {
   int pairs() const { return (opt->max_pairs > 0 && opt->max_pairs < max_pairs) ? opt->max_pairs : max_pairs; }
 };
 
-template <int EPI>
+template <int EPI, int CP = 1>
 inline cudaError_t i8_prepare(int* max_pairs, int sm_count) {
-  cudaError_t e = cudaFuncSetAttribute(i8_gemm_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(i8_gemm_kernel<EPI, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
   if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(2 * (sm_count / 2)); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES;
+  cfg.gridDim = dim3(2 * CP * (sm_count / (2 * CP))); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES;
   int nc = 0;
-  e = cudaOccupancyMaxActiveClusters(&nc, i8_gemm_kernel<EPI>, &cfg);
+  e = cudaOccupancyMaxActiveClusters(&nc, i8_gemm_kernel<EPI, CP>, &cfg);
   if (e != cudaSuccess) return e;
   if (nc < 1) return cudaErrorLaunchOutOfResources;
   if (*max_pairs == 0 || nc < *max_pairs) *max_pairs = nc;
@@ -495,6 +528,7 @@ inline cudaError_t mix_plan_create(MixPlan* pl, const Layout& L, char* ws, int s
     if ((e = make_map(enc, &pl->mT8, ws + L.off_T8, B8, 1, rows, np)) != cudaSuccess) return e;
     if ((e = i8_prepare<EPI_A1>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
     if ((e = i8_prepare<EPI_A2>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
+    if ((e = i8_prepare<EPI_A1, 2>(&pl->max_quads, sm_count)) != cudaSuccess) { pl->max_quads = 0; (void)cudaGetLastError(); }
   }
   if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
   if (2 * pl->max_pairs > I8_SCRATCH_CTAS) pl->max_pairs = I8_SCRATCH_CTAS / 2;
@@ -559,6 +593,15 @@ struct MixSeq {
       // a1: T = W S^T (FP64 out), then its rows sliced for a2
       p.mapA = pl.mW8; p.mapB = pl.mS8; p.expA = eW; p.expB = eS; p.out64 = reinterpret_cast<double*>(ws + L.off_T);
       if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
+      // clusters of two pairs (B slices shared by TMA multicast) when the option is on and the tile rows pair up
+      int quads = pl.max_quads;
+      if (pl.opt->max_pairs > 0 && pl.opt->max_pairs / 2 < quads) quads = pl.opt->max_pairs / 2;
+      if (2 * quads * 2 > I8_SCRATCH_CTAS) quads = I8_SCRATCH_CTAS / 4;
+      if (pl.opt->i8_cluster && quads > 0 && p.macro_tiles % 2 == 0) {
+        const int super_tiles = (p.macro_tiles / 2) * p.macro_tiles;
+        const int nq = super_tiles < quads ? super_tiles : quads;
+        i8_gemm_kernel<EPI_A1, 2><<<4 * nq, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      } else
       i8_gemm_kernel<EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
       slice_rows_kernel<double><<<small_grid((size_t)L.np), 256, 0, s>>>(p.out64, L.np, (int)L.np, (int)L.np, p.orders,
                                                                  reinterpret_cast<int8_t*>(ws + L.off_T8), eT, st);

@@ -402,3 +402,34 @@ def test_final_check_option_skips_only_evaluations_whose_outcome_is_known(mode):
         with pytest.raises(b.ZfacError):
             zf.set_option("final_check", 0)
         zf.set_option("final_check", 1)
+
+
+def test_i8_cluster_option_is_scheduling_only():
+    """ZFAC_OPT_I8_CLUSTER (include/zfac.h): a1 of F64_I8 on clusters of two CTA pairs that share the B slices by TMA
+    multicast.  Same arithmetic per tile, exact FP64 sums: T, the history and Z are bit-identical to the default, for an
+    even number of 256-row tiles (the cluster path), for an odd one (falls back to the pair kernel) and under
+    ZFAC_OPT_MAX_PAIRS; refused outside F64_I8."""
+    b = zb()
+    for n, seed in ((1024, 5), (1500, 6), (700, 7)):          # padded to 1024 (4 tile rows), 1536 (6), 768 (3: fallback)
+        w = W.random_spd_general(n, seed=seed, kappa=100.0, pert=0.05, fp32_stored=False)
+        S, Z0 = _dev(w.S), _dev(w.Z0)
+        with b.Zfac(n, "f64i8", DEV) as zf:
+            ref = None
+            for opts in ({"i8_cluster": 0}, {"i8_cluster": 1}, {"i8_cluster": 1, "max_pairs": 5}):
+                for k, v in opts.items():
+                    zf.set_option(k, v)
+                Z, it, err, fl = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+                T = zf.peek(b.ZFAC_BUF_T)
+                if ref is None:
+                    ref = (Z.clone(), it, err.copy(), fl, T.clone())
+                    assert O.final_residual_per_sqrt_n(w.S, Z.cpu().numpy()) < 1e-12
+                else:
+                    assert it == ref[1] and fl == ref[3], (n, opts)
+                    assert torch.equal(Z, ref[0]) and torch.equal(T, ref[4]), (n, opts)
+                    if "max_pairs" in opts:       # a2 keeps one partial sum per CTA: Err[] depends on the grid in its last bits
+                        assert np.allclose(err, ref[2], rtol=1e-9, atol=0.0), (n, opts)
+                    else:
+                        assert np.array_equal(err, ref[2]), (n, opts)
+    with b.Zfac(256, "f64mix", DEV) as zf:
+        with pytest.raises(b.ZfacError):
+            zf.set_option("i8_cluster", 1)
