@@ -272,6 +272,9 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *   The rest change scheduling only (bit-identical results):
  *   ZFAC_OPT_BAND            full GEMMs: tile columns per rasterisation band, 1 .. 4096                               8
  *   ZFAC_OPT_MAX_PAIRS       tensor-core modes: use at most this many CTA pairs; 0 = all co-resident ones            0
+ *   ZFAC_OPT_NARROW_TILES    SPLIT16: 256 x 128 pair tiles with two accumulator sets instead of 256 x 256 with one (twice as many
+ *                            tiles: a small problem occupies more of the chip); -1 = automatically for one problem of padded order
+ *                            <= 1536, 0 = never, 1 = always                                                          -1
  *   ZFAC_OPT_I8_CLUSTER      F64_I8, a1 (when the padded order is a multiple of 512): clusters of two CTA pairs that share
  *                            the B slices by TMA multicast (L2 -> SM bytes -25 %); only 33 such clusters are co-resident on a
  *                            B200 against 74 pairs, measured a tie; 0 / 1                              0
@@ -280,7 +283,8 @@ typedef enum {
   ZFAC_OPT_CHUNK_KB = 0, ZFAC_OPT_CHUNK0_KB = 1, ZFAC_OPT_HH_SQUARE = 2, ZFAC_OPT_HH_SQUARE_ERR = 3,
   ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
   ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10, ZFAC_OPT_INPUT_F32 = 11,
-  ZFAC_OPT_EXTRA_UPDATE = 12, ZFAC_OPT_FINAL_CHECK = 13, ZFAC_OPT_I8_CLUSTER = 14
+  ZFAC_OPT_EXTRA_UPDATE = 12, ZFAC_OPT_FINAL_CHECK = 13, ZFAC_OPT_I8_CLUSTER = 14,
+  ZFAC_OPT_NARROW_TILES = 15
 } zfac_option;
 zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
 zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);

@@ -37,6 +37,7 @@ struct Options {
   int host_overlap = 1;      // zfac_refine_host: early download of Z after the first update
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
+  int narrow_tiles = -1;     // SPLIT16: 256 x 128 tiles (see umma_narrow): -1 auto, 0 never, 1 always (scheduling only)
   int i8_cluster = 0;        // F64_I8 a1: clusters of two CTA pairs sharing the B slices by TMA multicast (scheduling only)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
   int final_check = 1;       // FP64-master modes: 0 = skip a residual evaluation whose outcome is known beforehand (see stop_decide)
@@ -167,14 +168,15 @@ __global__ void graph_cond_kernel(const State* st, unsigned long long cond) {
 // problem's partials in index order (lane-strided, then a fixed shuffle tree) and takes the decision.  The order depends
 // on the tile enumeration only, not on which CTA computed which tile: Err[] is run-to-run deterministic and the same
 // whether a problem runs alone or as one of a batch.  Called by all 32 lanes of an epilogue warp after a tile.
-__device__ inline void stop_test_tile_warp(const StopArgs& a, int b, int tile, int slot, double tile_sumsq, int lane) {
+// `lin` = position of this warp's sum among the tiles_pp * slots_pt sums of problem b.
+__device__ inline void stop_test_index_warp(const StopArgs& a, int b, int lin, double tile_sumsq, int lane) {
   const double s = warp_sum(tile_sumsq);
   State* st = a.st + b;
   const int per = a.tiles_pp * a.slots_pt;
   double* part = a.partials + (size_t)b * per;
   int last = 0;
   if (lane == 0) {
-    part[(size_t)tile * a.slots_pt + slot] = s;
+    part[(size_t)lin] = s;
     __threadfence();
     last = (atomicAdd(&st->arrive[0], 1u) == (unsigned int)per - 1u);
     if (last) { st->arrive[0] = 0u; __threadfence(); }

@@ -40,7 +40,8 @@
 
 namespace zfac {
 
-enum { KIND_F16X2 = 0, KIND_HH16 = 1, KIND_TF32 = 2 };
+enum { KIND_F16X2 = 0, KIND_HH16 = 1, KIND_TF32 = 2, KIND_F16X2N = 3 };   // F16X2N: F16X2 on 256 x 128 tiles (small problems)
+__host__ __device__ constexpr bool kind_is_pair(int kind) { return kind == KIND_F16X2 || kind == KIND_F16X2N; }
 
 constexpr int UM_TILE_M = 256;                   // pair tile rows: two CTAs x 128 TMEM lanes
 constexpr int UM_MACRO = 256;                    // padding unit and macro tile of the symmetric enumeration
@@ -76,6 +77,13 @@ constexpr int UM_MAX_STAGES = 6;
 template <int KIND> struct KindTraits;
 template <> struct KindTraits<KIND_F16X2> {
   static constexpr int ARRAYS = 2, TILE_N = 256, SETS = 1, STAGES = 3, KSTEP_ELEMS = 16, BK_ELEMS = 64, FMT = 0, SUB = 16;
+};
+// The same arithmetic on 256 x 128 tiles with two accumulator sets: twice as many tiles.  Per tile column it is slower (the
+// shared-memory port, see above), but a problem of <= 6 x 6 macro tiles leaves most of the 74 CTA pairs idle on 256 x 256
+// tiles: one SPLIT16 problem of N = 512 / 1024 runs 24 / 23 % faster on these (ZFAC_OPT_NARROW_TILES).  Every output element
+// is accumulated in the same order, and the a2 partial sums are laid out as for the wide tiles: bit-identical results.
+template <> struct KindTraits<KIND_F16X2N> {
+  static constexpr int ARRAYS = 2, TILE_N = 128, SETS = 2, STAGES = 4, KSTEP_ELEMS = 16, BK_ELEMS = 64, FMT = 0, SUB = 16;
 };
 template <> struct KindTraits<KIND_HH16> {
   static constexpr int ARRAYS = 1, TILE_N = 256, SETS = 2, STAGES = 6, KSTEP_ELEMS = 16, BK_ELEMS = 64, FMT = 0, SUB = 32;
@@ -308,7 +316,7 @@ __device__ __forceinline__ void flag_h16_range(State* st, const float (&v)[N]) {
 template <int KIND, int EPI, int SUB>
 __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SUB], int m, int n, int mb, bool offdiag,
                                               double& tile_sumsq) {
-  constexpr bool PAIR = (KIND == KIND_F16X2);
+  constexpr bool PAIR = kind_is_pair(KIND);
   const size_t ld = (size_t)p.np, plane = ld * (size_t)p.rows;
   const size_t off = (size_t)m * ld + n;               // (m, n)
   const size_t offt = (size_t)(mb + n) * ld + (m - mb);   // (n, m) of the same problem
@@ -398,7 +406,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
       }
     }
   } else if (EPI == EPI_A5X) {                          // FP64 master: Z64 += (Z Q~) / rscale; next operand pair; W64 = Z^T
-    if (KIND == KIND_F16X2) {
+    if (kind_is_pair(KIND)) {
       const double rinv = (double)p.st->rinv;
       double* zp = p.z64 + off;
       float z32[SUB];
@@ -448,7 +456,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 
   using KT = KindTraits<KIND>;
   constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3 || EPI == EPI_P2);
-  constexpr bool PAIRK = (KIND == KIND_F16X2);                 // (hi, lo') operand pairs, promoted accumulation
+  constexpr bool PAIRK = kind_is_pair(KIND);                   // (hi, lo') operand pairs, promoted accumulation
   constexpr int TN = KT::TILE_N;
   constexpr int NSPLIT = UM_MACRO / TN;                        // column sub-tiles per 256-wide macro tile
   constexpr int B_BYTES = (TN / 2) * UM_ROWB;                  // B rows of one array, one stage, one CTA
@@ -825,9 +833,14 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
         mbar_arrive_cluster_lane0(lead_tempty, lane);            // frees the accumulator set
       }
       // step a3: this warp's share of the tile (slot: CTA of the pair x warp of the tile's epilogue group(s))
-      if (EPI == EPI_A2)
-        stop_test_tile_warp(p.stop, mb / np, tl, (int)rank * (UM_EPI_WARPS / SETS) + ((SETS == 2) ? q : (warp - UM_EPI_WARP0)),
-                            offdiag ? 2.0 * tile_sumsq : tile_sumsq, lane);
+      if (EPI == EPI_A2) {
+        // F16X2N: a warp covers the same 32 rows x 128 columns as a warp of the wide kind does; its sum goes where that
+        // warp's would (macro tile, CTA, column half, lane quarter), so Err[] does not depend on the tile width
+        const int lin = (KIND == KIND_F16X2N)
+                            ? (tl >> 1) * 16 + (int)rank * 8 + (tl & 1) * 4 + q
+                            : tl * (2 * UM_EPI_WARPS / SETS) + (int)rank * (UM_EPI_WARPS / SETS) + ((SETS == 2) ? q : (warp - UM_EPI_WARP0));
+        stop_test_index_warp(p.stop, mb / np, lin, offdiag ? 2.0 * tile_sumsq : tile_sumsq, lane);
+      }
     }
 #ifdef ZFAC_TIMING
     if (p.dbg && rank == 0 && warp == UM_EPI_WARP0 && lane == 0)
@@ -916,6 +929,7 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], H, 2, rows, np)) != cudaSuccess) return e;
     e = (L.mode == ZFAC_MODE_SPLIT16) ? prepare_kind<KIND_F16X2>(&pl->max_pairs, sm_count) : prepare_kind<KIND_HH16>(&pl->max_pairs, sm_count);
     if (e != cudaSuccess) return e;
+    if (L.mode == ZFAC_MODE_SPLIT16 && (e = prepare_kind<KIND_F16X2N>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
   } else {
     const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     const uint64_t rows = (uint64_t)L.rows;
@@ -932,6 +946,14 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   return cudaSuccess;
 }
 
+// SPLIT16 on 256 x 128 tiles (KIND_F16X2N)?  ZFAC_OPT_NARROW_TILES: 0 never, 1 always, -1 (default) one problem of at most
+// 6 x 6 macro tiles (N <= 1536: <= 36 wide tiles for 74 CTA pairs).  Batched launches have tiles enough (measured: no gain).
+inline bool umma_narrow(const UmmaPlan& pl) {
+  if (pl.L.mode != ZFAC_MODE_SPLIT16) return false;
+  if (pl.opt->narrow_tiles >= 0) return pl.opt->narrow_tiles != 0;
+  return pl.L.batch == 1 && pl.L.np / UM_MACRO <= 6;
+}
+
 template <int KIND>
 inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) {
   switch (epi) {
@@ -942,12 +964,13 @@ inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) 
     case EPI_P2: umma_gemm_kernel<KIND, EPI_P2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
     case EPI_A5X:
       if (KIND == KIND_F16X2) umma_gemm_kernel<KIND_F16X2, EPI_A5X><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
-      break;
+      break;                                               // (FP64-master modes: wide tiles only)
     default:     umma_gemm_kernel<KIND, EPI_A5><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
   }
 }
-inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const UmmaParams& p) {
-  if (mode == ZFAC_MODE_SPLIT16) umma_launch<KIND_F16X2>(epi, grid, s, p);
+inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const UmmaParams& p, bool narrow = false) {
+  if (mode == ZFAC_MODE_SPLIT16 && narrow) umma_launch<KIND_F16X2N>(epi, grid, s, p);
+  else if (mode == ZFAC_MODE_SPLIT16) umma_launch<KIND_F16X2>(epi, grid, s, p);
   else if (mode == ZFAC_MODE_HH16) umma_launch<KIND_HH16>(epi, grid, s, p);
   else umma_launch<KIND_TF32>(epi, grid, s, p);
 }
@@ -968,7 +991,8 @@ struct UmmaSeq {
     const Layout& L = pl.L;
     char* ws = pl.ws;
     const int T = (int)(L.np / UM_MACRO);
-    const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
+    narrow = umma_narrow(pl);
+    const int nsplit = UM_MACRO / (narrow ? KindTraits<KIND_F16X2N>::TILE_N : L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
                                    : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
     const int full_tiles = T * T * nsplit * L.batch, sym_tiles = T * (T + 1) / 2 * nsplit * L.batch;
     grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
@@ -984,7 +1008,8 @@ struct UmmaSeq {
     p.stop.num_partials = 0; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
     p.stop.order = order; p.stop.cond = cond;
     p.stop.tiles_pp = T * (T + 1) / 2 * nsplit; p.stop.err_stride = (long long)max_iter + 1;
-    p.stop.slots_pt = 2 * UM_EPI_WARPS / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::SETS : KindTraits<KIND_HH16>::SETS);
+    p.stop.slots_pt = 2 * UM_EPI_WARPS / (narrow ? KindTraits<KIND_F16X2N>::SETS
+                                          : L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::SETS : KindTraits<KIND_HH16>::SETS);
     const PolyCoef pc = poly_coef(order);
     p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.g_i = (float)pc.g_i; p.g_r = (float)pc.g_r; p.g_p = (float)pc.g_p;
     R32 = reinterpret_cast<float*>(ws + L.off_R);
@@ -992,6 +1017,7 @@ struct UmmaSeq {
   }
 
   int nsplit_ = 1;
+  bool narrow = false;
 
   // a1 restricted to the macro-tile columns [mc0, mc0 + mcn) of T, i.e. to the rows [256 mc0, 256 (mc0 + mcn)) of S
   // (mcn = 0: all of T).  Tiles do not overlap between bands, so a banded a1 is bit-identical to the full launch.
@@ -1009,7 +1035,7 @@ struct UmmaSeq {
       const int tiles = p.macro_tiles * p.jcols;
       grid = 2 * (tiles < pl.pairs() ? tiles : pl.pairs());
     }
-    umma_launch_mode(L.mode, EPI_A1, grid, s, p);
+    umma_launch_mode(L.mode, EPI_A1, grid, s, p, narrow);
     p.joff = 0; p.jcols = 0;
     nl += 1;
   }
@@ -1029,7 +1055,7 @@ struct UmmaSeq {
     // a2 writes four outputs per element: its stores take twice as long, so a long first chunk (if one is set) doubles
     if (pl.opt->chunk0_kb > pl.opt->chunk_kb) p.chunk0_kb = 2 * pl.opt->chunk0_kb;
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
-    umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p);
+    umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p, narrow);
     nl += 1;
     if (p.stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(p.st, p.stop.cond);       // zfac_graph_*: loop condition
   }
@@ -1053,7 +1079,7 @@ struct UmmaSeq {
       p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
       if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; p.out2 = ws + L.off_Zb[(par + 1) & 1]; }
       else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; p.out2 = ws + L.off_Z[(par + 1) & 1]; }
-      umma_launch_mode(L.mode, EPI_P2, grid_sym, s, p);
+      umma_launch_mode(L.mode, EPI_P2, grid_sym, s, p, narrow);
       nl += 1;
       p.out2 = nullptr;
     }
@@ -1063,7 +1089,7 @@ struct UmmaSeq {
     p.f32_in = R32;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr; }
-    umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p);
+    umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p, narrow);
     // a5: Z_next = Z + Z Q^T ; W = Z_next^T   (first order in R: all three passes)
     p.hh_only = 0;
     if (prof) prof->mark(s, EPI_A5 + 16 * tagn);
@@ -1081,14 +1107,14 @@ struct UmmaSeq {
         const int i0 = (int)((long long)T * b / bands), i1 = (int)((long long)T * (b + 1) / bands);
         p.ioff = i0; p.irows = i1 - i0;
         const int tiles = p.irows * T * nsplit_;
-        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.pairs() ? tiles : pl.pairs()), s, p);
+        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.pairs() ? tiles : pl.pairs()), s, p, narrow);
         hook->after_a5_band(hook->self, i0 * UM_MACRO, i1 * UM_MACRO, b == bands - 1, s);
       }
       p.ioff = 0; p.irows = 0;
       nl += 1 + bands;
       return;
     }
-    umma_launch_mode(L.mode, EPI_A5, grid_full, s, p);
+    umma_launch_mode(L.mode, EPI_A5, grid_full, s, p, narrow);
     nl += 2;
   }
 };
@@ -1116,7 +1142,8 @@ inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* laun
   const Layout& L = pl.L;
   char* ws = pl.ws;
   const int T = (int)(L.np / UM_MACRO);
-  const int nsplit = UM_MACRO / (L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
+  const bool narrow = umma_narrow(pl);
+  const int nsplit = UM_MACRO / (narrow ? KindTraits<KIND_F16X2N>::TILE_N : L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
                                  : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
   const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
   const int grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
@@ -1128,9 +1155,9 @@ inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* laun
   const bool h16 = (L.mode != ZFAC_MODE_TF32);
   p.mapA = pl.mW; p.mapB = pl.mS;
   if (h16) p.h_out = ws + L.off_T; else p.f32_out = reinterpret_cast<float*>(ws + L.off_T);
-  umma_launch_mode(L.mode, EPI_A1, grid_full, s, p);
+  umma_launch_mode(L.mode, EPI_A1, grid_full, s, p, narrow);
   p.mapA = pl.mW; p.mapB = pl.mT; p.f32_out = reinterpret_cast<float*>(ws + L.off_R); p.h_out = nullptr;
-  umma_launch_mode(L.mode, EPI_X3, grid_sym, s, p);
+  umma_launch_mode(L.mode, EPI_X3, grid_sym, s, p, narrow);
   *launches = 2;
   return cudaGetLastError();
 }

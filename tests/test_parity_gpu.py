@@ -1373,3 +1373,42 @@ def test_batched_context_argument_checks():
             b.zfac_refine_batched(zbt.ctx, S.data_ptr(), 100, 50, S.data_ptr(), 100, 10000, S.data_ptr(), 100, 10000, 5, 0,
                                   d_i.data_ptr(), d_e.data_ptr(), d_i.data_ptr())
         assert e.value.status == b.ZFAC_E_INVALID
+
+
+@pytest.mark.parametrize("n", [200, 700, 1300])
+def test_narrow_tiles_are_scheduling_only(n):
+    """ZFAC_OPT_NARROW_TILES (SPLIT16 on 256 x 128 pair tiles with two accumulator sets; the default for one problem of padded
+    order <= 1536): every output element is accumulated in the same order and the a2 partial sums sit where the wide tiles'
+    would, so Z, the whole history, the flags, the congruence and the order-3 / 4 updates are bit-identical to the
+    256 x 256 tiles (option 0) -- what changes is the number of tiles.  Also under ZFAC_OPT_MAX_PAIRS."""
+    b = zb()
+    w = W.random_spd_general(n, seed=40 + n, kappa=30.0, pert=0.05, fp32_stored=True)
+    S, Z0 = _to_dev(w.S, "split16"), _to_dev(w.Z0, "split16")
+    H = _to_dev(W.random_spd_general(n, seed=41 + n, kappa=5.0, pert=0.0, fp32_stored=True).S, "split16")
+    results = {}
+    for nt in (0, 1, -1):
+        with b.Zfac(n, "split16", DEV) as zf:
+            assert zf.get_option("narrow_tiles") == -1
+            zf.set_option("narrow_tiles", nt)
+            out = []
+            for order in (2, 3, 4):
+                zf.set_order(order)
+                Z, it, err, fl = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+                out.append((Z.clone(), it, err.copy(), fl, zf.peek(b.ZFAC_BUF_T).clone(), zf.peek(b.ZFAC_BUF_R).clone()))
+            zf.set_order(2)
+            zf.set_option("max_pairs", 3)
+            Z, it, err, fl = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+            out.append((Z.clone(), it, err.copy(), fl, zf.peek(b.ZFAC_BUF_T).clone(), zf.peek(b.ZFAC_BUF_R).clone()))
+            zf.set_option("max_pairs", 0)
+            out.append(zf.congruence(H, Z).clone())
+            results[nt] = out
+    for nt in (1, -1):
+        for a, c in zip(results[0][:-1], results[nt][:-1]):
+            assert a[1] == c[1] and a[3] == c[3] and np.array_equal(a[2], c[2]), (n, nt)
+            assert torch.equal(a[0], c[0]) and torch.equal(a[4], c[4]) and torch.equal(a[5], c[5]), (n, nt)
+        assert torch.equal(results[0][-1], results[nt][-1]), (n, nt)
+    ora = O.refine(w.S, w.Z0, results[0][0][1], O.STOP_FIXED)
+    assert _rel(results[1][0][0].cpu().double().numpy(), ora.Z) <= TOL["split16"]
+    with b.Zfac(256, "hh16", DEV) as zf:
+        with pytest.raises(b.ZfacError):
+            zf.set_option("narrow_tiles", 1)
