@@ -946,12 +946,14 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
   return cudaSuccess;
 }
 
-// SPLIT16 on 256 x 128 tiles (KIND_F16X2N)?  ZFAC_OPT_NARROW_TILES: 0 never, 1 always, -1 (default) one problem of at most
-// 6 x 6 macro tiles (N <= 1536: <= 36 wide tiles for 74 CTA pairs).  Batched launches have tiles enough (measured: no gain).
+// SPLIT16 on 256 x 128 tiles (KIND_F16X2N)?  ZFAC_OPT_NARROW_TILES: 0 never, 1 always, -1 (default) when the full GEMMs of
+// the launch have at most 37 wide tiles (one problem of N <= 1536, or a few smaller ones): the narrow ones then still fit
+// the 74 CTA pairs in one wave.  Larger launches have tiles enough (measured: no gain, a loss from N = 2048 on).
 inline bool umma_narrow(const UmmaPlan& pl) {
   if (pl.L.mode != ZFAC_MODE_SPLIT16) return false;
   if (pl.opt->narrow_tiles >= 0) return pl.opt->narrow_tiles != 0;
-  return pl.L.batch == 1 && pl.L.np / UM_MACRO <= 6;
+  const long T = (long)(pl.L.np / UM_MACRO);
+  return (long)pl.L.batch * T * T <= 37;
 }
 
 template <int KIND>
