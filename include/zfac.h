@@ -272,7 +272,7 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *   The rest change scheduling only (bit-identical results):
  *   ZFAC_OPT_BAND            full GEMMs: tile columns per rasterisation band, 1 .. 4096                               8
  *   ZFAC_OPT_MAX_PAIRS       tensor-core modes: use at most this many CTA pairs; 0 = all co-resident ones            0
- *   ZFAC_OPT_NARROW_TILES    SPLIT16: 256 x 128 pair tiles with two accumulator sets instead of 256 x 256 with one (twice as many
+ *   ZFAC_OPT_NARROW_TILES    SPLIT16, HH16, TF32: 256 x 128 pair tiles instead of 256 x 256 (twice as many
  *                            tiles: a small problem occupies more of the chip); -1 = automatically when batch x (padded order / 256)^2
  *                            <= 37 (one problem of padded order <= 1536, or a few smaller ones), 0 = never, 1 = always          -1
  *   ZFAC_OPT_I8_CLUSTER      F64_I8, a1 (when the padded order is a multiple of 512): clusters of two CTA pairs that share

@@ -37,7 +37,7 @@ struct Options {
   int host_overlap = 1;      // zfac_refine_host: early download of Z after the first update
   int host_upload_overlap = 1;   // zfac_refine_host: chunked upload of S overlapped with copy-in + a1
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
-  int narrow_tiles = -1;     // SPLIT16: 256 x 128 tiles (see umma_narrow): -1 auto, 0 never, 1 always (scheduling only)
+  int narrow_tiles = -1;     // tcgen05 modes: 256 x 128 tiles (see umma_narrow): -1 auto, 0 never, 1 always (scheduling only)
   int i8_cluster = 0;        // F64_I8 a1: clusters of two CTA pairs sharing the B slices by TMA multicast (scheduling only)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
   int final_check = 1;       // FP64-master modes: 0 = skip a residual evaluation whose outcome is known beforehand (see stop_decide)
@@ -62,7 +62,7 @@ struct StopArgs {
   int nocheck;               // FP64-master modes, ZFAC_OPT_FINAL_CHECK = 0 (see stop_decide)
   double floor;              // ... the smallest Err worth iterating towards: 2^-53 sqrt(N)
   int tiles_pp;
-  int slots_pt;              // partial sums per tile: 16 (SPLIT16: both epilogue groups work on a tile) or 8 (one-pass kinds)
+  int slots_pt;              // partial sums per tile: 16 per 256 x 256 tile, 8 per 256 x 128 tile (one per warp and 128-column half)
   long long err_stride;
 };
 // n_iter < 0 (inside the loop body of a zfac_graph, whose kernel parameters are fixed): the index comes from the device,

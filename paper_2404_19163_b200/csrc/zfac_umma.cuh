@@ -40,8 +40,11 @@
 
 namespace zfac {
 
-enum { KIND_F16X2 = 0, KIND_HH16 = 1, KIND_TF32 = 2, KIND_F16X2N = 3 };   // F16X2N: F16X2 on 256 x 128 tiles (small problems)
+// ...N: the same kind on 256 x 128 tiles (small launches, ZFAC_OPT_NARROW_TILES)
+enum { KIND_F16X2 = 0, KIND_HH16 = 1, KIND_TF32 = 2, KIND_F16X2N = 3, KIND_HH16N = 4, KIND_TF32N = 5 };
 __host__ __device__ constexpr bool kind_is_pair(int kind) { return kind == KIND_F16X2 || kind == KIND_F16X2N; }
+__host__ __device__ constexpr bool kind_is_tf32(int kind) { return kind == KIND_TF32 || kind == KIND_TF32N; }
+__host__ __device__ constexpr bool kind_is_narrow(int kind) { return kind >= KIND_F16X2N; }
 
 constexpr int UM_TILE_M = 256;                   // pair tile rows: two CTAs x 128 TMEM lanes
 constexpr int UM_MACRO = 256;                    // padding unit and macro tile of the symmetric enumeration
@@ -90,6 +93,12 @@ template <> struct KindTraits<KIND_HH16> {
 };
 template <> struct KindTraits<KIND_TF32> {
   static constexpr int ARRAYS = 1, TILE_N = 256, SETS = 2, STAGES = 6, KSTEP_ELEMS = 8, BK_ELEMS = 32, FMT = 2, SUB = 32;
+};
+template <> struct KindTraits<KIND_HH16N> {
+  static constexpr int ARRAYS = 1, TILE_N = 128, SETS = 2, STAGES = 6, KSTEP_ELEMS = 16, BK_ELEMS = 64, FMT = 0, SUB = 32;
+};
+template <> struct KindTraits<KIND_TF32N> {
+  static constexpr int ARRAYS = 1, TILE_N = 128, SETS = 2, STAGES = 6, KSTEP_ELEMS = 8, BK_ELEMS = 32, FMT = 2, SUB = 32;
 };
 
 struct UmmaParams {
@@ -191,7 +200,7 @@ __device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
 }
 template <int KIND>
 __device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
-  if (KIND == KIND_TF32) {
+  if (kind_is_tf32(KIND)) {
     asm volatile("{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum) : "memory");
   } else {
@@ -322,7 +331,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
   const size_t offt = (size_t)(mb + n) * ld + (m - mb);   // (n, m) of the same problem
   const int ml = m - mb;                               // local row: the diagonal is ml == n
   if (EPI == EPI_A1) {                                  // T = (S Z)^T
-    if (KIND == KIND_TF32) {
+    if (kind_is_tf32(KIND)) {
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
       store_f32_row<SUB>(p.f32_out + off, v);
@@ -343,12 +352,12 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
     }
     tile_sumsq += (double)ss;
     store_f32_row<SUB>(p.f32_out + off, v);
-    if (KIND != KIND_TF32) store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
+    if (!kind_is_tf32(KIND)) store_h_row<PAIR, SUB>(p.h_out, plane, off, v);
     if (offdiag) {
       // mirror: the operand of a4 needs the whole matrix -- the fp16 plane(s), or in TF32 mode the FP32 buffer itself.
       // The FP32 copy of the 16-bit modes is read by a4's / p2's epilogue only, at upper-triangle tiles: its lower
       // triangle is never written (zfac_peek reads the upper one).
-      if (KIND == KIND_TF32) {
+      if (kind_is_tf32(KIND)) {
 #pragma unroll
         for (int j = 0; j < SUB; ++j) p.f32_out[offt + (size_t)j * ld] = v[j];
       } else {
@@ -367,7 +376,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
     const float qd = p.scaled ? p.q_d * p.st->rinv : p.q_d;            // scaled operands: D = R~ R~ = rscale^2 R R
 #pragma unroll
     for (int j = 0; j < SUB; ++j) v[j] = p.q_r * r32[j] + qd * v[j];
-    if (KIND == KIND_TF32) {
+    if (kind_is_tf32(KIND)) {
 #pragma unroll
       for (int j = 0; j < SUB; ++j) v[j] = round_tf32(v[j]);
       store_f32_row<SUB>(p.f32_out + off, v);
@@ -387,7 +396,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
       for (int j = 0; j < SUB; ++j) g[j] = ((ml == n + j) ? p.g_i : 0.0f) + p.g_r * r32[j] + p.g_p * v[j];
     }
-    if (KIND == KIND_TF32) {
+    if (kind_is_tf32(KIND)) {
       float* g32 = static_cast<float*>(p.out2);
 #pragma unroll
       for (int j = 0; j < SUB; ++j) { v[j] = round_tf32(v[j]); g[j] = round_tf32(g[j]); }
@@ -427,7 +436,7 @@ __device__ __forceinline__ void epilogue_cols(const UmmaParams& p, float (&v)[SU
 #pragma unroll
     for (int j = 0; j < SUB; ++j) v[j] += z32[j];
     store_f32_row<SUB>(p.f32_out + off, v);
-    if (KIND == KIND_TF32) {
+    if (kind_is_tf32(KIND)) {
       float* wt = static_cast<float*>(p.h_out_t);
 #pragma unroll
       for (int j = 0; j < SUB; ++j) wt[offt + (size_t)j * ld] = round_tf32(v[j]);
@@ -750,7 +759,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       if (SETS == 2 && (li & 1) != g) continue;
       const uint32_t tuse = (SETS == 2) ? (uint32_t)(li >> 1) : (uint32_t)li;   // tiles this thread has finished
       const int m = m0 + row;
-      double tile_sumsq = 0.0;
+      double tile_sumsq = 0.0, first_half_sumsq = 0.0;
       if (PAIRK) {
         uint32_t hcnt = tuse * (uint32_t)NCH;                  // chunks drained from this set so far
         float sum[GCOLS];
@@ -826,6 +835,8 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
 #pragma unroll
             for (int j = 0; j < SUB; ++j) v[j] = __uint_as_float(r[j]);
           }
+          // a2 on a 256-column tile: one partial sum per 128-column half (as the 128-column kinds form them)
+          if (EPI == EPI_A2 && GCOLS == 256 && cc == GCOLS / SUB / 2) { first_half_sumsq = tile_sumsq; tile_sumsq = 0.0; }
           epilogue_cols<KIND, EPI, SUB>(p, v, m, n0 + col0 + cc * SUB, mb, offdiag, tile_sumsq);
         }
         tc_fence_before();
@@ -834,12 +845,18 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
       }
       // step a3: this warp's share of the tile (slot: CTA of the pair x warp of the tile's epilogue group(s))
       if (EPI == EPI_A2) {
-        // F16X2N: a warp covers the same 32 rows x 128 columns as a warp of the wide kind does; its sum goes where that
-        // warp's would (macro tile, CTA, column half, lane quarter), so Err[] does not depend on the tile width
-        const int lin = (KIND == KIND_F16X2N)
-                            ? (tl >> 1) * 16 + (int)rank * 8 + (tl & 1) * 4 + q
-                            : tl * (2 * UM_EPI_WARPS / SETS) + (int)rank * (UM_EPI_WARPS / SETS) + ((SETS == 2) ? q : (warp - UM_EPI_WARP0));
-        stop_test_index_warp(p.stop, mb / np, lin, offdiag ? 2.0 * tile_sumsq : tile_sumsq, lane);
+        // One sum per warp and 128-column half of a 256 x 256 macro tile, stored at (macro tile, CTA, column half, lane
+        // quarter): 16 per macro tile whatever the kind's tile width and accumulator sets, formed from the same elements in
+        // the same order -- Err[] does not depend on the tile width (ZFAC_OPT_NARROW_TILES).
+        const int macro = kind_is_narrow(KIND) ? (tl >> 1) : tl;
+        const int base = macro * 16 + (int)rank * 8 + q;
+        if (GCOLS == 256) {                                    // one-pass kinds on 256-column tiles: this thread holds both halves
+          stop_test_index_warp(p.stop, mb / np, base, offdiag ? 2.0 * first_half_sumsq : first_half_sumsq, lane);
+          stop_test_index_warp(p.stop, mb / np, base + 4, offdiag ? 2.0 * tile_sumsq : tile_sumsq, lane);
+        } else {
+          const int half = kind_is_narrow(KIND) ? (tl & 1) : g;   // F16X2 on 256 columns: group g holds columns [128 g, 128 g + 128)
+          stop_test_index_warp(p.stop, mb / np, base + half * 4, offdiag ? 2.0 * tile_sumsq : tile_sumsq, lane);
+        }
       }
     }
 #ifdef ZFAC_TIMING
@@ -929,7 +946,8 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Zb[1], H, 2, rows, np)) != cudaSuccess) return e;
     e = (L.mode == ZFAC_MODE_SPLIT16) ? prepare_kind<KIND_F16X2>(&pl->max_pairs, sm_count) : prepare_kind<KIND_HH16>(&pl->max_pairs, sm_count);
     if (e != cudaSuccess) return e;
-    if (L.mode == ZFAC_MODE_SPLIT16 && (e = prepare_kind<KIND_F16X2N>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
+    e = (L.mode == ZFAC_MODE_SPLIT16) ? prepare_kind<KIND_F16X2N>(&pl->max_pairs, sm_count) : prepare_kind<KIND_HH16N>(&pl->max_pairs, sm_count);
+    if (e != cudaSuccess) return e;
   } else {
     const CUtensorMapDataType F = CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     const uint64_t rows = (uint64_t)L.rows;
@@ -941,16 +959,16 @@ inline cudaError_t umma_plan_create(UmmaPlan* pl, const Layout& L, char* ws, int
     if ((e = make_map(enc, &pl->mZ[0], ws + L.off_Z[0], F, 4, rows, np)) != cudaSuccess) return e;
     if ((e = make_map(enc, &pl->mZ[1], ws + L.off_Z[1], F, 4, rows, np)) != cudaSuccess) return e;
     if ((e = prepare_kind<KIND_TF32>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
+    if ((e = prepare_kind<KIND_TF32N>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
   }
   if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
   return cudaSuccess;
 }
 
-// SPLIT16 on 256 x 128 tiles (KIND_F16X2N)?  ZFAC_OPT_NARROW_TILES: 0 never, 1 always, -1 (default) when the full GEMMs of
+// The mode's kind on 256 x 128 tiles (KIND_F16X2N / HH16N / TF32N)?  ZFAC_OPT_NARROW_TILES: 0 never, 1 always, -1 (default) when the full GEMMs of
 // the launch have at most 37 wide tiles (one problem of N <= 1536, or a few smaller ones): the narrow ones then still fit
 // the 74 CTA pairs in one wave.  Larger launches have tiles enough (measured: no gain, a loss from N = 2048 on).
 inline bool umma_narrow(const UmmaPlan& pl) {
-  if (pl.L.mode != ZFAC_MODE_SPLIT16) return false;
   if (pl.opt->narrow_tiles >= 0) return pl.opt->narrow_tiles != 0;
   const long T = (long)(pl.L.np / UM_MACRO);
   return (long)pl.L.batch * T * T <= 37;
@@ -971,10 +989,9 @@ inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) 
   }
 }
 inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const UmmaParams& p, bool narrow = false) {
-  if (mode == ZFAC_MODE_SPLIT16 && narrow) umma_launch<KIND_F16X2N>(epi, grid, s, p);
-  else if (mode == ZFAC_MODE_SPLIT16) umma_launch<KIND_F16X2>(epi, grid, s, p);
-  else if (mode == ZFAC_MODE_HH16) umma_launch<KIND_HH16>(epi, grid, s, p);
-  else umma_launch<KIND_TF32>(epi, grid, s, p);
+  if (mode == ZFAC_MODE_SPLIT16) { if (narrow) umma_launch<KIND_F16X2N>(epi, grid, s, p); else umma_launch<KIND_F16X2>(epi, grid, s, p); }
+  else if (mode == ZFAC_MODE_HH16) { if (narrow) umma_launch<KIND_HH16N>(epi, grid, s, p); else umma_launch<KIND_HH16>(epi, grid, s, p); }
+  else { if (narrow) umma_launch<KIND_TF32N>(epi, grid, s, p); else umma_launch<KIND_TF32>(epi, grid, s, p); }
 }
 
 // The two halves of one iteration as the host enqueues them.  The only dependence on the iteration index n is (i) the
@@ -994,8 +1011,7 @@ struct UmmaSeq {
     char* ws = pl.ws;
     const int T = (int)(L.np / UM_MACRO);
     narrow = umma_narrow(pl);
-    const int nsplit = UM_MACRO / (narrow ? KindTraits<KIND_F16X2N>::TILE_N : L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
-                                   : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
+    const int nsplit = narrow ? 2 : 1;                       // 256 / TILE_N of the kind that runs
     const int full_tiles = T * T * nsplit * L.batch, sym_tiles = T * (T + 1) / 2 * nsplit * L.batch;
     grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
     grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());
@@ -1010,8 +1026,7 @@ struct UmmaSeq {
     p.stop.num_partials = 0; p.stop.d_err = d_err; p.stop.max_iter = max_iter; p.stop.stop = stop;
     p.stop.order = order; p.stop.cond = cond;
     p.stop.tiles_pp = T * (T + 1) / 2 * nsplit; p.stop.err_stride = (long long)max_iter + 1;
-    p.stop.slots_pt = 2 * UM_EPI_WARPS / (narrow ? KindTraits<KIND_F16X2N>::SETS
-                                          : L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::SETS : KindTraits<KIND_HH16>::SETS);
+    p.stop.slots_pt = 16 / nsplit;                           // a2: 16 partial sums per 256 x 256 macro tile (see the epilogue)
     const PolyCoef pc = poly_coef(order);
     p.q_r = (float)pc.q_r; p.q_d = (float)pc.q_d; p.g_i = (float)pc.g_i; p.g_r = (float)pc.g_r; p.g_p = (float)pc.g_p;
     R32 = reinterpret_cast<float*>(ws + L.off_R);
@@ -1145,8 +1160,7 @@ inline cudaError_t umma_congruence(const UmmaPlan& pl, cudaStream_t s, int* laun
   char* ws = pl.ws;
   const int T = (int)(L.np / UM_MACRO);
   const bool narrow = umma_narrow(pl);
-  const int nsplit = UM_MACRO / (narrow ? KindTraits<KIND_F16X2N>::TILE_N : L.mode == ZFAC_MODE_SPLIT16 ? KindTraits<KIND_F16X2>::TILE_N
-                                 : L.mode == ZFAC_MODE_HH16 ? KindTraits<KIND_HH16>::TILE_N : KindTraits<KIND_TF32>::TILE_N);
+  const int nsplit = narrow ? 2 : 1;
   const int full_tiles = T * T * nsplit, sym_tiles = T * (T + 1) / 2 * nsplit;
   const int grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
   const int grid_sym = 2 * (sym_tiles < pl.pairs() ? sym_tiles : pl.pairs());

@@ -1375,19 +1375,20 @@ def test_batched_context_argument_checks():
         assert e.value.status == b.ZFAC_E_INVALID
 
 
+@pytest.mark.parametrize("mode", ["split16", "hh16", "tf32"])
 @pytest.mark.parametrize("n", [200, 700, 1300])
-def test_narrow_tiles_are_scheduling_only(n):
+def test_narrow_tiles_are_scheduling_only(n, mode):
     """ZFAC_OPT_NARROW_TILES (SPLIT16 on 256 x 128 pair tiles with two accumulator sets; the default for one problem of padded
     order <= 1536): every output element is accumulated in the same order and the a2 partial sums sit where the wide tiles'
     would, so Z, the whole history, the flags, the congruence and the order-3 / 4 updates are bit-identical to the
     256 x 256 tiles (option 0) -- what changes is the number of tiles.  Also under ZFAC_OPT_MAX_PAIRS."""
     b = zb()
     w = W.random_spd_general(n, seed=40 + n, kappa=30.0, pert=0.05, fp32_stored=True)
-    S, Z0 = _to_dev(w.S, "split16"), _to_dev(w.Z0, "split16")
-    H = _to_dev(W.random_spd_general(n, seed=41 + n, kappa=5.0, pert=0.0, fp32_stored=True).S, "split16")
+    S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
+    H = _to_dev(W.random_spd_general(n, seed=41 + n, kappa=5.0, pert=0.0, fp32_stored=True).S, mode)
     results = {}
     for nt in (0, 1, -1):
-        with b.Zfac(n, "split16", DEV) as zf:
+        with b.Zfac(n, mode, DEV) as zf:
             assert zf.get_option("narrow_tiles") == -1
             zf.set_option("narrow_tiles", nt)
             out = []
@@ -1408,7 +1409,7 @@ def test_narrow_tiles_are_scheduling_only(n):
             assert torch.equal(a[0], c[0]) and torch.equal(a[4], c[4]) and torch.equal(a[5], c[5]), (n, nt)
         assert torch.equal(results[0][-1], results[nt][-1]), (n, nt)
     ora = O.refine(w.S, w.Z0, results[0][0][1], O.STOP_FIXED)
-    assert _rel(results[1][0][0].cpu().double().numpy(), ora.Z) <= TOL["split16"]
-    with b.Zfac(256, "hh16", DEV) as zf:
+    assert _rel(results[1][0][0].cpu().double().numpy(), ora.Z) <= TOL[mode]
+    with b.Zfac(256, "f64", DEV) as zf:
         with pytest.raises(b.ZfacError):
             zf.set_option("narrow_tiles", 1)
