@@ -554,6 +554,13 @@ class ZfacBatch:
             raise ValueError("batch must be >= 1")
         self.n, self.batch, self.device = int(n), int(batch), torch.device(device)
         self.ctxs = [Zfac(n, mode, device) for _ in range(batch)]
+        # each context sees one problem and would pick 256 x 128 tiles for it (ZFAC_OPT_NARROW_TILES = -1); together the
+        # contexts fill the chip with wide tiles once batch x (padded n / 256)^2 exceeds 37 -- the library's own rule,
+        # applied here to the whole set (measured, 16 streams at n = 1024: 301 TFLOP/s wide, 219 narrow)
+        t = zfac_padded_n(self.n, self.ctxs[0].mode) // 256
+        if self.ctxs[0].mode in (ZFAC_MODE_SPLIT16, ZFAC_MODE_HH16, ZFAC_MODE_TF32) and self.batch * t * t > 37:
+            for c in self.ctxs:
+                c.set_option("narrow_tiles", 0)
         self.streams = [torch.cuda.Stream(self.device) for _ in range(batch)]
         self.dtype = self.ctxs[0].dtype
 
