@@ -312,7 +312,6 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
     m0 = I * UM_TILE_M; n0 = J * TN;
   };
 
-  double cta_sumsq = 0.0;
 
   if (warp == 0) {
     // ===================================================== TMA producer (both CTAs)
@@ -445,15 +444,16 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
           }
         }
       }
-      if (EPI == EPI_A2) cta_sumsq += offdiag ? 2.0 * tile_sumsq : tile_sumsq;
+      if (EPI == EPI_A2) {
+        // step a3, first half: one partial sum per tile, CTA of the pair, column half and lane quarter, stored by TILE index --
+        // Err[] does not depend on which pair computed which tile (ZFAC_OPT_MAX_PAIRS, another SM count)
+        const double ws_ = warp_sum(offdiag ? 2.0 * tile_sumsq : tile_sumsq);
+        if (lane == 0) { p.stop.partials[(size_t)t * 16 + rank * 8 + g * 4 + q] = ws_; __threadfence(); }
+      }
     }
   }
 
   // ------------------------------------------------------- teardown (+ step a3 for a2)
-  if (EPI == EPI_A2) {
-    const double s = warp_sum(warp >= UM_EPI_WARP0 ? cta_sumsq : 0.0);
-    if (lane == 0) red[warp] = s;
-  }
   tc_fence_before();
   __syncthreads();
   cluster_sync_all();
@@ -462,12 +462,8 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(UM_TMEM_COLS) : "memory");
   }
   if (EPI == EPI_A2) {
-    if (threadIdx.x == 0) {
-      double tot = 0.0;
-      for (int w = UM_EPI_WARP0; w < UM_EPI_WARP0 + UM_EPI_WARPS; ++w) tot += red[w];
-      if (*((volatile int*)&p.st->range) & 2) tot = nan("");   // a non-finite operand was met while slicing
-      p.stop.partials[blockIdx.x] = tot;
-    }
+    // a non-finite operand was met while slicing: Err[n] is NaN (one slot of this CTA's first tile carries it)
+    if (threadIdx.x == 0 && (*((volatile int*)&p.st->range) & 2)) p.stop.partials[(size_t)pair * 16 + rank * 8] = nan("");
     if (arrive_is_last(&p.st->arrive[0], gridDim.x, &last_flag)) stop_test_last_cta(p.stop, red);
   }
 }
@@ -587,7 +583,7 @@ struct MixSeq {
       p.np = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band > 1 ? pl.opt->band / 2 : 1;
       p.sa = p.sb = p.orders = pl.opt->i8_slices;
       p.scratch = reinterpret_cast<double*>(ws + L.off_scratch);
-      p.st = st; p.stop = stop; p.stop.num_partials = grid_sym;
+      p.st = st; p.stop = stop; p.stop.num_partials = 16 * p.macro_tiles * (p.macro_tiles + 1) / 2;     // a2: 16 per tile
       int* eS = reinterpret_cast<int*>(ws + L.off_exp);
       int* eW = eS + L.np; int* eT = eW + L.np;
       // a1: T = W S^T (FP64 out), then its rows sliced for a2
