@@ -356,7 +356,9 @@ static zfac_status refine_mix(zfac_ctx* c, int max_iter, zfac_stop stop, double*
   MixSeq q(c->mix, max_iter, (int)stop, d_err, 0ull);
   for (int n = 0; n <= max_iter; ++n) {
     if (n == max_iter && skip_last) break;
-    q.residual(n, n, s, &c->prof);
+    // zfac_refine_host, I8 engine: slicing of S + a1 of the first residual band by band, behind the row chunks of the upload
+    const bool banded = (n == 0) && hook && hook->first_a1 && hook->first_a1(hook->self, &q, s);
+    q.residual(n, n, s, &c->prof, banded);
     if (n == max_iter) break;
     if (hook && hook->before_update) hook->before_update(hook->self, n, s);
     q.update(n & 1, n, n, s, &c->prof);
@@ -394,6 +396,7 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
   if (mode_is_mix(c->mode)) {
     // FP64 master Z (+ S, W in FP64 for the DMMA engine), then the FP32 operand pair of Z; I8 engine: int8 slices of S and W
     const bool i8 = (c->mode == ZFAC_MODE_F64_I8);
+    const bool with_S = (what & 1) != 0;                       // what = 2: the host entry point slices S band by band (a1_band)
     ci.what = i8 ? (2 | 4) : 3;
     if (in_f32) copy_in_kernel<ZFAC_MODE_F64, float><<<gi, bi, 0, s>>>(ci);
     else copy_in_kernel<ZFAC_MODE_F64, double><<<gi, bi, 0, s>>>(ci);
@@ -404,7 +407,8 @@ static void launch_copy_in(zfac_ctx* c, const void* d_S, int64_t lds, const void
     if (i8) {
       int* eS = reinterpret_cast<int*>(ws + L.off_exp);
       int8_t* S8 = reinterpret_cast<int8_t*>(ws + L.off_S8);
-      if (in_f32) slice_rows_kernel<float><<<small_grid((size_t)L.np), 256, 0, s>>>(static_cast<const float*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
+      if (!with_S) {}
+      else if (in_f32) slice_rows_kernel<float><<<small_grid((size_t)L.np), 256, 0, s>>>(static_cast<const float*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
       else slice_rows_kernel<double><<<small_grid((size_t)L.np), 256, 0, s>>>(static_cast<const double*>(d_S), lds, (int)c->n, (int)L.np, c->opt.i8_slices, S8, eS, ci.st);
       MixSeq q(c->mix, 0, 0, nullptr, 0ull);
       q.w_slices(s);
@@ -547,6 +551,20 @@ static bool host_first_a1(void* self, void* seq, cudaStream_t s) {
   }
   return true;
 }
+// ... and the same for the I8 engine of ZFAC_MODE_F64_I8 (seq is a MixSeq): slices of the S rows of a chunk, then the tile
+// columns of T = W S^T that need exactly those rows.
+static bool host_first_a1_i8(void* self, void* seq, cudaStream_t s) {
+  HostOverlap* h = static_cast<HostOverlap*>(self);
+  if (h->chunks <= 0) return false;
+  zfac_ctx* c = h->c;
+  MixSeq* q = static_cast<MixSeq*>(seq);
+  for (int k = 0; k < h->chunks; ++k) {
+    int mc0, mcn; host_chunk_rows(c, h->chunks, k, &mc0, &mcn);
+    cudaStreamWaitEvent(s, c->ev_up[1 + k], 0);
+    q->a1_band(h->dS, c->n, c->opt.input_f32 != 0, (int)c->n, mc0, mcn, s);
+  }
+  return true;
+}
 static void host_before_update(void* self, int n, cudaStream_t s) {
   HostOverlap* h = static_cast<HostOverlap*>(self);
   if (n >= 1 && n <= h->early) cudaStreamWaitEvent(s, h->c->ev_copy, 0);      // the download of Z_n has left the master buffer
@@ -669,7 +687,7 @@ static zfac_status host_upload(zfac_ctx* c, const void* h_S, int64_t lds, const 
   const size_t elt = (mode_is_f64_elt(c->mode) && c->opt.input_f32) ? 4 : L.elt;      // element size of the INPUTS
   const size_t row = (size_t)c->n * elt;
   int chunks = 0;
-  if (mode_is_umma(c->mode) && L.np / UM_MACRO >= 4 && c->opt.host_upload_overlap) {
+  if ((mode_is_umma(c->mode) || c->mode == ZFAC_MODE_F64_I8) && L.np / UM_MACRO >= 4 && c->opt.host_upload_overlap) {
     cudaPointerAttributes pS{}, pZ{};
     if (cudaPointerGetAttributes(&pS, h_S) == cudaSuccess && pS.type == cudaMemoryTypeHost &&
         cudaPointerGetAttributes(&pZ, h_Z0) == cudaSuccess && pZ.type == cudaMemoryTypeHost) {
@@ -742,7 +760,7 @@ zfac_status zfac_refine_host(zfac_ctx* c, const void* h_S, int64_t lds, const vo
   HostOverlap ho{c, h_Z, ldz};
   ho.dS = dS; ho.chunks = chunks;
   IterHook hook{z_dev ? host_after_a5 : nullptr, &ho};
-  if (chunks > 0) hook.first_a1 = host_first_a1;
+  if (chunks > 0) hook.first_a1 = mode_is_mix(c->mode) ? host_first_a1_i8 : host_first_a1;
   if (z_dev && mode_is_mix(c->mode) && max_iter >= 2) {
     // one update of these modes (a full FP64-level residual) outlasts the download: the results of the first TWO updates
     // are sent early, each behind its update; the master is updated in place, so update n + 1 waits for the download of Z_n
@@ -820,7 +838,7 @@ zfac_status zfac_refine_refi_host(zfac_ctx* low, zfac_ctx* high, const void* h_S
   HostOverlap ho{low, nullptr, 0};
   ho.dS = dS; ho.chunks = chunks;
   IterHook low_hook{nullptr, &ho};
-  low_hook.first_a1 = host_first_a1;
+  low_hook.first_a1 = mode_is_mix(low->mode) ? host_first_a1_i8 : host_first_a1;
   const bool z_dev = high->opt.host_overlap && host_pinned(h_Z);
   RefiDownload rd{high, h_Z, ldz, refi_steps - 1};
   IterHook high_hook{refi_after_a5, &rd};

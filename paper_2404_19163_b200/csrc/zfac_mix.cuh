@@ -122,12 +122,14 @@ __device__ __forceinline__ void slice16(const double (&a)[16], int e, int slices
 // One CTA per row: pass 1 = row maximum, pass 2 = slices.  Used for S (from the caller's buffer) and T = (S Z)^T.
 template <typename Tin>
 __global__ void __launch_bounds__(256) slice_rows_kernel(const Tin* __restrict__ src, int64_t ld, int n, int np, int slices,
-                                                         int8_t* __restrict__ out, int* __restrict__ exps, State* st) {
+                                                         int8_t* __restrict__ out, int* __restrict__ exps, State* st,
+                                                         int row0 = 0, int rows = 0 /* 0: all np rows */) {
   if (*((volatile int*)&st->done)) return;
   __shared__ double red[8];
   __shared__ int e_sh;
   const int t = threadIdx.x;
-  for (int r = blockIdx.x; r < np; r += gridDim.x) {
+  const int r_end = rows > 0 ? row0 + rows : np;
+  for (int r = row0 + blockIdx.x; r < r_end; r += gridDim.x) {
   double mx = 0.0;
   if (r < n) {
     for (int c = t; c < n; c += 256) mx = fmax(mx, fabs((double)src[(size_t)r * ld + c]));
@@ -220,6 +222,8 @@ struct I8Params {
   double* out64;              // a1: T (FP64)
   float* out32;               // a2: R (FP32, both triangles)
   int band;
+  int joff, jcols;            // a1: this launch covers the tile columns [joff, joff + jcols) of T only (jcols = 0: all), i.e. the
+                              // rows [256 joff, ...) of S: zfac_refine_host runs a1 band by band while the row chunks of S arrive
 };
 
 __device__ __forceinline__ void tc_mma_pair_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum) {
@@ -284,7 +288,8 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
   const int np = p.np;
   const int KB = np / 128;                                   // k-blocks of 128 int8
   const int T = p.macro_tiles;
-  const int num_tiles = SYM ? T * (T + 1) / 2 : (T / CP) * T;
+  const int JC = (!SYM && p.jcols > 0) ? p.jcols : T;          // tile columns of this launch
+  const int num_tiles = SYM ? T * (T + 1) / 2 : (T / CP) * JC;
   const int ORD = p.orders;
 
   if (threadIdx.x == 0) {
@@ -308,7 +313,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
   auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
     int I, J;
     if (SYM) { tri_decode(t, I, J); offdiag = (I != J); }
-    else { band_decode(t, T / CP, T, p.band, I, J); I = I * CP + pp; offdiag = true; }
+    else { band_decode(t, T / CP, JC, p.band, I, J); I = I * CP + pp; J += p.joff; offdiag = true; }
     m0 = I * UM_TILE_M; n0 = J * TN;
   };
 
@@ -557,7 +562,7 @@ struct MixSeq {
     np2 = (size_t)L.np * (size_t)L.np;
   }
 
-  void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof) {
+  void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof, bool skip_a1 = false) {
     const Layout& L = pl.L;
     char* ws = pl.ws;
     stop.n_iter = n_stop;
@@ -589,6 +594,7 @@ struct MixSeq {
       // a1: T = W S^T (FP64 out), then its rows sliced for a2
       p.mapA = pl.mW8; p.mapB = pl.mS8; p.expA = eW; p.expB = eS; p.out64 = reinterpret_cast<double*>(ws + L.off_T);
       if (prof) prof->mark(s, EPI_A1 + 16 * tagn);
+      if (!skip_a1) {
       // clusters of two pairs (B slices shared by TMA multicast) when the option is on and the tile rows pair up
       int quads = pl.max_quads;
       if (pl.opt->max_pairs > 0 && pl.opt->max_pairs / 2 < quads) quads = pl.opt->max_pairs / 2;
@@ -599,13 +605,15 @@ struct MixSeq {
         i8_gemm_kernel<EPI_A1, 2><<<4 * nq, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
       } else
       i8_gemm_kernel<EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      ++nl;
+      }
       slice_rows_kernel<double><<<small_grid((size_t)L.np), 256, 0, s>>>(p.out64, L.np, (int)L.np, (int)L.np, p.orders,
                                                                  reinterpret_cast<int8_t*>(ws + L.off_T8), eT, st);
       // a2: R = I - W T^T (FP32 out, both triangles), sum R^2, stop test
       p.mapA = pl.mW8; p.mapB = pl.mT8; p.expA = eW; p.expB = eT; p.out64 = nullptr; p.out32 = reinterpret_cast<float*>(ws + L.off_R);
       if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
       i8_gemm_kernel<EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
-      nl += 3;
+      nl += 2;
       if (stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(st, stop.cond);
     }
   }
@@ -638,6 +646,29 @@ struct MixSeq {
     umma_launch<KIND_F16X2>(EPI_A5X, grid_full, s, p);
     nl += 3;
     if (L.mode == ZFAC_MODE_F64_I8) { w_slices(s); }
+  }
+
+  // I8 engine, zfac_refine_host: the rows [256 mc0, 256 (mc0 + mcn)) of S (at d_S, element type float if in_f32) are sliced
+  // and the tile columns [mc0, mc0 + mcn) of T = W S^T computed from them.  Tiles do not overlap between bands and every
+  // element is formed as in the full launch: bit-identical to it.
+  void a1_band(const void* d_S, int64_t lds, bool in_f32, int n, int mc0, int mcn, cudaStream_t s) {
+    const Layout& L = pl.L;
+    char* ws = pl.ws;
+    int* eS = reinterpret_cast<int*>(ws + L.off_exp);
+    int8_t* S8 = reinterpret_cast<int8_t*>(ws + L.off_S8);
+    const int row0 = mc0 * UM_MACRO, rows = mcn * UM_MACRO;
+    if (in_f32) slice_rows_kernel<float><<<small_grid((size_t)rows), 256, 0, s>>>(static_cast<const float*>(d_S), lds, n, (int)L.np, pl.opt->i8_slices, S8, eS, st, row0, rows);
+    else slice_rows_kernel<double><<<small_grid((size_t)rows), 256, 0, s>>>(static_cast<const double*>(d_S), lds, n, (int)L.np, pl.opt->i8_slices, S8, eS, st, row0, rows);
+    I8Params p{};
+    p.np = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band > 1 ? pl.opt->band / 2 : 1;
+    p.sa = p.sb = p.orders = pl.opt->i8_slices;
+    p.scratch = reinterpret_cast<double*>(ws + L.off_scratch);
+    p.st = st; p.stop = stop;
+    p.mapA = pl.mW8; p.mapB = pl.mS8; p.expA = eS + L.np; p.expB = eS; p.out64 = reinterpret_cast<double*>(ws + L.off_T);
+    p.joff = mc0; p.jcols = mcn;
+    const int tiles = p.macro_tiles * mcn;
+    i8_gemm_kernel<EPI_A1><<<2 * (tiles < pl.pairs() ? tiles : pl.pairs()), UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    nl += 2;
   }
 
   // I8 engine: W = Z^T as int8 slices (column maxima of Z, then transposed slicing)

@@ -430,3 +430,29 @@ def test_i8_cluster_option_is_scheduling_only():
     with b.Zfac(256, "f64mix", DEV) as zf:
         with pytest.raises(b.ZfacError):
             zf.set_option("i8_cluster", 1)
+
+
+@pytest.mark.parametrize("f32", [0, 1])
+def test_f64i8_host_entry_point_with_the_banded_upload_is_bitwise_the_device_entry_point(f32):
+    """zfac_refine_host in ZFAC_MODE_F64_I8 with pinned inputs and >= 4 tile rows: Z0 goes up first, S follows in row chunks,
+    each chunk sliced and multiplied (the tile columns of T = W S^T that need its rows) as it arrives.  Same tiles, same
+    arithmetic: Z, iters, Err[] and flags are the device entry point's bit for bit; with the option off as well."""
+    b = zb()
+    n = 1100                                                                  # padded to 1280: 5 tile rows, 5 upload chunks
+    w = W.random_spd_general(n, seed=61, kappa=200.0, pert=0.05, fp32_stored=True)
+    idt = torch.float32 if f32 else torch.float64
+    with b.Zfac(n, "f64i8", DEV) as zf:
+        zf.set_option("input_f32", f32)
+        Sd, Zd = _dev(w.S, idt), _dev(w.Z0, idt)
+        Zref, itref, errref, flref = zf.refine(Sd, Zd, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+        Zref = Zref.cpu()
+        assert O.final_residual_per_sqrt_n(w.S, Zref.numpy()) < 1e-12
+        hS = torch.full((n, n + 4), float("nan"), dtype=idt); hS[:, :n] = torch.from_numpy(w.S).to(idt)
+        hS = hS.pin_memory()
+        hZ0 = torch.from_numpy(np.ascontiguousarray(w.Z0)).to(idt).pin_memory()
+        for overlap in (1, 0):
+            zf.set_option("host_upload_overlap", overlap)
+            hZ = torch.full((n, n), -2.0, dtype=torch.float64).pin_memory()
+            _, it, err, fl = zf.refine_host(hS[:, :n], hZ0, hZ, max_iter=30, stop=b.ZFAC_STOP_PAPER)
+            assert it == itref and fl == flref and np.array_equal(err, errref), overlap
+            assert torch.equal(hZ, Zref), overlap
