@@ -143,6 +143,13 @@ def build_workload(name, n, dev, rank=0):
 
 
 # ----------------------------------------------------------------------------- reference arm (oracle on host cores)
+def bench_config(args, world):
+    """`config` of the JSON line: names the workload and how it is run; identical for both arms."""
+    return {"workload": f"{args.workload}_n{args.n}", "mode": args.mode, "options": args.option or None, "N": args.n,
+            "stop": args.stop, "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
+            "l2": "operands (2.4 GB) exceed L2 (126 MB); no flush needed"}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -179,7 +186,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{args.workload}_n{args.n}", "mode": "oracle_fp64", "N": args.n},
+            # the SAME config object as the arm it is compared with (the driver checks it); what the oracle computes in (FP64,
+            # numpy on the host cores) is said by `dtype` and `cpu_baseline`
+            "config": bench_config(args, int(os.environ.get("WORLD_SIZE", "1"))),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0, "Err0": e0}
@@ -866,9 +875,7 @@ def run_ours(args):
                       "hh16": "f16 (one pass), f32 accumulate", "f64mix": "f64 residual, f16-pair update into an f64 master",
                       "f64i8": "int8 slices (exact int32 accumulate) for the f64-level residual, f16-pair update into an f64 master"}[args.mode],
             "data": "synthetic",
-            "config": {"workload": f"{args.workload}_n{n}", "mode": args.mode, "options": args.option or None, "N": n, "stop": args.stop,
-                       "max_iter": args.max_iter, "parallelism": "replicas" if world > 1 else "single",
-                       "l2": "operands (2.4 GB) exceed L2 (126 MB); no flush needed"},
+            "config": bench_config(args, world),
             "iters": iters, "iters_per_s": primary["iters_per_s"] * world, "time_to_converged_ms": t_ms,
             "err_history": primary["err"], "flags": primary["flags"],
             "final_residual_per_sqrt_n": primary.get("final_residual_per_sqrt_n"),
