@@ -275,6 +275,10 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *   ZFAC_OPT_NARROW_TILES    SPLIT16, HH16, TF32: 256 x 128 pair tiles instead of 256 x 256 (twice as many
  *                            tiles: a small problem occupies more of the chip); -1 = automatically when batch x (padded order / 256)^2
  *                            <= 37 (one problem of padded order <= 1536, or a few smaller ones), 0 = never, 1 = always          -1
+ *   ZFAC_OPT_PDL             SPLIT16, HH16, TF32: programmatic dependent launch of the GEMM kernels (a kernel is scheduled while
+ *                            its predecessor still runs and waits for it on the device before it reads anything); not
+ *                            used inside zfac_graph_*; -1 = automatically (HH16 / TF32 up to padded order 2048, where it
+ *                            takes 7 .. 15 % off a call; SPLIT16: no gain measured), 0 = never, 1 = always               -1
  *   ZFAC_OPT_I8_CLUSTER      F64_I8, a1 (when the padded order is a multiple of 512): clusters of two CTA pairs that share
  *                            the B slices by TMA multicast (L2 -> SM bytes -25 %); only 33 such clusters are co-resident on a
  *                            B200 against 74 pairs, measured a tie; 0 / 1                              0
@@ -284,7 +288,7 @@ typedef enum {
   ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
   ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10, ZFAC_OPT_INPUT_F32 = 11,
   ZFAC_OPT_EXTRA_UPDATE = 12, ZFAC_OPT_FINAL_CHECK = 13, ZFAC_OPT_I8_CLUSTER = 14,
-  ZFAC_OPT_NARROW_TILES = 15
+  ZFAC_OPT_NARROW_TILES = 15, ZFAC_OPT_PDL = 16
 } zfac_option;
 zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
 zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);

@@ -461,7 +461,13 @@ template <int KIND, int EPI>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(UM_THREADS, 1)
 umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   // stop decided earlier in this call (uniform over the grid); in a batched launch finished problems are skipped tile by tile
+  // Programmatic dependent launch (launches with the attribute; a no-op otherwise): this grid may have been scheduled while
+  // its predecessor in the stream was still running.  Nothing of global memory is touched before the predecessor has
+  // completed (wait); then the successor is let in at once -- it takes SMs as they fall free and waits here in turn, so
+  // its launch latency is hidden behind this kernel (the kernels of a small problem, the early-exit launches behind the stop).
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   if (p.batch == 1 && *((volatile int*)&p.st->done)) return;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   using KT = KindTraits<KIND>;
   constexpr bool SYM = (EPI == EPI_A2 || EPI == EPI_A4 || EPI == EPI_X3 || EPI == EPI_P2);
@@ -974,24 +980,36 @@ inline bool umma_narrow(const UmmaPlan& pl) {
   return (long)pl.L.batch * T * T <= 37;
 }
 
+// pdl: launch with cudaLaunchAttributeProgrammaticStreamSerialization (see the head of the kernel)
+template <int KIND, int EPI>
+inline void umma_launch_one(int grid, cudaStream_t s, const UmmaParams& p, bool pdl) {
+  if (!pdl) { umma_gemm_kernel<KIND, EPI><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); return; }
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, umma_gemm_kernel<KIND, EPI>, p);
+}
 template <int KIND>
-inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p) {
+inline void umma_launch(int epi, int grid, cudaStream_t s, const UmmaParams& p, bool pdl = false) {
   switch (epi) {
-    case EPI_A1: umma_gemm_kernel<KIND, EPI_A1><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
-    case EPI_A2: umma_gemm_kernel<KIND, EPI_A2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
-    case EPI_X3: umma_gemm_kernel<KIND, EPI_X3><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
-    case EPI_A4: umma_gemm_kernel<KIND, EPI_A4><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
-    case EPI_P2: umma_gemm_kernel<KIND, EPI_P2><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    case EPI_A1: umma_launch_one<KIND, EPI_A1>(grid, s, p, pdl); break;
+    case EPI_A2: umma_launch_one<KIND, EPI_A2>(grid, s, p, pdl); break;
+    case EPI_X3: umma_launch_one<KIND, EPI_X3>(grid, s, p, pdl); break;
+    case EPI_A4: umma_launch_one<KIND, EPI_A4>(grid, s, p, pdl); break;
+    case EPI_P2: umma_launch_one<KIND, EPI_P2>(grid, s, p, pdl); break;
     case EPI_A5X:
-      if (KIND == KIND_F16X2) umma_gemm_kernel<KIND_F16X2, EPI_A5X><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      if (KIND == KIND_F16X2) umma_launch_one<KIND_F16X2, EPI_A5X>(grid, s, p, pdl);
       break;                                               // (FP64-master modes: wide tiles only)
-    default:     umma_gemm_kernel<KIND, EPI_A5><<<grid, UM_THREADS, UM_SMEM_BYTES, s>>>(p); break;
+    default:     umma_launch_one<KIND, EPI_A5>(grid, s, p, pdl); break;
   }
 }
-inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const UmmaParams& p, bool narrow = false) {
-  if (mode == ZFAC_MODE_SPLIT16) { if (narrow) umma_launch<KIND_F16X2N>(epi, grid, s, p); else umma_launch<KIND_F16X2>(epi, grid, s, p); }
-  else if (mode == ZFAC_MODE_HH16) { if (narrow) umma_launch<KIND_HH16N>(epi, grid, s, p); else umma_launch<KIND_HH16>(epi, grid, s, p); }
-  else { if (narrow) umma_launch<KIND_TF32N>(epi, grid, s, p); else umma_launch<KIND_TF32>(epi, grid, s, p); }
+inline void umma_launch_mode(int mode, int epi, int grid, cudaStream_t s, const UmmaParams& p, bool narrow = false, bool pdl = false) {
+  if (mode == ZFAC_MODE_SPLIT16) { if (narrow) umma_launch<KIND_F16X2N>(epi, grid, s, p, pdl); else umma_launch<KIND_F16X2>(epi, grid, s, p, pdl); }
+  else if (mode == ZFAC_MODE_HH16) { if (narrow) umma_launch<KIND_HH16N>(epi, grid, s, p, pdl); else umma_launch<KIND_HH16>(epi, grid, s, p, pdl); }
+  else { if (narrow) umma_launch<KIND_TF32N>(epi, grid, s, p, pdl); else umma_launch<KIND_TF32>(epi, grid, s, p, pdl); }
 }
 
 // The two halves of one iteration as the host enqueues them.  The only dependence on the iteration index n is (i) the
@@ -1011,6 +1029,9 @@ struct UmmaSeq {
     char* ws = pl.ws;
     const int T = (int)(L.np / UM_MACRO);
     narrow = umma_narrow(pl);
+    // measured (10 updates, on / off): HH16 N = 512 / 1024 / 2048 0.54 / 0.64 / 1.16 against 0.65 / 0.74 / 1.25 ms, TF32 alike, a tie
+    // at N = 3072; SPLIT16 +-1 % at every size -> automatic (-1): the one-pass modes up to 8 x 8 macro tiles
+    pdl = (cond == 0ull) && (pl.opt->pdl >= 0 ? pl.opt->pdl != 0 : (L.mode != ZFAC_MODE_SPLIT16 && T <= 8));
     const int nsplit = narrow ? 2 : 1;                       // 256 / TILE_N of the kind that runs
     const int full_tiles = T * T * nsplit * L.batch, sym_tiles = T * (T + 1) / 2 * nsplit * L.batch;
     grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());
@@ -1035,6 +1056,7 @@ struct UmmaSeq {
 
   int nsplit_ = 1;
   bool narrow = false;
+  bool pdl = false;            // programmatic dependent launch of the GEMM kernels (not inside a captured graph)
 
   // a1 restricted to the macro-tile columns [mc0, mc0 + mcn) of T, i.e. to the rows [256 mc0, 256 (mc0 + mcn)) of S
   // (mcn = 0: all of T).  Tiles do not overlap between bands, so a banded a1 is bit-identical to the full launch.
@@ -1052,7 +1074,7 @@ struct UmmaSeq {
       const int tiles = p.macro_tiles * p.jcols;
       grid = 2 * (tiles < pl.pairs() ? tiles : pl.pairs());
     }
-    umma_launch_mode(L.mode, EPI_A1, grid, s, p, narrow);
+    umma_launch_mode(L.mode, EPI_A1, grid, s, p, narrow, pdl);
     p.joff = 0; p.jcols = 0;
     nl += 1;
   }
@@ -1072,7 +1094,7 @@ struct UmmaSeq {
     // a2 writes four outputs per element: its stores take twice as long, so a long first chunk (if one is set) doubles
     if (pl.opt->chunk0_kb > pl.opt->chunk_kb) p.chunk0_kb = 2 * pl.opt->chunk0_kb;
     p.h_out = h16 ? ws + L.off_Rb : nullptr;
-    umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p, narrow);
+    umma_launch_mode(L.mode, EPI_A2, grid_sym, s, p, narrow, pdl);
     nl += 1;
     if (p.stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(p.st, p.stop.cond);       // zfac_graph_*: loop condition
   }
@@ -1096,7 +1118,7 @@ struct UmmaSeq {
       p.mapA = pl.mR; p.mapB = pl.mR; p.f32_in = R32;
       if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_T; p.out2 = ws + L.off_Zb[(par + 1) & 1]; }
       else { p.f32_out = reinterpret_cast<float*>(ws + L.off_T); p.h_out = nullptr; p.out2 = ws + L.off_Z[(par + 1) & 1]; }
-      umma_launch_mode(L.mode, EPI_P2, grid_sym, s, p, narrow);
+      umma_launch_mode(L.mode, EPI_P2, grid_sym, s, p, narrow, pdl);
       nl += 1;
       p.out2 = nullptr;
     }
@@ -1106,7 +1128,7 @@ struct UmmaSeq {
     p.f32_in = R32;
     if (h16) { p.f32_out = nullptr; p.h_out = ws + L.off_Qb; }
     else { p.f32_out = reinterpret_cast<float*>(ws + L.off_Q); p.h_out = nullptr; }
-    umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p, narrow);
+    umma_launch_mode(L.mode, EPI_A4, grid_sym, s, p, narrow, pdl);
     // a5: Z_next = Z + Z Q^T ; W = Z_next^T   (first order in R: all three passes)
     p.hh_only = 0;
     if (prof) prof->mark(s, EPI_A5 + 16 * tagn);
@@ -1124,14 +1146,14 @@ struct UmmaSeq {
         const int i0 = (int)((long long)T * b / bands), i1 = (int)((long long)T * (b + 1) / bands);
         p.ioff = i0; p.irows = i1 - i0;
         const int tiles = p.irows * T * nsplit_;
-        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.pairs() ? tiles : pl.pairs()), s, p, narrow);
+        umma_launch_mode(L.mode, EPI_A5, 2 * (tiles < pl.pairs() ? tiles : pl.pairs()), s, p, narrow, pdl);
         hook->after_a5_band(hook->self, i0 * UM_MACRO, i1 * UM_MACRO, b == bands - 1, s);
       }
       p.ioff = 0; p.irows = 0;
       nl += 1 + bands;
       return;
     }
-    umma_launch_mode(L.mode, EPI_A5, grid_full, s, p, narrow);
+    umma_launch_mode(L.mode, EPI_A5, grid_full, s, p, narrow, pdl);
     nl += 2;
   }
 };

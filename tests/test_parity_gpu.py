@@ -1413,3 +1413,40 @@ def test_narrow_tiles_are_scheduling_only(n, mode):
     with b.Zfac(256, "f64", DEV) as zf:
         with pytest.raises(b.ZfacError):
             zf.set_option("narrow_tiles", 1)
+
+
+@pytest.mark.parametrize("mode", ["split16", "hh16", "tf32"])
+def test_programmatic_dependent_launch_is_scheduling_only(mode):
+    """ZFAC_OPT_PDL: the GEMM kernels launched with programmatic stream serialization wait on the device
+    (griddepcontrol.wait) before they read anything -- Z, Err[], iters and flags are the plain launches' bit for bit, for
+    runs that stop early (the launches behind the stop return at once), fixed counts, the host entry point and Alg. 3."""
+    b = zb()
+    for n in (300, 1100):
+        w = W.random_spd_general(n, seed=70 + n, kappa=30.0, pert=0.05, fp32_stored=True)
+        S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
+        ref = None
+        for pdl in (0, 1, -1):
+            with b.Zfac(n, mode, DEV) as zf:
+                assert zf.get_option("pdl") == -1
+                zf.set_option("pdl", pdl)
+                a = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+                a = (a[0].clone(), a[1], a[2].copy(), a[3])
+                f = zf.refine(S, Z0, max_iter=3, stop=b.ZFAC_STOP_FIXED)
+                f = (f[0].clone(), f[1], f[2].copy(), f[3])
+                hS = S.cpu().pin_memory(); hZ0 = Z0.cpu().pin_memory(); hZ = torch.empty_like(hZ0).pin_memory()
+                _, hit, herr, hfl = zf.refine_host(hS, hZ0, hZ, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+                assert hit == a[1] and hfl == a[3] and np.array_equal(herr, a[2]) and torch.equal(hZ, a[0].cpu())
+                if mode != "split16":
+                    with b.Zfac(n, "split16", DEV) as hi:
+                        hi.set_option("pdl", pdl)
+                        r = zf.refine_refi(hi, S, Z0, max_iter=25, refi_steps=2)
+                        r = (r[0].clone(), r[1], r[2].copy(), r[3])
+                else:
+                    r = None
+            if ref is None:
+                ref = (a, f, r)
+                continue
+            for x, y in zip(ref, (a, f, r)):
+                if x is None:
+                    continue
+                assert x[1] == y[1] and x[3] == y[3] and np.array_equal(x[2], y[2], equal_nan=True) and torch.equal(x[0], y[0]), (n, pdl)
