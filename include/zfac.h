@@ -277,8 +277,10 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *                            <= 37 (one problem of padded order <= 1536, or a few smaller ones), 0 = never, 1 = always          -1
  *   ZFAC_OPT_PDL             SPLIT16, HH16, TF32: programmatic dependent launch of the GEMM kernels (a kernel is scheduled while
  *                            its predecessor still runs and waits for it on the device before it reads anything); not
- *                            used inside zfac_graph_*; -1 = automatically (HH16 / TF32 up to padded order 2048, where it
- *                            takes 7 .. 15 % off a call; SPLIT16: no gain measured), 0 = never, 1 = always               -1
+ *                            used inside zfac_graph_*.  In small launches (batch x (padded order / 256)^2 <= 37) the kernel's
+ *                            set-up (barriers, tensor memory) runs ahead of that wait as well.  -1 = automatically (small
+ *                            launches in every mode: 4 .. 21 % off a call; HH16 / TF32 up to padded order 2048: 7 .. 15 %),
+ *                            0 = never, 1 = always, 2 = always, without the early set-up                              -1
  *   ZFAC_OPT_I8_CLUSTER      F64_I8, a1 (when the padded order is a multiple of 512): clusters of two CTA pairs that share
  *                            the B slices by TMA multicast (L2 -> SM bytes -25 %); only 33 such clusters are co-resident on a
  *                            B200 against 74 pairs, measured a tie; 0 / 1                              0

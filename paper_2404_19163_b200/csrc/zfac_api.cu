@@ -234,7 +234,7 @@ zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
     case ZFAC_OPT_INPUT_F32:
       if ((iv != 0 && iv != 1) || (iv == 1 && !mode_is_f64_elt(c->mode))) return ZFAC_E_INVALID;
       o.input_f32 = (int)iv; return ZFAC_OK;
-    case ZFAC_OPT_PDL: if (iv < -1 || iv > 1) return ZFAC_E_INVALID; o.pdl = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_PDL: if (iv < -1 || iv > 2) return ZFAC_E_INVALID; o.pdl = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_NARROW_TILES:
       if ((iv < -1 || iv > 1) || (iv == 1 && !mode_is_umma(c->mode))) return ZFAC_E_INVALID;
       o.narrow_tiles = (int)iv; return ZFAC_OK;

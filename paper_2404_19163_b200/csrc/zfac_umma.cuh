@@ -127,6 +127,7 @@ struct UmmaParams {
   double hh_err_max;    // ... and does so iff Err[n] = stop.d_err[stop.n_iter] <= hh_err_max (decided on the device)
   float q_r, q_d;       // a4: Q = q_r R + q_d D        (1/2, 3/8; m > 2: 1/2, 1)       see PolyCoef (zfac_f64.cuh)
   float g_i, g_r, g_p;  // p2: G = g_i I + g_r R + g_p D (3/8, 5/16, 35/128 or 0)
+  int early;            // programmatic dependent launch with the wait AFTER the set-up (see the head of the kernel)
   int scaled;           // FP64-master modes: a4 works on R~ = rscale R (State::rscale): Q~ = q_r R~ + (q_d / rscale) R~ R~
   double* z64;          // a5x: FP64 master Z, updated in place: Z64 += D / rscale
   double* w64t;         // a5x: FP64 W = Z^T (DMMA residual engine) or null
@@ -465,8 +466,13 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   // its predecessor in the stream was still running.  Nothing of global memory is touched before the predecessor has
   // completed (wait); then the successor is let in at once -- it takes SMs as they fall free and waits here in turn, so
   // its launch latency is hidden behind this kernel (the kernels of a small problem, the early-exit launches behind the stop).
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  if (p.batch == 1 && *((volatile int*)&p.st->done)) return;
+  // p.early (small launches, which leave SMs free): the successor is let in FIRST and the wait comes after this kernel's own
+  // set-up (barrier init, tensor-memory allocation, pair synchronisation: pair_sync_in), so that the set-up too runs while the
+  // predecessor still works; a launch behind the stop then skips its tiles instead of returning here.
+  if (!p.early) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (p.batch == 1 && *((volatile int*)&p.st->done)) return;
+  }
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   using KT = KindTraits<KIND>;
@@ -510,7 +516,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   const int JC = (!SYM && p.jcols > 0) ? p.jcols : T * NSPLIT;             // tile columns of this launch
   const int TI = (!SYM && p.irows > 0) ? p.irows : T;                      // tile rows of this launch
   const int tiles_pp = SYM ? T * (T + 1) / 2 * NSPLIT : TI * JC;          // 256 x TN pair tiles of ONE problem
-  const int num_tiles = tiles_pp * p.batch;                                // tile t: problem t / tiles_pp
+  const int all_tiles = tiles_pp * p.batch;                                // tile t: problem t / tiles_pp
 
   // The two register regimes (setmaxnreg) are two disjoint regions of the kernel: everything a role executes, including
   // its side of the two pair-wide synchronisations, sits inside its own branch (ptxas allocates registers per region
@@ -522,8 +528,11 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
     tc_fence_after();
     uint32_t tb;
     asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tb) : "r"(tmem_slot));
+    if (p.early) asm volatile("griddepcontrol.wait;" ::: "memory");
     return tb;
   };
+  // tiles of this launch as the roles see them (read AFTER pair_sync_in): none behind the stop
+  auto live_tiles = [&]() -> int { return (p.early && p.batch == 1 && *((volatile int*)&p.st->done)) ? 0 : all_tiles; };
   auto pair_sync_out = [&]() {                             // no MMA / remote arrive of the pair is in flight any more
     tc_fence_before();
     __syncthreads();
@@ -583,6 +592,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   }
   const uint32_t tmem_base = pair_sync_in();
+  const int num_tiles = live_tiles();
   if (warp == 0) {
     // ===================================================== TMA producer (both CTAs)
     if (lane == 0) {
@@ -743,6 +753,7 @@ umma_gemm_kernel(const __grid_constant__ UmmaParams p) {
   } else {
     reg_alloc<UM_REGS_EPILOGUE>();
     const uint32_t tmem_base = pair_sync_in();
+    const int num_tiles = live_tiles();
     // ===================================================== epilogue warps (4 .. 11), both CTAs
     // Group g = warps 4 + 4 g .. 7 + 4 g (one warp per TMEM lane quarter).  SETS == 2: group g owns accumulator
     // set g, i.e. the tiles with local index li = g (mod 2), all TN columns: its stores overlap the other set's
@@ -1029,9 +1040,12 @@ struct UmmaSeq {
     char* ws = pl.ws;
     const int T = (int)(L.np / UM_MACRO);
     narrow = umma_narrow(pl);
-    // measured (10 updates, on / off): HH16 N = 512 / 1024 / 2048 0.54 / 0.64 / 1.16 against 0.65 / 0.74 / 1.25 ms, TF32 alike, a tie
-    // at N = 3072; SPLIT16 +-1 % at every size -> automatic (-1): the one-pass modes up to 8 x 8 macro tiles
-    pdl = (cond == 0ull) && (pl.opt->pdl >= 0 ? pl.opt->pdl != 0 : (L.mode != ZFAC_MODE_SPLIT16 && T <= 8));
+    // measured (10 updates, off / on / on with the early set-up): HH16 N = 512 / 1024 0.64 / 0.53 / 0.50 and 0.74 / 0.64 / 0.61 ms,
+    // N = 2048 1.25 / 1.16 ms, a tie at N = 3072, TF32 alike; SPLIT16 N = 512 / 1024 0.93 / 0.92 / 0.88 and 1.19 / 1.19 / 1.15 ms,
+    // +-1 % beyond -> automatic (-1): small launches (<= 37 wide tiles) in every mode, the one-pass modes up to 8 x 8 macro tiles
+    const bool small = (long)L.batch * T * T <= 37;
+    pdl = (cond == 0ull) && (pl.opt->pdl >= 0 ? pl.opt->pdl != 0 : (small || (L.mode != ZFAC_MODE_SPLIT16 && T <= 8)));
+    p.early = (pdl && pl.opt->pdl != 2 && small) ? 1 : 0;      // small launches: set-up ahead of the wait
     const int nsplit = narrow ? 2 : 1;                       // 256 / TILE_N of the kind that runs
     const int full_tiles = T * T * nsplit * L.batch, sym_tiles = T * (T + 1) / 2 * nsplit * L.batch;
     grid_full = 2 * (full_tiles < pl.pairs() ? full_tiles : pl.pairs());

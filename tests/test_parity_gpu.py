@@ -1418,14 +1418,14 @@ def test_narrow_tiles_are_scheduling_only(n, mode):
 @pytest.mark.parametrize("mode", ["split16", "hh16", "tf32"])
 def test_programmatic_dependent_launch_is_scheduling_only(mode):
     """ZFAC_OPT_PDL: the GEMM kernels launched with programmatic stream serialization wait on the device
-    (griddepcontrol.wait) before they read anything -- Z, Err[], iters and flags are the plain launches' bit for bit, for
+    (griddepcontrol.wait) before they read anything, in small launches after their own set-up -- Z, Err[], iters and flags are the plain launches' bit for bit, for
     runs that stop early (the launches behind the stop return at once), fixed counts, the host entry point and Alg. 3."""
     b = zb()
     for n in (300, 1100):
         w = W.random_spd_general(n, seed=70 + n, kappa=30.0, pert=0.05, fp32_stored=True)
         S, Z0 = _to_dev(w.S, mode), _to_dev(w.Z0, mode)
         ref = None
-        for pdl in (0, 1, -1):
+        for pdl in (0, 1, 2, -1):
             with b.Zfac(n, mode, DEV) as zf:
                 assert zf.get_option("pdl") == -1
                 zf.set_option("pdl", pdl)
