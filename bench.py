@@ -415,6 +415,40 @@ def cold_start_paths(zb, dev, max_iter=40):
             "path": best, "value_ms": ok[best]["ms"] if best else None, "paths": out}
 
 
+def small_n_paths(zb, dev, n=1024):
+    """One small problem (config 5 recipe, N = 1024): what the 256 x 128 tiles (ZFAC_OPT_NARROW_TILES) and programmatic
+    dependent launch (ZFAC_OPT_PDL) buy, measured in the same process with both switched off and at their defaults.
+    Results are bit-identical either way (tests); times in ms per call."""
+    import torch
+    from paper_2404_19163_b200 import workloads as W
+    w = W.config5(n, device=dev, fp32_stored=True)
+    S = torch.from_numpy(w.S).to(dev, torch.float32); Z0 = torch.from_numpy(w.Z0).to(dev, torch.float32)
+    out = {}
+
+    def timed(call, reps=9):
+        call(); call(); torch.cuda.synchronize(dev)
+        ts = []
+        for _ in range(reps):
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(); call(); e1.record(); torch.cuda.synchronize(dev)
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+
+    for label, opts in (("wide tiles, plain launches", {"narrow_tiles": 0, "pdl": 0}), ("defaults", {})):
+        row = {}
+        with zb.Zfac(n, "split16", dev) as zs, zb.Zfac(n, "hh16", dev) as zh:
+            for z in (zs, zh):
+                for k, v in opts.items():
+                    z.set_option(k, v)
+            Zr = torch.empty_like(Z0)
+            row["split16_10_updates_ms"] = timed(lambda: zs.refine(S, Z0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=Zr, sync=False))
+            row["hh16_10_updates_ms"] = timed(lambda: zh.refine(S, Z0, max_iter=10, stop=zb.ZFAC_STOP_FIXED, out=Zr, sync=False))
+            row["split16_to_stop_ms"] = timed(lambda: zs.refine(S, Z0, max_iter=40, stop=zb.ZFAC_STOP_PAPER, out=Zr, sync=False))
+            row["hh16+2xsplit16_to_stop_ms"] = timed(lambda: zh.refine_refi(zs, S, Z0, max_iter=40, refi_steps=2, final_check=False, out=Zr, sync=False))
+        out[label] = row
+    return {"workload": f"config5_n{n}", "paths": out}
+
+
 def oracle_iterates(w, kmax):
     """Z_k, k = 0..kmax, of the FP64 oracle (Alg. 2 steps as oracle/ defines them), computed ONCE outside every timed
     region; also the time of the first update step (R_0, Err[0], Z_1, R_1, Err[1]: 12 N^3 flop) for `cpu_baseline`."""
@@ -734,6 +768,10 @@ def run_ours(args):
             extra["cold_start"] = cold_start_paths(zb, dev)
         except Exception as ex:
             extra["cold_start"] = {"error": str(ex)[:200]}
+        try:
+            extra["small_n"] = small_n_paths(zb, dev)
+        except Exception as ex:
+            extra["small_n"] = {"error": str(ex)[:200]}
         # iterations / s (BASELINE.json's metric names it for split-FP16 and FP64 at N = 8192): SURVEY.md §8(d)'s difference
         # quotient over fixed-count runs, t_iter = (t(k2) - t(k1)) / (k2 - k1), which cancels copy-in, copy-out and the
         # first residual.  One iteration = a4, a5, a1, a2 = 8 N^3 flop in the paper's convention.
