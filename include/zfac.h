@@ -279,8 +279,9 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *                            its predecessor still runs and waits for it on the device before it reads anything); not
  *                            used inside zfac_graph_*.  In small launches (batch x (padded order / 256)^2 <= 37) the kernel's
  *                            set-up (barriers, tensor memory) runs ahead of that wait as well.  -1 = automatically (small
- *                            launches: 4 .. 21 % off a call; one problem of padded order <= 2048 in any mode: the launches
- *                            behind the stop cost half; HH16 / TF32 there: 7 .. 15 % off the working kernels too),
+ *                            launches: 4 .. 21 % off a call; one problem of any size: the launches behind the stop cost
+ *                            half; HH16 / TF32 up to padded order 2048: 7 .. 15 % off the working kernels too; larger
+ *                            batched launches: not used),
  *                            0 = never, 1 = always, 2 = always, without the early set-up                              -1
  *   ZFAC_OPT_I8_CLUSTER      F64_I8, a1 (when the padded order is a multiple of 512): clusters of two CTA pairs that share
  *                            the B slices by TMA multicast (L2 -> SM bytes -25 %); only 33 such clusters are co-resident on a

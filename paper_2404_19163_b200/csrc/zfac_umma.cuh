@@ -1043,9 +1043,10 @@ struct UmmaSeq {
     // measured (10 updates, off / on / on with the early set-up): HH16 N = 512 / 1024 0.64 / 0.53 / 0.50 and 0.74 / 0.64 / 0.61 ms,
     // N = 2048 1.25 / 1.16 ms, a tie at N = 3072, TF32 alike; SPLIT16 N = 512 / 1024 0.93 / 0.92 / 0.88 and 1.19 / 1.19 / 1.15 ms,
     // +-1.5 % beyond; a launch behind the stop costs 1.4 .. 1.9 us instead of 2.7 .. 4.2 us, which decides for runs that stop well
-    // before max_iter (SPLIT16 N = 2048 to its stop, max_iter = 40: 2.47 -> 2.2 ms) -> automatic (-1): up to 8 x 8 macro tiles
+    // before max_iter (SPLIT16 N = 2048 to its stop, max_iter = 40: 2.47 -> 2.2 ms)
     const bool small = (long)L.batch * T * T <= 37;
-    pdl = (cond == 0ull) && (pl.opt->pdl >= 0 ? pl.opt->pdl != 0 : (small || (L.batch == 1 && T <= 8)));   // (batched, not small: -4 % measured)
+    // N = 4096 / 8192: the working kernels within the noise, calls that stop well before max_iter -1.3 % -> every single problem
+    pdl = (cond == 0ull) && (pl.opt->pdl >= 0 ? pl.opt->pdl != 0 : (small || L.batch == 1));   // (batched, not small: -4 % measured)
     p.early = (pdl && pl.opt->pdl != 2 && small) ? 1 : 0;      // small launches: set-up ahead of the wait
     const int nsplit = narrow ? 2 : 1;                       // 256 / TILE_N of the kind that runs
     const int full_tiles = T * T * nsplit * L.batch, sym_tiles = T * (T + 1) / 2 * nsplit * L.batch;
