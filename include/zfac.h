@@ -283,6 +283,8 @@ zfac_status zfac_graph_destroy(zfac_graph* graph);
  *                            half; HH16 / TF32 up to padded order 2048: 7 .. 15 % off the working kernels too; larger
  *                            batched launches: not used),
  *                            0 = never, 1 = always, 2 = always, without the early set-up                              -1
+ *   ZFAC_OPT_I8_NARROW       F64_I8: the INT8 kernels on 256 x 128 tiles (T and R bit-identical, Err[] in its last bits only);
+ *                            -1 = automatically up to padded order 1536 (17 .. 24 % off a call), 0 = never, 1 = always   -1
  *   ZFAC_OPT_I8_CLUSTER      F64_I8, a1 (when the padded order is a multiple of 512): clusters of two CTA pairs that share
  *                            the B slices by TMA multicast (L2 -> SM bytes -25 %); only 33 such clusters are co-resident on a
  *                            B200 against 74 pairs, measured a tie; 0 / 1                              0
@@ -292,7 +294,7 @@ typedef enum {
   ZFAC_OPT_PROMOTE_UPDATE = 4, ZFAC_OPT_BAND = 5, ZFAC_OPT_MAX_PAIRS = 6, ZFAC_OPT_HOST_OVERLAP = 7,
   ZFAC_OPT_HOST_UPLOAD_OVERLAP = 8, ZFAC_OPT_HOST_A5_BANDS = 9, ZFAC_OPT_I8_SLICES = 10, ZFAC_OPT_INPUT_F32 = 11,
   ZFAC_OPT_EXTRA_UPDATE = 12, ZFAC_OPT_FINAL_CHECK = 13, ZFAC_OPT_I8_CLUSTER = 14,
-  ZFAC_OPT_NARROW_TILES = 15, ZFAC_OPT_PDL = 16
+  ZFAC_OPT_NARROW_TILES = 15, ZFAC_OPT_PDL = 16, ZFAC_OPT_I8_NARROW = 17
 } zfac_option;
 zfac_status zfac_set_option(zfac_ctx* ctx, zfac_option key, double value);
 zfac_status zfac_get_option(const zfac_ctx* ctx, zfac_option key, double* value);

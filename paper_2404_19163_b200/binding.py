@@ -25,12 +25,12 @@ ZFAC_BUF_T, ZFAC_BUF_R, ZFAC_BUF_Q, ZFAC_BUF_Z = 0, 1, 2, 3
 
 (ZFAC_OPT_CHUNK_KB, ZFAC_OPT_CHUNK0_KB, ZFAC_OPT_HH_SQUARE, ZFAC_OPT_HH_SQUARE_ERR, ZFAC_OPT_PROMOTE_UPDATE, ZFAC_OPT_BAND,
  ZFAC_OPT_MAX_PAIRS, ZFAC_OPT_HOST_OVERLAP, ZFAC_OPT_HOST_UPLOAD_OVERLAP, ZFAC_OPT_HOST_A5_BANDS, ZFAC_OPT_I8_SLICES,
- ZFAC_OPT_INPUT_F32, ZFAC_OPT_EXTRA_UPDATE, ZFAC_OPT_FINAL_CHECK, ZFAC_OPT_I8_CLUSTER, ZFAC_OPT_NARROW_TILES, ZFAC_OPT_PDL) = range(17)
+ ZFAC_OPT_INPUT_F32, ZFAC_OPT_EXTRA_UPDATE, ZFAC_OPT_FINAL_CHECK, ZFAC_OPT_I8_CLUSTER, ZFAC_OPT_NARROW_TILES, ZFAC_OPT_PDL, ZFAC_OPT_I8_NARROW) = range(18)
 OPTIONS = {"chunk_kb": ZFAC_OPT_CHUNK_KB, "chunk0_kb": ZFAC_OPT_CHUNK0_KB, "hh_square": ZFAC_OPT_HH_SQUARE,
            "hh_square_err": ZFAC_OPT_HH_SQUARE_ERR, "promote_update": ZFAC_OPT_PROMOTE_UPDATE, "band": ZFAC_OPT_BAND,
            "max_pairs": ZFAC_OPT_MAX_PAIRS, "host_overlap": ZFAC_OPT_HOST_OVERLAP,
            "host_upload_overlap": ZFAC_OPT_HOST_UPLOAD_OVERLAP, "host_a5_bands": ZFAC_OPT_HOST_A5_BANDS,
-           "i8_slices": ZFAC_OPT_I8_SLICES, "input_f32": ZFAC_OPT_INPUT_F32, "extra_update": ZFAC_OPT_EXTRA_UPDATE, "final_check": ZFAC_OPT_FINAL_CHECK, "i8_cluster": ZFAC_OPT_I8_CLUSTER, "narrow_tiles": ZFAC_OPT_NARROW_TILES, "pdl": ZFAC_OPT_PDL}
+           "i8_slices": ZFAC_OPT_I8_SLICES, "input_f32": ZFAC_OPT_INPUT_F32, "extra_update": ZFAC_OPT_EXTRA_UPDATE, "final_check": ZFAC_OPT_FINAL_CHECK, "i8_cluster": ZFAC_OPT_I8_CLUSTER, "narrow_tiles": ZFAC_OPT_NARROW_TILES, "pdl": ZFAC_OPT_PDL, "i8_narrow": ZFAC_OPT_I8_NARROW}
 
 MODES = {"split16": ZFAC_MODE_SPLIT16, "tf32": ZFAC_MODE_TF32, "f64": ZFAC_MODE_F64, "hh16": ZFAC_MODE_HH16,
          "f64mix": ZFAC_MODE_F64_MIXED, "f64i8": ZFAC_MODE_F64_I8}

@@ -234,6 +234,9 @@ zfac_status zfac_set_option(zfac_ctx* c, zfac_option key, double v) {
     case ZFAC_OPT_INPUT_F32:
       if ((iv != 0 && iv != 1) || (iv == 1 && !mode_is_f64_elt(c->mode))) return ZFAC_E_INVALID;
       o.input_f32 = (int)iv; return ZFAC_OK;
+    case ZFAC_OPT_I8_NARROW:
+      if (iv < -1 || iv > 1 || (iv == 1 && c->mode != ZFAC_MODE_F64_I8)) return ZFAC_E_INVALID;
+      o.i8_narrow = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_PDL: if (iv < -1 || iv > 2) return ZFAC_E_INVALID; o.pdl = (int)iv; return ZFAC_OK;
     case ZFAC_OPT_NARROW_TILES:
       if ((iv < -1 || iv > 1) || (iv == 1 && !mode_is_umma(c->mode))) return ZFAC_E_INVALID;
@@ -272,6 +275,7 @@ zfac_status zfac_get_option(const zfac_ctx* c, zfac_option key, double* v) {
     case ZFAC_OPT_I8_CLUSTER: *v = o.i8_cluster; return ZFAC_OK;
     case ZFAC_OPT_NARROW_TILES: *v = o.narrow_tiles; return ZFAC_OK;
     case ZFAC_OPT_PDL: *v = o.pdl; return ZFAC_OK;
+    case ZFAC_OPT_I8_NARROW: *v = o.i8_narrow; return ZFAC_OK;
   }
   return ZFAC_E_INVALID;
 }

@@ -39,6 +39,7 @@ struct Options {
   int host_a5_bands = 2;     // zfac_refine_host: row bands of the first a5 (each band downloaded as it completes)
   int narrow_tiles = -1;     // tcgen05 modes: 256 x 128 tiles (see umma_narrow): -1 auto, 0 never, 1 always (scheduling only)
   int pdl = -1;              // tcgen05 modes: programmatic dependent launch of the GEMM kernels: -1 auto, 0 off, 1 on, 2 on without the early set-up (scheduling only)
+  int i8_narrow = -1;        // F64_I8: 256 x 128 tiles in the INT8 kernels: -1 auto (up to 6 x 6 macro tiles), 0 never, 1 always
   int i8_cluster = 0;        // F64_I8 a1: clusters of two CTA pairs sharing the B slices by TMA multicast (scheduling only)
   int i8_slices = 8;         // F64_I8: int8 slices per operand row (= orders i + j kept)
   int final_check = 1;       // FP64-master modes: 0 = skip a residual evaluation whose outcome is known beforehand (see stop_decide)

@@ -258,13 +258,18 @@ __device__ __forceinline__ void tma_load_2d_pair_mc(uint32_t dst, const CUtensor
 // d - 1): 2/3 of a stage's bytes are shared, the L2 -> SM traffic falls by a third.  The two pairs then move in lockstep, a
 // stage at a time: a stage is refilled when BOTH pairs have released it (every MMA leader commits to the empty barriers of all
 // four CTAs).  Same arithmetic per tile: bit-identical results.
-template <int EPI, int CP = 1>
+// TN = 128 (CP = 1): the same on 256 x 128 tiles -- twice as many tiles for problems whose 256 x 256 tiles leave CTA pairs idle
+// (ZFAC_OPT_I8_NARROW); every element is the same exact integer sum, so T and R are bit-identical, and Err[] differs in its last
+// bits only (the partial sums of step a3 are grouped by tile).
+template <int EPI, int CP = 1, int TN = 256>
 __global__ void __cluster_dims__(2 * CP, 1, 1) __launch_bounds__(UM_THREADS, 1)
 i8_gemm_kernel(const __grid_constant__ I8Params p) {
   static_assert(CP == 1 || EPI == EPI_A1, "clusters of two pairs: full outputs only");
+  static_assert(TN == 256 || (TN == 128 && CP == 1), "tile widths");
   if (*((volatile int*)&p.st->done)) return;
   constexpr bool SYM = (EPI == EPI_A2);
-  constexpr int TN = 256;
+  constexpr int NS = 256 / TN;                                 // tiles per 256-column macro tile
+  constexpr int GC = TN / 2;                                   // columns per epilogue thread (two groups of warps)
   constexpr uint32_t IDESC = make_idesc_i8(TN);
 
   extern __shared__ unsigned char smem_raw[];
@@ -288,8 +293,8 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
   const int np = p.np;
   const int KB = np / 128;                                   // k-blocks of 128 int8
   const int T = p.macro_tiles;
-  const int JC = (!SYM && p.jcols > 0) ? p.jcols : T;          // tile columns of this launch
-  const int num_tiles = SYM ? T * (T + 1) / 2 : (T / CP) * JC;
+  const int JC = (!SYM && p.jcols > 0) ? p.jcols * NS : T * NS;   // tile columns of this launch (p.joff, p.jcols: macro columns)
+  const int num_tiles = SYM ? T * (T + 1) / 2 * NS : (T / CP) * JC;
   const int ORD = p.orders;
 
   if (threadIdx.x == 0) {
@@ -312,8 +317,8 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
 
   auto decode = [&](int t, int& m0, int& n0, bool& offdiag) {
     int I, J;
-    if (SYM) { tri_decode(t, I, J); offdiag = (I != J); }
-    else { band_decode(t, T / CP, JC, p.band, I, J); I = I * CP + pp; J += p.joff; offdiag = true; }
+    if (SYM) { const int macro = t / NS; tri_decode(macro, I, J); offdiag = (I != J); J = J * NS + (t - macro * NS); }
+    else { band_decode(t, T / CP, JC, p.band * NS, I, J); I = I * CP + pp; J += p.joff * NS; offdiag = true; }
     m0 = I * UM_TILE_M; n0 = J * TN;
   };
 
@@ -332,7 +337,7 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
             if (!v1 && !v2) continue;
             for (int kb = 0; kb < KB; ++kb) {
               mbar_wait(empty_bar(stage), phase ^ 1u);
-              if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * (uint32_t)UM_A_BYTES * (1u + (v1 ? 1u : 0u) + (v2 ? 1u : 0u)));
+              if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * ((uint32_t)UM_A_BYTES + (uint32_t)(GC * UM_ROWB) * ((v1 ? 1u : 0u) + (v2 ? 1u : 0u))));
               const uint32_t lead_full = mapa_u32(full_bar(stage), lead);
               const uint32_t sa = smem_base + stage * I8_STAGE_BYTES, sb1 = sa + UM_A_BYTES, sb2 = sb1 + UM_A_BYTES;
               const int kc = kb * 128;
@@ -341,8 +346,10 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
               for (int b = 0; b < UM_ROWS / UM_BOX_ROWS; ++b) {
                 tma_load_2d_pair(sa + b * UM_BOX_BYTES, &p.mapA, kc, i * np + m0 + aoff + b * UM_BOX_ROWS, lead_full);
                 if (CP == 1) {
-                  if (v1) tma_load_2d_pair(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
-                  if (v2) tma_load_2d_pair(sb2 + b * UM_BOX_BYTES, &p.mapB, kc, j2 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                  if (b < GC / UM_BOX_ROWS) {                  // TN / 2 rows of B per CTA: one box (TN = 128) or two
+                    if (v1) tma_load_2d_pair(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                    if (v2) tma_load_2d_pair(sb2 + b * UM_BOX_BYTES, &p.mapB, kc, j2 * np + n0 + boff + b * UM_BOX_ROWS, lead_full);
+                  }
                 } else if (pp == 0) {
                   if (v1) tma_load_2d_pair_mc(sb1 + b * UM_BOX_BYTES, &p.mapB, kc, j1 * np + n0 + boff + b * UM_BOX_ROWS, full_bar(stage), mc);
                 } else {
@@ -405,20 +412,20 @@ i8_gemm_kernel(const __grid_constant__ I8Params p) {
         const bool two = (d >= 1);                             // the sweep carries order d - 1 as well
         const bool first = (d == ORD - 1), last = (d <= 1);
         const double w1 = ldexp(1.0, -7 * d), w2 = ldexp(1.0, -7 * (d - 1));
-        const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + g * 128;
+        const uint32_t tbase = tmem_base + ((uint32_t)(q * 32) << 16) + g * GC;
 #pragma unroll 1
-        for (int c = 0; c < 4; ++c) {
+        for (int c = 0; c < GC / 32; ++c) {
           uint32_t r1[32], r2[32];
           tmem_ld(tbase + c * 32, r1);
           if (two) tmem_ld(tbase + TN + c * 32, r2);
           tmem_ld_wait();
-          if (c == 3) {                                        // accumulators read out: hand them back before the arithmetic
+          if (c == GC / 32 - 1) {                              // accumulators read out: hand them back before the arithmetic
             tc_fence_before();
             __syncwarp();
             mbar_arrive_cluster_lane0(lead_tempty, lane);
             asm volatile("fence.acq_rel.cta;" ::: "memory");
           }
-          const int col0 = g * 128 + c * 32;
+          const int col0 = g * GC + c * 32;
           double* sl = slab + (size_t)col0 * 128 + rowl;     // element (row, col) at (col * 128 + row): coalesced per column
           if (!last) {
 #pragma unroll
@@ -487,14 +494,14 @@ struct MixPlan {
   int pairs() const { return (opt->max_pairs > 0 && opt->max_pairs < max_pairs) ? opt->max_pairs : max_pairs; }
 };
 
-template <int EPI, int CP = 1>
+template <int EPI, int CP = 1, int TN = 256>
 inline cudaError_t i8_prepare(int* max_pairs, int sm_count) {
-  cudaError_t e = cudaFuncSetAttribute(i8_gemm_kernel<EPI, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
+  cudaError_t e = cudaFuncSetAttribute(i8_gemm_kernel<EPI, CP, TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, UM_SMEM_BYTES);
   if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(2 * CP * (sm_count / (2 * CP))); cfg.blockDim = dim3(UM_THREADS); cfg.dynamicSmemBytes = UM_SMEM_BYTES;
   int nc = 0;
-  e = cudaOccupancyMaxActiveClusters(&nc, i8_gemm_kernel<EPI, CP>, &cfg);
+  e = cudaOccupancyMaxActiveClusters(&nc, i8_gemm_kernel<EPI, CP, TN>, &cfg);
   if (e != cudaSuccess) return e;
   if (nc < 1) return cudaErrorLaunchOutOfResources;
   if (*max_pairs == 0 || nc < *max_pairs) *max_pairs = nc;
@@ -530,6 +537,8 @@ inline cudaError_t mix_plan_create(MixPlan* pl, const Layout& L, char* ws, int s
     if ((e = i8_prepare<EPI_A1>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
     if ((e = i8_prepare<EPI_A2>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
     if ((e = i8_prepare<EPI_A1, 2>(&pl->max_quads, sm_count)) != cudaSuccess) { pl->max_quads = 0; (void)cudaGetLastError(); }
+    if ((e = i8_prepare<EPI_A1, 1, 128>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
+    if ((e = i8_prepare<EPI_A2, 1, 128>(&pl->max_pairs, sm_count)) != cudaSuccess) return e;
   }
   if (pl->max_pairs > sm_count / 2) pl->max_pairs = sm_count / 2;
   if (2 * pl->max_pairs > I8_SCRATCH_CTAS) pl->max_pairs = I8_SCRATCH_CTAS / 2;
@@ -560,6 +569,14 @@ struct MixSeq {
     stop.nocheck = pl.opt->final_check ? 0 : 1; stop.floor = ldexp(1.0, -53) * sqrt((double)L.n);
     R32s = reinterpret_cast<float*>(ws + L.off_R32);
     np2 = (size_t)L.np * (size_t)L.np;
+    // I8 engine on 256 x 128 tiles: -1 (default) up to 6 x 6 macro tiles (4 updates, wide -> narrow: N = 512 / 1024 / 1536
+    // 1.56 / 2.16 / 2.83 -> 1.19 / 1.74 / 2.34 ms; N = 2048 / 3072 +5 / +15 %)
+    i8_narrow = (L.mode == ZFAC_MODE_F64_I8) && (pl.opt->i8_narrow >= 0 ? pl.opt->i8_narrow != 0 : T <= 6);
+  }
+  bool i8_narrow = false;
+  int i8_grid(int wide_tiles) const {
+    const int tiles = wide_tiles * (i8_narrow ? 2 : 1);
+    return 2 * (tiles < pl.pairs() ? tiles : pl.pairs());
   }
 
   void residual(int n_stop, int tagn, cudaStream_t s, Prof* prof, bool skip_a1 = false) {
@@ -588,7 +605,8 @@ struct MixSeq {
       p.np = (int)L.np; p.macro_tiles = (int)(L.np / UM_MACRO); p.band = pl.opt->band > 1 ? pl.opt->band / 2 : 1;
       p.sa = p.sb = p.orders = pl.opt->i8_slices;
       p.scratch = reinterpret_cast<double*>(ws + L.off_scratch);
-      p.st = st; p.stop = stop; p.stop.num_partials = 16 * p.macro_tiles * (p.macro_tiles + 1) / 2;     // a2: 16 per tile
+      p.st = st; p.stop = stop;
+      p.stop.num_partials = 16 * (i8_narrow ? 2 : 1) * p.macro_tiles * (p.macro_tiles + 1) / 2;           // a2: 16 per tile
       int* eS = reinterpret_cast<int*>(ws + L.off_exp);
       int* eW = eS + L.np; int* eT = eW + L.np;
       // a1: T = W S^T (FP64 out), then its rows sliced for a2
@@ -599,11 +617,13 @@ struct MixSeq {
       int quads = pl.max_quads;
       if (pl.opt->max_pairs > 0 && pl.opt->max_pairs / 2 < quads) quads = pl.opt->max_pairs / 2;
       if (2 * quads * 2 > I8_SCRATCH_CTAS) quads = I8_SCRATCH_CTAS / 4;
-      if (pl.opt->i8_cluster && quads > 0 && p.macro_tiles % 2 == 0) {
+      if (pl.opt->i8_cluster && !i8_narrow && quads > 0 && p.macro_tiles % 2 == 0) {
         const int super_tiles = (p.macro_tiles / 2) * p.macro_tiles;
         const int nq = super_tiles < quads ? super_tiles : quads;
         i8_gemm_kernel<EPI_A1, 2><<<4 * nq, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
-      } else
+      } else if (i8_narrow)
+      i8_gemm_kernel<EPI_A1, 1, 128><<<i8_grid(p.macro_tiles * p.macro_tiles), UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      else
       i8_gemm_kernel<EPI_A1><<<grid_full, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
       ++nl;
       }
@@ -612,7 +632,8 @@ struct MixSeq {
       // a2: R = I - W T^T (FP32 out, both triangles), sum R^2, stop test
       p.mapA = pl.mW8; p.mapB = pl.mT8; p.expA = eW; p.expB = eT; p.out64 = nullptr; p.out32 = reinterpret_cast<float*>(ws + L.off_R);
       if (prof) prof->mark(s, EPI_A2 + 16 * tagn);
-      i8_gemm_kernel<EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      if (i8_narrow) i8_gemm_kernel<EPI_A2, 1, 128><<<i8_grid(p.macro_tiles * (p.macro_tiles + 1) / 2), UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+      else i8_gemm_kernel<EPI_A2><<<grid_sym, UM_THREADS, UM_SMEM_BYTES, s>>>(p);
       nl += 2;
       if (stop.cond) graph_cond_kernel<<<1, 1, 0, s>>>(st, stop.cond);
     }
@@ -667,7 +688,8 @@ struct MixSeq {
     p.mapA = pl.mW8; p.mapB = pl.mS8; p.expA = eS + L.np; p.expB = eS; p.out64 = reinterpret_cast<double*>(ws + L.off_T);
     p.joff = mc0; p.jcols = mcn;
     const int tiles = p.macro_tiles * mcn;
-    i8_gemm_kernel<EPI_A1><<<2 * (tiles < pl.pairs() ? tiles : pl.pairs()), UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    if (i8_narrow) i8_gemm_kernel<EPI_A1, 1, 128><<<i8_grid(tiles), UM_THREADS, UM_SMEM_BYTES, s>>>(p);
+    else i8_gemm_kernel<EPI_A1><<<2 * (tiles < pl.pairs() ? tiles : pl.pairs()), UM_THREADS, UM_SMEM_BYTES, s>>>(p);
     nl += 2;
   }
 

@@ -456,3 +456,33 @@ def test_f64i8_host_entry_point_with_the_banded_upload_is_bitwise_the_device_ent
             _, it, err, fl = zf.refine_host(hS[:, :n], hZ0, hZ, max_iter=30, stop=b.ZFAC_STOP_PAPER)
             assert it == itref and fl == flref and np.array_equal(err, errref), overlap
             assert torch.equal(hZ, Zref), overlap
+
+
+@pytest.mark.parametrize("n", [200, 900, 1400])
+def test_i8_narrow_tiles_give_the_same_integers(n):
+    """ZFAC_OPT_I8_NARROW: the INT8 kernels on 256 x 128 tiles (default up to padded order 1536).  Every element of T and R is
+    the same exact integer sum whatever the tile: T, R and Z are bit-identical to the 256 x 256 tiles; Err[] agrees to the
+    last bits (its partial sums are grouped by tile).  Also through the host entry point and with ZFAC_OPT_MAX_PAIRS."""
+    b = zb()
+    w = W.random_spd_general(n, seed=90 + n, kappa=100.0, pert=0.05, fp32_stored=False)
+    S, Z0 = _dev(w.S), _dev(w.Z0)
+    res = {}
+    with b.Zfac(n, "f64i8", DEV) as zf:
+        assert zf.get_option("i8_narrow") == -1
+        for nar, pairs in ((0, 0), (1, 0), (-1, 0), (1, 3)):
+            zf.set_option("i8_narrow", nar); zf.set_option("max_pairs", pairs)
+            Z, it, err, fl = zf.refine(S, Z0, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+            res[(nar, pairs)] = (Z.clone(), it, err.copy(), fl, zf.peek(b.ZFAC_BUF_T).clone(), zf.peek(b.ZFAC_BUF_R).clone())
+        zf.set_option("max_pairs", 0); zf.set_option("i8_narrow", 1)
+        hS = torch.from_numpy(w.S).pin_memory(); hZ0 = torch.from_numpy(np.ascontiguousarray(w.Z0)).pin_memory()
+        hZ = torch.empty((n, n), dtype=torch.float64).pin_memory()
+        _, hit, herr, hfl = zf.refine_host(hS, hZ0, hZ, max_iter=25, stop=b.ZFAC_STOP_PAPER)
+    ref = res[(0, 0)]
+    assert O.final_residual_per_sqrt_n(w.S, ref[0].cpu().numpy()) < 1e-12
+    for key in ((1, 0), (-1, 0), (1, 3)):
+        r = res[key]
+        assert r[1] == ref[1] and r[3] == ref[3], key
+        assert torch.equal(r[0], ref[0]) and torch.equal(r[4], ref[4]) and torch.equal(r[5], ref[5]), key
+        assert np.allclose(r[2], ref[2], rtol=1e-13, atol=0.0), key
+    assert np.array_equal(res[(1, 0)][2], res[(-1, 0)][2]) and np.array_equal(res[(1, 0)][2], res[(1, 3)][2])   # same tiles: same Err bits
+    assert hit == ref[1] and hfl == ref[3] and np.array_equal(herr, res[(1, 0)][2]) and torch.equal(hZ, ref[0].cpu())
